@@ -1,0 +1,203 @@
+"""ctypes binding of the CPU oracle (oracle/libqtam_ref.so).  TEST INFRASTRUCTURE ONLY.
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may import
+this module.  Argument marshalling only; all arithmetic is in qtam_ref.cpp.
+"""
+import ctypes as C
+import os
+import sys
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+if _HERE not in sys.path:
+    sys.path.insert(0, _HERE)
+import build as _build  # noqa: E402  (oracle/build.py)
+
+_lib = None
+
+
+class Options(C.Structure):
+    _fields_ = [("window", C.c_int), ("clamp_mode", C.c_int), ("clamp_overlap", C.c_double),
+                ("max_window_bins", C.c_int64), ("cover_floor", C.c_double),
+                ("rows_are_bins_per_octave", C.c_int)]
+
+
+class Row(C.Structure):
+    _fields_ = [("plane", C.c_int), ("row", C.c_int), ("q", C.c_double), ("f_request", C.c_double),
+                ("f_center", C.c_double), ("kc", C.c_int64), ("dk", C.c_int64), ("L", C.c_int64),
+                ("M", C.c_int64), ("offset", C.c_int64), ("norm", C.c_double)]
+
+
+class Info(C.Structure):
+    _fields_ = [("n_planes", C.c_int), ("n_rows", C.c_int), ("n", C.c_int64), ("n_bins", C.c_int64),
+                ("coeffs_per_segment", C.c_int64), ("sum_L", C.c_int64), ("cover_lo", C.c_int64),
+                ("cover_hi", C.c_int64), ("holes", C.c_int64), ("cover_count", C.c_int64),
+                ("frame_A", C.c_double), ("frame_B", C.c_double)]
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        _lib = C.CDLL(_build.build())
+        vp, dp, fp = C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_float)
+        _lib.qtam_ref_plan_create.argtypes = [C.POINTER(vp), C.c_double, C.c_int64, dp, C.c_int,
+                                              C.c_double, C.c_double, C.c_double, C.POINTER(Options)]
+        _lib.qtam_ref_plan_destroy.argtypes = [vp]
+        _lib.qtam_ref_plan_destroy.restype = None
+        _lib.qtam_ref_plan_info.argtypes = [vp, C.POINTER(Info)]
+        _lib.qtam_ref_plan_rows.argtypes = [vp, C.POINTER(Row), C.c_int]
+        _lib.qtam_ref_plan_window.argtypes = [vp, C.c_int, dp]
+        _lib.qtam_ref_plan_frame.argtypes = [vp, C.c_int, dp, C.POINTER(C.c_uint8)]
+        _lib.qtam_ref_forward.argtypes = [vp, dp, C.c_int, dp, C.c_int]
+        _lib.qtam_ref_inverse.argtypes = [vp, dp, C.c_int, C.c_int, dp, C.c_int]
+        _lib.qtam_ref_dense.argtypes = [vp, dp, C.c_int, C.c_int, C.c_int, dp, C.c_int]
+        _lib.qtam_ref_brute_tile.argtypes = [vp, dp, C.c_int, dp]
+        _lib.qtam_ref_threshold_rowmedian.argtypes = [vp, dp, C.c_int, C.c_double]
+        _lib.qtam_ref_threshold_rowmedian_f32.argtypes = [vp, fp, C.c_int, C.c_float]
+        _lib.qtam_ref_project_cover.argtypes = [vp, dp, C.c_int, C.c_int, dp, C.c_int]
+        _lib.qtam_ref_spectrum.argtypes = [vp, dp, C.c_int, dp, C.c_int]
+        _lib.qtam_ref_dft.argtypes = [dp, dp, C.c_int64, C.c_int]
+        _lib.qtam_ref_fft.argtypes = [dp, dp, C.c_int64, C.c_int]
+        _lib.qtam_ref_threads.restype = C.c_int
+    return _lib
+
+
+def _dp(a):
+    return a.ctypes.data_as(C.POINTER(C.c_double))
+
+
+def _c2d(a):
+    """complex128 array -> float64 view (interleaved)"""
+    return np.ascontiguousarray(a, dtype=np.complex128).view(np.float64)
+
+
+def threads():
+    return int(lib().qtam_ref_threads())
+
+
+def dft(z, sign):
+    z = np.ascontiguousarray(z, dtype=np.complex128)
+    out = np.empty_like(z)
+    assert lib().qtam_ref_dft(_dp(z.view(np.float64)), _dp(out.view(np.float64)), z.size, sign) == 0
+    return out
+
+
+def fft(z, sign):
+    z = np.ascontiguousarray(z, dtype=np.complex128)
+    out = np.empty_like(z)
+    assert lib().qtam_ref_fft(_dp(z.view(np.float64)), _dp(out.view(np.float64)), z.size, sign) == 0
+    return out
+
+
+class RefPlan:
+    """Oracle plan; same constructor arguments as the CUDA library's plan."""
+
+    def __init__(self, fs, N, Q, fmin, fmax, spacing, clamp_mode=1, clamp_overlap=1.0,
+                 max_window_bins=0, cover_floor=1e-2, rows_are_bins_per_octave=0):
+        L = lib()
+        self._h = C.c_void_p()
+        q = np.ascontiguousarray(Q, dtype=np.float64)
+        opt = Options(0, clamp_mode, clamp_overlap, max_window_bins, cover_floor,
+                      rows_are_bins_per_octave)
+        rc = L.qtam_ref_plan_create(C.byref(self._h), float(fs), int(N), _dp(q), q.size,
+                                    float(fmin), float(fmax), float(spacing), C.byref(opt))
+        if rc != 0:
+            self._h = None
+            raise ValueError(f"qtam_ref_plan_create failed with code {rc}")
+        info = Info()
+        assert L.qtam_ref_plan_info(self._h, C.byref(info)) == 0
+        self.info = info
+        self.N = int(info.n)
+        self.n_bins = int(info.n_bins)
+        self.n_rows = int(info.n_rows)
+        self.n_planes = int(info.n_planes)
+        self.ctot = int(info.coeffs_per_segment)
+        rows = (Row * self.n_rows)()
+        assert L.qtam_ref_plan_rows(self._h, rows, self.n_rows) == 0
+        self.rows = list(rows)
+
+    def __del__(self):
+        if getattr(self, "_h", None):
+            lib().qtam_ref_plan_destroy(self._h)
+            self._h = None
+
+    def window(self, k):
+        out = np.empty(int(self.rows[k].L), dtype=np.float64)
+        assert lib().qtam_ref_plan_window(self._h, k, _dp(out)) == 0
+        return out
+
+    def frame(self, plane=-1):
+        P = np.empty(self.n_bins, dtype=np.float64)
+        cov = np.empty(self.n_bins, dtype=np.uint8)
+        assert lib().qtam_ref_plan_frame(self._h, plane, _dp(P),
+                                         cov.ctypes.data_as(C.POINTER(C.c_uint8))) == 0
+        return P, cov.astype(bool)
+
+    def _x(self, x):
+        x = np.ascontiguousarray(x, dtype=np.float64)
+        if x.ndim == 1:
+            x = x[None, :]
+        assert x.shape[1] == self.N
+        return x
+
+    def forward(self, x, engine=0):
+        x = self._x(x)
+        out = np.empty((x.shape[0], self.ctot), dtype=np.complex128)
+        assert lib().qtam_ref_forward(self._h, _dp(x), x.shape[0], _dp(out.view(np.float64)), engine) == 0
+        return out
+
+    def inverse(self, coef, plane=-1, engine=0):
+        c = np.ascontiguousarray(coef, dtype=np.complex128)
+        if c.ndim == 1:
+            c = c[None, :]
+        assert c.shape[1] == self.ctot
+        out = np.empty((c.shape[0], self.N), dtype=np.float64)
+        assert lib().qtam_ref_inverse(self._h, _dp(c.view(np.float64)), c.shape[0], plane, _dp(out), engine) == 0
+        return out
+
+    def dense(self, x, row_begin=0, row_end=None, engine=0):
+        x = self._x(x)
+        row_end = self.n_rows if row_end is None else row_end
+        out = np.empty((x.shape[0], row_end - row_begin, self.N), dtype=np.complex128)
+        assert lib().qtam_ref_dense(self._h, _dp(x), x.shape[0], row_begin, row_end,
+                                    _dp(out.view(np.float64)), engine) == 0
+        return out
+
+    def brute_tile(self, x, k):
+        x = np.ascontiguousarray(x, dtype=np.float64).reshape(-1)
+        assert x.size == self.N
+        out = np.empty(self.N, dtype=np.complex128)
+        assert lib().qtam_ref_brute_tile(self._h, _dp(x), k, _dp(out.view(np.float64))) == 0
+        return out
+
+    def threshold(self, coef, kappa=3.0):
+        c = np.array(coef, dtype=np.complex128, order="C", copy=True)
+        if c.ndim == 1:
+            c = c[None, :]
+        assert lib().qtam_ref_threshold_rowmedian(self._h, _dp(c.view(np.float64)), c.shape[0], kappa) == 0
+        return c
+
+    def threshold_f32(self, coef, kappa=3.0):
+        c = np.array(coef, dtype=np.complex64, order="C", copy=True)
+        if c.ndim == 1:
+            c = c[None, :]
+        ptr = c.view(np.float32).ctypes.data_as(C.POINTER(C.c_float))
+        assert lib().qtam_ref_threshold_rowmedian_f32(self._h, ptr, c.shape[0], kappa) == 0
+        return c
+
+    def project_cover(self, x, plane=-1, engine=0):
+        x = self._x(x)
+        out = np.empty_like(x)
+        assert lib().qtam_ref_project_cover(self._h, _dp(x), x.shape[0], plane, _dp(out), engine) == 0
+        return out
+
+    def spectrum(self, x, engine=0):
+        x = self._x(x)
+        out = np.empty((x.shape[0], self.n_bins), dtype=np.complex128)
+        assert lib().qtam_ref_spectrum(self._h, _dp(x), x.shape[0], _dp(out.view(np.float64)), engine) == 0
+        return out
+
+    def row_slice(self, k):
+        r = self.rows[k]
+        return slice(int(r.offset), int(r.offset + r.M))
