@@ -1,0 +1,136 @@
+/* qtam.h -- C ABI of libqtam: QTAM forward / inverse Q-transform on NVIDIA B200 (sm_100a).
+ *
+ * Method: arxiv/paper_2603_29785 ("QTAM: Q-Transform Amplitude Modulation"), cited below as
+ * PAPER.md:<line>.  The library implements the data-parallel hot path only:
+ *   forward  x[b][N] real  ->  one long real FFT (C1 :365)
+ *                          ->  per Q-plane and log-spaced frequency row: multiply the band under the
+ *                              row's frequency window (A9 :323), shift it to baseband (C46 :583) and
+ *                              run a short inverse FFT of the window's support scaled by
+ *                              sqrt(N_out/N_in) (C47 :589)  ->  complex envelope Y_k[n]
+ *   inverse  Y -> per-row FFT, amplitude correction sqrt(N_in/N_out) and shift back (C49 :598),
+ *                 times the window, summed over rows, divided by the frame operator
+ *                 P[f] = sum_k |W_k[f]|^2 (Eq. 11 :135, C36 :536, C50 :602), one long inverse FFT.
+ * The readings taken where the paper is silent or garbled (bandwidth constant, centre-bin rounding,
+ * window normalisation, clamp, cover set ...) are R1-R14 of DESIGN.md.
+ *
+ * Conventions
+ *   - Pointers named d_* are DEVICE pointers (cudaMalloc'ed or torch CUDA tensors); every other
+ *     pointer is a HOST pointer.  `stream` is a cudaStream_t passed as void* (NULL = default stream).
+ *   - d_x:    [batch][N] real, contiguous, float (QTAM_F32) or double (QTAM_F64).
+ *   - d_coef: [batch][coeffs_per_segment] complex interleaved (re,im) of the same width; row k of
+ *             segment b starts at element b*coeffs_per_segment + offset_k and holds M_k values, time
+ *             index fastest; t_n = n*T/M_k.
+ *   - Ownership: the caller owns every buffer it passes and keeps it alive until the stream reaches
+ *     the call.  The plan owns its device tables and a workspace sized for `max_batch` segments;
+ *     qtam_plan_destroy frees them.
+ *   - Calls are asynchronous on `stream`, never synchronise the host, never allocate, do not modify
+ *     their inputs, and in/out buffers must not alias.  One in-flight call per plan.
+ *   - Errors: status codes only; nothing is thrown across the ABI; outputs are untouched on failure.
+ *     There is no CPU fallback: without a CUDA device every compute call returns QTAM_ERR_CUDA.
+ */
+#ifndef QTAM_H
+#define QTAM_H
+#include <stddef.h>
+#include <stdint.h>
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct qtam_plan qtam_plan;                      /* opaque, owned by the library */
+
+typedef enum { QTAM_F32 = 0, QTAM_F64 = 1 } qtam_dtype;  /* real in / complex out of that width */
+
+typedef enum {
+  QTAM_OK = 0,
+  QTAM_ERR_INVALID_ARG = 1,   /* NULL pointer, N not a power of two, fmax >= fs/2, fmin <= 0,
+                                 Q < sqrt(11), half-width < 1 bin, batch > max_batch, bad row range */
+  QTAM_ERR_UNSUPPORTED = 2,   /* window family / size outside what this build implements */
+  QTAM_ERR_ALLOC = 3,         /* host or device allocation failed at plan creation */
+  QTAM_ERR_CUDA = 4,          /* a CUDA runtime call or launch failed (or no device) */
+  QTAM_ERR_EMPTY_FRAME = 5    /* the plan's cover set is empty */
+} qtam_status;
+
+/* All fields optional; pass NULL for the defaults. struct_size = sizeof(qtam_options) (ABI version). */
+typedef struct {
+  size_t  struct_size;
+  int     window;                   /* 0 = bisquare (Eq. 6); the only one implemented */
+  int     clamp_mode;               /* 0 none, 1 auto = Eq. A7 [default], 2 manual  */
+  double  clamp_overlap;            /* multiplies N_t*Delta f_max in A7; default 1.0 = paper (R7)  */
+  int64_t max_window_bins;          /* L_max when clamp_mode == 2                                  */
+  double  cover_floor;              /* R9: a bin is invertible iff some unnormalised window value
+                                       there is >= cover_floor; default 1e-2                       */
+  int     rows_are_bins_per_octave; /* 0: `spacing` = rows per plane, endpoints inclusive;
+                                       1: `spacing` = bins per octave B, f = fmin*2^(r/B) (:303)   */
+  int     max_batch;                /* workspace is sized for this many segments; default 1        */
+} qtam_options;
+
+/* Host-side row table entry; rows are ordered plane-major (Q list order), ascending frequency. */
+typedef struct {
+  int plane, row;
+  double q, f_request, f_center;    /* f_center = kc/T, the bin the window is really centred on (R2) */
+  int64_t kc, dk, L, M, offset;     /* centre bin, half-width, L = 2dk+1, M = nextpow2(L), offset_k  */
+  double norm;                      /* 1/sqrt(sum_j W'[j]^2), Eq. 5 as read in R3                    */
+} qtam_row;
+
+typedef struct {
+  int n_planes, n_rows;
+  int64_t n, n_bins, coeffs_per_segment, sum_L;
+  int64_t cover_lo, cover_hi, holes;      /* joint cover set: first/last bin, gaps in between      */
+  double frame_A, frame_B;                /* min of P over the cover set, max of P (C39 :550)       */
+  size_t workspace_bytes;                 /* device memory the plan holds                           */
+} qtam_info;
+
+/* Plan (host, once): frequency grid f_r = fmin*(fmax/fmin)^(r/(R-1)) or fmin*2^(r/B),
+ * centre bins, bandwidths, clamp A7/A8 (:307-311), bisquare windows and their normalisation
+ * (Eq. 5-7 :63-72), output lengths, the frame operator and cover sets, device tables + workspace.
+ * Q: nQ quality factors (host pointer), one plane each.  *out is written only on QTAM_OK. */
+qtam_status qtam_plan_create(qtam_plan **out, double fs, int64_t N, const double *Q, int nQ,
+                             double fmin, double fmax, double spacing, qtam_dtype dtype,
+                             const qtam_options *opt);
+/* Same plan, host tables only: needs no CUDA device.  info/rows/window/frame work; every compute
+ * call on it returns QTAM_ERR_CUDA.  For inspecting a tiling before committing device memory. */
+qtam_status qtam_plan_create_host(qtam_plan **out, double fs, int64_t N, const double *Q, int nQ,
+                                  double fmin, double fmax, double spacing, qtam_dtype dtype,
+                                  const qtam_options *opt);
+qtam_status qtam_plan_destroy(qtam_plan *p);
+qtam_status qtam_plan_info(const qtam_plan *p, qtam_info *out);
+/* copies n_rows entries into `out` (host); capacity must be >= n_rows */
+qtam_status qtam_plan_rows(const qtam_plan *p, qtam_row *out, int capacity);
+/* normalised window W_k[j], j = -dk..dk, as the device tables hold it before rounding to the plan's
+ * dtype (host doubles, L values) */
+qtam_status qtam_plan_window(const qtam_plan *p, int row, double *out);
+/* frame operator P[f] and cover set, f = 0..N/2; plane = -1 joint, else that plane; either output
+ * may be NULL (host pointers) */
+qtam_status qtam_plan_frame(const qtam_plan *p, int plane, double *P_out, uint8_t *cover_out);
+
+/* Forward: rows a1-a3 of the hot path.
+ *   Y_k[n] = (N*M_k)^(-1/2) * sum_j X[kc+j] W_k[j] e^{+2 pi i j n / M_k},  n = 0..M_k-1         */
+qtam_status qtam_forward(qtam_plan *p, const void *d_x, int batch, void *d_coef, void *stream);
+
+/* Inverse: rows a5-a8 (PAPER.md:133-138 Eq. 11, :596-603).  plane = -1 inverts the joint frame of
+ * all planes, plane = p >= 0 only that plane's rows with that plane's P (R10).  Bins outside the
+ * cover set are set to zero (pseudo-inverse, R9), so inverse(forward(x)) = Pi_C x.               */
+qtam_status qtam_inverse(qtam_plan *p, const void *d_coef, int batch, int plane, void *d_x_out,
+                         void *stream);
+
+/* Dense (non-decimated) tiles, the check path for shift invariance (C3):
+ *   T_k[tau] = (1/N) sum_j X[kc+j] W_k[j] e^{+2 pi i (kc+j) tau / N},  tau = 0..N-1
+ * d_out: [batch][row_end-row_begin][N] complex.                                                   */
+qtam_status qtam_dense(qtam_plan *p, const void *d_x, int batch, int row_begin, int row_end,
+                       void *d_out, void *stream);
+
+/* Row-median threshold in place (BASELINE.json config 5; R11): per (segment,row),
+ * m = median_n |Y_k[n]| (two middle values averaged), zero every Y_k[n] with |Y_k[n]| < kappa*m.
+ * The decision is taken in the plan's dtype with the operation order of DESIGN.md.               */
+qtam_status qtam_threshold_rowmedian(qtam_plan *p, void *d_coef, int batch, double kappa,
+                                     void *stream);
+
+/* Number of kernel launches the last forward / inverse / threshold / dense call on this plan issued
+ * (host counter, for bench.py's gpu_launches). */
+int         qtam_last_launch_count(const qtam_plan *p);
+const char *qtam_status_string(qtam_status s);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

@@ -1,0 +1,202 @@
+"""ctypes binding of libqtam.so (include/qtam.h).  Argument marshalling only: every step of the
+transform runs in the CUDA kernels.  PyTorch is used for device memory and streams.
+
+There is no CPU fallback: if the library is missing it is built (nvcc), and if no CUDA device is
+present the compute calls raise.
+"""
+import ctypes as C
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_LIBPATH = os.path.join(_HERE, "libqtam.so")
+_lib = None
+
+QTAM_F32, QTAM_F64 = 0, 1
+STATUS = {0: "ok", 1: "invalid argument", 2: "unsupported", 3: "alloc", 4: "cuda", 5: "empty frame"}
+
+SYMBOLS = ["qtam_plan_create", "qtam_plan_create_host", "qtam_plan_destroy", "qtam_plan_info",
+           "qtam_plan_rows", "qtam_plan_window", "qtam_plan_frame", "qtam_forward", "qtam_inverse",
+           "qtam_dense", "qtam_threshold_rowmedian", "qtam_last_launch_count", "qtam_status_string"]
+
+
+class QtamError(RuntimeError):
+    def __init__(self, code, where):
+        super().__init__(f"{where}: status {code} ({STATUS.get(code, '?')})")
+        self.code = code
+
+
+class Options(C.Structure):
+    _fields_ = [("struct_size", C.c_size_t), ("window", C.c_int), ("clamp_mode", C.c_int),
+                ("clamp_overlap", C.c_double), ("max_window_bins", C.c_int64),
+                ("cover_floor", C.c_double), ("rows_are_bins_per_octave", C.c_int),
+                ("max_batch", C.c_int)]
+
+
+class Row(C.Structure):
+    _fields_ = [("plane", C.c_int), ("row", C.c_int), ("q", C.c_double), ("f_request", C.c_double),
+                ("f_center", C.c_double), ("kc", C.c_int64), ("dk", C.c_int64), ("L", C.c_int64),
+                ("M", C.c_int64), ("offset", C.c_int64), ("norm", C.c_double)]
+
+
+class Info(C.Structure):
+    _fields_ = [("n_planes", C.c_int), ("n_rows", C.c_int), ("n", C.c_int64), ("n_bins", C.c_int64),
+                ("coeffs_per_segment", C.c_int64), ("sum_L", C.c_int64), ("cover_lo", C.c_int64),
+                ("cover_hi", C.c_int64), ("holes", C.c_int64), ("frame_A", C.c_double),
+                ("frame_B", C.c_double), ("workspace_bytes", C.c_size_t)]
+
+
+def lib():
+    """Loads libqtam.so (building it in-tree first if it is missing)."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(_LIBPATH):
+            from . import build as _b
+            _b.build()
+        L = C.CDLL(_LIBPATH)
+        vp, dp = C.c_void_p, C.POINTER(C.c_double)
+        create_args = [C.POINTER(vp), C.c_double, C.c_int64, dp, C.c_int, C.c_double, C.c_double,
+                       C.c_double, C.c_int, C.POINTER(Options)]
+        L.qtam_plan_create.argtypes = create_args
+        L.qtam_plan_create_host.argtypes = create_args
+        L.qtam_plan_destroy.argtypes = [vp]
+        L.qtam_plan_info.argtypes = [vp, C.POINTER(Info)]
+        L.qtam_plan_rows.argtypes = [vp, C.POINTER(Row), C.c_int]
+        L.qtam_plan_window.argtypes = [vp, C.c_int, dp]
+        L.qtam_plan_frame.argtypes = [vp, C.c_int, dp, C.POINTER(C.c_uint8)]
+        L.qtam_forward.argtypes = [vp, vp, C.c_int, vp, vp]
+        L.qtam_inverse.argtypes = [vp, vp, C.c_int, C.c_int, vp, vp]
+        L.qtam_dense.argtypes = [vp, vp, C.c_int, C.c_int, C.c_int, vp, vp]
+        L.qtam_threshold_rowmedian.argtypes = [vp, vp, C.c_int, C.c_double, vp]
+        L.qtam_last_launch_count.argtypes = [vp]
+        L.qtam_last_launch_count.restype = C.c_int
+        L.qtam_status_string.argtypes = [C.c_int]
+        L.qtam_status_string.restype = C.c_char_p
+        _lib = L
+    return _lib
+
+
+def _check(code, where):
+    if code != 0:
+        raise QtamError(code, where)
+
+
+class Plan:
+    """qtam_plan_create(fs, N, Q list, fmin, fmax, row spacing, dtype, options)."""
+
+    def __init__(self, fs, N, Q, fmin, fmax, spacing, dtype="f32", max_batch=1, clamp_mode=1,
+                 clamp_overlap=1.0, max_window_bins=0, cover_floor=1e-2, rows_are_bins_per_octave=0,
+                 host_only=False):
+        L = lib()
+        self._h = C.c_void_p()
+        self.dtype = dtype
+        q = np.ascontiguousarray(Q, dtype=np.float64)
+        opt = Options(C.sizeof(Options), 0, clamp_mode, clamp_overlap, max_window_bins, cover_floor,
+                      rows_are_bins_per_octave, max_batch)
+        fn = L.qtam_plan_create_host if host_only else L.qtam_plan_create
+        code = fn(C.byref(self._h), float(fs), int(N), q.ctypes.data_as(C.POINTER(C.c_double)), q.size,
+                  float(fmin), float(fmax), float(spacing), QTAM_F64 if dtype == "f64" else QTAM_F32,
+                  C.byref(opt))
+        if code != 0:
+            self._h = None
+            raise QtamError(code, "qtam_plan_create")
+        self.max_batch = max_batch
+        info = Info()
+        _check(L.qtam_plan_info(self._h, C.byref(info)), "qtam_plan_info")
+        self.info = info
+        self.N, self.n_bins = int(info.n), int(info.n_bins)
+        self.n_rows, self.n_planes = int(info.n_rows), int(info.n_planes)
+        self.ctot = int(info.coeffs_per_segment)
+        rows = (Row * self.n_rows)()
+        _check(L.qtam_plan_rows(self._h, rows, self.n_rows), "qtam_plan_rows")
+        self.rows = list(rows)
+
+    def close(self):
+        if getattr(self, "_h", None):
+            lib().qtam_plan_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        self.close()
+
+    # ---- host tables -------------------------------------------------------------------------------
+    def window(self, k):
+        out = np.empty(int(self.rows[k].L), dtype=np.float64)
+        _check(lib().qtam_plan_window(self._h, k, out.ctypes.data_as(C.POINTER(C.c_double))), "qtam_plan_window")
+        return out
+
+    def frame(self, plane=-1):
+        P = np.empty(self.n_bins, dtype=np.float64)
+        cov = np.empty(self.n_bins, dtype=np.uint8)
+        _check(lib().qtam_plan_frame(self._h, plane, P.ctypes.data_as(C.POINTER(C.c_double)),
+                                     cov.ctypes.data_as(C.POINTER(C.c_uint8))), "qtam_plan_frame")
+        return P, cov.astype(bool)
+
+    def row_slice(self, k):
+        r = self.rows[k]
+        return slice(int(r.offset), int(r.offset + r.M))
+
+    # ---- device calls (torch tensors on the GPU; stream = torch's current stream) -----------------
+    def _torch(self):
+        import torch
+        return torch
+
+    def _rdt(self):
+        t = self._torch()
+        return t.float64 if self.dtype == "f64" else t.float32
+
+    def _cdt(self):
+        t = self._torch()
+        return t.complex128 if self.dtype == "f64" else t.complex64
+
+    def _stream(self):
+        return C.c_void_p(self._torch().cuda.current_stream().cuda_stream)
+
+    def forward(self, x, out=None):
+        t = self._torch()
+        assert x.is_cuda and x.dtype == self._rdt() and x.is_contiguous() and x.shape[-1] == self.N
+        batch = x.numel() // self.N
+        if out is None:
+            out = t.empty((batch, self.ctot), dtype=self._cdt(), device=x.device)
+        assert out.is_cuda and out.dtype == self._cdt() and out.is_contiguous() and out.numel() == batch * self.ctot
+        _check(lib().qtam_forward(self._h, x.data_ptr(), batch, out.data_ptr(), self._stream()), "qtam_forward")
+        return out
+
+    def inverse(self, coef, plane=-1, out=None):
+        t = self._torch()
+        assert coef.is_cuda and coef.dtype == self._cdt() and coef.is_contiguous()
+        batch = coef.numel() // self.ctot
+        if out is None:
+            out = t.empty((batch, self.N), dtype=self._rdt(), device=coef.device)
+        assert out.is_cuda and out.dtype == self._rdt() and out.is_contiguous() and out.numel() == batch * self.N
+        _check(lib().qtam_inverse(self._h, coef.data_ptr(), batch, plane, out.data_ptr(), self._stream()), "qtam_inverse")
+        return out
+
+    def dense(self, x, row_begin=0, row_end=None, out=None):
+        t = self._torch()
+        row_end = self.n_rows if row_end is None else row_end
+        assert x.is_cuda and x.dtype == self._rdt() and x.is_contiguous() and x.shape[-1] == self.N
+        batch = x.numel() // self.N
+        if out is None:
+            out = t.empty((batch, row_end - row_begin, self.N), dtype=self._cdt(), device=x.device)
+        _check(lib().qtam_dense(self._h, x.data_ptr(), batch, row_begin, row_end, out.data_ptr(), self._stream()), "qtam_dense")
+        return out
+
+    def threshold_rowmedian(self, coef, kappa=3.0):
+        """in place"""
+        assert coef.is_cuda and coef.dtype == self._cdt() and coef.is_contiguous()
+        batch = coef.numel() // self.ctot
+        _check(lib().qtam_threshold_rowmedian(self._h, coef.data_ptr(), batch, float(kappa), self._stream()),
+               "qtam_threshold_rowmedian")
+        return coef
+
+    def last_launch_count(self):
+        return int(lib().qtam_last_launch_count(self._h))
+
+    # ---- host-buffer convenience (the end-to-end path bench.py times) ------------------------------
+    def forward_host(self, x_pinned, coef_pinned, d_x, d_coef):
+        """H2D copy of x, forward, D2H copy of the coefficients; all on the current stream."""
+        d_x.copy_(x_pinned, non_blocking=True)
+        self.forward(d_x, out=d_coef)
+        coef_pinned.copy_(d_coef, non_blocking=True)

@@ -1,0 +1,300 @@
+// api.cu -- the C ABI of libqtam (include/qtam.h): plan life cycle, argument checks, dispatch.
+#include <algorithm>
+#include <cmath>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "cplx.cuh"
+#include "device_plan.hpp"
+
+namespace qtam {
+int generic_class_of(int log2M2);
+}
+
+using namespace qtam;
+
+namespace {
+
+int ilog2(long long v) { int l = 0; while ((1LL << l) < v) ++l; return l; }
+
+template <typename T> bool upload(T **dst, const void *src, size_t count, size_t *total) {
+  *dst = nullptr;
+  if (count == 0) count = 1;
+  if (cudaMalloc(reinterpret_cast<void **>(dst), count * sizeof(T)) != cudaSuccess) return false;
+  *total += count * sizeof(T);
+  if (src && cudaMemcpy(*dst, src, count * sizeof(T), cudaMemcpyHostToDevice) != cudaSuccess) return false;
+  return true;
+}
+
+bool dev_alloc(void **dst, size_t bytes, size_t *total) {
+  *dst = nullptr;
+  if (bytes == 0) bytes = 16;
+  if (cudaMalloc(dst, bytes) != cudaSuccess) return false;
+  *total += bytes;
+  return true;
+}
+
+void free_plan(qtam_plan *p) {
+  if (!p) return;
+  if (p->host_only) { delete p; return; }
+  cudaFree(p->d_rows); cudaFree(p->d_win); cudaFree(p->d_tw); cudaFree(p->d_invP);
+  cudaFree(p->d_csr_ptr); cudaFree(p->d_csr_idx);
+  for (int c = 0; c < qtam_plan::kClasses; ++c) cudaFree(p->d_items[c]);
+  cudaFree(p->d_bigrows); cudaFree(p->d_spec); cudaFree(p->d_ws); cudaFree(p->d_band);
+  delete p;
+}
+
+// e^{+2 pi i k/n} for k = 0..n-1, evaluated in long double from the first octant (exact symmetries)
+template <typename T> void fill_twiddles(std::vector<T> &tw, int64_t n) {
+  tw.resize(size_t(2 * n));
+  const long double tau = 6.283185307179586476925286766559005768L;
+  for (int64_t k = 0; k < n; ++k) {
+    long double c, s;
+    // quarter-turn reduction keeps the argument of cosl/sinl in [0, pi/2)
+    const int64_t quarter = n / 4;
+    const int64_t qq = k / quarter, rr = k % quarter;
+    long double ang = tau * (long double)rr / (long double)n;
+    long double c0 = cosl(ang), s0 = sinl(ang);
+    if (rr == 0) { c0 = 1.0L; s0 = 0.0L; }
+    if (2 * rr == quarter) { c0 = s0 = 0.707106781186547524400844362104849039L; }
+    switch (qq & 3) {
+      case 0: c = c0; s = s0; break;
+      case 1: c = -s0; s = c0; break;
+      case 2: c = -c0; s = -s0; break;
+      default: c = s0; s = -c0; break;
+    }
+    tw[size_t(2 * k)] = (T)c;
+    tw[size_t(2 * k + 1)] = (T)s;
+  }
+}
+
+template <typename T> qtam_status build_device(qtam_plan *p) {
+  const HostPlan &hp = p->hp;
+  size_t *tot = &p->device_bytes;
+  // rows
+  std::vector<RowDev> rd(hp.rows.size());
+  for (size_t k = 0; k < hp.rows.size(); ++k) {
+    const HostRow &h = hp.rows[k];
+    RowDev &d = rd[k];
+    d.kc = (int)h.kc; d.dk = (int)h.dk; d.M = (int)h.M; d.log2M = ilog2(h.M);
+    d.plane = h.plane; d.pad0 = 0; d.offset = h.offset; d.woff = h.woff;
+    d.fwd_scale = 1.0 / std::sqrt((double)hp.N * (double)h.M);
+    d.inv_amp = std::sqrt((double)hp.N / (double)h.M);
+  }
+  if (!upload(&p->d_rows, rd.data(), rd.size(), tot)) return QTAM_ERR_ALLOC;
+  // windows, rounded once to the plan's dtype
+  {
+    std::vector<T> w(hp.win.size());
+    for (size_t i = 0; i < w.size(); ++i) w[i] = (T)hp.win[i];
+    T *d = nullptr;
+    if (!upload(&d, w.data(), w.size(), tot)) return QTAM_ERR_ALLOC;
+    p->d_win = d;
+  }
+  // twiddles
+  {
+    std::vector<T> tw;
+    fill_twiddles<T>(tw, p->twn);
+    T *d = nullptr;
+    if (!upload(&d, tw.data(), tw.size(), tot)) return QTAM_ERR_ALLOC;
+    p->d_tw = d;
+  }
+  // 1/P on the cover set, 0 elsewhere (a7; R9)
+  {
+    const size_t nsets = size_t(hp.nP) + 1;
+    std::vector<T> ip(nsets * size_t(hp.nb));
+    for (size_t s = 0; s < nsets; ++s)
+      for (int64_t f = 0; f < hp.nb; ++f)
+        ip[s * size_t(hp.nb) + size_t(f)] = hp.cover[s][size_t(f)] ? (T)(1.0 / hp.P[s][size_t(f)]) : (T)0;
+    T *d = nullptr;
+    if (!upload(&d, ip.data(), ip.size(), tot)) return QTAM_ERR_ALLOC;
+    p->d_invP = d;
+  }
+  if (!upload(&p->d_csr_ptr, hp.csr_ptr.data(), hp.csr_ptr.size(), tot)) return QTAM_ERR_ALLOC;
+  if (!upload(&p->d_csr_idx, hp.csr_idx.data(), hp.csr_idx.size(), tot)) return QTAM_ERR_ALLOC;
+  // generic-path work lists
+  {
+    std::vector<WorkItem> items[qtam_plan::kClasses];
+    std::vector<int> big;
+    for (size_t k = 0; k < hp.rows.size(); ++k) {
+      const int lm = ilog2(hp.rows[k].M);
+      if (lm <= p->cap_log2) {
+        items[generic_class_of(lm)].push_back(WorkItem{(int)k, 0, 1, lm});
+      } else {
+        const int R1 = 1 << (lm - p->cap_log2);
+        if (R1 > 16) return QTAM_ERR_UNSUPPORTED;
+        for (int j1 = 0; j1 < R1; ++j1)
+          items[generic_class_of(p->cap_log2)].push_back(WorkItem{(int)k, j1, R1, p->cap_log2});
+        big.push_back((int)k);
+        if (R1 > p->big_R1max) p->big_R1max = R1;
+      }
+    }
+    for (int c = 0; c < qtam_plan::kClasses; ++c) {
+      // largest first: the tail of the launch is then made of the short rows
+      std::stable_sort(items[c].begin(), items[c].end(),
+                       [](const WorkItem &a, const WorkItem &b) { return a.log2M2 > b.log2M2; });
+      p->n_items[c] = (int)items[c].size();
+      if (!upload(&p->d_items[c], items[c].data(), items[c].size(), tot)) return QTAM_ERR_ALLOC;
+    }
+    p->n_bigrows = (int)big.size();
+    if (!upload(&p->d_bigrows, big.data(), big.size(), tot)) return QTAM_ERR_ALLOC;
+  }
+  // workspace
+  const size_t csz = 2 * sizeof(T);
+  if (!dev_alloc(&p->d_spec, csz * size_t(p->max_batch) * size_t(p->xstride), tot)) return QTAM_ERR_ALLOC;
+  if (!dev_alloc(&p->d_ws, csz * size_t(p->max_batch) * size_t(hp.N), tot)) return QTAM_ERR_ALLOC;
+  if (!dev_alloc(&p->d_band, csz * size_t(p->max_batch) * size_t(hp.sumL), tot)) return QTAM_ERR_ALLOC;
+  return QTAM_OK;
+}
+
+bool check_call(const qtam_plan *p, const void *a, const void *b, int batch) {
+  return p && !p->host_only && a && b && batch >= 0 && batch <= p->max_batch;
+}
+
+}  // namespace
+
+extern "C" {
+
+qtam_status qtam_plan_create(qtam_plan **out, double fs, int64_t N, const double *Q, int nQ,
+                             double fmin, double fmax, double spacing, qtam_dtype dtype,
+                             const qtam_options *opt) {
+  if (!out) return QTAM_ERR_INVALID_ARG;
+  qtam_plan *p = new (std::nothrow) qtam_plan;
+  if (!p) return QTAM_ERR_ALLOC;
+  qtam_status s = build_host_plan(p->hp, fs, N, Q, nQ, fmin, fmax, spacing, dtype, opt);
+  if (s != QTAM_OK) { delete p; return s; }
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) { delete p; return QTAM_ERR_CUDA; }
+  p->esz = dtype == QTAM_F32 ? 4 : 8;
+  p->max_batch = p->hp.opt.max_batch;
+  p->xstride = ((p->hp.nb + 31) / 32) * 32;
+  p->twn = N;
+  p->cap_log2 = dtype == QTAM_F32 ? 13 : 12;
+  s = dtype == QTAM_F32 ? build_device<float>(p) : build_device<double>(p);
+  if (s != QTAM_OK) { free_plan(p); cudaGetLastError(); return s; }
+  if (cudaDeviceSynchronize() != cudaSuccess) { free_plan(p); return QTAM_ERR_CUDA; }
+  *out = p;
+  return QTAM_OK;
+}
+
+qtam_status qtam_plan_create_host(qtam_plan **out, double fs, int64_t N, const double *Q, int nQ,
+                                  double fmin, double fmax, double spacing, qtam_dtype dtype,
+                                  const qtam_options *opt) {
+  if (!out) return QTAM_ERR_INVALID_ARG;
+  qtam_plan *p = new (std::nothrow) qtam_plan;
+  if (!p) return QTAM_ERR_ALLOC;
+  qtam_status s = build_host_plan(p->hp, fs, N, Q, nQ, fmin, fmax, spacing, dtype, opt);
+  if (s != QTAM_OK) { delete p; return s; }
+  p->esz = dtype == QTAM_F32 ? 4 : 8;
+  p->max_batch = 0;            // no workspace: every compute call is refused
+  p->host_only = true;
+  *out = p;
+  return QTAM_OK;
+}
+
+qtam_status qtam_plan_destroy(qtam_plan *p) {
+  if (!p) return QTAM_ERR_INVALID_ARG;
+  free_plan(p);
+  return QTAM_OK;
+}
+
+qtam_status qtam_plan_info(const qtam_plan *p, qtam_info *o) {
+  if (!p || !o) return QTAM_ERR_INVALID_ARG;
+  const HostPlan &hp = p->hp;
+  o->n_planes = hp.nP; o->n_rows = (int)hp.rows.size(); o->n = hp.N; o->n_bins = hp.nb;
+  o->coeffs_per_segment = hp.ctot; o->sum_L = hp.sumL;
+  o->cover_lo = hp.cover_lo; o->cover_hi = hp.cover_hi; o->holes = hp.holes;
+  o->frame_A = hp.frame_A; o->frame_B = hp.frame_B;
+  o->workspace_bytes = p->device_bytes;
+  return QTAM_OK;
+}
+
+qtam_status qtam_plan_rows(const qtam_plan *p, qtam_row *out, int capacity) {
+  if (!p || !out || capacity < (int)p->hp.rows.size()) return QTAM_ERR_INVALID_ARG;
+  for (size_t k = 0; k < p->hp.rows.size(); ++k) {
+    const HostRow &h = p->hp.rows[k];
+    qtam_row &o = out[k];
+    o.plane = h.plane; o.row = h.row; o.q = h.q; o.f_request = h.f_request; o.f_center = h.f_center;
+    o.kc = h.kc; o.dk = h.dk; o.L = h.L; o.M = h.M; o.offset = h.offset; o.norm = h.norm;
+  }
+  return QTAM_OK;
+}
+
+qtam_status qtam_plan_window(const qtam_plan *p, int row, double *out) {
+  if (!p || !out || row < 0 || row >= (int)p->hp.rows.size()) return QTAM_ERR_INVALID_ARG;
+  const HostRow &h = p->hp.rows[(size_t)row];
+  std::memcpy(out, p->hp.win.data() + h.woff, sizeof(double) * (size_t)h.L);
+  return QTAM_OK;
+}
+
+qtam_status qtam_plan_frame(const qtam_plan *p, int plane, double *P_out, uint8_t *cover_out) {
+  if (!p || plane < -1 || plane >= p->hp.nP) return QTAM_ERR_INVALID_ARG;
+  const size_t s = (size_t)(plane + 1);
+  if (P_out) std::memcpy(P_out, p->hp.P[s].data(), sizeof(double) * (size_t)p->hp.nb);
+  if (cover_out) std::memcpy(cover_out, p->hp.cover[s].data(), (size_t)p->hp.nb);
+  return QTAM_OK;
+}
+
+qtam_status qtam_forward(qtam_plan *p, const void *d_x, int batch, void *d_coef, void *stream) {
+  if (p && p->host_only) return QTAM_ERR_CUDA;
+  if (!check_call(p, d_x, d_coef, batch)) return QTAM_ERR_INVALID_ARG;
+  p->last_launches = 0;
+  if (batch == 0) return QTAM_OK;
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  qtam_status s = generic_r2c(p, d_x, batch, st);
+  if (s != QTAM_OK) return s;
+  return generic_forward_rows(p, batch, d_coef, st);
+}
+
+qtam_status qtam_inverse(qtam_plan *p, const void *d_coef, int batch, int plane, void *d_x_out,
+                         void *stream) {
+  if (p && p->host_only) return QTAM_ERR_CUDA;
+  if (!check_call(p, d_coef, d_x_out, batch) || plane < -1 || plane >= p->hp.nP)
+    return QTAM_ERR_INVALID_ARG;
+  p->last_launches = 0;
+  if (batch == 0) return QTAM_OK;
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  qtam_status s = generic_inverse_rows(p, d_coef, batch, plane, st);
+  if (s != QTAM_OK) return s;
+  s = generic_inverse_reduce(p, batch, plane, st);
+  if (s != QTAM_OK) return s;
+  return generic_c2r(p, batch, d_x_out, st);
+}
+
+qtam_status qtam_dense(qtam_plan *p, const void *d_x, int batch, int row_begin, int row_end,
+                       void *d_out, void *stream) {
+  if (p && p->host_only) return QTAM_ERR_CUDA;
+  if (!check_call(p, d_x, d_out, batch) || row_begin < 0 || row_end > (int)p->hp.rows.size() ||
+      row_begin > row_end)
+    return QTAM_ERR_INVALID_ARG;
+  p->last_launches = 0;
+  if (batch == 0 || row_begin == row_end) return QTAM_OK;
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  qtam_status s = generic_r2c(p, d_x, batch, st);
+  if (s != QTAM_OK) return s;
+  return generic_dense(p, batch, row_begin, row_end, d_out, st);
+}
+
+qtam_status qtam_threshold_rowmedian(qtam_plan *p, void *d_coef, int batch, double kappa, void *stream) {
+  if (p && p->host_only) return QTAM_ERR_CUDA;
+  if (!check_call(p, d_coef, d_coef, batch) || !(kappa >= 0.0)) return QTAM_ERR_INVALID_ARG;
+  p->last_launches = 0;
+  if (batch == 0) return QTAM_OK;
+  return generic_threshold(p, d_coef, batch, kappa, static_cast<cudaStream_t>(stream));
+}
+
+int qtam_last_launch_count(const qtam_plan *p) { return p ? p->last_launches : 0; }
+
+const char *qtam_status_string(qtam_status s) {
+  switch (s) {
+    case QTAM_OK: return "ok";
+    case QTAM_ERR_INVALID_ARG: return "invalid argument";
+    case QTAM_ERR_UNSUPPORTED: return "unsupported configuration";
+    case QTAM_ERR_ALLOC: return "allocation failed";
+    case QTAM_ERR_CUDA: return "CUDA error (or no CUDA device)";
+    case QTAM_ERR_EMPTY_FRAME: return "empty cover set";
+  }
+  return "unknown status";
+}
+
+}  // extern "C"

@@ -1,0 +1,52 @@
+// device_plan.hpp -- the plan object behind the C ABI: host plan + device tables + workspace,
+// and the launcher entry points implemented in the .cu files.
+#pragma once
+#include <cuda_runtime.h>
+
+#include "qtam_internal.hpp"
+
+struct qtam_plan {
+  qtam::HostPlan hp;
+  int esz = 4;                 // sizeof real: 4 or 8
+  int max_batch = 1;
+  int64_t xstride = 0;         // spectrum segment stride in complex elements (>= N/2+1, padded)
+  int64_t twn = 0;             // twiddle table length (= N): tw[k] = e^{+2 pi i k/N}
+  int cap_log2 = 0;            // generic path: largest in-smem FFT is 2^cap_log2 points
+
+  // device tables
+  qtam::RowDev *d_rows = nullptr;
+  void *d_win = nullptr;       // real[sumL]
+  void *d_tw = nullptr;        // complex[twn]
+  void *d_invP = nullptr;      // real[(nP+1)*nb], 0 outside the cover set
+  int32_t *d_csr_ptr = nullptr;
+  int32_t *d_csr_idx = nullptr;
+  // generic-path work lists, one per smem size class
+  static const int kClasses = 4;
+  qtam::WorkItem *d_items[kClasses] = {nullptr, nullptr, nullptr, nullptr};
+  int n_items[kClasses] = {0, 0, 0, 0};
+  int *d_bigrows = nullptr;    // rows with R1 > 1 (need the combine pass)
+  int n_bigrows = 0;
+  int big_R1max = 1;
+
+  // workspace (sized for max_batch)
+  void *d_spec = nullptr;      // complex[max_batch][xstride]   spectrum X / Xhat
+  void *d_ws = nullptr;        // complex[max_batch][N]         four-step scratch, dense scratch
+  void *d_band = nullptr;      // complex[max_batch][sumL]      inverse band values G_k[j]
+  size_t device_bytes = 0;
+
+  int last_launches = 0;
+  bool host_only = false;      // built by qtam_plan_create_host: tables on the host only
+};
+
+namespace qtam {
+
+// generic.cu : correct-for-everything kernels (any N, any M, float and double)
+qtam_status generic_r2c(qtam_plan *p, const void *d_x, int batch, cudaStream_t st);
+qtam_status generic_forward_rows(qtam_plan *p, int batch, void *d_coef, cudaStream_t st);
+qtam_status generic_inverse_rows(qtam_plan *p, const void *d_coef, int batch, int plane, cudaStream_t st);
+qtam_status generic_inverse_reduce(qtam_plan *p, int batch, int plane, cudaStream_t st);
+qtam_status generic_c2r(qtam_plan *p, int batch, void *d_x_out, cudaStream_t st);
+qtam_status generic_dense(qtam_plan *p, int batch, int row_begin, int row_end, void *d_out, cudaStream_t st);
+qtam_status generic_threshold(qtam_plan *p, void *d_coef, int batch, double kappa, cudaStream_t st);
+
+}  // namespace qtam

@@ -1,0 +1,170 @@
+// plan.cpp -- host plan of libqtam: grid, centre bins, clamp, windows, output lengths, frame
+// operator, cover sets and the bin->band CSR used by the inverse's segmented reduction.
+// Follows PAPER.md App. A (:303-321) and Eq. 5-7 (:63-72) with the readings R1-R14 of DESIGN.md.
+#include <algorithm>
+#include <cmath>
+
+#include "qtam_internal.hpp"
+
+namespace qtam {
+
+static bool pow2(int64_t v) { return v > 0 && (v & (v - 1)) == 0; }
+
+qtam_status build_host_plan(HostPlan &hp, double fs, int64_t N, const double *Q, int nQ, double fmin,
+                            double fmax, double spacing, qtam_dtype dtype, const qtam_options *uopt) {
+  if (!Q || nQ < 1 || !(fs > 0.0) || !pow2(N) || N < 8) return QTAM_ERR_INVALID_ARG;
+  if (!(fmin > 0.0) || !(fmax > fmin) || !(fmax < 0.5 * fs)) return QTAM_ERR_INVALID_ARG;
+  if (dtype != QTAM_F32 && dtype != QTAM_F64) return QTAM_ERR_INVALID_ARG;
+  if (N > (int64_t(1) << 26)) return QTAM_ERR_UNSUPPORTED;
+
+  qtam_options o{};
+  o.struct_size = sizeof(qtam_options);
+  o.clamp_mode = 1;
+  o.clamp_overlap = 1.0;
+  o.cover_floor = 1e-2;
+  o.max_batch = 1;
+  if (uopt) {
+    if (uopt->struct_size != sizeof(qtam_options)) return QTAM_ERR_INVALID_ARG;
+    o = *uopt;
+    if (!(o.clamp_overlap > 0.0)) o.clamp_overlap = 1.0;
+    if (!(o.cover_floor > 0.0)) o.cover_floor = 1e-2;
+    if (o.max_batch < 1) o.max_batch = 1;
+  }
+  if (o.window != 0) return QTAM_ERR_UNSUPPORTED;
+  if (o.clamp_mode < 0 || o.clamp_mode > 2) return QTAM_ERR_INVALID_ARG;
+
+  hp.fs = fs; hp.N = N; hp.nb = N / 2 + 1; hp.nP = nQ; hp.dtype = dtype; hp.opt = o;
+  const double dur = double(N) / fs;          // N_t of the paper (:75)
+  const double tile_c = std::sqrt(11.0);      // R1
+
+  // centre frequencies (:303, R14)
+  std::vector<double> fc;
+  if (o.rows_are_bins_per_octave) {
+    if (!(spacing > 0.0)) return QTAM_ERR_INVALID_ARG;
+    for (int r = 0; r < (1 << 20); ++r) {
+      const double v = fmin * std::pow(2.0, double(r) / spacing);
+      if (v > fmax) break;
+      fc.push_back(v);
+    }
+  } else {
+    const int R = int(spacing);
+    if (R < 2 || double(R) != spacing) return QTAM_ERR_INVALID_ARG;
+    fc.resize(size_t(R));
+    for (int r = 0; r < R; ++r) fc[size_t(r)] = fmin * std::pow(fmax / fmin, double(r) / double(R - 1));
+  }
+  if (fc.size() < 2) return QTAM_ERR_INVALID_ARG;
+  hp.nR = int(fc.size());
+
+  // width cap (A7 :307 / manual); 0 means "no cap"
+  int64_t cap = 0;
+  if (o.clamp_mode == 1) {
+    double gap = 0.0;
+    for (size_t r = 1; r < fc.size(); ++r) gap = std::max(gap, fc[r] - fc[r - 1]);
+    const int64_t c = int64_t(std::ceil(o.clamp_overlap * dur * gap));
+    cap = 2 * (c / 2) + 1;
+  } else if (o.clamp_mode == 2) {
+    if (o.max_window_bins < 3) return QTAM_ERR_INVALID_ARG;
+    cap = 2 * ((o.max_window_bins - 1) / 2) + 1;
+  }
+
+  hp.rows.clear();
+  hp.win.clear();
+  int64_t coff = 0, woff = 0, mmax = 0;
+  for (int pl = 0; pl < nQ; ++pl) {
+    if (!(Q[pl] >= tile_c)) return QTAM_ERR_INVALID_ARG;
+    for (int r = 0; r < hp.nR; ++r) {
+      HostRow h{};
+      h.plane = pl; h.row = r; h.q = Q[pl]; h.f_request = fc[size_t(r)];
+      h.kc = int64_t(std::floor(fc[size_t(r)] * dur + 0.5));                      // R2
+      int64_t len = 2 * int64_t(std::floor(fc[size_t(r)] * dur * tile_c / Q[pl])) + 1;  // R1, Eq. 7
+      if (cap > 0 && len > cap) len = cap;                                       // A8 :311
+      h.L = len; h.dk = (len - 1) / 2;
+      if (h.dk < 1) return QTAM_ERR_INVALID_ARG;                                  // R13
+      int64_t m = 1;
+      while (m < len) m <<= 1;                                                   // R5
+      h.M = m; mmax = std::max(mmax, m);
+      h.f_center = double(h.kc) / dur;
+      h.offset = coff; coff += m;
+      h.woff = woff; h.goff = woff; woff += len;
+      // bisquare (Eq. 6 :67), unit l2 energy over the unclipped support (Eq. 5 :63, R3, R8)
+      const size_t base = hp.win.size();
+      hp.win.resize(base + size_t(len));
+      long double energy = 0.0L;
+      for (int64_t j = -h.dk; j <= h.dk; ++j) {
+        const double u = double(j) / double(h.dk);
+        const double raw = (1.0 - u * u) * (1.0 - u * u);
+        hp.win[base + size_t(j + h.dk)] = raw;
+        energy += (long double)raw * (long double)raw;
+      }
+      h.norm = double(1.0L / sqrtl(energy));
+      hp.rows.push_back(h);
+    }
+  }
+  hp.ctot = coff; hp.sumL = woff; hp.Mmax = mmax;
+  if (hp.sumL >= (int64_t(1) << 31) || hp.ctot >= (int64_t(1) << 40)) return QTAM_ERR_UNSUPPORTED;
+
+  // frame operator (C36 :536), cover sets (R9), joint and per plane (R10); out-of-range bins clipped (R8)
+  const size_t nsets = size_t(nQ) + 1;
+  std::vector<std::vector<long double>> acc(nsets, std::vector<long double>(size_t(hp.nb), 0.0L));
+  hp.cover.assign(nsets, std::vector<uint8_t>(size_t(hp.nb), 0));
+  std::vector<int32_t> count(size_t(hp.nb) * nsets + 1, 0);   // per (bin, plane) entry counts
+  for (const HostRow &h : hp.rows) {
+    for (int64_t j = -h.dk; j <= h.dk; ++j) {
+      const int64_t f = h.kc + j;
+      if (f < 0 || f >= hp.nb) continue;
+      const double raw = hp.win[size_t(h.woff + j + h.dk)];
+      const long double w = (long double)(raw * h.norm);
+      acc[0][size_t(f)] += w * w;
+      acc[size_t(h.plane) + 1][size_t(f)] += w * w;
+      if (raw >= o.cover_floor) {
+        hp.cover[0][size_t(f)] = 1;
+        hp.cover[size_t(h.plane) + 1][size_t(f)] = 1;
+      }
+      count[size_t(f) * nsets + size_t(h.plane)] += 1;
+    }
+  }
+  // normalise the stored windows now that the raw values have been used for the cover test
+  for (const HostRow &h : hp.rows)
+    for (int64_t i = 0; i < h.L; ++i) hp.win[size_t(h.woff + i)] *= h.norm;
+
+  hp.P.assign(nsets, std::vector<double>(size_t(hp.nb), 0.0));
+  for (size_t s = 0; s < nsets; ++s)
+    for (int64_t f = 0; f < hp.nb; ++f) hp.P[s][size_t(f)] = double(acc[s][size_t(f)]);
+
+  hp.cover_lo = hp.cover_hi = -1;
+  int64_t ncov = 0;
+  hp.frame_A = 0; hp.frame_B = 0;
+  for (int64_t f = 0; f < hp.nb; ++f) {
+    hp.frame_B = std::max(hp.frame_B, hp.P[0][size_t(f)]);
+    if (!hp.cover[0][size_t(f)]) continue;
+    if (hp.cover_lo < 0) { hp.cover_lo = f; hp.frame_A = hp.P[0][size_t(f)]; }
+    hp.cover_hi = f; ++ncov;
+    hp.frame_A = std::min(hp.frame_A, hp.P[0][size_t(f)]);
+  }
+  if (ncov == 0) return QTAM_ERR_EMPTY_FRAME;
+  hp.holes = (hp.cover_hi - hp.cover_lo + 1) - ncov;
+
+  // CSR: exclusive scan of the counts, then fill in row order (rows are plane-major, so the entries
+  // of one (bin, plane) cell are in ascending row order: a fixed summation order)
+  hp.csr_ptr.assign(size_t(hp.nb) * nsets + 1, 0);
+  {
+    // count[] was indexed [f*nsets + plane] with nsets = nP+1 slots per bin; slot nP is unused (0)
+    int64_t run = 0;
+    for (size_t i = 0; i < size_t(hp.nb) * nsets; ++i) {
+      hp.csr_ptr[i] = int32_t(run);
+      run += count[i];
+    }
+    hp.csr_ptr[size_t(hp.nb) * nsets] = int32_t(run);
+    hp.csr_idx.assign(size_t(run), 0);
+    std::vector<int32_t> fill(hp.csr_ptr.begin(), hp.csr_ptr.end() - 1);
+    for (const HostRow &h : hp.rows)
+      for (int64_t j = -h.dk; j <= h.dk; ++j) {
+        const int64_t f = h.kc + j;
+        if (f < 0 || f >= hp.nb) continue;
+        hp.csr_idx[size_t(fill[size_t(f) * nsets + size_t(h.plane)]++)] = int32_t(h.goff + j + h.dk);
+      }
+  }
+  return QTAM_OK;
+}
+
+}  // namespace qtam

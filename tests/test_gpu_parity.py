@@ -1,0 +1,265 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle on the same seeded inputs.
+
+Tolerances (BASELINE.json north_star): coefficients <= 1e-12 (fp64) / 2e-5 (fp32) relative L2 per
+segment over the whole coefficient vector; round trip <= 1e-12 (fp64) / 1e-5 (fp32) against the
+projection Pi_C x (R9).  For fp32 the oracle consumes the same fp32-rounded input
+promoted to double.  The threshold step is bit exact on identical inputs.
+"""
+import numpy as np
+import pytest
+
+from conftest import rel_l2
+from oracle.qtam_ref import RefPlan
+from paper_2603_29785_b200 import binding, inputs
+
+torch = pytest.importorskip("torch")
+pytestmark = pytest.mark.gpu
+
+TOL = {"f64": 1e-12, "f32": 2e-5}
+TOL_RT = {"f64": 1e-12, "f32": 1e-5}
+
+
+def dev(a):
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def worst_segment(got, want):
+    return max(rel_l2(got[b], want[b]) for b in range(want.shape[0]))
+
+
+def make_plans(args, dtype, max_batch, **kw):
+    g = binding.Plan(args[0], args[1], args[2], args[3], args[4], args[5], dtype=dtype, max_batch=max_batch, **kw)
+    r = RefPlan(args[0], args[1], args[2], args[3], args[4], args[5], **kw)
+    return g, r
+
+
+def pi_c(x64, cover):
+    X = np.fft.rfft(x64, axis=-1)
+    return np.fft.irfft(np.where(cover[None, :], X, 0), n=x64.shape[-1], axis=-1)
+
+
+def np_rdt(dtype):
+    return np.float64 if dtype == "f64" else np.float32
+
+
+# ---- small plans, both dtypes, every call ---------------------------------------------------------
+
+SMALL = [
+    (1024.0, 1024, [4.0, 8.0, 16.0], 16.0, 400.0, 12.0),      # M 8..64
+    (256.0, 256, [4.0, 8.0], 8.0, 100.0, 7.0),                # tiny N
+    (4096.0, 8192, [5.0, 20.0], 10.0, 1900.0, 24.0),          # M up to 512
+]
+
+
+@pytest.mark.parametrize("args", SMALL)
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+@pytest.mark.parametrize("ov", [1.0, 2.0])
+def test_small_forward_inverse_dense(args, dtype, ov):
+    g, r = make_plans(args, dtype, 3, clamp_overlap=ov)
+    x = inputs.white_noise(args[1], 100 + args[1], batch=3).astype(np_rdt(dtype))
+    x64 = x.astype(np.float64)
+    Yg = g.forward(dev(x)).cpu().numpy()
+    Yr = r.forward(x64, engine=0)
+    assert worst_segment(Yg, Yr) <= TOL[dtype]
+    # inverse of the ORACLE's coefficients (so the two inverses see identical input)
+    Yin = Yr.astype(np.complex128 if dtype == "f64" else np.complex64)
+    for plane in range(-1, g.n_planes):
+        xg = g.inverse(dev(Yin), plane=plane).cpu().numpy()
+        xr = r.inverse(Yin.astype(np.complex128), plane=plane, engine=0)
+        assert worst_segment(xg, xr) <= TOL[dtype], plane
+    # round trip through the GPU only
+    xrt = g.inverse(g.forward(dev(x))).cpu().numpy()
+    _, C = r.frame(-1)
+    assert worst_segment(xrt, pi_c(x64, C)) <= TOL_RT[dtype]
+    # dense tiles
+    Dg = g.dense(dev(x), 0, g.n_rows).cpu().numpy()
+    Dr = r.dense(x64, 0, r.n_rows, engine=1)
+    assert worst_segment(Dg.reshape(3, -1), Dr.reshape(3, -1)) <= TOL[dtype]
+
+
+def test_dense_shift_invariance_on_gpu():
+    """the check qtam_dense exists for: integer time shifts commute with the tiles"""
+    args = SMALL[0]
+    g, _ = make_plans(args, "f64", 1)
+    x = inputs.white_noise(args[1], 7)[0]
+    D = g.dense(dev(x[None, :])).cpu().numpy()[0]
+    for s in (1, 17, 500):
+        Ds = g.dense(dev(np.roll(x, s)[None, :])).cpu().numpy()[0]
+        assert rel_l2(Ds, np.roll(D, s, axis=-1)) <= 1e-12
+
+
+# ---- BASELINE configurations -------------------------------------------------------------------------
+
+def test_cfg1_fp64_full():
+    name = "cfg1"
+    g, r = make_plans(inputs.plan_args(name), "f64", 1)
+    x = inputs.make_batch(name)
+    Yg = g.forward(dev(x)).cpu().numpy()
+    Yr = r.forward(x, engine=0)
+    assert worst_segment(Yg, Yr) <= 1e-12
+    worst_row = max(rel_l2(Yg[0, r.row_slice(k)], Yr[0, r.row_slice(k)]) for k in range(r.n_rows))
+    assert worst_row <= 1e-11
+    for plane in (-1, 0, 1, 2):
+        xg = g.inverse(dev(Yr), plane=plane).cpu().numpy()
+        assert worst_segment(xg, r.inverse(Yr, plane=plane, engine=0)) <= 1e-12
+    _, C = r.frame(-1)
+    assert worst_segment(g.inverse(g.forward(dev(x))).cpu().numpy(), pi_c(x, C)) <= 1e-12
+    Dg = g.dense(dev(x)).cpu().numpy()
+    Dr = r.dense(x, engine=1)
+    assert rel_l2(Dg, Dr) <= 1e-12
+    # the injected sine-Gaussian (200 Hz) puts the plane's energy peak in a row near 200 Hz
+    e = [np.sum(np.abs(Yg[0, r.row_slice(k)]) ** 2) for k in range(32)]
+    assert abs(r.rows[int(np.argmax(e))].f_center - 200.0) < 40.0
+
+
+@pytest.mark.parametrize("name,nseg,ov", [("cfg2", 3, 1.0), ("cfg2", 2, 2.0), ("cfg3", 4, 1.0),
+                                          ("cfg3", 2, 2.0), ("cfg5", 8, 1.0), ("cfg5", 4, 2.0)])
+def test_config_fp32_forward_inverse(name, nseg, ov):
+    g, r = make_plans(inputs.plan_args(name), "f32", nseg, clamp_overlap=ov)
+    x = inputs.make_batch(name, batch=nseg)
+    x64 = x.astype(np.float64)
+    Yg = g.forward(dev(x)).cpu().numpy()
+    Yr = r.forward(x64, engine=1)
+    assert worst_segment(Yg, Yr) <= 2e-5
+    Yin = Yr.astype(np.complex64)
+    xg = g.inverse(dev(Yin)).cpu().numpy()
+    xr = r.inverse(Yin.astype(np.complex128), engine=1)
+    assert worst_segment(xg, xr) <= 2e-5
+    _, C = r.frame(-1)
+    assert worst_segment(g.inverse(g.forward(dev(x))).cpu().numpy(), pi_c(x64, C)) <= 1e-5
+    # one plane alone (R10)
+    pl = g.n_planes - 1
+    xg = g.inverse(dev(Yin), plane=pl).cpu().numpy()
+    assert worst_segment(xg, r.inverse(Yin.astype(np.complex128), plane=pl, engine=1)) <= 2e-5
+
+
+def test_cfg5_fp64_variant():
+    name = "cfg5"
+    g, r = make_plans(inputs.plan_args(name), "f64", 4)
+    x = inputs.make_batch(name, batch=4, dtype="f64")
+    Yg = g.forward(dev(x)).cpu().numpy()
+    Yr = r.forward(x, engine=1)
+    assert worst_segment(Yg, Yr) <= 1e-12
+    _, C = r.frame(-1)
+    assert worst_segment(g.inverse(g.forward(dev(x))).cpu().numpy(), pi_c(x, C)) <= 1e-12
+
+
+@pytest.mark.parametrize("ov", [1.0, 2.0])
+def test_cfg4_long_segment(ov):
+    """N = 2^20, rows up to M = 65536 (131072 with overlap 2): the multi-pass paths."""
+    name = "cfg4"
+    g, r = make_plans(inputs.plan_args(name), "f32", 1, clamp_overlap=ov)
+    x = inputs.make_batch(name, batch=1)
+    x64 = x.astype(np.float64)
+    Yg = g.forward(dev(x)).cpu().numpy()
+    Yr = r.forward(x64, engine=1)
+    assert worst_segment(Yg, Yr) <= 2e-5
+    Yin = Yr.astype(np.complex64)
+    xg = g.inverse(dev(Yin)).cpu().numpy()
+    xr = r.inverse(Yin.astype(np.complex128), engine=1)
+    assert worst_segment(xg, xr) <= 2e-5
+    _, C = r.frame(-1)
+    assert worst_segment(g.inverse(g.forward(dev(x))).cpu().numpy(), pi_c(x64, C)) <= 1e-5
+
+
+# ---- threshold (a4): bit exact --------------------------------------------------------------------------
+
+@pytest.mark.parametrize("dtype", ["f32", "f64"])
+def test_threshold_bit_exact_on_seeded_coefficients(dtype):
+    g, r = make_plans(inputs.plan_args("cfg5"), dtype, 5)
+    rng = np.random.default_rng(55)
+    cdt = np.complex64 if dtype == "f32" else np.complex128
+    Y = ((rng.standard_normal((5, r.ctot)) + 1j * rng.standard_normal((5, r.ctot)))
+         * rng.uniform(0.05, 4.0, (5, r.ctot))).astype(cdt)
+    Y[1, r.row_slice(3)] = 0            # an all-zero row: median 0, nothing is < 0
+    Y[2, r.row_slice(5)] = 1 + 1j       # a constant row: every magnitude equals the median
+    got = g.threshold_rowmedian(dev(Y).clone(), 3.0).cpu().numpy()
+    want = r.threshold_f32(Y, 3.0) if dtype == "f32" else r.threshold(Y, 3.0)
+    bits = np.uint32 if dtype == "f32" else np.uint64
+    assert np.array_equal(got.view(bits), want.view(bits))
+    assert 0 < np.count_nonzero(got) < got.size
+    assert np.array_equal(got[2, r.row_slice(5)], Y[2, r.row_slice(5)])
+
+
+def test_cfg5_denoise_pipeline_fp32():
+    """forward -> zero |c| < 3 x row median -> inverse, each stage against the oracle on the
+    oracle's own upstream output, plus the whole chain."""
+    name = "cfg5"
+    nseg = 8
+    g, r = make_plans(inputs.plan_args(name), "f32", nseg)
+    x = inputs.make_batch(name, batch=nseg)
+    x64 = x.astype(np.float64)
+    Yr32 = r.forward(x64, engine=1).astype(np.complex64)
+    want_thr = r.threshold_f32(Yr32, 3.0)
+    got_thr = g.threshold_rowmedian(dev(Yr32).clone(), 3.0).cpu().numpy()
+    assert np.array_equal(got_thr.view(np.uint32), want_thr.view(np.uint32))
+    xg = g.inverse(dev(want_thr)).cpu().numpy()
+    xr = r.inverse(want_thr.astype(np.complex128), engine=1)
+    assert worst_segment(xg, xr) <= 2e-5
+    # whole chain on the GPU; a coefficient within rounding of the threshold may flip, so compare
+    # the masks' agreement and the outputs loosely
+    Yg = g.forward(dev(x))
+    g.threshold_rowmedian(Yg, 3.0)
+    mask_g = (Yg.cpu().numpy() != 0)
+    mask_r = (want_thr != 0)
+    assert np.mean(mask_g != mask_r) < 1e-4
+    xchain = g.inverse(Yg).cpu().numpy()
+    assert worst_segment(xchain, xr) <= 5e-3
+    kept = mask_r.mean()
+    assert 0.005 < kept < 0.2     # kappa = 3 keeps the loud tail only
+
+
+# ---- edge cases and properties -------------------------------------------------------------------------
+
+def test_empty_batch_and_batch_limit():
+    g, _ = make_plans(SMALL[0], "f32", 2)
+    x = torch.zeros((0, g.N), dtype=torch.float32, device="cuda")
+    out = torch.empty((0, g.ctot), dtype=torch.complex64, device="cuda")
+    assert binding.lib().qtam_forward(g._h, x.data_ptr() or 16, 0, out.data_ptr() or 16, None) == 0
+    big = torch.zeros((3, g.N), dtype=torch.float32, device="cuda")
+    with pytest.raises(binding.QtamError) as e:
+        g.forward(big)
+    assert e.value.code == 1
+
+
+def test_inputs_are_not_modified_and_output_fully_written():
+    g, r = make_plans(inputs.plan_args("cfg3"), "f32", 2)
+    x = dev(inputs.make_batch("cfg3", batch=2))
+    x0 = x.clone()
+    out = torch.full((2, g.ctot), float("nan"), dtype=torch.complex64, device="cuda")
+    g.forward(x, out=out)
+    assert torch.equal(x, x0)
+    assert not torch.isnan(out.real).any() and not torch.isnan(out.imag).any()
+    c0 = out.clone()
+    xo = torch.full((2, g.N), float("nan"), dtype=torch.float32, device="cuda")
+    g.inverse(out, out=xo)
+    assert torch.equal(out, c0) and not torch.isnan(xo).any()
+
+
+def test_gpu_linearity_and_frame_energy_at_full_batch():
+    """properties that hold at any size, on BASELINE config 3 at its full batch (256 x 16384) in the
+    launch configuration bench.py times, plus sampled segments against the oracle."""
+    name = "cfg3"
+    B = inputs.CONFIGS[name]["batch"]
+    g, r = make_plans(inputs.plan_args(name), "f32", B)
+    x = inputs.make_batch(name, batch=B)
+    dx = dev(x)
+    Y = g.forward(dx)
+    # sampled segments, element by element
+    for b in (0, 101, B - 1):
+        Yr = r.forward(x[b].astype(np.float64), engine=1)[0]
+        assert rel_l2(Y[b].cpu().numpy(), Yr) <= 2e-5
+    # frame energy identity P6 on every segment: sum|Y|^2 = (1/N) sum_f |X[f]|^2 P[f]
+    P, C = r.frame(-1)
+    X = np.fft.rfft(x.astype(np.float64), axis=-1)
+    want = (np.abs(X) ** 2 * P[None, :]).sum(axis=1) / g.N
+    got = (Y.abs().double() ** 2).sum(dim=1).cpu().numpy()
+    assert np.max(np.abs(got - want) / want) <= 1e-5
+    # linearity P5
+    a, b = 0.7, -1.9
+    comb = g.forward((a * dx[:8] + b * dx[8:16]).contiguous())
+    assert rel_l2(comb.cpu().numpy(), (a * Y[:8] + b * Y[8:16]).cpu().numpy()) <= 1e-5
+    # round trip on every segment
+    xr = g.inverse(Y).cpu().numpy()
+    proj = pi_c(x.astype(np.float64), C)
+    assert worst_segment(xr, proj) <= 1e-5
