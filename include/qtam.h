@@ -130,6 +130,16 @@ qtam_status qtam_threshold_rowmedian(qtam_plan *p, void *d_coef, int batch, doub
 int         qtam_last_launch_count(const qtam_plan *p);
 const char *qtam_status_string(qtam_status s);
 
+/* Launch profile for bench.py's roofline line.  While enabled, every kernel launch of the compute
+ * calls is bracketed by CUDA events on the launch stream (pre-created: up to `max_launches` launches
+ * between two reads; further ones are not recorded).  qtam_profile_read waits for the recorded events,
+ * sums per kernel the launches, the device time (ms) and the ALGORITHMIC bytes the launches had to
+ * move, writes up to `capacity` entries to `out` (host), clears the record and
+ * returns the number of entries (-1 on error). */
+typedef struct { char name[48]; int launches; double ms; double algo_bytes; } qtam_kernel_stat;
+qtam_status qtam_profile_enable(qtam_plan *p, int on, int max_launches);
+int         qtam_profile_read(qtam_plan *p, qtam_kernel_stat *out, int capacity);
+
 #ifdef __cplusplus
 }
 #endif

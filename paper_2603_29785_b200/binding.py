@@ -18,7 +18,8 @@ STATUS = {0: "ok", 1: "invalid argument", 2: "unsupported", 3: "alloc", 4: "cuda
 
 SYMBOLS = ["qtam_plan_create", "qtam_plan_create_host", "qtam_plan_destroy", "qtam_plan_info",
            "qtam_plan_rows", "qtam_plan_window", "qtam_plan_frame", "qtam_forward", "qtam_inverse",
-           "qtam_dense", "qtam_threshold_rowmedian", "qtam_last_launch_count", "qtam_status_string"]
+           "qtam_dense", "qtam_threshold_rowmedian", "qtam_last_launch_count", "qtam_status_string",
+           "qtam_profile_enable", "qtam_profile_read"]
 
 
 class QtamError(RuntimeError):
@@ -47,6 +48,11 @@ class Info(C.Structure):
                 ("frame_B", C.c_double), ("workspace_bytes", C.c_size_t)]
 
 
+class KernelStat(C.Structure):
+    _fields_ = [("name", C.c_char * 48), ("launches", C.c_int), ("ms", C.c_double),
+                ("algo_bytes", C.c_double)]
+
+
 def lib():
     """Loads libqtam.so (building it in-tree first if it is missing)."""
     global _lib
@@ -73,6 +79,9 @@ def lib():
         L.qtam_last_launch_count.restype = C.c_int
         L.qtam_status_string.argtypes = [C.c_int]
         L.qtam_status_string.restype = C.c_char_p
+        L.qtam_profile_enable.argtypes = [vp, C.c_int, C.c_int]
+        L.qtam_profile_read.argtypes = [vp, C.POINTER(KernelStat), C.c_int]
+        L.qtam_profile_read.restype = C.c_int
         _lib = L
     return _lib
 
@@ -193,6 +202,18 @@ class Plan:
 
     def last_launch_count(self):
         return int(lib().qtam_last_launch_count(self._h))
+
+    def profile_enable(self, on=True, max_launches=4096):
+        _check(lib().qtam_profile_enable(self._h, 1 if on else 0, max_launches), "qtam_profile_enable")
+
+    def profile_read(self):
+        """[{name, launches, ms, algo_bytes}] since the last read (waits for the recorded events)"""
+        buf = (KernelStat * 32)()
+        n = lib().qtam_profile_read(self._h, buf, 32)
+        if n < 0:
+            raise QtamError(4, "qtam_profile_read")
+        return [dict(name=buf[i].name.decode(), launches=int(buf[i].launches), ms=float(buf[i].ms),
+                     algo_bytes=float(buf[i].algo_bytes)) for i in range(n)]
 
     # ---- host-buffer convenience (the end-to-end path bench.py times) ------------------------------
     def forward_host(self, x_pinned, coef_pinned, d_x, d_coef):

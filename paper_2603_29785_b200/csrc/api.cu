@@ -42,6 +42,7 @@ void free_plan(qtam_plan *p) {
   cudaFree(p->d_csr_ptr); cudaFree(p->d_csr_idx);
   for (int c = 0; c < qtam_plan::kClasses; ++c) cudaFree(p->d_items[c]);
   cudaFree(p->d_bigrows); cudaFree(p->d_spec); cudaFree(p->d_ws); cudaFree(p->d_band);
+  for (ProfRec &r : p->prof_pool) { cudaEventDestroy(r.e0); cudaEventDestroy(r.e1); }
   delete p;
 }
 
@@ -119,13 +120,18 @@ template <typename T> qtam_status build_device(qtam_plan *p) {
     for (size_t k = 0; k < hp.rows.size(); ++k) {
       const int lm = ilog2(hp.rows[k].M);
       if (lm <= p->cap_log2) {
-        items[generic_class_of(lm)].push_back(WorkItem{(int)k, 0, 1, lm});
+        const int c = generic_class_of(lm);
+        items[c].push_back(WorkItem{(int)k, 0, 1, lm});
+        p->class_L[c] += (double)hp.rows[k].L; p->class_M[c] += (double)hp.rows[k].M;
       } else {
         const int R1 = 1 << (lm - p->cap_log2);
         if (R1 > 16) return QTAM_ERR_UNSUPPORTED;
         for (int j1 = 0; j1 < R1; ++j1)
           items[generic_class_of(p->cap_log2)].push_back(WorkItem{(int)k, j1, R1, p->cap_log2});
         big.push_back((int)k);
+        p->class_L[generic_class_of(p->cap_log2)] += (double)hp.rows[k].L;
+        p->class_M[generic_class_of(p->cap_log2)] += (double)hp.rows[k].M;
+        p->big_M += (double)hp.rows[k].M;
         if (R1 > p->big_R1max) p->big_R1max = R1;
       }
     }
@@ -284,6 +290,49 @@ qtam_status qtam_threshold_rowmedian(qtam_plan *p, void *d_coef, int batch, doub
 }
 
 int qtam_last_launch_count(const qtam_plan *p) { return p ? p->last_launches : 0; }
+
+static const char *const kKernelNames[K_COUNT] = {
+    "cfft_seq", "cfft_cols", "cfft_rows", "r2c_post", "c2r_pre", "fwd_rows", "fwd_combine",
+    "inv_rows", "inv_reduce", "dense_place", "threshold"};
+
+qtam_status qtam_profile_enable(qtam_plan *p, int on, int max_launches) {
+  if (!p || p->host_only) return QTAM_ERR_INVALID_ARG;
+  if (on) {
+    if (max_launches < 1) max_launches = 4096;
+    while ((int)p->prof_pool.size() < max_launches) {
+      ProfRec r{};
+      if (cudaEventCreate(&r.e0) != cudaSuccess || cudaEventCreate(&r.e1) != cudaSuccess) return QTAM_ERR_CUDA;
+      p->prof_pool.push_back(r);
+    }
+  }
+  p->prof_on = on != 0;
+  p->prof_used = 0;
+  p->prof_dropped = 0;
+  return QTAM_OK;
+}
+
+int qtam_profile_read(qtam_plan *p, qtam_kernel_stat *out, int capacity) {
+  if (!p || !out || capacity < 1) return -1;
+  qtam_kernel_stat acc[K_COUNT];
+  for (int k = 0; k < K_COUNT; ++k) {
+    std::memset(&acc[k], 0, sizeof(acc[k]));
+    std::strncpy(acc[k].name, kKernelNames[k], sizeof(acc[k].name) - 1);
+  }
+  for (int i = 0; i < p->prof_used; ++i) {
+    ProfRec &r = p->prof_pool[(size_t)i];
+    if (cudaEventSynchronize(r.e1) != cudaSuccess) return -1;
+    float ms = 0.f;
+    if (cudaEventElapsedTime(&ms, r.e0, r.e1) != cudaSuccess) return -1;
+    acc[r.kid].launches += 1;
+    acc[r.kid].ms += (double)ms;
+    acc[r.kid].algo_bytes += r.bytes;
+  }
+  p->prof_used = 0;
+  int n = 0;
+  for (int k = 0; k < K_COUNT && n < capacity; ++k)
+    if (acc[k].launches > 0) out[n++] = acc[k];
+  return n;
+}
 
 const char *qtam_status_string(qtam_status s) {
   switch (s) {

@@ -3,7 +3,18 @@
 #pragma once
 #include <cuda_runtime.h>
 
+#include <vector>
+
 #include "qtam_internal.hpp"
+
+namespace qtam {
+// kernel ids for the launch profile (names in profile.cu)
+enum KernelId {
+  K_CFFT_SEQ = 0, K_CFFT_COLS, K_CFFT_ROWS, K_R2C_POST, K_C2R_PRE, K_FWD_ROWS, K_FWD_COMBINE,
+  K_INV_ROWS, K_INV_REDUCE, K_DENSE_PLACE, K_THRESHOLD, K_COUNT
+};
+struct ProfRec { int kid; double bytes; cudaEvent_t e0, e1; };
+}  // namespace qtam
 
 struct qtam_plan {
   qtam::HostPlan hp;
@@ -24,6 +35,9 @@ struct qtam_plan {
   static const int kClasses = 4;
   qtam::WorkItem *d_items[kClasses] = {nullptr, nullptr, nullptr, nullptr};
   int n_items[kClasses] = {0, 0, 0, 0};
+  double class_L[kClasses] = {0, 0, 0, 0};   // sum of band lengths / output lengths of a class's
+  double class_M[kClasses] = {0, 0, 0, 0};   // items (for the launch profile's byte counts)
+  double big_M = 0;                          // sum of M over the rows that need the combine pass
   int *d_bigrows = nullptr;    // rows with R1 > 1 (need the combine pass)
   int n_bigrows = 0;
   int big_R1max = 1;
@@ -35,10 +49,31 @@ struct qtam_plan {
   size_t device_bytes = 0;
 
   int last_launches = 0;
+  // launch profile (qtam_profile_enable / qtam_profile_read)
+  bool prof_on = false;
+  std::vector<qtam::ProfRec> prof_pool;   // pre-created event pairs
+  int prof_used = 0;
+  int prof_dropped = 0;
   bool host_only = false;      // built by qtam_plan_create_host: tables on the host only
 };
 
 namespace qtam {
+
+// Brackets one kernel launch: counts it and, when profiling is on, records CUDA events around it on
+// the launch stream.  `bytes` = algorithmic bytes of that launch.
+struct LaunchScope {
+  qtam_plan *p; cudaStream_t st; int slot;
+  LaunchScope(qtam_plan *plan, cudaStream_t stream, int kid, double bytes) : p(plan), st(stream), slot(-1) {
+    p->last_launches += 1;
+    if (!p->prof_on) return;
+    if (p->prof_used >= (int)p->prof_pool.size()) { p->prof_dropped += 1; return; }
+    slot = p->prof_used++;
+    p->prof_pool[(size_t)slot].kid = kid;
+    p->prof_pool[(size_t)slot].bytes = bytes;
+    cudaEventRecord(p->prof_pool[(size_t)slot].e0, st);
+  }
+  ~LaunchScope() { if (slot >= 0) cudaEventRecord(p->prof_pool[(size_t)slot].e1, st); }
+};
 
 // generic.cu : correct-for-everything kernels (any N, any M, float and double)
 qtam_status generic_r2c(qtam_plan *p, const void *d_x, int batch, cudaStream_t st);

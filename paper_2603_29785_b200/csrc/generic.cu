@@ -451,8 +451,10 @@ static qtam_status cfft(qtam_plan *p, const C2<T> *in, long long in_stride, C2<T
   if (log2n <= cap) {
     if (!set_smem(k_cfft_seq<T>, smem)) return QTAM_ERR_CUDA;
     const int thr = log2n >= 10 ? 512 : (log2n >= 8 ? 128 : 64);
-    k_cfft_seq<T><<<count, thr, smem, st>>>(in, in_stride, out, out_stride, log2n, dir, tw, log2twn, scale, bufpts);
-    p->last_launches += 1;
+    {
+      LaunchScope ls(p, st, K_CFFT_SEQ, 2.0 * sizeof(C2<T>) * (double)count * (double)(1 << log2n));
+      k_cfft_seq<T><<<count, thr, smem, st>>>(in, in_stride, out, out_stride, log2n, dir, tw, log2twn, scale, bufpts);
+    }
     QTAM_LAUNCH_CHECK();
     return QTAM_OK;
   }
@@ -462,11 +464,17 @@ static qtam_status cfft(qtam_plan *p, const C2<T> *in, long long in_stride, C2<T
   int ltr = cap - l2; if (ltr > l1) ltr = l1;
   if (!set_smem(k_cfft_cols<T>, smem) || !set_smem(k_cfft_rows<T>, smem)) return QTAM_ERR_CUDA;
   dim3 ga((1 << l2) >> ltc, count), gb((1 << l1) >> ltr, count);
-  k_cfft_cols<T><<<ga, 512, smem, st>>>(in, in_stride, tmp, tmp_stride, l1, l2, ltc, dir, tw, log2twn, bufpts);
+  const double pass_bytes = 2.0 * sizeof(C2<T>) * (double)count * (double)(1LL << log2n);
+  {
+    LaunchScope ls(p, st, K_CFFT_COLS, pass_bytes);
+    k_cfft_cols<T><<<ga, 512, smem, st>>>(in, in_stride, tmp, tmp_stride, l1, l2, ltc, dir, tw, log2twn, bufpts);
+  }
   QTAM_LAUNCH_CHECK();
-  k_cfft_rows<T><<<gb, 512, smem, st>>>(tmp, tmp_stride, out, out_stride, l1, l2, ltr, dir, tw, log2twn, scale, bufpts);
+  {
+    LaunchScope ls(p, st, K_CFFT_ROWS, pass_bytes);
+    k_cfft_rows<T><<<gb, 512, smem, st>>>(tmp, tmp_stride, out, out_stride, l1, l2, ltr, dir, tw, log2twn, scale, bufpts);
+  }
   QTAM_LAUNCH_CHECK();
-  p->last_launches += 2;
   return QTAM_OK;
 }
 
@@ -479,8 +487,10 @@ static qtam_status r2c_t(qtam_plan *p, const void *d_x, int batch, cudaStream_t 
                           ilog2(Nc), batch, -1, (T)1, st);
   if (s != QTAM_OK) return s;
   dim3 g((Nc / 2 + 1 + 255) / 256, batch);
-  k_r2c_post<T><<<g, 256, 0, st>>>(spec, p->xstride, Nc, static_cast<const C2<T> *>(p->d_tw));
-  p->last_launches += 1;
+  {
+    LaunchScope ls(p, st, K_R2C_POST, 2.0 * sizeof(C2<T>) * (double)batch * (double)Nc);
+    k_r2c_post<T><<<g, 256, 0, st>>>(spec, p->xstride, Nc, static_cast<const C2<T> *>(p->d_tw));
+  }
   QTAM_LAUNCH_CHECK();
   return QTAM_OK;
 }
@@ -499,17 +509,22 @@ static qtam_status fwd_rows_t(qtam_plan *p, int batch, void *d_coef, cudaStream_
     const size_t smem = 2 * sizeof(C2<T>) * (size_t)bufpts;
     if (!set_smem(k_fwd_rows<T>, smem)) return QTAM_ERR_CUDA;
     dim3 g(p->n_items[c], batch);
-    k_fwd_rows<T><<<g, kClassThreads[c], smem, st>>>(
-        p->d_rows, p->d_items[c], static_cast<const C2<T> *>(p->d_spec), p->xstride, (int)p->hp.nb,
-        static_cast<const T *>(p->d_win), tw, log2twn, static_cast<C2<T> *>(d_coef), p->hp.ctot, bufpts);
-    p->last_launches += 1;
+    {
+      // reads the bands (L values per row), writes M coefficients per row
+      LaunchScope ls(p, st, K_FWD_ROWS, sizeof(C2<T>) * (double)batch * (p->class_L[c] + p->class_M[c]));
+      k_fwd_rows<T><<<g, kClassThreads[c], smem, st>>>(
+          p->d_rows, p->d_items[c], static_cast<const C2<T> *>(p->d_spec), p->xstride, (int)p->hp.nb,
+          static_cast<const T *>(p->d_win), tw, log2twn, static_cast<C2<T> *>(d_coef), p->hp.ctot, bufpts);
+    }
     QTAM_LAUNCH_CHECK();
   }
   if (p->n_bigrows > 0) {
     dim3 g(((1 << p->cap_log2) + 255) / 256, p->n_bigrows, batch);
-    k_fwd_combine<T><<<g, 256, 0, st>>>(p->d_rows, p->d_bigrows, p->cap_log2, tw, log2twn,
-                                        static_cast<C2<T> *>(d_coef), p->hp.ctot);
-    p->last_launches += 1;
+    {
+      LaunchScope ls(p, st, K_FWD_COMBINE, 2.0 * sizeof(C2<T>) * (double)batch * p->big_M);
+      k_fwd_combine<T><<<g, 256, 0, st>>>(p->d_rows, p->d_bigrows, p->cap_log2, tw, log2twn,
+                                          static_cast<C2<T> *>(d_coef), p->hp.ctot);
+    }
     QTAM_LAUNCH_CHECK();
   }
   return QTAM_OK;
@@ -529,11 +544,13 @@ static qtam_status inv_rows_t(qtam_plan *p, const void *d_coef, int batch, int p
     const size_t smem = 2 * sizeof(C2<T>) * (size_t)bufpts;
     if (!set_smem(k_inv_rows<T>, smem)) return QTAM_ERR_CUDA;
     dim3 g(p->n_items[c], batch);
-    k_inv_rows<T><<<g, kClassThreads[c], smem, st>>>(
-        p->d_rows, p->d_items[c], static_cast<const C2<T> *>(d_coef), p->hp.ctot,
-        static_cast<const T *>(p->d_win), tw, log2twn, static_cast<C2<T> *>(p->d_band), p->hp.sumL,
-        (int)p->hp.nb, plane, bufpts);
-    p->last_launches += 1;
+    {
+      LaunchScope ls(p, st, K_INV_ROWS, sizeof(C2<T>) * (double)batch * (p->class_L[c] + p->class_M[c]));
+      k_inv_rows<T><<<g, kClassThreads[c], smem, st>>>(
+          p->d_rows, p->d_items[c], static_cast<const C2<T> *>(d_coef), p->hp.ctot,
+          static_cast<const T *>(p->d_win), tw, log2twn, static_cast<C2<T> *>(p->d_band), p->hp.sumL,
+          (int)p->hp.nb, plane, bufpts);
+    }
     QTAM_LAUNCH_CHECK();
   }
   return QTAM_OK;
@@ -547,10 +564,13 @@ qtam_status generic_inverse_rows(qtam_plan *p, const void *d_coef, int batch, in
 template <typename T>
 static qtam_status inv_reduce_t(qtam_plan *p, int batch, int plane, cudaStream_t st) {
   dim3 g((unsigned)((p->hp.nb + 255) / 256), batch);
-  k_inv_reduce<T><<<g, 256, 0, st>>>(static_cast<const C2<T> *>(p->d_band), p->hp.sumL, p->d_csr_ptr,
-                                     p->d_csr_idx, static_cast<const T *>(p->d_invP), (int)p->hp.nb,
-                                     p->hp.nP, plane, static_cast<C2<T> *>(p->d_spec), p->xstride);
-  p->last_launches += 1;
+  {
+    LaunchScope ls(p, st, K_INV_REDUCE,
+                   (double)batch * (sizeof(C2<T>) * ((double)p->hp.sumL + (double)p->hp.nb)));
+    k_inv_reduce<T><<<g, 256, 0, st>>>(static_cast<const C2<T> *>(p->d_band), p->hp.sumL, p->d_csr_ptr,
+                                       p->d_csr_idx, static_cast<const T *>(p->d_invP), (int)p->hp.nb,
+                                       p->hp.nP, plane, static_cast<C2<T> *>(p->d_spec), p->xstride);
+  }
   QTAM_LAUNCH_CHECK();
   return QTAM_OK;
 }
@@ -564,8 +584,10 @@ static qtam_status c2r_t(qtam_plan *p, int batch, void *d_x_out, cudaStream_t st
   const int Nc = (int)(p->hp.N / 2);
   C2<T> *spec = static_cast<C2<T> *>(p->d_spec);
   dim3 g((Nc / 2 + 1 + 255) / 256, batch);
-  k_c2r_pre<T><<<g, 256, 0, st>>>(spec, p->xstride, Nc, static_cast<const C2<T> *>(p->d_tw));
-  p->last_launches += 1;
+  {
+    LaunchScope ls(p, st, K_C2R_PRE, 2.0 * sizeof(C2<T>) * (double)batch * (double)Nc);
+    k_c2r_pre<T><<<g, 256, 0, st>>>(spec, p->xstride, Nc, static_cast<const C2<T> *>(p->d_tw));
+  }
   QTAM_LAUNCH_CHECK();
   return cfft<T>(p, spec, p->xstride, static_cast<C2<T> *>(d_x_out), Nc, static_cast<C2<T> *>(p->d_ws),
                  p->hp.N, ilog2(Nc), batch, +1, (T)1, st);
@@ -583,9 +605,11 @@ static qtam_status dense_t(qtam_plan *p, int batch, int row_begin, int row_end, 
   C2<T> *out = static_cast<C2<T> *>(d_out);
   for (int k = row_begin; k < row_end; ++k) {
     dim3 g((N + 255) / 256, batch);
-    k_dense_place<T><<<g, 256, 0, st>>>(p->d_rows, k, static_cast<const C2<T> *>(p->d_spec), p->xstride,
-                                        (int)p->hp.nb, static_cast<const T *>(p->d_win), ws, N);
-    p->last_launches += 1;
+    {
+      LaunchScope ls(p, st, K_DENSE_PLACE, sizeof(C2<T>) * (double)batch * (double)N);
+      k_dense_place<T><<<g, 256, 0, st>>>(p->d_rows, k, static_cast<const C2<T> *>(p->d_spec), p->xstride,
+                                          (int)p->hp.nb, static_cast<const T *>(p->d_win), ws, N);
+    }
     QTAM_LAUNCH_CHECK();
     qtam_status s = cfft<T>(p, ws, N, out + (long long)(k - row_begin) * N, (long long)nr * N, ws, N,
                             ilog2(N), batch, +1, (T)1, st);
@@ -605,8 +629,10 @@ static qtam_status threshold_t(qtam_plan *p, void *d_coef, int batch, double kap
   const size_t smem = sizeof(T) * (size_t)cache_pts;
   if (!set_smem(k_threshold<T>, smem)) return QTAM_ERR_CUDA;
   dim3 g((unsigned)p->hp.rows.size(), batch);
-  k_threshold<T><<<g, 256, smem, st>>>(p->d_rows, static_cast<C2<T> *>(d_coef), p->hp.ctot, (T)kappa, cache_pts);
-  p->last_launches += 1;
+  {
+    LaunchScope ls(p, st, K_THRESHOLD, 2.0 * sizeof(C2<T>) * (double)batch * (double)p->hp.ctot);
+    k_threshold<T><<<g, 256, smem, st>>>(p->d_rows, static_cast<C2<T> *>(d_coef), p->hp.ctot, (T)kappa, cache_pts);
+  }
   QTAM_LAUNCH_CHECK();
   return QTAM_OK;
 }

@@ -172,13 +172,15 @@ def test_threshold_bit_exact_on_seeded_coefficients(dtype):
     Y = ((rng.standard_normal((5, r.ctot)) + 1j * rng.standard_normal((5, r.ctot)))
          * rng.uniform(0.05, 4.0, (5, r.ctot))).astype(cdt)
     Y[1, r.row_slice(3)] = 0            # an all-zero row: median 0, nothing is < 0
-    Y[2, r.row_slice(5)] = 1 + 1j       # a constant row: every magnitude equals the median
+    Y[2, r.row_slice(5)] = 1 + 1j       # a constant row
     got = g.threshold_rowmedian(dev(Y).clone(), 3.0).cpu().numpy()
     want = r.threshold_f32(Y, 3.0) if dtype == "f32" else r.threshold(Y, 3.0)
     bits = np.uint32 if dtype == "f32" else np.uint64
     assert np.array_equal(got.view(bits), want.view(bits))
     assert 0 < np.count_nonzero(got) < got.size
-    assert np.array_equal(got[2, r.row_slice(5)], Y[2, r.row_slice(5)])
+    # a constant row: every magnitude equals the median m, and m < 3m, so the whole row is zeroed
+    assert not got[2, r.row_slice(5)].any()
+    assert not got[1, r.row_slice(3)].any()
 
 
 def test_cfg5_denoise_pipeline_fp32():
@@ -206,7 +208,8 @@ def test_cfg5_denoise_pipeline_fp32():
     xchain = g.inverse(Yg).cpu().numpy()
     assert worst_segment(xchain, xr) <= 5e-3
     kept = mask_r.mean()
-    assert 0.005 < kept < 0.2     # kappa = 3 keeps the loud tail only
+    # Rayleigh magnitudes: P(|c| > 3 median) = 2^-9 ~ 0.2 % for pure noise, more where a glitch sits
+    assert 1e-3 < kept < 0.05
 
 
 # ---- edge cases and properties -------------------------------------------------------------------------
