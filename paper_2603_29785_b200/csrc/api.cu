@@ -3,6 +3,7 @@
 #include <cmath>
 #include <cstring>
 #include <new>
+#include <utility>
 #include <vector>
 
 #include "cplx.cuh"
@@ -42,6 +43,7 @@ void free_plan(qtam_plan *p) {
   cudaFree(p->d_csr_ptr); cudaFree(p->d_csr_idx);
   for (int c = 0; c < qtam_plan::kClasses; ++c) cudaFree(p->d_items[c]);
   cudaFree(p->d_bigrows); cudaFree(p->d_spec); cudaFree(p->d_ws); cudaFree(p->d_band);
+  cudaFree(p->d_frows); cudaFree(p->d_fwin); cudaFree(p->d_ftw_fwd); cudaFree(p->d_ftw_inv);
   for (ProfRec &r : p->prof_pool) { cudaEventDestroy(r.e0); cudaEventDestroy(r.e1); }
   delete p;
 }
@@ -68,6 +70,66 @@ template <typename T> void fill_twiddles(std::vector<T> &tw, int64_t n) {
     tw[size_t(2 * k)] = (T)c;
     tw[size_t(2 * k + 1)] = (T)s;
   }
+}
+
+// tables of the fast float path (fast.cu)
+qtam_status build_fast(qtam_plan *p) {
+  const HostPlan &hp = p->hp;
+  size_t *tot = &p->device_bytes;
+  FastParams &F = p->fast;
+  std::memset(&F, 0, sizeof(F));
+  // one window per distinct half-width (the clamped rows all share one)
+  std::vector<float> fwin;
+  std::vector<std::pair<int64_t, int>> seen;   // (dk, offset)
+  auto window_of = [&](const HostRow &h) -> int {
+    for (auto &e : seen) if (e.first == h.dk) return e.second;
+    const int off = (int)fwin.size();
+    for (int64_t i = 0; i < h.L; ++i) fwin.push_back((float)hp.win[(size_t)(h.woff + i)]);
+    seen.push_back({h.dk, off});
+    return off;
+  };
+  std::vector<FastRow> frows;
+  std::vector<float> twf, twi;   // interleaved re,im
+  const long double tau = 6.283185307179586476925286766559005768L;
+  for (int lg = 5; lg >= 0; --lg) {
+    const int G = 1 << lg, M = 32 * G, Fr = 32 / G;
+    FastBucket B{};
+    B.log2G = lg; B.row_base = (int)frows.size(); B.tw_base = (int)(twf.size() / 2);
+    for (size_t k = 0; k < hp.rows.size(); ++k) {
+      const HostRow &h = hp.rows[k];
+      if (h.M != M) continue;
+      FastRow r{};
+      r.kc = (int)h.kc; r.dk = (int)h.dk; r.woff = window_of(h); r.goff = (int)h.goff;
+      r.offset = (int)h.offset; r.plane = h.plane;
+      frows.push_back(r);
+      F.sum_M += (double)h.M; F.sum_L += (double)h.L;
+    }
+    B.nrows = (int)frows.size() - B.row_base;
+    if (B.nrows == 0) continue;
+    B.ngroups = (B.nrows + Fr - 1) / Fr;
+    const double sf = 1.0 / std::sqrt((double)hp.N * (double)M), si = std::sqrt((double)hp.N / (double)M);
+    for (int n1 = 0; n1 < 32; ++n1)
+      for (int t = 0; t < G; ++t) {
+        const int m = (n1 * t) % M;
+        const long double a = tau * (long double)m / (long double)M;
+        const double c = (double)cosl(a), s = (double)sinl(a);
+        twf.push_back((float)(c * sf)); twf.push_back((float)(s * sf));
+        twi.push_back((float)(c * si)); twi.push_back((float)(-s * si));
+      }
+    F.groups_per_seg += B.ngroups;
+    F.b[F.nbuckets++] = B;
+  }
+  F.tw_total = (int)(twf.size() / 2);
+  if (hp.ctot >= (int64_t(1) << 31)) return QTAM_ERR_UNSUPPORTED;
+  if (!upload(&p->d_frows, frows.data(), frows.size(), tot)) return QTAM_ERR_ALLOC;
+  float *d = nullptr;
+  if (!upload(&d, fwin.data(), fwin.size(), tot)) return QTAM_ERR_ALLOC;
+  p->d_fwin = d;
+  if (!upload(&d, twf.data(), twf.size(), tot)) return QTAM_ERR_ALLOC;
+  p->d_ftw_fwd = d;
+  if (!upload(&d, twi.data(), twi.size(), tot)) return QTAM_ERR_ALLOC;
+  p->d_ftw_inv = d;
+  return QTAM_OK;
 }
 
 template <typename T> qtam_status build_device(qtam_plan *p) {
@@ -119,6 +181,7 @@ template <typename T> qtam_status build_device(qtam_plan *p) {
     std::vector<int> big;
     for (size_t k = 0; k < hp.rows.size(); ++k) {
       const int lm = ilog2(hp.rows[k].M);
+      if (p->fast_rows && lm >= 5 && lm <= 10) continue;   // handled by fast.cu
       if (lm <= p->cap_log2) {
         const int c = generic_class_of(lm);
         items[c].push_back(WorkItem{(int)k, 0, 1, lm});
@@ -176,7 +239,17 @@ qtam_status qtam_plan_create(qtam_plan **out, double fs, int64_t N, const double
   p->xstride = ((p->hp.nb + 31) / 32) * 32;
   p->twn = N;
   p->cap_log2 = dtype == QTAM_F32 ? 13 : 12;
+  {
+    int dev = 0, sms = 148;
+    if (cudaGetDevice(&dev) == cudaSuccess &&
+        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && sms > 0)
+      p->num_sms = sms;
+    const int lnc = ilog2(N) - 1;
+    p->fast_rows = dtype == QTAM_F32;
+    p->fast_long = dtype == QTAM_F32 && lnc >= 11 && lnc <= 14;
+  }
   s = dtype == QTAM_F32 ? build_device<float>(p) : build_device<double>(p);
+  if (s == QTAM_OK && p->fast_rows) s = build_fast(p);
   if (s != QTAM_OK) { free_plan(p); cudaGetLastError(); return s; }
   if (cudaDeviceSynchronize() != cudaSuccess) { free_plan(p); return QTAM_ERR_CUDA; }
   *out = p;
@@ -247,8 +320,12 @@ qtam_status qtam_forward(qtam_plan *p, const void *d_x, int batch, void *d_coef,
   p->last_launches = 0;
   if (batch == 0) return QTAM_OK;
   cudaStream_t st = static_cast<cudaStream_t>(stream);
-  qtam_status s = generic_r2c(p, d_x, batch, st);
+  qtam_status s = p->fast_long ? fast_r2c(p, d_x, batch, st) : generic_r2c(p, d_x, batch, st);
   if (s != QTAM_OK) return s;
+  if (p->fast_rows) {
+    s = fast_forward_rows(p, batch, d_coef, st);
+    if (s != QTAM_OK) return s;
+  }
   return generic_forward_rows(p, batch, d_coef, st);
 }
 
@@ -260,8 +337,14 @@ qtam_status qtam_inverse(qtam_plan *p, const void *d_coef, int batch, int plane,
   p->last_launches = 0;
   if (batch == 0) return QTAM_OK;
   cudaStream_t st = static_cast<cudaStream_t>(stream);
-  qtam_status s = generic_inverse_rows(p, d_coef, batch, plane, st);
+  qtam_status s = QTAM_OK;
+  if (p->fast_rows) {
+    s = fast_inverse_rows(p, d_coef, batch, plane, st);
+    if (s != QTAM_OK) return s;
+  }
+  s = generic_inverse_rows(p, d_coef, batch, plane, st);
   if (s != QTAM_OK) return s;
+  if (p->fast_long) return fast_reduce_c2r(p, batch, plane, d_x_out, st);
   s = generic_inverse_reduce(p, batch, plane, st);
   if (s != QTAM_OK) return s;
   return generic_c2r(p, batch, d_x_out, st);
@@ -276,7 +359,7 @@ qtam_status qtam_dense(qtam_plan *p, const void *d_x, int batch, int row_begin, 
   p->last_launches = 0;
   if (batch == 0 || row_begin == row_end) return QTAM_OK;
   cudaStream_t st = static_cast<cudaStream_t>(stream);
-  qtam_status s = generic_r2c(p, d_x, batch, st);
+  qtam_status s = p->fast_long ? fast_r2c(p, d_x, batch, st) : generic_r2c(p, d_x, batch, st);
   if (s != QTAM_OK) return s;
   return generic_dense(p, batch, row_begin, row_end, d_out, st);
 }
@@ -293,7 +376,8 @@ int qtam_last_launch_count(const qtam_plan *p) { return p ? p->last_launches : 0
 
 static const char *const kKernelNames[K_COUNT] = {
     "cfft_seq", "cfft_cols", "cfft_rows", "r2c_post", "c2r_pre", "fwd_rows", "fwd_combine",
-    "inv_rows", "inv_reduce", "dense_place", "threshold"};
+    "inv_rows", "inv_reduce", "dense_place", "threshold", "r2c_fast", "fwd_rows_fast", "inv_rows_fast",
+    "reduce_c2r_fast"};
 
 qtam_status qtam_profile_enable(qtam_plan *p, int on, int max_launches) {
   if (!p || p->host_only) return QTAM_ERR_INVALID_ARG;

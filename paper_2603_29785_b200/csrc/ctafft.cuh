@@ -1,0 +1,94 @@
+// ctafft.cuh -- one long complex FFT per CTA in shared memory (the half-length FFT behind the long
+// real transforms a1 / a8), float, Nc = 2^11 .. 2^14 points.
+// Stockham autosort in place: every pass loads its butterflies into registers, the CTA synchronises,
+// and the results go back to their autosorted positions; 2-3 passes of radix 8/16/32 done with the
+// in-register FFTs of fftreg.cuh.  Pass 1 writes with stride R, so it writes a skewed layout
+// phys(a) = a + (a >> log2 R1) that the second pass reads back; later passes use the natural layout.
+#pragma once
+#include "fftreg.cuh"
+
+namespace qtam {
+
+template <int LOG2NC> struct CtaFftPlan;
+template <> struct CtaFftPlan<11> { static constexpr int NT = 128, P = 3, R0 = 16, R1 = 16, R2 = 8; };
+template <> struct CtaFftPlan<12> { static constexpr int NT = 256, P = 3, R0 = 16, R1 = 16, R2 = 16; };
+template <> struct CtaFftPlan<13> { static constexpr int NT = 256, P = 3, R0 = 32, R1 = 16, R2 = 16; };
+template <> struct CtaFftPlan<14> { static constexpr int NT = 512, P = 3, R0 = 32, R1 = 32, R2 = 16; };
+
+template <int V> struct ILog2 { static constexpr int value = 1 + ILog2<V / 2>::value; };
+template <> struct ILog2<1> { static constexpr int value = 0; };
+
+// shared-memory elements the transform needs (skew padding included)
+template <int LOG2NC> constexpr int cta_fft_smem_elems() {
+  return (1 << LOG2NC) + ((1 << LOG2NC) >> ILog2<CtaFftPlan<LOG2NC>::R0>::value) + 2;
+}
+
+// One Stockham pass.  IN_MODE / OUT_MODE: 0 natural smem, 1 skewed smem, 2 global (natural).
+// tw: global table e^{+2 pi i m/twn}, log2twn >= LOG2NC.
+template <int LOG2NC, int NT, int R, int LOG2NS, int DIR, int IN_MODE, int OUT_MODE, int SKEW>
+__device__ __forceinline__ void cta_fft_pass(float2 *s, const float2 *__restrict__ gin,
+                                             float2 *__restrict__ gout, const float2 *__restrict__ tw,
+                                             int log2twn, float out_scale) {
+  constexpr int NC = 1 << LOG2NC;
+  constexpr int NBF = NC / R;                 // butterflies
+  constexpr int BPT = (NBF + NT - 1) / NT;    // per thread
+  constexpr int NS = 1 << LOG2NS;
+  float2 v[BPT][R];
+#pragma unroll
+  for (int u = 0; u < BPT; ++u) {
+    const int i = threadIdx.x + NT * u;
+    if (NBF % NT == 0 || i < NBF) {
+#pragma unroll
+      for (int r = 0; r < R; ++r) {
+        const int a = i + r * NBF;
+        if constexpr (IN_MODE == 2) v[u][r] = gin[a];
+        else if constexpr (IN_MODE == 1) v[u][r] = s[a + (a >> SKEW)];
+        else v[u][r] = s[a];
+      }
+      if constexpr (LOG2NS > 0) {
+        const int k = i & (NS - 1);
+        const int sh = log2twn - LOG2NS - ILog2<R>::value;   // w_{NS*R}^{k r} = tw[(k r) << sh]
+#pragma unroll
+        for (int r = 1; r < R; ++r) {
+          float2 w = __ldg(tw + ((size_t)(k * r) << sh));
+          if (DIR < 0) w.y = -w.y;
+          v[u][r] = pcmul(v[u][r], w);
+        }
+      }
+      RegFFT<R, DIR>::run(v[u]);
+    }
+  }
+  if constexpr (IN_MODE != 2 && OUT_MODE != 2) __syncthreads();   // all reads done before in-place writes
+#pragma unroll
+  for (int u = 0; u < BPT; ++u) {
+    const int i = threadIdx.x + NT * u;
+    if (NBF % NT == 0 || i < NBF) {
+      const int k = i & (NS - 1);
+      const int base = ((i - k) * R) + k;
+#pragma unroll
+      for (int r = 0; r < R; ++r) {
+        const int a = base + r * NS;
+        if constexpr (OUT_MODE == 2) gout[a] = pscale(v[u][r], out_scale);
+        else if constexpr (OUT_MODE == 1) s[a + (a >> SKEW)] = v[u][r];
+        else s[a] = v[u][r];
+      }
+    }
+  }
+  if constexpr (OUT_MODE != 2) __syncthreads();
+}
+
+// Whole transform.  FROM_GLOBAL: pass 1 reads gin (natural order) instead of s (natural layout).
+// TO_GLOBAL: the last pass writes gout (natural order, times out_scale) instead of s (natural layout).
+template <int LOG2NC, int DIR, bool FROM_GLOBAL, bool TO_GLOBAL>
+__device__ __forceinline__ void cta_fft(float2 *s, const float2 *__restrict__ gin, float2 *__restrict__ gout,
+                                        const float2 *__restrict__ tw, int log2twn, float out_scale) {
+  typedef CtaFftPlan<LOG2NC> PL;
+  constexpr int L0 = ILog2<PL::R0>::value, L1 = ILog2<PL::R1>::value;
+  static_assert(PL::P == 3, "three passes");
+  static_assert(L0 + L1 + ILog2<PL::R2>::value == LOG2NC, "radices must multiply to Nc");
+  cta_fft_pass<LOG2NC, PL::NT, PL::R0, 0, DIR, FROM_GLOBAL ? 2 : 0, 1, L0>(s, gin, gout, tw, log2twn, 1.f);
+  cta_fft_pass<LOG2NC, PL::NT, PL::R1, L0, DIR, 1, 0, L0>(s, gin, gout, tw, log2twn, 1.f);
+  cta_fft_pass<LOG2NC, PL::NT, PL::R2, L0 + L1, DIR, 0, TO_GLOBAL ? 2 : 0, L0>(s, gin, gout, tw, log2twn, out_scale);
+}
+
+}  // namespace qtam

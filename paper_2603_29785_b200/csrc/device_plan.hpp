@@ -11,7 +11,16 @@ namespace qtam {
 // kernel ids for the launch profile (names in profile.cu)
 enum KernelId {
   K_CFFT_SEQ = 0, K_CFFT_COLS, K_CFFT_ROWS, K_R2C_POST, K_C2R_PRE, K_FWD_ROWS, K_FWD_COMBINE,
-  K_INV_ROWS, K_INV_REDUCE, K_DENSE_PLACE, K_THRESHOLD, K_COUNT
+  K_INV_ROWS, K_INV_REDUCE, K_DENSE_PLACE, K_THRESHOLD, K_R2C_FAST, K_FWD_ROWS_FAST, K_INV_ROWS_FAST,
+  K_REDUCE_C2R_FAST, K_COUNT
+};
+// fast float path (fast.cu): rows with 32 <= M <= 1024, grouped by G = M/32 lanes per row
+struct FastRow { int kc, dk, woff, goff, offset, plane; };
+struct FastBucket { int log2G, nrows, ngroups, row_base, tw_base, pad; };
+struct FastParams {
+  int nbuckets, groups_per_seg, tw_total, pad;
+  double sum_M, sum_L;          // coefficients / band values per segment the fast rows cover
+  FastBucket b[6];
 };
 struct ProfRec { int kid; double bytes; cudaEvent_t e0, e1; };
 }  // namespace qtam
@@ -48,6 +57,16 @@ struct qtam_plan {
   void *d_band = nullptr;      // complex[max_batch][sumL]      inverse band values G_k[j]
   size_t device_bytes = 0;
 
+  // fast float path
+  bool fast_rows = false;      // rows 32..1024 points run in fast.cu
+  bool fast_long = false;      // long FFTs run in fast.cu (float, N = 2^12..2^15)
+  int num_sms = 148;
+  qtam::FastParams fast{};
+  qtam::FastRow *d_frows = nullptr;
+  void *d_fwin = nullptr;      // float windows, one per distinct half-width
+  void *d_ftw_fwd = nullptr;   // float2 pass-1 twiddles [bucket][n1][t], forward (x (N M)^-1/2)
+  void *d_ftw_inv = nullptr;   // same, inverse (conjugate, x sqrt(N/M))
+
   int last_launches = 0;
   // launch profile (qtam_profile_enable / qtam_profile_read)
   bool prof_on = false;
@@ -83,5 +102,11 @@ qtam_status generic_inverse_reduce(qtam_plan *p, int batch, int plane, cudaStrea
 qtam_status generic_c2r(qtam_plan *p, int batch, void *d_x_out, cudaStream_t st);
 qtam_status generic_dense(qtam_plan *p, int batch, int row_begin, int row_end, void *d_out, cudaStream_t st);
 qtam_status generic_threshold(qtam_plan *p, void *d_coef, int batch, double kappa, cudaStream_t st);
+
+// fast.cu
+qtam_status fast_r2c(qtam_plan *p, const void *d_x, int batch, cudaStream_t st);
+qtam_status fast_forward_rows(qtam_plan *p, int batch, void *d_coef, cudaStream_t st);
+qtam_status fast_inverse_rows(qtam_plan *p, const void *d_coef, int batch, int plane, cudaStream_t st);
+qtam_status fast_reduce_c2r(qtam_plan *p, int batch, int plane, void *d_x_out, cudaStream_t st);
 
 }  // namespace qtam

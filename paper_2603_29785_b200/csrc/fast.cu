@@ -1,0 +1,307 @@
+// fast.cu -- the tuned float path of libqtam for sm_100a.
+//   K1 k_r2c_fast      a1      one CTA per segment: long real FFT in shared memory (ctafft.cuh), spectrum
+//                              to the plan's L2-resident spectrum buffer
+//   K2 k_fwd_rows_fast a2+a3   one launch for every row with 32 <= M <= 1024: window gather + baseband
+//                              shift + short inverse FFT with the warp-level engine of rowfft.cuh
+//                              (G = M/32 lanes per row, 32 points per lane in registers)
+//   K3 k_inv_rows_fast a5      per-row forward FFT, sqrt(N/M), window; band values to the band workspace
+//   K4 k_reduce_c2r_fast a6-a8 one CTA per segment: segmented reduction over bins (fixed order, no
+//                              atomics), 1/P, Hermitian pre-processing and the long inverse FFT in smem
+// Rows outside 32..1024 points, double precision and N outside 2^12..2^15 run in generic.cu.
+#include "cplx.cuh"
+#include "ctafft.cuh"
+#include "device_plan.hpp"
+#include "rowfft.cuh"
+
+namespace qtam {
+
+#define QTAM_LAUNCH_CHECK()                                         \
+  do {                                                              \
+    if (cudaPeekAtLastError() != cudaSuccess) return QTAM_ERR_CUDA; \
+  } while (0)
+
+extern __shared__ __align__(16) unsigned char qtam_fast_smem[];
+
+// --------------------------------------------------------------------------------------------------
+// K1: long R2C.  z[m] = x[2m] + i x[2m+1]; Z = FFT_Nc(z);
+//     X[f] = (Z[f] + conj Z[Nc-f])/2 - (i/2) e^{-2 pi i f/N} (Z[f] - conj Z[Nc-f]),  f = 0..Nc  (C1)
+// --------------------------------------------------------------------------------------------------
+template <int LOG2NC>
+__global__ void __launch_bounds__(CtaFftPlan<LOG2NC>::NT)
+k_r2c_fast(const float *__restrict__ x, float2 *__restrict__ spec, long long xstride,
+           const float2 *__restrict__ tw, int log2twn) {
+  constexpr int NC = 1 << LOG2NC, NT = CtaFftPlan<LOG2NC>::NT;
+  float2 *s = reinterpret_cast<float2 *>(qtam_fast_smem);
+  const float2 *gin = reinterpret_cast<const float2 *>(x) + (size_t)blockIdx.x * NC;
+  cta_fft<LOG2NC, -1, true, false>(s, gin, nullptr, tw, log2twn, 1.f);
+  float2 *X = spec + (size_t)blockIdx.x * xstride;
+  for (int f = threadIdx.x; f <= NC / 2; f += NT) {
+    const int g = NC - f;
+    const float2 A = s[f];
+    const float2 B = (f == 0) ? A : s[g];
+    const float2 E = make_float2(0.5f * (A.x + B.x), 0.5f * (A.y - B.y));
+    const float2 D = make_float2(0.5f * (A.x - B.x), 0.5f * (A.y + B.y));
+    float2 w = __ldg(tw + ((size_t)f << (log2twn - LOG2NC - 1)));   // e^{+2 pi i f/N}
+    w.y = -w.y;
+    const float2 t = make_float2(w.x * D.x - w.y * D.y, w.x * D.y + w.y * D.x);
+    X[f] = make_float2(E.x + t.y, E.y - t.x);
+    if (g != f) X[g] = make_float2(E.x - t.y, -E.y - t.x);
+  }
+}
+
+// --------------------------------------------------------------------------------------------------
+// K2 / K3: rows.  Work items are ordered bucket-major (largest M first), then segment, then row group;
+// a CTA takes NWARPS consecutive items, i.e. neighbouring rows of one segment, so that the bands its
+// warps read overlap in L1.
+// --------------------------------------------------------------------------------------------------
+template <int LOG2G>
+__device__ __noinline__ void fwd_group(const FastBucket &B, const FastRow *__restrict__ frows, int seg, int grp,
+                                          int lane, float2 *ex, const float2 *tw1,
+                                          const float2 *__restrict__ spec, long long xstride, int nbins,
+                                          const float *__restrict__ fwin, float2 *__restrict__ coef,
+                                          long long ctot) {
+  constexpr int G = 1 << LOG2G, F = 32 / G, M = 32 * G;
+  const int t = lane & (G - 1), rw = lane >> LOG2G;
+  const int r = grp * F + rw;
+  const bool valid = r < B.nrows;
+  FastRow row;
+  if (valid) row = frows[B.row_base + r];
+  else { row.kc = 0; row.dk = -1; row.woff = 0; row.goff = 0; row.offset = 0; }
+  const float2 *X = spec + (size_t)seg * xstride + row.kc;
+  const float *W = fwin + row.woff + row.dk;
+  float2 v[32];
+#pragma unroll
+  for (int j1 = 0; j1 < 32; ++j1) {
+    const int jj = (j1 < 16) ? (t + G * j1) : (t + G * j1 - M);     // signed offset from the centre (R6)
+    const int f = row.kc + jj;
+    const bool ok = (jj <= row.dk) && (jj >= -row.dk) && (f >= 0) && (f < nbins);   // support, R8 clip
+    float2 xv = make_float2(0.f, 0.f);
+    if (ok) xv = pscale(X[jj], W[jj]);
+    v[j1] = xv;
+  }
+  RowFFT<LOG2G, +1>::run(v, ex, tw1, lane);
+  if (valid) {
+    float2 *dst = coef + (size_t)seg * ctot + row.offset + t;
+#pragma unroll
+    for (int i = 0; i < F; ++i)
+#pragma unroll
+      for (int n2 = 0; n2 < G; ++n2) __stcs(dst + G * i + 32 * n2, v[i * G + n2]);
+  }
+}
+
+template <int LOG2G>
+__device__ __noinline__ void inv_group(const FastBucket &B, const FastRow *__restrict__ frows, int seg, int grp,
+                                          int lane, float2 *ex, const float2 *tw1,
+                                          const float2 *__restrict__ coef, long long ctot, int nbins,
+                                          const float *__restrict__ fwin, float2 *__restrict__ band,
+                                          long long sumL, int plane) {
+  constexpr int G = 1 << LOG2G, F = 32 / G, M = 32 * G;
+  const int t = lane & (G - 1), rw = lane >> LOG2G;
+  const int r = grp * F + rw;
+  FastRow row;
+  bool valid = r < B.nrows;
+  if (valid) row = frows[B.row_base + r];
+  else { row.kc = 0; row.dk = -1; row.woff = 0; row.goff = 0; row.offset = 0; row.plane = -1; }
+  if (plane >= 0 && row.plane != plane) valid = false;
+  // a whole warp whose rows are all skipped can leave (uniform decision)
+  if (__ballot_sync(0xffffffffu, valid) == 0u) return;
+  const float2 *Y = coef + (size_t)seg * ctot + row.offset + t;
+  float2 v[32];
+#pragma unroll
+  for (int j1 = 0; j1 < 32; ++j1) v[j1] = valid ? __ldcs(Y + G * j1) : make_float2(0.f, 0.f);
+  RowFFT<LOG2G, -1>::run(v, ex, tw1, lane);
+  if (valid) {
+    float2 *Gb = band + (size_t)seg * sumL + row.goff + row.dk;
+    const float *W = fwin + row.woff + row.dk;
+#pragma unroll
+    for (int i = 0; i < F; ++i)
+#pragma unroll
+      for (int n2 = 0; n2 < G; ++n2) {
+        const int j = (t + G * i) + 32 * n2;
+        const int jj = (G == 1) ? (j < 16 ? j : j - M) : (n2 < G / 2 ? j : j - M);
+        const int f = row.kc + jj;
+        if (jj <= row.dk && jj >= -row.dk && f >= 0 && f < nbins) Gb[jj] = pscale(v[i * G + n2], W[jj]);
+      }
+  }
+}
+
+template <int NWARPS, bool FORWARD>
+__global__ void __launch_bounds__(NWARPS * 32)
+k_rows_fast(FastParams P, const FastRow *__restrict__ frows, const float2 *__restrict__ tw1g,
+            const float *__restrict__ fwin, const float2 *__restrict__ spec, long long xstride, int nbins,
+            float2 *__restrict__ coef, long long ctot, float2 *__restrict__ band, long long sumL,
+            int batch, int plane) {
+  float2 *tw1s = reinterpret_cast<float2 *>(qtam_fast_smem);
+  float2 *exall = tw1s + P.tw_total;
+  for (int i = threadIdx.x; i < P.tw_total; i += NWARPS * 32) tw1s[i] = tw1g[i];
+  __syncthreads();
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  float2 *ex = exall + warp * kExPerWarp;
+  const long long total = (long long)P.groups_per_seg * batch;
+  for (long long item = ((long long)blockIdx.x * NWARPS) + warp; item < total;
+       item += (long long)gridDim.x * NWARPS) {
+    // decode: buckets in order, each spanning ngroups*batch items
+    int q = 0;
+    long long rem = item;
+    while (q + 1 < P.nbuckets && rem >= (long long)P.b[q].ngroups * batch) {
+      rem -= (long long)P.b[q].ngroups * batch;
+      ++q;
+    }
+    const FastBucket B = P.b[q];
+    const int seg = (int)(rem / B.ngroups);
+    const int grp = (int)(rem - (long long)seg * B.ngroups);
+    const float2 *tw1 = tw1s + B.tw_base;
+#define QTAM_ROW_CASE(L)                                                                              \
+  case L:                                                                                             \
+    if (FORWARD) fwd_group<L>(B, frows, seg, grp, lane, ex, tw1, spec, xstride, nbins, fwin, coef, ctot); \
+    else inv_group<L>(B, frows, seg, grp, lane, ex, tw1, coef, ctot, nbins, fwin, band, sumL, plane);  \
+    break;
+    switch (B.log2G) {
+      QTAM_ROW_CASE(5) QTAM_ROW_CASE(4) QTAM_ROW_CASE(3) QTAM_ROW_CASE(2) QTAM_ROW_CASE(1) QTAM_ROW_CASE(0)
+      default: break;
+    }
+#undef QTAM_ROW_CASE
+  }
+}
+
+// --------------------------------------------------------------------------------------------------
+// K4: S[f] = sum of the bin's band values (CSR order = ascending row), Xhat = S/P on the cover set (R9),
+//     Z[f] = E + i O (E, O from Xhat[f], conj Xhat[Nc-f], e^{+2 pi i f/N}), scaled 1/Nc, then the long
+//     inverse FFT straight to x_out (row a8)
+// --------------------------------------------------------------------------------------------------
+template <int LOG2NC>
+__global__ void __launch_bounds__(CtaFftPlan<LOG2NC>::NT)
+k_reduce_c2r_fast(const float2 *__restrict__ band, long long sumL, const int32_t *__restrict__ ptr,
+                  const int32_t *__restrict__ idx, const float *__restrict__ invP, int nbins, int nP,
+                  int plane, const float2 *__restrict__ tw, int log2twn, float *__restrict__ x_out) {
+  constexpr int NC = 1 << LOG2NC, NT = CtaFftPlan<LOG2NC>::NT;
+  float2 *s = reinterpret_cast<float2 *>(qtam_fast_smem);
+  const float2 *Gb = band + (size_t)blockIdx.x * sumL;
+  const int nsets = nP + 1;
+  const int plo = plane < 0 ? 0 : plane, phi = plane < 0 ? nP : plane + 1;
+  const float *ip = invP + (size_t)(plane + 1) * nbins;
+  for (int f = threadIdx.x; f <= NC; f += NT) {
+    const int lo = ptr[(size_t)f * nsets + plo], hi = ptr[(size_t)f * nsets + phi];
+    float2 acc = make_float2(0.f, 0.f);
+    for (int e = lo; e < hi; ++e) acc = padd(acc, Gb[idx[e]]);
+    s[f] = pscale(acc, ip[f]);
+  }
+  __syncthreads();
+  const float h = 0.5f / (float)NC;
+  for (int f = threadIdx.x; f <= NC / 2; f += NT) {
+    const int g = NC - f;
+    float2 A = s[f], B = s[g];
+    if (f == 0) { A.y = 0.f; B.y = 0.f; }
+    const float2 E = make_float2(h * (A.x + B.x), h * (A.y - B.y));
+    const float2 D = make_float2(h * (A.x - B.x), h * (A.y + B.y));
+    const float2 w = __ldg(tw + ((size_t)f << (log2twn - LOG2NC - 1)));
+    const float2 O = make_float2(D.x * w.x - D.y * w.y, D.x * w.y + D.y * w.x);
+    s[f] = make_float2(E.x - O.y, E.y + O.x);
+    if (g != f && f != 0) s[g] = make_float2(E.x + O.y, -E.y + O.x);
+  }
+  __syncthreads();
+  float2 *gout = reinterpret_cast<float2 *>(x_out) + (size_t)blockIdx.x * NC;
+  cta_fft<LOG2NC, +1, false, true>(s, nullptr, gout, tw, log2twn, 1.f);
+}
+
+// --------------------------------------------------------------------------------------------------
+// host side
+// --------------------------------------------------------------------------------------------------
+static int ilog2(long long v) { int l = 0; while ((1LL << l) < v) ++l; return l; }
+
+template <typename K> static bool set_smem(K kernel, size_t bytes) {
+  return cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes) == cudaSuccess;
+}
+
+static const int kRowWarps = 8;
+
+template <int LOG2NC> static qtam_status r2c_launch(qtam_plan *p, const void *d_x, int batch, cudaStream_t st) {
+  const size_t smem = sizeof(float2) * (size_t)cta_fft_smem_elems<LOG2NC>();
+  if (!set_smem(k_r2c_fast<LOG2NC>, smem)) return QTAM_ERR_CUDA;
+  {
+    LaunchScope ls(p, st, K_R2C_FAST, (double)batch * (4.0 * (double)p->hp.N + 8.0 * (double)p->hp.nb));
+    k_r2c_fast<LOG2NC><<<batch, CtaFftPlan<LOG2NC>::NT, smem, st>>>(
+        static_cast<const float *>(d_x), static_cast<float2 *>(p->d_spec), p->xstride,
+        static_cast<const float2 *>(p->d_tw), ilog2(p->twn));
+  }
+  QTAM_LAUNCH_CHECK();
+  return QTAM_OK;
+}
+
+qtam_status fast_r2c(qtam_plan *p, const void *d_x, int batch, cudaStream_t st) {
+  switch (ilog2(p->hp.N) - 1) {
+    case 11: return r2c_launch<11>(p, d_x, batch, st);
+    case 12: return r2c_launch<12>(p, d_x, batch, st);
+    case 13: return r2c_launch<13>(p, d_x, batch, st);
+    case 14: return r2c_launch<14>(p, d_x, batch, st);
+    default: return QTAM_ERR_UNSUPPORTED;
+  }
+}
+
+template <bool FORWARD>
+static qtam_status rows_launch(qtam_plan *p, int batch, const void *d_coef_in, void *d_coef_out, int plane,
+                               cudaStream_t st) {
+  const FastParams &P = p->fast;
+  if (P.groups_per_seg == 0) return QTAM_OK;
+  const size_t smem = sizeof(float2) * ((size_t)P.tw_total + (size_t)kRowWarps * kExPerWarp);
+  auto kern = k_rows_fast<kRowWarps, FORWARD>;
+  if (!set_smem(kern, smem)) return QTAM_ERR_CUDA;
+  int occ = 1;
+  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, kRowWarps * 32, smem);
+  if (occ < 1) occ = 1;
+  const long long total = (long long)P.groups_per_seg * batch;
+  long long want = (total + kRowWarps - 1) / kRowWarps;
+  const long long resident = (long long)p->num_sms * occ;
+  // a few waves of resident CTAs, each looping: keeps the tail short without losing the twiddle preload
+  int grid = (int)(want < resident * 4 ? want : resident * 4);
+  if (grid < 1) grid = 1;
+  const double bytes = FORWARD ? (double)batch * 8.0 * (P.sum_M + (double)p->hp.nb)
+                               : (double)batch * 8.0 * (P.sum_M + P.sum_L);
+  {
+    LaunchScope ls(p, st, FORWARD ? K_FWD_ROWS_FAST : K_INV_ROWS_FAST, bytes);
+    kern<<<grid, kRowWarps * 32, smem, st>>>(
+        P, p->d_frows, static_cast<const float2 *>(FORWARD ? p->d_ftw_fwd : p->d_ftw_inv),
+        static_cast<const float *>(p->d_fwin), static_cast<const float2 *>(p->d_spec), p->xstride,
+        (int)p->hp.nb,
+        FORWARD ? static_cast<float2 *>(d_coef_out) : const_cast<float2 *>(static_cast<const float2 *>(d_coef_in)),
+        p->hp.ctot, static_cast<float2 *>(p->d_band), p->hp.sumL, batch, plane);
+  }
+  QTAM_LAUNCH_CHECK();
+  return QTAM_OK;
+}
+
+qtam_status fast_forward_rows(qtam_plan *p, int batch, void *d_coef, cudaStream_t st) {
+  return rows_launch<true>(p, batch, nullptr, d_coef, -1, st);
+}
+
+qtam_status fast_inverse_rows(qtam_plan *p, const void *d_coef, int batch, int plane, cudaStream_t st) {
+  return rows_launch<false>(p, batch, d_coef, nullptr, plane, st);
+}
+
+template <int LOG2NC>
+static qtam_status reduce_c2r_launch(qtam_plan *p, int batch, int plane, void *d_x_out, cudaStream_t st) {
+  const size_t smem = sizeof(float2) * (size_t)cta_fft_smem_elems<LOG2NC>();
+  if (!set_smem(k_reduce_c2r_fast<LOG2NC>, smem)) return QTAM_ERR_CUDA;
+  {
+    LaunchScope ls(p, st, K_REDUCE_C2R_FAST,
+                   (double)batch * (8.0 * (double)p->hp.sumL + 4.0 * (double)p->hp.N));
+    k_reduce_c2r_fast<LOG2NC><<<batch, CtaFftPlan<LOG2NC>::NT, smem, st>>>(
+        static_cast<const float2 *>(p->d_band), p->hp.sumL, p->d_csr_ptr, p->d_csr_idx,
+        static_cast<const float *>(p->d_invP), (int)p->hp.nb, p->hp.nP, plane,
+        static_cast<const float2 *>(p->d_tw), ilog2(p->twn), static_cast<float *>(d_x_out));
+  }
+  QTAM_LAUNCH_CHECK();
+  return QTAM_OK;
+}
+
+qtam_status fast_reduce_c2r(qtam_plan *p, int batch, int plane, void *d_x_out, cudaStream_t st) {
+  switch (ilog2(p->hp.N) - 1) {
+    case 11: return reduce_c2r_launch<11>(p, batch, plane, d_x_out, st);
+    case 12: return reduce_c2r_launch<12>(p, batch, plane, d_x_out, st);
+    case 13: return reduce_c2r_launch<13>(p, batch, plane, d_x_out, st);
+    case 14: return reduce_c2r_launch<14>(p, batch, plane, d_x_out, st);
+    default: return QTAM_ERR_UNSUPPORTED;
+  }
+}
+
+}  // namespace qtam
