@@ -1,6 +1,7 @@
 // api.cu -- the C ABI of libqtam (include/qtam.h): plan life cycle, argument checks, dispatch.
 #include <algorithm>
 #include <cmath>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <utility>
@@ -44,6 +45,7 @@ void free_plan(qtam_plan *p) {
   for (int c = 0; c < qtam_plan::kClasses; ++c) cudaFree(p->d_items[c]);
   cudaFree(p->d_bigrows); cudaFree(p->d_spec); cudaFree(p->d_ws); cudaFree(p->d_band);
   cudaFree(p->d_frows); cudaFree(p->d_fwin); cudaFree(p->d_ftw_fwd); cudaFree(p->d_ftw_inv);
+  cudaFree(p->d_tiny);
   for (ProfRec &r : p->prof_pool) { cudaEventDestroy(r.e0); cudaEventDestroy(r.e1); }
   delete p;
 }
@@ -120,6 +122,25 @@ qtam_status build_fast(qtam_plan *p) {
     F.b[F.nbuckets++] = B;
   }
   F.tw_total = (int)(twf.size() / 2);
+  // rows shorter than 32 points and the eligibility of the one-kernel inverse
+  std::vector<FastRow> tiny;
+  bool has_long_rows = false;
+  for (size_t k = 0; k < hp.rows.size(); ++k) {
+    const HostRow &h = hp.rows[k];
+    if (h.M > 1024) has_long_rows = true;
+    if (h.M >= 32) continue;
+    FastRow r{};
+    r.kc = (int)h.kc; r.dk = (int)h.dk; r.woff = window_of(h); r.goff = ilog2(h.M);
+    r.offset = (int)h.offset; r.plane = h.plane;
+    tiny.push_back(r);
+  }
+  p->n_tiny = (int)tiny.size();
+  if (!upload(&p->d_tiny, tiny.data(), tiny.size(), tot)) return QTAM_ERR_ALLOC;
+  {
+    const int lnc = ilog2(hp.N) - 1;
+    p->fused_inv = p->fast_long && lnc <= 13 && !has_long_rows && p->n_tiny <= 256;
+    if (getenv("QTAM_NO_FUSED_INV")) p->fused_inv = false;
+  }
   if (hp.ctot >= (int64_t(1) << 31)) return QTAM_ERR_UNSUPPORTED;
   if (!upload(&p->d_frows, frows.data(), frows.size(), tot)) return QTAM_ERR_ALLOC;
   float *d = nullptr;
@@ -337,6 +358,7 @@ qtam_status qtam_inverse(qtam_plan *p, const void *d_coef, int batch, int plane,
   p->last_launches = 0;
   if (batch == 0) return QTAM_OK;
   cudaStream_t st = static_cast<cudaStream_t>(stream);
+  if (p->fused_inv) return fused_inverse(p, d_coef, batch, plane, d_x_out, st);
   qtam_status s = QTAM_OK;
   if (p->fast_rows) {
     s = fast_inverse_rows(p, d_coef, batch, plane, st);
@@ -377,7 +399,7 @@ int qtam_last_launch_count(const qtam_plan *p) { return p ? p->last_launches : 0
 static const char *const kKernelNames[K_COUNT] = {
     "cfft_seq", "cfft_cols", "cfft_rows", "r2c_post", "c2r_pre", "fwd_rows", "fwd_combine",
     "inv_rows", "inv_reduce", "dense_place", "threshold", "r2c_fast", "fwd_rows_fast", "inv_rows_fast",
-    "reduce_c2r_fast"};
+    "reduce_c2r_fast", "inv_fused"};
 
 qtam_status qtam_profile_enable(qtam_plan *p, int on, int max_launches) {
   if (!p || p->host_only) return QTAM_ERR_INVALID_ARG;

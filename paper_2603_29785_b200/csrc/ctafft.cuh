@@ -9,18 +9,29 @@
 
 namespace qtam {
 
+// radices per (log2 Nc, threads per CTA); every pass has Nc/R butterflies spread over NT threads
+template <int LOG2NC, int NT> struct CtaFftRadix;
+template <> struct CtaFftRadix<11, 128> { static constexpr int R0 = 16, R1 = 16, R2 = 8; };
+template <> struct CtaFftRadix<11, 256> { static constexpr int R0 = 16, R1 = 16, R2 = 8; };
+template <> struct CtaFftRadix<11, 512> { static constexpr int R0 = 16, R1 = 16, R2 = 8; };
+template <> struct CtaFftRadix<12, 256> { static constexpr int R0 = 16, R1 = 16, R2 = 16; };
+template <> struct CtaFftRadix<12, 512> { static constexpr int R0 = 16, R1 = 16, R2 = 16; };
+template <> struct CtaFftRadix<13, 256> { static constexpr int R0 = 32, R1 = 16, R2 = 16; };
+template <> struct CtaFftRadix<13, 512> { static constexpr int R0 = 16, R1 = 16, R2 = 32; };
+template <> struct CtaFftRadix<14, 512> { static constexpr int R0 = 32, R1 = 32, R2 = 16; };
+// default thread count of the stand-alone long-FFT kernels
 template <int LOG2NC> struct CtaFftPlan;
-template <> struct CtaFftPlan<11> { static constexpr int NT = 128, P = 3, R0 = 16, R1 = 16, R2 = 8; };
-template <> struct CtaFftPlan<12> { static constexpr int NT = 256, P = 3, R0 = 16, R1 = 16, R2 = 16; };
-template <> struct CtaFftPlan<13> { static constexpr int NT = 256, P = 3, R0 = 32, R1 = 16, R2 = 16; };
-template <> struct CtaFftPlan<14> { static constexpr int NT = 512, P = 3, R0 = 32, R1 = 32, R2 = 16; };
+template <> struct CtaFftPlan<11> { static constexpr int NT = 128; };
+template <> struct CtaFftPlan<12> { static constexpr int NT = 256; };
+template <> struct CtaFftPlan<13> { static constexpr int NT = 256; };
+template <> struct CtaFftPlan<14> { static constexpr int NT = 512; };
 
 template <int V> struct ILog2 { static constexpr int value = 1 + ILog2<V / 2>::value; };
 template <> struct ILog2<1> { static constexpr int value = 0; };
 
 // shared-memory elements the transform needs (skew padding included)
-template <int LOG2NC> constexpr int cta_fft_smem_elems() {
-  return (1 << LOG2NC) + ((1 << LOG2NC) >> ILog2<CtaFftPlan<LOG2NC>::R0>::value) + 2;
+template <int LOG2NC> __host__ __device__ constexpr int cta_fft_smem_elems() {
+  return (1 << LOG2NC) + ((1 << LOG2NC) >> 4) + 2;   // the smallest first radix is 16
 }
 
 // One Stockham pass.  IN_MODE / OUT_MODE: 0 natural smem, 1 skewed smem, 2 global (natural).
@@ -77,18 +88,18 @@ __device__ __forceinline__ void cta_fft_pass(float2 *s, const float2 *__restrict
   if constexpr (OUT_MODE != 2) __syncthreads();
 }
 
-// Whole transform.  FROM_GLOBAL: pass 1 reads gin (natural order) instead of s (natural layout).
+// Whole transform with NT threads (all threads of the CTA must call it).
+// FROM_GLOBAL: pass 1 reads gin (natural order) instead of s (natural layout).
 // TO_GLOBAL: the last pass writes gout (natural order, times out_scale) instead of s (natural layout).
-template <int LOG2NC, int DIR, bool FROM_GLOBAL, bool TO_GLOBAL>
+template <int LOG2NC, int NT, int DIR, bool FROM_GLOBAL, bool TO_GLOBAL>
 __device__ __forceinline__ void cta_fft(float2 *s, const float2 *__restrict__ gin, float2 *__restrict__ gout,
                                         const float2 *__restrict__ tw, int log2twn, float out_scale) {
-  typedef CtaFftPlan<LOG2NC> PL;
+  typedef CtaFftRadix<LOG2NC, NT> PL;
   constexpr int L0 = ILog2<PL::R0>::value, L1 = ILog2<PL::R1>::value;
-  static_assert(PL::P == 3, "three passes");
   static_assert(L0 + L1 + ILog2<PL::R2>::value == LOG2NC, "radices must multiply to Nc");
-  cta_fft_pass<LOG2NC, PL::NT, PL::R0, 0, DIR, FROM_GLOBAL ? 2 : 0, 1, L0>(s, gin, gout, tw, log2twn, 1.f);
-  cta_fft_pass<LOG2NC, PL::NT, PL::R1, L0, DIR, 1, 0, L0>(s, gin, gout, tw, log2twn, 1.f);
-  cta_fft_pass<LOG2NC, PL::NT, PL::R2, L0 + L1, DIR, 0, TO_GLOBAL ? 2 : 0, L0>(s, gin, gout, tw, log2twn, out_scale);
+  cta_fft_pass<LOG2NC, NT, PL::R0, 0, DIR, FROM_GLOBAL ? 2 : 0, 1, L0>(s, gin, gout, tw, log2twn, 1.f);
+  cta_fft_pass<LOG2NC, NT, PL::R1, L0, DIR, 1, 0, L0>(s, gin, gout, tw, log2twn, 1.f);
+  cta_fft_pass<LOG2NC, NT, PL::R2, L0 + L1, DIR, 0, TO_GLOBAL ? 2 : 0, L0>(s, gin, gout, tw, log2twn, out_scale);
 }
 
 }  // namespace qtam

@@ -12,7 +12,7 @@ namespace qtam {
 enum KernelId {
   K_CFFT_SEQ = 0, K_CFFT_COLS, K_CFFT_ROWS, K_R2C_POST, K_C2R_PRE, K_FWD_ROWS, K_FWD_COMBINE,
   K_INV_ROWS, K_INV_REDUCE, K_DENSE_PLACE, K_THRESHOLD, K_R2C_FAST, K_FWD_ROWS_FAST, K_INV_ROWS_FAST,
-  K_REDUCE_C2R_FAST, K_COUNT
+  K_REDUCE_C2R_FAST, K_INV_FUSED, K_COUNT
 };
 // fast float path (fast.cu): rows with 32 <= M <= 1024, grouped by G = M/32 lanes per row
 struct FastRow { int kc, dk, woff, goff, offset, plane; };
@@ -66,6 +66,9 @@ struct qtam_plan {
   void *d_fwin = nullptr;      // float windows, one per distinct half-width
   void *d_ftw_fwd = nullptr;   // float2 pass-1 twiddles [bucket][n1][t], forward (x (N M)^-1/2)
   void *d_ftw_inv = nullptr;   // same, inverse (conjugate, x sqrt(N/M))
+  qtam::FastRow *d_tiny = nullptr;   // rows shorter than 32 points (goff holds log2 M), for fused_inv.cu
+  int n_tiny = 0;
+  bool fused_inv = false;      // the whole inverse runs in one kernel (fused_inv.cu)
 
   int last_launches = 0;
   // launch profile (qtam_profile_enable / qtam_profile_read)
@@ -108,5 +111,7 @@ qtam_status fast_r2c(qtam_plan *p, const void *d_x, int batch, cudaStream_t st);
 qtam_status fast_forward_rows(qtam_plan *p, int batch, void *d_coef, cudaStream_t st);
 qtam_status fast_inverse_rows(qtam_plan *p, const void *d_coef, int batch, int plane, cudaStream_t st);
 qtam_status fast_reduce_c2r(qtam_plan *p, int batch, int plane, void *d_x_out, cudaStream_t st);
+// fused_inv.cu
+qtam_status fused_inverse(qtam_plan *p, const void *d_coef, int batch, int plane, void *d_x_out, cudaStream_t st);
 
 }  // namespace qtam

@@ -8,6 +8,8 @@
 //   K4 k_reduce_c2r_fast a6-a8 one CTA per segment: segmented reduction over bins (fixed order, no
 //                              atomics), 1/P, Hermitian pre-processing and the long inverse FFT in smem
 // Rows outside 32..1024 points, double precision and N outside 2^12..2^15 run in generic.cu.
+#include <cstdlib>
+
 #include "cplx.cuh"
 #include "ctafft.cuh"
 #include "device_plan.hpp"
@@ -33,7 +35,7 @@ k_r2c_fast(const float *__restrict__ x, float2 *__restrict__ spec, long long xst
   constexpr int NC = 1 << LOG2NC, NT = CtaFftPlan<LOG2NC>::NT;
   float2 *s = reinterpret_cast<float2 *>(qtam_fast_smem);
   const float2 *gin = reinterpret_cast<const float2 *>(x) + (size_t)blockIdx.x * NC;
-  cta_fft<LOG2NC, -1, true, false>(s, gin, nullptr, tw, log2twn, 1.f);
+  cta_fft<LOG2NC, NT, -1, true, false>(s, gin, nullptr, tw, log2twn, 1.f);
   float2 *X = spec + (size_t)blockIdx.x * xstride;
   for (int f = threadIdx.x; f <= NC / 2; f += NT) {
     const int g = NC - f;
@@ -201,7 +203,7 @@ k_reduce_c2r_fast(const float2 *__restrict__ band, long long sumL, const int32_t
   }
   __syncthreads();
   float2 *gout = reinterpret_cast<float2 *>(x_out) + (size_t)blockIdx.x * NC;
-  cta_fft<LOG2NC, +1, false, true>(s, nullptr, gout, tw, log2twn, 1.f);
+  cta_fft<LOG2NC, NT, +1, false, true>(s, nullptr, gout, tw, log2twn, 1.f);
 }
 
 // --------------------------------------------------------------------------------------------------
@@ -212,8 +214,6 @@ static int ilog2(long long v) { int l = 0; while ((1LL << l) < v) ++l; return l;
 template <typename K> static bool set_smem(K kernel, size_t bytes) {
   return cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes) == cudaSuccess;
 }
-
-static const int kRowWarps = 8;
 
 template <int LOG2NC> static qtam_status r2c_launch(qtam_plan *p, const void *d_x, int batch, cudaStream_t st) {
   const size_t smem = sizeof(float2) * (size_t)cta_fft_smem_elems<LOG2NC>();
@@ -238,19 +238,19 @@ qtam_status fast_r2c(qtam_plan *p, const void *d_x, int batch, cudaStream_t st) 
   }
 }
 
-template <bool FORWARD>
-static qtam_status rows_launch(qtam_plan *p, int batch, const void *d_coef_in, void *d_coef_out, int plane,
-                               cudaStream_t st) {
+template <int NW, bool FORWARD>
+static qtam_status rows_launch_nw(qtam_plan *p, int batch, const void *d_coef_in, void *d_coef_out, int plane,
+                                  cudaStream_t st) {
   const FastParams &P = p->fast;
   if (P.groups_per_seg == 0) return QTAM_OK;
-  const size_t smem = sizeof(float2) * ((size_t)P.tw_total + (size_t)kRowWarps * kExPerWarp);
-  auto kern = k_rows_fast<kRowWarps, FORWARD>;
+  const size_t smem = sizeof(float2) * ((size_t)P.tw_total + (size_t)NW * kExPerWarp);
+  auto kern = k_rows_fast<NW, FORWARD>;
   if (!set_smem(kern, smem)) return QTAM_ERR_CUDA;
   int occ = 1;
-  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, kRowWarps * 32, smem);
+  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, NW * 32, smem);
   if (occ < 1) occ = 1;
   const long long total = (long long)P.groups_per_seg * batch;
-  long long want = (total + kRowWarps - 1) / kRowWarps;
+  long long want = (total + NW - 1) / NW;
   const long long resident = (long long)p->num_sms * occ;
   // a few waves of resident CTAs, each looping: keeps the tail short without losing the twiddle preload
   int grid = (int)(want < resident * 4 ? want : resident * 4);
@@ -259,7 +259,7 @@ static qtam_status rows_launch(qtam_plan *p, int batch, const void *d_coef_in, v
                                : (double)batch * 8.0 * (P.sum_M + P.sum_L);
   {
     LaunchScope ls(p, st, FORWARD ? K_FWD_ROWS_FAST : K_INV_ROWS_FAST, bytes);
-    kern<<<grid, kRowWarps * 32, smem, st>>>(
+    kern<<<grid, NW * 32, smem, st>>>(
         P, p->d_frows, static_cast<const float2 *>(FORWARD ? p->d_ftw_fwd : p->d_ftw_inv),
         static_cast<const float *>(p->d_fwin), static_cast<const float2 *>(p->d_spec), p->xstride,
         (int)p->hp.nb,
@@ -268,6 +268,28 @@ static qtam_status rows_launch(qtam_plan *p, int batch, const void *d_coef_in, v
   }
   QTAM_LAUNCH_CHECK();
   return QTAM_OK;
+}
+
+static int row_warps() {
+  static int v = -1;
+  if (v < 0) {
+    const char *e = getenv("QTAM_ROW_WARPS");
+    v = e ? atoi(e) : 8;
+  }
+  return v;
+}
+
+template <bool FORWARD>
+static qtam_status rows_launch(qtam_plan *p, int batch, const void *d_coef_in, void *d_coef_out, int plane,
+                               cudaStream_t st) {
+  switch (row_warps()) {
+    case 4: return rows_launch_nw<4, FORWARD>(p, batch, d_coef_in, d_coef_out, plane, st);
+    case 12: return rows_launch_nw<12, FORWARD>(p, batch, d_coef_in, d_coef_out, plane, st);
+    case 16: return rows_launch_nw<16, FORWARD>(p, batch, d_coef_in, d_coef_out, plane, st);
+    case 20: return rows_launch_nw<20, FORWARD>(p, batch, d_coef_in, d_coef_out, plane, st);
+    case 24: return rows_launch_nw<24, FORWARD>(p, batch, d_coef_in, d_coef_out, plane, st);
+    default: return rows_launch_nw<8, FORWARD>(p, batch, d_coef_in, d_coef_out, plane, st);
+  }
 }
 
 qtam_status fast_forward_rows(qtam_plan *p, int batch, void *d_coef, cudaStream_t st) {
