@@ -43,7 +43,8 @@ void free_plan(qtam_plan *p) {
   cudaFree(p->d_rows); cudaFree(p->d_win); cudaFree(p->d_tw); cudaFree(p->d_invP);
   cudaFree(p->d_csr_ptr); cudaFree(p->d_csr_idx);
   for (int c = 0; c < qtam_plan::kClasses; ++c) cudaFree(p->d_items[c]);
-  cudaFree(p->d_bigrows); cudaFree(p->d_spec); cudaFree(p->d_ws); cudaFree(p->d_band);
+  cudaFree(p->d_bigrows); cudaFree(p->d_spec_alloc); cudaFree(p->d_ws); cudaFree(p->d_band);
+  cudaFree(p->d_fwin2);
   cudaFree(p->d_frows); cudaFree(p->d_fwin); cudaFree(p->d_ftw_fwd); cudaFree(p->d_ftw_inv);
   cudaFree(p->d_tiny);
   for (ProfRec &r : p->prof_pool) { cudaEventDestroy(r.e0); cudaEventDestroy(r.e1); }
@@ -90,19 +91,35 @@ qtam_status build_fast(qtam_plan *p) {
     seen.push_back({h.dk, off});
     return off;
   };
+  // the same windows as (w,w) pairs, zero-padded to the M points of the row's short FFT and stored at
+  // the M-array index (j mod M): the fast gather multiplies without testing the support
+  std::vector<float> fwin2;
+  std::vector<std::pair<int64_t, int>> seen2;
+  auto wpad_of = [&](const HostRow &h) -> int {
+    for (auto &e : seen2) if (e.first == h.dk) return e.second;
+    const int off = (int)(fwin2.size() / 2);
+    fwin2.resize(fwin2.size() + 2 * (size_t)h.M, 0.0f);
+    for (int64_t jj = -h.dk; jj <= h.dk; ++jj) {
+      const int64_t j = (jj + h.M) % h.M;
+      const float w = (float)hp.win[(size_t)(h.woff + jj + h.dk)];
+      fwin2[2 * (size_t)(off + j)] = w; fwin2[2 * (size_t)(off + j) + 1] = w;
+    }
+    seen2.push_back({h.dk, off});
+    return off;
+  };
   std::vector<FastRow> frows;
-  std::vector<float> twf, twi;   // interleaved re,im
+  std::vector<float> twf, twi;   // (wx, wx, wy, wy) per entry
   const long double tau = 6.283185307179586476925286766559005768L;
   for (int lg = 5; lg >= 0; --lg) {
     const int G = 1 << lg, M = 32 * G, Fr = 32 / G;
     FastBucket B{};
-    B.log2G = lg; B.row_base = (int)frows.size(); B.tw_base = (int)(twf.size() / 2);
+    B.log2G = lg; B.row_base = (int)frows.size(); B.tw_base = (int)(twf.size() / 4);
     for (size_t k = 0; k < hp.rows.size(); ++k) {
       const HostRow &h = hp.rows[k];
       if (h.M != M) continue;
       FastRow r{};
       r.kc = (int)h.kc; r.dk = (int)h.dk; r.woff = window_of(h); r.goff = (int)h.goff;
-      r.offset = (int)h.offset; r.plane = h.plane;
+      r.offset = (int)h.offset; r.plane = h.plane; r.wpad = wpad_of(h);
       frows.push_back(r);
       F.sum_M += (double)h.M; F.sum_L += (double)h.L;
     }
@@ -115,13 +132,14 @@ qtam_status build_fast(qtam_plan *p) {
         const int m = (n1 * t) % M;
         const long double a = tau * (long double)m / (long double)M;
         const double c = (double)cosl(a), s = (double)sinl(a);
-        twf.push_back((float)(c * sf)); twf.push_back((float)(s * sf));
-        twi.push_back((float)(c * si)); twi.push_back((float)(-s * si));
+        twf.push_back((float)(c * sf)); twf.push_back((float)(c * sf));
+        twf.push_back((float)(s * sf)); twf.push_back((float)(s * sf));
+        twi.push_back((float)(c * si)); twi.push_back((float)(-s * si));   // inverse tables stay (wx, wy)
       }
     F.groups_per_seg += B.ngroups;
     F.b[F.nbuckets++] = B;
   }
-  F.tw_total = (int)(twf.size() / 2);
+  F.tw_total = (int)(twf.size() / 4);
   // rows shorter than 32 points and the eligibility of the one-kernel inverse
   std::vector<FastRow> tiny;
   bool has_long_rows = false;
@@ -146,6 +164,8 @@ qtam_status build_fast(qtam_plan *p) {
   float *d = nullptr;
   if (!upload(&d, fwin.data(), fwin.size(), tot)) return QTAM_ERR_ALLOC;
   p->d_fwin = d;
+  if (!upload(&d, fwin2.data(), fwin2.size(), tot)) return QTAM_ERR_ALLOC;
+  p->d_fwin2 = d;
   if (!upload(&d, twf.data(), twf.size(), tot)) return QTAM_ERR_ALLOC;
   p->d_ftw_fwd = d;
   if (!upload(&d, twi.data(), twi.size(), tot)) return QTAM_ERR_ALLOC;
@@ -231,7 +251,14 @@ template <typename T> qtam_status build_device(qtam_plan *p) {
   }
   // workspace
   const size_t csz = 2 * sizeof(T);
-  if (!dev_alloc(&p->d_spec, csz * size_t(p->max_batch) * size_t(p->xstride), tot)) return QTAM_ERR_ALLOC;
+  {
+    // every segment's spectrum has kSpecPad zero bins before and after it, so that the fast gather can
+    // read a full M-point neighbourhood of any centre bin without bounds checks (R8 clipping for free)
+    const size_t bytes = csz * (size_t(p->max_batch) * size_t(p->xstride) + 2 * size_t(kSpecPad));
+    if (!dev_alloc(&p->d_spec_alloc, bytes, tot)) return QTAM_ERR_ALLOC;
+    if (cudaMemset(p->d_spec_alloc, 0, bytes) != cudaSuccess) return QTAM_ERR_CUDA;
+    p->d_spec = static_cast<char *>(p->d_spec_alloc) + csz * size_t(kSpecPad);
+  }
   if (!dev_alloc(&p->d_ws, csz * size_t(p->max_batch) * size_t(hp.N), tot)) return QTAM_ERR_ALLOC;
   if (!dev_alloc(&p->d_band, csz * size_t(p->max_batch) * size_t(hp.sumL), tot)) return QTAM_ERR_ALLOC;
   return QTAM_OK;
@@ -257,7 +284,7 @@ qtam_status qtam_plan_create(qtam_plan **out, double fs, int64_t N, const double
   if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) { delete p; return QTAM_ERR_CUDA; }
   p->esz = dtype == QTAM_F32 ? 4 : 8;
   p->max_batch = p->hp.opt.max_batch;
-  p->xstride = ((p->hp.nb + 31) / 32) * 32;
+  p->xstride = ((p->hp.nb + kSpecPad + 31) / 32) * 32;
   p->twn = N;
   p->cap_log2 = dtype == QTAM_F32 ? 13 : 12;
   {

@@ -15,7 +15,7 @@ enum KernelId {
   K_REDUCE_C2R_FAST, K_INV_FUSED, K_COUNT
 };
 // fast float path (fast.cu): rows with 32 <= M <= 1024, grouped by G = M/32 lanes per row
-struct FastRow { int kc, dk, woff, goff, offset, plane; };
+struct FastRow { int kc, dk, woff, goff, offset, plane, wpad, pad; };   // wpad: offset into the padded window table
 struct FastBucket { int log2G, nrows, ngroups, row_base, tw_base, pad; };
 struct FastParams {
   int nbuckets, groups_per_seg, tw_total, pad;
@@ -24,6 +24,8 @@ struct FastParams {
 };
 struct ProfRec { int kid; double bytes; cudaEvent_t e0, e1; };
 }  // namespace qtam
+
+namespace qtam { constexpr int kSpecPad = 512; }   // zero bins kept on both sides of every segment's spectrum
 
 struct qtam_plan {
   qtam::HostPlan hp;
@@ -64,6 +66,8 @@ struct qtam_plan {
   qtam::FastParams fast{};
   qtam::FastRow *d_frows = nullptr;
   void *d_fwin = nullptr;      // float windows, one per distinct half-width
+  void *d_fwin2 = nullptr;     // float2 (w,w) windows zero-padded to M points in M-array order (index j mod M)
+  void *d_spec_alloc = nullptr;   // allocation behind d_spec (zero pads of kSpecPad bins on both sides)
   void *d_ftw_fwd = nullptr;   // float2 pass-1 twiddles [bucket][n1][t], forward (x (N M)^-1/2)
   void *d_ftw_inv = nullptr;   // same, inverse (conjugate, x sqrt(N/M))
   qtam::FastRow *d_tiny = nullptr;   // rows shorter than 32 points (goff holds log2 M), for fused_inv.cu

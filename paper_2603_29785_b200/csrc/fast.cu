@@ -9,6 +9,7 @@
 //                              atomics), 1/P, Hermitian pre-processing and the long inverse FFT in smem
 // Rows outside 32..1024 points, double precision and N outside 2^12..2^15 run in generic.cu.
 #include <cstdlib>
+#include <type_traits>
 
 #include "cplx.cuh"
 #include "ctafft.cuh"
@@ -23,6 +24,10 @@ namespace qtam {
   } while (0)
 
 extern __shared__ __align__(16) unsigned char qtam_fast_smem[];
+
+#ifndef QTAM_GROUP_INLINE
+#define QTAM_GROUP_INLINE __forceinline__
+#endif
 
 // --------------------------------------------------------------------------------------------------
 // K1: long R2C.  z[m] = x[2m] + i x[2m+1]; Z = FFT_Nc(z);
@@ -57,29 +62,26 @@ k_r2c_fast(const float *__restrict__ x, float2 *__restrict__ spec, long long xst
 // warps read overlap in L1.
 // --------------------------------------------------------------------------------------------------
 template <int LOG2G>
-__device__ __noinline__ void fwd_group(const FastBucket &B, const FastRow *__restrict__ frows, int seg, int grp,
-                                          int lane, float2 *ex, const float2 *tw1,
-                                          const float2 *__restrict__ spec, long long xstride, int nbins,
-                                          const float *__restrict__ fwin, float2 *__restrict__ coef,
-                                          long long ctot) {
+__device__ QTAM_GROUP_INLINE void fwd_group(const FastBucket &B, const FastRow *__restrict__ frows, int seg, int grp,
+                                       int lane, float2 *ex, const float4 *tw1,
+                                       const float2 *__restrict__ spec, long long xstride,
+                                       const float2 *__restrict__ fwin2, float2 *__restrict__ coef,
+                                       long long ctot) {
   constexpr int G = 1 << LOG2G, F = 32 / G, M = 32 * G;
   const int t = lane & (G - 1), rw = lane >> LOG2G;
   const int r = grp * F + rw;
   const bool valid = r < B.nrows;
-  FastRow row;
-  if (valid) row = frows[B.row_base + r];
-  else { row.kc = 0; row.dk = -1; row.woff = 0; row.goff = 0; row.offset = 0; }
-  const float2 *X = spec + (size_t)seg * xstride + row.kc;
-  const float *W = fwin + row.woff + row.dk;
+  // lanes past the end of the bucket recompute its first row and simply do not store
+  const FastRow row = frows[B.row_base + (valid ? r : 0)];
+  // B_k[j] = X[kc + jj(j)] * Wpad[j]: the window table is zero outside the support and the spectrum
+  // buffer has zero pads, so neither the support (A9) nor the clipping at DC / Nyquist (R8) needs a test
+  const float2 *X = spec + (size_t)seg * xstride + row.kc + t;
+  const float2 *W = fwin2 + row.wpad + t;
   float2 v[32];
 #pragma unroll
   for (int j1 = 0; j1 < 32; ++j1) {
-    const int jj = (j1 < 16) ? (t + G * j1) : (t + G * j1 - M);     // signed offset from the centre (R6)
-    const int f = row.kc + jj;
-    const bool ok = (jj <= row.dk) && (jj >= -row.dk) && (f >= 0) && (f < nbins);   // support, R8 clip
-    float2 xv = make_float2(0.f, 0.f);
-    if (ok) xv = pscale(X[jj], W[jj]);
-    v[j1] = xv;
+    const int jj = (j1 < 16) ? (G * j1) : (G * j1 - M);     // signed offset from the centre (R6), minus t
+    v[j1] = pmul(X[jj], W[G * j1]);
   }
   RowFFT<LOG2G, +1>::run(v, ex, tw1, lane);
   if (valid) {
@@ -92,7 +94,7 @@ __device__ __noinline__ void fwd_group(const FastBucket &B, const FastRow *__res
 }
 
 template <int LOG2G>
-__device__ __noinline__ void inv_group(const FastBucket &B, const FastRow *__restrict__ frows, int seg, int grp,
+__device__ QTAM_GROUP_INLINE void inv_group(const FastBucket &B, const FastRow *__restrict__ frows, int seg, int grp,
                                           int lane, float2 *ex, const float2 *tw1,
                                           const float2 *__restrict__ coef, long long ctot, int nbins,
                                           const float *__restrict__ fwin, float2 *__restrict__ band,
@@ -128,13 +130,17 @@ __device__ __noinline__ void inv_group(const FastBucket &B, const FastRow *__res
 }
 
 template <int NWARPS, bool FORWARD>
-__global__ void __launch_bounds__(NWARPS * 32)
-k_rows_fast(FastParams P, const FastRow *__restrict__ frows, const float2 *__restrict__ tw1g,
-            const float *__restrict__ fwin, const float2 *__restrict__ spec, long long xstride, int nbins,
+__global__ void __launch_bounds__(NWARPS * 32, NWARPS <= 8 ? 2 : 1)
+k_rows_fast(FastParams P, const FastRow *__restrict__ frows, const void *__restrict__ tw1g_,
+            const float *__restrict__ fwin, const float2 *__restrict__ fwin2,
+            const float2 *__restrict__ spec, long long xstride, int nbins,
             float2 *__restrict__ coef, long long ctot, float2 *__restrict__ band, long long sumL,
             int batch, int plane) {
-  float2 *tw1s = reinterpret_cast<float2 *>(qtam_fast_smem);
-  float2 *exall = tw1s + P.tw_total;
+  // forward tables are (wx, wx, wy, wy) float4, inverse tables (wx, wy) float2
+  typedef typename std::conditional<FORWARD, float4, float2>::type TW;
+  const TW *tw1g = static_cast<const TW *>(tw1g_);
+  TW *tw1s = reinterpret_cast<TW *>(qtam_fast_smem);
+  float2 *exall = reinterpret_cast<float2 *>(qtam_fast_smem + sizeof(float4) * (size_t)P.tw_total);
   for (int i = threadIdx.x; i < P.tw_total; i += NWARPS * 32) tw1s[i] = tw1g[i];
   __syncthreads();
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -152,10 +158,10 @@ k_rows_fast(FastParams P, const FastRow *__restrict__ frows, const float2 *__res
     const FastBucket B = P.b[q];
     const int seg = (int)(rem / B.ngroups);
     const int grp = (int)(rem - (long long)seg * B.ngroups);
-    const float2 *tw1 = tw1s + B.tw_base;
+    const TW *tw1 = tw1s + B.tw_base;
 #define QTAM_ROW_CASE(L)                                                                              \
   case L:                                                                                             \
-    if (FORWARD) fwd_group<L>(B, frows, seg, grp, lane, ex, tw1, spec, xstride, nbins, fwin, coef, ctot); \
+    if constexpr (FORWARD) fwd_group<L>(B, frows, seg, grp, lane, ex, tw1, spec, xstride, fwin2, coef, ctot); \
     else inv_group<L>(B, frows, seg, grp, lane, ex, tw1, coef, ctot, nbins, fwin, band, sumL, plane);  \
     break;
     switch (B.log2G) {
@@ -243,7 +249,7 @@ static qtam_status rows_launch_nw(qtam_plan *p, int batch, const void *d_coef_in
                                   cudaStream_t st) {
   const FastParams &P = p->fast;
   if (P.groups_per_seg == 0) return QTAM_OK;
-  const size_t smem = sizeof(float2) * ((size_t)P.tw_total + (size_t)NW * kExPerWarp);
+  const size_t smem = sizeof(float4) * (size_t)P.tw_total + sizeof(float2) * (size_t)NW * kExPerWarp;
   auto kern = k_rows_fast<NW, FORWARD>;
   if (!set_smem(kern, smem)) return QTAM_ERR_CUDA;
   int occ = 1;
@@ -260,8 +266,9 @@ static qtam_status rows_launch_nw(qtam_plan *p, int batch, const void *d_coef_in
   {
     LaunchScope ls(p, st, FORWARD ? K_FWD_ROWS_FAST : K_INV_ROWS_FAST, bytes);
     kern<<<grid, NW * 32, smem, st>>>(
-        P, p->d_frows, static_cast<const float2 *>(FORWARD ? p->d_ftw_fwd : p->d_ftw_inv),
-        static_cast<const float *>(p->d_fwin), static_cast<const float2 *>(p->d_spec), p->xstride,
+        P, p->d_frows, static_cast<const void *>(FORWARD ? p->d_ftw_fwd : p->d_ftw_inv),
+        static_cast<const float *>(p->d_fwin), static_cast<const float2 *>(p->d_fwin2),
+        static_cast<const float2 *>(p->d_spec), p->xstride,
         (int)p->hp.nb,
         FORWARD ? static_cast<float2 *>(d_coef_out) : const_cast<float2 *>(static_cast<const float2 *>(d_coef_in)),
         p->hp.ctot, static_cast<float2 *>(p->d_band), p->hp.sumL, batch, plane);

@@ -38,6 +38,10 @@ __device__ __forceinline__ float2 pfma(float2 a, float2 b, float2 c) {
 __device__ __forceinline__ float2 pcmul(float2 a, float2 w) {
   return pfma(a, make_float2(w.x, w.x), pmul(make_float2(-a.y, a.x), make_float2(w.y, w.y)));
 }
+// same with the twiddle stored pre-duplicated as (wx, wx, wy, wy): no pair-building moves
+__device__ __forceinline__ float2 pcmul4(float2 a, float4 w) {
+  return pfma(a, make_float2(w.x, w.y), pmul(make_float2(-a.y, a.x), make_float2(w.z, w.w)));
+}
 __device__ __forceinline__ float2 pscale(float2 a, float s) { return pmul(a, make_float2(s, s)); }
 
 // cos / sin of 2 pi k/32, exact on the axes

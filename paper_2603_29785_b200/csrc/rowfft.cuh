@@ -19,13 +19,21 @@ template <int LOG2G, int DIR> struct RowFFT {
   static constexpr int F = 32 / G;
   static constexpr int M = 32 * G;
 
-  static __device__ __forceinline__ void run(float2 (&v)[32], float2 *ex, const float2 *tw1, int lane) {
+  static __device__ __forceinline__ float2 twmulx(float2 a, float4 w) { return pcmul4(a, w); }
+  static __device__ __forceinline__ float2 twmulx(float2 a, float2 w) { return pcmul(a, w); }
+  static __device__ __forceinline__ float scale_of(float4 w) { return w.x; }
+  static __device__ __forceinline__ float scale_of(float2 w) { return w.x; }
+
+  // tw1: [n1][t] entries of w_M^{dir t n1} x scale, in shared or global memory; either plain float2
+  // (wx, wy) or pre-duplicated float4 (wx, wx, wy, wy) that needs no pair-building moves
+  template <typename TW>
+  static __device__ __forceinline__ void run(float2 (&v)[32], float2 *ex, const TW *tw1, int lane) {
     const int t = lane & (G - 1), rw = lane >> LOG2G;
     RegFFT<32, DIR>::run(v);
     if constexpr (G > 1) {
       float2 *exw = ex + rw * (G * kExPitch) + t * kExPitch;
 #pragma unroll
-      for (int n1 = 0; n1 < 32; ++n1) exw[n1] = pcmul(v[n1], tw1[n1 * G + t]);
+      for (int n1 = 0; n1 < 32; ++n1) exw[n1] = twmulx(v[n1], tw1[n1 * G + t]);
       __syncwarp();
       const float2 *exr = ex + rw * (G * kExPitch) + t;
 #pragma unroll
@@ -41,7 +49,7 @@ template <int LOG2G, int DIR> struct RowFFT {
     } else {
       // M = 32: one thread per row, only the scale remains
 #pragma unroll
-      for (int n1 = 0; n1 < 32; ++n1) v[n1] = pscale(v[n1], tw1[0].x);
+      for (int n1 = 0; n1 < 32; ++n1) v[n1] = pscale(v[n1], scale_of(tw1[0]));
     }
   }
 };
