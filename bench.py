@@ -27,7 +27,7 @@ if ROOT not in sys.path:
 
 import numpy as np  # noqa: E402
 
-from paper_2603_29785_b200 import inputs  # noqa: E402
+from paper_2603_29785_b200 import dist_utils, inputs  # noqa: E402
 
 METRIC = "QTAM fwd+inv input samples/s"
 UNIT = "samples/s"
@@ -234,7 +234,8 @@ def run_ours(args):
     cdt = torch.complex128 if dtype == "f64" else torch.complex64
 
     # each rank gets its own segments (weak scaling, no collective on the data path)
-    x_np = inputs.make_batch(args.workload, batch=batch, first_segment=rank * batch)
+    first, _ = dist_utils.shard_segments(rank, world, batch)
+    x_np = inputs.make_batch(args.workload, batch=batch, first_segment=first)
     x_pin = torch.from_numpy(x_np).pin_memory()
     d_x = x_pin.to(dev)
     d_coef = torch.empty((batch, plan.ctot), dtype=cdt, device=dev)
@@ -316,13 +317,10 @@ def run_ours(args):
     d2h = (out_pin.numel() * out_pin.element_size()) if "inverse" in calls else (coef_pin.numel() * coef_pin.element_size())
 
     # ---- max over ranks
-    t = torch.tensor([ms_total, ms_plain, ms_e2e], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    ms_total, ms_plain, ms_e2e = (float(v) for v in t.tolist())
+    ms_total, ms_plain, ms_e2e = dist_utils.max_over_ranks([ms_total, ms_plain, ms_e2e], device=dev)
     ms_step = ms_total / args.steps
     units = world * batch * N
-    value = units / (ms_step * 1e-3)
+    value = dist_utils.aggregate_throughput(world, batch, N, ms_step)
 
     # ---- round-trip error against Pi_C x (verification outside the timed region; torch.fft is
     # used here only to build the projection, never on the product path)
