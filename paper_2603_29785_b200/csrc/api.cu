@@ -44,7 +44,7 @@ void free_plan(qtam_plan *p) {
   cudaFree(p->d_csr_ptr); cudaFree(p->d_csr_idx);
   for (int c = 0; c < qtam_plan::kClasses; ++c) cudaFree(p->d_items[c]);
   cudaFree(p->d_bigrows); cudaFree(p->d_spec_alloc); cudaFree(p->d_ws); cudaFree(p->d_band);
-  cudaFree(p->d_fwin2);
+  cudaFree(p->d_fwinp); cudaFree(p->d_red);
   cudaFree(p->d_frows); cudaFree(p->d_fwin); cudaFree(p->d_ftw_fwd); cudaFree(p->d_ftw_inv);
   cudaFree(p->d_tiny);
   for (ProfRec &r : p->prof_pool) { cudaEventDestroy(r.e0); cudaEventDestroy(r.e1); }
@@ -91,23 +91,21 @@ qtam_status build_fast(qtam_plan *p) {
     seen.push_back({h.dk, off});
     return off;
   };
-  // the same windows as (w,w) pairs, zero-padded to the M points of the row's short FFT and stored at
-  // the M-array index (j mod M): the fast gather multiplies without testing the support
-  std::vector<float> fwin2;
+  // the same windows zero-padded to the M points of the row's short FFT and stored at the M-array
+  // index (j mod M): the fast gather multiplies without testing the support
+  std::vector<float> fwinp;
   std::vector<std::pair<int64_t, int>> seen2;
   auto wpad_of = [&](const HostRow &h) -> int {
     for (auto &e : seen2) if (e.first == h.dk) return e.second;
-    const int off = (int)(fwin2.size() / 2);
-    fwin2.resize(fwin2.size() + 2 * (size_t)h.M, 0.0f);
-    for (int64_t jj = -h.dk; jj <= h.dk; ++jj) {
-      const int64_t j = (jj + h.M) % h.M;
-      const float w = (float)hp.win[(size_t)(h.woff + jj + h.dk)];
-      fwin2[2 * (size_t)(off + j)] = w; fwin2[2 * (size_t)(off + j) + 1] = w;
-    }
+    const int off = (int)fwinp.size();
+    fwinp.resize(fwinp.size() + (size_t)h.M, 0.0f);
+    for (int64_t jj = -h.dk; jj <= h.dk; ++jj)
+      fwinp[(size_t)(off + (jj + h.M) % h.M)] = (float)hp.win[(size_t)(h.woff + jj + h.dk)];
     seen2.push_back({h.dk, off});
     return off;
   };
   std::vector<FastRow> frows;
+  std::vector<int4> red;
   std::vector<float> twf, twi;   // (wx, wx, wy, wy) per entry
   const long double tau = 6.283185307179586476925286766559005768L;
   for (int lg = 5; lg >= 0; --lg) {
@@ -121,6 +119,11 @@ qtam_status build_fast(qtam_plan *p) {
       r.kc = (int)h.kc; r.dk = (int)h.dk; r.woff = window_of(h); r.goff = (int)h.goff;
       r.offset = (int)h.offset; r.plane = h.plane; r.wpad = wpad_of(h);
       frows.push_back(r);
+      {
+        const int64_t lo = h.kc - h.dk;
+        const int64_t jb = lo < 0 ? -lo : 0, je = std::min<int64_t>(h.L, hp.nb - lo);
+        red.push_back(make_int4((int)(lo + jb), (int)std::max<int64_t>(je - jb, 0), (int)jb, h.plane));
+      }
       F.sum_M += (double)h.M; F.sum_L += (double)h.L;
     }
     B.nrows = (int)frows.size() - B.row_base;
@@ -164,8 +167,9 @@ qtam_status build_fast(qtam_plan *p) {
   float *d = nullptr;
   if (!upload(&d, fwin.data(), fwin.size(), tot)) return QTAM_ERR_ALLOC;
   p->d_fwin = d;
-  if (!upload(&d, fwin2.data(), fwin2.size(), tot)) return QTAM_ERR_ALLOC;
-  p->d_fwin2 = d;
+  if (!upload(&d, fwinp.data(), fwinp.size(), tot)) return QTAM_ERR_ALLOC;
+  p->d_fwinp = d;
+  if (!upload(&p->d_red, red.data(), red.size(), tot)) return QTAM_ERR_ALLOC;
   if (!upload(&d, twf.data(), twf.size(), tot)) return QTAM_ERR_ALLOC;
   p->d_ftw_fwd = d;
   if (!upload(&d, twi.data(), twi.size(), tot)) return QTAM_ERR_ALLOC;

@@ -14,6 +14,9 @@ template <int LOG2NC, int NT> struct CtaFftRadix;
 template <> struct CtaFftRadix<11, 128> { static constexpr int R0 = 16, R1 = 16, R2 = 8; };
 template <> struct CtaFftRadix<11, 256> { static constexpr int R0 = 16, R1 = 16, R2 = 8; };
 template <> struct CtaFftRadix<11, 512> { static constexpr int R0 = 16, R1 = 16, R2 = 8; };
+template <> struct CtaFftRadix<11, 384> { static constexpr int R0 = 16, R1 = 16, R2 = 8; };
+template <> struct CtaFftRadix<12, 384> { static constexpr int R0 = 16, R1 = 16, R2 = 16; };
+template <> struct CtaFftRadix<13, 384> { static constexpr int R0 = 16, R1 = 16, R2 = 32; };
 template <> struct CtaFftRadix<12, 256> { static constexpr int R0 = 16, R1 = 16, R2 = 16; };
 template <> struct CtaFftRadix<12, 512> { static constexpr int R0 = 16, R1 = 16, R2 = 16; };
 template <> struct CtaFftRadix<13, 256> { static constexpr int R0 = 32, R1 = 16, R2 = 16; };

@@ -66,7 +66,8 @@ struct qtam_plan {
   qtam::FastParams fast{};
   qtam::FastRow *d_frows = nullptr;
   void *d_fwin = nullptr;      // float windows, one per distinct half-width
-  void *d_fwin2 = nullptr;     // float2 (w,w) windows zero-padded to M points in M-array order (index j mod M)
+  void *d_fwinp = nullptr;     // float windows zero-padded to M points in M-array order (index j mod M)
+  int4 *d_red = nullptr;       // per fast row (frows order): first bin, bins, first band index (R8 clip), plane
   void *d_spec_alloc = nullptr;   // allocation behind d_spec (zero pads of kSpecPad bins on both sides)
   void *d_ftw_fwd = nullptr;   // float2 pass-1 twiddles [bucket][n1][t], forward (x (N M)^-1/2)
   void *d_ftw_inv = nullptr;   // same, inverse (conjugate, x sqrt(N/M))

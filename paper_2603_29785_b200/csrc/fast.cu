@@ -65,7 +65,7 @@ template <int LOG2G>
 __device__ QTAM_GROUP_INLINE void fwd_group(const FastBucket &B, const FastRow *__restrict__ frows, int seg, int grp,
                                        int lane, float2 *ex, const float4 *tw1,
                                        const float2 *__restrict__ spec, long long xstride,
-                                       const float2 *__restrict__ fwin2, float2 *__restrict__ coef,
+                                       const float *__restrict__ fwinp, float2 *__restrict__ coef,
                                        long long ctot) {
   constexpr int G = 1 << LOG2G, F = 32 / G, M = 32 * G;
   const int t = lane & (G - 1), rw = lane >> LOG2G;
@@ -76,12 +76,14 @@ __device__ QTAM_GROUP_INLINE void fwd_group(const FastBucket &B, const FastRow *
   // B_k[j] = X[kc + jj(j)] * Wpad[j]: the window table is zero outside the support and the spectrum
   // buffer has zero pads, so neither the support (A9) nor the clipping at DC / Nyquist (R8) needs a test
   const float2 *X = spec + (size_t)seg * xstride + row.kc + t;
-  const float2 *W = fwin2 + row.wpad + t;
+  const float *W = fwinp + row.wpad + t;
   float2 v[32];
 #pragma unroll
   for (int j1 = 0; j1 < 32; ++j1) {
     const int jj = (j1 < 16) ? (G * j1) : (G * j1 - M);     // signed offset from the centre (R6), minus t
-    v[j1] = pmul(X[jj], W[G * j1]);
+    const float2 xv = X[jj];
+    const float w = W[G * j1];
+    v[j1] = make_float2(xv.x * w, xv.y * w);
   }
   RowFFT<LOG2G, +1>::run(v, ex, tw1, lane);
   if (valid) {
@@ -132,7 +134,7 @@ __device__ QTAM_GROUP_INLINE void inv_group(const FastBucket &B, const FastRow *
 template <int NWARPS, bool FORWARD>
 __global__ void __launch_bounds__(NWARPS * 32, NWARPS <= 8 ? 2 : 1)
 k_rows_fast(FastParams P, const FastRow *__restrict__ frows, const void *__restrict__ tw1g_,
-            const float *__restrict__ fwin, const float2 *__restrict__ fwin2,
+            const float *__restrict__ fwin, const float *__restrict__ fwinp,
             const float2 *__restrict__ spec, long long xstride, int nbins,
             float2 *__restrict__ coef, long long ctot, float2 *__restrict__ band, long long sumL,
             int batch, int plane) {
@@ -161,7 +163,7 @@ k_rows_fast(FastParams P, const FastRow *__restrict__ frows, const void *__restr
     const TW *tw1 = tw1s + B.tw_base;
 #define QTAM_ROW_CASE(L)                                                                              \
   case L:                                                                                             \
-    if constexpr (FORWARD) fwd_group<L>(B, frows, seg, grp, lane, ex, tw1, spec, xstride, fwin2, coef, ctot); \
+    if constexpr (FORWARD) fwd_group<L>(B, frows, seg, grp, lane, ex, tw1, spec, xstride, fwinp, coef, ctot); \
     else inv_group<L>(B, frows, seg, grp, lane, ex, tw1, coef, ctot, nbins, fwin, band, sumL, plane);  \
     break;
     switch (B.log2G) {
@@ -267,7 +269,7 @@ static qtam_status rows_launch_nw(qtam_plan *p, int batch, const void *d_coef_in
     LaunchScope ls(p, st, FORWARD ? K_FWD_ROWS_FAST : K_INV_ROWS_FAST, bytes);
     kern<<<grid, NW * 32, smem, st>>>(
         P, p->d_frows, static_cast<const void *>(FORWARD ? p->d_ftw_fwd : p->d_ftw_inv),
-        static_cast<const float *>(p->d_fwin), static_cast<const float2 *>(p->d_fwin2),
+        static_cast<const float *>(p->d_fwin), static_cast<const float *>(p->d_fwinp),
         static_cast<const float2 *>(p->d_spec), p->xstride,
         (int)p->hp.nb,
         FORWARD ? static_cast<float2 *>(d_coef_out) : const_cast<float2 *>(static_cast<const float2 *>(d_coef_in)),

@@ -32,7 +32,7 @@ struct RoundRow { int lo, L, stage, active; };   // band start bin, length, offs
 template <int LOG2G>
 __device__ __noinline__ void inv_stage(const FastBucket &B, const FastRow *__restrict__ frows, int base, int warp,
                                        int lane, float2 *ex, const float2 *__restrict__ tw1,
-                                       const float2 *__restrict__ Yseg, const float2 *__restrict__ fwin2,
+                                       const float2 *__restrict__ Yseg, const float *__restrict__ fwinp,
                                        int plane) {
   constexpr int G = 1 << LOG2G, F = 32 / G, M = 32 * G;
   const int t = lane & (G - 1), rw = lane >> LOG2G;
@@ -50,14 +50,14 @@ __device__ __noinline__ void inv_stage(const FastBucket &B, const FastRow *__res
     // windowed band values G_k[jj] = Bhat_k[jj] W_k[jj] in natural bin order jj = -dk..dk; the window
     // table is stored at the M-array index, the same index the FFT output has
     float2 *stage = ex + rw * M + row.dk;
-    const float2 *W = fwin2 + row.wpad + t;
+    const float *W = fwinp + row.wpad + t;
 #pragma unroll
     for (int i = 0; i < F; ++i)
 #pragma unroll
       for (int n2 = 0; n2 < G; ++n2) {
         const int j = (t + G * i) + 32 * n2;
         const int jj = (G == 1) ? (j < 16 ? j : j - M) : (n2 < G / 2 ? j : j - M);
-        if (jj <= row.dk && jj >= -row.dk) stage[jj] = pmul(v[i * G + n2], W[G * i + 32 * n2]);
+        if (jj <= row.dk && jj >= -row.dk) stage[jj] = pscale(v[i * G + n2], W[G * i + 32 * n2]);
       }
   }
 }
@@ -65,7 +65,7 @@ __device__ __noinline__ void inv_stage(const FastBucket &B, const FastRow *__res
 template <int LOG2NC, int NW>
 __global__ void __launch_bounds__(NW * 32, NW <= 8 ? 2 : 1)
 k_inv_fused(FastParams P, const FastRow *__restrict__ frows, const FastRow *__restrict__ tiny, int n_tiny,
-            const float2 *__restrict__ tw1g, const float *__restrict__ fwin, const float2 *__restrict__ fwin2,
+            const float2 *__restrict__ tw1g, const float *__restrict__ fwin, const float *__restrict__ fwinp,
             const float2 *__restrict__ coef,
             long long ctot, const float *__restrict__ invP, int nbins, int plane,
             const float2 *__restrict__ tw, int log2twn, float *__restrict__ x_out) {
@@ -96,12 +96,12 @@ k_inv_fused(FastParams P, const FastRow *__restrict__ frows, const FastRow *__re
       }
       const float2 *tw1 = tw1g + B.tw_base;
       switch (B.log2G) {
-        case 5: inv_stage<5>(B, frows, base, warp, lane, ex, tw1, Yseg, fwin2, plane); break;
-        case 4: inv_stage<4>(B, frows, base, warp, lane, ex, tw1, Yseg, fwin2, plane); break;
-        case 3: inv_stage<3>(B, frows, base, warp, lane, ex, tw1, Yseg, fwin2, plane); break;
-        case 2: inv_stage<2>(B, frows, base, warp, lane, ex, tw1, Yseg, fwin2, plane); break;
-        case 1: inv_stage<1>(B, frows, base, warp, lane, ex, tw1, Yseg, fwin2, plane); break;
-        default: inv_stage<0>(B, frows, base, warp, lane, ex, tw1, Yseg, fwin2, plane); break;
+        case 5: inv_stage<5>(B, frows, base, warp, lane, ex, tw1, Yseg, fwinp, plane); break;
+        case 4: inv_stage<4>(B, frows, base, warp, lane, ex, tw1, Yseg, fwinp, plane); break;
+        case 3: inv_stage<3>(B, frows, base, warp, lane, ex, tw1, Yseg, fwinp, plane); break;
+        case 2: inv_stage<2>(B, frows, base, warp, lane, ex, tw1, Yseg, fwinp, plane); break;
+        case 1: inv_stage<1>(B, frows, base, warp, lane, ex, tw1, Yseg, fwinp, plane); break;
+        default: inv_stage<0>(B, frows, base, warp, lane, ex, tw1, Yseg, fwinp, plane); break;
       }
       __syncthreads();
       for (int s = 0; s < nr; ++s) {
@@ -189,7 +189,7 @@ static qtam_status launch(qtam_plan *p, const void *d_coef, int batch, int plane
     LaunchScope ls(p, st, K_INV_FUSED, (double)batch * (8.0 * (double)p->hp.ctot + 4.0 * (double)p->hp.N));
     kern<<<batch, NW * 32, smem, st>>>(
         p->fast, p->d_frows, p->d_tiny, p->n_tiny, static_cast<const float2 *>(p->d_ftw_inv),
-        static_cast<const float *>(p->d_fwin), static_cast<const float2 *>(p->d_fwin2),
+        static_cast<const float *>(p->d_fwin), static_cast<const float *>(p->d_fwinp),
         static_cast<const float2 *>(d_coef), p->hp.ctot,
         static_cast<const float *>(p->d_invP), (int)p->hp.nb, plane, static_cast<const float2 *>(p->d_tw),
         ilog2(p->twn), static_cast<float *>(d_x_out));
