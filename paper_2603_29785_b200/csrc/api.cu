@@ -47,6 +47,7 @@ void free_plan(qtam_plan *p) {
   cudaFree(p->d_fwinp); cudaFree(p->d_red);
   cudaFree(p->d_frows); cudaFree(p->d_fwin); cudaFree(p->d_ftw_fwd); cudaFree(p->d_ftw_inv);
   cudaFree(p->d_tiny);
+  cudaFree(p->d_trows); cudaFree(p->d_titems); cudaFree(p->d_part); cudaFree(p->d_counter);
   for (ProfRec &r : p->prof_pool) { cudaEventDestroy(r.e0); cudaEventDestroy(r.e1); }
   delete p;
 }
@@ -164,6 +165,7 @@ qtam_status build_fast(qtam_plan *p) {
   }
   if (hp.ctot >= (int64_t(1) << 31)) return QTAM_ERR_UNSUPPORTED;
   if (!upload(&p->d_frows, frows.data(), frows.size(), tot)) return QTAM_ERR_ALLOC;
+  p->h_frows = frows;
   float *d = nullptr;
   if (!upload(&d, fwin.data(), fwin.size(), tot)) return QTAM_ERR_ALLOC;
   p->d_fwin = d;
@@ -302,6 +304,7 @@ qtam_status qtam_plan_create(qtam_plan **out, double fs, int64_t N, const double
   }
   s = dtype == QTAM_F32 ? build_device<float>(p) : build_device<double>(p);
   if (s == QTAM_OK && p->fast_rows) s = build_fast(p);
+  if (s == QTAM_OK && p->fast_rows) s = build_inv_tiled(p);
   if (s != QTAM_OK) { free_plan(p); cudaGetLastError(); return s; }
   if (cudaDeviceSynchronize() != cudaSuccess) { free_plan(p); return QTAM_ERR_CUDA; }
   *out = p;
@@ -389,6 +392,7 @@ qtam_status qtam_inverse(qtam_plan *p, const void *d_coef, int batch, int plane,
   p->last_launches = 0;
   if (batch == 0) return QTAM_OK;
   cudaStream_t st = static_cast<cudaStream_t>(stream);
+  if (p->tiled_inv) return tiled_inverse(p, d_coef, batch, plane, d_x_out, st);
   if (p->fused_inv) return fused_inverse(p, d_coef, batch, plane, d_x_out, st);
   qtam_status s = QTAM_OK;
   if (p->fast_rows) {
@@ -430,7 +434,7 @@ int qtam_last_launch_count(const qtam_plan *p) { return p ? p->last_launches : 0
 static const char *const kKernelNames[K_COUNT] = {
     "cfft_seq", "cfft_cols", "cfft_rows", "r2c_post", "c2r_pre", "fwd_rows", "fwd_combine",
     "inv_rows", "inv_reduce", "dense_place", "threshold", "r2c_fast", "fwd_rows_fast", "inv_rows_fast",
-    "reduce_c2r_fast", "inv_fused"};
+    "reduce_c2r_fast", "inv_fused", "inv_tiles", "combine_c2r"};
 
 qtam_status qtam_profile_enable(qtam_plan *p, int on, int max_launches) {
   if (!p || p->host_only) return QTAM_ERR_INVALID_ARG;

@@ -12,7 +12,7 @@ namespace qtam {
 enum KernelId {
   K_CFFT_SEQ = 0, K_CFFT_COLS, K_CFFT_ROWS, K_R2C_POST, K_C2R_PRE, K_FWD_ROWS, K_FWD_COMBINE,
   K_INV_ROWS, K_INV_REDUCE, K_DENSE_PLACE, K_THRESHOLD, K_R2C_FAST, K_FWD_ROWS_FAST, K_INV_ROWS_FAST,
-  K_REDUCE_C2R_FAST, K_INV_FUSED, K_COUNT
+  K_REDUCE_C2R_FAST, K_INV_FUSED, K_INV_TILES, K_COMBINE_C2R, K_COUNT
 };
 // fast float path (fast.cu): rows with 32 <= M <= 1024, grouped by G = M/32 lanes per row
 struct FastRow { int kc, dk, woff, goff, offset, plane, wpad, pad; };   // wpad: offset into the padded window table
@@ -22,6 +22,11 @@ struct FastParams {
   double sum_M, sum_L;          // coefficients / band values per segment the fast rows cover
   FastBucket b[6];
 };
+// tiled inverse (inv_tiled.cu): a work item = consecutive rows (sorted by centre bin) of one length bucket
+// whose bands fit one warp-private accumulator of kAccBins bins
+struct __align__(16) TileRow { int kc, offset, wpad, jlo, jhi, plane, pad0, pad1; };   // jlo..jhi: band offsets kept (R8 clip)
+struct __align__(16) TileItem { int row0, nrows, log2G, tw_base, lo, nb, part_off, npass; };
+constexpr int kAccBins = 1280;
 struct ProfRec { int kid; double bytes; cudaEvent_t e0, e1; };
 }  // namespace qtam
 
@@ -74,6 +79,15 @@ struct qtam_plan {
   qtam::FastRow *d_tiny = nullptr;   // rows shorter than 32 points (goff holds log2 M), for fused_inv.cu
   int n_tiny = 0;
   bool fused_inv = false;      // the whole inverse runs in one kernel (fused_inv.cu)
+  // tiled inverse (inv_tiled.cu)
+  std::vector<qtam::FastRow> h_frows;   // host copy of d_frows (bucket-major), for build_inv_tiled
+  bool tiled_inv = false;
+  qtam::TileRow *d_trows = nullptr;
+  qtam::TileItem *d_titems = nullptr;
+  int n_titems = 0;
+  int64_t part_stride = 0;     // partial sums per segment (complex elements)
+  void *d_part = nullptr;      // complex[max_batch][part_stride]
+  unsigned int *d_counter = nullptr;   // work counter of the persistent tile kernel
 
   int last_launches = 0;
   // launch profile (qtam_profile_enable / qtam_profile_read)
@@ -116,6 +130,9 @@ qtam_status fast_r2c(qtam_plan *p, const void *d_x, int batch, cudaStream_t st);
 qtam_status fast_forward_rows(qtam_plan *p, int batch, void *d_coef, cudaStream_t st);
 qtam_status fast_inverse_rows(qtam_plan *p, const void *d_coef, int batch, int plane, cudaStream_t st);
 qtam_status fast_reduce_c2r(qtam_plan *p, int batch, int plane, void *d_x_out, cudaStream_t st);
+// inv_tiled.cu
+qtam_status build_inv_tiled(qtam_plan *p);
+qtam_status tiled_inverse(qtam_plan *p, const void *d_coef, int batch, int plane, void *d_x_out, cudaStream_t st);
 // fused_inv.cu
 qtam_status fused_inverse(qtam_plan *p, const void *d_coef, int batch, int plane, void *d_x_out, cudaStream_t st);
 
