@@ -47,6 +47,7 @@ void free_plan(qtam_plan *p) {
   cudaFree(p->d_fwinp); cudaFree(p->d_red);
   cudaFree(p->d_frows); cudaFree(p->d_fwin); cudaFree(p->d_ftw_fwd); cudaFree(p->d_ftw_inv);
   cudaFree(p->d_tiny);
+  cudaFree(p->d_thr_tasks); cudaFree(p->d_thr_offs);
   cudaFree(p->d_trows); cudaFree(p->d_titems); cudaFree(p->d_part); cudaFree(p->d_counter);
   for (ProfRec &r : p->prof_pool) { cudaEventDestroy(r.e0); cudaEventDestroy(r.e1); }
   delete p;
@@ -303,6 +304,7 @@ qtam_status qtam_plan_create(qtam_plan **out, double fs, int64_t N, const double
     p->fast_long = dtype == QTAM_F32 && lnc >= 11 && lnc <= 14;
   }
   s = dtype == QTAM_F32 ? build_device<float>(p) : build_device<double>(p);
+  if (s == QTAM_OK) s = build_thr_fast(p);
   if (s == QTAM_OK && p->fast_rows) s = build_fast(p);
   if (s == QTAM_OK && p->fast_rows) s = build_inv_tiled(p);
   if (s != QTAM_OK) { free_plan(p); cudaGetLastError(); return s; }
@@ -426,7 +428,10 @@ qtam_status qtam_threshold_rowmedian(qtam_plan *p, void *d_coef, int batch, doub
   if (!check_call(p, d_coef, d_coef, batch) || !(kappa >= 0.0)) return QTAM_ERR_INVALID_ARG;
   p->last_launches = 0;
   if (batch == 0) return QTAM_OK;
-  return generic_threshold(p, d_coef, batch, kappa, static_cast<cudaStream_t>(stream));
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  const qtam_status s = fast_threshold(p, d_coef, batch, kappa, st);
+  if (s != QTAM_OK || !p->thr_has_big) return s;
+  return generic_threshold(p, d_coef, batch, kappa, p->n_thr_tasks > 0 ? kThrFastLog2Max + 1 : 0, st);
 }
 
 int qtam_last_launch_count(const qtam_plan *p) { return p ? p->last_launches : 0; }
@@ -434,7 +439,7 @@ int qtam_last_launch_count(const qtam_plan *p) { return p ? p->last_launches : 0
 static const char *const kKernelNames[K_COUNT] = {
     "cfft_seq", "cfft_cols", "cfft_rows", "r2c_post", "c2r_pre", "fwd_rows", "fwd_combine",
     "inv_rows", "inv_reduce", "dense_place", "threshold", "r2c_fast", "fwd_rows_fast", "inv_rows_fast",
-    "reduce_c2r_fast", "inv_fused", "inv_tiles", "combine_c2r"};
+    "reduce_c2r_fast", "inv_fused", "inv_tiles", "combine_c2r", "threshold_fast"};
 
 qtam_status qtam_profile_enable(qtam_plan *p, int on, int max_launches) {
   if (!p || p->host_only) return QTAM_ERR_INVALID_ARG;

@@ -12,7 +12,7 @@ namespace qtam {
 enum KernelId {
   K_CFFT_SEQ = 0, K_CFFT_COLS, K_CFFT_ROWS, K_R2C_POST, K_C2R_PRE, K_FWD_ROWS, K_FWD_COMBINE,
   K_INV_ROWS, K_INV_REDUCE, K_DENSE_PLACE, K_THRESHOLD, K_R2C_FAST, K_FWD_ROWS_FAST, K_INV_ROWS_FAST,
-  K_REDUCE_C2R_FAST, K_INV_FUSED, K_INV_TILES, K_COMBINE_C2R, K_COUNT
+  K_REDUCE_C2R_FAST, K_INV_FUSED, K_INV_TILES, K_COMBINE_C2R, K_THRESHOLD_FAST, K_COUNT
 };
 // fast float path (fast.cu): rows with 32 <= M <= 1024, grouped by G = M/32 lanes per row
 struct FastRow { int kc, dk, woff, goff, offset, plane, wpad, pad; };   // wpad: offset into the padded window table
@@ -27,6 +27,9 @@ struct FastParams {
 struct __align__(16) TileRow { int kc, offset, wpad, jlo, jhi, plane, pad0, pad1; };   // jlo..jhi: band offsets kept (R8 clip)
 struct __align__(16) TileItem { int row0, nrows, log2G, tw_base, lo, nb, part_off, npass; };
 constexpr int kAccBins = 1280;
+// fast threshold (threshold_fast.cu): a warp task = up to 32/G rows of one length M = 32 G (or 32 rows of M < 32)
+struct ThrTask { int log2M, row0, nrows, pad; };
+constexpr int kThrFastLog2Max = 10;
 struct ProfRec { int kid; double bytes; cudaEvent_t e0, e1; };
 }  // namespace qtam
 
@@ -89,6 +92,12 @@ struct qtam_plan {
   void *d_part = nullptr;      // complex[max_batch][part_stride]
   unsigned int *d_counter = nullptr;   // work counter of the persistent tile kernel
 
+  // fast threshold (threshold_fast.cu)
+  qtam::ThrTask *d_thr_tasks = nullptr;
+  int *d_thr_offs = nullptr;      // coefficient offsets of the tasks' rows
+  int n_thr_tasks = 0;
+  bool thr_has_big = false;       // some row is longer than 2^kThrFastLog2Max points (generic kernel)
+
   int last_launches = 0;
   // launch profile (qtam_profile_enable / qtam_profile_read)
   bool prof_on = false;
@@ -123,13 +132,16 @@ qtam_status generic_inverse_rows(qtam_plan *p, const void *d_coef, int batch, in
 qtam_status generic_inverse_reduce(qtam_plan *p, int batch, int plane, cudaStream_t st);
 qtam_status generic_c2r(qtam_plan *p, int batch, void *d_x_out, cudaStream_t st);
 qtam_status generic_dense(qtam_plan *p, int batch, int row_begin, int row_end, void *d_out, cudaStream_t st);
-qtam_status generic_threshold(qtam_plan *p, void *d_coef, int batch, double kappa, cudaStream_t st);
+qtam_status generic_threshold(qtam_plan *p, void *d_coef, int batch, double kappa, int min_log2M, cudaStream_t st);
 
 // fast.cu
 qtam_status fast_r2c(qtam_plan *p, const void *d_x, int batch, cudaStream_t st);
 qtam_status fast_forward_rows(qtam_plan *p, int batch, void *d_coef, cudaStream_t st);
 qtam_status fast_inverse_rows(qtam_plan *p, const void *d_coef, int batch, int plane, cudaStream_t st);
 qtam_status fast_reduce_c2r(qtam_plan *p, int batch, int plane, void *d_x_out, cudaStream_t st);
+// threshold_fast.cu
+qtam_status build_thr_fast(qtam_plan *p);
+qtam_status fast_threshold(qtam_plan *p, void *d_coef, int batch, double kappa, cudaStream_t st);
 // inv_tiled.cu
 qtam_status build_inv_tiled(qtam_plan *p);
 qtam_status tiled_inverse(qtam_plan *p, const void *d_coef, int batch, int plane, void *d_x_out, cudaStream_t st);

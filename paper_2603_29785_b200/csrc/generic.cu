@@ -14,6 +14,7 @@
 
 #include "cplx.cuh"
 #include "device_plan.hpp"
+#include "thrbits.cuh"
 
 namespace qtam {
 
@@ -328,28 +329,6 @@ __global__ void k_dense_place(const RowDev *__restrict__ rows, int row, const C2
 // magnitudes; every operation correctly rounded in T, no fused multiply-add (DESIGN.md "threshold
 // arithmetic"), so the decisions equal the oracle's bit for bit on identical inputs.
 // ---------------------------------------------------------------------------------------------------
-template <typename T> struct Bits;
-template <> struct Bits<float> {
-  typedef unsigned int U; static const int nbits = 32;
-  static __device__ __forceinline__ U of(float v) { return __float_as_uint(v); }
-  static __device__ __forceinline__ float from(U u) { return __uint_as_float(u); }
-  static __device__ __forceinline__ float mag(float re, float im) {
-    return __fsqrt_rn(__fadd_rn(__fmul_rn(re, re), __fmul_rn(im, im)));
-  }
-  static __device__ __forceinline__ float mul(float a, float b) { return __fmul_rn(a, b); }
-  static __device__ __forceinline__ float add(float a, float b) { return __fadd_rn(a, b); }
-};
-template <> struct Bits<double> {
-  typedef unsigned long long U; static const int nbits = 64;
-  static __device__ __forceinline__ U of(double v) { return (U)__double_as_longlong(v); }
-  static __device__ __forceinline__ double from(U u) { return __longlong_as_double((long long)u); }
-  static __device__ __forceinline__ double mag(double re, double im) {
-    return __dsqrt_rn(__dadd_rn(__dmul_rn(re, re), __dmul_rn(im, im)));
-  }
-  static __device__ __forceinline__ double mul(double a, double b) { return __dmul_rn(a, b); }
-  static __device__ __forceinline__ double add(double a, double b) { return __dadd_rn(a, b); }
-};
-
 __device__ __forceinline__ int block_sum(int v, int *sm) {
   for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
   const int w = threadIdx.x >> 5, nw = (blockDim.x + 31) >> 5;
@@ -363,13 +342,14 @@ __device__ __forceinline__ int block_sum(int v, int *sm) {
 
 template <typename T>
 __global__ void k_threshold(const RowDev *__restrict__ rows, C2<T> *__restrict__ coef, long long ctot,
-                            T kappa, int cache_pts) {
+                            T kappa, int cache_pts, int min_log2M) {
   typedef C2<T> V;
   typedef typename Bits<T>::U U;
   __shared__ int red[32];
   __shared__ U red_min[32];
   T *cache = reinterpret_cast<T *>(qtam_smem);
   const RowDev r = rows[blockIdx.x];
+  if (r.log2M < min_log2M) return;   // shorter rows run in threshold_fast.cu
   V *Y = coef + (long long)blockIdx.y * ctot + r.offset;
   const int M = r.M;
   const bool cached = M <= cache_pts;
@@ -624,22 +604,22 @@ qtam_status generic_dense(qtam_plan *p, int batch, int row_begin, int row_end, v
 }
 
 template <typename T>
-static qtam_status threshold_t(qtam_plan *p, void *d_coef, int batch, double kappa, cudaStream_t st) {
+static qtam_status threshold_t(qtam_plan *p, void *d_coef, int batch, double kappa, int min_log2M, cudaStream_t st) {
   const int cache_pts = 8192;
   const size_t smem = sizeof(T) * (size_t)cache_pts;
   if (!set_smem(k_threshold<T>, smem)) return QTAM_ERR_CUDA;
   dim3 g((unsigned)p->hp.rows.size(), batch);
   {
     LaunchScope ls(p, st, K_THRESHOLD, 2.0 * sizeof(C2<T>) * (double)batch * (double)p->hp.ctot);
-    k_threshold<T><<<g, 256, smem, st>>>(p->d_rows, static_cast<C2<T> *>(d_coef), p->hp.ctot, (T)kappa, cache_pts);
+    k_threshold<T><<<g, 256, smem, st>>>(p->d_rows, static_cast<C2<T> *>(d_coef), p->hp.ctot, (T)kappa, cache_pts, min_log2M);
   }
   QTAM_LAUNCH_CHECK();
   return QTAM_OK;
 }
 
-qtam_status generic_threshold(qtam_plan *p, void *d_coef, int batch, double kappa, cudaStream_t st) {
-  return p->esz == 4 ? threshold_t<float>(p, d_coef, batch, kappa, st)
-                     : threshold_t<double>(p, d_coef, batch, kappa, st);
+qtam_status generic_threshold(qtam_plan *p, void *d_coef, int batch, double kappa, int min_log2M, cudaStream_t st) {
+  return p->esz == 4 ? threshold_t<float>(p, d_coef, batch, kappa, min_log2M, st)
+                     : threshold_t<double>(p, d_coef, batch, kappa, min_log2M, st);
 }
 
 }  // namespace qtam
