@@ -46,7 +46,7 @@ void free_plan(qtam_plan *p) {
   cudaFree(p->d_bigrows); cudaFree(p->d_spec_alloc); cudaFree(p->d_ws); cudaFree(p->d_band);
   cudaFree(p->d_fwinp); cudaFree(p->d_red);
   cudaFree(p->d_frows); cudaFree(p->d_fwin); cudaFree(p->d_ftw_fwd); cudaFree(p->d_ftw_inv);
-  cudaFree(p->d_tiny);
+  cudaFree(p->d_tiny); cudaFree(p->d_ptw);
   cudaFree(p->d_thr_tasks); cudaFree(p->d_thr_offs);
   cudaFree(p->d_trows); cudaFree(p->d_titems); cudaFree(p->d_part); cudaFree(p->d_counter);
   for (ProfRec &r : p->prof_pool) { cudaEventDestroy(r.e0); cudaEventDestroy(r.e1); }
@@ -145,12 +145,10 @@ qtam_status build_fast(qtam_plan *p) {
     F.b[F.nbuckets++] = B;
   }
   F.tw_total = (int)(twf.size() / 4);
-  // rows shorter than 32 points and the eligibility of the one-kernel inverse
+  // rows shorter than 32 points
   std::vector<FastRow> tiny;
-  bool has_long_rows = false;
   for (size_t k = 0; k < hp.rows.size(); ++k) {
     const HostRow &h = hp.rows[k];
-    if (h.M > 1024) has_long_rows = true;
     if (h.M >= 32) continue;
     FastRow r{};
     r.kc = (int)h.kc; r.dk = (int)h.dk; r.woff = window_of(h); r.goff = ilog2(h.M);
@@ -159,11 +157,6 @@ qtam_status build_fast(qtam_plan *p) {
   }
   p->n_tiny = (int)tiny.size();
   if (!upload(&p->d_tiny, tiny.data(), tiny.size(), tot)) return QTAM_ERR_ALLOC;
-  {
-    const int lnc = ilog2(hp.N) - 1;
-    p->fused_inv = p->fast_long && lnc <= 13 && !has_long_rows && p->n_tiny <= 256;
-    if (getenv("QTAM_NO_FUSED_INV")) p->fused_inv = false;
-  }
   if (hp.ctot >= (int64_t(1) << 31)) return QTAM_ERR_UNSUPPORTED;
   if (!upload(&p->d_frows, frows.data(), frows.size(), tot)) return QTAM_ERR_ALLOC;
   p->h_frows = frows;
@@ -306,6 +299,7 @@ qtam_status qtam_plan_create(qtam_plan **out, double fs, int64_t N, const double
   s = dtype == QTAM_F32 ? build_device<float>(p) : build_device<double>(p);
   if (s == QTAM_OK) s = build_thr_fast(p);
   if (s == QTAM_OK && p->fast_rows) s = build_fast(p);
+  if (s == QTAM_OK && p->fast_long) s = build_long_tables(p);
   if (s == QTAM_OK && p->fast_rows) s = build_inv_tiled(p);
   if (s != QTAM_OK) { free_plan(p); cudaGetLastError(); return s; }
   if (cudaDeviceSynchronize() != cudaSuccess) { free_plan(p); return QTAM_ERR_CUDA; }
@@ -395,7 +389,6 @@ qtam_status qtam_inverse(qtam_plan *p, const void *d_coef, int batch, int plane,
   if (batch == 0) return QTAM_OK;
   cudaStream_t st = static_cast<cudaStream_t>(stream);
   if (p->tiled_inv) return tiled_inverse(p, d_coef, batch, plane, d_x_out, st);
-  if (p->fused_inv) return fused_inverse(p, d_coef, batch, plane, d_x_out, st);
   qtam_status s = QTAM_OK;
   if (p->fast_rows) {
     s = fast_inverse_rows(p, d_coef, batch, plane, st);

@@ -5,6 +5,9 @@
 // in-register FFTs of fftreg.cuh.  Pass 1 writes with stride R, so it writes a skewed layout
 // phys(a) = a + (a >> log2 R1) that the second pass reads back; later passes use the natural layout.
 #pragma once
+#include <cmath>
+#include <vector>
+
 #include "fftreg.cuh"
 
 namespace qtam {
@@ -38,11 +41,10 @@ template <int LOG2NC> __host__ __device__ constexpr int cta_fft_smem_elems() {
 }
 
 // One Stockham pass.  IN_MODE / OUT_MODE: 0 natural smem, 1 skewed smem, 2 global (natural).
-// tw: global table e^{+2 pi i m/twn}, log2twn >= LOG2NC.
 template <int LOG2NC, int NT, int R, int LOG2NS, int DIR, int IN_MODE, int OUT_MODE, int SKEW>
 __device__ __forceinline__ void cta_fft_pass(float2 *s, const float2 *__restrict__ gin,
-                                             float2 *__restrict__ gout, const float2 *__restrict__ tw,
-                                             int log2twn, float out_scale) {
+                                             float2 *__restrict__ gout, const float2 *__restrict__ ptw,
+                                             float out_scale) {
   constexpr int NC = 1 << LOG2NC;
   constexpr int NBF = NC / R;                 // butterflies
   constexpr int BPT = (NBF + NT - 1) / NT;    // per thread
@@ -61,11 +63,24 @@ __device__ __forceinline__ void cta_fft_pass(float2 *s, const float2 *__restrict
       }
       if constexpr (LOG2NS > 0) {
         const int k = i & (NS - 1);
-        const int sh = log2twn - LOG2NS - ILog2<R>::value;   // w_{NS*R}^{k r} = tw[(k r) << sh]
+        // r = 4a + b: w_{NS R}^{kr} = w^{4ka} w^{kb} from R/4 - 1 + 3 table values and one product each.
+        // ptw: the pass's table [m][k] = e^{2 pi i k m/(NS R)}, m = 1, 2, 3, 4, 8, .. (coalesced over k)
+        constexpr int RA = R / 4;
+        float2 wb[4], wa[RA];
+#pragma unroll
+        for (int b = 1; b < 4; ++b) {
+          wb[b] = __ldg(ptw + (b - 1) * NS + k);
+          if (DIR < 0) wb[b].y = -wb[b].y;
+        }
+#pragma unroll
+        for (int a = 1; a < RA; ++a) {
+          wa[a] = __ldg(ptw + (2 + a) * NS + k);
+          if (DIR < 0) wa[a].y = -wa[a].y;
+        }
 #pragma unroll
         for (int r = 1; r < R; ++r) {
-          float2 w = __ldg(tw + ((size_t)(k * r) << sh));
-          if (DIR < 0) w.y = -w.y;
+          const int a = r >> 2, b = r & 3;
+          const float2 w = a == 0 ? wb[b] : (b == 0 ? wa[a] : pcmul(wa[a], wb[b]));
           v[u][r] = pcmul(v[u][r], w);
         }
       }
@@ -91,18 +106,50 @@ __device__ __forceinline__ void cta_fft_pass(float2 *s, const float2 *__restrict
   if constexpr (OUT_MODE != 2) __syncthreads();
 }
 
+// entries of the pass tables of one transform (passes 2 and 3), and the offset of pass 3's
+template <int LOG2NC, int NT> __host__ __device__ constexpr int cta_fft_ptw_off3() {
+  return (2 + CtaFftRadix<LOG2NC, NT>::R1 / 4) * CtaFftRadix<LOG2NC, NT>::R0;
+}
+template <int LOG2NC, int NT> __host__ __device__ constexpr int cta_fft_ptw_elems() {
+  return cta_fft_ptw_off3<LOG2NC, NT>() +
+         (2 + CtaFftRadix<LOG2NC, NT>::R2 / 4) * CtaFftRadix<LOG2NC, NT>::R0 * CtaFftRadix<LOG2NC, NT>::R1;
+}
+
+// host: the pass tables (interleaved re, im), long double evaluation with the index reduced mod the period
+template <int LOG2NC, int NT> inline void fill_cta_fft_tables(std::vector<float> &out) {
+  typedef CtaFftRadix<LOG2NC, NT> PL;
+  out.clear();
+  const long double tau = 6.283185307179586476925286766559005768L;
+  auto pass = [&](int R, int NS) {
+    const long long period = (long long)NS * R;
+    for (int row = 0; row < 2 + R / 4; ++row) {
+      const int m = row < 3 ? row + 1 : 4 * (row - 2);
+      for (int k = 0; k < NS; ++k) {
+        const long long e = ((long long)k * m) % period;
+        const long double a = tau * (long double)e / (long double)period;
+        out.push_back((float)cosl(a));
+        out.push_back((float)sinl(a));
+      }
+    }
+  };
+  pass(PL::R1, PL::R0);
+  pass(PL::R2, PL::R0 * PL::R1);
+}
+
 // Whole transform with NT threads (all threads of the CTA must call it).
 // FROM_GLOBAL: pass 1 reads gin (natural order) instead of s (natural layout).
 // TO_GLOBAL: the last pass writes gout (natural order, times out_scale) instead of s (natural layout).
+// ptw: the pass tables built by fill_cta_fft_tables (host) for this (LOG2NC, NT)'s radices.
 template <int LOG2NC, int NT, int DIR, bool FROM_GLOBAL, bool TO_GLOBAL>
 __device__ __forceinline__ void cta_fft(float2 *s, const float2 *__restrict__ gin, float2 *__restrict__ gout,
-                                        const float2 *__restrict__ tw, int log2twn, float out_scale) {
+                                        const float2 *__restrict__ ptw, float out_scale) {
   typedef CtaFftRadix<LOG2NC, NT> PL;
   constexpr int L0 = ILog2<PL::R0>::value, L1 = ILog2<PL::R1>::value;
   static_assert(L0 + L1 + ILog2<PL::R2>::value == LOG2NC, "radices must multiply to Nc");
-  cta_fft_pass<LOG2NC, NT, PL::R0, 0, DIR, FROM_GLOBAL ? 2 : 0, 1, L0>(s, gin, gout, tw, log2twn, 1.f);
-  cta_fft_pass<LOG2NC, NT, PL::R1, L0, DIR, 1, 0, L0>(s, gin, gout, tw, log2twn, 1.f);
-  cta_fft_pass<LOG2NC, NT, PL::R2, L0 + L1, DIR, 0, TO_GLOBAL ? 2 : 0, L0>(s, gin, gout, tw, log2twn, out_scale);
+  cta_fft_pass<LOG2NC, NT, PL::R0, 0, DIR, FROM_GLOBAL ? 2 : 0, 1, L0>(s, gin, gout, ptw, 1.f);
+  cta_fft_pass<LOG2NC, NT, PL::R1, L0, DIR, 1, 0, L0>(s, gin, gout, ptw, 1.f);
+  cta_fft_pass<LOG2NC, NT, PL::R2, L0 + L1, DIR, 0, TO_GLOBAL ? 2 : 0, L0>(
+      s, gin, gout, ptw + cta_fft_ptw_off3<LOG2NC, NT>(), out_scale);
 }
 
 }  // namespace qtam

@@ -79,9 +79,9 @@ struct qtam_plan {
   void *d_spec_alloc = nullptr;   // allocation behind d_spec (zero pads of kSpecPad bins on both sides)
   void *d_ftw_fwd = nullptr;   // float2 pass-1 twiddles [bucket][n1][t], forward (x (N M)^-1/2)
   void *d_ftw_inv = nullptr;   // same, inverse (conjugate, x sqrt(N/M))
-  qtam::FastRow *d_tiny = nullptr;   // rows shorter than 32 points (goff holds log2 M), for fused_inv.cu
+  void *d_ptw = nullptr;       // pass tables of the long FFT (ctafft.cuh)
+  qtam::FastRow *d_tiny = nullptr;   // rows shorter than 32 points (goff holds log2 M), for the combine kernel of inv_tiled.cu
   int n_tiny = 0;
-  bool fused_inv = false;      // the whole inverse runs in one kernel (fused_inv.cu)
   // tiled inverse (inv_tiled.cu)
   std::vector<qtam::FastRow> h_frows;   // host copy of d_frows (bucket-major), for build_inv_tiled
   bool tiled_inv = false;
@@ -135,6 +135,7 @@ qtam_status generic_dense(qtam_plan *p, int batch, int row_begin, int row_end, v
 qtam_status generic_threshold(qtam_plan *p, void *d_coef, int batch, double kappa, int min_log2M, cudaStream_t st);
 
 // fast.cu
+qtam_status build_long_tables(qtam_plan *p);
 qtam_status fast_r2c(qtam_plan *p, const void *d_x, int batch, cudaStream_t st);
 qtam_status fast_forward_rows(qtam_plan *p, int batch, void *d_coef, cudaStream_t st);
 qtam_status fast_inverse_rows(qtam_plan *p, const void *d_coef, int batch, int plane, cudaStream_t st);
@@ -145,7 +146,5 @@ qtam_status fast_threshold(qtam_plan *p, void *d_coef, int batch, double kappa, 
 // inv_tiled.cu
 qtam_status build_inv_tiled(qtam_plan *p);
 qtam_status tiled_inverse(qtam_plan *p, const void *d_coef, int batch, int plane, void *d_x_out, cudaStream_t st);
-// fused_inv.cu
-qtam_status fused_inverse(qtam_plan *p, const void *d_coef, int batch, int plane, void *d_x_out, cudaStream_t st);
 
 }  // namespace qtam

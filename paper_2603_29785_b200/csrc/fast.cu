@@ -36,11 +36,11 @@ extern __shared__ __align__(16) unsigned char qtam_fast_smem[];
 template <int LOG2NC>
 __global__ void __launch_bounds__(CtaFftPlan<LOG2NC>::NT)
 k_r2c_fast(const float *__restrict__ x, float2 *__restrict__ spec, long long xstride,
-           const float2 *__restrict__ tw, int log2twn) {
+           const float2 *__restrict__ tw, int log2twn, const float2 *__restrict__ ptw) {
   constexpr int NC = 1 << LOG2NC, NT = CtaFftPlan<LOG2NC>::NT;
   float2 *s = reinterpret_cast<float2 *>(qtam_fast_smem);
   const float2 *gin = reinterpret_cast<const float2 *>(x) + (size_t)blockIdx.x * NC;
-  cta_fft<LOG2NC, NT, -1, true, false>(s, gin, nullptr, tw, log2twn, 1.f);
+  cta_fft<LOG2NC, NT, -1, true, false>(s, gin, nullptr, ptw, 1.f);
   float2 *X = spec + (size_t)blockIdx.x * xstride;
   for (int f = threadIdx.x; f <= NC / 2; f += NT) {
     const int g = NC - f;
@@ -183,7 +183,8 @@ template <int LOG2NC>
 __global__ void __launch_bounds__(CtaFftPlan<LOG2NC>::NT)
 k_reduce_c2r_fast(const float2 *__restrict__ band, long long sumL, const int32_t *__restrict__ ptr,
                   const int32_t *__restrict__ idx, const float *__restrict__ invP, int nbins, int nP,
-                  int plane, const float2 *__restrict__ tw, int log2twn, float *__restrict__ x_out) {
+                  int plane, const float2 *__restrict__ tw, int log2twn, const float2 *__restrict__ ptw,
+                  float *__restrict__ x_out) {
   constexpr int NC = 1 << LOG2NC, NT = CtaFftPlan<LOG2NC>::NT;
   float2 *s = reinterpret_cast<float2 *>(qtam_fast_smem);
   const float2 *Gb = band + (size_t)blockIdx.x * sumL;
@@ -211,7 +212,7 @@ k_reduce_c2r_fast(const float2 *__restrict__ band, long long sumL, const int32_t
   }
   __syncthreads();
   float2 *gout = reinterpret_cast<float2 *>(x_out) + (size_t)blockIdx.x * NC;
-  cta_fft<LOG2NC, NT, +1, false, true>(s, nullptr, gout, tw, log2twn, 1.f);
+  cta_fft<LOG2NC, NT, +1, false, true>(s, nullptr, gout, ptw, 1.f);
 }
 
 // --------------------------------------------------------------------------------------------------
@@ -230,9 +231,27 @@ template <int LOG2NC> static qtam_status r2c_launch(qtam_plan *p, const void *d_
     LaunchScope ls(p, st, K_R2C_FAST, (double)batch * (4.0 * (double)p->hp.N + 8.0 * (double)p->hp.nb));
     k_r2c_fast<LOG2NC><<<batch, CtaFftPlan<LOG2NC>::NT, smem, st>>>(
         static_cast<const float *>(d_x), static_cast<float2 *>(p->d_spec), p->xstride,
-        static_cast<const float2 *>(p->d_tw), ilog2(p->twn));
+        static_cast<const float2 *>(p->d_tw), ilog2(p->twn), static_cast<const float2 *>(p->d_ptw));
   }
   QTAM_LAUNCH_CHECK();
+  return QTAM_OK;
+}
+
+// pass tables of the long FFT (ctafft.cuh); every kernel that runs the long transform of 2^LOG2NC points
+// uses radices equal to those of CtaFftPlan<LOG2NC>::NT (static_asserts at the kernels)
+qtam_status build_long_tables(qtam_plan *p) {
+  std::vector<float> t;
+  switch (ilog2(p->hp.N) - 1) {
+    case 11: fill_cta_fft_tables<11, CtaFftPlan<11>::NT>(t); break;
+    case 12: fill_cta_fft_tables<12, CtaFftPlan<12>::NT>(t); break;
+    case 13: fill_cta_fft_tables<13, CtaFftPlan<13>::NT>(t); break;
+    case 14: fill_cta_fft_tables<14, CtaFftPlan<14>::NT>(t); break;
+    default: return QTAM_OK;
+  }
+  if (cudaMalloc(&p->d_ptw, t.size() * sizeof(float)) != cudaSuccess) return QTAM_ERR_ALLOC;
+  p->device_bytes += t.size() * sizeof(float);
+  if (cudaMemcpy(p->d_ptw, t.data(), t.size() * sizeof(float), cudaMemcpyHostToDevice) != cudaSuccess)
+    return QTAM_ERR_CUDA;
   return QTAM_OK;
 }
 
@@ -319,7 +338,8 @@ static qtam_status reduce_c2r_launch(qtam_plan *p, int batch, int plane, void *d
     k_reduce_c2r_fast<LOG2NC><<<batch, CtaFftPlan<LOG2NC>::NT, smem, st>>>(
         static_cast<const float2 *>(p->d_band), p->hp.sumL, p->d_csr_ptr, p->d_csr_idx,
         static_cast<const float *>(p->d_invP), (int)p->hp.nb, p->hp.nP, plane,
-        static_cast<const float2 *>(p->d_tw), ilog2(p->twn), static_cast<float *>(d_x_out));
+        static_cast<const float2 *>(p->d_tw), ilog2(p->twn), static_cast<const float2 *>(p->d_ptw),
+        static_cast<float *>(d_x_out));
   }
   QTAM_LAUNCH_CHECK();
   return QTAM_OK;

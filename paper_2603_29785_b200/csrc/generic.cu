@@ -4,7 +4,7 @@
 //   - long FFT:   four-step  Nc = N1 x N2 (column FFTs + twiddle, then row FFTs)
 //   - long rows:  M = R1 x M2, decimation over the input residue (forward) or redundant first
 //                 butterfly (inverse), R1 <= 16
-// The fused/tuned kernels (fused.cu) take over the shapes they cover; everything else runs here.
+// The tuned kernels (fast.cu, inv_tiled.cu, threshold_fast.cu) take over the shapes they cover; everything else runs here.
 //
 // Hot-path steps: a1 long R2C, a2 window gather + baseband shift (PAPER.md:323-325,
 // C46 :583), a3 short inverse FFT scaled (N*M)^(-1/2) (C47 :589), a4 row-median threshold

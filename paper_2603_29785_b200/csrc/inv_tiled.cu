@@ -234,7 +234,10 @@ k_combine_c2r(const TileItem *__restrict__ items, int n_items, const float2 *__r
               long long part_stride, const FastRow *__restrict__ tiny, int n_tiny,
               const float *__restrict__ fwin, const float2 *__restrict__ coef, long long ctot,
               const float *__restrict__ invP, int nbins, int plane, const float2 *__restrict__ tw,
-              int log2twn, float *__restrict__ x_out) {
+              int log2twn, const float2 *__restrict__ ptw, float *__restrict__ x_out) {
+  typedef CtaFftRadix<LOG2NC, NT> PL;
+  typedef CtaFftRadix<LOG2NC, CtaFftPlan<LOG2NC>::NT> PL0;
+  static_assert(PL::R0 == PL0::R0 && PL::R1 == PL0::R1 && PL::R2 == PL0::R2, "pass tables are built for PL0");
   constexpr int NC = 1 << LOG2NC;
   float2 *S = reinterpret_cast<float2 *>(qtam_tiled_smem);
   float2 *tbuf = S + cta_fft_smem_elems<LOG2NC>();      // 32 band values per tiny row
@@ -242,35 +245,72 @@ k_combine_c2r(const TileItem *__restrict__ items, int n_items, const float2 *__r
   const float2 *Yseg = coef + (size_t)blockIdx.x * ctot;
 
   // rows shorter than 32 points: Bhat[jj] = sqrt(N/M) sum_n Y[n] e^{-2 pi i jj n/M} by direct summation
+  // (lane l holds Y[l] and e^{-2 pi i l/M}; the sum over n takes both from shuffles)
   for (int s = warp; s < n_tiny; s += NT / 32) {
     const FastRow row = tiny[s];              // goff holds log2 M for tiny rows
     float2 out = make_float2(0.f, 0.f);
-    if ((plane < 0 || row.plane == plane) && lane <= 2 * row.dk) {
+    if (plane < 0 || row.plane == plane) {    // warp-uniform
       const int lm = row.goff, M = 1 << lm;
+      float2 y = make_float2(0.f, 0.f), w = make_float2(1.f, 0.f);
+      if (lane < M) {
+        y = Yseg[row.offset + lane];
+        w = __ldg(tw + ((size_t)lane << (log2twn - lm)));
+        w.y = -w.y;
+      }
       const int jj = lane - row.dk;
-      const float2 *Y = Yseg + row.offset;
       float2 acc = make_float2(0.f, 0.f);
       for (int n = 0; n < M; ++n) {
         const int m = (jj * n) & (M - 1);
-        float2 w = __ldg(tw + ((size_t)m << (log2twn - lm)));
-        w.y = -w.y;
-        acc = padd(acc, pcmul(Y[n], w));
+        float2 yn, wm;
+        yn.x = __shfl_sync(0xffffffffu, y.x, n); yn.y = __shfl_sync(0xffffffffu, y.y, n);
+        wm.x = __shfl_sync(0xffffffffu, w.x, m); wm.y = __shfl_sync(0xffffffffu, w.y, m);
+        acc = padd(acc, pcmul(yn, wm));
       }
-      const float amp = sqrtf((float)(2 * NC) / (float)M);
-      out = pscale(acc, amp * fwin[row.woff + lane]);
+      if (lane <= 2 * row.dk) {
+        const float amp = sqrtf((float)(2 * NC) / (float)M);
+        out = pscale(acc, amp * fwin[row.woff + lane]);
+      }
     }
     tbuf[s * 32 + lane] = out;
   }
 
-  // S[f] = sum over the tiles' partial sums, tile order; thread t owns the bins f = t (mod NT)
-  for (int f = tid; f <= NC; f += NT) S[f] = make_float2(0.f, 0.f);
+  // S[f] = sum over the tiles' partial sums in tile order.  Warp w owns the bins [w BW, (w+1) BW), lane l
+  // the bins l + 32 q of that range, accumulated in registers: per tile that meets the range all the
+  // loads of a lane are independent (the partial sums come from L2).
+  constexpr int NWARP = NT / 32, BW = NC / NWARP, QB = BW / 32;
   const float2 *pseg = part + (size_t)blockIdx.x * part_stride;
-  for (int i = 0; i < n_items; ++i) {
-    const int4 b = __ldg(reinterpret_cast<const int4 *>(items + i) + 1);   // lo, nb, part_off, npass
-    const float2 *src = pseg + b.z;
-    for (int j = (tid - b.x) & (NT - 1); j < b.y; j += NT) {
-      const int f = b.x + j;
-      S[f] = padd(S[f], src[j]);
+  {
+    float2 acc[QB];
+#pragma unroll
+    for (int q = 0; q < QB; ++q) acc[q] = make_float2(0.f, 0.f);
+    const int f0 = warp * BW + lane;
+#pragma unroll 1
+    for (int i = 0; i < n_items; ++i) {
+      const int4 b = __ldg(reinterpret_cast<const int4 *>(items + i) + 1);   // lo, nb, part_off, npass
+      if (b.x + b.y <= warp * BW || b.x >= (warp + 1) * BW) continue;
+      const float2 *src = pseg + b.z - b.x;
+#pragma unroll
+      for (int q = 0; q < QB; ++q) {
+        const int f = f0 + 32 * q;
+        if ((unsigned)(f - b.x) < (unsigned)b.y) acc[q] = padd(acc[q], __ldcg(src + f));
+      }
+    }
+#pragma unroll
+    for (int q = 0; q < QB; ++q) S[f0 + 32 * q] = acc[q];
+    // the Nyquist bin: one tile per lane, fixed shuffle tree
+    if (warp == 0) {
+      float2 a = make_float2(0.f, 0.f);
+      for (int i = lane; i < n_items; i += 32) {
+        const int4 b = __ldg(reinterpret_cast<const int4 *>(items + i) + 1);
+        if ((unsigned)(NC - b.x) < (unsigned)b.y) a = padd(a, __ldcg(pseg + b.z + (NC - b.x)));
+      }
+      for (int o = 16; o > 0; o >>= 1) {
+        float2 other;
+        other.x = __shfl_xor_sync(0xffffffffu, a.x, o);
+        other.y = __shfl_xor_sync(0xffffffffu, a.y, o);
+        a = padd(a, other);
+      }
+      if (lane == 0) S[NC] = a;
     }
   }
   __syncthreads();
@@ -300,7 +340,7 @@ k_combine_c2r(const TileItem *__restrict__ items, int n_items, const float2 *__r
   }
   __syncthreads();
   float2 *gout = reinterpret_cast<float2 *>(x_out) + (size_t)blockIdx.x * NC;
-  cta_fft<LOG2NC, NT, +1, false, true>(S, nullptr, gout, tw, log2twn, 1.f);
+  cta_fft<LOG2NC, NT, +1, false, true>(S, nullptr, gout, ptw, 1.f);
 }
 
 // --------------------------------------------------------------------------------------------------
@@ -354,7 +394,7 @@ static qtam_status combine_launch(qtam_plan *p, const void *d_coef, int batch, i
         p->d_titems, p->n_titems, static_cast<const float2 *>(p->d_part), p->part_stride, p->d_tiny, p->n_tiny,
         static_cast<const float *>(p->d_fwin), static_cast<const float2 *>(d_coef), p->hp.ctot,
         static_cast<const float *>(p->d_invP), (int)p->hp.nb, plane, static_cast<const float2 *>(p->d_tw),
-        ilog2(p->twn), static_cast<float *>(d_x_out));
+        ilog2(p->twn), static_cast<const float2 *>(p->d_ptw), static_cast<float *>(d_x_out));
   }
   QTAM_LAUNCH_CHECK();
   return QTAM_OK;
@@ -371,7 +411,7 @@ qtam_status tiled_inverse(qtam_plan *p, const void *d_coef, int batch, int plane
   switch (ilog2(p->hp.N) - 1) {
     case 11: return combine_launch<11, 256>(p, d_coef, batch, plane, d_x_out, st);
     case 12: return combine_launch<12, 256>(p, d_coef, batch, plane, d_x_out, st);
-    case 13: return combine_launch<13, 512>(p, d_coef, batch, plane, d_x_out, st);
+    case 13: return combine_launch<13, 256>(p, d_coef, batch, plane, d_x_out, st);
     case 14: return combine_launch<14, 512>(p, d_coef, batch, plane, d_x_out, st);
     default: return QTAM_ERR_UNSUPPORTED;
   }
