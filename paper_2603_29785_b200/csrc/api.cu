@@ -48,6 +48,8 @@ void free_plan(qtam_plan *p) {
   cudaFree(p->d_frows); cudaFree(p->d_fwin); cudaFree(p->d_ftw_fwd); cudaFree(p->d_ftw_inv);
   cudaFree(p->d_tiny); cudaFree(p->d_ptw);
   cudaFree(p->d_thr_tasks); cudaFree(p->d_thr_offs);
+  for (int c = 0; c < 4; ++c) { cudaFree(p->d_cta_rowidx[c]); cudaFree(p->d_ptw_rows[c]); }
+  for (int b = 0; b < 3; ++b) cudaFree(p->d_twb[b]);
   cudaFree(p->d_trows); cudaFree(p->d_titems); cudaFree(p->d_part); cudaFree(p->d_counter);
   for (ProfRec &r : p->prof_pool) { cudaEventDestroy(r.e0); cudaEventDestroy(r.e1); }
   delete p;
@@ -223,6 +225,7 @@ template <typename T> qtam_status build_device(qtam_plan *p) {
     for (size_t k = 0; k < hp.rows.size(); ++k) {
       const int lm = ilog2(hp.rows[k].M);
       if (p->fast_rows && lm >= 5 && lm <= 10) continue;   // handled by fast.cu
+      if (p->fast_rows && lm >= kCtaLog2Min && lm <= kCtaLog2Max && hp.ctot < (int64_t(1) << 31)) continue;   // rows_cta.cu
       if (lm <= p->cap_log2) {
         const int c = generic_class_of(lm);
         items[c].push_back(WorkItem{(int)k, 0, 1, lm});
@@ -299,6 +302,7 @@ qtam_status qtam_plan_create(qtam_plan **out, double fs, int64_t N, const double
   s = dtype == QTAM_F32 ? build_device<float>(p) : build_device<double>(p);
   if (s == QTAM_OK) s = build_thr_fast(p);
   if (s == QTAM_OK && p->fast_rows) s = build_fast(p);
+  if (s == QTAM_OK && p->fast_rows) s = build_rows_cta(p);
   if (s == QTAM_OK && p->fast_long) s = build_long_tables(p);
   if (s == QTAM_OK && p->fast_rows) s = build_inv_tiled(p);
   if (s != QTAM_OK) { free_plan(p); cudaGetLastError(); return s; }
@@ -377,6 +381,10 @@ qtam_status qtam_forward(qtam_plan *p, const void *d_x, int batch, void *d_coef,
     s = fast_forward_rows(p, batch, d_coef, st);
     if (s != QTAM_OK) return s;
   }
+  if (p->cta_rows) {
+    s = cta_forward_rows(p, batch, d_coef, st);
+    if (s != QTAM_OK) return s;
+  }
   return generic_forward_rows(p, batch, d_coef, st);
 }
 
@@ -392,6 +400,10 @@ qtam_status qtam_inverse(qtam_plan *p, const void *d_coef, int batch, int plane,
   qtam_status s = QTAM_OK;
   if (p->fast_rows) {
     s = fast_inverse_rows(p, d_coef, batch, plane, st);
+    if (s != QTAM_OK) return s;
+  }
+  if (p->cta_rows) {
+    s = cta_inverse_rows(p, d_coef, batch, plane, st);
     if (s != QTAM_OK) return s;
   }
   s = generic_inverse_rows(p, d_coef, batch, plane, st);
@@ -432,7 +444,7 @@ int qtam_last_launch_count(const qtam_plan *p) { return p ? p->last_launches : 0
 static const char *const kKernelNames[K_COUNT] = {
     "cfft_seq", "cfft_cols", "cfft_rows", "r2c_post", "c2r_pre", "fwd_rows", "fwd_combine",
     "inv_rows", "inv_reduce", "dense_place", "threshold", "r2c_fast", "fwd_rows_fast", "inv_rows_fast",
-    "reduce_c2r_fast", "inv_fused", "inv_tiles", "combine_c2r", "threshold_fast"};
+    "reduce_c2r_fast", "inv_fused", "inv_tiles", "combine_c2r", "threshold_fast", "rows_cta_fwd", "rows_cta_inv"};
 
 qtam_status qtam_profile_enable(qtam_plan *p, int on, int max_launches) {
   if (!p || p->host_only) return QTAM_ERR_INVALID_ARG;

@@ -40,11 +40,24 @@ template <int LOG2NC> __host__ __device__ constexpr int cta_fft_smem_elems() {
   return (1 << LOG2NC) + ((1 << LOG2NC) >> 4) + 2;   // the smallest first radix is 16
 }
 
-// One Stockham pass.  IN_MODE / OUT_MODE: 0 natural smem, 1 skewed smem, 2 global (natural).
-template <int LOG2NC, int NT, int R, int LOG2NS, int DIR, int IN_MODE, int OUT_MODE, int SKEW>
-__device__ __forceinline__ void cta_fft_pass(float2 *s, const float2 *__restrict__ gin,
-                                             float2 *__restrict__ gout, const float2 *__restrict__ ptw,
-                                             float out_scale) {
+// sources / sinks of the transform's first / last pass (natural order index a)
+struct CtaFftGlobalIn {
+  const float2 *__restrict__ p;
+  __device__ __forceinline__ float2 operator()(int a) const { return p[a]; }
+};
+struct CtaFftGlobalOut {
+  float2 *__restrict__ p; float scale;
+  __device__ __forceinline__ void operator()(int a, float2 v) const { p[a] = pscale(v, scale); }
+};
+struct CtaFftNone {
+  __device__ __forceinline__ float2 operator()(int) const { return make_float2(0.f, 0.f); }
+  __device__ __forceinline__ void operator()(int, float2) const {}
+};
+
+// One Stockham pass.  IN_MODE / OUT_MODE: 0 natural smem, 1 skewed smem, 2 the functor `in` / `out`.
+template <int LOG2NC, int NT, int R, int LOG2NS, int DIR, int IN_MODE, int OUT_MODE, int SKEW, class In, class Out>
+__device__ __forceinline__ void cta_fft_pass(float2 *s, const In &in, const Out &out,
+                                             const float2 *__restrict__ ptw) {
   constexpr int NC = 1 << LOG2NC;
   constexpr int NBF = NC / R;                 // butterflies
   constexpr int BPT = (NBF + NT - 1) / NT;    // per thread
@@ -57,7 +70,7 @@ __device__ __forceinline__ void cta_fft_pass(float2 *s, const float2 *__restrict
 #pragma unroll
       for (int r = 0; r < R; ++r) {
         const int a = i + r * NBF;
-        if constexpr (IN_MODE == 2) v[u][r] = gin[a];
+        if constexpr (IN_MODE == 2) v[u][r] = in(a);
         else if constexpr (IN_MODE == 1) v[u][r] = s[a + (a >> SKEW)];
         else v[u][r] = s[a];
       }
@@ -97,7 +110,7 @@ __device__ __forceinline__ void cta_fft_pass(float2 *s, const float2 *__restrict
 #pragma unroll
       for (int r = 0; r < R; ++r) {
         const int a = base + r * NS;
-        if constexpr (OUT_MODE == 2) gout[a] = pscale(v[u][r], out_scale);
+        if constexpr (OUT_MODE == 2) out(a, v[u][r]);
         else if constexpr (OUT_MODE == 1) s[a + (a >> SKEW)] = v[u][r];
         else s[a] = v[u][r];
       }
@@ -137,19 +150,25 @@ template <int LOG2NC, int NT> inline void fill_cta_fft_tables(std::vector<float>
 }
 
 // Whole transform with NT threads (all threads of the CTA must call it).
-// FROM_GLOBAL: pass 1 reads gin (natural order) instead of s (natural layout).
-// TO_GLOBAL: the last pass writes gout (natural order, times out_scale) instead of s (natural layout).
+// FROM_GLOBAL: pass 1 takes its inputs from in(a), a = natural-order index, instead of s (natural layout).
+// TO_GLOBAL: the last pass hands its results to out(a, value) instead of writing s (natural layout).
 // ptw: the pass tables built by fill_cta_fft_tables (host) for this (LOG2NC, NT)'s radices.
-template <int LOG2NC, int NT, int DIR, bool FROM_GLOBAL, bool TO_GLOBAL>
-__device__ __forceinline__ void cta_fft(float2 *s, const float2 *__restrict__ gin, float2 *__restrict__ gout,
-                                        const float2 *__restrict__ ptw, float out_scale) {
+template <int LOG2NC, int NT, int DIR, bool FROM_GLOBAL, bool TO_GLOBAL, class In, class Out>
+__device__ __forceinline__ void cta_fft_io(float2 *s, const In &in, const Out &out, const float2 *__restrict__ ptw) {
   typedef CtaFftRadix<LOG2NC, NT> PL;
   constexpr int L0 = ILog2<PL::R0>::value, L1 = ILog2<PL::R1>::value;
   static_assert(L0 + L1 + ILog2<PL::R2>::value == LOG2NC, "radices must multiply to Nc");
-  cta_fft_pass<LOG2NC, NT, PL::R0, 0, DIR, FROM_GLOBAL ? 2 : 0, 1, L0>(s, gin, gout, ptw, 1.f);
-  cta_fft_pass<LOG2NC, NT, PL::R1, L0, DIR, 1, 0, L0>(s, gin, gout, ptw, 1.f);
+  cta_fft_pass<LOG2NC, NT, PL::R0, 0, DIR, FROM_GLOBAL ? 2 : 0, 1, L0>(s, in, out, ptw);
+  cta_fft_pass<LOG2NC, NT, PL::R1, L0, DIR, 1, 0, L0>(s, in, out, ptw);
   cta_fft_pass<LOG2NC, NT, PL::R2, L0 + L1, DIR, 0, TO_GLOBAL ? 2 : 0, L0>(
-      s, gin, gout, ptw + cta_fft_ptw_off3<LOG2NC, NT>(), out_scale);
+      s, in, out, ptw + cta_fft_ptw_off3<LOG2NC, NT>());
+}
+
+// the same with plain global pointers: gin read in natural order, gout written in natural order x out_scale
+template <int LOG2NC, int NT, int DIR, bool FROM_GLOBAL, bool TO_GLOBAL>
+__device__ __forceinline__ void cta_fft(float2 *s, const float2 *__restrict__ gin, float2 *__restrict__ gout,
+                                        const float2 *__restrict__ ptw, float out_scale) {
+  cta_fft_io<LOG2NC, NT, DIR, FROM_GLOBAL, TO_GLOBAL>(s, CtaFftGlobalIn{gin}, CtaFftGlobalOut{gout, out_scale}, ptw);
 }
 
 }  // namespace qtam

@@ -12,7 +12,7 @@ namespace qtam {
 enum KernelId {
   K_CFFT_SEQ = 0, K_CFFT_COLS, K_CFFT_ROWS, K_R2C_POST, K_C2R_PRE, K_FWD_ROWS, K_FWD_COMBINE,
   K_INV_ROWS, K_INV_REDUCE, K_DENSE_PLACE, K_THRESHOLD, K_R2C_FAST, K_FWD_ROWS_FAST, K_INV_ROWS_FAST,
-  K_REDUCE_C2R_FAST, K_INV_FUSED, K_INV_TILES, K_COMBINE_C2R, K_THRESHOLD_FAST, K_COUNT
+  K_REDUCE_C2R_FAST, K_INV_FUSED, K_INV_TILES, K_COMBINE_C2R, K_THRESHOLD_FAST, K_ROWS_CTA_FWD, K_ROWS_CTA_INV, K_COUNT
 };
 // fast float path (fast.cu): rows with 32 <= M <= 1024, grouped by G = M/32 lanes per row
 struct FastRow { int kc, dk, woff, goff, offset, plane, wpad, pad; };   // wpad: offset into the padded window table
@@ -30,6 +30,8 @@ constexpr int kAccBins = 1280;
 // fast threshold (threshold_fast.cu): a warp task = up to 32/G rows of one length M = 32 G (or 32 rows of M < 32)
 struct ThrTask { int log2M, row0, nrows, pad; };
 constexpr int kThrFastLog2Max = 10;
+// CTA-level rows (rows_cta.cu): 2^11 .. 2^14 points in one shared-memory transform, up to 2^17 in 2, 4 or 8
+constexpr int kCtaLog2Min = 11, kCtaLog2Max = 17;
 struct ProfRec { int kid; double bytes; cudaEvent_t e0, e1; };
 }  // namespace qtam
 
@@ -98,6 +100,15 @@ struct qtam_plan {
   int n_thr_tasks = 0;
   bool thr_has_big = false;       // some row is longer than 2^kThrFastLog2Max points (generic kernel)
 
+  // CTA-level rows (rows_cta.cu), one class per transform length 2^11 .. 2^14
+  bool cta_rows = false;
+  int *d_cta_rowidx[4] = {nullptr, nullptr, nullptr, nullptr};
+  int n_cta_rows[4] = {0, 0, 0, 0};
+  double cta_sumM[4] = {0, 0, 0, 0}, cta_sumL[4] = {0, 0, 0, 0};
+  int64_t cta_maxM = 0;           // longest row that needs the per-CTA scratch (0: none)
+  void *d_ptw_rows[4] = {nullptr, nullptr, nullptr, nullptr};   // pass tables per class
+  void *d_twb[3] = {nullptr, nullptr, nullptr};                 // e^{2 pi i n/M}, n < 2^14, M = 2^15..2^17
+
   int last_launches = 0;
   // launch profile (qtam_profile_enable / qtam_profile_read)
   bool prof_on = false;
@@ -140,6 +151,10 @@ qtam_status fast_r2c(qtam_plan *p, const void *d_x, int batch, cudaStream_t st);
 qtam_status fast_forward_rows(qtam_plan *p, int batch, void *d_coef, cudaStream_t st);
 qtam_status fast_inverse_rows(qtam_plan *p, const void *d_coef, int batch, int plane, cudaStream_t st);
 qtam_status fast_reduce_c2r(qtam_plan *p, int batch, int plane, void *d_x_out, cudaStream_t st);
+// rows_cta.cu
+qtam_status build_rows_cta(qtam_plan *p);
+qtam_status cta_forward_rows(qtam_plan *p, int batch, void *d_coef, cudaStream_t st);
+qtam_status cta_inverse_rows(qtam_plan *p, const void *d_coef, int batch, int plane, cudaStream_t st);
 // threshold_fast.cu
 qtam_status build_thr_fast(qtam_plan *p);
 qtam_status fast_threshold(qtam_plan *p, void *d_coef, int batch, double kappa, cudaStream_t st);
