@@ -110,12 +110,12 @@ qtam_status build_fast(qtam_plan *p) {
   };
   std::vector<FastRow> frows;
   std::vector<int4> red;
-  std::vector<float> twf, twi;   // (wx, wx, wy, wy) per entry
+  std::vector<float> twf, twi;   // (wx, wy) per entry
   const long double tau = 6.283185307179586476925286766559005768L;
   for (int lg = 5; lg >= 0; --lg) {
     const int G = 1 << lg, M = 32 * G, Fr = 32 / G;
     FastBucket B{};
-    B.log2G = lg; B.row_base = (int)frows.size(); B.tw_base = (int)(twf.size() / 4);
+    B.log2G = lg; B.row_base = (int)frows.size(); B.tw_base = (int)(twf.size() / 2);
     for (size_t k = 0; k < hp.rows.size(); ++k) {
       const HostRow &h = hp.rows[k];
       if (h.M != M) continue;
@@ -139,14 +139,14 @@ qtam_status build_fast(qtam_plan *p) {
         const int m = (n1 * t) % M;
         const long double a = tau * (long double)m / (long double)M;
         const double c = (double)cosl(a), s = (double)sinl(a);
-        twf.push_back((float)(c * sf)); twf.push_back((float)(c * sf));
-        twf.push_back((float)(s * sf)); twf.push_back((float)(s * sf));
-        twi.push_back((float)(c * si)); twi.push_back((float)(-s * si));   // inverse tables stay (wx, wy)
+        twf.push_back((float)(c * sf)); twf.push_back((float)(s * sf));
+        twi.push_back((float)(c * si)); twi.push_back((float)(-s * si));
       }
     F.groups_per_seg += B.ngroups;
     F.b[F.nbuckets++] = B;
   }
-  F.tw_total = (int)(twf.size() / 4);
+  F.tw_total = (int)(twf.size() / 2);
+  F.rows_smem = frows.size() <= 1024 ? (int)frows.size() : 0;
   // rows shorter than 32 points
   std::vector<FastRow> tiny;
   for (size_t k = 0; k < hp.rows.size(); ++k) {

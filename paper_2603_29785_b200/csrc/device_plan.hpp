@@ -18,7 +18,8 @@ enum KernelId {
 struct FastRow { int kc, dk, woff, goff, offset, plane, wpad, pad; };   // wpad: offset into the padded window table
 struct FastBucket { int log2G, nrows, ngroups, row_base, tw_base, pad; };
 struct FastParams {
-  int nbuckets, groups_per_seg, tw_total, pad;
+  int nbuckets, groups_per_seg, tw_total;
+  int rows_smem;                // rows staged in shared memory by k_rows_fast (0: table too long, read from global)
   double sum_M, sum_L;          // coefficients / band values per segment the fast rows cover
   FastBucket b[6];
 };

@@ -63,7 +63,7 @@ k_r2c_fast(const float *__restrict__ x, float2 *__restrict__ spec, long long xst
 // --------------------------------------------------------------------------------------------------
 template <int LOG2G>
 __device__ QTAM_GROUP_INLINE void fwd_group(const FastBucket &B, const FastRow *__restrict__ frows, int seg, int grp,
-                                       int lane, float2 *ex, const float4 *tw1,
+                                       int lane, float2 *ex, const float2 *tw1,
                                        const float2 *__restrict__ spec, long long xstride,
                                        const float *__restrict__ fwinp, float2 *__restrict__ coef,
                                        long long ctot) {
@@ -77,13 +77,19 @@ __device__ QTAM_GROUP_INLINE void fwd_group(const FastBucket &B, const FastRow *
   // buffer has zero pads, so neither the support (A9) nor the clipping at DC / Nyquist (R8) needs a test
   const float2 *X = spec + (size_t)seg * xstride + row.kc + t;
   const float *W = fwinp + row.wpad + t;
+  // ... and outside the support nothing is loaded at all: one compare per element saves the two loads
+  // of the 40-50 % of the M-array that the window leaves empty
+  const int hi = row.dk - t, lo = -row.dk - t;
   float2 v[32];
 #pragma unroll
   for (int j1 = 0; j1 < 32; ++j1) {
     const int jj = (j1 < 16) ? (G * j1) : (G * j1 - M);     // signed offset from the centre (R6), minus t
-    const float2 xv = X[jj];
-    const float w = W[G * j1];
-    v[j1] = make_float2(xv.x * w, xv.y * w);
+    v[j1] = make_float2(0.f, 0.f);
+    if ((j1 < 16) ? (jj <= hi) : (jj >= lo)) {
+      const float2 xv = X[jj];
+      const float w = W[G * j1];
+      v[j1] = make_float2(xv.x * w, xv.y * w);
+    }
   }
   RowFFT<LOG2G, +1>::run(v, ex, tw1, lane);
   if (valid) {
@@ -133,33 +139,40 @@ __device__ QTAM_GROUP_INLINE void inv_group(const FastBucket &B, const FastRow *
 
 template <int NWARPS, bool FORWARD>
 __global__ void __launch_bounds__(NWARPS * 32, NWARPS <= 8 ? 2 : 1)
-k_rows_fast(FastParams P, const FastRow *__restrict__ frows, const void *__restrict__ tw1g_,
+k_rows_fast(FastParams P, const FastRow *frows, const void *__restrict__ tw1g_,
             const float *__restrict__ fwin, const float *__restrict__ fwinp,
             const float2 *__restrict__ spec, long long xstride, int nbins,
             float2 *__restrict__ coef, long long ctot, float2 *__restrict__ band, long long sumL,
             int batch, int plane) {
-  // forward tables are (wx, wx, wy, wy) float4, inverse tables (wx, wy) float2
-  typedef typename std::conditional<FORWARD, float4, float2>::type TW;
+  typedef float2 TW;
   const TW *tw1g = static_cast<const TW *>(tw1g_);
   TW *tw1s = reinterpret_cast<TW *>(qtam_fast_smem);
-  float2 *exall = reinterpret_cast<float2 *>(qtam_fast_smem + sizeof(float4) * (size_t)P.tw_total);
+  float2 *exall = reinterpret_cast<float2 *>(qtam_fast_smem + sizeof(float2) * (size_t)((P.tw_total + 1) & ~1));
   for (int i = threadIdx.x; i < P.tw_total; i += NWARPS * 32) tw1s[i] = tw1g[i];
+  // the row table too, when it fits (P.rows_smem): a row's record is then one shared-memory read away
+  // instead of a global load the gather addresses have to wait for
+  if (P.rows_smem) {
+    int4 *dst = reinterpret_cast<int4 *>(exall + NWARPS * kExPerWarp);
+    const int4 *src = reinterpret_cast<const int4 *>(frows);
+    for (int i = threadIdx.x; i < 2 * P.rows_smem; i += NWARPS * 32) dst[i] = src[i];
+    frows = reinterpret_cast<const FastRow *>(dst);
+  }
   __syncthreads();
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   float2 *ex = exall + warp * kExPerWarp;
-  const long long total = (long long)P.groups_per_seg * batch;
-  for (long long item = ((long long)blockIdx.x * NWARPS) + warp; item < total;
-       item += (long long)gridDim.x * NWARPS) {
+  // (the host keeps groups_per_seg * batch below 2^31)
+  const unsigned total = (unsigned)P.groups_per_seg * (unsigned)batch;
+  for (unsigned item = blockIdx.x * NWARPS + warp; item < total; item += gridDim.x * NWARPS) {
     // decode: buckets in order, each spanning ngroups*batch items
     int q = 0;
-    long long rem = item;
-    while (q + 1 < P.nbuckets && rem >= (long long)P.b[q].ngroups * batch) {
-      rem -= (long long)P.b[q].ngroups * batch;
+    unsigned rem = item;
+    while (q + 1 < P.nbuckets && rem >= (unsigned)P.b[q].ngroups * (unsigned)batch) {
+      rem -= (unsigned)P.b[q].ngroups * (unsigned)batch;
       ++q;
     }
     const FastBucket B = P.b[q];
-    const int seg = (int)(rem / B.ngroups);
-    const int grp = (int)(rem - (long long)seg * B.ngroups);
+    const int seg = (int)(rem / (unsigned)B.ngroups);
+    const int grp = (int)(rem - (unsigned)seg * (unsigned)B.ngroups);
     const TW *tw1 = tw1s + B.tw_base;
 #define QTAM_ROW_CASE(L)                                                                              \
   case L:                                                                                             \
@@ -270,7 +283,9 @@ static qtam_status rows_launch_nw(qtam_plan *p, int batch, const void *d_coef_in
                                   cudaStream_t st) {
   const FastParams &P = p->fast;
   if (P.groups_per_seg == 0) return QTAM_OK;
-  const size_t smem = sizeof(float4) * (size_t)P.tw_total + sizeof(float2) * (size_t)NW * kExPerWarp;
+  const size_t smem = sizeof(float2) * (size_t)((P.tw_total + 1) & ~1) + sizeof(float2) * (size_t)NW * kExPerWarp +
+                      sizeof(FastRow) * (size_t)P.rows_smem;
+  if ((long long)P.groups_per_seg * batch >= (1LL << 31)) return QTAM_ERR_UNSUPPORTED;
   auto kern = k_rows_fast<NW, FORWARD>;
   if (!set_smem(kern, smem)) return QTAM_ERR_CUDA;
   int occ = 1;

@@ -19,21 +19,33 @@ template <int LOG2G, int DIR> struct RowFFT {
   static constexpr int F = 32 / G;
   static constexpr int M = 32 * G;
 
-  static __device__ __forceinline__ float2 twmulx(float2 a, float4 w) { return pcmul4(a, w); }
-  static __device__ __forceinline__ float2 twmulx(float2 a, float2 w) { return pcmul(a, w); }
-  static __device__ __forceinline__ float scale_of(float4 w) { return w.x; }
+  static __device__ __forceinline__ float2 twmulx(float2 a, float2 w) {
+    return make_float2(a.x * w.x - a.y * w.y, a.x * w.y + a.y * w.x);
+  }
   static __device__ __forceinline__ float scale_of(float2 w) { return w.x; }
 
-  // tw1: [n1][t] entries of w_M^{dir t n1} x scale, in shared or global memory; either plain float2
-  // (wx, wy) or pre-duplicated float4 (wx, wx, wy, wy) that needs no pair-building moves
+  // tw1: [n1][t] entries (wx, wy) of w_M^{dir t n1} x scale, in shared or global memory (64-bit loads:
+  // half the shared-memory wavefronts of a pre-duplicated (wx, wx, wy, wy) table, measured faster)
   template <typename TW>
   static __device__ __forceinline__ void run(float2 (&v)[32], float2 *ex, const TW *tw1, int lane) {
     const int t = lane & (G - 1), rw = lane >> LOG2G;
     RegFFT<32, DIR>::run(v);
     if constexpr (G > 1) {
       float2 *exw = ex + rw * (G * kExPitch) + t * kExPitch;
+      // twiddles in batches of 8, one batch ahead of the multiplies: the shared-memory latency is paid
+      // four times per row instead of once per element
+      TW w[2][8];
 #pragma unroll
-      for (int n1 = 0; n1 < 32; ++n1) exw[n1] = twmulx(v[n1], tw1[n1 * G + t]);
+      for (int k = 0; k < 8; ++k) w[0][k] = tw1[k * G + t];
+#pragma unroll
+      for (int c = 0; c < 4; ++c) {
+        if (c < 3) {
+#pragma unroll
+          for (int k = 0; k < 8; ++k) w[(c + 1) & 1][k] = tw1[(8 * (c + 1) + k) * G + t];
+        }
+#pragma unroll
+        for (int k = 0; k < 8; ++k) exw[8 * c + k] = twmulx(v[8 * c + k], w[c & 1][k]);
+      }
       __syncwarp();
       const float2 *exr = ex + rw * (G * kExPitch) + t;
 #pragma unroll
