@@ -154,7 +154,8 @@ qtam_status build_fast(qtam_plan *p) {
     if (h.M >= 32) continue;
     FastRow r{};
     r.kc = (int)h.kc; r.dk = (int)h.dk; r.woff = window_of(h); r.goff = ilog2(h.M);
-    r.offset = (int)h.offset; r.plane = h.plane;
+    r.offset = (int)h.offset; r.plane = h.plane; r.wpad = (int)h.goff;   // wpad: band offset (tiny rows)
+    p->tiny_sumM += (double)h.M; p->tiny_sumL += (double)h.L;
     tiny.push_back(r);
   }
   p->n_tiny = (int)tiny.size();
@@ -224,7 +225,7 @@ template <typename T> qtam_status build_device(qtam_plan *p) {
     std::vector<int> big;
     for (size_t k = 0; k < hp.rows.size(); ++k) {
       const int lm = ilog2(hp.rows[k].M);
-      if (p->fast_rows && lm >= 5 && lm <= 10) continue;   // handled by fast.cu
+      if (p->fast_rows && lm <= 10) continue;   // handled by fast.cu (32..1024: warp engine; < 32: one thread per row)
       if (p->fast_rows && lm >= kCtaLog2Min && lm <= kCtaLog2Max && hp.ctot < (int64_t(1) << 31)) continue;   // rows_cta.cu
       if (lm <= p->cap_log2) {
         const int c = generic_class_of(lm);
@@ -444,7 +445,8 @@ int qtam_last_launch_count(const qtam_plan *p) { return p ? p->last_launches : 0
 static const char *const kKernelNames[K_COUNT] = {
     "cfft_seq", "cfft_cols", "cfft_rows", "r2c_post", "c2r_pre", "fwd_rows", "fwd_combine",
     "inv_rows", "inv_reduce", "dense_place", "threshold", "r2c_fast", "fwd_rows_fast", "inv_rows_fast",
-    "reduce_c2r_fast", "inv_fused", "inv_tiles", "combine_c2r", "threshold_fast", "rows_cta_fwd", "rows_cta_inv"};
+    "reduce_c2r_fast", "inv_fused", "inv_tiles", "combine_c2r", "threshold_fast", "rows_cta_fwd", "rows_cta_inv",
+    "tiny_rows_fwd", "tiny_rows_inv"};
 
 qtam_status qtam_profile_enable(qtam_plan *p, int on, int max_launches) {
   if (!p || p->host_only) return QTAM_ERR_INVALID_ARG;

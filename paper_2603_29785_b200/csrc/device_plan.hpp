@@ -12,7 +12,8 @@ namespace qtam {
 enum KernelId {
   K_CFFT_SEQ = 0, K_CFFT_COLS, K_CFFT_ROWS, K_R2C_POST, K_C2R_PRE, K_FWD_ROWS, K_FWD_COMBINE,
   K_INV_ROWS, K_INV_REDUCE, K_DENSE_PLACE, K_THRESHOLD, K_R2C_FAST, K_FWD_ROWS_FAST, K_INV_ROWS_FAST,
-  K_REDUCE_C2R_FAST, K_INV_FUSED, K_INV_TILES, K_COMBINE_C2R, K_THRESHOLD_FAST, K_ROWS_CTA_FWD, K_ROWS_CTA_INV, K_COUNT
+  K_REDUCE_C2R_FAST, K_INV_FUSED, K_INV_TILES, K_COMBINE_C2R, K_THRESHOLD_FAST, K_ROWS_CTA_FWD, K_ROWS_CTA_INV,
+  K_TINY_FWD, K_TINY_INV, K_COUNT
 };
 // fast float path (fast.cu): rows with 32 <= M <= 1024, grouped by G = M/32 lanes per row
 struct FastRow { int kc, dk, woff, goff, offset, plane, wpad, pad; };   // wpad: offset into the padded window table
@@ -85,6 +86,7 @@ struct qtam_plan {
   void *d_ptw = nullptr;       // pass tables of the long FFT (ctafft.cuh)
   qtam::FastRow *d_tiny = nullptr;   // rows shorter than 32 points (goff holds log2 M), for the combine kernel of inv_tiled.cu
   int n_tiny = 0;
+  double tiny_sumM = 0, tiny_sumL = 0;   // coefficients / band values per segment of those rows
   // tiled inverse (inv_tiled.cu)
   std::vector<qtam::FastRow> h_frows;   // host copy of d_frows (bucket-major), for build_inv_tiled
   bool tiled_inv = false;

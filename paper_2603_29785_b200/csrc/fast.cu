@@ -57,6 +57,76 @@ k_r2c_fast(const float *__restrict__ x, float2 *__restrict__ spec, long long xst
 }
 
 // --------------------------------------------------------------------------------------------------
+// Rows shorter than 32 points (M = 4, 8, 16): one thread per (segment, row), the whole row in registers.
+// Forward: B[j] = X[kc + jj] W[jj] at j = jj mod M (R6; the spectrum's zero pads implement R8),
+// Y = (N M)^{-1/2} IFFT_M(B) (C47).  Inverse: G[jj] = sqrt(N/M) FFT_M(Y)[jj mod M] W[jj] to the band
+// workspace (C49).  For tiny rows FastRow::goff holds log2 M and FastRow::wpad the band offset.
+// --------------------------------------------------------------------------------------------------
+template <int M, bool FORWARD>
+__device__ __forceinline__ void tiny_row(const FastRow &row, const float2 *__restrict__ X, const float *__restrict__ fwin,
+                                         float2 *__restrict__ Y, float2 *__restrict__ Gb, int nbins, float scale) {
+  float2 v[M];
+  const float *W = fwin + row.woff + row.dk;
+  if constexpr (FORWARD) {
+#pragma unroll
+    for (int j = 0; j < M; ++j) {
+      const int jj = j < M / 2 ? j : j - M;
+      v[j] = make_float2(0.f, 0.f);
+      if (jj >= -row.dk && jj <= row.dk) v[j] = pscale(X[row.kc + jj], __ldg(W + jj) * scale);
+    }
+    RegFFT<M, +1>::run(v);
+    float4 *dst = reinterpret_cast<float4 *>(Y);
+#pragma unroll
+    for (int j = 0; j < M / 2; ++j) __stcs(dst + j, make_float4(v[2 * j].x, v[2 * j].y, v[2 * j + 1].x, v[2 * j + 1].y));
+  } else {
+    const float4 *src = reinterpret_cast<const float4 *>(Y);
+#pragma unroll
+    for (int j = 0; j < M / 2; ++j) {
+      const float4 q = __ldcs(src + j);
+      v[2 * j] = make_float2(q.x, q.y); v[2 * j + 1] = make_float2(q.z, q.w);
+    }
+    RegFFT<M, -1>::run(v);
+#pragma unroll
+    for (int j = 0; j < M; ++j) {
+      const int jj = j < M / 2 ? j : j - M;
+      const int f = row.kc + jj;
+      if (jj >= -row.dk && jj <= row.dk && (unsigned)f < (unsigned)nbins) Gb[jj] = pscale(v[j], __ldg(W + jj) * scale);
+    }
+  }
+}
+
+template <bool FORWARD>
+__device__ __forceinline__ void tiny_dispatch(long long id, const FastRow *__restrict__ tiny, int n_tiny,
+                                              const float *__restrict__ fwin, const float2 *__restrict__ spec,
+                                              long long xstride, int nbins, float2 *__restrict__ coef, long long ctot,
+                                              float2 *__restrict__ band, long long sumL, int plane, float n_samples) {
+  const int seg = (int)(id / n_tiny);
+  const FastRow row = tiny[id - (long long)seg * n_tiny];
+  if (!FORWARD && plane >= 0 && row.plane != plane) return;
+  const float2 *X = spec + (size_t)seg * xstride;
+  float2 *Y = coef + (size_t)seg * ctot + row.offset;
+  float2 *Gb = band + (size_t)seg * sumL + row.wpad + row.dk;
+  const float Mf = (float)(1 << row.goff);
+  const float scale = FORWARD ? rsqrtf(n_samples * Mf) : sqrtf(n_samples / Mf);
+  switch (row.goff) {
+    case 2: tiny_row<4, FORWARD>(row, X, fwin, Y, Gb, nbins, scale); break;
+    case 3: tiny_row<8, FORWARD>(row, X, fwin, Y, Gb, nbins, scale); break;
+    case 4: tiny_row<16, FORWARD>(row, X, fwin, Y, Gb, nbins, scale); break;
+    default: break;
+  }
+}
+
+template <bool FORWARD>
+__global__ void __launch_bounds__(128)
+k_tiny_rows(const FastRow *__restrict__ tiny, int n_tiny, const float *__restrict__ fwin,
+            const float2 *__restrict__ spec, long long xstride, int nbins, float2 *__restrict__ coef,
+            long long ctot, float2 *__restrict__ band, long long sumL, int batch, int plane, float n_samples) {
+  const long long id = (long long)blockIdx.x * 128 + threadIdx.x;
+  if (id >= (long long)n_tiny * batch) return;
+  tiny_dispatch<FORWARD>(id, tiny, n_tiny, fwin, spec, xstride, nbins, coef, ctot, band, sumL, plane, n_samples);
+}
+
+// --------------------------------------------------------------------------------------------------
 // K2 / K3: rows.  Work items are ordered bucket-major (largest M first), then segment, then row group;
 // a CTA takes NWARPS consecutive items, i.e. neighbouring rows of one segment, so that the bands its
 // warps read overlap in L1.
@@ -143,7 +213,7 @@ k_rows_fast(FastParams P, const FastRow *frows, const void *__restrict__ tw1g_,
             const float *__restrict__ fwin, const float *__restrict__ fwinp,
             const float2 *__restrict__ spec, long long xstride, int nbins,
             float2 *__restrict__ coef, long long ctot, float2 *__restrict__ band, long long sumL,
-            int batch, int plane) {
+            int batch, int plane, const FastRow *__restrict__ tiny, int n_tiny, float n_samples) {
   typedef float2 TW;
   const TW *tw1g = static_cast<const TW *>(tw1g_);
   TW *tw1s = reinterpret_cast<TW *>(qtam_fast_smem);
@@ -158,6 +228,12 @@ k_rows_fast(FastParams P, const FastRow *frows, const void *__restrict__ tw1g_,
     frows = reinterpret_cast<const FastRow *>(dst);
   }
   __syncthreads();
+  // rows shorter than 32 points ride along, one thread per (segment, row) (n_tiny = 0: separate launch)
+  if constexpr (FORWARD) {
+    const long long id = (long long)blockIdx.x * (NWARPS * 32) + threadIdx.x;
+    if (id < (long long)n_tiny * batch)
+      tiny_dispatch<true>(id, tiny, n_tiny, fwin, spec, xstride, nbins, coef, ctot, band, sumL, -1, n_samples);
+  }
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   float2 *ex = exall + warp * kExPerWarp;
   // (the host keeps groups_per_seg * batch below 2^31)
@@ -280,8 +356,9 @@ qtam_status fast_r2c(qtam_plan *p, const void *d_x, int batch, cudaStream_t st) 
 
 template <int NW, bool FORWARD>
 static qtam_status rows_launch_nw(qtam_plan *p, int batch, const void *d_coef_in, void *d_coef_out, int plane,
-                                  cudaStream_t st) {
+                                  cudaStream_t st, bool *tiny_rode) {
   const FastParams &P = p->fast;
+  if (tiny_rode) *tiny_rode = false;
   if (P.groups_per_seg == 0) return QTAM_OK;
   const size_t smem = sizeof(float2) * (size_t)((P.tw_total + 1) & ~1) + sizeof(float2) * (size_t)NW * kExPerWarp +
                       sizeof(FastRow) * (size_t)P.rows_smem;
@@ -297,7 +374,9 @@ static qtam_status rows_launch_nw(qtam_plan *p, int batch, const void *d_coef_in
   // a few waves of resident CTAs, each looping: keeps the tail short without losing the twiddle preload
   int grid = (int)(want < resident * 4 ? want : resident * 4);
   if (grid < 1) grid = 1;
-  const double bytes = FORWARD ? (double)batch * 8.0 * (P.sum_M + (double)p->hp.nb)
+  // the forward launch also takes the rows shorter than 32 points when its grid has a thread for each
+  const bool ride = FORWARD && p->n_tiny > 0 && (long long)grid * NW * 32 >= (long long)p->n_tiny * batch;
+  const double bytes = FORWARD ? (double)batch * 8.0 * (P.sum_M + (double)p->hp.nb + (ride ? p->tiny_sumM : 0.0))
                                : (double)batch * 8.0 * (P.sum_M + P.sum_L);
   {
     LaunchScope ls(p, st, FORWARD ? K_FWD_ROWS_FAST : K_INV_ROWS_FAST, bytes);
@@ -307,9 +386,11 @@ static qtam_status rows_launch_nw(qtam_plan *p, int batch, const void *d_coef_in
         static_cast<const float2 *>(p->d_spec), p->xstride,
         (int)p->hp.nb,
         FORWARD ? static_cast<float2 *>(d_coef_out) : const_cast<float2 *>(static_cast<const float2 *>(d_coef_in)),
-        p->hp.ctot, static_cast<float2 *>(p->d_band), p->hp.sumL, batch, plane);
+        p->hp.ctot, static_cast<float2 *>(p->d_band), p->hp.sumL, batch, plane, p->d_tiny, ride ? p->n_tiny : 0,
+        (float)p->hp.N);
   }
   QTAM_LAUNCH_CHECK();
+  if (tiny_rode) *tiny_rode = ride;
   return QTAM_OK;
 }
 
@@ -324,23 +405,43 @@ static int row_warps() {
 
 template <bool FORWARD>
 static qtam_status rows_launch(qtam_plan *p, int batch, const void *d_coef_in, void *d_coef_out, int plane,
-                               cudaStream_t st) {
+                               cudaStream_t st, bool *tiny_rode) {
   switch (row_warps()) {
-    case 4: return rows_launch_nw<4, FORWARD>(p, batch, d_coef_in, d_coef_out, plane, st);
-    case 12: return rows_launch_nw<12, FORWARD>(p, batch, d_coef_in, d_coef_out, plane, st);
-    case 16: return rows_launch_nw<16, FORWARD>(p, batch, d_coef_in, d_coef_out, plane, st);
-    case 20: return rows_launch_nw<20, FORWARD>(p, batch, d_coef_in, d_coef_out, plane, st);
-    case 24: return rows_launch_nw<24, FORWARD>(p, batch, d_coef_in, d_coef_out, plane, st);
-    default: return rows_launch_nw<8, FORWARD>(p, batch, d_coef_in, d_coef_out, plane, st);
+    case 4: return rows_launch_nw<4, FORWARD>(p, batch, d_coef_in, d_coef_out, plane, st, tiny_rode);
+    case 12: return rows_launch_nw<12, FORWARD>(p, batch, d_coef_in, d_coef_out, plane, st, tiny_rode);
+    case 16: return rows_launch_nw<16, FORWARD>(p, batch, d_coef_in, d_coef_out, plane, st, tiny_rode);
+    case 20: return rows_launch_nw<20, FORWARD>(p, batch, d_coef_in, d_coef_out, plane, st, tiny_rode);
+    case 24: return rows_launch_nw<24, FORWARD>(p, batch, d_coef_in, d_coef_out, plane, st, tiny_rode);
+    default: return rows_launch_nw<8, FORWARD>(p, batch, d_coef_in, d_coef_out, plane, st, tiny_rode);
   }
 }
 
+template <bool FORWARD>
+static qtam_status tiny_launch(qtam_plan *p, int batch, const void *d_coef, int plane, cudaStream_t st) {
+  if (p->n_tiny == 0) return QTAM_OK;
+  const long long total = (long long)p->n_tiny * batch;
+  {
+    LaunchScope ls(p, st, FORWARD ? K_TINY_FWD : K_TINY_INV, (double)batch * 8.0 * (p->tiny_sumM + p->tiny_sumL));
+    k_tiny_rows<FORWARD><<<(unsigned)((total + 127) / 128), 128, 0, st>>>(
+        p->d_tiny, p->n_tiny, static_cast<const float *>(p->d_fwin), static_cast<const float2 *>(p->d_spec),
+        p->xstride, (int)p->hp.nb, const_cast<float2 *>(static_cast<const float2 *>(d_coef)), p->hp.ctot,
+        static_cast<float2 *>(p->d_band), p->hp.sumL, batch, plane, (float)p->hp.N);
+  }
+  QTAM_LAUNCH_CHECK();
+  return QTAM_OK;
+}
+
 qtam_status fast_forward_rows(qtam_plan *p, int batch, void *d_coef, cudaStream_t st) {
-  return rows_launch<true>(p, batch, nullptr, d_coef, -1, st);
+  bool rode = false;
+  const qtam_status s = rows_launch<true>(p, batch, nullptr, d_coef, -1, st, &rode);
+  if (s != QTAM_OK || rode) return s;
+  return tiny_launch<true>(p, batch, d_coef, -1, st);
 }
 
 qtam_status fast_inverse_rows(qtam_plan *p, const void *d_coef, int batch, int plane, cudaStream_t st) {
-  return rows_launch<false>(p, batch, d_coef, nullptr, plane, st);
+  const qtam_status s = rows_launch<false>(p, batch, d_coef, nullptr, plane, st, nullptr);
+  if (s != QTAM_OK) return s;
+  return tiny_launch<false>(p, batch, d_coef, plane, st);
 }
 
 template <int LOG2NC>
