@@ -46,7 +46,7 @@ void free_plan(qtam_plan *p) {
   cudaFree(p->d_bigrows); cudaFree(p->d_spec_alloc); cudaFree(p->d_ws); cudaFree(p->d_band);
   cudaFree(p->d_fwinp); cudaFree(p->d_red);
   cudaFree(p->d_frows); cudaFree(p->d_fwin); cudaFree(p->d_ftw_fwd); cudaFree(p->d_ftw_inv);
-  cudaFree(p->d_tiny); cudaFree(p->d_ptw);
+  cudaFree(p->d_tiny); cudaFree(p->d_ptw); cudaFree(p->d_frows_fwd); cudaFree(p->d_fmem); cudaFree(p->d_tmem);
   cudaFree(p->d_thr_tasks); cudaFree(p->d_thr_offs);
   for (int c = 0; c < 4; ++c) { cudaFree(p->d_cta_rowidx[c]); cudaFree(p->d_ptw_rows[c]); }
   for (int b = 0; b < 3; ++b) cudaFree(p->d_twb[b]);
@@ -110,12 +110,22 @@ qtam_status build_fast(qtam_plan *p) {
   };
   std::vector<FastRow> frows;
   std::vector<int4> red;
+  // forward table: rows of one bucket with the same centre bin and half-width (the clamped rows of
+  // different Q-planes, A7/A8 :307-311: one window for all of them) have identical coefficients, so
+  // the forward transforms one "leader" per such set and stores the result at every member's offset.
+  // Leader records reuse FastRow: plane = number of members, pad = first entry in the member table.
+  FastParams &FF = p->fast_fwd;
+  std::memset(&FF, 0, sizeof(FF));
+  std::vector<FastRow> frowsF;
+  std::vector<int> fmem;
   std::vector<float> twf, twi;   // (wx, wy) per entry
   const long double tau = 6.283185307179586476925286766559005768L;
   for (int lg = 5; lg >= 0; --lg) {
     const int G = 1 << lg, M = 32 * G, Fr = 32 / G;
     FastBucket B{};
     B.log2G = lg; B.row_base = (int)frows.size(); B.tw_base = (int)(twf.size() / 2);
+    std::vector<FastRow> leaders;
+    std::vector<std::vector<int>> members;
     for (size_t k = 0; k < hp.rows.size(); ++k) {
       const HostRow &h = hp.rows[k];
       if (h.M != M) continue;
@@ -123,6 +133,12 @@ qtam_status build_fast(qtam_plan *p) {
       r.kc = (int)h.kc; r.dk = (int)h.dk; r.woff = window_of(h); r.goff = (int)h.goff;
       r.offset = (int)h.offset; r.plane = h.plane; r.wpad = wpad_of(h);
       frows.push_back(r);
+      {
+        size_t l = 0;
+        while (l < leaders.size() && !(leaders[l].kc == r.kc && leaders[l].dk == r.dk)) ++l;
+        if (l == leaders.size()) { leaders.push_back(r); members.emplace_back(); }
+        members[l].push_back(r.offset);
+      }
       {
         const int64_t lo = h.kc - h.dk;
         const int64_t jb = lo < 0 ? -lo : 0, je = std::min<int64_t>(h.L, hp.nb - lo);
@@ -133,6 +149,16 @@ qtam_status build_fast(qtam_plan *p) {
     B.nrows = (int)frows.size() - B.row_base;
     if (B.nrows == 0) continue;
     B.ngroups = (B.nrows + Fr - 1) / Fr;
+    FastBucket BF = B;
+    BF.row_base = (int)frowsF.size();
+    BF.nrows = (int)leaders.size();
+    BF.ngroups = (BF.nrows + Fr - 1) / Fr;
+    for (size_t l = 0; l < leaders.size(); ++l) {
+      leaders[l].plane = (int)members[l].size();
+      leaders[l].pad = (int)fmem.size();
+      fmem.insert(fmem.end(), members[l].begin(), members[l].end());
+      frowsF.push_back(leaders[l]);
+    }
     const double sf = 1.0 / std::sqrt((double)hp.N * (double)M), si = std::sqrt((double)hp.N / (double)M);
     for (int n1 = 0; n1 < 32; ++n1)
       for (int t = 0; t < G; ++t) {
@@ -144,9 +170,13 @@ qtam_status build_fast(qtam_plan *p) {
       }
     F.groups_per_seg += B.ngroups;
     F.b[F.nbuckets++] = B;
+    FF.groups_per_seg += BF.ngroups;
+    FF.b[FF.nbuckets++] = BF;
   }
   F.tw_total = (int)(twf.size() / 2);
   F.rows_smem = frows.size() <= 1024 ? (int)frows.size() : 0;
+  FF.tw_total = F.tw_total; FF.sum_M = F.sum_M; FF.sum_L = F.sum_L;
+  FF.rows_smem = frowsF.size() <= 1024 ? (int)frowsF.size() : 0;
   // rows shorter than 32 points
   std::vector<FastRow> tiny;
   for (size_t k = 0; k < hp.rows.size(); ++k) {
@@ -163,6 +193,8 @@ qtam_status build_fast(qtam_plan *p) {
   if (hp.ctot >= (int64_t(1) << 31)) return QTAM_ERR_UNSUPPORTED;
   if (!upload(&p->d_frows, frows.data(), frows.size(), tot)) return QTAM_ERR_ALLOC;
   p->h_frows = frows;
+  if (!upload(&p->d_frows_fwd, frowsF.data(), frowsF.size(), tot)) return QTAM_ERR_ALLOC;
+  if (!upload(&p->d_fmem, fmem.data(), fmem.size(), tot)) return QTAM_ERR_ALLOC;
   float *d = nullptr;
   if (!upload(&d, fwin.data(), fwin.size(), tot)) return QTAM_ERR_ALLOC;
   p->d_fwin = d;

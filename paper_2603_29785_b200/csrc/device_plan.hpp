@@ -77,6 +77,10 @@ struct qtam_plan {
   int num_sms = 148;
   qtam::FastParams fast{};
   qtam::FastRow *d_frows = nullptr;
+  qtam::FastParams fast_fwd{};        // forward: one leader per set of identical rows (same kc, dk)
+  qtam::FastRow *d_frows_fwd = nullptr;   // leaders: plane = number of members, pad = first entry in d_fmem
+  int *d_fmem = nullptr;              // coefficient offsets of the members
+  int2 *d_tmem = nullptr;             // tiled inverse: (coefficient offset, plane) of the members
   void *d_fwin = nullptr;      // float windows, one per distinct half-width
   void *d_fwinp = nullptr;     // float windows zero-padded to M points in M-array order (index j mod M)
   int4 *d_red = nullptr;       // per fast row (frows order): first bin, bins, first band index (R8 clip), plane

@@ -136,7 +136,7 @@ __device__ QTAM_GROUP_INLINE void fwd_group(const FastBucket &B, const FastRow *
                                        int lane, float2 *ex, const float2 *tw1,
                                        const float2 *__restrict__ spec, long long xstride,
                                        const float *__restrict__ fwinp, float2 *__restrict__ coef,
-                                       long long ctot) {
+                                       long long ctot, const int *__restrict__ fmem) {
   constexpr int G = 1 << LOG2G, F = 32 / G, M = 32 * G;
   const int t = lane & (G - 1), rw = lane >> LOG2G;
   const int r = grp * F + rw;
@@ -163,11 +163,15 @@ __device__ QTAM_GROUP_INLINE void fwd_group(const FastBucket &B, const FastRow *
   }
   RowFFT<LOG2G, +1>::run(v, ex, tw1, lane);
   if (valid) {
-    float2 *dst = coef + (size_t)seg * ctot + row.offset + t;
+    // every member of the leader's set (rows with this centre bin and half-width) gets the same values
+#pragma unroll 1
+    for (int m = 0; m < row.plane; ++m) {
+      float2 *dst = coef + (size_t)seg * ctot + __ldg(fmem + row.pad + m) + t;
 #pragma unroll
-    for (int i = 0; i < F; ++i)
+      for (int i = 0; i < F; ++i)
 #pragma unroll
-      for (int n2 = 0; n2 < G; ++n2) __stcs(dst + G * i + 32 * n2, v[i * G + n2]);
+        for (int n2 = 0; n2 < G; ++n2) __stcs(dst + G * i + 32 * n2, v[i * G + n2]);
+    }
   }
 }
 
@@ -213,7 +217,8 @@ k_rows_fast(FastParams P, const FastRow *frows, const void *__restrict__ tw1g_,
             const float *__restrict__ fwin, const float *__restrict__ fwinp,
             const float2 *__restrict__ spec, long long xstride, int nbins,
             float2 *__restrict__ coef, long long ctot, float2 *__restrict__ band, long long sumL,
-            int batch, int plane, const FastRow *__restrict__ tiny, int n_tiny, float n_samples) {
+            int batch, int plane, const FastRow *__restrict__ tiny, int n_tiny, float n_samples,
+            const int *__restrict__ fmem) {
   typedef float2 TW;
   const TW *tw1g = static_cast<const TW *>(tw1g_);
   TW *tw1s = reinterpret_cast<TW *>(qtam_fast_smem);
@@ -252,7 +257,7 @@ k_rows_fast(FastParams P, const FastRow *frows, const void *__restrict__ tw1g_,
     const TW *tw1 = tw1s + B.tw_base;
 #define QTAM_ROW_CASE(L)                                                                              \
   case L:                                                                                             \
-    if constexpr (FORWARD) fwd_group<L>(B, frows, seg, grp, lane, ex, tw1, spec, xstride, fwinp, coef, ctot); \
+    if constexpr (FORWARD) fwd_group<L>(B, frows, seg, grp, lane, ex, tw1, spec, xstride, fwinp, coef, ctot, fmem); \
     else inv_group<L>(B, frows, seg, grp, lane, ex, tw1, coef, ctot, nbins, fwin, band, sumL, plane);  \
     break;
     switch (B.log2G) {
@@ -357,7 +362,7 @@ qtam_status fast_r2c(qtam_plan *p, const void *d_x, int batch, cudaStream_t st) 
 template <int NW, bool FORWARD>
 static qtam_status rows_launch_nw(qtam_plan *p, int batch, const void *d_coef_in, void *d_coef_out, int plane,
                                   cudaStream_t st, bool *tiny_rode) {
-  const FastParams &P = p->fast;
+  const FastParams &P = FORWARD ? p->fast_fwd : p->fast;
   if (tiny_rode) *tiny_rode = false;
   if (P.groups_per_seg == 0) return QTAM_OK;
   const size_t smem = sizeof(float2) * (size_t)((P.tw_total + 1) & ~1) + sizeof(float2) * (size_t)NW * kExPerWarp +
@@ -381,13 +386,13 @@ static qtam_status rows_launch_nw(qtam_plan *p, int batch, const void *d_coef_in
   {
     LaunchScope ls(p, st, FORWARD ? K_FWD_ROWS_FAST : K_INV_ROWS_FAST, bytes);
     kern<<<grid, NW * 32, smem, st>>>(
-        P, p->d_frows, static_cast<const void *>(FORWARD ? p->d_ftw_fwd : p->d_ftw_inv),
+        P, FORWARD ? p->d_frows_fwd : p->d_frows, static_cast<const void *>(FORWARD ? p->d_ftw_fwd : p->d_ftw_inv),
         static_cast<const float *>(p->d_fwin), static_cast<const float *>(p->d_fwinp),
         static_cast<const float2 *>(p->d_spec), p->xstride,
         (int)p->hp.nb,
         FORWARD ? static_cast<float2 *>(d_coef_out) : const_cast<float2 *>(static_cast<const float2 *>(d_coef_in)),
         p->hp.ctot, static_cast<float2 *>(p->d_band), p->hp.sumL, batch, plane, p->d_tiny, ride ? p->n_tiny : 0,
-        (float)p->hp.N);
+        (float)p->hp.N, p->d_fmem);
   }
   QTAM_LAUNCH_CHECK();
   if (tiny_rode) *tiny_rode = ride;

@@ -48,16 +48,33 @@ qtam_status build_inv_tiled(qtam_plan *p) {
   const int max_pass = getenv("QTAM_TILE_PASSES") ? atoi(getenv("QTAM_TILE_PASSES")) : 8;
   std::vector<TileRow> trows;
   std::vector<TileItem> items;
+  std::vector<int2> tmem;                 // (coefficient offset, plane) of every member
+  std::vector<int> item_members;          // members per item, for the schedule
   for (int q = 0; q < F.nbuckets; ++q) {
     const FastBucket &B = F.b[q];
     const int G = 1 << B.log2G, Fr = 32 / G;
-    std::vector<FastRow> rows(p->h_frows.begin() + B.row_base, p->h_frows.begin() + B.row_base + B.nrows);
-    std::stable_sort(rows.begin(), rows.end(), [](const FastRow &a, const FastRow &b) { return a.kc < b.kc; });
+    std::vector<FastRow> all(p->h_frows.begin() + B.row_base, p->h_frows.begin() + B.row_base + B.nrows);
+    std::stable_sort(all.begin(), all.end(), [](const FastRow &a, const FastRow &b) {
+      return a.kc != b.kc ? a.kc < b.kc : a.dk < b.dk;
+    });
+    // rows with the same centre bin and half-width (the clamped rows of different Q-planes) share their
+    // window and their place in the spectrum: by linearity their coefficient rows are added before ONE
+    // transform.  `rows` = one leader per such set; pad0 / pad1 = first member / number of members.
+    std::vector<FastRow> rows;
+    for (size_t i = 0; i < all.size(); ++i) {
+      if (rows.empty() || rows.back().kc != all[i].kc || rows.back().dk != all[i].dk) {
+        rows.push_back(all[i]);
+        rows.back().pad = (int)tmem.size();
+        rows.back().goff = 0;            // member count
+      }
+      tmem.push_back(make_int2(all[i].offset, all[i].plane));
+      rows.back().goff += 1;
+    }
     size_t i = 0;
     while (i < rows.size()) {
       TileItem it{};
       it.row0 = (int)trows.size(); it.log2G = B.log2G; it.tw_base = B.tw_base;
-      int lo = 1 << 30, hi = -(1 << 30);
+      int lo = 1 << 30, hi = -(1 << 30), nmem = 0;
       while (i < rows.size() && it.npass < max_pass) {
         const size_t e = std::min(rows.size(), i + (size_t)Fr);
         int lo2 = lo, hi2 = hi;
@@ -77,6 +94,8 @@ qtam_status build_inv_tiled(qtam_plan *p) {
           t.kc = rows[r].kc; t.offset = rows[r].offset; t.wpad = rows[r].wpad; t.plane = rows[r].plane;
           t.jlo = std::max(-rows[r].dk, -rows[r].kc);
           t.jhi = std::min(rows[r].dk, (int)hp.nb - 1 - rows[r].kc);
+          t.pad0 = rows[r].pad; t.pad1 = rows[r].goff;
+          nmem += rows[r].goff;
           trows.push_back(t);
         }
         it.npass += 1; it.nrows += (int)(e - i);
@@ -85,12 +104,23 @@ qtam_status build_inv_tiled(qtam_plan *p) {
       if (hi < lo) { lo = 0; hi = -1; }
       it.lo = lo; it.nb = hi - lo + 1;
       items.push_back(it);
+      item_members.push_back(nmem);
     }
   }
   // heaviest items first: the dynamic schedule then ends on the short ones
-  std::stable_sort(items.begin(), items.end(), [](const TileItem &a, const TileItem &b) {
-    return a.npass * (10 + a.log2G) > b.npass * (10 + b.log2G);
-  });
+  {
+    // weight = transforms + member rows to load (both in units of one pass of the bucket)
+    std::vector<size_t> order(items.size());
+    for (size_t i = 0; i < order.size(); ++i) order[i] = i;
+    auto weight = [&](size_t i) {
+      const int Fr = 32 >> items[i].log2G;
+      return items[i].npass * (10 + items[i].log2G) + 6 * ((item_members[i] + Fr - 1) / Fr);
+    };
+    std::stable_sort(order.begin(), order.end(), [&](size_t a, size_t b) { return weight(a) > weight(b); });
+    std::vector<TileItem> sorted;
+    for (size_t i : order) sorted.push_back(items[i]);
+    items.swap(sorted);
+  }
   int64_t off = 0;
   for (TileItem &it : items) { it.part_off = (int)off; off += (it.nb + 1) & ~1; }   // 16-byte aligned slots
   if (off * (int64_t)p->max_batch >= (int64_t(1) << 40)) return QTAM_OK;
@@ -105,6 +135,7 @@ qtam_status build_inv_tiled(qtam_plan *p) {
   };
   if (!up(reinterpret_cast<void **>(&p->d_trows), trows.data(), trows.size() * sizeof(TileRow))) return QTAM_ERR_ALLOC;
   if (!up(reinterpret_cast<void **>(&p->d_titems), items.data(), items.size() * sizeof(TileItem))) return QTAM_ERR_ALLOC;
+  if (!up(reinterpret_cast<void **>(&p->d_tmem), tmem.data(), tmem.size() * sizeof(int2))) return QTAM_ERR_ALLOC;
   if (!up(&p->d_part, nullptr, sizeof(float2) * (size_t)p->max_batch * (size_t)off)) return QTAM_ERR_ALLOC;
   if (!up(reinterpret_cast<void **>(&p->d_counter), nullptr, 256)) return QTAM_ERR_ALLOC;
   p->tiled_inv = true;
@@ -118,20 +149,38 @@ qtam_status build_inv_tiled(qtam_plan *p) {
 template <int LOG2G>
 __device__ __forceinline__ void tile_pass(const TileItem &it, const TileRow *__restrict__ trows, int pass, int lane,
                                           float2 *ex, const float2 *tw1, const float2 *__restrict__ Yseg,
-                                          const float *__restrict__ fwinp, int plane, float2 *acc) {
+                                          const float *__restrict__ fwinp, int plane, float2 *acc,
+                                          const int2 *__restrict__ tmem) {
   constexpr int G = 1 << LOG2G, F = 32 / G, M = 32 * G;
   const int t = lane & (G - 1), rw = lane >> LOG2G;
   const int r = pass * F + rw;
   const bool inb = r < it.nrows;
   // lanes past the end of the tile recompute its last row and contribute nothing
   TileRow row = trows[it.row0 + (inb ? r : it.nrows - 1)];
-  const bool active = inb && (plane < 0 || row.plane == plane) && row.jlo <= row.jhi;
+  // members of the leader's set that take part (all of them, or those of the requested plane)
+  int nmatch = 0;
+  if (inb && row.jlo <= row.jhi) {
+    if (plane < 0) nmatch = row.pad1;
+    else for (int m = 0; m < row.pad1; ++m) nmatch += (__ldg(&tmem[row.pad0 + m].y) == plane) ? 1 : 0;
+  }
+  const bool active = nmatch > 0;
   if (__ballot_sync(0xffffffffu, active) == 0u) return;
-  if (!active) { row.jlo = 1; row.jhi = 0; }
-  const float2 *Y = Yseg + row.offset + t;
+  if (!active) { row.jlo = 1; row.jhi = 0; row.pad1 = 0; }
   float2 v[32];
 #pragma unroll
-  for (int j1 = 0; j1 < 32; ++j1) v[j1] = __ldcs(Y + G * j1);
+  for (int j1 = 0; j1 < 32; ++j1) v[j1] = make_float2(0.f, 0.f);
+  // sum of the members' coefficient rows (linearity of the transform; Eq. 11's sum over k)
+#pragma unroll 1
+  for (int m = 0; m < row.pad1; ++m) {
+    const int2 mb = __ldg(tmem + row.pad0 + m);
+    if (plane >= 0 && mb.y != plane) continue;
+    const float2 *Y = Yseg + mb.x + t;
+    float2 y[32];
+#pragma unroll
+    for (int j1 = 0; j1 < 32; ++j1) y[j1] = __ldcs(Y + G * j1);
+#pragma unroll
+    for (int j1 = 0; j1 < 32; ++j1) v[j1] = padd(v[j1], y[j1]);
+  }
   RowFFT<LOG2G, -1>::run(v, ex, tw1, lane);
   // G_k[jj] = Bhat_k[jj] W_k[jj] (C49); the window table is stored at the M-array index of the FFT output
   const float *W = fwinp + row.wpad + t;
@@ -179,7 +228,8 @@ __global__ void __launch_bounds__(NW * 32, 1)
 k_inv_tiles(const TileItem *__restrict__ items, int n_items, const TileRow *__restrict__ trows,
             const float2 *__restrict__ tw1g, int tw_total, const float *__restrict__ fwinp,
             const float2 *__restrict__ coef, long long ctot, int batch, int plane,
-            float2 *__restrict__ part, long long part_stride, unsigned int *__restrict__ counter) {
+            float2 *__restrict__ part, long long part_stride, unsigned int *__restrict__ counter,
+            const int2 *__restrict__ tmem) {
   float2 *tw1s = reinterpret_cast<float2 *>(qtam_tiled_smem);
   float2 *warp_base = tw1s + ((tw_total + 1) & ~1);
   for (int i = threadIdx.x; i < tw_total; i += NW * 32) tw1s[i] = tw1g[i];
@@ -210,7 +260,7 @@ k_inv_tiles(const TileItem *__restrict__ items, int n_items, const TileRow *__re
 #define QTAM_TILE_CASE(L)                                                                      \
   case L:                                                                                      \
     _Pragma("unroll 1") for (int pass = 0; pass < it.npass; ++pass)                            \
-        tile_pass<L>(it, trows, pass, lane, ex, tw1, Yseg, fwinp, plane, acc);                 \
+        tile_pass<L>(it, trows, pass, lane, ex, tw1, Yseg, fwinp, plane, acc, tmem);           \
     break;
     switch (it.log2G) {
       QTAM_TILE_CASE(5) QTAM_TILE_CASE(4) QTAM_TILE_CASE(3) QTAM_TILE_CASE(2) QTAM_TILE_CASE(1) QTAM_TILE_CASE(0)
@@ -375,7 +425,7 @@ static qtam_status tiles_launch(qtam_plan *p, const void *d_coef, int batch, int
     kern<<<(int)grid, NW * 32, smem, st>>>(
         p->d_titems, p->n_titems, p->d_trows, static_cast<const float2 *>(p->d_ftw_inv), twt,
         static_cast<const float *>(p->d_fwinp), static_cast<const float2 *>(d_coef), p->hp.ctot, batch, plane,
-        static_cast<float2 *>(p->d_part), p->part_stride, p->d_counter);
+        static_cast<float2 *>(p->d_part), p->part_stride, p->d_counter, p->d_tmem);
   }
   QTAM_LAUNCH_CHECK();
   return QTAM_OK;
