@@ -161,12 +161,15 @@ __device__ QTAM_GROUP_INLINE void fwd_group(const FastBucket &B, const FastRow *
       v[j1] = make_float2(xv.x * w, xv.y * w);
     }
   }
+  // the first member's offset is fetched before the transform, every further one an iteration ahead
+  int moff = __ldg(fmem + row.pad);
   RowFFT<LOG2G, +1>::run(v, ex, tw1, lane);
   if (valid) {
     // every member of the leader's set (rows with this centre bin and half-width) gets the same values
 #pragma unroll 1
     for (int m = 0; m < row.plane; ++m) {
-      float2 *dst = coef + (size_t)seg * ctot + __ldg(fmem + row.pad + m) + t;
+      float2 *dst = coef + (size_t)seg * ctot + moff + t;
+      if (m + 1 < row.plane) moff = __ldg(fmem + row.pad + m + 1);
 #pragma unroll
       for (int i = 0; i < F; ++i)
 #pragma unroll
@@ -377,7 +380,8 @@ static qtam_status rows_launch_nw(qtam_plan *p, int batch, const void *d_coef_in
   long long want = (total + NW - 1) / NW;
   const long long resident = (long long)p->num_sms * occ;
   // a few waves of resident CTAs, each looping: keeps the tail short without losing the twiddle preload
-  int grid = (int)(want < resident * 4 ? want : resident * 4);
+  static const int waves = getenv("QTAM_ROW_WAVES") ? atoi(getenv("QTAM_ROW_WAVES")) : 1;
+  int grid = (int)(want < resident * waves ? want : resident * waves);
   if (grid < 1) grid = 1;
   // the forward launch also takes the rows shorter than 32 points when its grid has a thread for each
   const bool ride = FORWARD && p->n_tiny > 0 && (long long)grid * NW * 32 >= (long long)p->n_tiny * batch;
