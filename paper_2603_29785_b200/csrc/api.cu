@@ -41,14 +41,14 @@ void free_plan(qtam_plan *p) {
   if (!p) return;
   if (p->host_only) { delete p; return; }
   cudaFree(p->d_rows); cudaFree(p->d_win); cudaFree(p->d_tw); cudaFree(p->d_invP);
-  cudaFree(p->d_csr_ptr); cudaFree(p->d_csr_idx);
+  cudaFree(p->d_csr_ptr); cudaFree(p->d_csr_idx); cudaFree(p->d_csrj_ptr); cudaFree(p->d_csrj_idx);
   for (int c = 0; c < qtam_plan::kClasses; ++c) cudaFree(p->d_items[c]);
   cudaFree(p->d_bigrows); cudaFree(p->d_spec_alloc); cudaFree(p->d_ws); cudaFree(p->d_band);
   cudaFree(p->d_fwinp); cudaFree(p->d_red);
   cudaFree(p->d_frows); cudaFree(p->d_fwin); cudaFree(p->d_ftw_fwd); cudaFree(p->d_ftw_inv);
   cudaFree(p->d_tiny); cudaFree(p->d_ptw); cudaFree(p->d_frows_fwd); cudaFree(p->d_fmem); cudaFree(p->d_tmem);
   cudaFree(p->d_thr_tasks); cudaFree(p->d_thr_offs);
-  for (int c = 0; c < 4; ++c) { cudaFree(p->d_cta_rowidx[c]); cudaFree(p->d_ptw_rows[c]); }
+  for (int c = 0; c < 4; ++c) { cudaFree(p->d_cta_rowidx[c]); cudaFree(p->d_ptw_rows[c]); cudaFree(p->d_cta_memptr[c]); cudaFree(p->d_cta_mem[c]); }
   for (int b = 0; b < 3; ++b) cudaFree(p->d_twb[b]);
   cudaFree(p->d_trows); cudaFree(p->d_titems); cudaFree(p->d_part); cudaFree(p->d_counter);
   for (ProfRec &r : p->prof_pool) { cudaEventDestroy(r.e0); cudaEventDestroy(r.e1); }

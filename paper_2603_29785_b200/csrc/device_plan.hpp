@@ -34,6 +34,7 @@ struct ThrTask { int log2M, row0, nrows, pad; };
 constexpr int kThrFastLog2Max = 10;
 // CTA-level rows (rows_cta.cu): 2^11 .. 2^14 points in one shared-memory transform, up to 2^17 in 2, 4 or 8
 constexpr int kCtaLog2Min = 11, kCtaLog2Max = 17;
+constexpr int kCtaMaxMembers = 32;   // rows per leader (same centre bin and half-width) in rows_cta.cu
 struct ProfRec { int kid; double bytes; cudaEvent_t e0, e1; };
 }  // namespace qtam
 
@@ -54,6 +55,10 @@ struct qtam_plan {
   void *d_invP = nullptr;      // real[(nP+1)*nb], 0 outside the cover set
   int32_t *d_csr_ptr = nullptr;
   int32_t *d_csr_idx = nullptr;
+  // joint-inverse CSR without the band slots of follower rows (rows_cta.cu adds a set of identical rows
+  // into its leader's slot); one set per bin.  Null when the plan has no followers.
+  int32_t *d_csrj_ptr = nullptr;
+  int32_t *d_csrj_idx = nullptr;
   // generic-path work lists, one per smem size class
   static const int kClasses = 4;
   qtam::WorkItem *d_items[kClasses] = {nullptr, nullptr, nullptr, nullptr};
@@ -109,7 +114,9 @@ struct qtam_plan {
 
   // CTA-level rows (rows_cta.cu), one class per transform length 2^11 .. 2^14
   bool cta_rows = false;
-  int *d_cta_rowidx[4] = {nullptr, nullptr, nullptr, nullptr};
+  int *d_cta_rowidx[4] = {nullptr, nullptr, nullptr, nullptr};   // one leader per set of identical rows
+  int *d_cta_memptr[4] = {nullptr, nullptr, nullptr, nullptr};   // members of leader i: d_cta_mem[memptr[i] .. memptr[i+1])
+  int *d_cta_mem[4] = {nullptr, nullptr, nullptr, nullptr};
   int n_cta_rows[4] = {0, 0, 0, 0};
   double cta_sumM[4] = {0, 0, 0, 0}, cta_sumL[4] = {0, 0, 0, 0};
   int64_t cta_maxM = 0;           // longest row that needs the per-CTA scratch (0: none)
@@ -142,6 +149,13 @@ struct LaunchScope {
   }
   ~LaunchScope() { if (slot >= 0) cudaEventRecord(p->prof_pool[(size_t)slot].e1, st); }
 };
+
+// which CSR a reduction over the band workspace walks: sets plo .. phi-1 of nsets per bin
+struct CsrSel { const int32_t *ptr, *idx; int nsets, plo, phi; };
+inline CsrSel csr_select(const qtam_plan *p, int plane) {
+  if (plane < 0 && p->d_csrj_ptr) return CsrSel{p->d_csrj_ptr, p->d_csrj_idx, 1, 0, 1};
+  return CsrSel{p->d_csr_ptr, p->d_csr_idx, p->hp.nP + 1, plane < 0 ? 0 : plane, plane < 0 ? p->hp.nP : plane + 1};
+}
 
 // generic.cu : correct-for-everything kernels (any N, any M, float and double)
 qtam_status generic_r2c(qtam_plan *p, const void *d_x, int batch, cudaStream_t st);

@@ -279,14 +279,12 @@ k_rows_fast(FastParams P, const FastRow *frows, const void *__restrict__ tw1g_,
 template <int LOG2NC>
 __global__ void __launch_bounds__(CtaFftPlan<LOG2NC>::NT)
 k_reduce_c2r_fast(const float2 *__restrict__ band, long long sumL, const int32_t *__restrict__ ptr,
-                  const int32_t *__restrict__ idx, const float *__restrict__ invP, int nbins, int nP,
-                  int plane, const float2 *__restrict__ tw, int log2twn, const float2 *__restrict__ ptw,
-                  float *__restrict__ x_out) {
+                  const int32_t *__restrict__ idx, const float *__restrict__ invP, int nbins, int nsets,
+                  int plo, int phi, int plane, const float2 *__restrict__ tw, int log2twn,
+                  const float2 *__restrict__ ptw, float *__restrict__ x_out) {
   constexpr int NC = 1 << LOG2NC, NT = CtaFftPlan<LOG2NC>::NT;
   float2 *s = reinterpret_cast<float2 *>(qtam_fast_smem);
   const float2 *Gb = band + (size_t)blockIdx.x * sumL;
-  const int nsets = nP + 1;
-  const int plo = plane < 0 ? 0 : plane, phi = plane < 0 ? nP : plane + 1;
   const float *ip = invP + (size_t)(plane + 1) * nbins;
   for (int f = threadIdx.x; f <= NC; f += NT) {
     const int lo = ptr[(size_t)f * nsets + plo], hi = ptr[(size_t)f * nsets + phi];
@@ -458,11 +456,12 @@ static qtam_status reduce_c2r_launch(qtam_plan *p, int batch, int plane, void *d
   const size_t smem = sizeof(float2) * (size_t)cta_fft_smem_elems<LOG2NC>();
   if (!set_smem(k_reduce_c2r_fast<LOG2NC>, smem)) return QTAM_ERR_CUDA;
   {
+    const CsrSel cs = csr_select(p, plane);
     LaunchScope ls(p, st, K_REDUCE_C2R_FAST,
                    (double)batch * (8.0 * (double)p->hp.sumL + 4.0 * (double)p->hp.N));
     k_reduce_c2r_fast<LOG2NC><<<batch, CtaFftPlan<LOG2NC>::NT, smem, st>>>(
-        static_cast<const float2 *>(p->d_band), p->hp.sumL, p->d_csr_ptr, p->d_csr_idx,
-        static_cast<const float *>(p->d_invP), (int)p->hp.nb, p->hp.nP, plane,
+        static_cast<const float2 *>(p->d_band), p->hp.sumL, cs.ptr, cs.idx,
+        static_cast<const float *>(p->d_invP), (int)p->hp.nb, cs.nsets, cs.plo, cs.phi, plane,
         static_cast<const float2 *>(p->d_tw), ilog2(p->twn), static_cast<const float2 *>(p->d_ptw),
         static_cast<float *>(d_x_out));
   }

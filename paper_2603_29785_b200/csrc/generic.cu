@@ -291,14 +291,14 @@ __global__ void k_inv_rows(const RowDev *__restrict__ rows, const WorkItem *__re
 template <typename T>
 __global__ void k_inv_reduce(const C2<T> *__restrict__ band, long long sumL,
                              const int32_t *__restrict__ ptr, const int32_t *__restrict__ idx,
-                             const T *__restrict__ invP, int nbins, int nP, int plane,
+                             const T *__restrict__ invP, int nbins, int nsets, int plo, int phi, int plane,
                              C2<T> *__restrict__ spec, long long xstride) {
   typedef C2<T> V;
   const int f = blockIdx.x * blockDim.x + threadIdx.x;
   if (f >= nbins) return;
-  const int nsets = nP + 1;
-  const int lo = ptr[(long long)f * nsets + (plane < 0 ? 0 : plane)];
-  const int hi = ptr[(long long)f * nsets + (plane < 0 ? nP : plane + 1)];
+  // the bin's entries: sets plo .. phi-1 of the CSR's nsets per bin (see csr_select)
+  const int lo = ptr[(long long)f * nsets + plo];
+  const int hi = ptr[(long long)f * nsets + phi];
   const V *G = band + (long long)blockIdx.y * sumL;
   V s = cmk<T>(0, 0);
   for (int e = lo; e < hi; ++e) s = cadd(s, G[idx[e]]);
@@ -547,9 +547,10 @@ static qtam_status inv_reduce_t(qtam_plan *p, int batch, int plane, cudaStream_t
   {
     LaunchScope ls(p, st, K_INV_REDUCE,
                    (double)batch * (sizeof(C2<T>) * ((double)p->hp.sumL + (double)p->hp.nb)));
-    k_inv_reduce<T><<<g, 256, 0, st>>>(static_cast<const C2<T> *>(p->d_band), p->hp.sumL, p->d_csr_ptr,
-                                       p->d_csr_idx, static_cast<const T *>(p->d_invP), (int)p->hp.nb,
-                                       p->hp.nP, plane, static_cast<C2<T> *>(p->d_spec), p->xstride);
+    const CsrSel cs = csr_select(p, plane);
+    k_inv_reduce<T><<<g, 256, 0, st>>>(static_cast<const C2<T> *>(p->d_band), p->hp.sumL, cs.ptr, cs.idx,
+                                       static_cast<const T *>(p->d_invP), (int)p->hp.nb, cs.nsets, cs.plo,
+                                       cs.phi, plane, static_cast<C2<T> *>(p->d_spec), p->xstride);
   }
   QTAM_LAUNCH_CHECK();
   return QTAM_OK;

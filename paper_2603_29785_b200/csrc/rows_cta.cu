@@ -17,6 +17,7 @@
 // Grids are persistent (CTAs loop over work items) because the scratch is per resident CTA.
 #include <algorithm>
 #include <cmath>
+#include <cstdint>
 #include <vector>
 
 #include "ctafft.cuh"
@@ -46,7 +47,7 @@ template <int MB> __device__ __forceinline__ void powers(float2 w, float2 (&pw)[
 // forward radix-MB step: scratch [jb][n'] -> coefficients
 template <int MB, int NT, int M2>
 __device__ __forceinline__ void fwd_combine(const float2 *__restrict__ z, const float2 *__restrict__ twb,
-                                            float2 *__restrict__ Y, float scale) {
+                                            float2 *__restrict__ Yseg, const long long *off, int nm, float scale) {
 #pragma unroll 1
   for (int n = threadIdx.x; n < M2; n += NT) {
     float2 v[MB], pw[MB];
@@ -57,14 +58,19 @@ __device__ __forceinline__ void fwd_combine(const float2 *__restrict__ z, const 
     for (int jb = 1; jb < MB; ++jb) v[jb] = pcmul(v[jb], pw[jb]);
     RegFFT<MB, +1>::run(v);
 #pragma unroll
-    for (int nb = 0; nb < MB; ++nb) __stcs(Y + n + nb * M2, pscale(v[nb], scale));
+    for (int nb = 0; nb < MB; ++nb) v[nb] = pscale(v[nb], scale);
+    for (int m = 0; m < nm; ++m) {
+      float2 *Y = Yseg + off[m] + n;
+#pragma unroll
+      for (int nb = 0; nb < MB; ++nb) __stcs(Y + nb * M2, v[nb]);
+    }
   }
 }
 
 // inverse radix-MB step: coefficients -> scratch [jb][n']
 template <int MB, int NT, int M2>
-__device__ __forceinline__ void inv_split(const float2 *__restrict__ Y, const float2 *__restrict__ twb,
-                                          float2 *__restrict__ z) {
+__device__ __forceinline__ void inv_split(const float2 *__restrict__ Yseg, const long long *off, int nm,
+                                          const float2 *__restrict__ twb, float2 *__restrict__ z) {
 #pragma unroll 1
   for (int n = threadIdx.x; n < M2; n += NT) {
     float2 v[MB], pw[MB];
@@ -72,7 +78,12 @@ __device__ __forceinline__ void inv_split(const float2 *__restrict__ Y, const fl
     w.y = -w.y;
     powers<MB>(w, pw);
 #pragma unroll
-    for (int nb = 0; nb < MB; ++nb) v[nb] = __ldcs(Y + n + nb * M2);
+    for (int nb = 0; nb < MB; ++nb) v[nb] = __ldcs(Yseg + off[0] + n + nb * M2);
+    for (int m = 1; m < nm; ++m) {      // members of the leader's set: rows are added before the transform
+      const float2 *Y = Yseg + off[m] + n;
+#pragma unroll
+      for (int nb = 0; nb < MB; ++nb) v[nb] = padd(v[nb], __ldcs(Y + nb * M2));
+    }
     RegFFT<MB, -1>::run(v);
 #pragma unroll
     for (int jb = 0; jb < MB; ++jb) z[jb * M2 + n] = jb ? pcmul(v[jb], pw[jb]) : v[0];
@@ -95,13 +106,20 @@ struct GatherIn {      // B[j] = X[kc + jj] W_k[jj] at M-array index j = jb + Mb
     return v;
   }
 };
-struct CoefOut {
-  float2 *__restrict__ p; float scale;
-  __device__ __forceinline__ void operator()(int a, float2 v) const { __stcs(p + a, pscale(v, scale)); }
+struct CoefOut {      // the same coefficients go to every member of the leader's set
+  float2 *__restrict__ seg; const long long *off; int nm; float scale;
+  __device__ __forceinline__ void operator()(int a, float2 v) const {
+    v = pscale(v, scale);
+    for (int m = 0; m < nm; ++m) __stcs(seg + off[m] + a, v);
+  }
 };
-struct CoefIn {
-  const float2 *__restrict__ p;
-  __device__ __forceinline__ float2 operator()(int a) const { return __ldcs(p + a); }
+struct CoefIn {       // sum of the members' coefficients
+  const float2 *__restrict__ seg; const long long *off; int nm;
+  __device__ __forceinline__ float2 operator()(int a) const {
+    float2 v = __ldcs(seg + off[0] + a);
+    for (int m = 1; m < nm; ++m) v = padd(v, __ldcs(seg + off[m] + a));
+    return v;
+  }
 };
 struct ScratchOut {
   float2 *__restrict__ p;
@@ -114,7 +132,8 @@ struct ScratchIn {
 
 template <int L2, bool FORWARD>
 __global__ void __launch_bounds__(CtaFftPlan<L2>::NT)
-k_rows_cta(const int *__restrict__ rowidx, int nrows, const RowDev *__restrict__ rows,
+k_rows_cta(const int *__restrict__ rowidx, const int *__restrict__ memptr, const int *__restrict__ mem, int nrows,
+           const RowDev *__restrict__ rows,
            const float *__restrict__ win, const float2 *__restrict__ spec, long long xstride, int nbins,
            float2 *__restrict__ coef, long long ctot, float2 *__restrict__ band, long long sumL,
            float2 *__restrict__ scratch, long long scratch_stride, const float2 *__restrict__ ptw,
@@ -122,19 +141,40 @@ k_rows_cta(const int *__restrict__ rowidx, int nrows, const RowDev *__restrict__
   constexpr int M2 = 1 << L2, NT = CtaFftPlan<L2>::NT;
   float2 *s = reinterpret_cast<float2 *>(qtam_cta_smem);
   float2 *z = scratch + (size_t)blockIdx.x * scratch_stride;
+  // rows with the same centre bin and half-width (the clamped rows of different Q-planes) have the same
+  // window: `rowidx` lists one leader per such set, mem[memptr[i] .. memptr[i+1]) its members.  Forward:
+  // one transform, stored at every member's offset; inverse: the members' rows are added first.
+  __shared__ int s_nm;
+  __shared__ long long s_off[kCtaMaxMembers];
+  __shared__ long long s_slot;      // inverse: band slot that takes the sum (the first member taking part)
   const long long total = (long long)nrows * batch;
   for (long long item = blockIdx.x; item < total; item += gridDim.x) {
     const int seg = (int)(item / nrows);
-    const RowDev r = rows[rowidx[item - (long long)seg * nrows]];
-    if (!FORWARD && plane >= 0 && r.plane != plane) continue;
+    const int li = (int)(item - (long long)seg * nrows);
+    const RowDev r = rows[rowidx[li]];
+    __syncthreads();
+    if (threadIdx.x == 0) {
+      int n = 0;
+      for (int m = memptr[li]; m < memptr[li + 1]; ++m) {
+        const RowDev &rm = rows[mem[m]];
+        if (FORWARD || plane < 0 || rm.plane == plane) {
+          if (n == 0) s_slot = rm.woff;
+          s_off[n++] = rm.offset;
+        }
+      }
+      s_nm = n;
+    }
+    __syncthreads();
+    const int nm = s_nm;
+    if (nm == 0) continue;
     const int lb = r.log2M - L2, Mb = 1 << lb;
     const float *W = win + r.woff + r.dk;
-    float2 *Y = coef + (size_t)seg * ctot + r.offset;
+    float2 *Yseg = coef + (size_t)seg * ctot;
     const float2 *tb = lb > 0 ? twb.t[lb - 1] : nullptr;
     if constexpr (FORWARD) {
       GatherIn in{spec + (size_t)seg * xstride, W, r.kc, r.dk, nbins, r.M, lb, 0};
       if (Mb == 1) {
-        cta_fft_io<L2, NT, +1, true, true>(s, in, CoefOut{Y, (float)r.fwd_scale}, ptw);
+        cta_fft_io<L2, NT, +1, true, true>(s, in, CoefOut{Yseg, s_off, nm, (float)r.fwd_scale}, ptw);
         __syncthreads();
       } else {
         for (int jb = 0; jb < Mb; ++jb) {
@@ -143,25 +183,25 @@ k_rows_cta(const int *__restrict__ rowidx, int nrows, const RowDev *__restrict__
           __syncthreads();
         }
         switch (lb) {
-          case 1: fwd_combine<2, NT, M2>(z, tb, Y, (float)r.fwd_scale); break;
-          case 2: fwd_combine<4, NT, M2>(z, tb, Y, (float)r.fwd_scale); break;
-          default: fwd_combine<8, NT, M2>(z, tb, Y, (float)r.fwd_scale); break;
+          case 1: fwd_combine<2, NT, M2>(z, tb, Yseg, s_off, nm, (float)r.fwd_scale); break;
+          case 2: fwd_combine<4, NT, M2>(z, tb, Yseg, s_off, nm, (float)r.fwd_scale); break;
+          default: fwd_combine<8, NT, M2>(z, tb, Yseg, s_off, nm, (float)r.fwd_scale); break;
         }
         __syncthreads();   // the scratch is rewritten by the next row
       }
     } else {
       if (Mb > 1) {
         switch (lb) {
-          case 1: inv_split<2, NT, M2>(Y, tb, z); break;
-          case 2: inv_split<4, NT, M2>(Y, tb, z); break;
-          default: inv_split<8, NT, M2>(Y, tb, z); break;
+          case 1: inv_split<2, NT, M2>(Yseg, s_off, nm, tb, z); break;
+          case 2: inv_split<4, NT, M2>(Yseg, s_off, nm, tb, z); break;
+          default: inv_split<8, NT, M2>(Yseg, s_off, nm, tb, z); break;
         }
         __syncthreads();
       }
-      float2 *Gb = band + (size_t)seg * sumL + r.woff + r.dk;
+      float2 *Gb = band + (size_t)seg * sumL + s_slot + r.dk;
       const float amp = (float)r.inv_amp;
       for (int jb = 0; jb < Mb; ++jb) {
-        if (Mb == 1) cta_fft_io<L2, NT, -1, true, false>(s, CoefIn{Y}, CtaFftNone{}, ptw);
+        if (Mb == 1) cta_fft_io<L2, NT, -1, true, false>(s, CoefIn{Yseg, s_off, nm}, CtaFftNone{}, ptw);
         else cta_fft_io<L2, NT, -1, true, false>(s, ScratchIn{z + (size_t)jb * M2}, CtaFftNone{}, ptw);
         // G_k[jj] = sqrt(N/M) Bhat[jj] W_k[jj] on the support, clipped to the one-sided spectrum (R8)
         for (int jp = threadIdx.x; jp < M2; jp += NT) {
@@ -192,6 +232,7 @@ qtam_status build_rows_cta(qtam_plan *p) {
     return bytes == 0 || cudaMemcpy(*dst, src, bytes, cudaMemcpyHostToDevice) == cudaSuccess;
   };
   bool need_twb[3] = {false, false, false};
+  std::vector<int> followers;   // rows whose band slot the joint inverse leaves unwritten
   for (int c = 0; c < 4; ++c) {
     const int L2 = kCtaLog2Min + c;
     std::vector<int> idx;
@@ -205,9 +246,29 @@ qtam_status build_rows_cta(qtam_plan *p) {
     }
     // longest rows first within a segment
     std::stable_sort(idx.begin(), idx.end(), [&](int a, int b) { return hp.rows[(size_t)a].M > hp.rows[(size_t)b].M; });
-    p->n_cta_rows[c] = (int)idx.size();
-    if (idx.empty()) continue;
-    if (!up(reinterpret_cast<void **>(&p->d_cta_rowidx[c]), idx.data(), idx.size() * sizeof(int))) return QTAM_ERR_ALLOC;
+    if (idx.empty()) { p->n_cta_rows[c] = 0; continue; }
+    // one leader per set of rows with the same centre bin and half-width
+    std::vector<int> lead;
+    std::vector<std::vector<int>> members;
+    for (int k : idx) {
+      size_t l = 0;
+      while (l < lead.size() && !(hp.rows[(size_t)lead[l]].kc == hp.rows[(size_t)k].kc &&
+                                  hp.rows[(size_t)lead[l]].dk == hp.rows[(size_t)k].dk &&
+                                  (int)members[l].size() < kCtaMaxMembers &&
+                                  std::none_of(members[l].begin(), members[l].end(), [&](int m) {
+                                    return hp.rows[(size_t)m].plane == hp.rows[(size_t)k].plane; }))) ++l;
+      if (l == lead.size()) { lead.push_back(k); members.emplace_back(); }
+      members[l].push_back(k);
+    }
+    std::vector<int> memptr(1, 0), mem;
+    for (auto &m : members) {
+      mem.insert(mem.end(), m.begin(), m.end()); memptr.push_back((int)mem.size());
+      for (size_t i = 1; i < m.size(); ++i) followers.push_back(m[i]);
+    }
+    p->n_cta_rows[c] = (int)lead.size();
+    if (!up(reinterpret_cast<void **>(&p->d_cta_rowidx[c]), lead.data(), lead.size() * sizeof(int))) return QTAM_ERR_ALLOC;
+    if (!up(reinterpret_cast<void **>(&p->d_cta_memptr[c]), memptr.data(), memptr.size() * sizeof(int))) return QTAM_ERR_ALLOC;
+    if (!up(reinterpret_cast<void **>(&p->d_cta_mem[c]), mem.data(), mem.size() * sizeof(int))) return QTAM_ERR_ALLOC;
     std::vector<float> t;
     switch (L2) {
       case 11: fill_class_table<11>(t); break;
@@ -217,6 +278,22 @@ qtam_status build_rows_cta(qtam_plan *p) {
     }
     if (!up(&p->d_ptw_rows[c], t.data(), t.size() * sizeof(float))) return QTAM_ERR_ALLOC;
     p->cta_rows = true;
+  }
+  if (!followers.empty()) {
+    // joint CSR (one set per bin) without the followers' band slots
+    std::vector<uint8_t> skip((size_t)hp.sumL, 0);
+    for (int k : followers)
+      for (int64_t i = 0; i < hp.rows[(size_t)k].L; ++i) skip[(size_t)(hp.rows[(size_t)k].goff + i)] = 1;
+    const int nsets = hp.nP + 1;
+    std::vector<int32_t> jptr((size_t)hp.nb + 1, 0), jidx;
+    for (int64_t f = 0; f < hp.nb; ++f) {
+      jptr[(size_t)f] = (int32_t)jidx.size();
+      for (int32_t e = hp.csr_ptr[(size_t)(f * nsets)]; e < hp.csr_ptr[(size_t)(f * nsets + hp.nP)]; ++e)
+        if (!skip[(size_t)hp.csr_idx[(size_t)e]]) jidx.push_back(hp.csr_idx[(size_t)e]);
+    }
+    jptr[(size_t)hp.nb] = (int32_t)jidx.size();
+    if (!up(reinterpret_cast<void **>(&p->d_csrj_ptr), jptr.data(), jptr.size() * sizeof(int32_t))) return QTAM_ERR_ALLOC;
+    if (!up(reinterpret_cast<void **>(&p->d_csrj_idx), jidx.data(), jidx.size() * sizeof(int32_t))) return QTAM_ERR_ALLOC;
   }
   const long double tau = 6.283185307179586476925286766559005768L;
   for (int b = 0; b < 3; ++b) {
@@ -259,7 +336,7 @@ static qtam_status rows_cta_launch(qtam_plan *p, int c, int batch, void *d_coef,
   {
     LaunchScope ls(p, st, FORWARD ? K_ROWS_CTA_FWD : K_ROWS_CTA_INV, bytes);
     kern<<<(unsigned)grid, NT, smem, st>>>(
-        p->d_cta_rowidx[c], p->n_cta_rows[c], p->d_rows, static_cast<const float *>(p->d_win),
+        p->d_cta_rowidx[c], p->d_cta_memptr[c], p->d_cta_mem[c], p->n_cta_rows[c], p->d_rows, static_cast<const float *>(p->d_win),
         static_cast<const float2 *>(p->d_spec), p->xstride, (int)p->hp.nb, static_cast<float2 *>(d_coef),
         p->hp.ctot, static_cast<float2 *>(p->d_band), p->hp.sumL, static_cast<float2 *>(p->d_ws), stride,
         static_cast<const float2 *>(p->d_ptw_rows[c]), tb, batch, plane);
