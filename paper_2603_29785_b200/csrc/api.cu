@@ -46,7 +46,7 @@ void free_plan(qtam_plan *p) {
   cudaFree(p->d_bigrows); cudaFree(p->d_spec_alloc); cudaFree(p->d_ws); cudaFree(p->d_band);
   cudaFree(p->d_fwinp); cudaFree(p->d_red);
   cudaFree(p->d_frows); cudaFree(p->d_fwin); cudaFree(p->d_ftw_fwd); cudaFree(p->d_ftw_inv);
-  cudaFree(p->d_tiny); cudaFree(p->d_ptw); cudaFree(p->d_frows_fwd); cudaFree(p->d_fmem); cudaFree(p->d_tmem);
+  cudaFree(p->d_tiny); cudaFree(p->d_ptw); cudaFree(p->d_ptw_long); cudaFree(p->d_frows_fwd); cudaFree(p->d_fmem); cudaFree(p->d_tmem);
   cudaFree(p->d_thr_tasks); cudaFree(p->d_thr_offs);
   for (int c = 0; c < 4; ++c) { cudaFree(p->d_cta_rowidx[c]); cudaFree(p->d_ptw_rows[c]); cudaFree(p->d_cta_memptr[c]); cudaFree(p->d_cta_mem[c]); }
   for (int b = 0; b < 3; ++b) cudaFree(p->d_twb[b]);
@@ -337,6 +337,7 @@ qtam_status qtam_plan_create(qtam_plan **out, double fs, int64_t N, const double
   if (s == QTAM_OK && p->fast_rows) s = build_fast(p);
   if (s == QTAM_OK && p->fast_rows) s = build_rows_cta(p);
   if (s == QTAM_OK && p->fast_long) s = build_long_tables(p);
+  if (s == QTAM_OK && p->fast_rows) s = build_long_fft(p);
   if (s == QTAM_OK && p->fast_rows) s = build_inv_tiled(p);
   if (s != QTAM_OK) { free_plan(p); cudaGetLastError(); return s; }
   if (cudaDeviceSynchronize() != cudaSuccess) { free_plan(p); return QTAM_ERR_CUDA; }
@@ -478,7 +479,7 @@ static const char *const kKernelNames[K_COUNT] = {
     "cfft_seq", "cfft_cols", "cfft_rows", "r2c_post", "c2r_pre", "fwd_rows", "fwd_combine",
     "inv_rows", "inv_reduce", "dense_place", "threshold", "r2c_fast", "fwd_rows_fast", "inv_rows_fast",
     "reduce_c2r_fast", "inv_fused", "inv_tiles", "combine_c2r", "threshold_fast", "rows_cta_fwd", "rows_cta_inv",
-    "tiny_rows_fwd", "tiny_rows_inv"};
+    "tiny_rows_fwd", "tiny_rows_inv", "long_fft_a", "long_fft_b"};
 
 qtam_status qtam_profile_enable(qtam_plan *p, int on, int max_launches) {
   if (!p || p->host_only) return QTAM_ERR_INVALID_ARG;

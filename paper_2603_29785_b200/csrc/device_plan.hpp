@@ -13,7 +13,7 @@ enum KernelId {
   K_CFFT_SEQ = 0, K_CFFT_COLS, K_CFFT_ROWS, K_R2C_POST, K_C2R_PRE, K_FWD_ROWS, K_FWD_COMBINE,
   K_INV_ROWS, K_INV_REDUCE, K_DENSE_PLACE, K_THRESHOLD, K_R2C_FAST, K_FWD_ROWS_FAST, K_INV_ROWS_FAST,
   K_REDUCE_C2R_FAST, K_INV_FUSED, K_INV_TILES, K_COMBINE_C2R, K_THRESHOLD_FAST, K_ROWS_CTA_FWD, K_ROWS_CTA_INV,
-  K_TINY_FWD, K_TINY_INV, K_COUNT
+  K_TINY_FWD, K_TINY_INV, K_LONG_A, K_LONG_B, K_COUNT
 };
 // fast float path (fast.cu): rows with 32 <= M <= 1024, grouped by G = M/32 lanes per row
 struct FastRow { int kc, dk, woff, goff, offset, plane, wpad, pad; };   // wpad: offset into the padded window table
@@ -93,6 +93,7 @@ struct qtam_plan {
   void *d_ftw_fwd = nullptr;   // float2 pass-1 twiddles [bucket][n1][t], forward (x (N M)^-1/2)
   void *d_ftw_inv = nullptr;   // same, inverse (conjugate, x sqrt(N/M))
   void *d_ptw = nullptr;       // pass tables of the long FFT (ctafft.cuh)
+  void *d_ptw_long = nullptr;  // pass tables of the 2^14-point stage of long_fft.cu (N = 2^16 .. 2^20)
   qtam::FastRow *d_tiny = nullptr;   // rows shorter than 32 points (goff holds log2 M), for the combine kernel of inv_tiled.cu
   int n_tiny = 0;
   double tiny_sumM = 0, tiny_sumL = 0;   // coefficients / band values per segment of those rows
@@ -172,6 +173,12 @@ qtam_status fast_r2c(qtam_plan *p, const void *d_x, int batch, cudaStream_t st);
 qtam_status fast_forward_rows(qtam_plan *p, int batch, void *d_coef, cudaStream_t st);
 qtam_status fast_inverse_rows(qtam_plan *p, const void *d_coef, int batch, int plane, cudaStream_t st);
 qtam_status fast_reduce_c2r(qtam_plan *p, int batch, int plane, void *d_x_out, cudaStream_t st);
+// long_fft.cu
+qtam_status build_long_fft(qtam_plan *p);
+bool fast_cfft_long_ok(const qtam_plan *p, int log2n);
+qtam_status fast_cfft_long(qtam_plan *p, const void *in, long long in_stride, void *out, long long out_stride,
+                           void *tmp, long long tmp_stride, int log2n, int count, int dir, float scale,
+                           cudaStream_t st);
 // rows_cta.cu
 qtam_status build_rows_cta(qtam_plan *p);
 qtam_status cta_forward_rows(qtam_plan *p, int batch, void *d_coef, cudaStream_t st);

@@ -10,6 +10,7 @@
 // C46 :583), a3 short inverse FFT scaled (N*M)^(-1/2) (C47 :589), a4 row-median threshold
 // (BASELINE.json cfg 5), a5 per-row FFT + window + sqrt(N/M) (C49 :598), a6 sum over rows as a
 // segmented reduction over bins, a7 division by P (Eq. 11 :135), a8 long C2R, a9 dense tiles (C3 :377).
+#include <cstdlib>
 #include <cstdio>
 
 #include "cplx.cuh"
@@ -423,6 +424,10 @@ template <typename T>
 static qtam_status cfft(qtam_plan *p, const C2<T> *in, long long in_stride, C2<T> *out,
                         long long out_stride, C2<T> *tmp, long long tmp_stride, int log2n, int count,
                         int dir, T scale, cudaStream_t st) {
+  if constexpr (sizeof(T) == 4) {
+    if (!getenv("QTAM_NO_FAST_LONG") && fast_cfft_long_ok(p, log2n) && tmp != out)
+      return fast_cfft_long(p, in, in_stride, out, out_stride, tmp, tmp_stride, log2n, count, dir, scale, st);
+  }
   const int cap = p->cap_log2;
   const C2<T> *tw = static_cast<const C2<T> *>(p->d_tw);
   const int log2twn = ilog2(p->twn);

@@ -151,6 +151,22 @@ def test_inverse_of_arbitrary_coefficients(name, ov):
     assert worst_segment(xg, r.inverse(Yin.astype(np.complex128), plane=-1, engine=1)) <= 2e-5
 
 
+@pytest.mark.parametrize("log2n", [16, 17, 18, 19])
+def test_mid_length_segments(log2n):
+    """N = 2^16 .. 2^19: the long real FFT runs as the two-kernel transform of long_fft.cu
+    (radix 2 .. 16 across stride 2^14, then 2^14-point transforms in shared memory)."""
+    N = 1 << log2n
+    args = (16384.0, N, [6.0, 24.0], 30.0, 7000.0, 20.0)
+    g, r = make_plans(args, "f32", 1)
+    rng = np.random.default_rng(log2n)
+    x = rng.standard_normal((1, N)).astype(np.float32)
+    x64 = x.astype(np.float64)
+    Yg = g.forward(dev(x)).cpu().numpy()
+    assert worst_segment(Yg, r.forward(x64, engine=1)) <= 2e-5
+    _, C = r.frame(-1)
+    assert worst_segment(g.inverse(g.forward(dev(x))).cpu().numpy(), pi_c(x64, C)) <= 1e-5
+
+
 def test_cfg5_fp64_variant():
     name = "cfg5"
     g, r = make_plans(inputs.plan_args(name), "f64", 4)
