@@ -89,11 +89,48 @@ __device__ __forceinline__ void thr_group(C2<T> *__restrict__ Y, int G, int t, T
     const U hi_mask = top >= Bits<T>::nbits - 1 ? (U)0 : ~((((U)1) << (top + 1)) - 1);
     prefix &= hi_mask;
   }
-#pragma unroll
-  for (int e = 0; e < E; ++e) x[e] ^= prefix;
-  // rank M/2-1 (0-based), most significant undecided bit first; stops when one candidate is left
   int kk = M / 2 - 1;
   int alive = M;
+  // Short cut: the squared magnitudes of a noise row are close to exponentially distributed, so the
+  // median sits near ln 2 times their mean.  The aligned block of bit patterns that contains
+  // mean ln2 (1 -+ 2.5/sqrt(M)) is tested with one exact counting pass; when the wanted order statistic
+  // lies inside it (it nearly always does), the select starts at the block's prefix and needs about
+  // log2(block population) steps instead of one per undecided exponent and mantissa bit.  A wrong guess
+  // costs the counting pass and nothing else: every decision below is still exact.
+  {
+    float sum = 0.f;
+#pragma unroll
+    for (int e = 0; e < E; ++e) sum += (float)Bits<T>::from(x[e]);
+    for (int o = G >> 1; o > 0; o >>= 1) sum += __shfl_xor_sync(0xffffffffu, sum, o);
+    const float est = 0.6931472f * sum / (float)M;
+    const float dl = fminf(0.9f, 2.5f * rsqrtf((float)M));
+    const U blo = Bits<T>::of((T)(est * (1.f - dl))), bhi = Bits<T>::of((T)(est * (1.f + dl)));
+    int sb = 0;
+    U P = 0, Pend = 0;
+    const bool sane = blo > 0 && blo <= bhi && bhi < Bits<T>::inf_bits();
+    if (sane) {
+      const U d = blo ^ bhi;
+      sb = d == 0 ? 0 : Bits<T>::nbits - (sizeof(U) == 8 ? __clzll((long long)d) : __clz((int)d));
+      P = (blo >> sb) << sb;
+      Pend = P + (((U)1) << sb);
+    }
+    int c_lo = 0, c_hi = 0;
+#pragma unroll
+    for (int e = 0; e < E; ++e) {
+      c_lo += (x[e] < P) ? 1 : 0;
+      c_hi += (x[e] < Pend) ? 1 : 0;
+    }
+    for (int o = G >> 1; o > 0; o >>= 1) {
+      c_lo += __shfl_xor_sync(0xffffffffu, c_lo, o);
+      c_hi += __shfl_xor_sync(0xffffffffu, c_hi, o);
+    }
+    if (sane && c_lo <= kk && kk < c_hi && sb - 1 < top) {
+      prefix = P; top = sb - 1; kk -= c_lo; alive = c_hi - c_lo;
+    }
+  }
+#pragma unroll
+  for (int e = 0; e < E; ++e) x[e] ^= prefix;
+  // rank kk among the candidates, most significant undecided bit first; stops when one candidate is left
   int bit = top;
   // (the groups of a warp sit at different bits and stop at different times, but all lanes take the
   // shuffles together: a finished group counts against a zero limit and changes nothing)
