@@ -45,7 +45,7 @@ qtam_status build_inv_tiled(qtam_plan *p) {
   if (!p->fast_long || getenv("QTAM_NO_TILED_INV")) return QTAM_OK;
   if (ilog2(hp.N) - 1 > 14 || p->n_tiny > 256) return QTAM_OK;
   for (const HostRow &h : hp.rows) if (h.M > 1024) return QTAM_OK;
-  const int max_pass = getenv("QTAM_TILE_PASSES") ? atoi(getenv("QTAM_TILE_PASSES")) : 8;
+  const int max_pass = getenv("QTAM_TILE_PASSES") ? atoi(getenv("QTAM_TILE_PASSES")) : 12;
   std::vector<TileRow> trows;
   std::vector<TileItem> items;
   std::vector<int2> tmem;                 // (coefficient offset, plane) of every member
