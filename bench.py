@@ -57,6 +57,21 @@ def measured_peaks():
     return 6650.0, "fallback (B200_PROFILING.md: 6.65 TB/s)"
 
 
+def measured_traffic(workload, batch, kernel):
+    """dram__bytes_read + dram__bytes_write of one launch from the committed ncu --set full capture
+    (profiles/r1_dram_traffic.csv, see the .md beside it); None when no capture matches this run."""
+    path = os.path.join(ROOT, "profiles", "r1_dram_traffic.csv")
+    try:
+        with open(path) as f:
+            for line in f.read().splitlines()[1:]:
+                w, b, k, v = line.split(",")
+                if w == workload and int(b) == batch and k == kernel:
+                    return float(v)
+    except Exception:
+        pass
+    return None
+
+
 def compulsory_bytes_per_segment(cfg, ctot):
     """forward r*N + c*C_tot, inverse c*C_tot + r*N; threshold fused -> 0 extra, as a
     separate in-place pass 2*c*C_tot (what this build does today)."""
@@ -349,10 +364,13 @@ def run_ours(args):
             avg_ms = s["ms"] / s["launches"]
             gbs = s["algo_bytes"] / s["launches"] / (avg_ms * 1e-3) / 1e9
             kernels.append({"name": s["name"], "launches_per_step": s["launches"] / args.steps,
-                            "avg_ms": avg_ms, "share": s["ms"] / tot_ms, "algo_gbs": gbs})
+                            "avg_ms": avg_ms, "share": s["ms"] / tot_ms, "algo_gbs": gbs,
+                            "algo_bytes": s["algo_bytes"] / s["launches"]})
         top = kernels[0]
         roof = {"bound": "hbm", "kernel": top["name"], "achieved": top["algo_gbs"], "peak": peak,
-                "unit": "GB/s", "frac": top["algo_gbs"] / peak, "traffic": None,
+                "unit": "GB/s", "frac": top["algo_gbs"] / peak,
+                "traffic": measured_traffic(args.workload, batch, top["name"]),
+                "algo_bytes_per_launch": top["algo_bytes"],
                 "peak_source": peak_src, "avg_launch_ms": top["avg_ms"], "share_of_step": top["share"]}
     comp = compulsory_bytes_per_segment(cfg, plan.ctot) * batch
     path_gbs = comp / (ms_step * 1e-3) / 1e9
