@@ -43,6 +43,8 @@ def parse_args():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--overlap", type=float, default=1.0, help="clamp_overlap (R7); 1.0 = paper literal")
+    ap.add_argument("--no-largest-batch", action="store_true",
+                    help="skip the extra pass at a batch of 8 segments per SM (SURVEY.md 8(d) 'largest batch')")
     return ap.parse_args()
 
 
@@ -163,7 +165,7 @@ def oracle_step_fn(cfg, name, overlap, nseg):
     return step, threads()
 
 
-def time_oracle(cfg, name, overlap, budget_s=12.0, max_seg=None):
+def time_oracle(cfg, name, overlap, budget_s=25.0, max_seg=None):
     """times the oracle's FFT-engine path on a bounded sample sized for about `budget_s` of work"""
     probe = 4
     step, cores = oracle_step_fn(cfg, name, overlap, probe)
@@ -375,6 +377,47 @@ def run_ours(args):
     comp = compulsory_bytes_per_segment(cfg, plan.ctot) * batch
     path_gbs = comp / (ms_step * 1e-3) / 1e9
 
+    # ---- the same step at a batch that fills every SM several times over ("largest batch")
+    largest = None
+    if world == 1 and not args.batch and not args.no_largest_batch and cfg["N"] <= 32768:
+        sms = torch.cuda.get_device_properties(dev).multi_processor_count
+        big = 8 * sms
+        x_big = torch.from_numpy(inputs.make_batch(args.workload, batch=min(big, 2 * batch))).to(dev)
+        x_big = x_big.repeat((big + x_big.shape[0] - 1) // x_big.shape[0], 1)[:big].contiguous()
+        plan_b = binding.Plan(fs, N, Q, fmin, fmax, rows, dtype=dtype, max_batch=big, clamp_overlap=args.overlap)
+        c_big = torch.empty((big, plan_b.ctot), dtype=cdt, device=dev)
+        o_big = torch.empty((big, N), dtype=rdt, device=dev)
+
+        def step_big():
+            plan_b.forward(x_big, out=c_big)
+            if "threshold" in calls:
+                plan_b.threshold_rowmedian(c_big, 3.0)
+            if "inverse" in calls:
+                plan_b.inverse(c_big, out=o_big)
+
+        for _ in range(3):
+            step_big()
+        torch.cuda.synchronize()
+        nb = 10
+        plan_b.profile_enable(True, max_launches=64 * nb)
+        evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(nb)]
+        for s0, e0_ in evs:
+            flush.zero_()
+            s0.record(); step_big(); e0_.record()
+        torch.cuda.synchronize()
+        ms_b = sum(a.elapsed_time(b) for a, b in evs) / nb
+        st_b = plan_b.profile_read()
+        plan_b.profile_enable(False)
+        comp_b = compulsory_bytes_per_segment(cfg, plan_b.ctot) * big
+        largest = {"batch": big, "ms_per_step": ms_b, "value": big * N / (ms_b * 1e-3), "unit": UNIT,
+                   "path_gbs": comp_b / (ms_b * 1e-3) / 1e9, "path_frac_of_peak": comp_b / (ms_b * 1e-3) / 1e9 / peak,
+                   "kernels": [{"name": k["name"], "avg_ms": k["ms"] / k["launches"],
+                                "algo_gbs": k["algo_bytes"] / k["ms"] / 1e6,
+                                "frac_of_peak": k["algo_bytes"] / k["ms"] / 1e6 / peak}
+                               for k in sorted(st_b, key=lambda k: -k["ms"])]}
+        plan_b.close()
+        del x_big, c_big, o_big
+
     cpu = None
     if world == 1 and not args.no_cpu_baseline:
         v, cores, nseg, dt = time_oracle(cfg, args.workload, args.overlap)
@@ -395,6 +438,7 @@ def run_ours(args):
                  "frac_of_8tbs": path_gbs / 8000.0, "ms_per_step_unprofiled": ms_plain / args.steps},
         "kernels": kernels,
         "round_trip_err": rt_err,
+        "largest_batch": largest,
         "cpu_baseline": cpu,
     }
     print(json.dumps(line))
