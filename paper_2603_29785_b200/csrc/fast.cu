@@ -15,6 +15,7 @@
 #include "ctafft.cuh"
 #include "device_plan.hpp"
 #include "rowfft.cuh"
+#include "tinyrow.cuh"
 
 namespace qtam {
 
@@ -62,39 +63,6 @@ k_r2c_fast(const float *__restrict__ x, float2 *__restrict__ spec, long long xst
 // Y = (N M)^{-1/2} IFFT_M(B) (C47).  Inverse: G[jj] = sqrt(N/M) FFT_M(Y)[jj mod M] W[jj] to the band
 // workspace (C49).  For tiny rows FastRow::goff holds log2 M and FastRow::wpad the band offset.
 // --------------------------------------------------------------------------------------------------
-template <int M, bool FORWARD>
-__device__ __forceinline__ void tiny_row(const FastRow &row, const float2 *__restrict__ X, const float *__restrict__ fwin,
-                                         float2 *__restrict__ Y, float2 *__restrict__ Gb, int nbins, float scale) {
-  float2 v[M];
-  const float *W = fwin + row.woff + row.dk;
-  if constexpr (FORWARD) {
-#pragma unroll
-    for (int j = 0; j < M; ++j) {
-      const int jj = j < M / 2 ? j : j - M;
-      v[j] = make_float2(0.f, 0.f);
-      if (jj >= -row.dk && jj <= row.dk) v[j] = pscale(X[row.kc + jj], __ldg(W + jj) * scale);
-    }
-    RegFFT<M, +1>::run(v);
-    float4 *dst = reinterpret_cast<float4 *>(Y);
-#pragma unroll
-    for (int j = 0; j < M / 2; ++j) __stcs(dst + j, make_float4(v[2 * j].x, v[2 * j].y, v[2 * j + 1].x, v[2 * j + 1].y));
-  } else {
-    const float4 *src = reinterpret_cast<const float4 *>(Y);
-#pragma unroll
-    for (int j = 0; j < M / 2; ++j) {
-      const float4 q = __ldcs(src + j);
-      v[2 * j] = make_float2(q.x, q.y); v[2 * j + 1] = make_float2(q.z, q.w);
-    }
-    RegFFT<M, -1>::run(v);
-#pragma unroll
-    for (int j = 0; j < M; ++j) {
-      const int jj = j < M / 2 ? j : j - M;
-      const int f = row.kc + jj;
-      if (jj >= -row.dk && jj <= row.dk && (unsigned)f < (unsigned)nbins) Gb[jj] = pscale(v[j], __ldg(W + jj) * scale);
-    }
-  }
-}
-
 template <bool FORWARD>
 __device__ __forceinline__ void tiny_dispatch(long long id, const FastRow *__restrict__ tiny, int n_tiny,
                                               const float *__restrict__ fwin, const float2 *__restrict__ spec,

@@ -23,6 +23,7 @@
 #include "ctafft.cuh"
 #include "device_plan.hpp"
 #include "rowfft.cuh"
+#include "tinyrow.cuh"
 
 namespace qtam {
 
@@ -294,73 +295,46 @@ k_combine_c2r(const TileItem *__restrict__ items, int n_items, const float2 *__r
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const float2 *Yseg = coef + (size_t)blockIdx.x * ctot;
 
-  // rows shorter than 32 points: Bhat[jj] = sqrt(N/M) sum_n Y[n] e^{-2 pi i jj n/M} by direct summation
-  // (lane l holds Y[l] and e^{-2 pi i l/M}; the sum over n takes both from shuffles)
-  for (int s = warp; s < n_tiny; s += NT / 32) {
+  // rows shorter than 32 points: one thread per row, transform in registers (tinyrow.cuh); the windowed
+  // band (at most 31 values) goes to tbuf[s][jj + dk], zero where the offset leaves the spectrum (R8)
+  for (int s = tid; s < n_tiny; s += NT) {
     const FastRow row = tiny[s];              // goff holds log2 M for tiny rows
-    float2 out = make_float2(0.f, 0.f);
-    if (plane < 0 || row.plane == plane) {    // warp-uniform
-      const int lm = row.goff, M = 1 << lm;
-      float2 y = make_float2(0.f, 0.f), w = make_float2(1.f, 0.f);
-      if (lane < M) {
-        y = Yseg[row.offset + lane];
-        w = __ldg(tw + ((size_t)lane << (log2twn - lm)));
-        w.y = -w.y;
-      }
-      const int jj = lane - row.dk;
-      float2 acc = make_float2(0.f, 0.f);
-      for (int n = 0; n < M; ++n) {
-        const int m = (jj * n) & (M - 1);
-        float2 yn, wm;
-        yn.x = __shfl_sync(0xffffffffu, y.x, n); yn.y = __shfl_sync(0xffffffffu, y.y, n);
-        wm.x = __shfl_sync(0xffffffffu, w.x, m); wm.y = __shfl_sync(0xffffffffu, w.y, m);
-        acc = padd(acc, pcmul(yn, wm));
-      }
-      if (lane <= 2 * row.dk) {
-        const float amp = sqrtf((float)(2 * NC) / (float)M);
-        out = pscale(acc, amp * fwin[row.woff + lane]);
+    float2 *tb = tbuf + s * 32;
+#pragma unroll
+    for (int j = 0; j < 32; ++j) tb[j] = make_float2(0.f, 0.f);
+    if (plane < 0 || row.plane == plane) {
+      const float amp = sqrtf((float)(2 * NC) / (float)(1 << row.goff));
+      float2 *Y = const_cast<float2 *>(Yseg) + row.offset;
+      switch (row.goff) {
+        case 2: tiny_row<4, false>(row, nullptr, fwin, Y, tb + row.dk, nbins, amp); break;
+        case 3: tiny_row<8, false>(row, nullptr, fwin, Y, tb + row.dk, nbins, amp); break;
+        case 4: tiny_row<16, false>(row, nullptr, fwin, Y, tb + row.dk, nbins, amp); break;
+        default: break;
       }
     }
-    tbuf[s * 32 + lane] = out;
   }
 
-  // S[f] = sum over the tiles' partial sums in tile order.  Warp w owns the bins [w BW, (w+1) BW), lane l
-  // the bins l + 32 q of that range, accumulated in registers: per tile that meets the range all the
-  // loads of a lane are independent (the partial sums come from L2).
-  constexpr int NWARP = NT / 32, BW = NC / NWARP, QB = BW / 32;
+  // S[f] = sum over the tiles' partial sums in tile order.  Thread t owns the bins f = t (mod NT): for
+  // every tile it adds the tile's values at its bins into S (shared memory), so each bin is updated by one
+  // thread, in tile order (fixed summation order, no atomics), and every thread has the same amount of work.
+  for (int f = tid; f <= NC; f += NT) S[f] = make_float2(0.f, 0.f);
   const float2 *pseg = part + (size_t)blockIdx.x * part_stride;
-  {
-    float2 acc[QB];
+  constexpr int KMAX = (kAccBins + NT - 1) / NT;
+#pragma unroll 4
+  for (int i = 0; i < n_items; ++i) {
+    const int4 b = __ldg(reinterpret_cast<const int4 *>(items + i) + 1);   // lo, nb, part_off, npass
+    const int f0 = b.x + ((tid - b.x) & (NT - 1));
+    const float2 *src = pseg + b.z - b.x;
+    float2 pv[KMAX];
 #pragma unroll
-    for (int q = 0; q < QB; ++q) acc[q] = make_float2(0.f, 0.f);
-    const int f0 = warp * BW + lane;
-#pragma unroll 1
-    for (int i = 0; i < n_items; ++i) {
-      const int4 b = __ldg(reinterpret_cast<const int4 *>(items + i) + 1);   // lo, nb, part_off, npass
-      if (b.x + b.y <= warp * BW || b.x >= (warp + 1) * BW) continue;
-      const float2 *src = pseg + b.z - b.x;
-#pragma unroll
-      for (int q = 0; q < QB; ++q) {
-        const int f = f0 + 32 * q;
-        if ((unsigned)(f - b.x) < (unsigned)b.y) acc[q] = padd(acc[q], __ldcg(src + f));
-      }
+    for (int k = 0; k < KMAX; ++k) {
+      const int f = f0 + k * NT;
+      pv[k] = (f < b.x + b.y) ? __ldcg(src + f) : make_float2(0.f, 0.f);
     }
 #pragma unroll
-    for (int q = 0; q < QB; ++q) S[f0 + 32 * q] = acc[q];
-    // the Nyquist bin: one tile per lane, fixed shuffle tree
-    if (warp == 0) {
-      float2 a = make_float2(0.f, 0.f);
-      for (int i = lane; i < n_items; i += 32) {
-        const int4 b = __ldg(reinterpret_cast<const int4 *>(items + i) + 1);
-        if ((unsigned)(NC - b.x) < (unsigned)b.y) a = padd(a, __ldcg(pseg + b.z + (NC - b.x)));
-      }
-      for (int o = 16; o > 0; o >>= 1) {
-        float2 other;
-        other.x = __shfl_xor_sync(0xffffffffu, a.x, o);
-        other.y = __shfl_xor_sync(0xffffffffu, a.y, o);
-        a = padd(a, other);
-      }
-      if (lane == 0) S[NC] = a;
+    for (int k = 0; k < KMAX; ++k) {
+      const int f = f0 + k * NT;
+      if (f < b.x + b.y) S[f] = padd(S[f], pv[k]);
     }
   }
   __syncthreads();
