@@ -193,15 +193,61 @@ int qtam_ref_fft(const double *in, double *out, int64_t n, int sign) {
   return 0;
 }
 
+// I_0(x), modified Bessel function of the first kind, by its power series sum_k ((x/2)^k / k!)^2
+static long double bessel_i0(long double x) {
+  const long double h = 0.5L * x;
+  long double term = 1.0L, sum = 1.0L;
+  for (int k = 1; k < 500; ++k) {
+    term *= (h / (long double)k) * (h / (long double)k);
+    sum += term;
+    if (term < 1e-22L * sum) break;
+  }
+  return sum;
+}
+
+// Unnormalised window value at offset j of a row with half-width dk (u = j/dk), App. A:
+//   0 bisquare (A1 :272)  (1 - u^2)^2
+//   1 Hann (A2 :276)      (1 + cos(pi u))/2
+//   2 Kaiser (A3 :280)    I0(beta sqrt(1 - u^2)) / I0(beta)
+//   3 Tukey (A4 :284)     1 for |u| <= 1 - a;  (1 + cos(pi (|u| - (1 - a))/a))/2 up to |u| = 1
+//   4 Planck-taper (A5-A6 :293-299)  1 for |u| <= 1 - a, 0 at |u| = 1, else 1/(e^Z + 1) with, d = 1 - |u|,
+//       Z = a/d + a/(d - a)   (reading R15: A6 as printed has the second denominator's sign flipped, which
+//       would make the window tend to 0 instead of 1 at the inner edge of the transition)
+static double raw_window(int type, double par, int64_t j, int64_t dk) {
+  const long double PI = 3.141592653589793238462643383279502884L;
+  const long double u = (long double)j / (long double)dk, au = fabsl(u);
+  switch (type) {
+    case 0: return (double)((1.0L - u * u) * (1.0L - u * u));
+    case 1: return (double)(0.5L * (1.0L + cosl(PI * u)));
+    case 2: return (double)(bessel_i0((long double)par * sqrtl(1.0L - u * u)) / bessel_i0((long double)par));
+    case 3: {
+      const long double a = par;
+      if (au <= 1.0L - a) return 1.0;
+      return (double)(0.5L * (1.0L + cosl(PI * (au - (1.0L - a)) / a)));
+    }
+    default: {
+      const long double a = par, d = 1.0L - au;
+      if (d >= a) return 1.0;
+      if (d <= 0.0L) return 0.0;
+      const long double Z = a / d + a / (d - a);
+      return (double)(1.0L / (expl(Z) + 1.0L));
+    }
+  }
+}
+
 int qtam_ref_plan_create(qtam_ref_plan **out, double fs, int64_t N, const double *Q, int nQ,
                          double fmin, double fmax, double spacing, const qtam_ref_options *opt) {
   if (!out || !Q || nQ < 1 || !(fs > 0) || !is_pow2(N) || N < 8) return 1;
-  if (!(fmin > 0) || !(fmax > fmin) || !(fmax < fs / 2)) return 1;
   qtam_ref_options o;
   o.window = 0; o.clamp_mode = 1; o.clamp_overlap = 1.0; o.max_window_bins = 0;
-  o.cover_floor = 1e-2; o.rows_are_bins_per_octave = 0;
+  o.cover_floor = 1e-2; o.rows_are_bins_per_octave = 0; o.window_param = 0.0; o.freqs = nullptr; o.n_freqs = 0;
   if (opt) o = *opt;
-  if (o.window != 0) return 2;
+  const bool manual = o.freqs != nullptr && o.n_freqs >= 2;
+  if (manual) { fmin = o.freqs[0]; fmax = o.freqs[o.n_freqs - 1]; }
+  if (!(fmin > 0) || !(fmax > fmin) || !(fmax < fs / 2)) return 1;
+  if (o.window < 0 || o.window > 4) return 2;
+  if (o.window == 2 && !(o.window_param > 0)) return 1;
+  if (o.window >= 3 && !(o.window_param > 0 && o.window_param <= 1.0)) return 1;
   if (!(o.clamp_overlap > 0)) o.clamp_overlap = 1.0;
   if (!(o.cover_floor > 0)) o.cover_floor = 1e-2;
 
@@ -210,7 +256,12 @@ int qtam_ref_plan_create(qtam_ref_plan **out, double fs, int64_t N, const double
 
   // frequency grid (R14)
   std::vector<double> f;
-  if (o.rows_are_bins_per_octave) {
+  if (manual) {
+    for (int r = 0; r < o.n_freqs; ++r) {
+      if (r > 0 && !(o.freqs[r] > o.freqs[r - 1])) return 1;   // ascending
+      f.push_back(o.freqs[r]);
+    }
+  } else if (o.rows_are_bins_per_octave) {
     if (!(spacing > 0)) return 1;
     for (int r = 0;; ++r) {
       double fr = fmin * std::pow(2.0, (double)r / spacing);
@@ -259,8 +310,7 @@ int qtam_ref_plan_create(qtam_ref_plan **out, double fs, int64_t N, const double
       row.wraw.resize((size_t)L); row.w.resize((size_t)L);
       ld e = 0;
       for (int64_t j = -row.dk; j <= row.dk; ++j) {
-        double u = (double)j / (double)row.dk;
-        double v = (1.0 - u * u) * (1.0 - u * u);
+        double v = raw_window(o.window, o.window_param, j, row.dk);
         row.wraw[(size_t)(j + row.dk)] = v;
         e += (ld)v * (ld)v;
       }

@@ -34,12 +34,16 @@ extern "C" {
 typedef struct qtam_ref_plan qtam_ref_plan;
 
 typedef struct {
-  int     window;                   /* 0 = bisquare (PAPER.md:67 Eq. 6, :272 Eq. A1)                 */
+  int     window;                   /* 0 bisquare (PAPER.md:67 Eq. 6, :272 A1), 1 Hann (A2 :276), 2 Kaiser
+                                       (A3 :280), 3 Tukey (A4 :284), 4 Planck-taper (A5-A6 :293-299)    */
   int     clamp_mode;               /* 0 none, 1 auto (PAPER.md:307 Eq. A7), 2 manual                */
   double  clamp_overlap;            /* multiplies N_t*Delta f_max in A7; 1.0 = paper literal (R7)    */
   int64_t max_window_bins;          /* L_max when clamp_mode == 2                                    */
   double  cover_floor;              /* R9, default 1e-2                                              */
   int     rows_are_bins_per_octave; /* 0: `spacing` = rows per plane; 1: bins per octave B (:303)    */
+  double  window_param;             /* Kaiser beta > 0, Tukey alpha_T in (0,1], Planck alpha_P in (0,1] */
+  const double *freqs;              /* manual grid (:303): n_freqs ascending centre frequencies; when    */
+  int     n_freqs;                  /* n_freqs >= 2 it replaces fmin / fmax / spacing                    */
 } qtam_ref_options;
 
 typedef struct {

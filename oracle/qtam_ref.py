@@ -20,7 +20,11 @@ _lib = None
 class Options(C.Structure):
     _fields_ = [("window", C.c_int), ("clamp_mode", C.c_int), ("clamp_overlap", C.c_double),
                 ("max_window_bins", C.c_int64), ("cover_floor", C.c_double),
-                ("rows_are_bins_per_octave", C.c_int)]
+                ("rows_are_bins_per_octave", C.c_int), ("window_param", C.c_double),
+                ("freqs", C.POINTER(C.c_double)), ("n_freqs", C.c_int)]
+
+
+WINDOWS = {"bisquare": 0, "hann": 1, "kaiser": 2, "tukey": 3, "planck": 4}
 
 
 class Row(C.Structure):
@@ -94,12 +98,16 @@ class RefPlan:
     """Oracle plan; same constructor arguments as the CUDA library's plan."""
 
     def __init__(self, fs, N, Q, fmin, fmax, spacing, clamp_mode=1, clamp_overlap=1.0,
-                 max_window_bins=0, cover_floor=1e-2, rows_are_bins_per_octave=0):
+                 max_window_bins=0, cover_floor=1e-2, rows_are_bins_per_octave=0,
+                 window="bisquare", window_param=0.0, freqs=None):
         L = lib()
         self._h = C.c_void_p()
         q = np.ascontiguousarray(Q, dtype=np.float64)
-        opt = Options(0, clamp_mode, clamp_overlap, max_window_bins, cover_floor,
-                      rows_are_bins_per_octave)
+        fr = None if freqs is None else np.ascontiguousarray(freqs, dtype=np.float64)
+        opt = Options(WINDOWS[window], clamp_mode, clamp_overlap, max_window_bins, cover_floor,
+                      rows_are_bins_per_octave, float(window_param),
+                      None if fr is None else fr.ctypes.data_as(C.POINTER(C.c_double)),
+                      0 if fr is None else fr.size)
         rc = L.qtam_ref_plan_create(C.byref(self._h), float(fs), int(N), _dp(q), q.size,
                                     float(fmin), float(fmax), float(spacing), C.byref(opt))
         if rc != 0:

@@ -465,3 +465,86 @@ def test_threshold_rowmedian_f32_bitwise(plan1k):
             t = np.float32(3.0) * m
             expect = np.where(mag < t, np.complex64(0), y)
             assert np.array_equal(out[b, p.row_slice(k)].view(np.uint32), expect.view(np.uint32))
+
+
+# ---- window families (App. A, A2-A6) and manual grids (:303) ---------------------------
+
+WINDOW_CASES = [("hann", 0.0), ("kaiser", 6.5), ("tukey", 0.4), ("planck", 0.5)]
+
+
+@pytest.mark.parametrize("name,par", WINDOW_CASES[:3])
+def test_window_families_vs_scipy(name, par):
+    """A2 / A3 / A4 sampled at j/dk equal scipy's symmetric windows of length 2 dk + 1 (an outside
+    library's own formulas: hann 0.5 - 0.5 cos(2 pi n/(L-1)), kaiser I0(beta sqrt(1-(2n/(L-1)-1)^2))/I0(beta),
+    tukey with alpha = tapered fraction), normalised to unit energy (Eq. 5 / R3)."""
+    sw = pytest.importorskip("scipy.signal.windows")
+    ref = {"hann": lambda L: sw.hann(L, sym=True), "kaiser": lambda L: sw.kaiser(L, par),
+           "tukey": lambda L: sw.tukey(L, par)}[name]
+    p = RefPlan(1024.0, 1024, [4.0, 8.0], 16.0, 400.0, 12, window=name, window_param=par)
+    for k, r in enumerate(p.rows):
+        w = ref(r.L)
+        assert np.abs(p.window(k) - w / np.sqrt(np.sum(w ** 2))).max() <= 1e-14
+
+
+def test_planck_taper_closed_form_values():
+    """A5/A6 (reading R15): with d = 1 - |u|, Z = a/d + a/(d - a): W = 1 on |u| <= 1 - a, W = 1/2 at
+    d = a/2 (Z = 0), W = 1/(e^{8/3} + 1) at d = a/4 (Z = 4 - 4/3), W = 0 at |u| = 1; even, non-increasing
+    in |u|.  dk = 40 and a = 1/2 put those points on the integer offsets 30 and 35."""
+    p = RefPlan(1024.0, 1024, [4.0], 16.0, 400.0, 12, clamp_mode=2, max_window_bins=81,
+                window="planck", window_param=0.5)
+    k = [i for i, r in enumerate(p.rows) if r.dk == 40][0]
+    w = p.window(k)
+    raw = w / w[40]                        # centre value is 1 before normalisation
+    assert np.all(raw[20:61] == 1.0)       # |j| <= 20 = dk (1 - a)
+    assert abs(raw[40 + 30] - 0.5) <= 1e-15 and abs(raw[40 - 30] - 0.5) <= 1e-15
+    assert abs(raw[40 + 35] - 1.0 / (np.exp(8.0 / 3.0) + 1.0)) <= 1e-15
+    assert raw[0] == 0.0 and raw[80] == 0.0
+    assert np.array_equal(raw, raw[::-1])
+    assert np.all(np.diff(raw[40:]) <= 0)
+    assert abs(np.sum(w ** 2) - 1.0) <= 1e-14      # Eq. 5 / R3
+
+
+@pytest.mark.parametrize("name,par", WINDOW_CASES)
+def test_window_families_round_trip_and_frame_energy(name, par):
+    """P4 and P6 hold for any window: exact reconstruction on the cover set (C44-C45 :566-577) and
+    sum |Y|^2 = (1/N) sum_f |X|^2 P (C36 :536, one-sided weights)."""
+    p = RefPlan(1024.0, 1024, [4.0, 8.0, 16.0], 16.0, 400.0, 12, window=name, window_param=par, clamp_overlap=2.0)
+    x = inputs.white_noise(p.N, 61, batch=2)
+    Y = p.forward(x, engine=0)
+    X = np.fft.rfft(x, axis=-1)
+    P, C = p.frame(-1)
+    proj = np.fft.irfft(np.where(C[None, :], X, 0), n=p.N, axis=-1)
+    assert rel_l2(p.inverse(Y, engine=0), proj) <= 1e-12
+    for b in range(2):
+        lhs = np.sum(np.abs(Y[b]) ** 2)
+        rhs = np.sum(np.abs(X[b]) ** 2 * P) / p.N
+        assert abs(lhs - rhs) <= 1e-12 * rhs
+    # the forward against the library construction (rfft, windowed band, ifft) for this window
+    for k, r in enumerate(p.rows):
+        w = p.window(k)
+        B = np.zeros(r.M, complex)
+        for j in range(-r.dk, r.dk + 1):
+            if 0 <= r.kc + j < p.n_bins:
+                B[j % r.M] = X[0][r.kc + j] * w[j + r.dk]
+        assert rel_l2(Y[0][p.row_slice(k)], np.fft.ifft(B) * np.sqrt(r.M / p.N)) <= 1e-12
+
+
+def test_manual_frequency_grid():
+    """:303 "defined ... manually, by passing a specific list of target frequencies": centre bins
+    floor(f T + 1/2) (R2), clamp A7 from the largest gap of the list, round trip exact on the cover set."""
+    freqs = [20.0, 30.0, 47.0, 80.0, 150.0, 260.0, 400.0]
+    fs, N = 1024.0, 2048
+    T = N / fs
+    p = RefPlan(fs, N, [4.0, 12.0], 0.0, 0.0, 0, freqs=freqs)
+    assert p.n_rows == 2 * len(freqs)
+    Lmax = 2 * (int(np.ceil(T * 140.0)) // 2) + 1          # A7 with the largest gap, 400 - 260 = 140 Hz
+    for i, r in enumerate(p.rows):
+        f = freqs[i % len(freqs)]
+        assert r.kc == int(np.floor(f * T + 0.5))
+        assert r.L == min(2 * int(np.floor(f * T * np.sqrt(11.0) / r.q)) + 1, Lmax)
+    x = inputs.white_noise(N, 62)
+    _, C = p.frame(-1)
+    proj = np.fft.irfft(np.where(C[None, :], np.fft.rfft(x, axis=-1), 0), n=N, axis=-1)
+    assert rel_l2(p.inverse(p.forward(x, engine=1), engine=1), proj) <= 1e-12
+    with pytest.raises(ValueError):
+        RefPlan(fs, N, [4.0], 0.0, 0.0, 0, freqs=[20.0, 20.0, 30.0])      # not ascending
