@@ -53,7 +53,10 @@ typedef enum {
 /* All fields optional; pass NULL for the defaults. struct_size = sizeof(qtam_options) (ABI version). */
 typedef struct {
   size_t  struct_size;
-  int     window;                   /* 0 = bisquare (Eq. 6); the only one implemented */
+  int     window;                   /* PAPER.md App. A: 0 bisquare (Eq. 6 :67, A1 :272) [default], 1 Hann
+                                       (A2 :276), 2 Kaiser (A3 :280), 3 Tukey (A4 :284), 4 Planck-taper
+                                       (A5-A6 :293-299, R15).  The half-width is the same for
+                                       every family (R1)                                               */
   int     clamp_mode;               /* 0 none, 1 auto = Eq. A7 [default], 2 manual  */
   double  clamp_overlap;            /* multiplies N_t*Delta f_max in A7; default 1.0 = paper (R7)  */
   int64_t max_window_bins;          /* L_max when clamp_mode == 2                                  */
@@ -62,6 +65,10 @@ typedef struct {
   int     rows_are_bins_per_octave; /* 0: `spacing` = rows per plane, endpoints inclusive;
                                        1: `spacing` = bins per octave B, f = fmin*2^(r/B) (:303)   */
   int     max_batch;                /* workspace is sized for this many segments; default 1        */
+  double  window_param;             /* Kaiser beta > 0; Tukey alpha_T, Planck alpha_P in (0, 1]     */
+  const double *freqs;              /* manual grid (:303): n_freqs ascending centre frequencies in Hz
+                                       (host pointer, read during plan creation only); when           */
+  int     n_freqs;                  /* n_freqs >= 2 they replace fmin / fmax / spacing              */
 } qtam_options;
 
 /* Host-side row table entry; rows are ordered plane-major (Q list order), ascending frequency. */
@@ -81,7 +88,7 @@ typedef struct {
 } qtam_info;
 
 /* Plan (host, once): frequency grid f_r = fmin*(fmax/fmin)^(r/(R-1)) or fmin*2^(r/B),
- * centre bins, bandwidths, clamp A7/A8 (:307-311), bisquare windows and their normalisation
+ * centre bins, bandwidths, clamp A7/A8 (:307-311), the windows (App. A) and their normalisation
  * (Eq. 5-7 :63-72), output lengths, the frame operator and cover sets, device tables + workspace.
  * Q: nQ quality factors (host pointer), one plane each.  *out is written only on QTAM_OK. */
 qtam_status qtam_plan_create(qtam_plan **out, double fs, int64_t N, const double *Q, int nQ,

@@ -217,7 +217,7 @@ static double raw_window(int type, double par, int64_t j, int64_t dk) {
   const long double PI = 3.141592653589793238462643383279502884L;
   const long double u = (long double)j / (long double)dk, au = fabsl(u);
   switch (type) {
-    case 0: return (double)((1.0L - u * u) * (1.0L - u * u));
+    case 0: { const double ud = (double)j / (double)dk; return (1.0 - ud * ud) * (1.0 - ud * ud); }   // as before the families
     case 1: return (double)(0.5L * (1.0L + cosl(PI * u)));
     case 2: return (double)(bessel_i0((long double)par * sqrtl(1.0L - u * u)) / bessel_i0((long double)par));
     case 3: {

@@ -32,7 +32,11 @@ class Options(C.Structure):
     _fields_ = [("struct_size", C.c_size_t), ("window", C.c_int), ("clamp_mode", C.c_int),
                 ("clamp_overlap", C.c_double), ("max_window_bins", C.c_int64),
                 ("cover_floor", C.c_double), ("rows_are_bins_per_octave", C.c_int),
-                ("max_batch", C.c_int)]
+                ("max_batch", C.c_int), ("window_param", C.c_double),
+                ("freqs", C.POINTER(C.c_double)), ("n_freqs", C.c_int)]
+
+
+WINDOWS = {"bisquare": 0, "hann": 1, "kaiser": 2, "tukey": 3, "planck": 4}
 
 
 class Row(C.Structure):
@@ -96,13 +100,16 @@ class Plan:
 
     def __init__(self, fs, N, Q, fmin, fmax, spacing, dtype="f32", max_batch=1, clamp_mode=1,
                  clamp_overlap=1.0, max_window_bins=0, cover_floor=1e-2, rows_are_bins_per_octave=0,
-                 host_only=False):
+                 host_only=False, window="bisquare", window_param=0.0, freqs=None):
         L = lib()
         self._h = C.c_void_p()
         self.dtype = dtype
         q = np.ascontiguousarray(Q, dtype=np.float64)
-        opt = Options(C.sizeof(Options), 0, clamp_mode, clamp_overlap, max_window_bins, cover_floor,
-                      rows_are_bins_per_octave, max_batch)
+        fr = None if freqs is None else np.ascontiguousarray(freqs, dtype=np.float64)
+        opt = Options(C.sizeof(Options), WINDOWS[window], clamp_mode, clamp_overlap, max_window_bins,
+                      cover_floor, rows_are_bins_per_octave, max_batch, float(window_param),
+                      None if fr is None else fr.ctypes.data_as(C.POINTER(C.c_double)),
+                      0 if fr is None else fr.size)
         fn = L.qtam_plan_create_host if host_only else L.qtam_plan_create
         code = fn(C.byref(self._h), float(fs), int(N), q.ctypes.data_as(C.POINTER(C.c_double)), q.size,
                   float(fmin), float(fmax), float(spacing), QTAM_F64 if dtype == "f64" else QTAM_F32,

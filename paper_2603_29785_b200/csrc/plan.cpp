@@ -10,10 +10,31 @@ namespace qtam {
 
 static bool pow2(int64_t v) { return v > 0 && (v & (v - 1)) == 0; }
 
+// Unnormalised window value at offset j of a row with half-width dk, u = j/dk (App. A):
+// bisquare A1 :272, Hann A2 :276, Kaiser A3 :280 (I_0 from <cmath>), Tukey A4 :284, Planck-taper A5-A6
+// :293-299 with Z = a/d + a/(d - a), d = 1 - |u| (R15).
+static double window_value(int type, double par, int64_t j, int64_t dk) {
+  const double pi = 3.14159265358979323846;
+  const double u = double(j) / double(dk), au = std::fabs(u);
+  switch (type) {
+    case 1: return 0.5 * (1.0 + std::cos(pi * u));
+    case 2: return std::cyl_bessel_i(0.0, par * std::sqrt(std::max(0.0, 1.0 - u * u))) / std::cyl_bessel_i(0.0, par);
+    case 3:
+      if (au <= 1.0 - par) return 1.0;
+      return 0.5 * (1.0 + std::cos(pi * (au - (1.0 - par)) / par));
+    case 4: {
+      const double d = 1.0 - au;
+      if (d >= par) return 1.0;
+      if (d <= 0.0) return 0.0;
+      return 1.0 / (std::exp(par / d + par / (d - par)) + 1.0);
+    }
+    default: return (1.0 - u * u) * (1.0 - u * u);
+  }
+}
+
 qtam_status build_host_plan(HostPlan &hp, double fs, int64_t N, const double *Q, int nQ, double fmin,
                             double fmax, double spacing, qtam_dtype dtype, const qtam_options *uopt) {
   if (!Q || nQ < 1 || !(fs > 0.0) || !pow2(N) || N < 8) return QTAM_ERR_INVALID_ARG;
-  if (!(fmin > 0.0) || !(fmax > fmin) || !(fmax < 0.5 * fs)) return QTAM_ERR_INVALID_ARG;
   if (dtype != QTAM_F32 && dtype != QTAM_F64) return QTAM_ERR_INVALID_ARG;
   if (N > (int64_t(1) << 26)) return QTAM_ERR_UNSUPPORTED;
 
@@ -30,16 +51,27 @@ qtam_status build_host_plan(HostPlan &hp, double fs, int64_t N, const double *Q,
     if (!(o.cover_floor > 0.0)) o.cover_floor = 1e-2;
     if (o.max_batch < 1) o.max_batch = 1;
   }
-  if (o.window != 0) return QTAM_ERR_UNSUPPORTED;
+  if (o.window < 0 || o.window > 4) return QTAM_ERR_UNSUPPORTED;
+  if (o.window == 2 && !(o.window_param > 0.0)) return QTAM_ERR_INVALID_ARG;
+  if (o.window >= 3 && !(o.window_param > 0.0 && o.window_param <= 1.0)) return QTAM_ERR_INVALID_ARG;
+  const bool manual = o.freqs != nullptr && o.n_freqs >= 2;
+  if (manual) { fmin = o.freqs[0]; fmax = o.freqs[o.n_freqs - 1]; }
+  if (!(fmin > 0.0) || !(fmax > fmin) || !(fmax < 0.5 * fs)) return QTAM_ERR_INVALID_ARG;
   if (o.clamp_mode < 0 || o.clamp_mode > 2) return QTAM_ERR_INVALID_ARG;
 
   hp.fs = fs; hp.N = N; hp.nb = N / 2 + 1; hp.nP = nQ; hp.dtype = dtype; hp.opt = o;
+  hp.opt.freqs = nullptr;                     // the caller's list is only read here
   const double dur = double(N) / fs;          // N_t of the paper (:75)
   const double tile_c = std::sqrt(11.0);      // R1
 
   // centre frequencies (:303, R14)
   std::vector<double> fc;
-  if (o.rows_are_bins_per_octave) {
+  if (manual) {
+    for (int r = 0; r < o.n_freqs; ++r) {
+      if (r > 0 && !(o.freqs[r] > o.freqs[r - 1])) return QTAM_ERR_INVALID_ARG;   // ascending
+      fc.push_back(o.freqs[r]);
+    }
+  } else if (o.rows_are_bins_per_octave) {
     if (!(spacing > 0.0)) return QTAM_ERR_INVALID_ARG;
     for (int r = 0; r < (1 << 20); ++r) {
       const double v = fmin * std::pow(2.0, double(r) / spacing);
@@ -86,13 +118,12 @@ qtam_status build_host_plan(HostPlan &hp, double fs, int64_t N, const double *Q,
       h.f_center = double(h.kc) / dur;
       h.offset = coff; coff += m;
       h.woff = woff; h.goff = woff; woff += len;
-      // bisquare (Eq. 6 :67), unit l2 energy over the unclipped support (Eq. 5 :63, R3, R8)
+      // the window (App. A), unit l2 energy over the unclipped support (Eq. 5 :63, R3, R8)
       const size_t base = hp.win.size();
       hp.win.resize(base + size_t(len));
       long double energy = 0.0L;
       for (int64_t j = -h.dk; j <= h.dk; ++j) {
-        const double u = double(j) / double(h.dk);
-        const double raw = (1.0 - u * u) * (1.0 - u * u);
+        const double raw = window_value(o.window, o.window_param, j, h.dk);
         hp.win[base + size_t(j + h.dk)] = raw;
         energy += (long double)raw * (long double)raw;
       }

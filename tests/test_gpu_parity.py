@@ -167,6 +167,40 @@ def test_mid_length_segments(log2n):
     assert worst_segment(g.inverse(g.forward(dev(x))).cpu().numpy(), pi_c(x64, C)) <= 1e-5
 
 
+@pytest.mark.parametrize("window,par", [("hann", 0.0), ("kaiser", 6.5), ("tukey", 0.4), ("planck", 0.5)])
+@pytest.mark.parametrize("dtype", ["f32", "f64"])
+def test_window_families(window, par, dtype):
+    """App. A, A2-A6: the kernels read the plan's window tables, so every family runs the same path."""
+    args = (4096.0, 8192, [5.0, 10.0, 20.0], 10.0, 1900.0, 24.0)
+    g, r = make_plans(args, dtype, 2, window=window, window_param=par)
+    for k in (0, g.n_rows // 2, g.n_rows - 1):
+        assert np.abs(g.window(k) - r.window(k)).max() <= 1e-14 * r.window(k).max()
+    x = inputs.white_noise(args[1], 71, batch=2).astype(np_rdt(dtype))
+    x64 = x.astype(np.float64)
+    Yg = g.forward(dev(x)).cpu().numpy()
+    assert worst_segment(Yg, r.forward(x64, engine=1)) <= TOL[dtype]
+    rng = np.random.default_rng(72)
+    Yin = (rng.standard_normal((2, g.ctot)) + 1j * rng.standard_normal((2, g.ctot))).astype(Yg.dtype)
+    for plane in (-1, 1):
+        xg = g.inverse(dev(Yin), plane=plane).cpu().numpy()
+        assert worst_segment(xg, r.inverse(Yin.astype(np.complex128), plane=plane, engine=1)) <= TOL[dtype]
+    _, C = r.frame(-1)
+    assert worst_segment(g.inverse(g.forward(dev(x))).cpu().numpy(), pi_c(x64, C)) <= TOL_RT[dtype]
+
+
+def test_manual_frequency_grid_on_gpu():
+    freqs = [20.0, 30.0, 47.0, 80.0, 150.0, 260.0, 400.0, 700.0, 1100.0, 1500.0, 1900.0]
+    kw = dict(freqs=freqs)
+    g = binding.Plan(4096.0, 16384, [4.0, 12.0, 40.0], 0.0, 0.0, 0.0, dtype="f32", max_batch=2, **kw)
+    r = RefPlan(4096.0, 16384, [4.0, 12.0, 40.0], 0.0, 0.0, 0.0, **kw)
+    assert [(a.kc, a.dk, a.M, a.offset) for a in g.rows] == [(b.kc, b.dk, b.M, b.offset) for b in r.rows]
+    x = inputs.white_noise(16384, 73, batch=2).astype(np.float32)
+    x64 = x.astype(np.float64)
+    assert worst_segment(g.forward(dev(x)).cpu().numpy(), r.forward(x64, engine=1)) <= 2e-5
+    _, C = r.frame(-1)
+    assert worst_segment(g.inverse(g.forward(dev(x))).cpu().numpy(), pi_c(x64, C)) <= 1e-5
+
+
 def test_cfg5_fp64_variant():
     name = "cfg5"
     g, r = make_plans(inputs.plan_args(name), "f64", 4)

@@ -116,3 +116,35 @@ def test_product_package_does_not_touch_the_oracle():
             if f.endswith((".py", ".cu", ".cpp", ".hpp", ".cuh", ".h")):
                 src = open(os.path.join(dirpath, f)).read()
                 assert "qtam_ref" not in src and "import oracle" not in src and "from oracle" not in src, f
+
+
+@pytest.mark.parametrize("window,par", [("hann", 0.0), ("kaiser", 6.5), ("tukey", 0.4), ("planck", 0.5)])
+def test_window_families_host_plan_matches_oracle(window, par):
+    """App. A, A2-A6: the library's window tables (its own evaluation, Bessel I_0 from <cmath>) against
+    the oracle's (power series in long double); cover sets equal, P to a few ulp."""
+    args = (4096.0, 4096, [4.0, 8.0, 16.0], 16.0, 1024.0, 32)
+    p = binding.Plan(*args, dtype="f64", host_only=True, window=window, window_param=par)
+    r = RefPlan(*args, window=window, window_param=par)
+    assert [(a.kc, a.dk, a.M, a.offset) for a in p.rows] == [(b.kc, b.dk, b.M, b.offset) for b in r.rows]
+    for k in range(p.n_rows):
+        wb = r.window(k)
+        assert np.max(np.abs(p.window(k) - wb)) <= 1e-14 * np.max(wb)     # cyl_bessel_i is good to a few ulp
+    Pa, Ca = p.frame(-1)
+    Pb, Cb = r.frame(-1)
+    assert np.array_equal(Ca, Cb)
+    assert np.max(np.abs(Pa - Pb)) <= 1e-14 * np.max(Pb)
+
+
+def test_window_parameters_and_manual_grid_are_validated():
+    args = (4096.0, 4096, [4.0, 8.0], 16.0, 1024.0, 16)
+    with pytest.raises(binding.QtamError):
+        binding.Plan(*args, host_only=True, window="kaiser", window_param=0.0)
+    with pytest.raises(binding.QtamError):
+        binding.Plan(*args, host_only=True, window="tukey", window_param=1.5)
+    with pytest.raises(binding.QtamError):
+        binding.Plan(4096.0, 4096, [4.0], 0.0, 0.0, 0.0, host_only=True, freqs=[50.0, 40.0, 90.0])
+    freqs = [20.0, 30.0, 47.0, 80.0, 150.0, 260.0, 400.0]
+    p = binding.Plan(4096.0, 4096, [4.0, 12.0], 0.0, 0.0, 0.0, host_only=True, freqs=freqs)
+    r = RefPlan(4096.0, 4096, [4.0, 12.0], 0.0, 0.0, 0.0, freqs=freqs)
+    assert [(a.kc, a.dk, a.M, a.offset, a.f_request) for a in p.rows] == \
+           [(b.kc, b.dk, b.M, b.offset, b.f_request) for b in r.rows]
