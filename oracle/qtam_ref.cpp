@@ -630,4 +630,31 @@ int qtam_ref_threshold_rowmedian_f32(const qtam_ref_plan *p, float *coef, int ba
   return 0;
 }
 
+// Multi-Q scan: per (segment, Q-plane) a quality metric of the plane's spectrogram
+// |Y_k[n]|^2 -- metric 0: total energy sum_{k in plane} sum_n |Y_k[n]|^2, metric 1: peak pixel
+// max_{k,n} |Y_k[n]|^2 -- and "optimal selection": the plane with the largest metric, independently for
+// every segment (lowest plane index on ties).
+int qtam_ref_plane_metric(const qtam_ref_plan *p, const double *coef, int batch, int metric,
+                          double *out_metric, int32_t *out_best) {
+  if (!p || !coef || batch < 0 || !out_metric || metric < 0 || metric > 1) return 1;
+  for (int b = 0; b < batch; ++b) {
+    std::vector<ld> val((size_t)p->nP, 0.0L);
+    for (const Row &r : p->rows) {
+      const cd *Y = reinterpret_cast<const cd *>(coef) + (size_t)b * p->ctot + r.offset;
+      for (int64_t n = 0; n < r.M; ++n) {
+        const ld e = (ld)Y[n].real() * (ld)Y[n].real() + (ld)Y[n].imag() * (ld)Y[n].imag();
+        if (metric == 0) val[(size_t)r.plane] += e;
+        else if (e > val[(size_t)r.plane]) val[(size_t)r.plane] = e;
+      }
+    }
+    int best = 0;
+    for (int q = 0; q < p->nP; ++q) {
+      out_metric[(size_t)b * p->nP + q] = (double)val[(size_t)q];
+      if (val[(size_t)q] > val[(size_t)best]) best = q;
+    }
+    if (out_best) out_best[b] = best;
+  }
+  return 0;
+}
+
 }  // extern "C"

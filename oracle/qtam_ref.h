@@ -88,6 +88,12 @@ int  qtam_ref_brute_tile(const qtam_ref_plan *p, const double *x, int row, doubl
  * stated in DESIGN.md ("threshold arithmetic") so that a float kernel can match it bit for bit. */
 int  qtam_ref_threshold_rowmedian(const qtam_ref_plan *p, double *coef, int batch, double kappa);
 int  qtam_ref_threshold_rowmedian_f32(const qtam_ref_plan *p, float *coef, int batch, float kappa);
+
+/* Multi-Q scan: out_metric[batch][n_planes] = total energy (metric 0) or peak pixel
+ * (metric 1) of every plane's |Y|^2, out_best[batch] = the plane with the largest value per segment
+ * (lowest index on ties; may be NULL). */
+int  qtam_ref_plane_metric(const qtam_ref_plan *p, const double *coef, int batch, int metric,
+                           double *out_metric, int32_t *out_best);
 /* Projection onto the cover set: one-sided DFT of x, zero the bins outside C, inverse (R9). */
 int  qtam_ref_project_cover(const qtam_ref_plan *p, const double *x, int batch, int plane,
                             double *x_out, int engine);

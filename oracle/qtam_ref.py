@@ -59,6 +59,7 @@ def lib():
         _lib.qtam_ref_brute_tile.argtypes = [vp, dp, C.c_int, dp]
         _lib.qtam_ref_threshold_rowmedian.argtypes = [vp, dp, C.c_int, C.c_double]
         _lib.qtam_ref_threshold_rowmedian_f32.argtypes = [vp, fp, C.c_int, C.c_float]
+        _lib.qtam_ref_plane_metric.argtypes = [vp, dp, C.c_int, C.c_int, dp, C.POINTER(C.c_int32)]
         _lib.qtam_ref_project_cover.argtypes = [vp, dp, C.c_int, C.c_int, dp, C.c_int]
         _lib.qtam_ref_spectrum.argtypes = [vp, dp, C.c_int, dp, C.c_int]
         _lib.qtam_ref_dft.argtypes = [dp, dp, C.c_int64, C.c_int]
@@ -185,6 +186,17 @@ class RefPlan:
             c = c[None, :]
         assert lib().qtam_ref_threshold_rowmedian(self._h, _dp(c.view(np.float64)), c.shape[0], kappa) == 0
         return c
+
+    def plane_metric(self, coef, metric="energy"):
+        """(values[batch][n_planes], best[batch]) of the multi-Q scan's plane selection"""
+        c = np.ascontiguousarray(np.atleast_2d(coef), dtype=np.complex128)
+        vals = np.zeros((c.shape[0], self.n_planes))
+        best = np.zeros(c.shape[0], dtype=np.int32)
+        rc = lib().qtam_ref_plane_metric(self._h, _dp(c.view(np.float64)), c.shape[0],
+                                         {"energy": 0, "peak": 1}[metric], _dp(vals),
+                                         best.ctypes.data_as(C.POINTER(C.c_int32)))
+        assert rc == 0
+        return vals, best
 
     def threshold_f32(self, coef, kappa=3.0):
         c = np.array(coef, dtype=np.complex64, order="C", copy=True)

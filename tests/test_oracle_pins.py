@@ -548,3 +548,39 @@ def test_manual_frequency_grid():
     assert rel_l2(p.inverse(p.forward(x, engine=1), engine=1), proj) <= 1e-12
     with pytest.raises(ValueError):
         RefPlan(fs, N, [4.0], 0.0, 0.0, 0, freqs=[20.0, 20.0, 30.0])      # not ascending
+
+
+# ---- multi-Q scan: plane metric and optimal-plane selection ----------------------
+
+def test_plane_energy_is_the_per_plane_frame_energy():
+    """metric 0 against C36 (:536) restricted to one plane: sum_{k in plane, n} |Y_k[n]|^2 =
+    (1/N) sum_f w_f |X[f]|^2 P_plane[f] ... evaluated with numpy's rfft and the plan's own P_plane."""
+    p = RefPlan(1024.0, 1024, [4.0, 8.0, 16.0], 16.0, 400.0, 12)
+    x = inputs.white_noise(p.N, 81, batch=3)
+    vals, best = p.plane_metric(p.forward(x, engine=0), "energy")
+    X = np.fft.rfft(x, axis=-1)
+    for q in range(p.n_planes):
+        Pq, _ = p.frame(q)
+        expect = np.sum(np.abs(X) ** 2 * Pq[None, :], axis=-1) / p.N
+        assert np.max(np.abs(vals[:, q] - expect) / expect) <= 1e-12
+    assert np.array_equal(best, np.argmax(vals, axis=1))
+
+
+def test_plane_peak_of_a_pure_sinusoid_closed_form():
+    """metric 1 against P7's closed form: for x = cos(2 pi k0 n/N) every pixel of row k has
+    |Y_k[n]|^2 = (N/M_k) W_k[k0 - kc]^2 / 4, so a plane's peak is the largest such value over its rows, and
+    the optimal plane is the one that holds it."""
+    p = RefPlan(1024.0, 1024, [4.0, 8.0, 16.0], 16.0, 400.0, 12)
+    k0 = 93
+    x = np.cos(2 * np.pi * k0 * np.arange(p.N) / p.N)
+    vals, best = p.plane_metric(p.forward(x, engine=0), "peak")
+    expect = np.zeros(p.n_planes)
+    for k, r in enumerate(p.rows):
+        j = k0 - r.kc
+        if abs(j) <= r.dk:
+            expect[r.plane] = max(expect[r.plane], (p.N / r.M) * p.window(k)[j + r.dk] ** 2 / 4.0)
+    assert np.max(np.abs(vals[0] - expect)) <= 1e-12 * expect.max()
+    assert best[0] == int(np.argmax(expect))
+    # scaling one segment changes its metrics quadratically and not its choice; selection is per segment
+    v2, b2 = p.plane_metric(p.forward(np.stack([x, 3.0 * x]), engine=0), "peak")
+    assert np.allclose(v2[1], 9.0 * v2[0], rtol=1e-12) and b2[0] == b2[1] == best[0]
