@@ -132,6 +132,16 @@ qtam_status qtam_dense(qtam_plan *p, const void *d_x, int batch, int row_begin, 
 qtam_status qtam_threshold_rowmedian(qtam_plan *p, void *d_coef, int batch, double kappa,
                                      void *stream);
 
+/* Multi-Q scan selection ("for each resolution plane ... a signal quality metric (e.g., total
+ * energy or peak pixel intensity)"; "optimal selection mode ... independently for each signal in the batch").
+ * metric 0: sum over the plane's rows k and samples n of |Y_k[n]|^2; metric 1: max of |Y_k[n]|^2.
+ * d_coef: [batch][coeffs_per_segment] as written by qtam_forward (not modified).
+ * d_metric: [batch][n_planes] real of the plan's dtype (device, caller-owned, overwritten).
+ * d_best: [batch] int32 (device) = the plane with the largest metric, lowest index on ties; may be NULL. */
+typedef enum { QTAM_METRIC_ENERGY = 0, QTAM_METRIC_PEAK = 1 } qtam_metric;
+qtam_status qtam_plane_metric(qtam_plan *p, const void *d_coef, int batch, int metric, void *d_metric,
+                              int32_t *d_best, void *stream);
+
 /* Number of kernel launches the last forward / inverse / threshold / dense call on this plan issued
  * (host counter, for bench.py's gpu_launches). */
 int         qtam_last_launch_count(const qtam_plan *p);

@@ -18,7 +18,7 @@ STATUS = {0: "ok", 1: "invalid argument", 2: "unsupported", 3: "alloc", 4: "cuda
 
 SYMBOLS = ["qtam_plan_create", "qtam_plan_create_host", "qtam_plan_destroy", "qtam_plan_info",
            "qtam_plan_rows", "qtam_plan_window", "qtam_plan_frame", "qtam_forward", "qtam_inverse",
-           "qtam_dense", "qtam_threshold_rowmedian", "qtam_last_launch_count", "qtam_status_string",
+           "qtam_dense", "qtam_threshold_rowmedian", "qtam_plane_metric", "qtam_last_launch_count", "qtam_status_string",
            "qtam_profile_enable", "qtam_profile_read"]
 
 
@@ -79,6 +79,7 @@ def lib():
         L.qtam_inverse.argtypes = [vp, vp, C.c_int, C.c_int, vp, vp]
         L.qtam_dense.argtypes = [vp, vp, C.c_int, C.c_int, C.c_int, vp, vp]
         L.qtam_threshold_rowmedian.argtypes = [vp, vp, C.c_int, C.c_double, vp]
+        L.qtam_plane_metric.argtypes = [vp, vp, C.c_int, C.c_int, vp, vp, vp]
         L.qtam_last_launch_count.argtypes = [vp]
         L.qtam_last_launch_count.restype = C.c_int
         L.qtam_status_string.argtypes = [C.c_int]
@@ -206,6 +207,17 @@ class Plan:
         _check(lib().qtam_threshold_rowmedian(self._h, coef.data_ptr(), batch, float(kappa), self._stream()),
                "qtam_threshold_rowmedian")
         return coef
+
+    def plane_metric(self, coef, metric="energy"):
+        """(values[batch][n_planes], best[batch] int32) of the multi-Q scan's plane selection"""
+        t = self._torch()
+        assert coef.is_cuda and coef.dtype == self._cdt() and coef.is_contiguous()
+        batch = coef.numel() // self.ctot
+        vals = t.empty((batch, self.n_planes), dtype=self._rdt(), device=coef.device)
+        best = t.empty((batch,), dtype=t.int32, device=coef.device)
+        _check(lib().qtam_plane_metric(self._h, coef.data_ptr(), batch, {"energy": 0, "peak": 1}[metric],
+                                       vals.data_ptr(), best.data_ptr(), self._stream()), "qtam_plane_metric")
+        return vals, best
 
     def last_launch_count(self):
         return int(lib().qtam_last_launch_count(self._h))

@@ -41,7 +41,7 @@ void free_plan(qtam_plan *p) {
   if (!p) return;
   if (p->host_only) { delete p; return; }
   cudaFree(p->d_rows); cudaFree(p->d_win); cudaFree(p->d_tw); cudaFree(p->d_invP);
-  cudaFree(p->d_csr_ptr); cudaFree(p->d_csr_idx); cudaFree(p->d_csrj_ptr); cudaFree(p->d_csrj_idx);
+  cudaFree(p->d_csr_ptr); cudaFree(p->d_csr_idx); cudaFree(p->d_csrj_ptr); cudaFree(p->d_csrj_idx); cudaFree(p->d_plane_off);
   for (int c = 0; c < qtam_plan::kClasses; ++c) cudaFree(p->d_items[c]);
   cudaFree(p->d_bigrows); cudaFree(p->d_spec_alloc); cudaFree(p->d_ws); cudaFree(p->d_band);
   cudaFree(p->d_fwinp); cudaFree(p->d_red);
@@ -248,6 +248,11 @@ template <typename T> qtam_status build_device(qtam_plan *p) {
     T *d = nullptr;
     if (!upload(&d, ip.data(), ip.size(), tot)) return QTAM_ERR_ALLOC;
     p->d_invP = d;
+  }
+  {
+    std::vector<long long> po(size_t(hp.nP) + 1, hp.ctot);
+    for (size_t k = hp.rows.size(); k-- > 0;) po[size_t(hp.rows[k].plane)] = hp.rows[k].offset;
+    if (!upload(&p->d_plane_off, po.data(), po.size(), tot)) return QTAM_ERR_ALLOC;
   }
   if (!upload(&p->d_csr_ptr, hp.csr_ptr.data(), hp.csr_ptr.size(), tot)) return QTAM_ERR_ALLOC;
   if (!upload(&p->d_csr_idx, hp.csr_idx.data(), hp.csr_idx.size(), tot)) return QTAM_ERR_ALLOC;
@@ -473,13 +478,22 @@ qtam_status qtam_threshold_rowmedian(qtam_plan *p, void *d_coef, int batch, doub
   return generic_threshold(p, d_coef, batch, kappa, p->n_thr_tasks > 0 ? kThrFastLog2Max + 1 : 0, st);
 }
 
+qtam_status qtam_plane_metric(qtam_plan *p, const void *d_coef, int batch, int metric, void *d_metric,
+                              int32_t *d_best, void *stream) {
+  if (p && p->host_only) return QTAM_ERR_CUDA;
+  if (!check_call(p, d_coef, d_metric, batch) || metric < 0 || metric > 1) return QTAM_ERR_INVALID_ARG;
+  p->last_launches = 0;
+  if (batch == 0) return QTAM_OK;
+  return plane_metric(p, d_coef, batch, metric, d_metric, d_best, static_cast<cudaStream_t>(stream));
+}
+
 int qtam_last_launch_count(const qtam_plan *p) { return p ? p->last_launches : 0; }
 
 static const char *const kKernelNames[K_COUNT] = {
     "cfft_seq", "cfft_cols", "cfft_rows", "r2c_post", "c2r_pre", "fwd_rows", "fwd_combine",
     "inv_rows", "inv_reduce", "dense_place", "threshold", "r2c_fast", "fwd_rows_fast", "inv_rows_fast",
     "reduce_c2r_fast", "inv_fused", "inv_tiles", "combine_c2r", "threshold_fast", "rows_cta_fwd", "rows_cta_inv",
-    "tiny_rows_fwd", "tiny_rows_inv", "long_fft_a", "long_fft_b"};
+    "tiny_rows_fwd", "tiny_rows_inv", "long_fft_a", "long_fft_b", "plane_metric", "best_plane"};
 
 qtam_status qtam_profile_enable(qtam_plan *p, int on, int max_launches) {
   if (!p || p->host_only) return QTAM_ERR_INVALID_ARG;

@@ -1,0 +1,100 @@
+// scan.cu -- multi-Q scan selection: per (segment, Q-plane) a quality metric of the plane's
+// spectrogram |Y_k[n]|^2 (total energy or peak pixel) and, per segment, the plane that maximises it.
+// The coefficients of a plane are contiguous in the ABI layout (rows are plane-major), so the metric is one
+// streaming reduction per (plane, segment): one CTA each, 128-bit loads, per-thread partial results in the
+// plan's dtype, then a fixed shuffle / shared-memory tree in double (same result on every run, no atomics).
+#include "cplx.cuh"
+#include "device_plan.hpp"
+
+namespace qtam {
+
+#define QTAM_LAUNCH_CHECK()                                         \
+  do {                                                              \
+    if (cudaPeekAtLastError() != cudaSuccess) return QTAM_ERR_CUDA; \
+  } while (0)
+
+template <typename T> struct Vec4;
+template <> struct Vec4<float> { typedef float4 type; };
+template <> struct Vec4<double> { typedef double4 type; };
+
+template <typename T, int METRIC>
+__global__ void __launch_bounds__(512)
+k_plane_metric(const C2<T> *__restrict__ coef, long long ctot, const long long *__restrict__ plane_off, int nP,
+               T *__restrict__ out) {
+  typedef typename Vec4<T>::type V4;
+  const int q = blockIdx.x, seg = blockIdx.y;
+  const long long lo = plane_off[q], n = plane_off[q + 1] - lo;     // both multiples of 4 (every M >= 4)
+  const V4 *src = reinterpret_cast<const V4 *>(coef + (size_t)seg * ctot + lo);
+  T acc[4] = {0, 0, 0, 0};
+  const long long n2 = n / 2;                                       // two coefficients per load
+  for (long long i = threadIdx.x; i < n2; i += 4 * 512) {
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+      const long long k = i + (long long)u * 512;
+      if (k < n2) {
+        const V4 v = src[k];
+        const T e0 = v.x * v.x + v.y * v.y, e1 = v.z * v.z + v.w * v.w;
+        if (METRIC == 0) acc[u] += e0 + e1;
+        else acc[u] = fmax(acc[u], fmax(e0, e1));
+      }
+    }
+  }
+  double r = METRIC == 0 ? ((double)acc[0] + (double)acc[1]) + ((double)acc[2] + (double)acc[3])
+                         : fmax(fmax((double)acc[0], (double)acc[1]), fmax((double)acc[2], (double)acc[3]));
+  for (int o = 16; o > 0; o >>= 1) {
+    const double other = __shfl_xor_sync(0xffffffffu, r, o);
+    r = METRIC == 0 ? r + other : fmax(r, other);
+  }
+  __shared__ double part[16];
+  if ((threadIdx.x & 31) == 0) part[threadIdx.x >> 5] = r;
+  __syncthreads();
+  if (threadIdx.x < 32) {
+    r = threadIdx.x < 16 ? part[threadIdx.x] : 0.0;
+    for (int o = 8; o > 0; o >>= 1) {
+      const double other = __shfl_xor_sync(0xffffffffu, r, o);
+      r = METRIC == 0 ? r + other : fmax(r, other);
+    }
+    if (threadIdx.x == 0) out[(size_t)seg * nP + q] = (T)r;
+  }
+}
+
+// optimal selection: the plane with the largest metric, lowest index on ties, independently per segment
+template <typename T>
+__global__ void k_best_plane(const T *__restrict__ metric, int nP, int batch, int32_t *__restrict__ best) {
+  const int seg = blockIdx.x * blockDim.x + threadIdx.x;
+  if (seg >= batch) return;
+  const T *m = metric + (size_t)seg * nP;
+  int b = 0;
+  for (int q = 1; q < nP; ++q) if (m[q] > m[b]) b = q;
+  best[seg] = b;
+}
+
+template <typename T>
+static qtam_status metric_t(qtam_plan *p, const void *d_coef, int batch, int metric, void *d_metric,
+                            int32_t *d_best, cudaStream_t st) {
+  dim3 g(p->hp.nP, batch);
+  {
+    LaunchScope ls(p, st, K_PLANE_METRIC, (double)batch * (sizeof(C2<T>) * (double)p->hp.ctot));
+    if (metric == 0)
+      k_plane_metric<T, 0><<<g, 512, 0, st>>>(static_cast<const C2<T> *>(d_coef), p->hp.ctot, p->d_plane_off,
+                                              p->hp.nP, static_cast<T *>(d_metric));
+    else
+      k_plane_metric<T, 1><<<g, 512, 0, st>>>(static_cast<const C2<T> *>(d_coef), p->hp.ctot, p->d_plane_off,
+                                              p->hp.nP, static_cast<T *>(d_metric));
+  }
+  QTAM_LAUNCH_CHECK();
+  if (d_best) {
+    LaunchScope ls(p, st, K_BEST_PLANE, (double)batch * (sizeof(T) * (double)p->hp.nP + 4.0));
+    k_best_plane<T><<<(batch + 127) / 128, 128, 0, st>>>(static_cast<const T *>(d_metric), p->hp.nP, batch, d_best);
+  }
+  QTAM_LAUNCH_CHECK();
+  return QTAM_OK;
+}
+
+qtam_status plane_metric(qtam_plan *p, const void *d_coef, int batch, int metric, void *d_metric, int32_t *d_best,
+                         cudaStream_t st) {
+  return p->esz == 4 ? metric_t<float>(p, d_coef, batch, metric, d_metric, d_best, st)
+                     : metric_t<double>(p, d_coef, batch, metric, d_metric, d_best, st);
+}
+
+}  // namespace qtam

@@ -201,6 +201,36 @@ def test_manual_frequency_grid_on_gpu():
     assert worst_segment(g.inverse(g.forward(dev(x))).cpu().numpy(), pi_c(x64, C)) <= 1e-5
 
 
+@pytest.mark.parametrize("name,dtype,nseg", [("cfg3", "f32", 6), ("cfg5", "f64", 5), ("cfg2", "f32", 2)])
+@pytest.mark.parametrize("metric", ["energy", "peak"])
+def test_plane_metric_and_optimal_plane(name, dtype, nseg, metric):
+    """Multi-Q scan selection.  Values to the coefficient tolerance; the selected plane is
+    compared through what is unique: where the oracle's best and runner-up are separated by more than the
+    tolerance the index must be equal, otherwise the kernel's choice must be one of the near-maximal planes."""
+    g, r = make_plans(inputs.plan_args(name), dtype, nseg)
+    x = inputs.make_batch(name, batch=nseg, dtype=dtype) if dtype == "f64" else inputs.make_batch(name, batch=nseg)
+    x = x.astype(np_rdt(dtype))
+    Y = g.forward(dev(x))
+    vals, best = g.plane_metric(Y, metric)
+    vr, br = r.plane_metric(Y.cpu().numpy().astype(np.complex128), metric)
+    tol = 1e-12 if dtype == "f64" else 1e-5
+    assert np.max(np.abs(vals.cpu().numpy() - vr) / vr) <= tol
+    bg = best.cpu().numpy()
+    for b in range(nseg):
+        top = np.sort(vr[b])[::-1]
+        if top[0] - top[1] > 4 * tol * top[0]:
+            assert bg[b] == br[b]
+        else:
+            assert vr[b][bg[b]] >= top[0] * (1 - 4 * tol)
+    # a segment with a strong narrow-band line must prefer a different plane than a broadband one does
+    if name == "cfg3":
+        t = np.arange(g.N) / 4096.0
+        xs = np.stack([np.cos(2 * np.pi * 300.0 * t), inputs.white_noise(g.N, 5)[0]]).astype(np.float32)
+        _, b2 = g.plane_metric(g.forward(dev(xs)), "peak")
+        _, r2 = r.plane_metric(r.forward(xs.astype(np.float64), engine=1), "peak")
+        assert np.array_equal(b2.cpu().numpy(), r2) and r2[0] == g.n_planes - 1
+
+
 def test_cfg5_fp64_variant():
     name = "cfg5"
     g, r = make_plans(inputs.plan_args(name), "f64", 4)
