@@ -135,7 +135,10 @@ class Plan:
             self._h = None
 
     def __del__(self):
-        self.close()
+        try:
+            self.close()
+        except Exception:      # interpreter shutdown: the module globals may already be gone
+            pass
 
     # ---- host tables -------------------------------------------------------------------------------
     def window(self, k):
