@@ -43,6 +43,7 @@ def parse_args():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--overlap", type=float, default=1.0, help="clamp_overlap (R7); 1.0 = paper literal")
+    ap.add_argument("--e2e-chunks", type=int, default=2, help="chunks of the batch pipelined over H2D | kernels | D2H")
     ap.add_argument("--no-largest-batch", action="store_true",
                     help="skip the extra pass at a batch of 8 segments per SM (SURVEY.md 8(d) 'largest batch')")
     return ap.parse_args()
@@ -306,30 +307,77 @@ def run_ours(args):
     # context: the same steps without the per-launch events
     ms_plain, _, _ = timed(args.steps, False)
 
-    # ---- end to end through the public API with host buffers (pinned), copies inside the timing
-    def e2e_step():
-        d_x.copy_(x_pin, non_blocking=True)
-        step()
-        result = d_out if "inverse" in calls else d_coef
-        if "inverse" in calls:
-            out_pin.copy_(result, non_blocking=True)
-        else:
-            coef_pin.copy_(result, non_blocking=True)
-
+    # ---- end to end through the public API with host buffers (pinned), copies inside the timing.
+    # The batch goes through in `--e2e-chunks` chunks on three streams (H2D | forward[+threshold]+inverse |
+    # D2H), so that the PCIe copies of one chunk overlap the kernels of another; every step still copies
+    # all of its inputs in and all of its results out.
     coef_pin = None
     if "inverse" not in calls:
         coef_pin = torch.empty((batch, plan.ctot), dtype=cdt).pin_memory()
+    nch = max(1, min(args.e2e_chunks, batch))
+    bounds = [(c * batch // nch, (c + 1) * batch // nch) for c in range(nch)]
+    s_in, s_cmp, s_out = torch.cuda.Stream(dev), torch.cuda.Stream(dev), torch.cuda.Stream(dev)
+    ev_in = [torch.cuda.Event() for _ in bounds]
+    ev_cmp = [torch.cuda.Event() for _ in bounds]
+    ev_out = [torch.cuda.Event() for _ in bounds]
+    primed = [False]
+
+    def e2e_step():
+        for c, (lo, hi) in enumerate(bounds):
+            with torch.cuda.stream(s_in):
+                if primed[0]:
+                    s_in.wait_event(ev_cmp[c])          # the previous step's kernels have read d_x[lo:hi]
+                d_x[lo:hi].copy_(x_pin[lo:hi], non_blocking=True)
+                ev_in[c].record(s_in)
+            with torch.cuda.stream(s_cmp):
+                s_cmp.wait_event(ev_in[c])
+                if primed[0]:
+                    s_cmp.wait_event(ev_out[c])         # the previous step's D2H has read the result buffer
+                plan.forward(d_x[lo:hi], out=d_coef[lo:hi])
+                launches[0] += plan.last_launch_count()
+                if "threshold" in calls:
+                    plan.threshold_rowmedian(d_coef[lo:hi], 3.0)
+                if "inverse" in calls:
+                    plan.inverse(d_coef[lo:hi], out=d_out[lo:hi])
+                ev_cmp[c].record(s_cmp)
+            with torch.cuda.stream(s_out):
+                s_out.wait_event(ev_cmp[c])
+                if "inverse" in calls:
+                    out_pin[lo:hi].copy_(d_out[lo:hi], non_blocking=True)
+                else:
+                    coef_pin[lo:hi].copy_(d_coef[lo:hi], non_blocking=True)
+                ev_out[c].record(s_out)
+        primed[0] = True
+
+    def fork():
+        cur = torch.cuda.current_stream()
+        for s_ in (s_in, s_cmp, s_out):
+            s_.wait_stream(cur)
+
+    def join():
+        cur = torch.cuda.current_stream()
+        for s_ in (s_in, s_cmp, s_out):
+            cur.wait_stream(s_)
+
+    fork()
     for _ in range(3):
         e2e_step()
+    join()
     barrier()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     n_e2e = max(3, min(args.steps, 50))
     e0.record()
+    fork()
     for _ in range(n_e2e):
         e2e_step()
+    join()
     e1.record()
     barrier()
     ms_e2e = e0.elapsed_time(e1) / n_e2e
+    # what came back over PCIe is what the device-resident path computes (kernels are deterministic)
+    step()
+    torch.cuda.synchronize()
+    e2e_ok = bool(torch.equal(out_pin, d_out.cpu())) if "inverse" in calls else bool(torch.equal(coef_pin, d_coef.cpu()))
     h2d = x_pin.numel() * x_pin.element_size()
     d2h = (out_pin.numel() * out_pin.element_size()) if "inverse" in calls else (coef_pin.numel() * coef_pin.element_size())
 
@@ -431,7 +479,8 @@ def run_ours(args):
         "config": workload_config(args, cfg, batch, plan),
         "clocks": clocks,
         "e2e": {"value": units / (ms_e2e * 1e-3), "unit": UNIT, "h2d_bytes_per_step": h2d,
-                "d2h_bytes_per_step": d2h, "ms_per_step": ms_e2e},
+                "d2h_bytes_per_step": d2h, "ms_per_step": ms_e2e, "chunks": nch,
+                "equals_device_resident_result": e2e_ok},
         "gpu_launches": n_launch,
         "roofline": roof,
         "path": {"compulsory_bytes_per_step": comp, "achieved_gbs": path_gbs, "frac_of_peak": path_gbs / peak,
