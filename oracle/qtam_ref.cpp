@@ -240,7 +240,7 @@ int qtam_ref_plan_create(qtam_ref_plan **out, double fs, int64_t N, const double
   if (!out || !Q || nQ < 1 || !(fs > 0) || !is_pow2(N) || N < 8) return 1;
   qtam_ref_options o;
   o.window = 0; o.clamp_mode = 1; o.clamp_overlap = 1.0; o.max_window_bins = 0;
-  o.cover_floor = 1e-2; o.rows_are_bins_per_octave = 0; o.window_param = 0.0; o.freqs = nullptr; o.n_freqs = 0;
+  o.cover_floor = 1e-2; o.rows_are_bins_per_octave = 0; o.window_param = 0.0; o.freqs = nullptr; o.n_freqs = 0; o.tile_length = 0;
   if (opt) o = *opt;
   const bool manual = o.freqs != nullptr && o.n_freqs >= 2;
   if (manual) { fmin = o.freqs[0]; fmax = o.freqs[o.n_freqs - 1]; }
@@ -286,6 +286,21 @@ int qtam_ref_plan_create(qtam_ref_plan **out, double fs, int64_t N, const double
     Lmax = 2 * ((o.max_window_bins - 1) / 2) + 1;  // odd, <= request
   } else if (o.clamp_mode != 0) return 1;
 
+  // uniform tile length (every row zero-padded to the largest window): the longest support
+  int64_t Luni = 0;
+  for (int pl = 0; pl < nQ; ++pl)
+    for (int r = 0; r < R; ++r) {
+      int64_t L = 2 * (int64_t)std::floor(f[(size_t)r] * T * SQRT11 / Q[pl]) + 1;
+      if (Lmax > 0) L = std::min(L, Lmax);
+      Luni = std::max(Luni, L);
+    }
+  int64_t Muni = 0;
+  if (o.tile_length == -1) Muni = next_pow2(Luni);
+  else if (o.tile_length > 0) {
+    if (!is_pow2(o.tile_length) || o.tile_length < Luni) return 1;
+    Muni = o.tile_length;
+  } else if (o.tile_length != 0) return 1;
+
   qtam_ref_plan *p = new (std::nothrow) qtam_ref_plan;
   if (!p) return 3;
   p->fs = fs; p->N = N; p->nb = N / 2 + 1; p->nP = nQ; p->nR = R;
@@ -302,7 +317,7 @@ int qtam_ref_plan_create(qtam_ref_plan **out, double fs, int64_t N, const double
       if (Lmax > 0) L = std::min(L, Lmax);                                  // A8
       row.L = L; row.dk = (L - 1) / 2;
       if (row.dk < 1) { delete p; return 1; }                               // R13
-      row.M = next_pow2(L);                                                 // R5
+      row.M = Muni > 0 ? Muni : next_pow2(L);                               // R5 / uniform layout
       row.f_center = (double)row.kc / T;
       row.offset = offset; offset += row.M; sumL += L;
       // bisquare window (Eq. 6) and unit-energy normalisation (Eq. 5 / R3);
@@ -626,6 +641,28 @@ int qtam_ref_threshold_rowmedian_f32(const qtam_ref_plan *p, float *coef, int ba
       volatile float t = kappa * m;
       for (int64_t n = 0; n < r.M; ++n)
         if (mag[(size_t)n] < t) { Y[2 * n] = 0.0f; Y[2 * n + 1] = 0.0f; }
+    }
+  return 0;
+}
+
+// Re-modulation with the carrier (Eq. 10a :113-117; :129 "re-modulated with the carrier to recover the
+// original T_k"): the decimated envelope times e^{+2 pi i kc n / M_k}, and the amplitude of C47 undone, gives
+// the dense tile on the coarse time grid t_n = n T / M_k:  T_k[n N/M_k] = sqrt(M_k/N) e^{2 pi i kc n/M_k} Y_k[n].
+int qtam_ref_remodulate(const qtam_ref_plan *p, const double *coef, int batch, double *out) {
+  if (!p || !coef || !out || batch < 0) return 1;
+  const ld TAU = 6.283185307179586476925286766559005768L;
+  for (int b = 0; b < batch; ++b)
+    for (const Row &r : p->rows) {
+      const cd *Y = reinterpret_cast<const cd *>(coef) + (size_t)b * p->ctot + r.offset;
+      cd *O = reinterpret_cast<cd *>(out) + (size_t)b * p->ctot + r.offset;
+      const ld amp = sqrtl((ld)r.M / (ld)p->N);
+      for (int64_t n = 0; n < r.M; ++n) {
+        const int64_t m = (int64_t)(((__int128)r.kc * n) % r.M);       // R12: index reduced in integers
+        const ld a = TAU * (ld)m / (ld)r.M;
+        const ld c = cosl(a), s = sinl(a);
+        O[n] = cd((double)(amp * ((ld)Y[n].real() * c - (ld)Y[n].imag() * s)),
+                  (double)(amp * ((ld)Y[n].real() * s + (ld)Y[n].imag() * c)));
+      }
     }
   return 0;
 }

@@ -44,6 +44,9 @@ typedef struct {
   double  window_param;             /* Kaiser beta > 0, Tukey alpha_T in (0,1], Planck alpha_P in (0,1] */
   const double *freqs;              /* manual grid (:303): n_freqs ascending centre frequencies; when    */
   int     n_freqs;                  /* n_freqs >= 2 it replaces fmin / fmax / spacing                    */
+  int64_t tile_length;              /* output length per row: 0 = nextpow2(L_k) per row (R5, default);
+                                       -1 = uniform, nextpow2 of the largest window (the paper's padded
+                                       layout :127-129); n > 0 = uniform user-set n, a power of two >= max L */
 } qtam_ref_options;
 
 typedef struct {
@@ -88,6 +91,10 @@ int  qtam_ref_brute_tile(const qtam_ref_plan *p, const double *x, int row, doubl
  * stated in DESIGN.md ("threshold arithmetic") so that a float kernel can match it bit for bit. */
 int  qtam_ref_threshold_rowmedian(const qtam_ref_plan *p, double *coef, int batch, double kappa);
 int  qtam_ref_threshold_rowmedian_f32(const qtam_ref_plan *p, float *coef, int batch, float kappa);
+
+/* Re-modulation (Eq. 10a :113-117, :129): out[b][offset_k + n] = sqrt(M_k/N) e^{+2 pi i kc n/M_k} Y_k[n]
+ * = the dense tile T_k at tau = n N/M_k (identity P2).  Same layout as the coefficients. */
+int  qtam_ref_remodulate(const qtam_ref_plan *p, const double *coef, int batch, double *out);
 
 /* Multi-Q scan: out_metric[batch][n_planes] = total energy (metric 0) or peak pixel
  * (metric 1) of every plane's |Y|^2, out_best[batch] = the plane with the largest value per segment

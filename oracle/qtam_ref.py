@@ -21,7 +21,7 @@ class Options(C.Structure):
     _fields_ = [("window", C.c_int), ("clamp_mode", C.c_int), ("clamp_overlap", C.c_double),
                 ("max_window_bins", C.c_int64), ("cover_floor", C.c_double),
                 ("rows_are_bins_per_octave", C.c_int), ("window_param", C.c_double),
-                ("freqs", C.POINTER(C.c_double)), ("n_freqs", C.c_int)]
+                ("freqs", C.POINTER(C.c_double)), ("n_freqs", C.c_int), ("tile_length", C.c_int64)]
 
 
 WINDOWS = {"bisquare": 0, "hann": 1, "kaiser": 2, "tukey": 3, "planck": 4}
@@ -59,6 +59,7 @@ def lib():
         _lib.qtam_ref_brute_tile.argtypes = [vp, dp, C.c_int, dp]
         _lib.qtam_ref_threshold_rowmedian.argtypes = [vp, dp, C.c_int, C.c_double]
         _lib.qtam_ref_threshold_rowmedian_f32.argtypes = [vp, fp, C.c_int, C.c_float]
+        _lib.qtam_ref_remodulate.argtypes = [vp, dp, C.c_int, dp]
         _lib.qtam_ref_plane_metric.argtypes = [vp, dp, C.c_int, C.c_int, dp, C.POINTER(C.c_int32)]
         _lib.qtam_ref_project_cover.argtypes = [vp, dp, C.c_int, C.c_int, dp, C.c_int]
         _lib.qtam_ref_spectrum.argtypes = [vp, dp, C.c_int, dp, C.c_int]
@@ -100,7 +101,7 @@ class RefPlan:
 
     def __init__(self, fs, N, Q, fmin, fmax, spacing, clamp_mode=1, clamp_overlap=1.0,
                  max_window_bins=0, cover_floor=1e-2, rows_are_bins_per_octave=0,
-                 window="bisquare", window_param=0.0, freqs=None):
+                 window="bisquare", window_param=0.0, freqs=None, tile_length=0):
         L = lib()
         self._h = C.c_void_p()
         q = np.ascontiguousarray(Q, dtype=np.float64)
@@ -108,7 +109,7 @@ class RefPlan:
         opt = Options(WINDOWS[window], clamp_mode, clamp_overlap, max_window_bins, cover_floor,
                       rows_are_bins_per_octave, float(window_param),
                       None if fr is None else fr.ctypes.data_as(C.POINTER(C.c_double)),
-                      0 if fr is None else fr.size)
+                      0 if fr is None else fr.size, int(tile_length))
         rc = L.qtam_ref_plan_create(C.byref(self._h), float(fs), int(N), _dp(q), q.size,
                                     float(fmin), float(fmax), float(spacing), C.byref(opt))
         if rc != 0:
@@ -186,6 +187,13 @@ class RefPlan:
             c = c[None, :]
         assert lib().qtam_ref_threshold_rowmedian(self._h, _dp(c.view(np.float64)), c.shape[0], kappa) == 0
         return c
+
+    def remodulate(self, coef):
+        """decimated envelopes -> samples of the dense tiles T_k[n N/M_k] (Eq. 10a, identity P2)"""
+        c = np.ascontiguousarray(np.atleast_2d(coef), dtype=np.complex128)
+        out = np.empty_like(c)
+        assert lib().qtam_ref_remodulate(self._h, _dp(c.view(np.float64)), c.shape[0], _dp(out.view(np.float64))) == 0
+        return out
 
     def plane_metric(self, coef, metric="energy"):
         """(values[batch][n_planes], best[batch]) of the multi-Q scan's plane selection"""

@@ -584,3 +584,47 @@ def test_plane_peak_of_a_pure_sinusoid_closed_form():
     # scaling one segment changes its metrics quadratically and not its choice; selection is per segment
     v2, b2 = p.plane_metric(p.forward(np.stack([x, 3.0 * x]), engine=0), "peak")
     assert np.allclose(v2[1], 9.0 * v2[0], rtol=1e-12) and b2[0] == b2[1] == best[0]
+
+
+# ---- paper-native layouts: uniform tile length, re-modulation ----------------
+
+@pytest.mark.parametrize("tile_length", [-1, 512])
+def test_uniform_tile_length_is_an_upsampled_view_of_the_ragged_layout(tile_length):
+    """:127-129: "symmetrically zero padded ... so that all the tiles have the same length".  Zero-padding the
+    baseband spectrum only resamples the same band-limited envelope: with M' >= M both powers of two,
+    Y'[n M'/M] = sqrt(M/M') Y[n] (the factor is C47's (N M)^{-1/2}), the row energy is unchanged (C48 :592),
+    and the round trip is still exact on the cover set."""
+    args = (1024.0, 1024, [4.0, 8.0, 16.0], 16.0, 400.0, 12)
+    p = RefPlan(*args)
+    u = RefPlan(*args, tile_length=tile_length)
+    Mu = {r.M for r in u.rows}
+    assert len(Mu) == 1 and Mu.pop() == (128 if tile_length == -1 else 512)
+    assert u.ctot == u.n_rows * u.rows[0].M and [r.offset for r in u.rows] == [i * u.rows[0].M for i in range(u.n_rows)]
+    x = inputs.white_noise(p.N, 91)
+    Y, Yu = p.forward(x, engine=0)[0], u.forward(x, engine=0)[0]
+    for k, (r, ru) in enumerate(zip(p.rows, u.rows)):
+        assert (r.kc, r.dk, r.L) == (ru.kc, ru.dk, ru.L)
+        a, b = Y[p.row_slice(k)], Yu[u.row_slice(k)]
+        step = ru.M // r.M
+        assert rel_l2(b[::step], np.sqrt(r.M / ru.M) * a) <= 1e-12
+        assert abs(np.sum(np.abs(a) ** 2) - np.sum(np.abs(b) ** 2)) <= 1e-12 * np.sum(np.abs(a) ** 2)
+    _, C = u.frame(-1)
+    proj = np.fft.irfft(np.where(C[None, :], np.fft.rfft(x, axis=-1), 0), n=p.N, axis=-1)
+    assert rel_l2(u.inverse(Yu[None, :], engine=0), proj) <= 1e-12
+    with pytest.raises(ValueError):
+        RefPlan(*args, tile_length=64)          # shorter than the largest window
+    with pytest.raises(ValueError):
+        RefPlan(*args, tile_length=384)         # not a power of two
+
+
+def test_remodulation_gives_samples_of_the_dense_tile():
+    """Eq. 10a (:113-117) / P2: sqrt(M/N) e^{2 pi i kc n/M} Y_k[n] = T_k[n N/M], against O-dense (pinned by the
+    brute-force convolution P1), in the ragged and in the uniform layout."""
+    args = (256.0, 256, [4.0, 8.0], 8.0, 100.0, 7)
+    for tl in (0, -1):
+        p = RefPlan(*args, tile_length=tl)
+        x = inputs.white_noise(p.N, 92)
+        R = p.remodulate(p.forward(x, engine=0))[0]
+        D = p.dense(x, engine=0)[0]
+        for k, r in enumerate(p.rows):
+            assert rel_l2(R[p.row_slice(k)], D[k][:: p.N // r.M]) <= 1e-12
