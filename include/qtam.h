@@ -69,6 +69,10 @@ typedef struct {
   const double *freqs;              /* manual grid (:303): n_freqs ascending centre frequencies in Hz
                                        (host pointer, read during plan creation only); when           */
   int     n_freqs;                  /* n_freqs >= 2 they replace fmin / fmax / spacing              */
+  int64_t tile_length;              /* output samples per row: 0 = nextpow2(L_k) per row (R5) [default];
+                                       -1 = uniform, nextpow2 of the largest window: the paper's
+                                       zero-padded layout (:127-129), coefficients = [rows][M] per
+                                       segment; n > 0 = uniform, user-set power of two >= max L     */
 } qtam_options;
 
 /* Host-side row table entry; rows are ordered plane-major (Q list order), ascending frequency. */
@@ -131,6 +135,11 @@ qtam_status qtam_dense(qtam_plan *p, const void *d_x, int batch, int row_begin, 
  * The decision is taken in the plan's dtype with the operation order of DESIGN.md.               */
 qtam_status qtam_threshold_rowmedian(qtam_plan *p, void *d_coef, int batch, double kappa,
                                      void *stream);
+
+/* Re-modulation with the carrier (Eq. 10a): d_out[b][offset_k + n] =
+ * sqrt(M_k/N) e^{+2 pi i kc n/M_k} Y_k[n], which is the dense tile T_k at tau = n N/M_k (P2).
+ * d_coef, d_out: [batch][coeffs_per_segment], same layout; d_out may equal d_coef (in place). */
+qtam_status qtam_remodulate(qtam_plan *p, const void *d_coef, int batch, void *d_out, void *stream);
 
 /* Multi-Q scan selection ("for each resolution plane ... a signal quality metric (e.g., total
  * energy or peak pixel intensity)"; "optimal selection mode ... independently for each signal in the batch").

@@ -18,7 +18,7 @@ STATUS = {0: "ok", 1: "invalid argument", 2: "unsupported", 3: "alloc", 4: "cuda
 
 SYMBOLS = ["qtam_plan_create", "qtam_plan_create_host", "qtam_plan_destroy", "qtam_plan_info",
            "qtam_plan_rows", "qtam_plan_window", "qtam_plan_frame", "qtam_forward", "qtam_inverse",
-           "qtam_dense", "qtam_threshold_rowmedian", "qtam_plane_metric", "qtam_last_launch_count", "qtam_status_string",
+           "qtam_dense", "qtam_threshold_rowmedian", "qtam_plane_metric", "qtam_remodulate", "qtam_last_launch_count", "qtam_status_string",
            "qtam_profile_enable", "qtam_profile_read"]
 
 
@@ -33,7 +33,7 @@ class Options(C.Structure):
                 ("clamp_overlap", C.c_double), ("max_window_bins", C.c_int64),
                 ("cover_floor", C.c_double), ("rows_are_bins_per_octave", C.c_int),
                 ("max_batch", C.c_int), ("window_param", C.c_double),
-                ("freqs", C.POINTER(C.c_double)), ("n_freqs", C.c_int)]
+                ("freqs", C.POINTER(C.c_double)), ("n_freqs", C.c_int), ("tile_length", C.c_int64)]
 
 
 WINDOWS = {"bisquare": 0, "hann": 1, "kaiser": 2, "tukey": 3, "planck": 4}
@@ -80,6 +80,7 @@ def lib():
         L.qtam_dense.argtypes = [vp, vp, C.c_int, C.c_int, C.c_int, vp, vp]
         L.qtam_threshold_rowmedian.argtypes = [vp, vp, C.c_int, C.c_double, vp]
         L.qtam_plane_metric.argtypes = [vp, vp, C.c_int, C.c_int, vp, vp, vp]
+        L.qtam_remodulate.argtypes = [vp, vp, C.c_int, vp, vp]
         L.qtam_last_launch_count.argtypes = [vp]
         L.qtam_last_launch_count.restype = C.c_int
         L.qtam_status_string.argtypes = [C.c_int]
@@ -101,7 +102,7 @@ class Plan:
 
     def __init__(self, fs, N, Q, fmin, fmax, spacing, dtype="f32", max_batch=1, clamp_mode=1,
                  clamp_overlap=1.0, max_window_bins=0, cover_floor=1e-2, rows_are_bins_per_octave=0,
-                 host_only=False, window="bisquare", window_param=0.0, freqs=None):
+                 host_only=False, window="bisquare", window_param=0.0, freqs=None, tile_length=0):
         L = lib()
         self._h = C.c_void_p()
         self.dtype = dtype
@@ -110,7 +111,7 @@ class Plan:
         opt = Options(C.sizeof(Options), WINDOWS[window], clamp_mode, clamp_overlap, max_window_bins,
                       cover_floor, rows_are_bins_per_octave, max_batch, float(window_param),
                       None if fr is None else fr.ctypes.data_as(C.POINTER(C.c_double)),
-                      0 if fr is None else fr.size)
+                      0 if fr is None else fr.size, int(tile_length))
         fn = L.qtam_plan_create_host if host_only else L.qtam_plan_create
         code = fn(C.byref(self._h), float(fs), int(N), q.ctypes.data_as(C.POINTER(C.c_double)), q.size,
                   float(fmin), float(fmax), float(spacing), QTAM_F64 if dtype == "f64" else QTAM_F32,
@@ -210,6 +211,16 @@ class Plan:
         _check(lib().qtam_threshold_rowmedian(self._h, coef.data_ptr(), batch, float(kappa), self._stream()),
                "qtam_threshold_rowmedian")
         return coef
+
+    def remodulate(self, coef, out=None):
+        """decimated envelopes -> samples of the dense tiles (Eq. 10a); out may be coef (in place)"""
+        t = self._torch()
+        assert coef.is_cuda and coef.dtype == self._cdt() and coef.is_contiguous()
+        batch = coef.numel() // self.ctot
+        if out is None:
+            out = t.empty_like(coef)
+        _check(lib().qtam_remodulate(self._h, coef.data_ptr(), batch, out.data_ptr(), self._stream()), "qtam_remodulate")
+        return out
 
     def plane_metric(self, coef, metric="energy"):
         """(values[batch][n_planes], best[batch] int32) of the multi-Q scan's plane selection"""

@@ -99,6 +99,21 @@ qtam_status build_host_plan(HostPlan &hp, double fs, int64_t N, const double *Q,
     cap = 2 * ((o.max_window_bins - 1) / 2) + 1;
   }
 
+  // uniform tile length (:127-129, every row zero-padded to the largest window) or per-row lengths (R5)
+  int64_t m_uniform = 0;
+  if (o.tile_length != 0) {
+    int64_t lmaxrow = 0;
+    for (int pl = 0; pl < nQ; ++pl)
+      for (int r = 0; r < hp.nR; ++r) {
+        int64_t len = 2 * int64_t(std::floor(fc[size_t(r)] * dur * tile_c / Q[pl])) + 1;
+        if (cap > 0 && len > cap) len = cap;
+        lmaxrow = std::max(lmaxrow, len);
+      }
+    if (o.tile_length == -1) { m_uniform = 1; while (m_uniform < lmaxrow) m_uniform <<= 1; }
+    else if (o.tile_length > 0 && pow2(o.tile_length) && o.tile_length >= lmaxrow) m_uniform = o.tile_length;
+    else return QTAM_ERR_INVALID_ARG;
+  }
+
   hp.rows.clear();
   hp.win.clear();
   int64_t coff = 0, woff = 0, mmax = 0;
@@ -114,6 +129,7 @@ qtam_status build_host_plan(HostPlan &hp, double fs, int64_t N, const double *Q,
       if (h.dk < 1) return QTAM_ERR_INVALID_ARG;                                  // R13
       int64_t m = 1;
       while (m < len) m <<= 1;                                                   // R5
+      if (m_uniform > 0) m = m_uniform;
       h.M = m; mmax = std::max(mmax, m);
       h.f_center = double(h.kc) / dur;
       h.offset = coff; coff += m;

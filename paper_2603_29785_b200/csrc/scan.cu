@@ -69,6 +69,41 @@ __global__ void k_best_plane(const T *__restrict__ metric, int nP, int batch, in
   best[seg] = b;
 }
 
+// Re-modulation (Eq. 10a :113-117): out = sqrt(M/N) e^{+2 pi i kc n/M} Y_k[n].  One CTA per (row, segment);
+// the phase index kc n mod M is reduced in integers (R12) and goes through sincospi.
+template <typename T>
+__global__ void __launch_bounds__(128)
+k_remodulate(const RowDev *__restrict__ rows, const C2<T> *__restrict__ coef, long long ctot, int n_samples,
+             C2<T> *__restrict__ out) {
+  const RowDev r = rows[blockIdx.x];
+  const C2<T> *Y = coef + (size_t)blockIdx.y * ctot + r.offset;
+  C2<T> *O = out + (size_t)blockIdx.y * ctot + r.offset;
+  const T amp = sqrt((T)r.M / (T)n_samples);
+  const T inv = (T)2 / (T)r.M;
+  for (int n = threadIdx.x; n < r.M; n += 128) {
+    const int m = (int)(((long long)r.kc * n) & (r.M - 1));
+    T s, c;
+    sincospi((T)m * inv, &s, &c);
+    const C2<T> y = Y[n];
+    O[n] = cmk<T>(amp * (y.x * c - y.y * s), amp * (y.x * s + y.y * c));
+  }
+}
+
+qtam_status remodulate(qtam_plan *p, const void *d_coef, int batch, void *d_out, cudaStream_t st) {
+  dim3 g((unsigned)p->hp.rows.size(), batch);
+  {
+    LaunchScope ls(p, st, K_REMODULATE, 4.0 * p->esz * (double)batch * (double)p->hp.ctot);
+    if (p->esz == 4)
+      k_remodulate<float><<<g, 128, 0, st>>>(p->d_rows, static_cast<const float2 *>(d_coef), p->hp.ctot, (int)p->hp.N,
+                                            static_cast<float2 *>(d_out));
+    else
+      k_remodulate<double><<<g, 128, 0, st>>>(p->d_rows, static_cast<const double2 *>(d_coef), p->hp.ctot,
+                                             (int)p->hp.N, static_cast<double2 *>(d_out));
+  }
+  QTAM_LAUNCH_CHECK();
+  return QTAM_OK;
+}
+
 template <typename T>
 static qtam_status metric_t(qtam_plan *p, const void *d_coef, int batch, int metric, void *d_metric,
                             int32_t *d_best, cudaStream_t st) {

@@ -231,6 +231,38 @@ def test_plane_metric_and_optimal_plane(name, dtype, nseg, metric):
         assert np.array_equal(b2.cpu().numpy(), r2) and r2[0] == g.n_planes - 1
 
 
+@pytest.mark.parametrize("dtype", ["f32", "f64"])
+@pytest.mark.parametrize("tile_length", [-1, 2048])
+def test_uniform_tile_layout_and_remodulation(dtype, tile_length):
+    """the paper's zero-padded layout (every row the same length, :127-129) and the
+    carrier re-modulation back to samples of the dense tile (Eq. 10a)."""
+    args = (4096.0, 8192, [5.0, 10.0, 20.0], 10.0, 1900.0, 24.0)
+    g, r = make_plans(args, dtype, 2, tile_length=tile_length)
+    assert {a.M for a in g.rows} == {b.M for b in r.rows} and len({a.M for a in g.rows}) == 1
+    assert g.ctot == r.ctot == g.n_rows * g.rows[0].M
+    x = inputs.white_noise(args[1], 75, batch=2).astype(np_rdt(dtype))
+    x64 = x.astype(np.float64)
+    Y = g.forward(dev(x))
+    Yr = r.forward(x64, engine=1)
+    assert worst_segment(Y.cpu().numpy(), Yr) <= TOL[dtype]
+    _, C = r.frame(-1)
+    assert worst_segment(g.inverse(Y).cpu().numpy(), pi_c(x64, C)) <= TOL_RT[dtype]
+    Yin = Yr.astype(Y.cpu().numpy().dtype)
+    R = g.remodulate(dev(Yin)).cpu().numpy()
+    assert worst_segment(R, r.remodulate(Yin.astype(np.complex128))) <= TOL[dtype]
+    # in place, and in the ragged default layout
+    Z = dev(Yin.copy())
+    g.remodulate(Z, out=Z)
+    assert np.array_equal(Z.cpu().numpy(), R)
+
+
+def test_remodulation_ragged_layout_cfg3():
+    g, r = make_plans(inputs.plan_args("cfg3"), "f32", 3)
+    rng = np.random.default_rng(76)
+    Yin = (rng.standard_normal((3, g.ctot)) + 1j * rng.standard_normal((3, g.ctot))).astype(np.complex64)
+    assert worst_segment(g.remodulate(dev(Yin)).cpu().numpy(), r.remodulate(Yin.astype(np.complex128))) <= 2e-5
+
+
 def test_cfg5_fp64_variant():
     name = "cfg5"
     g, r = make_plans(inputs.plan_args(name), "f64", 4)

@@ -148,3 +148,16 @@ def test_window_parameters_and_manual_grid_are_validated():
     r = RefPlan(4096.0, 4096, [4.0, 12.0], 0.0, 0.0, 0.0, freqs=freqs)
     assert [(a.kc, a.dk, a.M, a.offset, a.f_request) for a in p.rows] == \
            [(b.kc, b.dk, b.M, b.offset, b.f_request) for b in r.rows]
+
+
+@pytest.mark.parametrize("tile_length", [-1, 4096])
+def test_uniform_tile_length_host_plan_matches_oracle(tile_length):
+    args = (4096.0, 4096, [4.0, 8.0, 16.0], 16.0, 1024.0, 32)
+    p = binding.Plan(*args, dtype="f64", host_only=True, tile_length=tile_length)
+    r = RefPlan(*args, tile_length=tile_length)
+    assert [(a.kc, a.dk, a.L, a.M, a.offset) for a in p.rows] == [(b.kc, b.dk, b.L, b.M, b.offset) for b in r.rows]
+    assert p.ctot == r.ctot
+    with pytest.raises(binding.QtamError):
+        binding.Plan(*args, host_only=True, tile_length=96)
+    with pytest.raises(binding.QtamError):
+        binding.Plan(*args, host_only=True, tile_length=64)
