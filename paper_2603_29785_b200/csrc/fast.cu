@@ -26,6 +26,9 @@ namespace qtam {
 
 extern __shared__ __align__(16) unsigned char qtam_fast_smem[];
 
+#ifndef QTAM_FWD_STORE
+#define QTAM_FWD_STORE(p, v) __stcs(p, v)
+#endif
 #ifndef QTAM_GROUP_INLINE
 #define QTAM_GROUP_INLINE __forceinline__
 #endif
@@ -141,7 +144,7 @@ __device__ QTAM_GROUP_INLINE void fwd_group(const FastBucket &B, const FastRow *
 #pragma unroll
       for (int i = 0; i < F; ++i)
 #pragma unroll
-        for (int n2 = 0; n2 < G; ++n2) __stcs(dst + G * i + 32 * n2, v[i * G + n2]);
+        for (int n2 = 0; n2 < G; ++n2) QTAM_FWD_STORE(dst + G * i + 32 * n2, v[i * G + n2]);
     }
   }
 }
