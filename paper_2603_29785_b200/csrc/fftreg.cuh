@@ -62,9 +62,15 @@ __device__ __forceinline__ float2 twmul(float2 o) {
   else if constexpr (k == 16) return make_float2(-o.x, -o.y);
   else if constexpr (k == 24) return DIR > 0 ? make_float2(o.y, -o.x) : make_float2(-o.y, o.x);
   else {
+    // o (c + i s) = o (c, c) + (-o.y, o.x) (s, s): two packed instructions -- the swap and the sign of the
+    // second factor fold into FMUL2's operand modifiers, (c, c) and (s, s) are scalar-broadcast operands
     constexpr float c = cos32(k);
     constexpr float s = DIR > 0 ? sin32(k) : -sin32(k);
+#ifdef QTAM_SCALAR_TWIDDLES
     return make_float2(o.x * c - o.y * s, o.x * s + o.y * c);
+#else
+    return pfma(o, make_float2(c, c), pmul(make_float2(-o.y, o.x), make_float2(s, s)));
+#endif
   }
 }
 
