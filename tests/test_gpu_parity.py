@@ -396,3 +396,51 @@ def test_gpu_linearity_and_frame_energy_at_full_batch():
     xr = g.inverse(Y).cpu().numpy()
     proj = pi_c(x.astype(np.float64), C)
     assert worst_segment(xr, proj) <= 1e-5
+
+
+def test_cfg5_full_batch_in_bench_configuration():
+    """BASELINE config 5 at its full batch (1024 x 4096) as bench.py launches it: forward, threshold and
+    inverse on sampled segments against the oracle (threshold bit for bit on the kernel's own coefficients),
+    the frame-energy identity on every segment before the threshold."""
+    name = "cfg5"
+    B = inputs.CONFIGS[name]["batch"]
+    g, r = make_plans(inputs.plan_args(name), "f32", B)
+    x = inputs.make_batch(name, batch=B)
+    Y = g.forward(dev(x))
+    P, _ = r.frame(-1)
+    X = np.fft.rfft(x.astype(np.float64), axis=-1)
+    want = (np.abs(X) ** 2 * P[None, :]).sum(axis=1) / g.N
+    got = (Y.abs().double() ** 2).sum(dim=1).cpu().numpy()
+    assert np.max(np.abs(got - want) / want) <= 1e-5
+    sample = [0, 3, 517, B - 1]
+    Yh = Y.cpu().numpy()
+    for b in sample:
+        assert rel_l2(Yh[b], r.forward(x[b].astype(np.float64), engine=1)[0]) <= 2e-5
+    g.threshold_rowmedian(Y, 3.0)
+    Yt = Y.cpu().numpy()
+    want_thr = r.threshold_f32(Yh[sample], 3.0)
+    assert np.array_equal(Yt[sample].view(np.uint32), want_thr.view(np.uint32))
+    xg = g.inverse(Y).cpu().numpy()
+    xr = r.inverse(want_thr.astype(np.complex128), engine=1)
+    for i, b in enumerate(sample):
+        assert rel_l2(xg[b], xr[i]) <= 2e-5
+
+
+@pytest.mark.parametrize("name", ["cfg2", "cfg4"])
+def test_long_row_configs_full_batch_in_bench_configuration(name):
+    """BASELINE configs 2 and 4 at their full batch: sampled segments against the oracle, the frame-energy
+    identity and (cfg4) the round trip on every segment."""
+    cfg = inputs.CONFIGS[name]
+    B = cfg["batch"]
+    g, r = make_plans(inputs.plan_args(name), "f32", B)
+    x = inputs.make_batch(name, batch=B)
+    Y = g.forward(dev(x))
+    for b in (0, B - 1):
+        assert rel_l2(Y[b].cpu().numpy(), r.forward(x[b].astype(np.float64), engine=1)[0]) <= 2e-5
+    P, C = r.frame(-1)
+    X = np.fft.rfft(x.astype(np.float64), axis=-1)
+    want = (np.abs(X) ** 2 * P[None, :]).sum(axis=1) / g.N
+    got = (Y.abs().double() ** 2).sum(dim=1).cpu().numpy()
+    assert np.max(np.abs(got - want) / want) <= 1e-5
+    if "inverse" in cfg["calls"]:
+        assert worst_segment(g.inverse(Y).cpu().numpy(), pi_c(x.astype(np.float64), C)) <= 1e-5
