@@ -667,6 +667,30 @@ int qtam_ref_remodulate(const qtam_ref_plan *p, const double *coef, int batch, d
   return 0;
 }
 
+// Instantaneous frequency (Fig. 5 :182: "the time-derivative of the unwrapped phase" of the
+// demodulated tile).  Reading R16: the derivative is the forward difference on the row's own time grid
+// t_n = n T/M_k, circular like the transform; unwrapping makes successive phase differences fall in
+// (-pi, pi], so the difference of the unwrapped phase is Arg(Y[n+1] conj Y[n]).  The carrier the
+// demodulation removed is added back:  f_inst[n] = (kc + (M_k / 2 pi) Arg(Y_k[(n+1) mod M_k] conj Y_k[n])) / T  [Hz].
+int qtam_ref_instantaneous_frequency(const qtam_ref_plan *p, const double *coef, int batch, double *out) {
+  if (!p || !coef || !out || batch < 0) return 1;
+  const ld TAU = 6.283185307179586476925286766559005768L;
+  const ld T = (ld)p->N / (ld)p->fs;
+  for (int b = 0; b < batch; ++b)
+    for (const Row &r : p->rows) {
+      const cd *Y = reinterpret_cast<const cd *>(coef) + (size_t)b * p->ctot + r.offset;
+      double *O = out + (size_t)b * p->ctot + r.offset;
+      for (int64_t n = 0; n < r.M; ++n) {
+        const cd a = Y[n], c = Y[(n + 1) % r.M];
+        const ld re = (ld)c.real() * (ld)a.real() + (ld)c.imag() * (ld)a.imag();
+        const ld im = (ld)c.imag() * (ld)a.real() - (ld)c.real() * (ld)a.imag();
+        const ld dphi = atan2l(im, re);
+        O[n] = (double)(((ld)r.kc + (ld)r.M * dphi / TAU) / T);
+      }
+    }
+  return 0;
+}
+
 // Multi-Q scan: per (segment, Q-plane) a quality metric of the plane's spectrogram
 // |Y_k[n]|^2 -- metric 0: total energy sum_{k in plane} sum_n |Y_k[n]|^2, metric 1: peak pixel
 // max_{k,n} |Y_k[n]|^2 -- and "optimal selection": the plane with the largest metric, independently for

@@ -96,6 +96,10 @@ int  qtam_ref_threshold_rowmedian_f32(const qtam_ref_plan *p, float *coef, int b
  * = the dense tile T_k at tau = n N/M_k (identity P2).  Same layout as the coefficients. */
 int  qtam_ref_remodulate(const qtam_ref_plan *p, const double *coef, int batch, double *out);
 
+/* Instantaneous frequency (Fig. 5): out[b][offset_k + n] =
+ * (kc + (M_k/2 pi) Arg(Y_k[(n+1) mod M_k] conj Y_k[n])) / T in Hz (reading R16). out: real, coefficient layout. */
+int  qtam_ref_instantaneous_frequency(const qtam_ref_plan *p, const double *coef, int batch, double *out);
+
 /* Multi-Q scan: out_metric[batch][n_planes] = total energy (metric 0) or peak pixel
  * (metric 1) of every plane's |Y|^2, out_best[batch] = the plane with the largest value per segment
  * (lowest index on ties; may be NULL). */

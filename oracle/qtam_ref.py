@@ -60,6 +60,7 @@ def lib():
         _lib.qtam_ref_threshold_rowmedian.argtypes = [vp, dp, C.c_int, C.c_double]
         _lib.qtam_ref_threshold_rowmedian_f32.argtypes = [vp, fp, C.c_int, C.c_float]
         _lib.qtam_ref_remodulate.argtypes = [vp, dp, C.c_int, dp]
+        _lib.qtam_ref_instantaneous_frequency.argtypes = [vp, dp, C.c_int, dp]
         _lib.qtam_ref_plane_metric.argtypes = [vp, dp, C.c_int, C.c_int, dp, C.POINTER(C.c_int32)]
         _lib.qtam_ref_project_cover.argtypes = [vp, dp, C.c_int, C.c_int, dp, C.c_int]
         _lib.qtam_ref_spectrum.argtypes = [vp, dp, C.c_int, dp, C.c_int]
@@ -193,6 +194,13 @@ class RefPlan:
         c = np.ascontiguousarray(np.atleast_2d(coef), dtype=np.complex128)
         out = np.empty_like(c)
         assert lib().qtam_ref_remodulate(self._h, _dp(c.view(np.float64)), c.shape[0], _dp(out.view(np.float64))) == 0
+        return out
+
+    def instantaneous_frequency(self, coef):
+        """[batch][ctot] real: forward difference of the unwrapped baseband phase plus the carrier, in Hz"""
+        c = np.ascontiguousarray(np.atleast_2d(coef), dtype=np.complex128)
+        out = np.empty(c.shape, dtype=np.float64)
+        assert lib().qtam_ref_instantaneous_frequency(self._h, _dp(c.view(np.float64)), c.shape[0], _dp(out)) == 0
         return out
 
     def plane_metric(self, coef, metric="energy"):

@@ -628,3 +628,38 @@ def test_remodulation_gives_samples_of_the_dense_tile():
         D = p.dense(x, engine=0)[0]
         for k, r in enumerate(p.rows):
             assert rel_l2(R[p.row_slice(k)], D[k][:: p.N // r.M]) <= 1e-12
+
+
+# ---- instantaneous frequency (Fig. 5) -------------------------------------------------
+
+def test_instantaneous_frequency_of_a_sinusoid_is_its_frequency():
+    """closed form: for x = cos(2 pi k0 n/N) the envelope of every row that sees bin k0 is
+    ~ e^{2 pi i (k0 - kc) n/M} (P7), so the phase advances by 2 pi (k0 - kc)/M per sample and
+    f_inst = (kc + (k0 - kc))/T = k0/T on the whole row -- the carrier comes back exactly."""
+    p = RefPlan(1024.0, 1024, [4.0, 8.0, 16.0], 16.0, 400.0, 12)
+    k0, T = 93, 1.0
+    x = np.cos(2 * np.pi * k0 * np.arange(p.N) / p.N)
+    F = p.instantaneous_frequency(p.forward(x, engine=0))[0]
+    seen = 0
+    for k, r in enumerate(p.rows):
+        if abs(k0 - r.kc) < r.dk:          # inside the window, away from its zero end points
+            assert np.max(np.abs(F[p.row_slice(k)] - k0 / T)) <= 1e-9
+            seen += 1
+    assert seen >= 6
+
+
+def test_instantaneous_frequency_vs_numpy_unwrap():
+    """the definition through a library routine: diff(unwrap(angle(Y))) M/(2 pi T) + kc/T for n = 0..M-2,
+    and the circular last sample; compared on the circle where a difference sits on the branch cut."""
+    p = RefPlan(1024.0, 1024, [4.0, 8.0], 16.0, 400.0, 12)
+    x = inputs.white_noise(p.N, 95)
+    Y = p.forward(x, engine=0)[0]
+    F = p.instantaneous_frequency(Y)[0]
+    T = p.N / 1024.0
+    for k, r in enumerate(p.rows):
+        y = Y[p.row_slice(k)]
+        ph = np.unwrap(np.angle(np.concatenate([y, y[:1]])))
+        want = np.diff(ph) * r.M / (2 * np.pi * T) + r.kc / T
+        d = (F[p.row_slice(k)] - want) * T / r.M           # in turns
+        assert np.max(np.abs(d - np.round(d))) <= 1e-9
+        assert np.mean(np.round(d) != 0) < 0.01            # only exact branch-cut cases may differ by a turn
