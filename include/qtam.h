@@ -141,6 +141,11 @@ qtam_status qtam_threshold_rowmedian(qtam_plan *p, void *d_coef, int batch, doub
  * d_coef, d_out: [batch][coeffs_per_segment], same layout; d_out may equal d_coef (in place). */
 qtam_status qtam_remodulate(qtam_plan *p, const void *d_coef, int batch, void *d_out, void *stream);
 
+/* Instantaneous frequency of the demodulated tiles (Fig. 5 "the time-derivative of the unwrapped
+ * phase"; R16): d_out[b][offset_k + n] = (kc + (M_k/2 pi) Arg(Y_k[(n+1) mod M_k] conj Y_k[n])) / T in Hz.
+ * d_out: [batch][coeffs_per_segment] REAL of the plan's dtype (device, caller-owned); must not alias d_coef. */
+qtam_status qtam_instantaneous_frequency(qtam_plan *p, const void *d_coef, int batch, void *d_out, void *stream);
+
 /* Multi-Q scan selection ("for each resolution plane ... a signal quality metric (e.g., total
  * energy or peak pixel intensity)"; "optimal selection mode ... independently for each signal in the batch").
  * metric 0: sum over the plane's rows k and samples n of |Y_k[n]|^2; metric 1: max of |Y_k[n]|^2.

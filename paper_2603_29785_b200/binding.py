@@ -18,7 +18,7 @@ STATUS = {0: "ok", 1: "invalid argument", 2: "unsupported", 3: "alloc", 4: "cuda
 
 SYMBOLS = ["qtam_plan_create", "qtam_plan_create_host", "qtam_plan_destroy", "qtam_plan_info",
            "qtam_plan_rows", "qtam_plan_window", "qtam_plan_frame", "qtam_forward", "qtam_inverse",
-           "qtam_dense", "qtam_threshold_rowmedian", "qtam_plane_metric", "qtam_remodulate", "qtam_last_launch_count", "qtam_status_string",
+           "qtam_dense", "qtam_threshold_rowmedian", "qtam_plane_metric", "qtam_remodulate", "qtam_instantaneous_frequency", "qtam_last_launch_count", "qtam_status_string",
            "qtam_profile_enable", "qtam_profile_read"]
 
 
@@ -81,6 +81,7 @@ def lib():
         L.qtam_threshold_rowmedian.argtypes = [vp, vp, C.c_int, C.c_double, vp]
         L.qtam_plane_metric.argtypes = [vp, vp, C.c_int, C.c_int, vp, vp, vp]
         L.qtam_remodulate.argtypes = [vp, vp, C.c_int, vp, vp]
+        L.qtam_instantaneous_frequency.argtypes = [vp, vp, C.c_int, vp, vp]
         L.qtam_last_launch_count.argtypes = [vp]
         L.qtam_last_launch_count.restype = C.c_int
         L.qtam_status_string.argtypes = [C.c_int]
@@ -220,6 +221,16 @@ class Plan:
         if out is None:
             out = t.empty_like(coef)
         _check(lib().qtam_remodulate(self._h, coef.data_ptr(), batch, out.data_ptr(), self._stream()), "qtam_remodulate")
+        return out
+
+    def instantaneous_frequency(self, coef):
+        """[batch][ctot] real, Hz: circular forward difference of the unwrapped baseband phase plus the carrier"""
+        t = self._torch()
+        assert coef.is_cuda and coef.dtype == self._cdt() and coef.is_contiguous()
+        batch = coef.numel() // self.ctot
+        out = t.empty((batch, self.ctot), dtype=self._rdt(), device=coef.device)
+        _check(lib().qtam_instantaneous_frequency(self._h, coef.data_ptr(), batch, out.data_ptr(), self._stream()),
+               "qtam_instantaneous_frequency")
         return out
 
     def plane_metric(self, coef, metric="energy"):

@@ -486,6 +486,14 @@ qtam_status qtam_remodulate(qtam_plan *p, const void *d_coef, int batch, void *d
   return remodulate(p, d_coef, batch, d_out, static_cast<cudaStream_t>(stream));
 }
 
+qtam_status qtam_instantaneous_frequency(qtam_plan *p, const void *d_coef, int batch, void *d_out, void *stream) {
+  if (p && p->host_only) return QTAM_ERR_CUDA;
+  if (!check_call(p, d_coef, d_out, batch)) return QTAM_ERR_INVALID_ARG;
+  p->last_launches = 0;
+  if (batch == 0) return QTAM_OK;
+  return instantaneous_frequency(p, d_coef, batch, d_out, static_cast<cudaStream_t>(stream));
+}
+
 qtam_status qtam_plane_metric(qtam_plan *p, const void *d_coef, int batch, int metric, void *d_metric,
                               int32_t *d_best, void *stream) {
   if (p && p->host_only) return QTAM_ERR_CUDA;
@@ -501,7 +509,7 @@ static const char *const kKernelNames[K_COUNT] = {
     "cfft_seq", "cfft_cols", "cfft_rows", "r2c_post", "c2r_pre", "fwd_rows", "fwd_combine",
     "inv_rows", "inv_reduce", "dense_place", "threshold", "r2c_fast", "fwd_rows_fast", "inv_rows_fast",
     "reduce_c2r_fast", "inv_fused", "inv_tiles", "combine_c2r", "threshold_fast", "rows_cta_fwd", "rows_cta_inv",
-    "tiny_rows_fwd", "tiny_rows_inv", "long_fft_a", "long_fft_b", "plane_metric", "best_plane", "remodulate"};
+    "tiny_rows_fwd", "tiny_rows_inv", "long_fft_a", "long_fft_b", "plane_metric", "best_plane", "remodulate", "inst_freq"};
 
 qtam_status qtam_profile_enable(qtam_plan *p, int on, int max_launches) {
   if (!p || p->host_only) return QTAM_ERR_INVALID_ARG;

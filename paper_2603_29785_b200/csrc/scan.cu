@@ -89,6 +89,40 @@ k_remodulate(const RowDev *__restrict__ rows, const C2<T> *__restrict__ coef, lo
   }
 }
 
+// Instantaneous frequency (Fig. 5; R16): the circular forward difference of the
+// unwrapped baseband phase, Arg(Y[n+1] conj Y[n]), scaled to Hz on the row's time grid, plus the carrier kc/T.
+template <typename T>
+__global__ void __launch_bounds__(128)
+k_inst_freq(const RowDev *__restrict__ rows, const C2<T> *__restrict__ coef, long long ctot, T inv_duration,
+            T *__restrict__ out) {
+  const RowDev r = rows[blockIdx.x];
+  const C2<T> *Y = coef + (size_t)blockIdx.y * ctot + r.offset;
+  T *O = out + (size_t)blockIdx.y * ctot + r.offset;
+  const T scale = (T)r.M * (T)0.15915494309189533577 * inv_duration;      // M / (2 pi T)
+  const T carrier = (T)r.kc * inv_duration;
+  for (int n = threadIdx.x; n < r.M; n += 128) {
+    const C2<T> a = Y[n], c = Y[(n + 1) & (r.M - 1)];
+    const T re = c.x * a.x + c.y * a.y, im = c.y * a.x - c.x * a.y;
+    O[n] = carrier + scale * atan2(im, re);
+  }
+}
+
+qtam_status instantaneous_frequency(qtam_plan *p, const void *d_coef, int batch, void *d_out, cudaStream_t st) {
+  dim3 g((unsigned)p->hp.rows.size(), batch);
+  const double inv_t = p->hp.fs / (double)p->hp.N;
+  {
+    LaunchScope ls(p, st, K_INST_FREQ, 3.0 * p->esz * (double)batch * (double)p->hp.ctot);
+    if (p->esz == 4)
+      k_inst_freq<float><<<g, 128, 0, st>>>(p->d_rows, static_cast<const float2 *>(d_coef), p->hp.ctot, (float)inv_t,
+                                           static_cast<float *>(d_out));
+    else
+      k_inst_freq<double><<<g, 128, 0, st>>>(p->d_rows, static_cast<const double2 *>(d_coef), p->hp.ctot, inv_t,
+                                            static_cast<double *>(d_out));
+  }
+  QTAM_LAUNCH_CHECK();
+  return QTAM_OK;
+}
+
 qtam_status remodulate(qtam_plan *p, const void *d_coef, int batch, void *d_out, cudaStream_t st) {
   dim3 g((unsigned)p->hp.rows.size(), batch);
   {

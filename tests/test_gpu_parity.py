@@ -444,3 +444,31 @@ def test_long_row_configs_full_batch_in_bench_configuration(name):
     assert np.max(np.abs(got - want) / want) <= 1e-5
     if "inverse" in cfg["calls"]:
         assert worst_segment(g.inverse(Y).cpu().numpy(), pi_c(x.astype(np.float64), C)) <= 1e-5
+
+
+@pytest.mark.parametrize("name,dtype", [("cfg3", "f32"), ("cfg1", "f64"), ("cfg2", "f32")])
+def test_instantaneous_frequency(name, dtype):
+    """PAPER.md:176 / Fig. 5.  The phase difference is compared on the circle (a value on the branch cut may
+    come out as +pi or -pi: both are the same angle), in turns per sample: |d - round(d)| small."""
+    nseg = 2
+    g, r = make_plans(inputs.plan_args(name), dtype, nseg)
+    x = inputs.make_batch(name, batch=nseg).astype(np_rdt(dtype))
+    Y = g.forward(dev(x))
+    F = g.instantaneous_frequency(Y).cpu().numpy().astype(np.float64)
+    Fr = r.instantaneous_frequency(Y.cpu().numpy().astype(np.complex128))
+    T = g.N / inputs.CONFIGS[name]["fs"]
+    tol = 1e-11 if dtype == "f64" else 2e-5
+    for k, row in enumerate(r.rows):
+        sl = slice(row.offset, row.offset + row.M)
+        d = (F[:, sl] - Fr[:, sl]) * T / row.M                    # turns per sample
+        assert np.max(np.abs(d - np.round(d))) <= tol, k
+    # the chirp / sinusoid check of the closed form on the GPU: a pure tone reads back its own frequency
+    t = np.arange(g.N) / inputs.CONFIGS[name]["fs"]
+    k0 = 300
+    tone = np.cos(2 * np.pi * (k0 / T) * t)[None, :].astype(np_rdt(dtype))
+    Ft = g.instantaneous_frequency(g.forward(dev(np.repeat(tone, nseg, axis=0)))).cpu().numpy()
+    hit = [k for k, row in enumerate(r.rows) if abs(k0 - row.kc) < row.dk // 2]
+    assert hit
+    for k in hit:
+        row = r.rows[k]
+        assert np.max(np.abs(Ft[0, row.offset:row.offset + row.M] - k0 / T)) <= (1e-6 if dtype == "f64" else 2e-2)
