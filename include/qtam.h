@@ -156,6 +156,13 @@ typedef enum { QTAM_METRIC_ENERGY = 0, QTAM_METRIC_PEAK = 1 } qtam_metric;
 qtam_status qtam_plane_metric(qtam_plan *p, const void *d_coef, int batch, int metric, void *d_metric,
                               int32_t *d_best, void *stream);
 
+/* qtam_forward followed by qtam_threshold_rowmedian(kappa) on its output, with the same result bit for bit
+ * (BASELINE.json config 5: "forward -> zero decimated coeffs with |c| below 3x row-median").  For float plans the
+ * threshold runs in the epilogue of the row kernel while a row is still in registers (rows of at most 1024
+ * points), so the coefficients are written once, already thresholded, and never re-read. */
+qtam_status qtam_forward_threshold(qtam_plan *p, const void *d_x, int batch, double kappa, void *d_coef,
+                                   void *stream);
+
 /* Number of kernel launches the last forward / inverse / threshold / dense call on this plan issued
  * (host counter, for bench.py's gpu_launches). */
 int         qtam_last_launch_count(const qtam_plan *p);

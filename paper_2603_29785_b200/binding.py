@@ -18,7 +18,7 @@ STATUS = {0: "ok", 1: "invalid argument", 2: "unsupported", 3: "alloc", 4: "cuda
 
 SYMBOLS = ["qtam_plan_create", "qtam_plan_create_host", "qtam_plan_destroy", "qtam_plan_info",
            "qtam_plan_rows", "qtam_plan_window", "qtam_plan_frame", "qtam_forward", "qtam_inverse",
-           "qtam_dense", "qtam_threshold_rowmedian", "qtam_plane_metric", "qtam_remodulate", "qtam_instantaneous_frequency", "qtam_last_launch_count", "qtam_status_string",
+           "qtam_dense", "qtam_threshold_rowmedian", "qtam_forward_threshold", "qtam_plane_metric", "qtam_remodulate", "qtam_instantaneous_frequency", "qtam_last_launch_count", "qtam_status_string",
            "qtam_profile_enable", "qtam_profile_read"]
 
 
@@ -79,6 +79,7 @@ def lib():
         L.qtam_inverse.argtypes = [vp, vp, C.c_int, C.c_int, vp, vp]
         L.qtam_dense.argtypes = [vp, vp, C.c_int, C.c_int, C.c_int, vp, vp]
         L.qtam_threshold_rowmedian.argtypes = [vp, vp, C.c_int, C.c_double, vp]
+        L.qtam_forward_threshold.argtypes = [vp, vp, C.c_int, C.c_double, vp, vp]
         L.qtam_plane_metric.argtypes = [vp, vp, C.c_int, C.c_int, vp, vp, vp]
         L.qtam_remodulate.argtypes = [vp, vp, C.c_int, vp, vp]
         L.qtam_instantaneous_frequency.argtypes = [vp, vp, C.c_int, vp, vp]
@@ -203,6 +204,18 @@ class Plan:
         if out is None:
             out = t.empty((batch, row_end - row_begin, self.N), dtype=self._cdt(), device=x.device)
         _check(lib().qtam_dense(self._h, x.data_ptr(), batch, row_begin, row_end, out.data_ptr(), self._stream()), "qtam_dense")
+        return out
+
+    def forward_threshold(self, x, kappa=3.0, out=None):
+        """forward + row-median threshold in one call (fused for float plans)"""
+        t = self._torch()
+        assert x.is_cuda and x.dtype == self._rdt() and x.is_contiguous() and x.shape[-1] == self.N
+        batch = x.numel() // self.N
+        if out is None:
+            out = t.empty((batch, self.ctot), dtype=self._cdt(), device=x.device)
+        assert out.is_cuda and out.dtype == self._cdt() and out.is_contiguous() and out.numel() == batch * self.ctot
+        _check(lib().qtam_forward_threshold(self._h, x.data_ptr(), batch, float(kappa), out.data_ptr(), self._stream()),
+               "qtam_forward_threshold")
         return out
 
     def threshold_rowmedian(self, coef, kappa=3.0):

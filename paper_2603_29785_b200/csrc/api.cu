@@ -427,6 +427,47 @@ qtam_status qtam_forward(qtam_plan *p, const void *d_x, int batch, void *d_coef,
   return generic_forward_rows(p, batch, d_coef, st);
 }
 
+qtam_status qtam_forward_threshold(qtam_plan *p, const void *d_x, int batch, double kappa, void *d_coef,
+                                   void *stream) {
+  if (p && p->host_only) return QTAM_ERR_CUDA;
+  if (!check_call(p, d_x, d_coef, batch) || !(kappa >= 0.0)) return QTAM_ERR_INVALID_ARG;
+  p->last_launches = 0;
+  if (batch == 0) return QTAM_OK;
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  if (p->fast_rows && p->esz == 4) {
+    // the threshold rides in the epilogue of the row kernel for every row of at most 1024 points
+    qtam_status s = p->fast_long ? fast_r2c(p, d_x, batch, st) : generic_r2c(p, d_x, batch, st);
+    if (s != QTAM_OK) return s;
+    bool fused = false;
+    s = fast_forward_rows_threshold(p, batch, d_coef, (float)kappa, st, &fused);
+    if (s != QTAM_OK) return s;
+    if (fused) {
+      if (p->cta_rows) {
+        s = cta_forward_rows(p, batch, d_coef, st);
+        if (s != QTAM_OK) return s;
+      }
+      s = generic_forward_rows(p, batch, d_coef, st);
+      if (s != QTAM_OK || !p->thr_has_big) return s;
+      return generic_threshold(p, d_coef, batch, kappa, kThrFastLog2Max + 1, st);   // rows longer than 1024 points
+    }
+    // not fusable for this plan / batch: the two steps one after the other
+    s = fast_forward_rows(p, batch, d_coef, st);
+    if (s == QTAM_OK && p->cta_rows) s = cta_forward_rows(p, batch, d_coef, st);
+    if (s == QTAM_OK) s = generic_forward_rows(p, batch, d_coef, st);
+    if (s != QTAM_OK) return s;
+    const int n1 = p->last_launches;
+    s = qtam_threshold_rowmedian(p, d_coef, batch, kappa, stream);
+    p->last_launches += n1;
+    return s;
+  }
+  qtam_status s = qtam_forward(p, d_x, batch, d_coef, stream);
+  if (s != QTAM_OK) return s;
+  const int n1 = p->last_launches;
+  s = qtam_threshold_rowmedian(p, d_coef, batch, kappa, stream);
+  p->last_launches += n1;
+  return s;
+}
+
 qtam_status qtam_inverse(qtam_plan *p, const void *d_coef, int batch, int plane, void *d_x_out,
                          void *stream) {
   if (p && p->host_only) return QTAM_ERR_CUDA;
@@ -509,7 +550,7 @@ static const char *const kKernelNames[K_COUNT] = {
     "cfft_seq", "cfft_cols", "cfft_rows", "r2c_post", "c2r_pre", "fwd_rows", "fwd_combine",
     "inv_rows", "inv_reduce", "dense_place", "threshold", "r2c_fast", "fwd_rows_fast", "inv_rows_fast",
     "reduce_c2r_fast", "inv_fused", "inv_tiles", "combine_c2r", "threshold_fast", "rows_cta_fwd", "rows_cta_inv",
-    "tiny_rows_fwd", "tiny_rows_inv", "long_fft_a", "long_fft_b", "plane_metric", "best_plane", "remodulate", "inst_freq"};
+    "tiny_rows_fwd", "tiny_rows_inv", "long_fft_a", "long_fft_b", "plane_metric", "best_plane", "remodulate", "inst_freq", "fwd_rows_thr"};
 
 qtam_status qtam_profile_enable(qtam_plan *p, int on, int max_launches) {
   if (!p || p->host_only) return QTAM_ERR_INVALID_ARG;

@@ -13,7 +13,7 @@ enum KernelId {
   K_CFFT_SEQ = 0, K_CFFT_COLS, K_CFFT_ROWS, K_R2C_POST, K_C2R_PRE, K_FWD_ROWS, K_FWD_COMBINE,
   K_INV_ROWS, K_INV_REDUCE, K_DENSE_PLACE, K_THRESHOLD, K_R2C_FAST, K_FWD_ROWS_FAST, K_INV_ROWS_FAST,
   K_REDUCE_C2R_FAST, K_INV_FUSED, K_INV_TILES, K_COMBINE_C2R, K_THRESHOLD_FAST, K_ROWS_CTA_FWD, K_ROWS_CTA_INV,
-  K_TINY_FWD, K_TINY_INV, K_LONG_A, K_LONG_B, K_PLANE_METRIC, K_BEST_PLANE, K_REMODULATE, K_INST_FREQ, K_COUNT
+  K_TINY_FWD, K_TINY_INV, K_LONG_A, K_LONG_B, K_PLANE_METRIC, K_BEST_PLANE, K_REMODULATE, K_INST_FREQ, K_FWD_ROWS_THR, K_COUNT
 };
 // fast float path (fast.cu): rows with 32 <= M <= 1024, grouped by G = M/32 lanes per row
 struct FastRow { int kc, dk, woff, goff, offset, plane, wpad, pad; };   // wpad: offset into the padded window table
@@ -173,6 +173,8 @@ qtam_status build_long_tables(qtam_plan *p);
 qtam_status fast_r2c(qtam_plan *p, const void *d_x, int batch, cudaStream_t st);
 qtam_status fast_forward_rows(qtam_plan *p, int batch, void *d_coef, cudaStream_t st);
 qtam_status fast_inverse_rows(qtam_plan *p, const void *d_coef, int batch, int plane, cudaStream_t st);
+qtam_status fast_forward_rows_threshold(qtam_plan *p, int batch, void *d_coef, float kappa, cudaStream_t st,
+                                        bool *done);
 qtam_status fast_reduce_c2r(qtam_plan *p, int batch, int plane, void *d_x_out, cudaStream_t st);
 // long_fft.cu
 qtam_status build_long_fft(qtam_plan *p);

@@ -15,6 +15,7 @@
 #include "ctafft.cuh"
 #include "device_plan.hpp"
 #include "rowfft.cuh"
+#include "thrselect.cuh"
 #include "tinyrow.cuh"
 
 namespace qtam {
@@ -66,11 +67,12 @@ k_r2c_fast(const float *__restrict__ x, float2 *__restrict__ spec, long long xst
 // Y = (N M)^{-1/2} IFFT_M(B) (C47).  Inverse: G[jj] = sqrt(N/M) FFT_M(Y)[jj mod M] W[jj] to the band
 // workspace (C49).  For tiny rows FastRow::goff holds log2 M and FastRow::wpad the band offset.
 // --------------------------------------------------------------------------------------------------
-template <bool FORWARD>
+template <bool FORWARD, bool THRESH = false>
 __device__ __forceinline__ void tiny_dispatch(long long id, const FastRow *__restrict__ tiny, int n_tiny,
                                               const float *__restrict__ fwin, const float2 *__restrict__ spec,
                                               long long xstride, int nbins, float2 *__restrict__ coef, long long ctot,
-                                              float2 *__restrict__ band, long long sumL, int plane, float n_samples) {
+                                              float2 *__restrict__ band, long long sumL, int plane, float n_samples,
+                                              float kappa = 0.f) {
   const int seg = (int)(id / n_tiny);
   const FastRow row = tiny[id - (long long)seg * n_tiny];
   if (!FORWARD && plane >= 0 && row.plane != plane) return;
@@ -80,9 +82,9 @@ __device__ __forceinline__ void tiny_dispatch(long long id, const FastRow *__res
   const float Mf = (float)(1 << row.goff);
   const float scale = FORWARD ? rsqrtf(n_samples * Mf) : sqrtf(n_samples / Mf);
   switch (row.goff) {
-    case 2: tiny_row<4, FORWARD>(row, X, fwin, Y, Gb, nbins, scale); break;
-    case 3: tiny_row<8, FORWARD>(row, X, fwin, Y, Gb, nbins, scale); break;
-    case 4: tiny_row<16, FORWARD>(row, X, fwin, Y, Gb, nbins, scale); break;
+    case 2: tiny_row<4, FORWARD, THRESH>(row, X, fwin, Y, Gb, nbins, scale, kappa); break;
+    case 3: tiny_row<8, FORWARD, THRESH>(row, X, fwin, Y, Gb, nbins, scale, kappa); break;
+    case 4: tiny_row<16, FORWARD, THRESH>(row, X, fwin, Y, Gb, nbins, scale, kappa); break;
     default: break;
   }
 }
@@ -102,12 +104,12 @@ k_tiny_rows(const FastRow *__restrict__ tiny, int n_tiny, const float *__restric
 // a CTA takes NWARPS consecutive items, i.e. neighbouring rows of one segment, so that the bands its
 // warps read overlap in L1.
 // --------------------------------------------------------------------------------------------------
-template <int LOG2G>
+template <int LOG2G, bool THRESH = false>
 __device__ QTAM_GROUP_INLINE void fwd_group(const FastBucket &B, const FastRow *__restrict__ frows, int seg, int grp,
                                        int lane, float2 *ex, const float2 *tw1,
                                        const float2 *__restrict__ spec, long long xstride,
                                        const float *__restrict__ fwinp, float2 *__restrict__ coef,
-                                       long long ctot, const int *__restrict__ fmem) {
+                                       long long ctot, const int *__restrict__ fmem, float kappa = 0.f) {
   constexpr int G = 1 << LOG2G, F = 32 / G, M = 32 * G;
   const int t = lane & (G - 1), rw = lane >> LOG2G;
   const int r = grp * F + rw;
@@ -135,6 +137,20 @@ __device__ QTAM_GROUP_INLINE void fwd_group(const FastBucket &B, const FastRow *
   // the first member's offset is fetched before the transform, every further one an iteration ahead
   int moff = __ldg(fmem + row.pad);
   RowFFT<LOG2G, +1>::run(v, ex, tw1, lane);
+  if constexpr (THRESH) {
+    // a4 fused into the epilogue: the row is in the registers of its G lanes; same decisions, bit for bit,
+    // as qtam_threshold_rowmedian on the stored coefficients (thrselect.cuh)
+    unsigned x[32], vor = 0u, vand = ~0u;
+#pragma unroll
+    for (int e = 0; e < 32; ++e) {
+      x[e] = Bits<float>::of(Bits<float>::add(Bits<float>::mul(v[e].x, v[e].x), Bits<float>::mul(v[e].y, v[e].y)));
+      vor |= x[e]; vand &= x[e];
+    }
+    unsigned prefix;
+    const unsigned cut = thr_select<float, 32>(x, vor, vand, G, kappa, prefix);
+#pragma unroll
+    for (int e = 0; e < 32; ++e) if ((x[e] ^ prefix) < cut) v[e] = make_float2(0.f, 0.f);
+  }
   if (valid) {
     // every member of the leader's set (rows with this centre bin and half-width) gets the same values
 #pragma unroll 1
@@ -185,14 +201,14 @@ __device__ QTAM_GROUP_INLINE void inv_group(const FastBucket &B, const FastRow *
   }
 }
 
-template <int NWARPS, bool FORWARD>
+template <int NWARPS, bool FORWARD, bool THRESH = false>
 __global__ void __launch_bounds__(NWARPS * 32, NWARPS <= 8 ? 2 : 1)
 k_rows_fast(FastParams P, const FastRow *frows, const void *__restrict__ tw1g_,
             const float *__restrict__ fwin, const float *__restrict__ fwinp,
             const float2 *__restrict__ spec, long long xstride, int nbins,
             float2 *__restrict__ coef, long long ctot, float2 *__restrict__ band, long long sumL,
             int batch, int plane, const FastRow *__restrict__ tiny, int n_tiny, float n_samples,
-            const int *__restrict__ fmem) {
+            const int *__restrict__ fmem, float kappa) {
   typedef float2 TW;
   const TW *tw1g = static_cast<const TW *>(tw1g_);
   TW *tw1s = reinterpret_cast<TW *>(qtam_fast_smem);
@@ -211,7 +227,7 @@ k_rows_fast(FastParams P, const FastRow *frows, const void *__restrict__ tw1g_,
   if constexpr (FORWARD) {
     const long long id = (long long)blockIdx.x * (NWARPS * 32) + threadIdx.x;
     if (id < (long long)n_tiny * batch)
-      tiny_dispatch<true>(id, tiny, n_tiny, fwin, spec, xstride, nbins, coef, ctot, band, sumL, -1, n_samples);
+      tiny_dispatch<true, THRESH>(id, tiny, n_tiny, fwin, spec, xstride, nbins, coef, ctot, band, sumL, -1, n_samples, kappa);
   }
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   float2 *ex = exall + warp * kExPerWarp;
@@ -231,7 +247,7 @@ k_rows_fast(FastParams P, const FastRow *frows, const void *__restrict__ tw1g_,
     const TW *tw1 = tw1s + B.tw_base;
 #define QTAM_ROW_CASE(L)                                                                              \
   case L:                                                                                             \
-    if constexpr (FORWARD) fwd_group<L>(B, frows, seg, grp, lane, ex, tw1, spec, xstride, fwinp, coef, ctot, fmem); \
+    if constexpr (FORWARD) fwd_group<L, THRESH>(B, frows, seg, grp, lane, ex, tw1, spec, xstride, fwinp, coef, ctot, fmem, kappa); \
     else inv_group<L>(B, frows, seg, grp, lane, ex, tw1, coef, ctot, nbins, fwin, band, sumL, plane);  \
     break;
     switch (B.log2G) {
@@ -331,16 +347,16 @@ qtam_status fast_r2c(qtam_plan *p, const void *d_x, int batch, cudaStream_t st) 
   }
 }
 
-template <int NW, bool FORWARD>
+template <int NW, bool FORWARD, bool THRESH = false>
 static qtam_status rows_launch_nw(qtam_plan *p, int batch, const void *d_coef_in, void *d_coef_out, int plane,
-                                  cudaStream_t st, bool *tiny_rode) {
+                                  cudaStream_t st, bool *tiny_rode, float kappa = 0.f) {
   const FastParams &P = FORWARD ? p->fast_fwd : p->fast;
   if (tiny_rode) *tiny_rode = false;
   if (P.groups_per_seg == 0) return QTAM_OK;
   const size_t smem = sizeof(float2) * (size_t)((P.tw_total + 1) & ~1) + sizeof(float2) * (size_t)NW * kExPerWarp +
                       sizeof(FastRow) * (size_t)P.rows_smem;
   if ((long long)P.groups_per_seg * batch >= (1LL << 31)) return QTAM_ERR_UNSUPPORTED;
-  auto kern = k_rows_fast<NW, FORWARD>;
+  auto kern = k_rows_fast<NW, FORWARD, THRESH>;
   if (!set_smem(kern, smem)) return QTAM_ERR_CUDA;
   int occ = 1;
   cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, NW * 32, smem);
@@ -357,7 +373,7 @@ static qtam_status rows_launch_nw(qtam_plan *p, int batch, const void *d_coef_in
   const double bytes = FORWARD ? (double)batch * 8.0 * (P.sum_M + (double)p->hp.nb + (ride ? p->tiny_sumM : 0.0))
                                : (double)batch * 8.0 * (P.sum_M + P.sum_L);
   {
-    LaunchScope ls(p, st, FORWARD ? K_FWD_ROWS_FAST : K_INV_ROWS_FAST, bytes);
+    LaunchScope ls(p, st, FORWARD ? (THRESH ? K_FWD_ROWS_THR : K_FWD_ROWS_FAST) : K_INV_ROWS_FAST, bytes);
     kern<<<grid, NW * 32, smem, st>>>(
         P, FORWARD ? p->d_frows_fwd : p->d_frows, static_cast<const void *>(FORWARD ? p->d_ftw_fwd : p->d_ftw_inv),
         static_cast<const float *>(p->d_fwin), static_cast<const float *>(p->d_fwinp),
@@ -365,7 +381,7 @@ static qtam_status rows_launch_nw(qtam_plan *p, int batch, const void *d_coef_in
         (int)p->hp.nb,
         FORWARD ? static_cast<float2 *>(d_coef_out) : const_cast<float2 *>(static_cast<const float2 *>(d_coef_in)),
         p->hp.ctot, static_cast<float2 *>(p->d_band), p->hp.sumL, batch, plane, p->d_tiny, ride ? p->n_tiny : 0,
-        (float)p->hp.N, p->d_fmem);
+        (float)p->hp.N, p->d_fmem, kappa);
   }
   QTAM_LAUNCH_CHECK();
   if (tiny_rode) *tiny_rode = ride;
@@ -414,6 +430,24 @@ qtam_status fast_forward_rows(qtam_plan *p, int batch, void *d_coef, cudaStream_
   const qtam_status s = rows_launch<true>(p, batch, nullptr, d_coef, -1, st, &rode);
   if (s != QTAM_OK || rode) return s;
   return tiny_launch<true>(p, batch, d_coef, -1, st);
+}
+
+// a2 + a3 + a4 in one launch for every row of at most 1024 points; `*done` = false when the plan's rows
+// shorter than 32 points could not ride along (the caller then runs forward and threshold separately)
+qtam_status fast_forward_rows_threshold(qtam_plan *p, int batch, void *d_coef, float kappa, cudaStream_t st,
+                                        bool *done) {
+  *done = false;
+  const FastParams &P = p->fast_fwd;
+  // (a lower bound of the launch's grid: the rows shorter than 32 points need one thread each)
+  const long long want = ((long long)P.groups_per_seg * batch + 7) / 8;
+  const long long sure_threads = (want < p->num_sms ? want : (long long)p->num_sms) * 256;
+  if (P.groups_per_seg == 0 || (p->n_tiny > 0 && sure_threads < (long long)p->n_tiny * batch)) return QTAM_OK;
+  bool rode = false;
+  const qtam_status s = rows_launch_nw<8, true, true>(p, batch, nullptr, d_coef, -1, st, &rode, kappa);
+  if (s != QTAM_OK) return s;
+  if (p->n_tiny > 0 && !rode) return QTAM_ERR_UNSUPPORTED;   // cannot happen given the test above
+  *done = true;
+  return QTAM_OK;
 }
 
 qtam_status fast_inverse_rows(qtam_plan *p, const void *d_coef, int batch, int plane, cudaStream_t st) {

@@ -504,3 +504,16 @@ def test_forward_inverse_under_cuda_graph_capture():
         ref_Y = g.forward(src)
         ref_x = g.inverse(ref_Y)
         assert torch.equal(got_Y, ref_Y) and torch.equal(got_x, ref_x)
+
+
+@pytest.mark.parametrize("name,dtype,nseg", [("cfg5", "f32", 16), ("cfg3", "f32", 3), ("cfg2", "f32", 2), ("cfg5", "f64", 3),
+                                             ("cfg5", "f32", 1)])
+def test_forward_threshold_fused_equals_the_two_calls(name, dtype, nseg):
+    """qtam_forward_threshold = qtam_forward then qtam_threshold_rowmedian, bit for bit (the decisions are taken
+    on the same binary32 values, in registers instead of after a round trip through memory)."""
+    g, _ = make_plans(inputs.plan_args(name), dtype, nseg)
+    x = dev(inputs.make_batch(name, batch=nseg).astype(np_rdt(dtype)))
+    two = g.threshold_rowmedian(g.forward(x), 3.0)
+    one = g.forward_threshold(x, 3.0)
+    assert torch.equal(torch.view_as_real(one), torch.view_as_real(two))
+    assert 0 < (one != 0).float().mean().item() < 0.2
