@@ -96,7 +96,13 @@ k_threshold_fast(const ThrTask *__restrict__ tasks, int n_tasks, const int *__re
     case 2: thr_group<T, 4>(Y, 1, 0, kappa); break;
     case 3: thr_group<T, 8>(Y, 1, 0, kappa); break;
     case 4: thr_group<T, 16>(Y, 1, 0, kappa); break;
-    default: thr_group<T, 32>(Y, G, t, kappa); break;
+    // (the lanes-per-row count as a literal: the shuffle loops of the select unroll)
+    case 5: thr_group<T, 32>(Y, 1, t, kappa); break;
+    case 6: thr_group<T, 32>(Y, 2, t, kappa); break;
+    case 7: thr_group<T, 32>(Y, 4, t, kappa); break;
+    case 8: thr_group<T, 32>(Y, 8, t, kappa); break;
+    case 9: thr_group<T, 32>(Y, 16, t, kappa); break;
+    default: thr_group<T, 32>(Y, 32, t, kappa); break;
   }
 }
 
