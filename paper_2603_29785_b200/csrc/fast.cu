@@ -225,8 +225,8 @@ k_rows_fast(FastParams P, const FastRow *frows, const void *__restrict__ tw1g_,
   __syncthreads();
   // rows shorter than 32 points ride along, one thread per (segment, row) (n_tiny = 0: separate launch)
   if constexpr (FORWARD) {
-    const long long id = (long long)blockIdx.x * (NWARPS * 32) + threadIdx.x;
-    if (id < (long long)n_tiny * batch)
+    for (long long id = (long long)blockIdx.x * (NWARPS * 32) + threadIdx.x; id < (long long)n_tiny * batch;
+         id += (long long)gridDim.x * (NWARPS * 32))
       tiny_dispatch<true, THRESH>(id, tiny, n_tiny, fwin, spec, xstride, nbins, coef, ctot, band, sumL, -1, n_samples, kappa);
   }
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -368,8 +368,8 @@ static qtam_status rows_launch_nw(qtam_plan *p, int batch, const void *d_coef_in
   static const int waves = getenv("QTAM_ROW_WAVES") ? atoi(getenv("QTAM_ROW_WAVES")) : 1;
   int grid = (int)(want < resident * waves ? want : resident * waves);
   if (grid < 1) grid = 1;
-  // the forward launch also takes the rows shorter than 32 points when its grid has a thread for each
-  const bool ride = FORWARD && p->n_tiny > 0 && (long long)grid * NW * 32 >= (long long)p->n_tiny * batch;
+  // the forward launch also takes the rows shorter than 32 points, one thread per (segment, row)
+  const bool ride = FORWARD && p->n_tiny > 0;    // grid-stride loop in the kernel: any count rides
   const double bytes = FORWARD ? (double)batch * 8.0 * (P.sum_M + (double)p->hp.nb + (ride ? p->tiny_sumM : 0.0))
                                : (double)batch * 8.0 * (P.sum_M + P.sum_L);
   {
@@ -438,10 +438,7 @@ qtam_status fast_forward_rows_threshold(qtam_plan *p, int batch, void *d_coef, f
                                         bool *done) {
   *done = false;
   const FastParams &P = p->fast_fwd;
-  // (a lower bound of the launch's grid: the rows shorter than 32 points need one thread each)
-  const long long want = ((long long)P.groups_per_seg * batch + 7) / 8;
-  const long long sure_threads = (want < p->num_sms ? want : (long long)p->num_sms) * 256;
-  if (P.groups_per_seg == 0 || (p->n_tiny > 0 && sure_threads < (long long)p->n_tiny * batch)) return QTAM_OK;
+  if (P.groups_per_seg == 0) return QTAM_OK;
   bool rode = false;
   const qtam_status s = rows_launch_nw<8, true, true>(p, batch, nullptr, d_coef, -1, st, &rode, kappa);
   if (s != QTAM_OK) return s;
