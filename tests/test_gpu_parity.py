@@ -517,3 +517,64 @@ def test_forward_threshold_fused_equals_the_two_calls(name, dtype, nseg):
     one = g.forward_threshold(x, 3.0)
     assert torch.equal(torch.view_as_real(one), torch.view_as_real(two))
     assert 0 < (one != 0).float().mean().item() < 0.2
+
+
+def _random_plan_cases():
+    """seeded sweep over plan shapes: segment lengths 2^8..2^17, 1-4 planes, clamp settings, window families,
+    tile-length modes, bins-per-octave grids -- the dispatch takes different kernels for different shapes"""
+    rng = np.random.default_rng(20260329785 % (2 ** 32))
+    cases = []
+    for i in range(14):
+        log2n = int(rng.integers(8, 18))
+        N = 1 << log2n
+        fs = float(rng.choice([1024.0, 4096.0, 16384.0]))
+        nq = int(rng.integers(1, 5))
+        Q = sorted(float(q) for q in rng.uniform(3.4, 60.0, size=nq))
+        fmax = float(rng.uniform(0.2, 0.49)) * fs
+        T = N / fs
+        fmin = max(float(rng.uniform(2.0, 30.0)) * max(Q) / (np.sqrt(11.0) * T), 2.0 / T)   # half-width >= 1 bin
+        if fmin >= 0.5 * fmax:
+            fmin = 0.25 * fmax
+        kw = dict(clamp_overlap=float(rng.choice([1.0, 1.5, 2.0])))
+        mode = int(rng.integers(0, 4))
+        if mode == 1:
+            kw["window"], kw["window_param"] = "tukey", float(rng.uniform(0.2, 0.9))
+        elif mode == 2:
+            kw["window"], kw["window_param"] = "kaiser", float(rng.uniform(2.0, 9.0))
+        elif mode == 3:
+            kw["tile_length"] = -1
+        if rng.integers(0, 3) == 0:
+            kw["rows_are_bins_per_octave"] = 1
+            spacing = float(rng.integers(3, 12))
+        else:
+            spacing = float(rng.integers(5, 40))
+        cases.append((i, fs, N, Q, fmin, fmax, spacing, "f64" if i % 3 == 2 else "f32", kw))
+    return cases
+
+
+@pytest.mark.parametrize("case", _random_plan_cases(), ids=lambda c: f"case{c[0]}-N{c[2]}-{c[7]}")
+def test_random_plan_shapes(case):
+    i, fs, N, Q, fmin, fmax, spacing, dtype, kw = case
+    try:
+        r = RefPlan(fs, N, Q, fmin, fmax, spacing, **kw)
+    except ValueError:
+        with pytest.raises(binding.QtamError):
+            binding.Plan(fs, N, Q, fmin, fmax, spacing, dtype=dtype, max_batch=2, **kw)
+        return
+    g = binding.Plan(fs, N, Q, fmin, fmax, spacing, dtype=dtype, max_batch=2, **kw)
+    assert [(a.kc, a.dk, a.M, a.offset) for a in g.rows] == [(b.kc, b.dk, b.M, b.offset) for b in r.rows]
+    x = inputs.white_noise(N, 1000 + i, batch=2).astype(np_rdt(dtype))
+    x64 = x.astype(np.float64)
+    Y = g.forward(dev(x))
+    assert worst_segment(Y.cpu().numpy(), r.forward(x64, engine=1)) <= TOL[dtype]
+    rng = np.random.default_rng(2000 + i)
+    Yin = (rng.standard_normal((2, g.ctot)) + 1j * rng.standard_normal((2, g.ctot))).astype(Y.cpu().numpy().dtype)
+    for plane in (-1, g.n_planes - 1):
+        xg = g.inverse(dev(Yin), plane=plane).cpu().numpy()
+        xr = r.inverse(Yin.astype(np.complex128), plane=plane, engine=1)
+        assert worst_segment(xg, xr) <= TOL[dtype], plane
+    _, C = r.frame(-1)
+    assert worst_segment(g.inverse(Y).cpu().numpy(), pi_c(x64, C)) <= TOL_RT[dtype]
+    two = g.threshold_rowmedian(g.forward(dev(x)), 2.5)
+    one = g.forward_threshold(dev(x), 2.5)
+    assert torch.equal(torch.view_as_real(one), torch.view_as_real(two))
