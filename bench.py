@@ -488,6 +488,42 @@ def run_ours(args):
         plan_b.close()
         del x_big, c_big, o_big
 
+    # ---- cuFFT (through torch.fft) on the same shapes, side by side as a reference only (north_star): the
+    # long real transforms and one batched complex transform per length bucket -- cuFFT does the FFTs alone,
+    # without the gather / window / shift, the overlap sum or 1/P, and writes one row per (plane, row)
+    cufft = None
+    if world == 1:
+        def ev_time(fn, reps=10):
+            fn(); torch.cuda.synchronize()
+            tot = 0.0
+            for _ in range(reps):
+                flush.zero_()
+                a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                a.record(); fn(); b.record(); torch.cuda.synchronize()
+                tot += a.elapsed_time(b)
+            return tot / reps
+        try:
+            spec_t = torch.fft.rfft(d_x, dim=-1)
+            cufft = {"rfft_ms": ev_time(lambda: torch.fft.rfft(d_x, dim=-1)),
+                     "irfft_ms": ev_time(lambda: torch.fft.irfft(spec_t, n=N, dim=-1)), "buckets": []}
+            hist = {}
+            for r_ in plan.rows:
+                hist[int(r_.M)] = hist.get(int(r_.M), 0) + 1
+            tot_c2c = 0.0
+            for M_, cnt in sorted(hist.items()):
+                if batch * cnt * M_ * 8 > (6 << 30):
+                    continue
+                buf = torch.randn(batch * cnt, M_, dtype=cdt, device=dev)
+                t_ = ev_time(lambda: torch.fft.ifft(buf, dim=-1))
+                cufft["buckets"].append({"M": M_, "rows": cnt, "c2c_ms": t_})
+                tot_c2c += t_
+                del buf
+            cufft["c2c_all_buckets_ms"] = tot_c2c
+            cufft["note"] = "FFTs only, out of place, one launch per length; context, not the target"
+            del spec_t
+        except Exception as exc:
+            cufft = {"unavailable": str(exc)}
+
     cpu = None
     if world == 1 and not args.no_cpu_baseline:
         v, cores, nseg, dt = time_oracle(cfg, args.workload, args.overlap)
@@ -510,6 +546,7 @@ def run_ours(args):
         "kernels": kernels,
         "round_trip_err": rt_err,
         "largest_batch": largest,
+        "cufft_side_by_side": cufft,
         "cpu_baseline": cpu,
     }
     print(json.dumps(line))
