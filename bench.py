@@ -151,7 +151,9 @@ def physical_gpu_index(local):
 # reference arm: the CPU oracle, as it stands, on the host cores
 # --------------------------------------------------------------------------------------------------
 def oracle_step_fn(cfg, name, overlap, nseg):
-    from oracle.qtam_ref import RefPlan, threads
+    from oracle.qtam_ref import RefPlan, set_threads, threads
+    # torchrun exports OMP_NUM_THREADS=1 for every rank; the baseline is "the oracle on the box's host cores"
+    set_threads(len(os.sched_getaffinity(0)) if hasattr(os, "sched_getaffinity") else (os.cpu_count() or 1))
     fs, N, Q, fmin, fmax, rows = inputs.plan_args(name)
     plan = RefPlan(fs, N, Q, fmin, fmax, rows, clamp_overlap=overlap)
     x = inputs.make_batch(name, batch=nseg).astype(np.float64)

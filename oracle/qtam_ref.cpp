@@ -181,6 +181,15 @@ int qtam_ref_threads(void) {
 #endif
 }
 
+// lets the caller undo a launcher's OMP_NUM_THREADS=1 default (torchrun sets it for every rank)
+void qtam_ref_set_threads(int n) {
+#ifdef _OPENMP
+  if (n > 0) omp_set_num_threads(n);
+#else
+  (void)n;
+#endif
+}
+
 int qtam_ref_dft(const double *in, double *out, int64_t n, int sign) {
   if (!in || !out || n < 1 || (sign != 1 && sign != -1)) return 1;
   dft_naive(reinterpret_cast<const cd *>(in), reinterpret_cast<cd *>(out), n, sign);

@@ -117,6 +117,7 @@ int  qtam_ref_dft(const double *in, double *out, int64_t n, int sign);
 int  qtam_ref_fft(const double *in, double *out, int64_t n, int sign);
 /* Number of OpenMP threads the batch loops use. */
 int  qtam_ref_threads(void);
+void qtam_ref_set_threads(int n);
 
 #ifdef __cplusplus
 }

@@ -83,6 +83,10 @@ def threads():
     return int(lib().qtam_ref_threads())
 
 
+def set_threads(n):
+    lib().qtam_ref_set_threads(int(n))
+
+
 def dft(z, sign):
     z = np.ascontiguousarray(z, dtype=np.complex128)
     out = np.empty_like(z)
