@@ -727,4 +727,27 @@ int qtam_ref_plane_metric(const qtam_ref_plan *p, const double *coef, int batch,
   return 0;
 }
 
+// "Optimal selection mode": the composite output built from each segment's best plane.  Planes
+// have different sizes in the ragged layout, so the output is [batch][max_p C_p], plane best[b] of segment b
+// copied to its start and the rest zero.
+int qtam_ref_gather_plane(const qtam_ref_plan *p, const double *coef, int batch, const int32_t *best, double *out) {
+  if (!p || !coef || !best || !out || batch < 0) return 1;
+  std::vector<int64_t> lo((size_t)p->nP, p->ctot), hi((size_t)p->nP, 0);
+  for (const Row &r : p->rows) {
+    lo[(size_t)r.plane] = std::min(lo[(size_t)r.plane], r.offset);
+    hi[(size_t)r.plane] = std::max(hi[(size_t)r.plane], r.offset + r.M);
+  }
+  int64_t cmax = 0;
+  for (int q = 0; q < p->nP; ++q) cmax = std::max(cmax, hi[(size_t)q] - lo[(size_t)q]);
+  for (int b = 0; b < batch; ++b) {
+    if (best[b] < 0 || best[b] >= p->nP) return 1;
+    const int64_t a = lo[(size_t)best[b]], n = hi[(size_t)best[b]] - a;
+    for (int64_t i = 0; i < cmax; ++i) {
+      out[2 * ((size_t)b * cmax + i)] = i < n ? coef[2 * ((size_t)b * p->ctot + a + i)] : 0.0;
+      out[2 * ((size_t)b * cmax + i) + 1] = i < n ? coef[2 * ((size_t)b * p->ctot + a + i) + 1] : 0.0;
+    }
+  }
+  return 0;
+}
+
 }  // extern "C"

@@ -115,6 +115,10 @@ int  qtam_ref_spectrum(const qtam_ref_plan *p, const double *x, int batch, doubl
  * never scaled. qtam_ref_dft: naive sums. qtam_ref_fft: recursive radix-2, n a power of two.      */
 int  qtam_ref_dft(const double *in, double *out, int64_t n, int sign);
 int  qtam_ref_fft(const double *in, double *out, int64_t n, int sign);
+/* Optimal-selection output: out[batch][max_p C_p] complex, plane best[b] of segment b at its
+ * start, zero after it. */
+int  qtam_ref_gather_plane(const qtam_ref_plan *p, const double *coef, int batch, const int32_t *best, double *out);
+
 /* Number of OpenMP threads the batch loops use. */
 int  qtam_ref_threads(void);
 void qtam_ref_set_threads(int n);

@@ -61,6 +61,7 @@ def lib():
         _lib.qtam_ref_threshold_rowmedian_f32.argtypes = [vp, fp, C.c_int, C.c_float]
         _lib.qtam_ref_remodulate.argtypes = [vp, dp, C.c_int, dp]
         _lib.qtam_ref_instantaneous_frequency.argtypes = [vp, dp, C.c_int, dp]
+        _lib.qtam_ref_gather_plane.argtypes = [vp, dp, C.c_int, C.POINTER(C.c_int32), dp]
         _lib.qtam_ref_plane_metric.argtypes = [vp, dp, C.c_int, C.c_int, dp, C.POINTER(C.c_int32)]
         _lib.qtam_ref_project_cover.argtypes = [vp, dp, C.c_int, C.c_int, dp, C.c_int]
         _lib.qtam_ref_spectrum.argtypes = [vp, dp, C.c_int, dp, C.c_int]
@@ -205,6 +206,22 @@ class RefPlan:
         c = np.ascontiguousarray(np.atleast_2d(coef), dtype=np.complex128)
         out = np.empty(c.shape, dtype=np.float64)
         assert lib().qtam_ref_instantaneous_frequency(self._h, _dp(c.view(np.float64)), c.shape[0], _dp(out)) == 0
+        return out
+
+    def plane_sizes(self):
+        """coefficients per plane in the layout"""
+        sizes = np.zeros(self.n_planes, dtype=np.int64)
+        for r in self.rows:
+            sizes[r.plane] += r.M
+        return sizes
+
+    def gather_plane(self, coef, best):
+        c = np.ascontiguousarray(np.atleast_2d(coef), dtype=np.complex128)
+        b = np.ascontiguousarray(best, dtype=np.int32)
+        out = np.empty((c.shape[0], int(self.plane_sizes().max())), dtype=np.complex128)
+        rc = lib().qtam_ref_gather_plane(self._h, _dp(c.view(np.float64)), c.shape[0],
+                                         b.ctypes.data_as(C.POINTER(C.c_int32)), _dp(out.view(np.float64)))
+        assert rc == 0
         return out
 
     def plane_metric(self, coef, metric="energy"):

@@ -663,3 +663,24 @@ def test_instantaneous_frequency_vs_numpy_unwrap():
         d = (F[p.row_slice(k)] - want) * T / r.M           # in turns
         assert np.max(np.abs(d - np.round(d))) <= 1e-9
         assert np.mean(np.round(d) != 0) < 0.01            # only exact branch-cut cases may differ by a turn
+
+
+def test_gathered_optimal_plane_carries_exactly_the_winning_plane():
+    """the composite output of the optimal-selection mode (:329): its energy equals the winning plane's metric,
+    its leading C_p entries are that plane's rows in layout order, the padding is zero; a different choice per
+    segment gives different rows (selection is per signal)."""
+    p = RefPlan(1024.0, 1024, [4.0, 8.0, 16.0], 16.0, 400.0, 12)
+    x = inputs.white_noise(p.N, 83, batch=3)
+    Y = p.forward(x, engine=0)
+    vals, _ = p.plane_metric(Y, "energy")
+    best = np.array([2, 0, 1], dtype=np.int32)
+    out = p.gather_plane(Y, best)
+    sizes = p.plane_sizes()
+    assert out.shape == (3, sizes.max())
+    for b in range(3):
+        q = best[b]
+        assert abs(np.sum(np.abs(out[b]) ** 2) - vals[b, q]) <= 1e-12 * vals[b, q]
+        rows = [k for k, r in enumerate(p.rows) if r.plane == q]
+        first = p.rows[rows[0]].offset
+        assert np.array_equal(out[b, :sizes[q]], Y[b, first:first + sizes[q]])
+        assert np.all(out[b, sizes[q]:] == 0)
