@@ -163,6 +163,14 @@ qtam_status qtam_plane_metric(qtam_plan *p, const void *d_coef, int batch, int m
 qtam_status qtam_forward_threshold(qtam_plan *p, const void *d_x, int batch, double kappa, void *d_coef,
                                    void *stream);
 
+/* Optimal-selection output ("a composite output tensor constructed from the optimal planes"):
+ * d_out[b][0 .. C_q) = the coefficients of plane q = d_best[b] of segment b (its rows in layout order), zero up
+ * to qtam_max_plane_coeffs(p), the row length of d_out ([batch][max plane size] complex, device, caller-owned).
+ * d_best: [batch] int32 on the device, e.g. from qtam_plane_metric; out-of-range entries are clamped. */
+int64_t     qtam_max_plane_coeffs(const qtam_plan *p);
+qtam_status qtam_gather_plane(qtam_plan *p, const void *d_coef, int batch, const int32_t *d_best, void *d_out,
+                              void *stream);
+
 /* Number of kernel launches the last forward / inverse / threshold / dense call on this plan issued
  * (host counter, for bench.py's gpu_launches). */
 int         qtam_last_launch_count(const qtam_plan *p);

@@ -18,7 +18,7 @@ STATUS = {0: "ok", 1: "invalid argument", 2: "unsupported", 3: "alloc", 4: "cuda
 
 SYMBOLS = ["qtam_plan_create", "qtam_plan_create_host", "qtam_plan_destroy", "qtam_plan_info",
            "qtam_plan_rows", "qtam_plan_window", "qtam_plan_frame", "qtam_forward", "qtam_inverse",
-           "qtam_dense", "qtam_threshold_rowmedian", "qtam_forward_threshold", "qtam_plane_metric", "qtam_remodulate", "qtam_instantaneous_frequency", "qtam_last_launch_count", "qtam_status_string",
+           "qtam_dense", "qtam_threshold_rowmedian", "qtam_forward_threshold", "qtam_plane_metric", "qtam_gather_plane", "qtam_max_plane_coeffs", "qtam_remodulate", "qtam_instantaneous_frequency", "qtam_last_launch_count", "qtam_status_string",
            "qtam_profile_enable", "qtam_profile_read"]
 
 
@@ -82,6 +82,9 @@ def lib():
         L.qtam_forward_threshold.argtypes = [vp, vp, C.c_int, C.c_double, vp, vp]
         L.qtam_plane_metric.argtypes = [vp, vp, C.c_int, C.c_int, vp, vp, vp]
         L.qtam_remodulate.argtypes = [vp, vp, C.c_int, vp, vp]
+        L.qtam_gather_plane.argtypes = [vp, vp, C.c_int, vp, vp, vp]
+        L.qtam_max_plane_coeffs.argtypes = [vp]
+        L.qtam_max_plane_coeffs.restype = C.c_int64
         L.qtam_instantaneous_frequency.argtypes = [vp, vp, C.c_int, vp, vp]
         L.qtam_last_launch_count.argtypes = [vp]
         L.qtam_last_launch_count.restype = C.c_int
@@ -244,6 +247,17 @@ class Plan:
         out = t.empty((batch, self.ctot), dtype=self._rdt(), device=coef.device)
         _check(lib().qtam_instantaneous_frequency(self._h, coef.data_ptr(), batch, out.data_ptr(), self._stream()),
                "qtam_instantaneous_frequency")
+        return out
+
+    def gather_plane(self, coef, best):
+        """[batch][max plane size]: plane best[b] of every segment, zero padded (optimal-selection mode)"""
+        t = self._torch()
+        assert coef.is_cuda and coef.dtype == self._cdt() and coef.is_contiguous()
+        assert best.is_cuda and best.dtype == t.int32 and best.is_contiguous()
+        batch = coef.numel() // self.ctot
+        out = t.empty((batch, int(lib().qtam_max_plane_coeffs(self._h))), dtype=self._cdt(), device=coef.device)
+        _check(lib().qtam_gather_plane(self._h, coef.data_ptr(), batch, best.data_ptr(), out.data_ptr(), self._stream()),
+               "qtam_gather_plane")
         return out
 
     def plane_metric(self, coef, metric="energy"):

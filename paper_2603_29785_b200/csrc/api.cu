@@ -253,6 +253,7 @@ template <typename T> qtam_status build_device(qtam_plan *p) {
     std::vector<long long> po(size_t(hp.nP) + 1, hp.ctot);
     for (size_t k = hp.rows.size(); k-- > 0;) po[size_t(hp.rows[k].plane)] = hp.rows[k].offset;
     if (!upload(&p->d_plane_off, po.data(), po.size(), tot)) return QTAM_ERR_ALLOC;
+    for (int q = 0; q < hp.nP; ++q) p->max_plane_coeffs = std::max(p->max_plane_coeffs, po[size_t(q) + 1] - po[size_t(q)]);
   }
   if (!upload(&p->d_csr_ptr, hp.csr_ptr.data(), hp.csr_ptr.size(), tot)) return QTAM_ERR_ALLOC;
   if (!upload(&p->d_csr_idx, hp.csr_idx.data(), hp.csr_idx.size(), tot)) return QTAM_ERR_ALLOC;
@@ -535,6 +536,22 @@ qtam_status qtam_instantaneous_frequency(qtam_plan *p, const void *d_coef, int b
   return instantaneous_frequency(p, d_coef, batch, d_out, static_cast<cudaStream_t>(stream));
 }
 
+qtam_status qtam_gather_plane(qtam_plan *p, const void *d_coef, int batch, const int32_t *d_best, void *d_out,
+                              void *stream) {
+  if (p && p->host_only) return QTAM_ERR_CUDA;
+  if (!check_call(p, d_coef, d_out, batch) || !d_best) return QTAM_ERR_INVALID_ARG;
+  p->last_launches = 0;
+  if (batch == 0) return QTAM_OK;
+  return gather_plane(p, d_coef, batch, d_best, d_out, static_cast<cudaStream_t>(stream));
+}
+
+int64_t qtam_max_plane_coeffs(const qtam_plan *p) {
+  if (!p) return 0;
+  std::vector<int64_t> size(size_t(p->hp.nP), 0);
+  for (const HostRow &h : p->hp.rows) size[size_t(h.plane)] += h.M;
+  return *std::max_element(size.begin(), size.end());
+}
+
 qtam_status qtam_plane_metric(qtam_plan *p, const void *d_coef, int batch, int metric, void *d_metric,
                               int32_t *d_best, void *stream) {
   if (p && p->host_only) return QTAM_ERR_CUDA;
@@ -550,7 +567,7 @@ static const char *const kKernelNames[K_COUNT] = {
     "cfft_seq", "cfft_cols", "cfft_rows", "r2c_post", "c2r_pre", "fwd_rows", "fwd_combine",
     "inv_rows", "inv_reduce", "dense_place", "threshold", "r2c_fast", "fwd_rows_fast", "inv_rows_fast",
     "reduce_c2r_fast", "inv_fused", "inv_tiles", "combine_c2r", "threshold_fast", "rows_cta_fwd", "rows_cta_inv",
-    "tiny_rows_fwd", "tiny_rows_inv", "long_fft_a", "long_fft_b", "plane_metric", "best_plane", "remodulate", "inst_freq", "fwd_rows_thr"};
+    "tiny_rows_fwd", "tiny_rows_inv", "long_fft_a", "long_fft_b", "plane_metric", "best_plane", "remodulate", "inst_freq", "fwd_rows_thr", "gather_plane"};
 
 qtam_status qtam_profile_enable(qtam_plan *p, int on, int max_launches) {
   if (!p || p->host_only) return QTAM_ERR_INVALID_ARG;

@@ -13,7 +13,7 @@ enum KernelId {
   K_CFFT_SEQ = 0, K_CFFT_COLS, K_CFFT_ROWS, K_R2C_POST, K_C2R_PRE, K_FWD_ROWS, K_FWD_COMBINE,
   K_INV_ROWS, K_INV_REDUCE, K_DENSE_PLACE, K_THRESHOLD, K_R2C_FAST, K_FWD_ROWS_FAST, K_INV_ROWS_FAST,
   K_REDUCE_C2R_FAST, K_INV_FUSED, K_INV_TILES, K_COMBINE_C2R, K_THRESHOLD_FAST, K_ROWS_CTA_FWD, K_ROWS_CTA_INV,
-  K_TINY_FWD, K_TINY_INV, K_LONG_A, K_LONG_B, K_PLANE_METRIC, K_BEST_PLANE, K_REMODULATE, K_INST_FREQ, K_FWD_ROWS_THR, K_COUNT
+  K_TINY_FWD, K_TINY_INV, K_LONG_A, K_LONG_B, K_PLANE_METRIC, K_BEST_PLANE, K_REMODULATE, K_INST_FREQ, K_FWD_ROWS_THR, K_GATHER_PLANE, K_COUNT
 };
 // fast float path (fast.cu): rows with 32 <= M <= 1024, grouped by G = M/32 lanes per row
 struct FastRow { int kc, dk, woff, goff, offset, plane, wpad, pad; };   // wpad: offset into the padded window table
@@ -55,6 +55,7 @@ struct qtam_plan {
   void *d_invP = nullptr;      // real[(nP+1)*nb], 0 outside the cover set
   int32_t *d_csr_ptr = nullptr;
   int32_t *d_csr_idx = nullptr;
+  long long max_plane_coeffs = 0;     // largest plane (coefficients), the row length of qtam_gather_plane's output
   long long *d_plane_off = nullptr;   // [nP+1] first coefficient of every plane (planes are contiguous)
   // joint-inverse CSR without the band slots of follower rows (rows_cta.cu adds a set of identical rows
   // into its leader's slot); one set per bin.  Null when the plan has no followers.
@@ -184,6 +185,8 @@ qtam_status fast_cfft_long(qtam_plan *p, const void *in, long long in_stride, vo
                            cudaStream_t st);
 // scan.cu
 qtam_status plane_metric(qtam_plan *p, const void *d_coef, int batch, int metric, void *d_metric, int32_t *d_best,
+                         cudaStream_t st);
+qtam_status gather_plane(qtam_plan *p, const void *d_coef, int batch, const int32_t *d_best, void *d_out,
                          cudaStream_t st);
 qtam_status remodulate(qtam_plan *p, const void *d_coef, int batch, void *d_out, cudaStream_t st);
 qtam_status instantaneous_frequency(qtam_plan *p, const void *d_coef, int batch, void *d_out, cudaStream_t st);

@@ -3,6 +3,8 @@
 // The coefficients of a plane are contiguous in the ABI layout (rows are plane-major), so the metric is one
 // streaming reduction per (plane, segment): one CTA each, 128-bit loads, per-thread partial results in the
 // plan's dtype, then a fixed shuffle / shared-memory tree in double (same result on every run, no atomics).
+#include <algorithm>
+
 #include "cplx.cuh"
 #include "device_plan.hpp"
 
@@ -133,6 +135,41 @@ qtam_status remodulate(qtam_plan *p, const void *d_coef, int batch, void *d_out,
     else
       k_remodulate<double><<<g, 128, 0, st>>>(p->d_rows, static_cast<const double2 *>(d_coef), p->hp.ctot,
                                              (int)p->hp.N, static_cast<double2 *>(d_out));
+  }
+  QTAM_LAUNCH_CHECK();
+  return QTAM_OK;
+}
+
+// the composite output of the optimal-selection mode (:329): plane best[seg] of every segment, copied to the
+// start of out[seg][cmax] and zero padded (planes differ in size in the ragged layout).  16-byte copies.
+template <typename T>
+__global__ void __launch_bounds__(256)
+k_gather_plane(const C2<T> *__restrict__ coef, long long ctot, const long long *__restrict__ plane_off, int nP,
+               const int32_t *__restrict__ best, long long cmax, C2<T> *__restrict__ out) {
+  typedef typename Vec4<T>::type V4;
+  const int seg = blockIdx.y;
+  int q = best[seg];
+  q = q < 0 ? 0 : (q >= nP ? nP - 1 : q);
+  const long long lo = plane_off[q], n2 = (plane_off[q + 1] - lo) / 2, c2 = cmax / 2;
+  const V4 *src = reinterpret_cast<const V4 *>(coef + (size_t)seg * ctot + lo);
+  V4 *dst = reinterpret_cast<V4 *>(out + (size_t)seg * cmax);
+  V4 zero; zero.x = zero.y = zero.z = zero.w = 0;
+  for (long long i = (long long)blockIdx.x * 256 + threadIdx.x; i < c2; i += (long long)gridDim.x * 256)
+    dst[i] = i < n2 ? src[i] : zero;
+}
+
+qtam_status gather_plane(qtam_plan *p, const void *d_coef, int batch, const int32_t *d_best, void *d_out,
+                         cudaStream_t st) {
+  const long long cmax = p->max_plane_coeffs;
+  dim3 g((unsigned)std::min<long long>((cmax / 2 + 255) / 256, 64), batch);
+  {
+    LaunchScope ls(p, st, K_GATHER_PLANE, 4.0 * p->esz * (double)batch * (double)cmax);
+    if (p->esz == 4)
+      k_gather_plane<float><<<g, 256, 0, st>>>(static_cast<const float2 *>(d_coef), p->hp.ctot, p->d_plane_off, p->hp.nP,
+                                              d_best, cmax, static_cast<float2 *>(d_out));
+    else
+      k_gather_plane<double><<<g, 256, 0, st>>>(static_cast<const double2 *>(d_coef), p->hp.ctot, p->d_plane_off,
+                                               p->hp.nP, d_best, cmax, static_cast<double2 *>(d_out));
   }
   QTAM_LAUNCH_CHECK();
   return QTAM_OK;

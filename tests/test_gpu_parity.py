@@ -578,3 +578,18 @@ def test_random_plan_shapes(case):
     two = g.threshold_rowmedian(g.forward(dev(x)), 2.5)
     one = g.forward_threshold(dev(x), 2.5)
     assert torch.equal(torch.view_as_real(one), torch.view_as_real(two))
+
+
+@pytest.mark.parametrize("name,dtype", [("cfg3", "f32"), ("cfg5", "f64")])
+def test_gather_of_the_optimal_plane(name, dtype):
+    nseg = 5
+    g, r = make_plans(inputs.plan_args(name), dtype, nseg)
+    x = inputs.make_batch(name, batch=nseg).astype(np_rdt(dtype))
+    Y = g.forward(dev(x))
+    _, best = g.plane_metric(Y, "peak")
+    out = g.gather_plane(Y, best).cpu().numpy()
+    want = r.gather_plane(Y.cpu().numpy().astype(np.complex128), best.cpu().numpy())
+    assert out.shape == want.shape and np.array_equal(out.astype(np.complex128), want)     # a copy: bit exact
+    forced = torch.tensor([i % g.n_planes for i in range(nseg)], dtype=torch.int32, device="cuda")
+    out2 = g.gather_plane(Y, forced).cpu().numpy()
+    assert np.array_equal(out2.astype(np.complex128), r.gather_plane(Y.cpu().numpy().astype(np.complex128), forced.cpu().numpy()))
