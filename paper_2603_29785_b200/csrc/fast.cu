@@ -1,13 +1,17 @@
 // fast.cu -- the tuned float path of libqtam for sm_100a.
 //   K1 k_r2c_fast      a1      one CTA per segment: long real FFT in shared memory (ctafft.cuh), spectrum
-//                              to the plan's L2-resident spectrum buffer
-//   K2 k_fwd_rows_fast a2+a3   one launch for every row with 32 <= M <= 1024: window gather + baseband
-//                              shift + short inverse FFT with the warp-level engine of rowfft.cuh
-//                              (G = M/32 lanes per row, 32 points per lane in registers)
-//   K3 k_inv_rows_fast a5      per-row forward FFT, sqrt(N/M), window; band values to the band workspace
+//                              to the plan's L2-resident spectrum buffer (N = 2^12 .. 2^15)
+//   K2 k_rows_fast<.,true>  a2+a3 [+a4]  one launch, one wave of CTAs, for every row with M <= 1024: window
+//                              gather + baseband shift + short inverse FFT with the warp-level engine of
+//                              rowfft.cuh (G = M/32 lanes per row, 32 points per lane in registers); one
+//                              transform per set of identical rows (same centre bin and half-width), stored
+//                              to every member; rows shorter than 32 points ride along, one thread each
+//                              (tinyrow.cuh); THRESH: the row-median threshold in the epilogue (thrselect.cuh)
+//   K3 k_rows_fast<.,false> a5 per-row forward FFT, sqrt(N/M), window; band values to the band workspace
+//                              (plans whose inverse does not run in inv_tiled.cu)
 //   K4 k_reduce_c2r_fast a6-a8 one CTA per segment: segmented reduction over bins (fixed order, no
 //                              atomics), 1/P, Hermitian pre-processing and the long inverse FFT in smem
-// Rows outside 32..1024 points, double precision and N outside 2^12..2^15 run in generic.cu.
+// Rows of 2^11 .. 2^17 points run in rows_cta.cu, N = 2^16 .. 2^20 in long_fft.cu, double precision in generic.cu.
 #include <cstdlib>
 #include <type_traits>
 

@@ -1,6 +1,8 @@
 // inv_tiled.cu -- the float inverse (rows a5-a8) as two kernels with no band workspace and no atomics.
 //
-//   K1 k_inv_tiles   a5 + a6   persistent warps.  A work item = (segment, tile); a tile = a run of rows
+//   K1 k_inv_tiles   a5 + a6   persistent warps.  A work item = (segment, tile); a tile = a run of leaders
+//                              (one per set of identical rows: their coefficient rows are added before the
+//                              one transform)
 //                              of one length bucket, consecutive in centre bin, whose bands fit a
 //                              warp-private accumulator of kAccBins bins in shared memory.  The warp takes
 //                              the tile's rows pass by pass (32/G rows of M = 32 G points per pass):
@@ -11,8 +13,8 @@
 //                              a fixed summation order: no atomics on data, no block barrier.  The
 //                              finished partial sum (<= kAccBins bins) goes to the partial buffer.
 //   K2 k_combine_c2r a6-a8     one CTA per segment: S[f] = sum of the tiles' partial sums in tile order
-//                              (thread t owns the bins f = t mod NT), rows shorter than 32 points by
-//                              direct summation, Xhat = S/P on the cover set (C50, R9), Hermitian
+//                              (thread t owns the bins f = t mod NT), rows shorter than 32 points one per
+//                              thread (tinyrow.cuh), Xhat = S/P on the cover set (C50, R9), Hermitian
 //                              pre-processing and the long inverse FFT in shared memory (ctafft.cuh).
 // HBM traffic = coefficients in, time series out; the partial sums (about ΣL/3 values per segment) are
 // written and read back once and are meant to stay in L2.
