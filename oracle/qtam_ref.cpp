@@ -46,6 +46,7 @@ struct Row {
 }  // namespace
 
 struct qtam_ref_plan {
+  double epsilon = 0.0;   // Eq. 12: unnormalised stop-band value of the dense windows
   double fs;
   int64_t N, nb;   // nb = N/2+1 one-sided bins
   int nP, nR;      // planes, rows per plane
@@ -249,7 +250,7 @@ int qtam_ref_plan_create(qtam_ref_plan **out, double fs, int64_t N, const double
   if (!out || !Q || nQ < 1 || !(fs > 0) || !is_pow2(N) || N < 8) return 1;
   qtam_ref_options o;
   o.window = 0; o.clamp_mode = 1; o.clamp_overlap = 1.0; o.max_window_bins = 0;
-  o.cover_floor = 1e-2; o.rows_are_bins_per_octave = 0; o.window_param = 0.0; o.freqs = nullptr; o.n_freqs = 0; o.tile_length = 0;
+  o.cover_floor = 1e-2; o.rows_are_bins_per_octave = 0; o.window_param = 0.0; o.freqs = nullptr; o.n_freqs = 0; o.tile_length = 0; o.epsilon = 0.0;
   if (opt) o = *opt;
   const bool manual = o.freqs != nullptr && o.n_freqs >= 2;
   if (manual) { fmin = o.freqs[0]; fmax = o.freqs[o.n_freqs - 1]; }
@@ -257,6 +258,7 @@ int qtam_ref_plan_create(qtam_ref_plan **out, double fs, int64_t N, const double
   if (o.window < 0 || o.window > 4) return 2;
   if (o.window == 2 && !(o.window_param > 0)) return 1;
   if (o.window >= 3 && !(o.window_param > 0 && o.window_param <= 1.0)) return 1;
+  if (!(o.epsilon >= 0.0)) return 1;
   if (!(o.clamp_overlap > 0)) o.clamp_overlap = 1.0;
   if (!(o.cover_floor > 0)) o.cover_floor = 1e-2;
 
@@ -312,7 +314,7 @@ int qtam_ref_plan_create(qtam_ref_plan **out, double fs, int64_t N, const double
 
   qtam_ref_plan *p = new (std::nothrow) qtam_ref_plan;
   if (!p) return 3;
-  p->fs = fs; p->N = N; p->nb = N / 2 + 1; p->nP = nQ; p->nR = R;
+  p->fs = fs; p->N = N; p->nb = N / 2 + 1; p->nP = nQ; p->nR = R; p->epsilon = o.epsilon;
   p->Q.assign(Q, Q + nQ);
   int64_t offset = 0, sumL = 0;
   for (int pl = 0; pl < nQ; ++pl) {
@@ -473,6 +475,16 @@ int qtam_ref_forward(const qtam_ref_plan *p, const double *x, int batch, double 
   return 0;
 }
 
+// Eq. 12 as read in R17: the dense window of row r at bin f is norm * max(W'[f - kc], epsilon)
+// on the support and norm * epsilon off it (the floor also lifts the window's exact zeros at |j| = dk, which
+// Eq. 12 as printed would leave non-invertible).  epsilon = 0: the plain window, zero off the support.
+static inline double dense_window(const qtam_ref_plan *p, const Row &r, int64_t f) {
+  const int64_t j = f - r.kc;
+  if (j < -r.dk || j > r.dk) return p->epsilon * r.norm;
+  if (p->epsilon > 0) return std::max(r.wraw[(size_t)(j + r.dk)], p->epsilon) * r.norm;
+  return r.w[(size_t)(j + r.dk)];
+}
+
 // T_k[tau] = (1/N) sum_j X[kc+j] W_k[j] e^{+2 pi i (kc+j) tau/N}, tau = 0..N-1 (C3)
 int qtam_ref_dense(const qtam_ref_plan *p, const double *x, int batch, int row_begin, int row_end,
                    double *out, int engine) {
@@ -482,6 +494,7 @@ int qtam_ref_dense(const qtam_ref_plan *p, const double *x, int batch, int row_b
   const int64_t N = p->N;
   const int nr = row_end - row_begin;
   std::vector<uint8_t> need = needed_bins(p, row_begin, row_end);
+  if (p->epsilon > 0) std::fill(need.begin(), need.end(), (uint8_t)1);
   for (int b = 0; b < batch; ++b) {
     std::vector<cd> X((size_t)p->nb);
     spectrum_onesided(x + (size_t)b * N, N, X.data(), need.data(), engine);
@@ -494,10 +507,15 @@ int qtam_ref_dense(const qtam_ref_plan *p, const double *x, int batch, int row_b
         for (int64_t m = 0; m < N; ++m) tw[(size_t)m] = cis(m, N);
         for (int64_t tau = 0; tau < N; ++tau) {
           cld acc(0, 0);
-          for (int64_t j = -r.dk; j <= r.dk; ++j) {
-            int64_t f = r.kc + j;
-            if (f < 0 || f >= p->nb) continue;
-            acc += cld(X[(size_t)f]) * (ld)r.w[(size_t)(j + r.dk)] * tw[(size_t)((f * tau) % N)];
+          if (p->epsilon > 0) {             // Eq. 12: every one-sided bin takes part
+            for (int64_t f = 0; f < p->nb; ++f)
+              acc += cld(X[(size_t)f]) * (ld)dense_window(p, r, f) * tw[(size_t)((f * tau) % N)];
+          } else {
+            for (int64_t j = -r.dk; j <= r.dk; ++j) {
+              int64_t f = r.kc + j;
+              if (f < 0 || f >= p->nb) continue;
+              acc += cld(X[(size_t)f]) * (ld)r.w[(size_t)(j + r.dk)] * tw[(size_t)((f * tau) % N)];
+            }
           }
           acc /= (ld)N;
           Tk[tau] = cd((double)acc.real(), (double)acc.imag());
@@ -509,6 +527,8 @@ int qtam_ref_dense(const qtam_ref_plan *p, const double *x, int batch, int row_b
           if (f < 0 || f >= p->nb) continue;
           a[(size_t)f] = X[(size_t)f] * r.w[(size_t)(j + r.dk)];
         }
+        if (p->epsilon > 0)
+          for (int64_t f = 0; f < p->nb; ++f) a[(size_t)f] = X[(size_t)f] * dense_window(p, r, f);
         fft_radix2(a.data(), o.data(), N, +1);
         for (int64_t tau = 0; tau < N; ++tau) Tk[tau] = o[(size_t)tau] / (double)N;
       }
@@ -651,6 +671,33 @@ int qtam_ref_threshold_rowmedian_f32(const qtam_ref_plan *p, float *coef, int ba
       for (int64_t n = 0; n < r.M; ++n)
         if (mag[(size_t)n] < t) { Y[2 * n] = 0.0f; Y[2 * n + 1] = 0.0f; }
     }
+  return 0;
+}
+
+// Eq. 13: x = F^{-1}{ T~_k[f] / W~_k[f] } from ONE dense tile, with the window of Eq. 12
+// (epsilon off the support).  T~_k[f] = sum_tau T_k[tau] e^{-2 pi i f tau/N} = X[f] W_k[f] for f = 0..N/2 (C33
+// :523); the real series comes back through the one-sided inverse DFT of C2 (:371).  Naive sums throughout.
+int qtam_ref_dense_invert(const qtam_ref_plan *p, const double *tile, int batch, int row, double *x_out) {
+  if (!p || !tile || !x_out || batch < 0 || row < 0 || row >= (int)p->rows.size()) return 1;
+  if (!(p->epsilon > 0)) return 2;
+  const int64_t N = p->N;
+  const Row &r = p->rows[(size_t)row];
+  std::vector<cld> tw((size_t)N);
+  for (int64_t m = 0; m < N; ++m) tw[(size_t)m] = cis(m, N);
+  for (int b = 0; b < batch; ++b) {
+    const cd *Tk = reinterpret_cast<const cd *>(tile) + (size_t)b * N;
+    std::vector<cld> Xh((size_t)p->nb);
+    for (int64_t f = 0; f < p->nb; ++f) {
+      cld acc(0, 0);
+      for (int64_t tau = 0; tau < N; ++tau) acc += cld(Tk[tau]) * std::conj(tw[(size_t)((f * tau) % N)]);
+      Xh[(size_t)f] = acc / (ld)dense_window(p, r, f);
+    }
+    for (int64_t n = 0; n < N; ++n) {
+      ld acc = Xh[0].real() + ((n & 1) ? -1.0L : 1.0L) * Xh[(size_t)(N / 2)].real();
+      for (int64_t f = 1; f < N / 2; ++f) acc += 2.0L * (Xh[(size_t)f] * tw[(size_t)((f * n) % N)]).real();
+      x_out[(size_t)b * N + n] = (double)(acc / (ld)N);
+    }
+  }
   return 0;
 }
 

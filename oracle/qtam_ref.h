@@ -47,6 +47,8 @@ typedef struct {
   int64_t tile_length;              /* output length per row: 0 = nextpow2(L_k) per row (R5, default);
                                        -1 = uniform, nextpow2 of the largest window (the paper's padded
                                        layout :127-129); n > 0 = uniform user-set n, a power of two >= max L */
+  double  epsilon;                  /* Eq. 12 (:143): unnormalised window value outside the support, used by
+                                       the dense tiles and their single-tile inversion only; 0 = none       */
 } qtam_ref_options;
 
 typedef struct {
@@ -91,6 +93,12 @@ int  qtam_ref_brute_tile(const qtam_ref_plan *p, const double *x, int row, doubl
  * stated in DESIGN.md ("threshold arithmetic") so that a float kernel can match it bit for bit. */
 int  qtam_ref_threshold_rowmedian(const qtam_ref_plan *p, double *coef, int batch, double kappa);
 int  qtam_ref_threshold_rowmedian_f32(const qtam_ref_plan *p, float *coef, int batch, float kappa);
+
+/* Single-tile inversion by spectral division (Eq. 13 :148), demodulation bypassed: tile = ONE dense tile T_k
+ * of every segment ([batch][N] complex, as qtam_ref_dense writes it with epsilon > 0);
+ * x = F^{-1}{ F[T_k][f] / W_k[f] }, W_k[f] = norm_k * (window on the support, epsilon elsewhere), f = 0..N/2.
+ * Returns nonzero when the plan's epsilon is 0 (the division is undefined off the support). */
+int  qtam_ref_dense_invert(const qtam_ref_plan *p, const double *tile, int batch, int row, double *x_out);
 
 /* Re-modulation (Eq. 10a :113-117, :129): out[b][offset_k + n] = sqrt(M_k/N) e^{+2 pi i kc n/M_k} Y_k[n]
  * = the dense tile T_k at tau = n N/M_k (identity P2).  Same layout as the coefficients. */

@@ -21,7 +21,7 @@ class Options(C.Structure):
     _fields_ = [("window", C.c_int), ("clamp_mode", C.c_int), ("clamp_overlap", C.c_double),
                 ("max_window_bins", C.c_int64), ("cover_floor", C.c_double),
                 ("rows_are_bins_per_octave", C.c_int), ("window_param", C.c_double),
-                ("freqs", C.POINTER(C.c_double)), ("n_freqs", C.c_int), ("tile_length", C.c_int64)]
+                ("freqs", C.POINTER(C.c_double)), ("n_freqs", C.c_int), ("tile_length", C.c_int64), ("epsilon", C.c_double)]
 
 
 WINDOWS = {"bisquare": 0, "hann": 1, "kaiser": 2, "tukey": 3, "planck": 4}
@@ -62,6 +62,7 @@ def lib():
         _lib.qtam_ref_remodulate.argtypes = [vp, dp, C.c_int, dp]
         _lib.qtam_ref_instantaneous_frequency.argtypes = [vp, dp, C.c_int, dp]
         _lib.qtam_ref_gather_plane.argtypes = [vp, dp, C.c_int, C.POINTER(C.c_int32), dp]
+        _lib.qtam_ref_dense_invert.argtypes = [vp, dp, C.c_int, C.c_int, dp]
         _lib.qtam_ref_plane_metric.argtypes = [vp, dp, C.c_int, C.c_int, dp, C.POINTER(C.c_int32)]
         _lib.qtam_ref_project_cover.argtypes = [vp, dp, C.c_int, C.c_int, dp, C.c_int]
         _lib.qtam_ref_spectrum.argtypes = [vp, dp, C.c_int, dp, C.c_int]
@@ -107,7 +108,7 @@ class RefPlan:
 
     def __init__(self, fs, N, Q, fmin, fmax, spacing, clamp_mode=1, clamp_overlap=1.0,
                  max_window_bins=0, cover_floor=1e-2, rows_are_bins_per_octave=0,
-                 window="bisquare", window_param=0.0, freqs=None, tile_length=0):
+                 window="bisquare", window_param=0.0, freqs=None, tile_length=0, epsilon=0.0):
         L = lib()
         self._h = C.c_void_p()
         q = np.ascontiguousarray(Q, dtype=np.float64)
@@ -115,7 +116,7 @@ class RefPlan:
         opt = Options(WINDOWS[window], clamp_mode, clamp_overlap, max_window_bins, cover_floor,
                       rows_are_bins_per_octave, float(window_param),
                       None if fr is None else fr.ctypes.data_as(C.POINTER(C.c_double)),
-                      0 if fr is None else fr.size, int(tile_length))
+                      0 if fr is None else fr.size, int(tile_length), float(epsilon))
         rc = L.qtam_ref_plan_create(C.byref(self._h), float(fs), int(N), _dp(q), q.size,
                                     float(fmin), float(fmax), float(spacing), C.byref(opt))
         if rc != 0:
@@ -222,6 +223,15 @@ class RefPlan:
         rc = lib().qtam_ref_gather_plane(self._h, _dp(c.view(np.float64)), c.shape[0],
                                          b.ctypes.data_as(C.POINTER(C.c_int32)), _dp(out.view(np.float64)))
         assert rc == 0
+        return out
+
+    def dense_invert(self, tile, row):
+        """x[batch][N] from ONE dense tile per segment (Eq. 13); the plan needs epsilon > 0"""
+        c = np.ascontiguousarray(np.atleast_2d(tile), dtype=np.complex128)
+        out = np.empty((c.shape[0], self.N), dtype=np.float64)
+        rc = lib().qtam_ref_dense_invert(self._h, _dp(c.view(np.float64)), c.shape[0], int(row), _dp(out))
+        if rc != 0:
+            raise ValueError(f"qtam_ref_dense_invert failed with code {rc}")
         return out
 
     def plane_metric(self, coef, metric="energy"):

@@ -684,3 +684,34 @@ def test_gathered_optimal_plane_carries_exactly_the_winning_plane():
         first = p.rows[rows[0]].offset
         assert np.array_equal(out[b, :sizes[q]], Y[b, first:first + sizes[q]])
         assert np.all(out[b, sizes[q]:] == 0)
+
+
+# ---- epsilon-regularised windows and single-tile inversion (Eq. 12-13) -------------
+
+def test_single_tile_inversion_recovers_the_signal():
+    """Eq. 13: with the window floored at epsilon (Eq. 12, reading R17) ONE dense tile determines the whole
+    signal: x = F^{-1}{F[T_k]/W_k}.  Checked for a low, a middle and a high row, and against the same
+    construction through numpy's fft / irfft (library routines)."""
+    args = (256.0, 256, [4.0, 8.0], 8.0, 100.0, 7)
+    eps = 1e-4
+    p = RefPlan(*args, epsilon=eps)
+    p0 = RefPlan(*args)
+    x = inputs.white_noise(p.N, 97, batch=2)
+    for k in (0, p.n_rows // 2, p.n_rows - 1):
+        T = p.dense(x, engine=0, row_begin=k, row_end=k + 1)[:, 0, :]
+        assert rel_l2(p.dense_invert(T, k), x) <= 1e-10          # conditioning 1/eps on the stop band
+        # the tile differs from the plain one only by the epsilon-weighted rest of the spectrum
+        T0 = p0.dense(x, engine=0, row_begin=k, row_end=k + 1)[:, 0, :]
+        assert 0 < rel_l2(T, T0) < 50 * eps
+        r = p.rows[k]
+        W = np.full(p.n_bins, eps * r.norm)
+        w = p0.window(k) / r.norm                                   # unnormalised window values
+        for j in range(-r.dk, r.dk + 1):
+            if 0 <= r.kc + j < p.n_bins:
+                W[r.kc + j] = max(w[j + r.dk], eps) * r.norm
+        Xh = np.fft.fft(T, axis=-1)[:, :p.n_bins] / W[None, :]
+        Xh[:, 0] = Xh[:, 0].real
+        Xh[:, -1] = Xh[:, -1].real
+        assert rel_l2(p.dense_invert(T, k), np.fft.irfft(Xh, n=p.N, axis=-1)) <= 1e-10
+    with pytest.raises(ValueError):
+        p0.dense_invert(np.zeros((1, p0.N), complex), 0)             # epsilon = 0: undefined
