@@ -73,6 +73,9 @@ typedef struct {
                                        -1 = uniform, nextpow2 of the largest window: the paper's
                                        zero-padded layout (:127-129), coefficients = [rows][M] per
                                        segment; n > 0 = uniform, user-set power of two >= max L     */
+  double  epsilon;                  /* Eq. 12 (R17): unnormalised window value
+                                       off the support (and floor on it) for qtam_dense and
+                                       qtam_dense_invert only; 0 = plain windows [default]           */
 } qtam_options;
 
 /* Host-side row table entry; rows are ordered plane-major (Q list order), ascending frequency. */
@@ -129,6 +132,13 @@ qtam_status qtam_inverse(qtam_plan *p, const void *d_coef, int batch, int plane,
  * d_out: [batch][row_end-row_begin][N] complex.                                                   */
 qtam_status qtam_dense(qtam_plan *p, const void *d_x, int batch, int row_begin, int row_end,
                        void *d_out, void *stream);
+
+/* Single-tile inversion by spectral division (Eq. 13; demodulation bypassed): d_tile = ONE dense
+ * tile T_row per segment, [batch][N] complex as qtam_dense writes it on a plan with epsilon > 0;
+ * x = F^{-1}{ F[T_row][f] / W_row[f] } -> d_x_out [batch][N] real.  Conditioning: errors of the tile are
+ * amplified by up to 1/epsilon.  N up to 8192 (float) / 4096 (double): a check path like qtam_dense.
+ * QTAM_ERR_INVALID_ARG when the plan's epsilon is 0. */
+qtam_status qtam_dense_invert(qtam_plan *p, const void *d_tile, int batch, int row, void *d_x_out, void *stream);
 
 /* Row-median threshold in place (BASELINE.json config 5; R11): per (segment,row),
  * m = median_n |Y_k[n]| (two middle values averaged), zero every Y_k[n] with |Y_k[n]| < kappa*m.

@@ -18,7 +18,7 @@ STATUS = {0: "ok", 1: "invalid argument", 2: "unsupported", 3: "alloc", 4: "cuda
 
 SYMBOLS = ["qtam_plan_create", "qtam_plan_create_host", "qtam_plan_destroy", "qtam_plan_info",
            "qtam_plan_rows", "qtam_plan_window", "qtam_plan_frame", "qtam_forward", "qtam_inverse",
-           "qtam_dense", "qtam_threshold_rowmedian", "qtam_forward_threshold", "qtam_plane_metric", "qtam_gather_plane", "qtam_max_plane_coeffs", "qtam_remodulate", "qtam_instantaneous_frequency", "qtam_last_launch_count", "qtam_status_string",
+           "qtam_dense", "qtam_dense_invert", "qtam_threshold_rowmedian", "qtam_forward_threshold", "qtam_plane_metric", "qtam_gather_plane", "qtam_max_plane_coeffs", "qtam_remodulate", "qtam_instantaneous_frequency", "qtam_last_launch_count", "qtam_status_string",
            "qtam_profile_enable", "qtam_profile_read"]
 
 
@@ -33,7 +33,7 @@ class Options(C.Structure):
                 ("clamp_overlap", C.c_double), ("max_window_bins", C.c_int64),
                 ("cover_floor", C.c_double), ("rows_are_bins_per_octave", C.c_int),
                 ("max_batch", C.c_int), ("window_param", C.c_double),
-                ("freqs", C.POINTER(C.c_double)), ("n_freqs", C.c_int), ("tile_length", C.c_int64)]
+                ("freqs", C.POINTER(C.c_double)), ("n_freqs", C.c_int), ("tile_length", C.c_int64), ("epsilon", C.c_double)]
 
 
 WINDOWS = {"bisquare": 0, "hann": 1, "kaiser": 2, "tukey": 3, "planck": 4}
@@ -82,6 +82,7 @@ def lib():
         L.qtam_forward_threshold.argtypes = [vp, vp, C.c_int, C.c_double, vp, vp]
         L.qtam_plane_metric.argtypes = [vp, vp, C.c_int, C.c_int, vp, vp, vp]
         L.qtam_remodulate.argtypes = [vp, vp, C.c_int, vp, vp]
+        L.qtam_dense_invert.argtypes = [vp, vp, C.c_int, C.c_int, vp, vp]
         L.qtam_gather_plane.argtypes = [vp, vp, C.c_int, vp, vp, vp]
         L.qtam_max_plane_coeffs.argtypes = [vp]
         L.qtam_max_plane_coeffs.restype = C.c_int64
@@ -107,7 +108,7 @@ class Plan:
 
     def __init__(self, fs, N, Q, fmin, fmax, spacing, dtype="f32", max_batch=1, clamp_mode=1,
                  clamp_overlap=1.0, max_window_bins=0, cover_floor=1e-2, rows_are_bins_per_octave=0,
-                 host_only=False, window="bisquare", window_param=0.0, freqs=None, tile_length=0):
+                 host_only=False, window="bisquare", window_param=0.0, freqs=None, tile_length=0, epsilon=0.0):
         L = lib()
         self._h = C.c_void_p()
         self.dtype = dtype
@@ -116,7 +117,7 @@ class Plan:
         opt = Options(C.sizeof(Options), WINDOWS[window], clamp_mode, clamp_overlap, max_window_bins,
                       cover_floor, rows_are_bins_per_octave, max_batch, float(window_param),
                       None if fr is None else fr.ctypes.data_as(C.POINTER(C.c_double)),
-                      0 if fr is None else fr.size, int(tile_length))
+                      0 if fr is None else fr.size, int(tile_length), float(epsilon))
         fn = L.qtam_plan_create_host if host_only else L.qtam_plan_create
         code = fn(C.byref(self._h), float(fs), int(N), q.ctypes.data_as(C.POINTER(C.c_double)), q.size,
                   float(fmin), float(fmax), float(spacing), QTAM_F64 if dtype == "f64" else QTAM_F32,
@@ -219,6 +220,16 @@ class Plan:
         assert out.is_cuda and out.dtype == self._cdt() and out.is_contiguous() and out.numel() == batch * self.ctot
         _check(lib().qtam_forward_threshold(self._h, x.data_ptr(), batch, float(kappa), out.data_ptr(), self._stream()),
                "qtam_forward_threshold")
+        return out
+
+    def dense_invert(self, tile, row):
+        """x[batch][N] from one dense tile per segment (Eq. 13); the plan needs epsilon > 0"""
+        t = self._torch()
+        assert tile.is_cuda and tile.dtype == self._cdt() and tile.is_contiguous() and tile.shape[-1] == self.N
+        batch = tile.numel() // self.N
+        out = t.empty((batch, self.N), dtype=self._rdt(), device=tile.device)
+        _check(lib().qtam_dense_invert(self._h, tile.data_ptr(), batch, int(row), out.data_ptr(), self._stream()),
+               "qtam_dense_invert")
         return out
 
     def threshold_rowmedian(self, coef, kappa=3.0):

@@ -509,6 +509,16 @@ qtam_status qtam_dense(qtam_plan *p, const void *d_x, int batch, int row_begin, 
   return generic_dense(p, batch, row_begin, row_end, d_out, st);
 }
 
+qtam_status qtam_dense_invert(qtam_plan *p, const void *d_tile, int batch, int row, void *d_x_out, void *stream) {
+  if (p && p->host_only) return QTAM_ERR_CUDA;
+  if (!check_call(p, d_tile, d_x_out, batch) || row < 0 || row >= (int)p->hp.rows.size() ||
+      !(p->hp.opt.epsilon > 0.0))
+    return QTAM_ERR_INVALID_ARG;
+  p->last_launches = 0;
+  if (batch == 0) return QTAM_OK;
+  return generic_dense_invert(p, d_tile, batch, row, d_x_out, static_cast<cudaStream_t>(stream));
+}
+
 qtam_status qtam_threshold_rowmedian(qtam_plan *p, void *d_coef, int batch, double kappa, void *stream) {
   if (p && p->host_only) return QTAM_ERR_CUDA;
   if (!check_call(p, d_coef, d_coef, batch) || !(kappa >= 0.0)) return QTAM_ERR_INVALID_ARG;

@@ -167,6 +167,7 @@ qtam_status generic_inverse_rows(qtam_plan *p, const void *d_coef, int batch, in
 qtam_status generic_inverse_reduce(qtam_plan *p, int batch, int plane, cudaStream_t st);
 qtam_status generic_c2r(qtam_plan *p, int batch, void *d_x_out, cudaStream_t st);
 qtam_status generic_dense(qtam_plan *p, int batch, int row_begin, int row_end, void *d_out, cudaStream_t st);
+qtam_status generic_dense_invert(qtam_plan *p, const void *d_tile, int batch, int row, void *d_x_out, cudaStream_t st);
 qtam_status generic_threshold(qtam_plan *p, void *d_coef, int batch, double kappa, int min_log2M, cudaStream_t st);
 
 // fast.cu

@@ -311,18 +311,40 @@ __global__ void k_inv_reduce(const C2<T> *__restrict__ band, long long sumL,
 template <typename T>
 __global__ void k_dense_place(const RowDev *__restrict__ rows, int row, const C2<T> *__restrict__ spec,
                               long long xstride, int nbins, const T *__restrict__ win,
-                              C2<T> *__restrict__ ws, int N) {
+                              C2<T> *__restrict__ ws, int N, T eps_norm) {
   typedef C2<T> V;
   const int f = blockIdx.x * blockDim.x + threadIdx.x;
   if (f >= N) return;
   const RowDev r = rows[row];
   const int jj = f - r.kc;
   V v = cmk<T>(0, 0);
+  // eps_norm = epsilon x the row's norm (Eq. 12 :143, R17): the window is floored there on the support and
+  // equals it on the rest of the one-sided spectrum; 0 = the plain window
   if (jj >= -r.dk && jj <= r.dk && f < nbins) {
-    const T w = win[r.woff + jj + r.dk] / (T)N;
-    v = cscale(spec[(long long)blockIdx.y * xstride + f], w);
+    T w = win[r.woff + jj + r.dk];
+    if (w < eps_norm) w = eps_norm;
+    v = cscale(spec[(long long)blockIdx.y * xstride + f], w / (T)N);
+  } else if (eps_norm > (T)0 && f < nbins) {
+    v = cscale(spec[(long long)blockIdx.y * xstride + f], eps_norm / (T)N);
   }
   ws[(long long)blockIdx.y * N + f] = v;
+}
+
+// Eq. 13 (:148): Xhat[f] = F[T_k][f] / W_k[f], f = 0..N/2, with the window of Eq. 12
+template <typename T>
+__global__ void k_dense_divide(const RowDev *__restrict__ rows, int row, const C2<T> *__restrict__ ft, int N,
+                               const T *__restrict__ win, T eps_norm, int nbins, C2<T> *__restrict__ spec,
+                               long long xstride) {
+  const int f = blockIdx.x * blockDim.x + threadIdx.x;
+  if (f >= nbins) return;
+  const RowDev r = rows[row];
+  const int jj = f - r.kc;
+  T w = eps_norm;
+  if (jj >= -r.dk && jj <= r.dk) {
+    w = win[r.woff + jj + r.dk];
+    if (w < eps_norm) w = eps_norm;
+  }
+  spec[(long long)blockIdx.y * xstride + f] = cscale(ft[(long long)blockIdx.y * N + f], (T)1 / w);
 }
 
 // ---------------------------------------------------------------------------------------------------
@@ -594,7 +616,8 @@ static qtam_status dense_t(qtam_plan *p, int batch, int row_begin, int row_end, 
     {
       LaunchScope ls(p, st, K_DENSE_PLACE, sizeof(C2<T>) * (double)batch * (double)N);
       k_dense_place<T><<<g, 256, 0, st>>>(p->d_rows, k, static_cast<const C2<T> *>(p->d_spec), p->xstride,
-                                          (int)p->hp.nb, static_cast<const T *>(p->d_win), ws, N);
+                                          (int)p->hp.nb, static_cast<const T *>(p->d_win), ws, N,
+                                          (T)(p->hp.opt.epsilon * p->hp.rows[(size_t)k].norm));
     }
     QTAM_LAUNCH_CHECK();
     qtam_status s = cfft<T>(p, ws, N, out + (long long)(k - row_begin) * N, (long long)nr * N, ws, N,
@@ -602,6 +625,31 @@ static qtam_status dense_t(qtam_plan *p, int batch, int row_begin, int row_end, 
     if (s != QTAM_OK) return s;
   }
   return QTAM_OK;
+}
+
+template <typename T>
+static qtam_status dense_invert_t(qtam_plan *p, const void *d_tile, int batch, int row, void *d_x_out, cudaStream_t st) {
+  const int N = (int)p->hp.N;
+  // the forward transform of the tile needs no scratch only while it fits one CTA (this is a check path
+  // for small configurations, like qtam_dense)
+  if (ilog2(N) > p->cap_log2) return QTAM_ERR_UNSUPPORTED;
+  C2<T> *ws = static_cast<C2<T> *>(p->d_ws);
+  qtam_status s = cfft<T>(p, static_cast<const C2<T> *>(d_tile), N, ws, N, ws, N, ilog2(N), batch, -1, (T)1, st);
+  if (s != QTAM_OK) return s;
+  dim3 g((unsigned)((p->hp.nb + 255) / 256), batch);
+  {
+    LaunchScope ls(p, st, K_DENSE_PLACE, sizeof(C2<T>) * (double)batch * (double)p->hp.nb * 2.0);
+    k_dense_divide<T><<<g, 256, 0, st>>>(p->d_rows, row, ws, N, static_cast<const T *>(p->d_win),
+                                         (T)(p->hp.opt.epsilon * p->hp.rows[(size_t)row].norm), (int)p->hp.nb,
+                                         static_cast<C2<T> *>(p->d_spec), p->xstride);
+  }
+  QTAM_LAUNCH_CHECK();
+  return c2r_t<T>(p, batch, d_x_out, st);
+}
+
+qtam_status generic_dense_invert(qtam_plan *p, const void *d_tile, int batch, int row, void *d_x_out, cudaStream_t st) {
+  return p->esz == 4 ? dense_invert_t<float>(p, d_tile, batch, row, d_x_out, st)
+                     : dense_invert_t<double>(p, d_tile, batch, row, d_x_out, st);
 }
 
 qtam_status generic_dense(qtam_plan *p, int batch, int row_begin, int row_end, void *d_out, cudaStream_t st) {

@@ -593,3 +593,25 @@ def test_gather_of_the_optimal_plane(name, dtype):
     forced = torch.tensor([i % g.n_planes for i in range(nseg)], dtype=torch.int32, device="cuda")
     out2 = g.gather_plane(Y, forced).cpu().numpy()
     assert np.array_equal(out2.astype(np.complex128), r.gather_plane(Y.cpu().numpy().astype(np.complex128), forced.cpu().numpy()))
+
+
+@pytest.mark.parametrize("dtype,eps,tol", [("f64", 1e-5, 1e-9), ("f32", 1e-2, 2e-4)])
+def test_epsilon_windows_and_single_tile_inversion(dtype, eps, tol):
+    """Eq. 12-13 (:140-148): dense tiles with the epsilon-floored window against the oracle, and the whole signal
+    back from ONE tile by spectral division (errors of the tile are amplified by up to 1/epsilon, hence the
+    tolerances)."""
+    args = (1024.0, 1024, [4.0, 8.0, 16.0], 16.0, 400.0, 12.0)
+    g, r = make_plans(args, dtype, 2, epsilon=eps)
+    x = inputs.white_noise(args[1], 99, batch=2).astype(np_rdt(dtype))
+    x64 = x.astype(np.float64)
+    for k in (1, g.n_rows // 2, g.n_rows - 1):
+        T = g.dense(dev(x), row_begin=k, row_end=k + 1)
+        Tr = r.dense(x64, row_begin=k, row_end=k + 1, engine=1)
+        assert worst_segment(T.cpu().numpy()[:, 0, :], Tr[:, 0, :]) <= TOL[dtype]
+        xg = g.dense_invert(T[:, 0, :].contiguous(), k).cpu().numpy()
+        assert worst_segment(xg, x64) <= tol
+        # against the oracle's inversion of the oracle's tile
+        assert worst_segment(xg, r.dense_invert(Tr[:, 0, :], k)) <= tol
+    g0, _ = make_plans(args, dtype, 2)
+    with pytest.raises(binding.QtamError):
+        g0.dense_invert(torch.zeros((2, args[1]), dtype=torch.complex128 if dtype == "f64" else torch.complex64, device="cuda"), 0)
