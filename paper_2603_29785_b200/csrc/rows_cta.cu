@@ -131,7 +131,7 @@ struct ScratchIn {
 };
 
 template <int L2, bool FORWARD>
-__global__ void __launch_bounds__(CtaFftPlan<L2>::NT)
+__global__ void __launch_bounds__(CtaFftPlan<L2>::NT, (L2 == 13 || L2 == 12) ? 2 : 1)
 k_rows_cta(const int *__restrict__ rowidx, const int *__restrict__ memptr, const int *__restrict__ mem, int nrows,
            const RowDev *__restrict__ rows,
            const float *__restrict__ win, const float2 *__restrict__ spec, long long xstride, int nbins,
