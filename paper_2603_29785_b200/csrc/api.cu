@@ -42,7 +42,8 @@ void free_plan(qtam_plan *p) {
   if (p->host_only) { delete p; return; }
   cudaFree(p->d_rows); cudaFree(p->d_win); cudaFree(p->d_tw); cudaFree(p->d_invP);
   cudaFree(p->d_csr_ptr); cudaFree(p->d_csr_idx); cudaFree(p->d_csrj_ptr); cudaFree(p->d_csrj_idx); cudaFree(p->d_plane_off);
-  for (int c = 0; c < qtam_plan::kClasses; ++c) cudaFree(p->d_items[c]);
+  for (int c = 0; c < qtam_plan::kClasses; ++c) { cudaFree(p->d_items[c]); cudaFree(p->d_items_fwd[c]); }
+  cudaFree(p->d_gfol_ptr); cudaFree(p->d_gfol_off);
   cudaFree(p->d_bigrows); cudaFree(p->d_spec_alloc); cudaFree(p->d_ws); cudaFree(p->d_band);
   cudaFree(p->d_fwinp); cudaFree(p->d_red);
   cudaFree(p->d_frows); cudaFree(p->d_fwin); cudaFree(p->d_ftw_fwd); cudaFree(p->d_ftw_inv);
@@ -259,8 +260,10 @@ template <typename T> qtam_status build_device(qtam_plan *p) {
   if (!upload(&p->d_csr_idx, hp.csr_idx.data(), hp.csr_idx.size(), tot)) return QTAM_ERR_ALLOC;
   // generic-path work lists
   {
-    std::vector<WorkItem> items[qtam_plan::kClasses];
+    std::vector<WorkItem> items[qtam_plan::kClasses], items_fwd[qtam_plan::kClasses];
     std::vector<int> big;
+    std::vector<std::vector<long long>> followers(hp.rows.size());   // per leader row: follower offsets
+    std::vector<int> gen_leaders;                                    // single-transform rows seen so far
     for (size_t k = 0; k < hp.rows.size(); ++k) {
       const int lm = ilog2(hp.rows[k].M);
       if (p->fast_rows && lm <= 10) continue;   // handled by fast.cu (32..1024: warp engine; < 32: one thread per row)
@@ -268,12 +271,24 @@ template <typename T> qtam_status build_device(qtam_plan *p) {
       if (lm <= p->cap_log2) {
         const int c = generic_class_of(lm);
         items[c].push_back(WorkItem{(int)k, 0, 1, lm});
+        {
+          // forward: identical rows (same centre bin and half-width) are transformed once
+          int leader = -1;
+          for (int l : gen_leaders)
+            if (hp.rows[(size_t)l].kc == hp.rows[k].kc && hp.rows[(size_t)l].dk == hp.rows[k].dk &&
+                hp.rows[(size_t)l].M == hp.rows[k].M) { leader = l; break; }
+          if (leader < 0) { gen_leaders.push_back((int)k); items_fwd[c].push_back(WorkItem{(int)k, 0, 1, lm}); }
+          else followers[(size_t)leader].push_back(hp.rows[k].offset);
+        }
         p->class_L[c] += (double)hp.rows[k].L; p->class_M[c] += (double)hp.rows[k].M;
       } else {
         const int R1 = 1 << (lm - p->cap_log2);
         if (R1 > 16) return QTAM_ERR_UNSUPPORTED;
         for (int j1 = 0; j1 < R1; ++j1)
-          items[generic_class_of(p->cap_log2)].push_back(WorkItem{(int)k, j1, R1, p->cap_log2});
+          {
+            items[generic_class_of(p->cap_log2)].push_back(WorkItem{(int)k, j1, R1, p->cap_log2});
+            items_fwd[generic_class_of(p->cap_log2)].push_back(WorkItem{(int)k, j1, R1, p->cap_log2});
+          }
         big.push_back((int)k);
         p->class_L[generic_class_of(p->cap_log2)] += (double)hp.rows[k].L;
         p->class_M[generic_class_of(p->cap_log2)] += (double)hp.rows[k].M;
@@ -287,6 +302,21 @@ template <typename T> qtam_status build_device(qtam_plan *p) {
                        [](const WorkItem &a, const WorkItem &b) { return a.log2M2 > b.log2M2; });
       p->n_items[c] = (int)items[c].size();
       if (!upload(&p->d_items[c], items[c].data(), items[c].size(), tot)) return QTAM_ERR_ALLOC;
+      std::stable_sort(items_fwd[c].begin(), items_fwd[c].end(),
+                       [](const WorkItem &a, const WorkItem &b) { return a.log2M2 > b.log2M2; });
+      p->n_items_fwd[c] = (int)items_fwd[c].size();
+      if (!upload(&p->d_items_fwd[c], items_fwd[c].data(), items_fwd[c].size(), tot)) return QTAM_ERR_ALLOC;
+    }
+    {
+      std::vector<int> fptr(hp.rows.size() + 1, 0);
+      std::vector<long long> foff;
+      for (size_t k = 0; k < hp.rows.size(); ++k) {
+        fptr[k] = (int)foff.size();
+        foff.insert(foff.end(), followers[k].begin(), followers[k].end());
+      }
+      fptr[hp.rows.size()] = (int)foff.size();
+      if (!upload(&p->d_gfol_ptr, fptr.data(), fptr.size(), tot)) return QTAM_ERR_ALLOC;
+      if (!upload(&p->d_gfol_off, foff.data(), foff.size(), tot)) return QTAM_ERR_ALLOC;
     }
     p->n_bigrows = (int)big.size();
     if (!upload(&p->d_bigrows, big.data(), big.size(), tot)) return QTAM_ERR_ALLOC;

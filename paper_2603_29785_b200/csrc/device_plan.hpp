@@ -65,6 +65,12 @@ struct qtam_plan {
   static const int kClasses = 4;
   qtam::WorkItem *d_items[kClasses] = {nullptr, nullptr, nullptr, nullptr};
   int n_items[kClasses] = {0, 0, 0, 0};
+  // forward lists: one leader per set of identical rows (same kc, dk; single-transform rows only); the
+  // followers' coefficient offsets per leader row: d_gfol_off[d_gfol_ptr[row] .. d_gfol_ptr[row+1])
+  qtam::WorkItem *d_items_fwd[kClasses] = {nullptr, nullptr, nullptr, nullptr};
+  int n_items_fwd[kClasses] = {0, 0, 0, 0};
+  int *d_gfol_ptr = nullptr;
+  long long *d_gfol_off = nullptr;
   double class_L[kClasses] = {0, 0, 0, 0};   // sum of band lengths / output lengths of a class's
   double class_M[kClasses] = {0, 0, 0, 0};   // items (for the launch profile's byte counts)
   double big_M = 0;                          // sum of M over the rows that need the combine pass

@@ -84,7 +84,8 @@ template <typename T>
 __global__ void k_fwd_rows(const RowDev *__restrict__ rows, const WorkItem *__restrict__ items,
                            const C2<T> *__restrict__ spec, long long xstride, int nbins,
                            const T *__restrict__ win, const C2<T> *__restrict__ tw, int log2twn,
-                           C2<T> *__restrict__ coef, long long ctot, int bufpts) {
+                           C2<T> *__restrict__ coef, long long ctot, int bufpts,
+                           const int *__restrict__ fol_ptr, const long long *__restrict__ fol_off) {
   typedef C2<T> V;
   V *a = reinterpret_cast<V *>(qtam_smem);
   V *bb = a + bufpts;
@@ -110,7 +111,11 @@ __global__ void k_fwd_rows(const RowDev *__restrict__ rows, const WorkItem *__re
   for (int i = threadIdx.x; i < M2; i += blockDim.x) {
     V v = res[i];
     if (it.R1 > 1) v = cmul(v, tw_get(tw, (long long)(it.j1 * i) << (log2twn - r.log2M), +1));
-    out[i] = cscale(v, sc);
+    v = cscale(v, sc);
+    out[i] = v;
+    // rows with the same centre bin and half-width (other Q-planes under the clamp) have these very values
+    for (int e = fol_ptr[it.row]; e < fol_ptr[it.row + 1]; ++e)
+      coef[(long long)blockIdx.y * ctot + fol_off[e] + i] = v;
   }
 }
 
@@ -511,17 +516,18 @@ static qtam_status fwd_rows_t(qtam_plan *p, int batch, void *d_coef, cudaStream_
   const C2<T> *tw = static_cast<const C2<T> *>(p->d_tw);
   const int log2twn = ilog2(p->twn);
   for (int c = 0; c < qtam_plan::kClasses; ++c) {
-    if (p->n_items[c] == 0) continue;
+    if (p->n_items_fwd[c] == 0) continue;
     const int bufpts = 1 << kClassLog2[c];
     const size_t smem = 2 * sizeof(C2<T>) * (size_t)bufpts;
     if (!set_smem(k_fwd_rows<T>, smem)) return QTAM_ERR_CUDA;
-    dim3 g(p->n_items[c], batch);
+    dim3 g(p->n_items_fwd[c], batch);
     {
       // reads the bands (L values per row), writes M coefficients per row
       LaunchScope ls(p, st, K_FWD_ROWS, sizeof(C2<T>) * (double)batch * (p->class_L[c] + p->class_M[c]));
       k_fwd_rows<T><<<g, kClassThreads[c], smem, st>>>(
-          p->d_rows, p->d_items[c], static_cast<const C2<T> *>(p->d_spec), p->xstride, (int)p->hp.nb,
-          static_cast<const T *>(p->d_win), tw, log2twn, static_cast<C2<T> *>(d_coef), p->hp.ctot, bufpts);
+          p->d_rows, p->d_items_fwd[c], static_cast<const C2<T> *>(p->d_spec), p->xstride, (int)p->hp.nb,
+          static_cast<const T *>(p->d_win), tw, log2twn, static_cast<C2<T> *>(d_coef), p->hp.ctot, bufpts,
+          p->d_gfol_ptr, p->d_gfol_off);
     }
     QTAM_LAUNCH_CHECK();
   }
