@@ -43,7 +43,7 @@ void free_plan(qtam_plan *p) {
   cudaFree(p->d_rows); cudaFree(p->d_win); cudaFree(p->d_tw); cudaFree(p->d_invP);
   cudaFree(p->d_csr_ptr); cudaFree(p->d_csr_idx); cudaFree(p->d_csrj_ptr); cudaFree(p->d_csrj_idx); cudaFree(p->d_plane_off);
   for (int c = 0; c < qtam_plan::kClasses; ++c) { cudaFree(p->d_items[c]); cudaFree(p->d_items_fwd[c]); }
-  cudaFree(p->d_gfol_ptr); cudaFree(p->d_gfol_off);
+  cudaFree(p->d_gfol_ptr); cudaFree(p->d_gfol_off); cudaFree(p->d_gfol_woff);
   cudaFree(p->d_bigrows); cudaFree(p->d_spec_alloc); cudaFree(p->d_ws); cudaFree(p->d_band);
   cudaFree(p->d_fwinp); cudaFree(p->d_red);
   cudaFree(p->d_frows); cudaFree(p->d_fwin); cudaFree(p->d_ftw_fwd); cudaFree(p->d_ftw_inv);
@@ -263,6 +263,7 @@ template <typename T> qtam_status build_device(qtam_plan *p) {
     std::vector<WorkItem> items[qtam_plan::kClasses], items_fwd[qtam_plan::kClasses];
     std::vector<int> big;
     std::vector<std::vector<long long>> followers(hp.rows.size());   // per leader row: follower offsets
+    std::vector<std::vector<long long>> followers_w(hp.rows.size()); // ... and their band offsets
     std::vector<int> gen_leaders;                                    // single-transform rows seen so far
     for (size_t k = 0; k < hp.rows.size(); ++k) {
       const int lm = ilog2(hp.rows[k].M);
@@ -278,7 +279,7 @@ template <typename T> qtam_status build_device(qtam_plan *p) {
             if (hp.rows[(size_t)l].kc == hp.rows[k].kc && hp.rows[(size_t)l].dk == hp.rows[k].dk &&
                 hp.rows[(size_t)l].M == hp.rows[k].M) { leader = l; break; }
           if (leader < 0) { gen_leaders.push_back((int)k); items_fwd[c].push_back(WorkItem{(int)k, 0, 1, lm}); }
-          else followers[(size_t)leader].push_back(hp.rows[k].offset);
+          else { followers[(size_t)leader].push_back(hp.rows[k].offset); followers_w[(size_t)leader].push_back(hp.rows[k].woff); }
         }
         p->class_L[c] += (double)hp.rows[k].L; p->class_M[c] += (double)hp.rows[k].M;
       } else {
@@ -309,14 +310,16 @@ template <typename T> qtam_status build_device(qtam_plan *p) {
     }
     {
       std::vector<int> fptr(hp.rows.size() + 1, 0);
-      std::vector<long long> foff;
+      std::vector<long long> foff, fwoff;
       for (size_t k = 0; k < hp.rows.size(); ++k) {
         fptr[k] = (int)foff.size();
         foff.insert(foff.end(), followers[k].begin(), followers[k].end());
+        fwoff.insert(fwoff.end(), followers_w[k].begin(), followers_w[k].end());
       }
       fptr[hp.rows.size()] = (int)foff.size();
       if (!upload(&p->d_gfol_ptr, fptr.data(), fptr.size(), tot)) return QTAM_ERR_ALLOC;
       if (!upload(&p->d_gfol_off, foff.data(), foff.size(), tot)) return QTAM_ERR_ALLOC;
+      if (!upload(&p->d_gfol_woff, fwoff.data(), fwoff.size(), tot)) return QTAM_ERR_ALLOC;
     }
     p->n_bigrows = (int)big.size();
     if (!upload(&p->d_bigrows, big.data(), big.size(), tot)) return QTAM_ERR_ALLOC;

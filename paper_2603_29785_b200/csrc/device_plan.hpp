@@ -71,6 +71,7 @@ struct qtam_plan {
   int n_items_fwd[kClasses] = {0, 0, 0, 0};
   int *d_gfol_ptr = nullptr;
   long long *d_gfol_off = nullptr;
+  long long *d_gfol_woff = nullptr;   // the followers' band-workspace offsets (joint inverse zeroes their slots)
   double class_L[kClasses] = {0, 0, 0, 0};   // sum of band lengths / output lengths of a class's
   double class_M[kClasses] = {0, 0, 0, 0};   // items (for the launch profile's byte counts)
   double big_M = 0;                          // sum of M over the rows that need the combine pass

@@ -258,7 +258,9 @@ template <typename T>
 __global__ void k_inv_rows(const RowDev *__restrict__ rows, const WorkItem *__restrict__ items,
                            const C2<T> *__restrict__ coef, long long ctot, const T *__restrict__ win,
                            const C2<T> *__restrict__ tw, int log2twn, C2<T> *__restrict__ band,
-                           long long sumL, int nbins, int plane, int bufpts) {
+                           long long sumL, int nbins, int plane, int bufpts,
+                           const int *__restrict__ fol_ptr, const long long *__restrict__ fol_off,
+                           const long long *__restrict__ fol_woff) {
   typedef C2<T> V;
   V *a = reinterpret_cast<V *>(qtam_smem);
   V *bb = a + bufpts;
@@ -267,8 +269,15 @@ __global__ void k_inv_rows(const RowDev *__restrict__ rows, const WorkItem *__re
   if (plane >= 0 && r.plane != plane) return;
   const int M2 = 1 << it.log2M2;
   const V *Y = coef + (long long)blockIdx.y * ctot + r.offset;
+  // joint inverse (fol_ptr != nullptr): the item list holds one leader per set of identical rows; the
+  // followers' coefficient rows are added before the transform (linearity) and their band slots are zeroed
+  const int e0 = fol_ptr ? fol_ptr[it.row] : 0, e1 = fol_ptr ? fol_ptr[it.row + 1] : 0;
   if (it.R1 == 1) {
-    for (int i = threadIdx.x; i < M2; i += blockDim.x) a[i] = Y[i];
+    for (int i = threadIdx.x; i < M2; i += blockDim.x) {
+      V acc = Y[i];
+      for (int e = e0; e < e1; ++e) acc = cadd(acc, coef[(long long)blockIdx.y * ctot + fol_off[e] + i]);
+      a[i] = acc;
+    }
   } else {
     const int log2R1 = r.log2M - it.log2M2;
     for (int i = threadIdx.x; i < M2; i += blockDim.x) {
@@ -289,6 +298,7 @@ __global__ void k_inv_rows(const RowDev *__restrict__ rows, const WorkItem *__re
     if (jj >= -r.dk && jj <= r.dk && f >= 0 && f < nbins) {
       const T w = win[r.woff + jj + r.dk] * amp;
       G[jj + r.dk] = cscale(res[i], w);
+      for (int e = e0; e < e1; ++e) band[(long long)blockIdx.y * sumL + fol_woff[e] + jj + r.dk] = cmk<T>(0, 0);
     }
   }
 }
@@ -552,17 +562,20 @@ static qtam_status inv_rows_t(qtam_plan *p, const void *d_coef, int batch, int p
   const C2<T> *tw = static_cast<const C2<T> *>(p->d_tw);
   const int log2twn = ilog2(p->twn);
   for (int c = 0; c < qtam_plan::kClasses; ++c) {
-    if (p->n_items[c] == 0) continue;
+    // the joint inverse takes the leader lists (identical rows added first), one plane alone every row
+    const bool lead = plane < 0;
+    const int n_it = lead ? p->n_items_fwd[c] : p->n_items[c];
+    if (n_it == 0) continue;
     const int bufpts = 1 << kClassLog2[c];
     const size_t smem = 2 * sizeof(C2<T>) * (size_t)bufpts;
     if (!set_smem(k_inv_rows<T>, smem)) return QTAM_ERR_CUDA;
-    dim3 g(p->n_items[c], batch);
+    dim3 g(n_it, batch);
     {
       LaunchScope ls(p, st, K_INV_ROWS, sizeof(C2<T>) * (double)batch * (p->class_L[c] + p->class_M[c]));
       k_inv_rows<T><<<g, kClassThreads[c], smem, st>>>(
-          p->d_rows, p->d_items[c], static_cast<const C2<T> *>(d_coef), p->hp.ctot,
+          p->d_rows, lead ? p->d_items_fwd[c] : p->d_items[c], static_cast<const C2<T> *>(d_coef), p->hp.ctot,
           static_cast<const T *>(p->d_win), tw, log2twn, static_cast<C2<T> *>(p->d_band), p->hp.sumL,
-          (int)p->hp.nb, plane, bufpts);
+          (int)p->hp.nb, plane, bufpts, lead ? p->d_gfol_ptr : nullptr, p->d_gfol_off, p->d_gfol_woff);
     }
     QTAM_LAUNCH_CHECK();
   }
