@@ -1,13 +1,15 @@
 #!/usr/bin/env python
 """bench.py -- QTAM forward+inverse throughput on B200 through the C ABI (libqtam.so).
 
-  python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg3] [--batch B] [--impl reference]
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg4] [--batch B] [--impl reference]
 
 A step is one pass of the whole hot path over one batch of synthetic strain: forward (long R2C,
 window gather + baseband shift + short IFFT per row), [row-median threshold for cfg5], inverse
-(per-row FFT, overlap reduction, 1/P, long C2R).  Default workload: BASELINE.json configs[2]
-("cfg3": 256 x 4 s at 4096 Hz, complex64, forward+inverse), the first configuration that exercises
-the forward+inverse metric; see DESIGN.md "Measurement".  One JSON line is printed by rank 0.
+(per-row FFT, overlap reduction, 1/P, long C2R).  Default workload: BASELINE.json configs[3]
+("cfg4": 16 x 64 s at 16384 Hz, N = 2^20, complex64, forward+inverse), the largest single-GPU
+configuration (2.93 GB of compulsory traffic per step); the same run also times configs 2, 3, 5 and the
+fp64 variant of 5 (`configs` in the JSON line), each at its own batch and at a larger one.
+"Measurement".  One JSON line is printed by rank 0.
 
 Timing: W >= 3 warm-up steps, then K steps each bracketed by CUDA events on the launch stream with an
 L2 flush (a 512 MB device memset) before every step, outside the event brackets; barrier +
@@ -36,16 +38,19 @@ UNIT = "samples/s"
 def parse_args():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=100)
+    ap.add_argument("--steps", type=int, default=50)
     ap.add_argument("--warmup", type=int, default=10)
-    ap.add_argument("--workload", default="cfg3", choices=sorted(inputs.CONFIGS))
+    ap.add_argument("--workload", default="cfg4", choices=sorted(inputs.CONFIGS))
     ap.add_argument("--batch", type=int, default=0, help="segments per GPU (default: the configuration's)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--overlap", type=float, default=1.0, help="clamp_overlap (R7); 1.0 = paper literal")
     ap.add_argument("--e2e-chunks", type=int, default=2, help="chunks of the batch pipelined over H2D | kernels | D2H")
     ap.add_argument("--no-largest-batch", action="store_true",
-                    help="skip the extra pass at a batch of 8 segments per SM (SURVEY.md 8(d) 'largest batch')")
+                    help="skip the extra passes at a batch scaled up until throughput saturates (SURVEY.md 8(d))")
+    ap.add_argument("--no-other-configs", action="store_true",
+                    help="skip the records of the other BASELINE configurations (`configs` in the JSON line)")
+    ap.add_argument("--dtype", default="", choices=["", "f32", "f64"], help="override the configuration's dtype")
     return ap.parse_args()
 
 
@@ -60,24 +65,44 @@ def measured_peaks():
     return 6650.0, "fallback (B200_PROFILING.md: 6.65 TB/s)"
 
 
+def csrc_hash():
+    """sha256 (first 16 hex digits) over the kernel sources: a DRAM-traffic capture is only valid for the
+    sources it was taken from"""
+    import hashlib
+    d = os.path.join(ROOT, "paper_2603_29785_b200", "csrc")
+    h = hashlib.sha256()
+    for name in sorted(os.listdir(d)):
+        if name.endswith((".cu", ".cuh", ".hpp", ".cpp")):
+            h.update(name.encode())
+            h.update(open(os.path.join(d, name), "rb").read())
+    return h.hexdigest()[:16]
+
+
 def measured_traffic(workload, batch, kernel):
-    """dram__bytes_read + dram__bytes_write of one launch from the committed ncu --set full capture
-    (profiles/r1_dram_traffic.csv, see the .md beside it); None when no capture matches this run."""
-    path = os.path.join(ROOT, "profiles", "r1_dram_traffic.csv")
+    """(dram__bytes_read + dram__bytes_write of one launch, source) from the committed ncu --set full capture
+    profiles/r2_dram_traffic.csv (see the .md beside it).  A row counts only if it was captured from the very
+    kernel sources of this run (csrc hash) at this workload and batch: (None, why) otherwise -- ncu cannot
+    run inside a timed bench, so the number can only come from a capture, never from this process."""
+    path = os.path.join(ROOT, "profiles", "r2_dram_traffic.csv")
+    want = csrc_hash()
+    seen = False
     try:
         with open(path) as f:
             for line in f.read().splitlines()[1:]:
-                w, b, k, v = line.split(",")
+                w, b, k, v, sha = line.split(",")[:5]
                 if w == workload and int(b) == batch and k == kernel:
-                    return float(v)
+                    seen = True
+                    if sha == want:
+                        return float(v), f"profiles/r2_dram_traffic.csv (ncu --set full, csrc {sha})"
     except Exception:
         pass
-    return None
+    return None, ("capture is from other kernel sources (csrc hash mismatch)" if seen
+                  else "no ncu capture for this workload / batch / kernel")
 
 
 def compulsory_bytes_per_segment(cfg, ctot):
-    """forward r*N + c*C_tot, inverse c*C_tot + r*N; threshold fused -> 0 extra, as a
-    separate in-place pass 2*c*C_tot (what this build does today)."""
+    """forward r*N + c*C_tot, inverse c*C_tot + r*N; the threshold moves no compulsory bytes
+    (float plans run it in the forward's epilogue; as a separate in-place pass it is design traffic)."""
     r = 8 if cfg["dtype"] == "f64" else 4
     c = 2 * r
     n = cfg["N"]
@@ -216,20 +241,129 @@ def workload_config(args, cfg, batch, plan):
     c = {
         "workload": f"{args.workload}: {batch} x {cfg['N']} samples at {cfg['fs']:g} Hz, "
                     f"Q-planes {cfg['Q']}, {cfg['rows']} rows each over {cfg['fmin']:g}-{cfg['fmax']:g} Hz, "
-                    f"calls {'+'.join(cfg['calls'])}",
+                    f"calls {', '.join(cfg['calls'])}",
         "baseline_config_index": cfg["idx"] - 1,
         "batch_per_gpu": batch, "N": cfg["N"], "fs": cfg["fs"], "clamp_overlap": args.overlap,
         "l2_policy": "512 MB device memset before every timed step (outside the event brackets)",
     }
-    if plan is not None:
-        c["coeffs_per_segment"] = plan.ctot
-        c["rows"] = plan.n_rows
     return c
 
 
 # --------------------------------------------------------------------------------------------------
 # our arm
 # --------------------------------------------------------------------------------------------------
+LARGEST = {"cfg2": 592, "cfg3": 1184, "cfg4": 48, "cfg5": 4096}   # batches at which throughput has saturated
+
+
+class Workload:
+    """one configuration at one batch on this rank: plan, device buffers, the step, timing helpers"""
+
+    def __init__(self, torch, binding, dev, name, dtype, batch, overlap, first_segment=0, x_np=None):
+        self.torch, self.name, self.dtype, self.batch, self.dev = torch, name, dtype, batch, dev
+        self.cfg = dict(inputs.CONFIGS[name], dtype=dtype)
+        fs, N, Q, fmin, fmax, rows = inputs.plan_args(name)
+        self.N = N
+        self.plan = binding.Plan(fs, N, Q, fmin, fmax, rows, dtype=dtype, max_batch=batch, clamp_overlap=overlap)
+        self.rdt = torch.float64 if dtype == "f64" else torch.float32
+        self.cdt = torch.complex128 if dtype == "f64" else torch.complex64
+        if x_np is None:
+            x_np = inputs.make_batch(name, batch=batch, first_segment=first_segment, dtype=dtype)
+        elif x_np.shape[0] < batch:       # a larger batch re-uses the generated segments (the path is data-oblivious)
+            x_np = np.tile(x_np, ((batch + x_np.shape[0] - 1) // x_np.shape[0], 1))[:batch]
+        self.x_np = np.ascontiguousarray(x_np[:batch])
+        self.d_x = torch.from_numpy(self.x_np).to(dev)
+        self.d_coef = torch.empty((batch, self.plan.ctot), dtype=self.cdt, device=dev)
+        self.d_out = torch.empty((batch, N), dtype=self.rdt, device=dev)
+        self.calls = self.cfg["calls"]
+        self.launches = 0
+
+    def step(self, lo=0, hi=None):
+        p, hi = self.plan, self.batch if hi is None else hi
+        if "threshold" in self.calls:
+            p.forward_threshold(self.d_x[lo:hi], 3.0, out=self.d_coef[lo:hi])   # forward + row-median threshold
+        else:
+            p.forward(self.d_x[lo:hi], out=self.d_coef[lo:hi])
+        self.launches += p.last_launch_count()
+        if "inverse" in self.calls:
+            p.inverse(self.d_coef[lo:hi], out=self.d_out[lo:hi])
+            self.launches += p.last_launch_count()
+
+    def timed(self, nsteps, profile, flush, barrier):
+        """nsteps steps, each bracketed by CUDA events on the launch stream with an L2 flush before it (outside
+        the brackets); returns (sum of ms, per-kernel stats, launches)"""
+        torch = self.torch
+        self.plan.profile_enable(profile, max_launches=max(64, 64 * nsteps))
+        ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(nsteps)]
+        self.launches = 0
+        barrier()
+        for s, e in ev:
+            flush.zero_()
+            s.record()
+            self.step()
+            e.record()
+        barrier()
+        ms = sum(s.elapsed_time(e) for s, e in ev)
+        stats = self.plan.profile_read() if profile else []
+        self.plan.profile_enable(False)
+        return ms, stats, self.launches
+
+    def compulsory_bytes(self):
+        return compulsory_bytes_per_segment(self.cfg, self.plan.ctot) * self.batch
+
+    def round_trip_err(self):
+        """worst segment of |inverse(forward(x)) - Pi_C x| / |Pi_C x| (verification outside the timed region;
+        torch.fft only builds the projection, it is never on the product path)"""
+        torch = self.torch
+        if "inverse" not in self.calls or "threshold" in self.calls:
+            return None
+        _, cover = self.plan.frame(-1)
+        cov = torch.from_numpy(cover).to(self.dev)
+        self.step()
+        worst = 0.0
+        for b0 in range(0, self.batch, 64):
+            xs = self.d_x[b0:b0 + 64].double()
+            X = torch.fft.rfft(xs, dim=-1)
+            proj = torch.fft.irfft(torch.where(cov[None, :], X, torch.zeros_like(X)), n=self.N, dim=-1)
+            err = (self.d_out[b0:b0 + 64].double() - proj).norm(dim=-1) / proj.norm(dim=-1)
+            worst = max(worst, float(err.max().item()))
+        return worst
+
+    def close(self):
+        self.plan.close()
+        del self.d_x, self.d_coef, self.d_out
+
+
+def kernel_table(stats, nsteps, peak):
+    """per kernel: launches per step, average launch duration, share of the summed kernel time, compulsory
+    (algo) and design bytes per launch and the rates they imply"""
+    out = []
+    tot_ms = sum(s["ms"] for s in stats) or 1.0
+    for s in sorted(stats, key=lambda s: -s["ms"]):
+        avg_ms = s["ms"] / s["launches"]
+        algo, design = s["algo_bytes"] / s["launches"], s["design_bytes"] / s["launches"]
+        out.append({"name": s["name"], "launches_per_step": s["launches"] / nsteps, "avg_ms": avg_ms,
+                    "share": s["ms"] / tot_ms, "algo_bytes": algo, "design_bytes": design,
+                    "algo_gbs": algo / (avg_ms * 1e-3) / 1e9, "frac_of_peak": algo / (avg_ms * 1e-3) / 1e9 / peak,
+                    "design_gbs": design / (avg_ms * 1e-3) / 1e9})
+    return out
+
+
+def record(w, nsteps, warmup, flush, barrier, peak):
+    """ms per step, samples/s, fraction of the HBM roofline on compulsory bytes and the per-kernel table"""
+    for _ in range(max(3, warmup)):
+        w.step()
+    w.torch.cuda.synchronize()
+    ms_plain, _, n_launch = w.timed(nsteps, False, flush, barrier)
+    ms_prof, stats, _ = w.timed(nsteps, True, flush, barrier)
+    ms = ms_plain / nsteps
+    comp = w.compulsory_bytes()
+    gbs = comp / (ms * 1e-3) / 1e9
+    return {"batch": w.batch, "dtype": w.dtype, "steps": nsteps, "ms_per_step": ms,
+            "value": w.batch * w.N / (ms * 1e-3), "unit": UNIT, "compulsory_bytes_per_step": comp,
+            "path_gbs": gbs, "path_frac_of_peak": gbs / peak, "gpu_launches_per_step": n_launch / nsteps,
+            "ms_per_step_with_launch_profile": ms_prof / nsteps, "kernels": kernel_table(stats, nsteps, peak)}
+
+
 def run_ours(args):
     import torch
     import torch.distributed as dist
@@ -247,68 +381,33 @@ def run_ours(args):
 
     cfg = inputs.CONFIGS[args.workload]
     batch = args.batch or cfg["batch"]
-    dtype = cfg["dtype"]
-    fs, N, Q, fmin, fmax, rows = inputs.plan_args(args.workload)
-    plan = binding.Plan(fs, N, Q, fmin, fmax, rows, dtype=dtype, max_batch=batch, clamp_overlap=args.overlap)
-    rdt = torch.float64 if dtype == "f64" else torch.float32
-    cdt = torch.complex128 if dtype == "f64" else torch.complex64
-
-    # each rank gets its own segments (weak scaling, no collective on the data path)
-    first, _ = dist_utils.shard_segments(rank, world, batch)
-    x_np = inputs.make_batch(args.workload, batch=batch, first_segment=first)
-    x_pin = torch.from_numpy(x_np).pin_memory()
-    d_x = x_pin.to(dev)
-    d_coef = torch.empty((batch, plan.ctot), dtype=cdt, device=dev)
-    d_out = torch.empty((batch, N), dtype=rdt, device=dev)
-    out_pin = torch.empty((batch, N), dtype=rdt).pin_memory()
-    flush = torch.empty(512 * 1024 * 1024, dtype=torch.uint8, device=dev)
-    calls = cfg["calls"]
-    launches = [0]
-
-    def step():
-        if "threshold" in calls:
-            plan.forward_threshold(d_x, 3.0, out=d_coef)     # forward + row-median threshold, one call
-        else:
-            plan.forward(d_x, out=d_coef)
-        launches[0] += plan.last_launch_count()
-        if "inverse" in calls:
-            plan.inverse(d_coef, out=d_out)
-            launches[0] += plan.last_launch_count()
+    dtype = args.dtype or cfg["dtype"]
+    N = cfg["N"]
+    peak, peak_src = measured_peaks()
 
     def barrier():
         if world > 1:
             dist.barrier()
         torch.cuda.synchronize()
 
-    def timed(nsteps, profile):
-        plan.profile_enable(profile, max_launches=max(64, 64 * nsteps))
-        ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(nsteps)]
-        launches[0] = 0
-        barrier()
-        for s, e in ev:
-            flush.zero_()
-            s.record()
-            step()
-            e.record()
-        barrier()
-        ms = sum(s.elapsed_time(e) for s, e in ev)
-        stats = plan.profile_read() if profile else []
-        plan.profile_enable(False)
-        return ms, stats, launches[0]
+    # each rank gets its own segments (weak scaling, no collective on the data path)
+    first, _ = dist_utils.shard_segments(rank, world, batch)
+    w = Workload(torch, binding, dev, args.workload, dtype, batch, args.overlap, first_segment=first)
+    plan, calls = w.plan, w.calls
+    flush = torch.empty(512 * 1024 * 1024, dtype=torch.uint8, device=dev)
 
     W = max(args.warmup, 3)
     for _ in range(W):
-        step()
+        w.step()
     torch.cuda.synchronize()
 
     # ---- the timed region: exactly K steps, each bracketed by CUDA events on the launch stream (-> value),
     # then the same K steps again with the library's launch profile on (two more events around every kernel
-    # launch: about 8 % of a cfg3 step) for the per-kernel durations of the roofline line.  Clocks are
-    # sampled across both passes.
+    # launch) for the per-kernel durations of the roofline line.  Clocks are sampled across both passes.
     sampler = ClockSampler(physical_gpu_index(local))
     sampler.start()
-    ms_plain, _, n_launch = timed(args.steps, False)
-    ms_total, stats, _ = timed(args.steps, True)
+    ms_plain, _, n_launch = w.timed(args.steps, False, flush, barrier)
+    ms_total, stats, _ = w.timed(args.steps, True, flush, barrier)
     clocks = sampler.stop()
 
     # context: the same step captured once into a CUDA graph and replayed (the calls neither allocate nor
@@ -318,7 +417,7 @@ def run_ours(args):
         try:
             cg = torch.cuda.CUDAGraph()
             with torch.cuda.graph(cg):
-                step()
+                w.step()
             ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
             torch.cuda.synchronize()
             for s0, s1 in ev:
@@ -333,9 +432,12 @@ def run_ours(args):
     # The batch goes through in `--e2e-chunks` chunks on three streams (H2D | forward[+threshold]+inverse |
     # D2H), so that the PCIe copies of one chunk overlap the kernels of another; every step still copies
     # all of its inputs in and all of its results out.
+    x_pin = torch.from_numpy(w.x_np).pin_memory()
+    d_x, d_coef, d_out = w.d_x, w.d_coef, w.d_out
+    out_pin = torch.empty((batch, N), dtype=w.rdt).pin_memory()
     coef_pin = None
     if "inverse" not in calls:
-        coef_pin = torch.empty((batch, plan.ctot), dtype=cdt).pin_memory()
+        coef_pin = torch.empty((batch, plan.ctot), dtype=w.cdt).pin_memory()
     nch = max(1, min(args.e2e_chunks, batch))
     bounds = [(c * batch // nch, (c + 1) * batch // nch) for c in range(nch)]
     s_in, s_cmp, s_out = torch.cuda.Stream(dev), torch.cuda.Stream(dev), torch.cuda.Stream(dev)
@@ -355,13 +457,7 @@ def run_ours(args):
                 s_cmp.wait_event(ev_in[c])
                 if primed[0]:
                     s_cmp.wait_event(ev_out[c])         # the previous step's D2H has read the result buffer
-                if "threshold" in calls:
-                    plan.forward_threshold(d_x[lo:hi], 3.0, out=d_coef[lo:hi])
-                else:
-                    plan.forward(d_x[lo:hi], out=d_coef[lo:hi])
-                launches[0] += plan.last_launch_count()
-                if "inverse" in calls:
-                    plan.inverse(d_coef[lo:hi], out=d_out[lo:hi])
+                w.step(lo, hi)
                 ev_cmp[c].record(s_cmp)
             with torch.cuda.stream(s_out):
                 s_out.wait_event(ev_cmp[c])
@@ -398,101 +494,81 @@ def run_ours(args):
     barrier()
     ms_e2e = e0.elapsed_time(e1) / n_e2e
     # what came back over PCIe is what the device-resident path computes (kernels are deterministic)
-    step()
+    w.step()
     torch.cuda.synchronize()
     e2e_ok = bool(torch.equal(out_pin, d_out.cpu())) if "inverse" in calls else bool(torch.equal(coef_pin, d_coef.cpu()))
     h2d = x_pin.numel() * x_pin.element_size()
     d2h = (out_pin.numel() * out_pin.element_size()) if "inverse" in calls else (coef_pin.numel() * coef_pin.element_size())
+    del x_pin, out_pin, coef_pin
 
     # ---- max over ranks
     ms_total, ms_plain, ms_e2e = dist_utils.max_over_ranks([ms_total, ms_plain, ms_e2e], device=dev)
     ms_step = ms_plain / args.steps
     units = world * batch * N
     value = dist_utils.aggregate_throughput(world, batch, N, ms_step)
-
-    # ---- round-trip error against Pi_C x (verification outside the timed region; torch.fft is
-    # used here only to build the projection, never on the product path)
-    rt_err = None
-    if "inverse" in calls and "threshold" not in calls:
-        _, cover = plan.frame(-1)
-        cov = torch.from_numpy(cover).to(dev)
-        X = torch.fft.rfft(d_x.double(), dim=-1)
-        proj = torch.fft.irfft(torch.where(cov[None, :], X, torch.zeros_like(X)), n=N, dim=-1)
-        step()
-        err = (d_out.double() - proj).norm(dim=-1) / proj.norm(dim=-1)
-        rt_err = float(err.max().item())
+    rt_err = w.round_trip_err()
 
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
         return
 
-    # ---- roofline of the dominant kernel, from the launch profile of the timed region
-    peak, peak_src = measured_peaks()
+    # ---- roofline of the dominant kernel, from the launch profile of the timed region: COMPULSORY bytes of
+    # that launch (samples in / coefficients / samples out) over its CUDA-event duration
+    kernels = kernel_table(stats, args.steps, peak)
     roof = None
-    kernels = []
-    if stats:
-        tot_ms = sum(s["ms"] for s in stats)
-        for s in sorted(stats, key=lambda s: -s["ms"]):
-            avg_ms = s["ms"] / s["launches"]
-            gbs = s["algo_bytes"] / s["launches"] / (avg_ms * 1e-3) / 1e9
-            kernels.append({"name": s["name"], "launches_per_step": s["launches"] / args.steps,
-                            "avg_ms": avg_ms, "share": s["ms"] / tot_ms, "algo_gbs": gbs,
-                            "algo_bytes": s["algo_bytes"] / s["launches"]})
+    if kernels:
         top = kernels[0]
+        traffic, traffic_src = measured_traffic(args.workload, batch, top["name"])
         roof = {"bound": "hbm", "kernel": top["name"], "achieved": top["algo_gbs"], "peak": peak,
-                "unit": "GB/s", "frac": top["algo_gbs"] / peak,
-                "traffic": measured_traffic(args.workload, batch, top["name"]),
-                "algo_bytes_per_launch": top["algo_bytes"],
+                "unit": "GB/s", "frac": top["algo_gbs"] / peak, "traffic": traffic, "traffic_source": traffic_src,
+                "algo_bytes_per_launch": top["algo_bytes"], "design_bytes_per_launch": top["design_bytes"],
                 "peak_source": peak_src, "avg_launch_ms": top["avg_ms"], "share_of_step": top["share"]}
-    comp = compulsory_bytes_per_segment(cfg, plan.ctot) * batch
+    comp = w.compulsory_bytes()
     path_gbs = comp / (ms_step * 1e-3) / 1e9
 
-    # ---- the same step at a batch that fills every SM several times over ("largest batch")
-    largest = None
-    if world == 1 and not args.batch and not args.no_largest_batch and cfg["N"] <= 32768:
-        sms = torch.cuda.get_device_properties(dev).multi_processor_count
-        big = 8 * sms
-        x_big = torch.from_numpy(inputs.make_batch(args.workload, batch=min(big, 2 * batch))).to(dev)
-        x_big = x_big.repeat((big + x_big.shape[0] - 1) // x_big.shape[0], 1)[:big].contiguous()
-        plan_b = binding.Plan(fs, N, Q, fmin, fmax, rows, dtype=dtype, max_batch=big, clamp_overlap=args.overlap)
-        c_big = torch.empty((big, plan_b.ctot), dtype=cdt, device=dev)
-        o_big = torch.empty((big, N), dtype=rdt, device=dev)
-
-        def step_big():
-            if "threshold" in calls:
-                plan_b.forward_threshold(x_big, 3.0, out=c_big)
-            else:
-                plan_b.forward(x_big, out=c_big)
-            if "inverse" in calls:
-                plan_b.inverse(c_big, out=o_big)
-
-        for _ in range(3):
-            step_big()
-        torch.cuda.synchronize()
-        nb = 10
-        plan_b.profile_enable(True, max_launches=64 * nb)
-        evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(nb)]
-        for s0, e0_ in evs:
-            flush.zero_()
-            s0.record(); step_big(); e0_.record()
-        torch.cuda.synchronize()
-        ms_b = sum(a.elapsed_time(b) for a, b in evs) / nb
-        st_b = plan_b.profile_read()
-        plan_b.profile_enable(False)
-        comp_b = compulsory_bytes_per_segment(cfg, plan_b.ctot) * big
-        largest = {"batch": big, "ms_per_step": ms_b, "value": big * N / (ms_b * 1e-3), "unit": UNIT,
-                   "path_gbs": comp_b / (ms_b * 1e-3) / 1e9, "path_frac_of_peak": comp_b / (ms_b * 1e-3) / 1e9 / peak,
-                   "kernels": [{"name": k["name"], "avg_ms": k["ms"] / k["launches"],
-                                "algo_gbs": k["algo_bytes"] / k["ms"] / 1e6,
-                                "frac_of_peak": k["algo_bytes"] / k["ms"] / 1e6 / peak}
-                               for k in sorted(st_b, key=lambda k: -k["ms"])]}
-        plan_b.close()
-        del x_big, c_big, o_big
+    # ---- the same step at a batch that has saturated the throughput ("largest batch"), and the
+    # other BASELINE configurations at their own batch and at their largest one (fewer steps each)
+    n_side = max(5, min(args.steps, 20))
+    largest, others = None, {}
+    x_main = w.x_np
+    if world == 1 and not args.batch and not args.no_largest_batch:
+        big = LARGEST[args.workload] if args.workload in LARGEST else None
+        if big and big > batch:
+            w.close()
+            wb = Workload(torch, binding, dev, args.workload, dtype, big, args.overlap, x_np=x_main)
+            largest = record(wb, n_side, 3, flush, barrier, peak)
+            wb.close()
+            del wb
+            w = None
+    if world == 1 and not args.batch and not args.no_other_configs:
+        if w is not None:
+            w.close()
+            w = None
+        for name, dt in (("cfg2", "f32"), ("cfg3", "f32"), ("cfg5", "f32"), ("cfg5", "f64"), ("cfg4", "f32"), ("cfg1", "f64")):
+            if name == args.workload and dt == dtype:
+                continue
+            key = name if dt == inputs.CONFIGS[name]["dtype"] else f"{name}_{dt}"
+            try:
+                wo = Workload(torch, binding, dev, name, dt, inputs.CONFIGS[name]["batch"], args.overlap)
+                rec = record(wo, n_side, 3, flush, barrier, peak)
+                rec["round_trip_err"] = wo.round_trip_err()
+                xo = wo.x_np
+                wo.close()
+                big = LARGEST.get(name)
+                if big and not args.no_largest_batch:
+                    if dt == "f64":
+                        big //= 2
+                    wb = Workload(torch, binding, dev, name, dt, big, args.overlap, x_np=xo)
+                    rec["largest_batch"] = record(wb, max(5, n_side // 2), 3, flush, barrier, peak)
+                    wb.close()
+                others[key] = rec
+            except Exception as exc:          # one configuration failing must not lose the headline
+                others[key] = {"error": str(exc)}
+            torch.cuda.empty_cache()
 
     # ---- cuFFT (through torch.fft) on the same shapes, side by side as a reference only (north_star): the
-    # long real transforms and one batched complex transform per length bucket -- cuFFT does the FFTs alone,
-    # without the gather / window / shift, the overlap sum or 1/P, and writes one row per (plane, row)
+    # long real transforms alone, without the gather / window / shift, the overlap sum or 1/P
     cufft = None
     if world == 1:
         def ev_time(fn, reps=10):
@@ -505,24 +581,12 @@ def run_ours(args):
                 tot += a.elapsed_time(b)
             return tot / reps
         try:
-            spec_t = torch.fft.rfft(d_x, dim=-1)
-            cufft = {"rfft_ms": ev_time(lambda: torch.fft.rfft(d_x, dim=-1)),
-                     "irfft_ms": ev_time(lambda: torch.fft.irfft(spec_t, n=N, dim=-1)), "buckets": []}
-            hist = {}
-            for r_ in plan.rows:
-                hist[int(r_.M)] = hist.get(int(r_.M), 0) + 1
-            tot_c2c = 0.0
-            for M_, cnt in sorted(hist.items()):
-                if batch * cnt * M_ * 8 > (6 << 30):
-                    continue
-                buf = torch.randn(batch * cnt, M_, dtype=cdt, device=dev)
-                t_ = ev_time(lambda: torch.fft.ifft(buf, dim=-1))
-                cufft["buckets"].append({"M": M_, "rows": cnt, "c2c_ms": t_})
-                tot_c2c += t_
-                del buf
-            cufft["c2c_all_buckets_ms"] = tot_c2c
-            cufft["note"] = "FFTs only, out of place, one launch per length; context, not the target"
-            del spec_t
+            xs = torch.from_numpy(x_main).to(dev)
+            spec_t = torch.fft.rfft(xs, dim=-1)
+            cufft = {"rfft_ms": ev_time(lambda: torch.fft.rfft(xs, dim=-1)),
+                     "irfft_ms": ev_time(lambda: torch.fft.irfft(spec_t, n=N, dim=-1)),
+                     "note": "the long real FFTs only, out of place; context, not the target"}
+            del spec_t, xs
         except Exception as exc:
             cufft = {"unavailable": str(exc)}
 
@@ -535,7 +599,7 @@ def run_ours(args):
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": W, "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak",
-        "vs_baseline": None, "dtype": "f32" if dtype == "f32" else "f64", "data": "synthetic",
+        "vs_baseline": None, "dtype": dtype, "data": "synthetic",
         "config": workload_config(args, cfg, batch, plan),
         "clocks": clocks,
         "e2e": {"value": units / (ms_e2e * 1e-3), "unit": UNIT, "h2d_bytes_per_step": h2d,
@@ -544,12 +608,15 @@ def run_ours(args):
         "gpu_launches": n_launch,
         "roofline": roof,
         "path": {"compulsory_bytes_per_step": comp, "achieved_gbs": path_gbs, "frac_of_peak": path_gbs / peak,
-                 "frac_of_8tbs": path_gbs / 8000.0, "ms_per_step_with_launch_profile": ms_total / args.steps, "ms_per_step_cuda_graph": ms_graph},
+                 "frac_of_8tbs": path_gbs / 8000.0, "ms_per_step_with_launch_profile": ms_total / args.steps,
+                 "ms_per_step_cuda_graph": ms_graph, "coeffs_per_segment": plan.ctot, "rows": plan.n_rows},
         "kernels": kernels,
         "round_trip_err": rt_err,
         "largest_batch": largest,
+        "configs": others,
         "cufft_side_by_side": cufft,
         "cpu_baseline": cpu,
+        "csrc_hash": csrc_hash(),
     }
     print(json.dumps(line))
     if world > 1:

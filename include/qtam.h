@@ -43,7 +43,8 @@ typedef enum { QTAM_F32 = 0, QTAM_F64 = 1 } qtam_dtype;  /* real in / complex ou
 typedef enum {
   QTAM_OK = 0,
   QTAM_ERR_INVALID_ARG = 1,   /* NULL pointer, N not a power of two, fmax >= fs/2, fmin <= 0,
-                                 Q < sqrt(11), half-width < 1 bin, batch > max_batch, bad row range */
+                                 Q < sqrt(11), half-width < 1 bin, batch > max_batch, bad row range,
+                                 max_batch > 65535 */
   QTAM_ERR_UNSUPPORTED = 2,   /* window family / size outside what this build implements */
   QTAM_ERR_ALLOC = 3,         /* host or device allocation failed at plan creation */
   QTAM_ERR_CUDA = 4,          /* a CUDA runtime call or launch failed (or no device) */
@@ -64,7 +65,8 @@ typedef struct {
                                        there is >= cover_floor; default 1e-2                       */
   int     rows_are_bins_per_octave; /* 0: `spacing` = rows per plane, endpoints inclusive;
                                        1: `spacing` = bins per octave B, f = fmin*2^(r/B) (:303)   */
-  int     max_batch;                /* workspace is sized for this many segments; default 1        */
+  int     max_batch;                /* workspace is sized for this many segments; default 1; at most
+                                       65535 (the batch index is a grid dimension of several kernels) */
   double  window_param;             /* Kaiser beta > 0; Tukey alpha_T, Planck alpha_P in (0, 1]     */
   const double *freqs;              /* manual grid (:303): n_freqs ascending centre frequencies in Hz
                                        (host pointer, read during plan creation only); when           */
@@ -189,10 +191,12 @@ const char *qtam_status_string(qtam_status s);
 /* Launch profile for bench.py's roofline line.  While enabled, every kernel launch of the compute
  * calls is bracketed by CUDA events on the launch stream (pre-created: up to `max_launches` launches
  * between two reads; further ones are not recorded).  qtam_profile_read waits for the recorded events,
- * sums per kernel the launches, the device time (ms) and the ALGORITHMIC bytes the launches had to
- * move, writes up to `capacity` entries to `out` (host), clears the record and
- * returns the number of entries (-1 on error). */
-typedef struct { char name[48]; int launches; double ms; double algo_bytes; } qtam_kernel_stat;
+ * sums per kernel the launches, the device time (ms), the COMPULSORY bytes of those launches (algo_bytes:
+ * input samples read, coefficients written or read, output samples written -- SURVEY.md 8(d)) and the bytes
+ * the launches move by design (design_bytes: compulsory + spectrum, partial sums, band workspace, scratch;
+ * DESIGN.md "Kernels"), writes up to `capacity` entries to `out` (host), clears the record and returns the
+ * number of entries (-1 on error). */
+typedef struct { char name[48]; int launches; double ms; double algo_bytes; double design_bytes; } qtam_kernel_stat;
 qtam_status qtam_profile_enable(qtam_plan *p, int on, int max_launches);
 int         qtam_profile_read(qtam_plan *p, qtam_kernel_stat *out, int capacity);
 

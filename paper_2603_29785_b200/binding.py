@@ -54,7 +54,7 @@ class Info(C.Structure):
 
 class KernelStat(C.Structure):
     _fields_ = [("name", C.c_char * 48), ("launches", C.c_int), ("ms", C.c_double),
-                ("algo_bytes", C.c_double)]
+                ("algo_bytes", C.c_double), ("design_bytes", C.c_double)]
 
 
 def lib():
@@ -180,44 +180,69 @@ class Plan:
     def _stream(self):
         return C.c_void_p(self._torch().cuda.current_stream().cuda_stream)
 
+    # argument checks: explicit errors (an `assert` disappears under python -O, and a mis-sized tensor would
+    # become an out-of-bounds device write inside the library)
+    def _need(self, t, dtype, what, numel=None, last=None):
+        if not (hasattr(t, "is_cuda") and t.is_cuda):
+            raise ValueError(f"{what}: expected a CUDA tensor")
+        if t.dtype != dtype:
+            raise ValueError(f"{what}: dtype {t.dtype}, expected {dtype}")
+        if not t.is_contiguous():
+            raise ValueError(f"{what}: must be contiguous")
+        if last is not None and (t.dim() < 1 or t.shape[-1] != last):
+            raise ValueError(f"{what}: last dimension {tuple(t.shape)}, expected {last}")
+        if numel is not None and t.numel() != numel:
+            raise ValueError(f"{what}: {t.numel()} elements, expected {numel}")
+
+    def _batch(self, t, per_segment, what):
+        if per_segment <= 0 or t.numel() % per_segment != 0:
+            raise ValueError(f"{what}: {t.numel()} elements is not a multiple of {per_segment}")
+        b = t.numel() // per_segment
+        if b > self.max_batch:
+            raise QtamError(1, f"{what}: batch {b} exceeds the plan's max_batch {self.max_batch}")
+        return b
+
     def forward(self, x, out=None):
         t = self._torch()
-        assert x.is_cuda and x.dtype == self._rdt() and x.is_contiguous() and x.shape[-1] == self.N
-        batch = x.numel() // self.N
+        self._need(x, self._rdt(), "x", last=self.N)
+        batch = self._batch(x, self.N, "x")
         if out is None:
             out = t.empty((batch, self.ctot), dtype=self._cdt(), device=x.device)
-        assert out.is_cuda and out.dtype == self._cdt() and out.is_contiguous() and out.numel() == batch * self.ctot
+        self._need(out, self._cdt(), "out", numel=batch * self.ctot)
         _check(lib().qtam_forward(self._h, x.data_ptr(), batch, out.data_ptr(), self._stream()), "qtam_forward")
         return out
 
     def inverse(self, coef, plane=-1, out=None):
         t = self._torch()
-        assert coef.is_cuda and coef.dtype == self._cdt() and coef.is_contiguous()
-        batch = coef.numel() // self.ctot
+        self._need(coef, self._cdt(), "coef")
+        batch = self._batch(coef, self.ctot, "coef")
         if out is None:
             out = t.empty((batch, self.N), dtype=self._rdt(), device=coef.device)
-        assert out.is_cuda and out.dtype == self._rdt() and out.is_contiguous() and out.numel() == batch * self.N
+        self._need(out, self._rdt(), "out", numel=batch * self.N)
         _check(lib().qtam_inverse(self._h, coef.data_ptr(), batch, plane, out.data_ptr(), self._stream()), "qtam_inverse")
         return out
 
     def dense(self, x, row_begin=0, row_end=None, out=None):
         t = self._torch()
         row_end = self.n_rows if row_end is None else row_end
-        assert x.is_cuda and x.dtype == self._rdt() and x.is_contiguous() and x.shape[-1] == self.N
-        batch = x.numel() // self.N
+        if not (0 <= row_begin <= row_end <= self.n_rows):
+            raise ValueError(f"row range [{row_begin}, {row_end}) outside [0, {self.n_rows})")
+        self._need(x, self._rdt(), "x", last=self.N)
+        batch = self._batch(x, self.N, "x")
         if out is None:
             out = t.empty((batch, row_end - row_begin, self.N), dtype=self._cdt(), device=x.device)
+        self._need(out, self._cdt(), "out", numel=batch * (row_end - row_begin) * self.N)
         _check(lib().qtam_dense(self._h, x.data_ptr(), batch, row_begin, row_end, out.data_ptr(), self._stream()), "qtam_dense")
         return out
 
     def forward_threshold(self, x, kappa=3.0, out=None):
         """forward + row-median threshold in one call (fused for float plans)"""
         t = self._torch()
-        assert x.is_cuda and x.dtype == self._rdt() and x.is_contiguous() and x.shape[-1] == self.N
-        batch = x.numel() // self.N
+        self._need(x, self._rdt(), "x", last=self.N)
+        batch = self._batch(x, self.N, "x")
         if out is None:
             out = t.empty((batch, self.ctot), dtype=self._cdt(), device=x.device)
-        assert out.is_cuda and out.dtype == self._cdt() and out.is_contiguous() and out.numel() == batch * self.ctot
+        self._need(out, self._cdt(), "out", numel=batch * self.ctot)
         _check(lib().qtam_forward_threshold(self._h, x.data_ptr(), batch, float(kappa), out.data_ptr(), self._stream()),
                "qtam_forward_threshold")
         return out
@@ -225,8 +250,8 @@ class Plan:
     def dense_invert(self, tile, row):
         """x[batch][N] from one dense tile per segment (Eq. 13); the plan needs epsilon > 0"""
         t = self._torch()
-        assert tile.is_cuda and tile.dtype == self._cdt() and tile.is_contiguous() and tile.shape[-1] == self.N
-        batch = tile.numel() // self.N
+        self._need(tile, self._cdt(), "tile", last=self.N)
+        batch = self._batch(tile, self.N, "tile")
         out = t.empty((batch, self.N), dtype=self._rdt(), device=tile.device)
         _check(lib().qtam_dense_invert(self._h, tile.data_ptr(), batch, int(row), out.data_ptr(), self._stream()),
                "qtam_dense_invert")
@@ -234,8 +259,8 @@ class Plan:
 
     def threshold_rowmedian(self, coef, kappa=3.0):
         """in place"""
-        assert coef.is_cuda and coef.dtype == self._cdt() and coef.is_contiguous()
-        batch = coef.numel() // self.ctot
+        self._need(coef, self._cdt(), "coef")
+        batch = self._batch(coef, self.ctot, "coef")
         _check(lib().qtam_threshold_rowmedian(self._h, coef.data_ptr(), batch, float(kappa), self._stream()),
                "qtam_threshold_rowmedian")
         return coef
@@ -243,18 +268,19 @@ class Plan:
     def remodulate(self, coef, out=None):
         """decimated envelopes -> samples of the dense tiles (Eq. 10a); out may be coef (in place)"""
         t = self._torch()
-        assert coef.is_cuda and coef.dtype == self._cdt() and coef.is_contiguous()
-        batch = coef.numel() // self.ctot
+        self._need(coef, self._cdt(), "coef")
+        batch = self._batch(coef, self.ctot, "coef")
         if out is None:
             out = t.empty_like(coef)
+        self._need(out, self._cdt(), "out", numel=batch * self.ctot)
         _check(lib().qtam_remodulate(self._h, coef.data_ptr(), batch, out.data_ptr(), self._stream()), "qtam_remodulate")
         return out
 
     def instantaneous_frequency(self, coef):
         """[batch][ctot] real, Hz: circular forward difference of the unwrapped baseband phase plus the carrier"""
         t = self._torch()
-        assert coef.is_cuda and coef.dtype == self._cdt() and coef.is_contiguous()
-        batch = coef.numel() // self.ctot
+        self._need(coef, self._cdt(), "coef")
+        batch = self._batch(coef, self.ctot, "coef")
         out = t.empty((batch, self.ctot), dtype=self._rdt(), device=coef.device)
         _check(lib().qtam_instantaneous_frequency(self._h, coef.data_ptr(), batch, out.data_ptr(), self._stream()),
                "qtam_instantaneous_frequency")
@@ -263,9 +289,9 @@ class Plan:
     def gather_plane(self, coef, best):
         """[batch][max plane size]: plane best[b] of every segment, zero padded (optimal-selection mode)"""
         t = self._torch()
-        assert coef.is_cuda and coef.dtype == self._cdt() and coef.is_contiguous()
-        assert best.is_cuda and best.dtype == t.int32 and best.is_contiguous()
-        batch = coef.numel() // self.ctot
+        self._need(coef, self._cdt(), "coef")
+        batch = self._batch(coef, self.ctot, "coef")
+        self._need(best, t.int32, "best", numel=batch)
         out = t.empty((batch, int(lib().qtam_max_plane_coeffs(self._h))), dtype=self._cdt(), device=coef.device)
         _check(lib().qtam_gather_plane(self._h, coef.data_ptr(), batch, best.data_ptr(), out.data_ptr(), self._stream()),
                "qtam_gather_plane")
@@ -274,8 +300,10 @@ class Plan:
     def plane_metric(self, coef, metric="energy"):
         """(values[batch][n_planes], best[batch] int32) of the multi-Q scan's plane selection"""
         t = self._torch()
-        assert coef.is_cuda and coef.dtype == self._cdt() and coef.is_contiguous()
-        batch = coef.numel() // self.ctot
+        self._need(coef, self._cdt(), "coef")
+        batch = self._batch(coef, self.ctot, "coef")
+        if metric not in ("energy", "peak"):
+            raise ValueError(f"metric {metric!r}: expected 'energy' or 'peak'")
         vals = t.empty((batch, self.n_planes), dtype=self._rdt(), device=coef.device)
         best = t.empty((batch,), dtype=t.int32, device=coef.device)
         _check(lib().qtam_plane_metric(self._h, coef.data_ptr(), batch, {"energy": 0, "peak": 1}[metric],
@@ -289,13 +317,13 @@ class Plan:
         _check(lib().qtam_profile_enable(self._h, 1 if on else 0, max_launches), "qtam_profile_enable")
 
     def profile_read(self):
-        """[{name, launches, ms, algo_bytes}] since the last read (waits for the recorded events)"""
+        """[{name, launches, ms, algo_bytes, design_bytes}] since the last read (waits for the recorded events)"""
         buf = (KernelStat * 32)()
         n = lib().qtam_profile_read(self._h, buf, 32)
         if n < 0:
             raise QtamError(4, "qtam_profile_read")
         return [dict(name=buf[i].name.decode(), launches=int(buf[i].launches), ms=float(buf[i].ms),
-                     algo_bytes=float(buf[i].algo_bytes)) for i in range(n)]
+                     algo_bytes=float(buf[i].algo_bytes), design_bytes=float(buf[i].design_bytes)) for i in range(n)]
 
     # ---- host-buffer convenience (the end-to-end path bench.py times) ------------------------------
     def forward_host(self, x_pinned, coef_pinned, d_x, d_coef):

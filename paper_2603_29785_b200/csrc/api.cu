@@ -191,7 +191,6 @@ qtam_status build_fast(qtam_plan *p) {
   }
   p->n_tiny = (int)tiny.size();
   if (!upload(&p->d_tiny, tiny.data(), tiny.size(), tot)) return QTAM_ERR_ALLOC;
-  if (hp.ctot >= (int64_t(1) << 31)) return QTAM_ERR_UNSUPPORTED;
   if (!upload(&p->d_frows, frows.data(), frows.size(), tot)) return QTAM_ERR_ALLOC;
   p->h_frows = frows;
   if (!upload(&p->d_frows_fwd, frowsF.data(), frowsF.size(), tot)) return QTAM_ERR_ALLOC;
@@ -268,7 +267,7 @@ template <typename T> qtam_status build_device(qtam_plan *p) {
     for (size_t k = 0; k < hp.rows.size(); ++k) {
       const int lm = ilog2(hp.rows[k].M);
       if (p->fast_rows && lm <= 10) continue;   // handled by fast.cu (32..1024: warp engine; < 32: one thread per row)
-      if (p->fast_rows && lm >= kCtaLog2Min && lm <= kCtaLog2Max && hp.ctot < (int64_t(1) << 31)) continue;   // rows_cta.cu
+      if (p->fast_rows && lm >= kCtaLog2Min && lm <= kCtaLog2Max) continue;   // rows_cta.cu
       if (lm <= p->cap_log2) {
         const int c = generic_class_of(lm);
         items[c].push_back(WorkItem{(int)k, 0, 1, lm});
@@ -340,7 +339,9 @@ template <typename T> qtam_status build_device(qtam_plan *p) {
 }
 
 bool check_call(const qtam_plan *p, const void *a, const void *b, int batch) {
-  return p && !p->host_only && a && b && batch >= 0 && batch <= p->max_batch;
+  if (!(p && !p->host_only && a && b && batch >= 0 && batch <= p->max_batch)) return false;
+  cudaGetLastError();   // clear a stale error of an earlier (foreign) call: the launch checks below report only ours
+  return true;
 }
 
 }  // namespace
@@ -355,6 +356,8 @@ qtam_status qtam_plan_create(qtam_plan **out, double fs, int64_t N, const double
   if (!p) return QTAM_ERR_ALLOC;
   qtam_status s = build_host_plan(p->hp, fs, N, Q, nQ, fmin, fmax, spacing, dtype, opt);
   if (s != QTAM_OK) { delete p; return s; }
+  // the batch index is a grid dimension (y or z) of several kernels: 65535 at most
+  if (p->hp.opt.max_batch > 65535) { delete p; return QTAM_ERR_INVALID_ARG; }
   int ndev = 0;
   if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) { delete p; return QTAM_ERR_CUDA; }
   p->esz = dtype == QTAM_F32 ? 4 : 8;
@@ -368,16 +371,21 @@ qtam_status qtam_plan_create(qtam_plan **out, double fs, int64_t N, const double
         cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && sms > 0)
       p->num_sms = sms;
     const int lnc = ilog2(N) - 1;
-    p->fast_rows = dtype == QTAM_F32;
+    // the tuned float kernels keep coefficient offsets in 32-bit integers; a plan with more coefficients per
+    // segment runs every row in the generic kernels (64-bit offsets)
+    p->fast_rows = dtype == QTAM_F32 && p->hp.ctot < (int64_t(1) << 31);
     p->fast_long = dtype == QTAM_F32 && lnc >= 11 && lnc <= 14;
   }
+  cudaGetLastError();   // an error left behind by an earlier library call is not this plan's
   s = dtype == QTAM_F32 ? build_device<float>(p) : build_device<double>(p);
+  if (s == QTAM_OK) s = prepare_generic(p);
   if (s == QTAM_OK) s = build_thr_fast(p);
   if (s == QTAM_OK && p->fast_rows) s = build_fast(p);
   if (s == QTAM_OK && p->fast_rows) s = build_rows_cta(p);
   if (s == QTAM_OK && p->fast_long) s = build_long_tables(p);
   if (s == QTAM_OK && p->fast_rows) s = build_long_fft(p);
   if (s == QTAM_OK && p->fast_rows) s = build_inv_tiled(p);
+  if (s == QTAM_OK) s = prepare_fast(p);
   if (s != QTAM_OK) { free_plan(p); cudaGetLastError(); return s; }
   if (cudaDeviceSynchronize() != cudaSuccess) { free_plan(p); return QTAM_ERR_CUDA; }
   *out = p;
@@ -643,6 +651,7 @@ int qtam_profile_read(qtam_plan *p, qtam_kernel_stat *out, int capacity) {
     acc[r.kid].launches += 1;
     acc[r.kid].ms += (double)ms;
     acc[r.kid].algo_bytes += r.bytes;
+    acc[r.kid].design_bytes += r.design;
   }
   p->prof_used = 0;
   int n = 0;

@@ -35,10 +35,34 @@ constexpr int kThrFastLog2Max = 10;
 // CTA-level rows (rows_cta.cu): 2^11 .. 2^14 points in one shared-memory transform, up to 2^17 in 2, 4 or 8
 constexpr int kCtaLog2Min = 11, kCtaLog2Max = 17;
 constexpr int kCtaMaxMembers = 32;   // rows per leader (same centre bin and half-width) in rows_cta.cu
-struct ProfRec { int kid; double bytes; cudaEvent_t e0, e1; };
+struct ProfRec { int kid; double bytes, design; cudaEvent_t e0, e1; };
 }  // namespace qtam
 
-namespace qtam { constexpr int kSpecPad = 512; }   // zero bins kept on both sides of every segment's spectrum
+namespace qtam { constexpr int kSpecPad = 512; }
+
+// A failed launch is reported once and cleared (cudaGetLastError), so that one bad call does not poison every
+// later call on any plan; the compute entry points also clear whatever an earlier library left behind.
+#define QTAM_LAUNCH_CHECK()                                        \
+  do {                                                             \
+    if (cudaGetLastError() != cudaSuccess) return QTAM_ERR_CUDA;   \
+  } while (0)
+
+namespace qtam {
+// Launch configuration of one kernel instantiation, fixed when the plan is created (qtam_plan_create sets the
+// dynamic shared-memory limit and asks the occupancy calculator once; the compute calls only read this).
+struct KernelCfg { int occ = 0; size_t smem = 0; bool ready = false; };
+template <typename K> inline bool kernel_prepare(KernelCfg &c, K kernel, int threads, size_t smem) {
+  c.smem = smem; c.occ = 1; c.ready = false;
+  if (smem > 48 * 1024 &&
+      cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
+    return false;
+  int occ = 0;
+  if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kernel, threads, smem) != cudaSuccess) return false;
+  c.occ = occ < 1 ? 1 : occ;
+  c.ready = true;
+  return true;
+}
+}  // namespace qtam   // zero bins kept on both sides of every segment's spectrum
 
 struct qtam_plan {
   qtam::HostPlan hp;
@@ -133,6 +157,10 @@ struct qtam_plan {
   void *d_ptw_rows[4] = {nullptr, nullptr, nullptr, nullptr};   // pass tables per class
   void *d_twb[3] = {nullptr, nullptr, nullptr};                 // e^{2 pi i n/M}, n < 2^14, M = 2^15..2^17
 
+  // launch configurations fixed at plan creation (see KernelCfg)
+  qtam::KernelCfg cfg_r2c, cfg_reduce_c2r, cfg_rows_fwd, cfg_rows_thr, cfg_rows_inv, cfg_tiles, cfg_combine,
+      cfg_long_b, cfg_rows_cta[4][2];
+
   int last_launches = 0;
   // launch profile (qtam_profile_enable / qtam_profile_read)
   bool prof_on = false;
@@ -145,16 +173,20 @@ struct qtam_plan {
 namespace qtam {
 
 // Brackets one kernel launch: counts it and, when profiling is on, records CUDA events around it on
-// the launch stream.  `bytes` = algorithmic bytes of that launch.
+// the launch stream.  `bytes` = the COMPULSORY bytes of SURVEY.md 8(d) this launch moves (input samples read,
+// coefficients written / read, output samples written: what the method itself must move); `design` = everything
+// the launch moves by design (compulsory + spectrum, partial sums, band workspace, scratch); < 0: same as bytes.
 struct LaunchScope {
   qtam_plan *p; cudaStream_t st; int slot;
-  LaunchScope(qtam_plan *plan, cudaStream_t stream, int kid, double bytes) : p(plan), st(stream), slot(-1) {
+  LaunchScope(qtam_plan *plan, cudaStream_t stream, int kid, double bytes, double design = -1.0)
+      : p(plan), st(stream), slot(-1) {
     p->last_launches += 1;
     if (!p->prof_on) return;
     if (p->prof_used >= (int)p->prof_pool.size()) { p->prof_dropped += 1; return; }
     slot = p->prof_used++;
     p->prof_pool[(size_t)slot].kid = kid;
     p->prof_pool[(size_t)slot].bytes = bytes;
+    p->prof_pool[(size_t)slot].design = design < 0.0 ? bytes : design;
     cudaEventRecord(p->prof_pool[(size_t)slot].e0, st);
   }
   ~LaunchScope() { if (slot >= 0) cudaEventRecord(p->prof_pool[(size_t)slot].e1, st); }
@@ -179,6 +211,8 @@ qtam_status generic_threshold(qtam_plan *p, void *d_coef, int batch, double kapp
 
 // fast.cu
 qtam_status build_long_tables(qtam_plan *p);
+qtam_status prepare_fast(qtam_plan *p);
+qtam_status prepare_generic(qtam_plan *p);
 qtam_status fast_r2c(qtam_plan *p, const void *d_x, int batch, cudaStream_t st);
 qtam_status fast_forward_rows(qtam_plan *p, int batch, void *d_coef, cudaStream_t st);
 qtam_status fast_inverse_rows(qtam_plan *p, const void *d_coef, int batch, int plane, cudaStream_t st);
@@ -190,7 +224,7 @@ qtam_status build_long_fft(qtam_plan *p);
 bool fast_cfft_long_ok(const qtam_plan *p, int log2n);
 qtam_status fast_cfft_long(qtam_plan *p, const void *in, long long in_stride, void *out, long long out_stride,
                            void *tmp, long long tmp_stride, int log2n, int count, int dir, float scale,
-                           cudaStream_t st);
+                           cudaStream_t st, double algo_in, double algo_out);
 // scan.cu
 qtam_status plane_metric(qtam_plan *p, const void *d_coef, int batch, int metric, void *d_metric, int32_t *d_best,
                          cudaStream_t st);

@@ -12,7 +12,6 @@
 //   K4 k_reduce_c2r_fast a6-a8 one CTA per segment: segmented reduction over bins (fixed order, no
 //                              atomics), 1/P, Hermitian pre-processing and the long inverse FFT in smem
 // Rows of 2^11 .. 2^17 points run in rows_cta.cu, N = 2^16 .. 2^20 in long_fft.cu, double precision in generic.cu.
-#include <cstdlib>
 #include <type_traits>
 
 #include "cplx.cuh"
@@ -24,19 +23,7 @@
 
 namespace qtam {
 
-#define QTAM_LAUNCH_CHECK()                                         \
-  do {                                                              \
-    if (cudaPeekAtLastError() != cudaSuccess) return QTAM_ERR_CUDA; \
-  } while (0)
-
 extern __shared__ __align__(16) unsigned char qtam_fast_smem[];
-
-#ifndef QTAM_FWD_STORE
-#define QTAM_FWD_STORE(p, v) __stcs(p, v)
-#endif
-#ifndef QTAM_GROUP_INLINE
-#define QTAM_GROUP_INLINE __forceinline__
-#endif
 
 // --------------------------------------------------------------------------------------------------
 // K1: long R2C.  z[m] = x[2m] + i x[2m+1]; Z = FFT_Nc(z);
@@ -109,7 +96,7 @@ k_tiny_rows(const FastRow *__restrict__ tiny, int n_tiny, const float *__restric
 // warps read overlap in L1.
 // --------------------------------------------------------------------------------------------------
 template <int LOG2G, bool THRESH = false>
-__device__ QTAM_GROUP_INLINE void fwd_group(const FastBucket &B, const FastRow *__restrict__ frows, int seg, int grp,
+__device__ __forceinline__ void fwd_group(const FastBucket &B, const FastRow *__restrict__ frows, int seg, int grp,
                                        int lane, float2 *ex, const float2 *tw1,
                                        const float2 *__restrict__ spec, long long xstride,
                                        const float *__restrict__ fwinp, float2 *__restrict__ coef,
@@ -164,13 +151,13 @@ __device__ QTAM_GROUP_INLINE void fwd_group(const FastBucket &B, const FastRow *
 #pragma unroll
       for (int i = 0; i < F; ++i)
 #pragma unroll
-        for (int n2 = 0; n2 < G; ++n2) QTAM_FWD_STORE(dst + G * i + 32 * n2, v[i * G + n2]);
+        for (int n2 = 0; n2 < G; ++n2) __stcs(dst + G * i + 32 * n2, v[i * G + n2]);
     }
   }
 }
 
 template <int LOG2G>
-__device__ QTAM_GROUP_INLINE void inv_group(const FastBucket &B, const FastRow *__restrict__ frows, int seg, int grp,
+__device__ __forceinline__ void inv_group(const FastBucket &B, const FastRow *__restrict__ frows, int seg, int grp,
                                           int lane, float2 *ex, const float2 *tw1,
                                           const float2 *__restrict__ coef, long long ctot, int nbins,
                                           const float *__restrict__ fwin, float2 *__restrict__ band,
@@ -306,15 +293,13 @@ k_reduce_c2r_fast(const float2 *__restrict__ band, long long sumL, const int32_t
 // --------------------------------------------------------------------------------------------------
 static int ilog2(long long v) { int l = 0; while ((1LL << l) < v) ++l; return l; }
 
-template <typename K> static bool set_smem(K kernel, size_t bytes) {
-  return cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes) == cudaSuccess;
-}
+constexpr int kRowWarps = 8;   // warps per CTA of k_rows_fast (two CTAs per SM)
 
 template <int LOG2NC> static qtam_status r2c_launch(qtam_plan *p, const void *d_x, int batch, cudaStream_t st) {
-  const size_t smem = sizeof(float2) * (size_t)cta_fft_smem_elems<LOG2NC>();
-  if (!set_smem(k_r2c_fast<LOG2NC>, smem)) return QTAM_ERR_CUDA;
+  const size_t smem = p->cfg_r2c.smem;
   {
-    LaunchScope ls(p, st, K_R2C_FAST, (double)batch * (4.0 * (double)p->hp.N + 8.0 * (double)p->hp.nb));
+    LaunchScope ls(p, st, K_R2C_FAST, (double)batch * 4.0 * (double)p->hp.N,
+                   (double)batch * (4.0 * (double)p->hp.N + 8.0 * (double)p->hp.nb));
     k_r2c_fast<LOG2NC><<<batch, CtaFftPlan<LOG2NC>::NT, smem, st>>>(
         static_cast<const float *>(d_x), static_cast<float2 *>(p->d_spec), p->xstride,
         static_cast<const float2 *>(p->d_tw), ilog2(p->twn), static_cast<const float2 *>(p->d_ptw));
@@ -357,27 +342,24 @@ static qtam_status rows_launch_nw(qtam_plan *p, int batch, const void *d_coef_in
   const FastParams &P = FORWARD ? p->fast_fwd : p->fast;
   if (tiny_rode) *tiny_rode = false;
   if (P.groups_per_seg == 0) return QTAM_OK;
-  const size_t smem = sizeof(float2) * (size_t)((P.tw_total + 1) & ~1) + sizeof(float2) * (size_t)NW * kExPerWarp +
-                      sizeof(FastRow) * (size_t)P.rows_smem;
+  const KernelCfg &cfg = FORWARD ? (THRESH ? p->cfg_rows_thr : p->cfg_rows_fwd) : p->cfg_rows_inv;
+  if (!cfg.ready) return QTAM_ERR_CUDA;
+  const size_t smem = cfg.smem;
   if ((long long)P.groups_per_seg * batch >= (1LL << 31)) return QTAM_ERR_UNSUPPORTED;
   auto kern = k_rows_fast<NW, FORWARD, THRESH>;
-  if (!set_smem(kern, smem)) return QTAM_ERR_CUDA;
-  int occ = 1;
-  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, NW * 32, smem);
-  if (occ < 1) occ = 1;
   const long long total = (long long)P.groups_per_seg * batch;
   long long want = (total + NW - 1) / NW;
-  const long long resident = (long long)p->num_sms * occ;
-  // a few waves of resident CTAs, each looping: keeps the tail short without losing the twiddle preload
-  static const int waves = getenv("QTAM_ROW_WAVES") ? atoi(getenv("QTAM_ROW_WAVES")) : 1;
-  int grid = (int)(want < resident * waves ? want : resident * waves);
+  const long long resident = (long long)p->num_sms * cfg.occ;
+  // one wave of resident CTAs, each looping over its items
+  int grid = (int)(want < resident ? want : resident);
   if (grid < 1) grid = 1;
   // the forward launch also takes the rows shorter than 32 points, one thread per (segment, row)
   const bool ride = FORWARD && p->n_tiny > 0;    // grid-stride loop in the kernel: any count rides
-  const double bytes = FORWARD ? (double)batch * 8.0 * (P.sum_M + (double)p->hp.nb + (ride ? p->tiny_sumM : 0.0))
-                               : (double)batch * 8.0 * (P.sum_M + P.sum_L);
+  // compulsory: the coefficients written (forward) or read (inverse); by design also the spectrum / the bands
+  const double bytes = (double)batch * 8.0 * (P.sum_M + (ride ? p->tiny_sumM : 0.0));
+  const double design = bytes + (double)batch * 8.0 * (FORWARD ? (double)p->hp.nb : P.sum_L);
   {
-    LaunchScope ls(p, st, FORWARD ? (THRESH ? K_FWD_ROWS_THR : K_FWD_ROWS_FAST) : K_INV_ROWS_FAST, bytes);
+    LaunchScope ls(p, st, FORWARD ? (THRESH ? K_FWD_ROWS_THR : K_FWD_ROWS_FAST) : K_INV_ROWS_FAST, bytes, design);
     kern<<<grid, NW * 32, smem, st>>>(
         P, FORWARD ? p->d_frows_fwd : p->d_frows, static_cast<const void *>(FORWARD ? p->d_ftw_fwd : p->d_ftw_inv),
         static_cast<const float *>(p->d_fwin), static_cast<const float *>(p->d_fwinp),
@@ -392,26 +374,10 @@ static qtam_status rows_launch_nw(qtam_plan *p, int batch, const void *d_coef_in
   return QTAM_OK;
 }
 
-static int row_warps() {
-  static int v = -1;
-  if (v < 0) {
-    const char *e = getenv("QTAM_ROW_WARPS");
-    v = e ? atoi(e) : 8;
-  }
-  return v;
-}
-
 template <bool FORWARD>
 static qtam_status rows_launch(qtam_plan *p, int batch, const void *d_coef_in, void *d_coef_out, int plane,
                                cudaStream_t st, bool *tiny_rode) {
-  switch (row_warps()) {
-    case 4: return rows_launch_nw<4, FORWARD>(p, batch, d_coef_in, d_coef_out, plane, st, tiny_rode);
-    case 12: return rows_launch_nw<12, FORWARD>(p, batch, d_coef_in, d_coef_out, plane, st, tiny_rode);
-    case 16: return rows_launch_nw<16, FORWARD>(p, batch, d_coef_in, d_coef_out, plane, st, tiny_rode);
-    case 20: return rows_launch_nw<20, FORWARD>(p, batch, d_coef_in, d_coef_out, plane, st, tiny_rode);
-    case 24: return rows_launch_nw<24, FORWARD>(p, batch, d_coef_in, d_coef_out, plane, st, tiny_rode);
-    default: return rows_launch_nw<8, FORWARD>(p, batch, d_coef_in, d_coef_out, plane, st, tiny_rode);
-  }
+  return rows_launch_nw<kRowWarps, FORWARD>(p, batch, d_coef_in, d_coef_out, plane, st, tiny_rode);
 }
 
 template <bool FORWARD>
@@ -419,7 +385,8 @@ static qtam_status tiny_launch(qtam_plan *p, int batch, const void *d_coef, int 
   if (p->n_tiny == 0) return QTAM_OK;
   const long long total = (long long)p->n_tiny * batch;
   {
-    LaunchScope ls(p, st, FORWARD ? K_TINY_FWD : K_TINY_INV, (double)batch * 8.0 * (p->tiny_sumM + p->tiny_sumL));
+    LaunchScope ls(p, st, FORWARD ? K_TINY_FWD : K_TINY_INV, (double)batch * 8.0 * p->tiny_sumM,
+                   (double)batch * 8.0 * (p->tiny_sumM + p->tiny_sumL));
     k_tiny_rows<FORWARD><<<(unsigned)((total + 127) / 128), 128, 0, st>>>(
         p->d_tiny, p->n_tiny, static_cast<const float *>(p->d_fwin), static_cast<const float2 *>(p->d_spec),
         p->xstride, (int)p->hp.nb, const_cast<float2 *>(static_cast<const float2 *>(d_coef)), p->hp.ctot,
@@ -444,7 +411,7 @@ qtam_status fast_forward_rows_threshold(qtam_plan *p, int batch, void *d_coef, f
   const FastParams &P = p->fast_fwd;
   if (P.groups_per_seg == 0) return QTAM_OK;
   bool rode = false;
-  const qtam_status s = rows_launch_nw<8, true, true>(p, batch, nullptr, d_coef, -1, st, &rode, kappa);
+  const qtam_status s = rows_launch_nw<kRowWarps, true, true>(p, batch, nullptr, d_coef, -1, st, &rode, kappa);
   if (s != QTAM_OK) return s;
   if (p->n_tiny > 0 && !rode) return QTAM_ERR_UNSUPPORTED;   // cannot happen given the test above
   *done = true;
@@ -459,11 +426,10 @@ qtam_status fast_inverse_rows(qtam_plan *p, const void *d_coef, int batch, int p
 
 template <int LOG2NC>
 static qtam_status reduce_c2r_launch(qtam_plan *p, int batch, int plane, void *d_x_out, cudaStream_t st) {
-  const size_t smem = sizeof(float2) * (size_t)cta_fft_smem_elems<LOG2NC>();
-  if (!set_smem(k_reduce_c2r_fast<LOG2NC>, smem)) return QTAM_ERR_CUDA;
+  const size_t smem = p->cfg_reduce_c2r.smem;
   {
     const CsrSel cs = csr_select(p, plane);
-    LaunchScope ls(p, st, K_REDUCE_C2R_FAST,
+    LaunchScope ls(p, st, K_REDUCE_C2R_FAST, (double)batch * 4.0 * (double)p->hp.N,
                    (double)batch * (8.0 * (double)p->hp.sumL + 4.0 * (double)p->hp.N));
     k_reduce_c2r_fast<LOG2NC><<<batch, CtaFftPlan<LOG2NC>::NT, smem, st>>>(
         static_cast<const float2 *>(p->d_band), p->hp.sumL, cs.ptr, cs.idx,
@@ -472,6 +438,38 @@ static qtam_status reduce_c2r_launch(qtam_plan *p, int batch, int plane, void *d
         static_cast<float *>(d_x_out));
   }
   QTAM_LAUNCH_CHECK();
+  return QTAM_OK;
+}
+
+// launch configurations of this file's kernels, fixed at plan creation
+template <int LOG2NC> static bool prepare_long(qtam_plan *p) {
+  const size_t smem = sizeof(float2) * (size_t)cta_fft_smem_elems<LOG2NC>();
+  return kernel_prepare(p->cfg_r2c, k_r2c_fast<LOG2NC>, CtaFftPlan<LOG2NC>::NT, smem) &&
+         kernel_prepare(p->cfg_reduce_c2r, k_reduce_c2r_fast<LOG2NC>, CtaFftPlan<LOG2NC>::NT, smem);
+}
+
+qtam_status prepare_fast(qtam_plan *p) {
+  if (p->fast_long) {
+    bool ok = false;
+    switch (ilog2(p->hp.N) - 1) {
+      case 11: ok = prepare_long<11>(p); break;
+      case 12: ok = prepare_long<12>(p); break;
+      case 13: ok = prepare_long<13>(p); break;
+      case 14: ok = prepare_long<14>(p); break;
+      default: break;
+    }
+    if (!ok) return QTAM_ERR_CUDA;
+  }
+  if (p->fast_rows) {
+    auto smem_of = [](const FastParams &P) {
+      return sizeof(float2) * (size_t)((P.tw_total + 1) & ~1) + sizeof(float2) * (size_t)kRowWarps * kExPerWarp +
+             sizeof(FastRow) * (size_t)P.rows_smem;
+    };
+    if (!kernel_prepare(p->cfg_rows_fwd, k_rows_fast<kRowWarps, true, false>, kRowWarps * 32, smem_of(p->fast_fwd)) ||
+        !kernel_prepare(p->cfg_rows_thr, k_rows_fast<kRowWarps, true, true>, kRowWarps * 32, smem_of(p->fast_fwd)) ||
+        !kernel_prepare(p->cfg_rows_inv, k_rows_fast<kRowWarps, false, false>, kRowWarps * 32, smem_of(p->fast)))
+      return QTAM_ERR_CUDA;
+  }
   return QTAM_OK;
 }
 

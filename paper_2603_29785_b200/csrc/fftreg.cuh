@@ -66,11 +66,7 @@ __device__ __forceinline__ float2 twmul(float2 o) {
     // second factor fold into FMUL2's operand modifiers, (c, c) and (s, s) are scalar-broadcast operands
     constexpr float c = cos32(k);
     constexpr float s = DIR > 0 ? sin32(k) : -sin32(k);
-#ifdef QTAM_SCALAR_TWIDDLES
-    return make_float2(o.x * c - o.y * s, o.x * s + o.y * c);
-#else
     return pfma(o, make_float2(c, c), pmul(make_float2(-o.y, o.x), make_float2(s, s)));
-#endif
   }
 }
 

@@ -10,19 +10,12 @@
 // C46 :583), a3 short inverse FFT scaled (N*M)^(-1/2) (C47 :589), a4 row-median threshold
 // (BASELINE.json cfg 5), a5 per-row FFT + window + sqrt(N/M) (C49 :598), a6 sum over rows as a
 // segmented reduction over bins, a7 division by P (Eq. 11 :135), a8 long C2R, a9 dense tiles (C3 :377).
-#include <cstdlib>
-#include <cstdio>
 
 #include "cplx.cuh"
 #include "device_plan.hpp"
 #include "thrbits.cuh"
 
 namespace qtam {
-
-#define QTAM_LAUNCH_CHECK()                                   \
-  do {                                                        \
-    if (cudaPeekAtLastError() != cudaSuccess) return QTAM_ERR_CUDA; \
-  } while (0)
 
 // ---------------------------------------------------------------------------------------------------
 // Block-level Stockham FFT on `total` = S*M points in shared memory; S sequences of length
@@ -162,9 +155,11 @@ __global__ void k_cfft_seq(const C2<T> *__restrict__ in, long long in_stride, C2
   for (int i = threadIdx.x; i < n; i += blockDim.x) dst[i] = cscale(res[i], scale);
 }
 
-// four-step, step A: for a tile of Tc columns j2, FFT over j1 (stride N2), times w_Nc^{dir n1 j2}
+// four-step, step A: for a tile of Tc columns j2, FFT over j1 (stride N2), times w_Nc^{dir n1 j2}.
+// `in` may equal `out` (the dense path runs it in place: a CTA reads its whole address set into shared memory
+// before it stores to the same set, and CTAs touch disjoint sets), so neither pointer is __restrict__.
 template <typename T>
-__global__ void k_cfft_cols(const C2<T> *__restrict__ in, long long in_stride, C2<T> *__restrict__ out,
+__global__ void k_cfft_cols(const C2<T> *in, long long in_stride, C2<T> *out,
                             long long out_stride, int log2N1, int log2N2, int log2Tc, int dir,
                             const C2<T> *__restrict__ tw, int log2twn, int bufpts) {
   typedef C2<T> V;
@@ -445,6 +440,16 @@ template <typename K> static bool set_smem(K kernel, size_t bytes) {
   return cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes) == cudaSuccess;
 }
 
+constexpr int kThrCachePts = 8192;   // magnitudes k_threshold keeps in shared memory
+
+// dynamic shared-memory limits of this file's kernels, set once at plan creation (the largest any launch asks for)
+template <typename T> static bool prepare_t(const qtam_plan *p) {
+  const size_t fft = 2 * sizeof(C2<T>) * ((size_t)1 << p->cap_log2);
+  return set_smem(k_cfft_seq<T>, fft) && set_smem(k_cfft_cols<T>, fft) && set_smem(k_cfft_rows<T>, fft) &&
+         set_smem(k_fwd_rows<T>, fft) && set_smem(k_inv_rows<T>, fft) &&
+         set_smem(k_threshold<T>, sizeof(T) * (size_t)kThrCachePts);
+}
+
 // class c of the row kernels handles sub-transforms of up to 2^kClassLog2[c] points
 static const int kClassLog2[qtam_plan::kClasses] = {8, 10, 12, 13};
 static const int kClassThreads[qtam_plan::kClasses] = {64, 128, 256, 512};
@@ -457,13 +462,16 @@ int generic_class_of(int log2M2) {
 
 // complex FFT of `count` sequences of n = 2^log2n points: in -> out (tmp used when n > cap; tmp may
 // alias in, never out).  Strides in complex elements.  Unscaled times `scale`.
+// algo_in / algo_out: compulsory bytes the first pass reads / the last pass writes, for the
+// launch profile: the time series of the long R2C (in) or C2R (out); 0 for transforms of intermediates.
 template <typename T>
 static qtam_status cfft(qtam_plan *p, const C2<T> *in, long long in_stride, C2<T> *out,
                         long long out_stride, C2<T> *tmp, long long tmp_stride, int log2n, int count,
-                        int dir, T scale, cudaStream_t st) {
+                        int dir, T scale, cudaStream_t st, double algo_in = 0.0, double algo_out = 0.0) {
   if constexpr (sizeof(T) == 4) {
-    if (!getenv("QTAM_NO_FAST_LONG") && fast_cfft_long_ok(p, log2n) && tmp != out)
-      return fast_cfft_long(p, in, in_stride, out, out_stride, tmp, tmp_stride, log2n, count, dir, scale, st);
+    if (fast_cfft_long_ok(p, log2n) && tmp != out)
+      return fast_cfft_long(p, in, in_stride, out, out_stride, tmp, tmp_stride, log2n, count, dir, scale, st,
+                            algo_in, algo_out);
   }
   const int cap = p->cap_log2;
   const C2<T> *tw = static_cast<const C2<T> *>(p->d_tw);
@@ -471,10 +479,9 @@ static qtam_status cfft(qtam_plan *p, const C2<T> *in, long long in_stride, C2<T
   const int bufpts = 1 << cap;
   const size_t smem = 2 * sizeof(C2<T>) * (size_t)bufpts;
   if (log2n <= cap) {
-    if (!set_smem(k_cfft_seq<T>, smem)) return QTAM_ERR_CUDA;
     const int thr = log2n >= 10 ? 512 : (log2n >= 8 ? 128 : 64);
     {
-      LaunchScope ls(p, st, K_CFFT_SEQ, 2.0 * sizeof(C2<T>) * (double)count * (double)(1 << log2n));
+      LaunchScope ls(p, st, K_CFFT_SEQ, algo_in + algo_out, 2.0 * sizeof(C2<T>) * (double)count * (double)(1 << log2n));
       k_cfft_seq<T><<<count, thr, smem, st>>>(in, in_stride, out, out_stride, log2n, dir, tw, log2twn, scale, bufpts);
     }
     QTAM_LAUNCH_CHECK();
@@ -484,16 +491,15 @@ static qtam_status cfft(qtam_plan *p, const C2<T> *in, long long in_stride, C2<T
   if (l2 > cap) return QTAM_ERR_UNSUPPORTED;
   int ltc = cap - l1; if (ltc > l2) ltc = l2;
   int ltr = cap - l2; if (ltr > l1) ltr = l1;
-  if (!set_smem(k_cfft_cols<T>, smem) || !set_smem(k_cfft_rows<T>, smem)) return QTAM_ERR_CUDA;
   dim3 ga((1 << l2) >> ltc, count), gb((1 << l1) >> ltr, count);
   const double pass_bytes = 2.0 * sizeof(C2<T>) * (double)count * (double)(1LL << log2n);
   {
-    LaunchScope ls(p, st, K_CFFT_COLS, pass_bytes);
+    LaunchScope ls(p, st, K_CFFT_COLS, algo_in, pass_bytes);
     k_cfft_cols<T><<<ga, 512, smem, st>>>(in, in_stride, tmp, tmp_stride, l1, l2, ltc, dir, tw, log2twn, bufpts);
   }
   QTAM_LAUNCH_CHECK();
   {
-    LaunchScope ls(p, st, K_CFFT_ROWS, pass_bytes);
+    LaunchScope ls(p, st, K_CFFT_ROWS, algo_out, pass_bytes);
     k_cfft_rows<T><<<gb, 512, smem, st>>>(tmp, tmp_stride, out, out_stride, l1, l2, ltr, dir, tw, log2twn, scale, bufpts);
   }
   QTAM_LAUNCH_CHECK();
@@ -506,11 +512,11 @@ static qtam_status r2c_t(qtam_plan *p, const void *d_x, int batch, cudaStream_t 
   C2<T> *spec = static_cast<C2<T> *>(p->d_spec);
   C2<T> *ws = static_cast<C2<T> *>(p->d_ws);
   qtam_status s = cfft<T>(p, static_cast<const C2<T> *>(d_x), Nc, spec, p->xstride, ws, p->hp.N,
-                          ilog2(Nc), batch, -1, (T)1, st);
+                          ilog2(Nc), batch, -1, (T)1, st, (double)batch * sizeof(T) * (double)p->hp.N, 0.0);
   if (s != QTAM_OK) return s;
   dim3 g((Nc / 2 + 1 + 255) / 256, batch);
   {
-    LaunchScope ls(p, st, K_R2C_POST, 2.0 * sizeof(C2<T>) * (double)batch * (double)Nc);
+    LaunchScope ls(p, st, K_R2C_POST, 0.0, 2.0 * sizeof(C2<T>) * (double)batch * (double)Nc);
     k_r2c_post<T><<<g, 256, 0, st>>>(spec, p->xstride, Nc, static_cast<const C2<T> *>(p->d_tw));
   }
   QTAM_LAUNCH_CHECK();
@@ -529,11 +535,11 @@ static qtam_status fwd_rows_t(qtam_plan *p, int batch, void *d_coef, cudaStream_
     if (p->n_items_fwd[c] == 0) continue;
     const int bufpts = 1 << kClassLog2[c];
     const size_t smem = 2 * sizeof(C2<T>) * (size_t)bufpts;
-    if (!set_smem(k_fwd_rows<T>, smem)) return QTAM_ERR_CUDA;
     dim3 g(p->n_items_fwd[c], batch);
     {
       // reads the bands (L values per row), writes M coefficients per row
-      LaunchScope ls(p, st, K_FWD_ROWS, sizeof(C2<T>) * (double)batch * (p->class_L[c] + p->class_M[c]));
+      LaunchScope ls(p, st, K_FWD_ROWS, sizeof(C2<T>) * (double)batch * p->class_M[c],
+                     sizeof(C2<T>) * (double)batch * (p->class_L[c] + p->class_M[c]));
       k_fwd_rows<T><<<g, kClassThreads[c], smem, st>>>(
           p->d_rows, p->d_items_fwd[c], static_cast<const C2<T> *>(p->d_spec), p->xstride, (int)p->hp.nb,
           static_cast<const T *>(p->d_win), tw, log2twn, static_cast<C2<T> *>(d_coef), p->hp.ctot, bufpts,
@@ -544,7 +550,7 @@ static qtam_status fwd_rows_t(qtam_plan *p, int batch, void *d_coef, cudaStream_
   if (p->n_bigrows > 0) {
     dim3 g(((1 << p->cap_log2) + 255) / 256, p->n_bigrows, batch);
     {
-      LaunchScope ls(p, st, K_FWD_COMBINE, 2.0 * sizeof(C2<T>) * (double)batch * p->big_M);
+      LaunchScope ls(p, st, K_FWD_COMBINE, 0.0, 2.0 * sizeof(C2<T>) * (double)batch * p->big_M);
       k_fwd_combine<T><<<g, 256, 0, st>>>(p->d_rows, p->d_bigrows, p->cap_log2, tw, log2twn,
                                           static_cast<C2<T> *>(d_coef), p->hp.ctot);
     }
@@ -568,10 +574,10 @@ static qtam_status inv_rows_t(qtam_plan *p, const void *d_coef, int batch, int p
     if (n_it == 0) continue;
     const int bufpts = 1 << kClassLog2[c];
     const size_t smem = 2 * sizeof(C2<T>) * (size_t)bufpts;
-    if (!set_smem(k_inv_rows<T>, smem)) return QTAM_ERR_CUDA;
     dim3 g(n_it, batch);
     {
-      LaunchScope ls(p, st, K_INV_ROWS, sizeof(C2<T>) * (double)batch * (p->class_L[c] + p->class_M[c]));
+      LaunchScope ls(p, st, K_INV_ROWS, sizeof(C2<T>) * (double)batch * p->class_M[c],
+                     sizeof(C2<T>) * (double)batch * (p->class_L[c] + p->class_M[c]));
       k_inv_rows<T><<<g, kClassThreads[c], smem, st>>>(
           p->d_rows, lead ? p->d_items_fwd[c] : p->d_items[c], static_cast<const C2<T> *>(d_coef), p->hp.ctot,
           static_cast<const T *>(p->d_win), tw, log2twn, static_cast<C2<T> *>(p->d_band), p->hp.sumL,
@@ -591,7 +597,7 @@ template <typename T>
 static qtam_status inv_reduce_t(qtam_plan *p, int batch, int plane, cudaStream_t st) {
   dim3 g((unsigned)((p->hp.nb + 255) / 256), batch);
   {
-    LaunchScope ls(p, st, K_INV_REDUCE,
+    LaunchScope ls(p, st, K_INV_REDUCE, 0.0,
                    (double)batch * (sizeof(C2<T>) * ((double)p->hp.sumL + (double)p->hp.nb)));
     const CsrSel cs = csr_select(p, plane);
     k_inv_reduce<T><<<g, 256, 0, st>>>(static_cast<const C2<T> *>(p->d_band), p->hp.sumL, cs.ptr, cs.idx,
@@ -612,12 +618,12 @@ static qtam_status c2r_t(qtam_plan *p, int batch, void *d_x_out, cudaStream_t st
   C2<T> *spec = static_cast<C2<T> *>(p->d_spec);
   dim3 g((Nc / 2 + 1 + 255) / 256, batch);
   {
-    LaunchScope ls(p, st, K_C2R_PRE, 2.0 * sizeof(C2<T>) * (double)batch * (double)Nc);
+    LaunchScope ls(p, st, K_C2R_PRE, 0.0, 2.0 * sizeof(C2<T>) * (double)batch * (double)Nc);
     k_c2r_pre<T><<<g, 256, 0, st>>>(spec, p->xstride, Nc, static_cast<const C2<T> *>(p->d_tw));
   }
   QTAM_LAUNCH_CHECK();
   return cfft<T>(p, spec, p->xstride, static_cast<C2<T> *>(d_x_out), Nc, static_cast<C2<T> *>(p->d_ws),
-                 p->hp.N, ilog2(Nc), batch, +1, (T)1, st);
+                 p->hp.N, ilog2(Nc), batch, +1, (T)1, st, 0.0, (double)batch * sizeof(T) * (double)p->hp.N);
 }
 
 qtam_status generic_c2r(qtam_plan *p, int batch, void *d_x_out, cudaStream_t st) {
@@ -678,16 +684,19 @@ qtam_status generic_dense(qtam_plan *p, int batch, int row_begin, int row_end, v
 
 template <typename T>
 static qtam_status threshold_t(qtam_plan *p, void *d_coef, int batch, double kappa, int min_log2M, cudaStream_t st) {
-  const int cache_pts = 8192;
+  const int cache_pts = kThrCachePts;
   const size_t smem = sizeof(T) * (size_t)cache_pts;
-  if (!set_smem(k_threshold<T>, smem)) return QTAM_ERR_CUDA;
   dim3 g((unsigned)p->hp.rows.size(), batch);
   {
-    LaunchScope ls(p, st, K_THRESHOLD, 2.0 * sizeof(C2<T>) * (double)batch * (double)p->hp.ctot);
+    LaunchScope ls(p, st, K_THRESHOLD, 0.0, 2.0 * sizeof(C2<T>) * (double)batch * (double)p->hp.ctot);
     k_threshold<T><<<g, 256, smem, st>>>(p->d_rows, static_cast<C2<T> *>(d_coef), p->hp.ctot, (T)kappa, cache_pts, min_log2M);
   }
   QTAM_LAUNCH_CHECK();
   return QTAM_OK;
+}
+
+qtam_status prepare_generic(qtam_plan *p) {
+  return (p->esz == 4 ? prepare_t<float>(p) : prepare_t<double>(p)) ? QTAM_OK : QTAM_ERR_CUDA;
 }
 
 qtam_status generic_threshold(qtam_plan *p, void *d_coef, int batch, double kappa, int min_log2M, cudaStream_t st) {

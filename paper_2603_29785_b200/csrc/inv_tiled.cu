@@ -19,7 +19,6 @@
 // HBM traffic = coefficients in, time series out; the partial sums (about ΣL/3 values per segment) are
 // written and read back once and are meant to stay in L2.
 #include <algorithm>
-#include <cstdlib>
 #include <vector>
 
 #include "ctafft.cuh"
@@ -29,14 +28,10 @@
 
 namespace qtam {
 
-#define QTAM_LAUNCH_CHECK()                                         \
-  do {                                                              \
-    if (cudaPeekAtLastError() != cudaSuccess) return QTAM_ERR_CUDA; \
-  } while (0)
-
 extern __shared__ __align__(16) unsigned char qtam_tiled_smem[];
 
 static int ilog2(long long v) { int l = 0; while ((1LL << l) < v) ++l; return l; }
+static bool prepare_tiled(qtam_plan *p);   // launch configurations of the two kernels (end of this file)
 
 // --------------------------------------------------------------------------------------------------
 // host: tiles
@@ -45,10 +40,10 @@ qtam_status build_inv_tiled(qtam_plan *p) {
   const HostPlan &hp = p->hp;
   const FastParams &F = p->fast;
   p->tiled_inv = false;
-  if (!p->fast_long || getenv("QTAM_NO_TILED_INV")) return QTAM_OK;
+  if (!p->fast_long) return QTAM_OK;
   if (ilog2(hp.N) - 1 > 14 || p->n_tiny > 256) return QTAM_OK;
   for (const HostRow &h : hp.rows) if (h.M > 1024) return QTAM_OK;
-  const int max_pass = getenv("QTAM_TILE_PASSES") ? atoi(getenv("QTAM_TILE_PASSES")) : 12;
+  const int max_pass = 12;   // passes per tile: longer tiles mean fewer partial sums, shorter ones a finer schedule
   std::vector<TileRow> trows;
   std::vector<TileItem> items;
   std::vector<int2> tmem;                 // (coefficient offset, plane) of every member
@@ -141,6 +136,7 @@ qtam_status build_inv_tiled(qtam_plan *p) {
   if (!up(reinterpret_cast<void **>(&p->d_tmem), tmem.data(), tmem.size() * sizeof(int2))) return QTAM_ERR_ALLOC;
   if (!up(&p->d_part, nullptr, sizeof(float2) * (size_t)p->max_batch * (size_t)off)) return QTAM_ERR_ALLOC;
   if (!up(reinterpret_cast<void **>(&p->d_counter), nullptr, 256)) return QTAM_ERR_ALLOC;
+  if (!prepare_tiled(p)) return QTAM_ERR_CUDA;
   p->tiled_inv = true;
   return QTAM_OK;
 }
@@ -372,32 +368,22 @@ k_combine_c2r(const TileItem *__restrict__ items, int n_items, const float2 *__r
 // --------------------------------------------------------------------------------------------------
 // host side
 // --------------------------------------------------------------------------------------------------
-static int tile_warps() {
-  static int v = -1;
-  if (v < 0) {
-    const char *e = getenv("QTAM_TILE_WARPS");
-    v = e ? atoi(e) : 11;
-  }
-  return v;
-}
+constexpr int kTileWarps = 11;   // warps per CTA of k_inv_tiles: 18 KB of shared memory each, one CTA per SM
 
 template <int NW>
 static qtam_status tiles_launch(qtam_plan *p, const void *d_coef, int batch, int plane, cudaStream_t st) {
   const int twt = p->fast.tw_total;
-  const size_t smem = sizeof(float2) * ((size_t)((twt + 1) & ~1) + (size_t)NW * (kExPerWarp + kAccBins));
+  if (!p->cfg_tiles.ready) return QTAM_ERR_CUDA;
+  const size_t smem = p->cfg_tiles.smem;
   auto kern = k_inv_tiles<NW>;
-  if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
-    return QTAM_ERR_CUDA;
-  int occ = 1;
-  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, NW * 32, smem);
-  if (occ < 1) occ = 1;
   const long long total = (long long)p->n_titems * batch;
-  long long grid = (long long)p->num_sms * occ;
+  long long grid = (long long)p->num_sms * p->cfg_tiles.occ;
   if (grid * NW > total) grid = (total + NW - 1) / NW;
   if (grid < 1) grid = 1;
   if (cudaMemsetAsync(p->d_counter, 0, sizeof(unsigned int), st) != cudaSuccess) return QTAM_ERR_CUDA;
   {
-    LaunchScope ls(p, st, K_INV_TILES, (double)batch * 8.0 * (p->fast.sum_M + (double)p->part_stride));
+    LaunchScope ls(p, st, K_INV_TILES, (double)batch * 8.0 * p->fast.sum_M,
+                   (double)batch * 8.0 * (p->fast.sum_M + (double)p->part_stride));
     kern<<<(int)grid, NW * 32, smem, st>>>(
         p->d_titems, p->n_titems, p->d_trows, static_cast<const float2 *>(p->d_ftw_inv), twt,
         static_cast<const float *>(p->d_fwinp), static_cast<const float2 *>(d_coef), p->hp.ctot, batch, plane,
@@ -410,12 +396,12 @@ static qtam_status tiles_launch(qtam_plan *p, const void *d_coef, int batch, int
 template <int LOG2NC, int NT>
 static qtam_status combine_launch(qtam_plan *p, const void *d_coef, int batch, int plane, void *d_x_out,
                                   cudaStream_t st) {
-  const size_t smem = sizeof(float2) * ((size_t)cta_fft_smem_elems<LOG2NC>() + 32 * (size_t)p->n_tiny);
+  if (!p->cfg_combine.ready) return QTAM_ERR_CUDA;
+  const size_t smem = p->cfg_combine.smem;
   auto kern = k_combine_c2r<LOG2NC, NT>;
-  if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
-    return QTAM_ERR_CUDA;
   {
-    LaunchScope ls(p, st, K_COMBINE_C2R, (double)batch * (8.0 * (double)p->part_stride + 4.0 * (double)p->hp.N));
+    LaunchScope ls(p, st, K_COMBINE_C2R, (double)batch * (4.0 * (double)p->hp.N + 8.0 * p->tiny_sumM),
+                   (double)batch * (8.0 * ((double)p->part_stride + p->tiny_sumM) + 4.0 * (double)p->hp.N));
     kern<<<batch, NT, smem, st>>>(
         p->d_titems, p->n_titems, static_cast<const float2 *>(p->d_part), p->part_stride, p->d_tiny, p->n_tiny,
         static_cast<const float *>(p->d_fwin), static_cast<const float2 *>(d_coef), p->hp.ctot,
@@ -426,13 +412,25 @@ static qtam_status combine_launch(qtam_plan *p, const void *d_coef, int batch, i
   return QTAM_OK;
 }
 
-qtam_status tiled_inverse(qtam_plan *p, const void *d_coef, int batch, int plane, void *d_x_out, cudaStream_t st) {
-  qtam_status s;
-  switch (tile_warps()) {
-    case 5: s = tiles_launch<5>(p, d_coef, batch, plane, st); break;
-    case 8: s = tiles_launch<8>(p, d_coef, batch, plane, st); break;
-    default: s = tiles_launch<11>(p, d_coef, batch, plane, st); break;
+template <int LOG2NC, int NT> static bool prepare_combine(qtam_plan *p) {
+  const size_t smem = sizeof(float2) * ((size_t)cta_fft_smem_elems<LOG2NC>() + 32 * (size_t)p->n_tiny);
+  return kernel_prepare(p->cfg_combine, k_combine_c2r<LOG2NC, NT>, NT, smem);
+}
+
+static bool prepare_tiled(qtam_plan *p) {
+  const size_t smem = sizeof(float2) * ((size_t)((p->fast.tw_total + 1) & ~1) + (size_t)kTileWarps * (kExPerWarp + kAccBins));
+  if (!kernel_prepare(p->cfg_tiles, k_inv_tiles<kTileWarps>, kTileWarps * 32, smem)) return false;
+  switch (ilog2(p->hp.N) - 1) {
+    case 11: return prepare_combine<11, 256>(p);
+    case 12: return prepare_combine<12, 256>(p);
+    case 13: return prepare_combine<13, 256>(p);
+    case 14: return prepare_combine<14, 512>(p);
+    default: return false;
   }
+}
+
+qtam_status tiled_inverse(qtam_plan *p, const void *d_coef, int batch, int plane, void *d_x_out, cudaStream_t st) {
+  const qtam_status s = tiles_launch<kTileWarps>(p, d_coef, batch, plane, st);
   if (s != QTAM_OK) return s;
   switch (ilog2(p->hp.N) - 1) {
     case 11: return combine_launch<11, 256>(p, d_coef, batch, plane, d_x_out, st);

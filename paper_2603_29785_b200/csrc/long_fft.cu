@@ -12,19 +12,14 @@
 
 namespace qtam {
 
-#define QTAM_LAUNCH_CHECK()                                         \
-  do {                                                              \
-    if (cudaPeekAtLastError() != cudaSuccess) return QTAM_ERR_CUDA; \
-  } while (0)
-
 extern __shared__ __align__(16) unsigned char qtam_long_smem[];
 
 constexpr int kLongLog2N2 = 14;
 
 template <int LOG2R, int DIR>
 __global__ void __launch_bounds__(256)
-k_long_a(const float2 *__restrict__ in, long long in_stride, float2 *__restrict__ out, long long out_stride,
-         const float2 *__restrict__ tw, int tw_shift) {
+k_long_a(const float2 *in, long long in_stride, float2 *out, long long out_stride,
+         const float2 *__restrict__ tw, int tw_shift) {   // in may equal out: a thread loads its R points, then stores to the same R addresses
   constexpr int R = 1 << LOG2R, N2 = 1 << kLongLog2N2;
   const int j2 = blockIdx.x * 256 + threadIdx.x;
   const float2 *src = in + (size_t)blockIdx.y * in_stride + j2;
@@ -71,7 +66,7 @@ k_long_b(const float2 *__restrict__ in, long long in_stride, float2 *__restrict_
 template <int LOG2R>
 static qtam_status long_launch(qtam_plan *p, const float2 *in, long long in_stride, float2 *out,
                                long long out_stride, float2 *tmp, long long tmp_stride, int count, int dir,
-                               float scale, cudaStream_t st) {
+                               float scale, cudaStream_t st, double algo_in, double algo_out) {
   constexpr int NT = CtaFftPlan<kLongLog2N2>::NT;
   const int log2n = kLongLog2N2 + LOG2R;
   int log2twn = 0;
@@ -84,22 +79,15 @@ static qtam_status long_launch(qtam_plan *p, const float2 *in, long long in_stri
   const size_t smem = sizeof(float2) * (size_t)cta_fft_smem_elems<kLongLog2N2>();
   dim3 ga((1 << kLongLog2N2) / 256, count), gb(1 << LOG2R, count);
   {
-    LaunchScope ls(p, st, K_LONG_A, pass_bytes);
+    LaunchScope ls(p, st, K_LONG_A, algo_in, pass_bytes);
     if (dir < 0) k_long_a<LOG2R, -1><<<ga, 256, 0, st>>>(in, in_stride, tmp, tmp_stride, tw, tw_shift);
     else k_long_a<LOG2R, +1><<<ga, 256, 0, st>>>(in, in_stride, tmp, tmp_stride, tw, tw_shift);
   }
   QTAM_LAUNCH_CHECK();
   {
-    LaunchScope ls(p, st, K_LONG_B, pass_bytes);
-    if (dir < 0) {
-      if (cudaFuncSetAttribute(k_long_b<-1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
-        return QTAM_ERR_CUDA;
-      k_long_b<-1><<<gb, NT, smem, st>>>(tmp, tmp_stride, out, out_stride, LOG2R, ptw, scale);
-    } else {
-      if (cudaFuncSetAttribute(k_long_b<+1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
-        return QTAM_ERR_CUDA;
-      k_long_b<+1><<<gb, NT, smem, st>>>(tmp, tmp_stride, out, out_stride, LOG2R, ptw, scale);
-    }
+    LaunchScope ls(p, st, K_LONG_B, algo_out, pass_bytes);
+    if (dir < 0) k_long_b<-1><<<gb, NT, smem, st>>>(tmp, tmp_stride, out, out_stride, LOG2R, ptw, scale);
+    else k_long_b<+1><<<gb, NT, smem, st>>>(tmp, tmp_stride, out, out_stride, LOG2R, ptw, scale);
   }
   QTAM_LAUNCH_CHECK();
   return QTAM_OK;
@@ -111,15 +99,15 @@ bool fast_cfft_long_ok(const qtam_plan *p, int log2n) {
 
 qtam_status fast_cfft_long(qtam_plan *p, const void *in, long long in_stride, void *out, long long out_stride,
                            void *tmp, long long tmp_stride, int log2n, int count, int dir, float scale,
-                           cudaStream_t st) {
+                           cudaStream_t st, double algo_in, double algo_out) {
   const float2 *i = static_cast<const float2 *>(in);
   float2 *o = static_cast<float2 *>(out), *t = static_cast<float2 *>(tmp);
   switch (log2n - kLongLog2N2) {
-    case 1: return long_launch<1>(p, i, in_stride, o, out_stride, t, tmp_stride, count, dir, scale, st);
-    case 2: return long_launch<2>(p, i, in_stride, o, out_stride, t, tmp_stride, count, dir, scale, st);
-    case 3: return long_launch<3>(p, i, in_stride, o, out_stride, t, tmp_stride, count, dir, scale, st);
-    case 4: return long_launch<4>(p, i, in_stride, o, out_stride, t, tmp_stride, count, dir, scale, st);
-    case 5: return long_launch<5>(p, i, in_stride, o, out_stride, t, tmp_stride, count, dir, scale, st);
+    case 1: return long_launch<1>(p, i, in_stride, o, out_stride, t, tmp_stride, count, dir, scale, st, algo_in, algo_out);
+    case 2: return long_launch<2>(p, i, in_stride, o, out_stride, t, tmp_stride, count, dir, scale, st, algo_in, algo_out);
+    case 3: return long_launch<3>(p, i, in_stride, o, out_stride, t, tmp_stride, count, dir, scale, st, algo_in, algo_out);
+    case 4: return long_launch<4>(p, i, in_stride, o, out_stride, t, tmp_stride, count, dir, scale, st, algo_in, algo_out);
+    case 5: return long_launch<5>(p, i, in_stride, o, out_stride, t, tmp_stride, count, dir, scale, st, algo_in, algo_out);
     default: return QTAM_ERR_UNSUPPORTED;
   }
 }
@@ -133,6 +121,10 @@ qtam_status build_long_fft(qtam_plan *p) {
   if (cudaMalloc(&p->d_ptw_long, t.size() * sizeof(float)) != cudaSuccess) return QTAM_ERR_ALLOC;
   p->device_bytes += t.size() * sizeof(float);
   if (cudaMemcpy(p->d_ptw_long, t.data(), t.size() * sizeof(float), cudaMemcpyHostToDevice) != cudaSuccess)
+    return QTAM_ERR_CUDA;
+  const size_t smem = sizeof(float2) * (size_t)cta_fft_smem_elems<kLongLog2N2>();
+  if (cudaFuncSetAttribute(k_long_b<-1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess ||
+      cudaFuncSetAttribute(k_long_b<+1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
     return QTAM_ERR_CUDA;
   return QTAM_OK;
 }

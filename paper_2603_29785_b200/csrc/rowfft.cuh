@@ -20,11 +20,7 @@ template <int LOG2G, int DIR> struct RowFFT {
   static constexpr int M = 32 * G;
 
   static __device__ __forceinline__ float2 twmulx(float2 a, float2 w) {
-#ifdef QTAM_SCALAR_TWIDDLES
-    return make_float2(a.x * w.x - a.y * w.y, a.x * w.y + a.y * w.x);
-#else
     return pcmul(a, w);      // FMUL2 + FFMA2 (swap/negate and the broadcasts are operand modifiers)
-#endif
   }
   static __device__ __forceinline__ float scale_of(float2 w) { return w.x; }
 

@@ -25,11 +25,6 @@
 
 namespace qtam {
 
-#define QTAM_LAUNCH_CHECK()                                         \
-  do {                                                              \
-    if (cudaPeekAtLastError() != cudaSuccess) return QTAM_ERR_CUDA; \
-  } while (0)
-
 extern __shared__ __align__(16) unsigned char qtam_cta_smem[];
 
 static int ilog2(long long v) { int l = 0; while ((1LL << l) < v) ++l; return l; }
@@ -220,11 +215,16 @@ k_rows_cta(const int *__restrict__ rowidx, const int *__restrict__ memptr, const
 // host side
 // --------------------------------------------------------------------------------------------------
 template <int L2> static void fill_class_table(std::vector<float> &t) { fill_cta_fft_tables<L2, CtaFftPlan<L2>::NT>(t); }
+template <int L2> static bool prepare_class(qtam_plan *p, int c) {
+  const size_t smem = sizeof(float2) * (size_t)cta_fft_smem_elems<L2>();
+  return kernel_prepare(p->cfg_rows_cta[c][1], k_rows_cta<L2, true>, CtaFftPlan<L2>::NT, smem) &&
+         kernel_prepare(p->cfg_rows_cta[c][0], k_rows_cta<L2, false>, CtaFftPlan<L2>::NT, smem);
+}
 
 qtam_status build_rows_cta(qtam_plan *p) {
   const HostPlan &hp = p->hp;
   p->cta_rows = false;
-  if (!p->fast_rows || hp.ctot >= (int64_t(1) << 31)) return QTAM_OK;
+  if (!p->fast_rows) return QTAM_OK;
   auto up = [&](void **dst, const void *src, size_t bytes) -> bool {
     *dst = nullptr;
     if (cudaMalloc(dst, bytes ? bytes : 16) != cudaSuccess) return false;
@@ -270,12 +270,14 @@ qtam_status build_rows_cta(qtam_plan *p) {
     if (!up(reinterpret_cast<void **>(&p->d_cta_memptr[c]), memptr.data(), memptr.size() * sizeof(int))) return QTAM_ERR_ALLOC;
     if (!up(reinterpret_cast<void **>(&p->d_cta_mem[c]), mem.data(), mem.size() * sizeof(int))) return QTAM_ERR_ALLOC;
     std::vector<float> t;
+    bool ok = false;
     switch (L2) {
-      case 11: fill_class_table<11>(t); break;
-      case 12: fill_class_table<12>(t); break;
-      case 13: fill_class_table<13>(t); break;
-      default: fill_class_table<14>(t); break;
+      case 11: fill_class_table<11>(t); ok = prepare_class<11>(p, c); break;
+      case 12: fill_class_table<12>(t); ok = prepare_class<12>(p, c); break;
+      case 13: fill_class_table<13>(t); ok = prepare_class<13>(p, c); break;
+      default: fill_class_table<14>(t); ok = prepare_class<14>(p, c); break;
     }
+    if (!ok) return QTAM_ERR_CUDA;
     if (!up(&p->d_ptw_rows[c], t.data(), t.size() * sizeof(float))) return QTAM_ERR_ALLOC;
     p->cta_rows = true;
   }
@@ -313,15 +315,12 @@ template <int L2, bool FORWARD>
 static qtam_status rows_cta_launch(qtam_plan *p, int c, int batch, void *d_coef, int plane, cudaStream_t st) {
   if (p->n_cta_rows[c] == 0) return QTAM_OK;
   constexpr int NT = CtaFftPlan<L2>::NT;
-  const size_t smem = sizeof(float2) * (size_t)cta_fft_smem_elems<L2>();
+  const KernelCfg &cfg = p->cfg_rows_cta[c][FORWARD ? 1 : 0];
+  if (!cfg.ready) return QTAM_ERR_CUDA;
+  const size_t smem = cfg.smem;
   auto kern = k_rows_cta<L2, FORWARD>;
-  if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
-    return QTAM_ERR_CUDA;
-  int occ = 1;
-  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, NT, smem);
-  if (occ < 1) occ = 1;
   const long long total = (long long)p->n_cta_rows[c] * batch;
-  long long grid = std::min<long long>(total, (long long)p->num_sms * occ);
+  long long grid = std::min<long long>(total, (long long)p->num_sms * cfg.occ);
   // per-CTA scratch (rows longer than one transform) comes out of the plan's [max_batch][N] workspace
   long long stride = 0;
   if (c == 3 && p->cta_maxM > 0) {
@@ -331,10 +330,9 @@ static qtam_status rows_cta_launch(qtam_plan *p, int c, int batch, void *d_coef,
   }
   TwbTables tb;
   for (int b = 0; b < 3; ++b) tb.t[b] = static_cast<const float2 *>(p->d_twb[b]);
-  const double bytes = FORWARD ? (double)batch * 8.0 * (p->cta_sumM[c] + p->cta_sumL[c])
-                               : (double)batch * 8.0 * (p->cta_sumM[c] + p->cta_sumL[c]);
+  const double bytes = (double)batch * 8.0 * p->cta_sumM[c];     // compulsory: the coefficients
   {
-    LaunchScope ls(p, st, FORWARD ? K_ROWS_CTA_FWD : K_ROWS_CTA_INV, bytes);
+    LaunchScope ls(p, st, FORWARD ? K_ROWS_CTA_FWD : K_ROWS_CTA_INV, bytes, bytes + (double)batch * 8.0 * p->cta_sumL[c]);
     kern<<<(unsigned)grid, NT, smem, st>>>(
         p->d_cta_rowidx[c], p->d_cta_memptr[c], p->d_cta_mem[c], p->n_cta_rows[c], p->d_rows, static_cast<const float *>(p->d_win),
         static_cast<const float2 *>(p->d_spec), p->xstride, (int)p->hp.nb, static_cast<float2 *>(d_coef),

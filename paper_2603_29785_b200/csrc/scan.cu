@@ -10,11 +10,6 @@
 
 namespace qtam {
 
-#define QTAM_LAUNCH_CHECK()                                         \
-  do {                                                              \
-    if (cudaPeekAtLastError() != cudaSuccess) return QTAM_ERR_CUDA; \
-  } while (0)
-
 template <typename T> struct Vec4;
 template <> struct Vec4<float> { typedef float4 type; };
 template <> struct Vec4<double> { typedef double4 type; };

@@ -17,11 +17,6 @@
 
 namespace qtam {
 
-#define QTAM_LAUNCH_CHECK()                                         \
-  do {                                                              \
-    if (cudaPeekAtLastError() != cudaSuccess) return QTAM_ERR_CUDA; \
-  } while (0)
-
 static int ilog2(long long v) { int l = 0; while ((1LL << l) < v) ++l; return l; }
 
 qtam_status build_thr_fast(qtam_plan *p) {
@@ -114,7 +109,8 @@ static qtam_status thr_launch(qtam_plan *p, void *d_coef, int batch, double kapp
   double elems = 0;
   for (const HostRow &h : p->hp.rows) if (ilog2(h.M) <= kThrFastLog2Max) elems += (double)h.M;
   {
-    LaunchScope ls(p, st, K_THRESHOLD_FAST, 2.0 * sizeof(C2<T>) * (double)batch * elems);
+    // a separate threshold pass moves no compulsory bytes (zero extra when fused)
+    LaunchScope ls(p, st, K_THRESHOLD_FAST, 0.0, 2.0 * sizeof(C2<T>) * (double)batch * elems);
     k_threshold_fast<T, NW><<<(unsigned)((total + NW - 1) / NW), NW * 32, 0, st>>>(
         p->d_thr_tasks, p->n_thr_tasks, p->d_thr_offs, static_cast<C2<T> *>(d_coef), p->hp.ctot, batch, (T)kappa);
   }

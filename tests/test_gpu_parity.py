@@ -27,6 +27,18 @@ def worst_segment(got, want):
     return max(rel_l2(got[b], want[b]) for b in range(want.shape[0]))
 
 
+def worst_row(got, want, plan):
+    """largest per-(segment, row) relative L2 error: a short row (M = 4..16 is ~1/300 of a segment's energy)
+    cannot hide in the norm of the whole coefficient vector"""
+    offs = np.array([int(r.offset) for r in plan.rows], dtype=np.int64)
+    num = np.add.reduceat(np.abs(got - want) ** 2, offs, axis=-1)
+    den = np.add.reduceat(np.abs(want) ** 2, offs, axis=-1)
+    return float(np.sqrt((num / np.maximum(den, 1e-300)).max()))
+
+
+TOL_ROW = {"f64": 1e-11, "f32": 1e-4}
+
+
 def make_plans(args, dtype, max_batch, **kw):
     g = binding.Plan(args[0], args[1], args[2], args[3], args[4], args[5], dtype=dtype, max_batch=max_batch, **kw)
     r = RefPlan(args[0], args[1], args[2], args[3], args[4], args[5], **kw)
@@ -61,6 +73,7 @@ def test_small_forward_inverse_dense(args, dtype, ov):
     Yg = g.forward(dev(x)).cpu().numpy()
     Yr = r.forward(x64, engine=0)
     assert worst_segment(Yg, Yr) <= TOL[dtype]
+    assert worst_row(Yg, Yr, r) <= TOL_ROW[dtype]
     # inverse of the ORACLE's coefficients (so the two inverses see identical input)
     Yin = Yr.astype(np.complex128 if dtype == "f64" else np.complex64)
     for plane in range(-1, g.n_planes):
@@ -121,6 +134,7 @@ def test_config_fp32_forward_inverse(name, nseg, ov):
     Yg = g.forward(dev(x)).cpu().numpy()
     Yr = r.forward(x64, engine=1)
     assert worst_segment(Yg, Yr) <= 2e-5
+    assert worst_row(Yg, Yr, r) <= TOL_ROW["f32"]
     Yin = Yr.astype(np.complex64)
     xg = g.inverse(dev(Yin)).cpu().numpy()
     xr = r.inverse(Yin.astype(np.complex128), engine=1)
@@ -133,22 +147,26 @@ def test_config_fp32_forward_inverse(name, nseg, ov):
     assert worst_segment(xg, r.inverse(Yin.astype(np.complex128), plane=pl, engine=1)) <= 2e-5
 
 
-@pytest.mark.parametrize("name,ov", [("cfg2", 1.0), ("cfg3", 1.0), ("cfg3", 2.0), ("cfg5", 1.0), ("cfg4", 1.0)])
-def test_inverse_of_arbitrary_coefficients(name, ov):
+@pytest.mark.parametrize("name,ov,dtype", [("cfg2", 1.0, "f32"), ("cfg3", 1.0, "f32"), ("cfg3", 2.0, "f32"),
+                                           ("cfg5", 1.0, "f32"), ("cfg4", 1.0, "f32"), ("cfg5", 1.0, "f64"),
+                                           ("cfg1", 1.0, "f64")])
+def test_inverse_of_arbitrary_coefficients(name, ov, dtype):
     """The inverse is defined for any coefficient array (masked / edited tiles), not only
     for the image of the forward: rows of different Q-planes that share centre bin and window (the
-    clamped rows) carry DIFFERENT values here, so a path that merges such rows must add them."""
+    clamped rows) carry DIFFERENT values here, so a path that merges such rows must add them -- in both
+    precisions (the double-precision rows merge leaders and followers too)."""
     nseg = 1 if name == "cfg4" else 2
-    g, r = make_plans(inputs.plan_args(name), "f32", nseg, clamp_overlap=ov)
+    g, r = make_plans(inputs.plan_args(name), dtype, nseg, clamp_overlap=ov)
+    keys = [(int(a.kc), int(a.dk), int(a.M)) for a in g.rows]
+    assert len(set(keys)) < len(keys), "the plan has no identical rows: the merge would not be exercised"
     rng = np.random.default_rng(20260329 + g.ctot % 1000)
-    Yin = (rng.standard_normal((nseg, g.ctot)) + 1j * rng.standard_normal((nseg, g.ctot))).astype(np.complex64)
-    for plane in (-1, 0, g.n_planes - 1):
+    cdt = np.complex64 if dtype == "f32" else np.complex128
+    Yin = (rng.standard_normal((nseg, g.ctot)) + 1j * rng.standard_normal((nseg, g.ctot))).astype(cdt)
+    # joint, per plane, joint again: no state may survive in the workspaces between the calls
+    for plane in (-1, 0, g.n_planes - 1, -1):
         xg = g.inverse(dev(Yin), plane=plane).cpu().numpy()
         xr = r.inverse(Yin.astype(np.complex128), plane=plane, engine=1)
-        assert worst_segment(xg, xr) <= 2e-5, plane
-    # joint again after the per-plane calls: no state may survive in the workspaces
-    xg = g.inverse(dev(Yin), plane=-1).cpu().numpy()
-    assert worst_segment(xg, r.inverse(Yin.astype(np.complex128), plane=-1, engine=1)) <= 2e-5
+        assert worst_segment(xg, xr) <= TOL[dtype], plane
 
 
 @pytest.mark.parametrize("log2n", [16, 17, 18, 19])
@@ -284,6 +302,7 @@ def test_cfg4_long_segment(ov):
     Yg = g.forward(dev(x)).cpu().numpy()
     Yr = r.forward(x64, engine=1)
     assert worst_segment(Yg, Yr) <= 2e-5
+    assert worst_row(Yg, Yr, r) <= TOL_ROW["f32"]
     Yin = Yr.astype(np.complex64)
     xg = g.inverse(dev(Yin)).cpu().numpy()
     xr = r.inverse(Yin.astype(np.complex128), engine=1)
@@ -369,81 +388,87 @@ def test_inputs_are_not_modified_and_output_fully_written():
     assert torch.equal(out, c0) and not torch.isnan(xo).any()
 
 
-def test_gpu_linearity_and_frame_energy_at_full_batch():
-    """properties that hold at any size, on BASELINE config 3 at its full batch (256 x 16384) in the
-    launch configuration bench.py times, plus sampled segments against the oracle."""
-    name = "cfg3"
-    B = inputs.CONFIGS[name]["batch"]
-    g, r = make_plans(inputs.plan_args(name), "f32", B)
-    x = inputs.make_batch(name, batch=B)
-    dx = dev(x)
-    Y = g.forward(dx)
-    # sampled segments, element by element
-    for b in (0, 101, B - 1):
-        Yr = r.forward(x[b].astype(np.float64), engine=1)[0]
-        assert rel_l2(Y[b].cpu().numpy(), Yr) <= 2e-5
-    # frame energy identity P6 on every segment: sum|Y|^2 = (1/N) sum_f |X[f]|^2 P[f]
-    P, C = r.frame(-1)
-    X = np.fft.rfft(x.astype(np.float64), axis=-1)
-    want = (np.abs(X) ** 2 * P[None, :]).sum(axis=1) / g.N
-    got = (Y.abs().double() ** 2).sum(dim=1).cpu().numpy()
-    assert np.max(np.abs(got - want) / want) <= 1e-5
-    # linearity P5
-    a, b = 0.7, -1.9
-    comb = g.forward((a * dx[:8] + b * dx[8:16]).contiguous())
-    assert rel_l2(comb.cpu().numpy(), (a * Y[:8] + b * Y[8:16]).cpu().numpy()) <= 1e-5
-    # round trip on every segment
-    xr = g.inverse(Y).cpu().numpy()
-    proj = pi_c(x.astype(np.float64), C)
-    assert worst_segment(xr, proj) <= 1e-5
-
-
-def test_cfg5_full_batch_in_bench_configuration():
-    """BASELINE config 5 at its full batch (1024 x 4096) as bench.py launches it: forward, threshold and
-    inverse on sampled segments against the oracle (threshold bit for bit on the kernel's own coefficients),
-    the frame-energy identity on every segment before the threshold."""
-    name = "cfg5"
-    B = inputs.CONFIGS[name]["batch"]
-    g, r = make_plans(inputs.plan_args(name), "f32", B)
-    x = inputs.make_batch(name, batch=B)
-    Y = g.forward(dev(x))
+def _frame_energy_err(Y, x64, r, N):
+    """P6 on every segment: sum|Y|^2 = (1/N) sum_f |X[f]|^2 P[f]"""
     P, _ = r.frame(-1)
-    X = np.fft.rfft(x.astype(np.float64), axis=-1)
-    want = (np.abs(X) ** 2 * P[None, :]).sum(axis=1) / g.N
+    X = np.fft.rfft(x64, axis=-1)
+    want = (np.abs(X) ** 2 * P[None, :]).sum(axis=1) / N
     got = (Y.abs().double() ** 2).sum(dim=1).cpu().numpy()
-    assert np.max(np.abs(got - want) / want) <= 1e-5
-    sample = [0, 3, 517, B - 1]
-    Yh = Y.cpu().numpy()
-    for b in sample:
-        assert rel_l2(Yh[b], r.forward(x[b].astype(np.float64), engine=1)[0]) <= 2e-5
-    g.threshold_rowmedian(Y, 3.0)
-    Yt = Y.cpu().numpy()
-    want_thr = r.threshold_f32(Yh[sample], 3.0)
-    assert np.array_equal(Yt[sample].view(np.uint32), want_thr.view(np.uint32))
-    xg = g.inverse(Y).cpu().numpy()
-    xr = r.inverse(want_thr.astype(np.complex128), engine=1)
-    for i, b in enumerate(sample):
-        assert rel_l2(xg[b], xr[i]) <= 2e-5
+    return float(np.max(np.abs(got - want) / want))
 
 
-@pytest.mark.parametrize("name", ["cfg2", "cfg4"])
-def test_long_row_configs_full_batch_in_bench_configuration(name):
-    """BASELINE configs 2 and 4 at their full batch: sampled segments against the oracle, the frame-energy
-    identity and (cfg4) the round trip on every segment."""
+@pytest.mark.parametrize("name", ["cfg2", "cfg3", "cfg4", "cfg5"])
+def test_full_batch_every_segment_against_the_oracle(name):
+    """BASELINE configs 2-5 at their full batch, in the launch configuration bench.py times: EVERY segment is
+    compared with the oracle element by element -- the forward on the same input, the inverse (where the
+    configuration calls it) on the oracle's coefficients -- with a bound on the whole vector of every segment
+    and on every single row; then the round trip, the frame-energy identity P6 and linearity P5 as extras."""
     cfg = inputs.CONFIGS[name]
     B = cfg["batch"]
     g, r = make_plans(inputs.plan_args(name), "f32", B)
     x = inputs.make_batch(name, batch=B)
+    dx = dev(x)
+    Y = g.forward(dx)
+    xo = g.inverse(Y) if "inverse" in cfg["calls"] else None
+    Yin_dev = torch.empty_like(Y)
+    chunk = 4 if name == "cfg4" else 64
+    worst = worst_r = 0.0
+    for b0 in range(0, B, chunk):
+        b1 = min(B, b0 + chunk)
+        Yr = r.forward(x[b0:b1].astype(np.float64), engine=1)
+        Yg = Y[b0:b1].cpu().numpy()
+        worst = max(worst, worst_segment(Yg, Yr))
+        worst_r = max(worst_r, worst_row(Yg, Yr, r))
+        Yin_dev[b0:b1] = dev(Yr.astype(np.complex64))
+    assert worst <= 2e-5 and worst_r <= TOL_ROW["f32"], (worst, worst_r)
+    assert _frame_energy_err(Y, x.astype(np.float64), r, g.N) <= 1e-5
+    a, b = 0.7, -1.9
+    h = min(8, B // 2)
+    comb = g.forward((a * dx[:h] + b * dx[h:2 * h]).contiguous())
+    assert rel_l2(comb.cpu().numpy(), (a * Y[:h] + b * Y[h:2 * h]).cpu().numpy()) <= 1e-5
+    if xo is None:
+        return
+    # the inverse of the ORACLE's coefficients (rounded to complex64), every segment, at the full batch
+    xg = g.inverse(Yin_dev).cpu().numpy()
+    worst = 0.0
+    for b0 in range(0, B, chunk):
+        b1 = min(B, b0 + chunk)
+        xr = r.inverse(Yin_dev[b0:b1].cpu().numpy().astype(np.complex128), engine=1)
+        worst = max(worst, worst_segment(xg[b0:b1], xr))
+    assert worst <= 2e-5, worst
+    _, C = r.frame(-1)
+    assert worst_segment(xo.cpu().numpy(), pi_c(x.astype(np.float64), C)) <= 1e-5
+
+
+@pytest.mark.parametrize("dtype", ["f32", "f64"])
+def test_cfg5_denoise_chain_full_batch(dtype):
+    """BASELINE config 5 (complex64 plus the fp64 variant) at its full batch of 1024 segments, as bench.py
+    launches it: forward (every segment, every row), threshold bit for bit on the kernel's own coefficients
+    (every segment), inverse of the thresholded coefficients (every segment), and the fused
+    forward+threshold call = the two calls."""
+    name = "cfg5"
+    B = inputs.CONFIGS[name]["batch"]
+    g, r = make_plans(inputs.plan_args(name), dtype, B)
+    x = inputs.make_batch(name, batch=B, dtype=dtype).astype(np_rdt(dtype))
+    x64 = x.astype(np.float64)
     Y = g.forward(dev(x))
-    for b in (0, B - 1):
-        assert rel_l2(Y[b].cpu().numpy(), r.forward(x[b].astype(np.float64), engine=1)[0]) <= 2e-5
-    P, C = r.frame(-1)
-    X = np.fft.rfft(x.astype(np.float64), axis=-1)
-    want = (np.abs(X) ** 2 * P[None, :]).sum(axis=1) / g.N
-    got = (Y.abs().double() ** 2).sum(dim=1).cpu().numpy()
-    assert np.max(np.abs(got - want) / want) <= 1e-5
-    if "inverse" in cfg["calls"]:
-        assert worst_segment(g.inverse(Y).cpu().numpy(), pi_c(x.astype(np.float64), C)) <= 1e-5
+    Yh = Y.cpu().numpy()
+    Yr = r.forward(x64, engine=1)
+    assert worst_segment(Yh, Yr) <= TOL[dtype]
+    assert worst_row(Yh, Yr, r) <= TOL_ROW[dtype]
+    assert _frame_energy_err(Y, x64, r, g.N) <= (1e-5 if dtype == "f32" else 1e-12)
+    fused = g.forward_threshold(dev(x), 3.0)
+    g.threshold_rowmedian(Y, 3.0)
+    assert torch.equal(torch.view_as_real(fused), torch.view_as_real(Y))
+    Yt = Y.cpu().numpy()
+    want_thr = r.threshold_f32(Yh, 3.0) if dtype == "f32" else r.threshold(Yh, 3.0)
+    bits = np.uint32 if dtype == "f32" else np.uint64
+    assert np.array_equal(Yt.view(bits), want_thr.view(bits))
+    kept = float((Yt != 0).mean())
+    assert 1e-3 < kept < 0.05
+    xg = g.inverse(Y).cpu().numpy()
+    xr = r.inverse(want_thr.astype(np.complex128), engine=1)
+    assert worst_segment(xg, xr) <= TOL[dtype]
 
 
 @pytest.mark.parametrize("name,dtype", [("cfg3", "f32"), ("cfg1", "f64"), ("cfg2", "f32")])
@@ -566,7 +591,9 @@ def test_random_plan_shapes(case):
     x = inputs.white_noise(N, 1000 + i, batch=2).astype(np_rdt(dtype))
     x64 = x.astype(np.float64)
     Y = g.forward(dev(x))
-    assert worst_segment(Y.cpu().numpy(), r.forward(x64, engine=1)) <= TOL[dtype]
+    Yr = r.forward(x64, engine=1)
+    assert worst_segment(Y.cpu().numpy(), Yr) <= TOL[dtype]
+    assert worst_row(Y.cpu().numpy(), Yr, r) <= TOL_ROW[dtype]
     rng = np.random.default_rng(2000 + i)
     Yin = (rng.standard_normal((2, g.ctot)) + 1j * rng.standard_normal((2, g.ctot))).astype(Y.cpu().numpy().dtype)
     for plane in (-1, g.n_planes - 1):
