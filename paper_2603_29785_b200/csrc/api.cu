@@ -41,7 +41,7 @@ void free_plan(qtam_plan *p) {
   if (!p) return;
   if (p->host_only) { delete p; return; }
   cudaFree(p->d_rows); cudaFree(p->d_win); cudaFree(p->d_tw); cudaFree(p->d_invP);
-  cudaFree(p->d_csr_ptr); cudaFree(p->d_csr_idx); cudaFree(p->d_csrj_ptr); cudaFree(p->d_csrj_idx); cudaFree(p->d_plane_off);
+  cudaFree(p->d_csr_ptr); cudaFree(p->d_csr_idx); cudaFree(p->d_plane_off);
   for (int c = 0; c < qtam_plan::kClasses; ++c) { cudaFree(p->d_items[c]); cudaFree(p->d_items_fwd[c]); }
   cudaFree(p->d_gfol_ptr); cudaFree(p->d_gfol_off); cudaFree(p->d_gfol_woff);
   cudaFree(p->d_bigrows); cudaFree(p->d_spec_alloc); cudaFree(p->d_ws); cudaFree(p->d_band);
@@ -49,8 +49,10 @@ void free_plan(qtam_plan *p) {
   cudaFree(p->d_frows); cudaFree(p->d_fwin); cudaFree(p->d_ftw_fwd); cudaFree(p->d_ftw_inv);
   cudaFree(p->d_tiny); cudaFree(p->d_ptw); cudaFree(p->d_ptw_long); cudaFree(p->d_frows_fwd); cudaFree(p->d_fmem); cudaFree(p->d_tmem);
   cudaFree(p->d_thr_tasks); cudaFree(p->d_thr_offs);
-  for (int c = 0; c < 4; ++c) { cudaFree(p->d_cta_rowidx[c]); cudaFree(p->d_ptw_rows[c]); cudaFree(p->d_cta_memptr[c]); cudaFree(p->d_cta_mem[c]); }
-  for (int b = 0; b < 3; ++b) cudaFree(p->d_twb[b]);
+  for (int c = 0; c < kCtaClasses; ++c) { cudaFree(p->d_cta_lead[c]); cudaFree(p->d_ptw_rows[c]); cudaFree(p->d_cta_groups[c]); cudaFree(p->d_cta_mem[c]); }
+  for (int c = 0; c < kClClasses; ++c) { cudaFree(p->d_cl_lead[c]); cudaFree(p->d_cl_mem[c]); cudaFree(p->d_cl_groups[c]); cudaFree(p->d_cl_ftw[c]); }
+  cudaFree(p->d_cl_ptw[0]); cudaFree(p->d_cl_ptw[1]);
+  cudaFree(p->d_runs); cudaFree(p->d_run_ptr); cudaFree(p->d_run_idx);
   cudaFree(p->d_trows); cudaFree(p->d_titems); cudaFree(p->d_part); cudaFree(p->d_counter);
   for (ProfRec &r : p->prof_pool) { cudaEventDestroy(r.e0); cudaEventDestroy(r.e1); }
   delete p;
@@ -267,7 +269,7 @@ template <typename T> qtam_status build_device(qtam_plan *p) {
     for (size_t k = 0; k < hp.rows.size(); ++k) {
       const int lm = ilog2(hp.rows[k].M);
       if (p->fast_rows && lm <= 10) continue;   // handled by fast.cu (32..1024: warp engine; < 32: one thread per row)
-      if (p->fast_rows && lm >= kCtaLog2Min && lm <= kCtaLog2Max) continue;   // rows_cta.cu
+      if (p->fast_rows && lm >= kCtaLog2Min && lm <= kCtaLog2Max) continue;   // rows_cta.cu, rows_cluster.cu
       if (lm <= p->cap_log2) {
         const int c = generic_class_of(lm);
         items[c].push_back(WorkItem{(int)k, 0, 1, lm});
@@ -381,10 +383,13 @@ qtam_status qtam_plan_create(qtam_plan **out, double fs, int64_t N, const double
   if (s == QTAM_OK) s = prepare_generic(p);
   if (s == QTAM_OK) s = build_thr_fast(p);
   if (s == QTAM_OK && p->fast_rows) s = build_fast(p);
-  if (s == QTAM_OK && p->fast_rows) s = build_rows_cta(p);
   if (s == QTAM_OK && p->fast_long) s = build_long_tables(p);
   if (s == QTAM_OK && p->fast_rows) s = build_long_fft(p);
+  // the inverse's partial sums, in summation order: tiles, CTA groups, cluster groups (then the band slots)
   if (s == QTAM_OK && p->fast_rows) s = build_inv_tiled(p);
+  if (s == QTAM_OK && p->fast_rows) s = build_rows_cta(p);
+  if (s == QTAM_OK && p->fast_rows) s = build_rows_cluster(p);
+  if (s == QTAM_OK && p->fast_rows) s = build_runs(p);
   if (s == QTAM_OK) s = prepare_fast(p);
   if (s != QTAM_OK) { free_plan(p); cudaGetLastError(); return s; }
   if (cudaDeviceSynchronize() != cudaSuccess) { free_plan(p); return QTAM_ERR_CUDA; }
@@ -466,6 +471,10 @@ qtam_status qtam_forward(qtam_plan *p, const void *d_x, int batch, void *d_coef,
     s = cta_forward_rows(p, batch, d_coef, st);
     if (s != QTAM_OK) return s;
   }
+  if (p->cl_rows) {
+    s = cluster_forward_rows(p, batch, d_coef, st);
+    if (s != QTAM_OK) return s;
+  }
   return generic_forward_rows(p, batch, d_coef, st);
 }
 
@@ -488,6 +497,10 @@ qtam_status qtam_forward_threshold(qtam_plan *p, const void *d_x, int batch, dou
         s = cta_forward_rows(p, batch, d_coef, st);
         if (s != QTAM_OK) return s;
       }
+      if (p->cl_rows) {
+        s = cluster_forward_rows(p, batch, d_coef, st);
+        if (s != QTAM_OK) return s;
+      }
       s = generic_forward_rows(p, batch, d_coef, st);
       if (s != QTAM_OK || !p->thr_has_big) return s;
       return generic_threshold(p, d_coef, batch, kappa, kThrFastLog2Max + 1, st);   // rows longer than 1024 points
@@ -495,6 +508,7 @@ qtam_status qtam_forward_threshold(qtam_plan *p, const void *d_x, int batch, dou
     // not fusable for this plan / batch: the two steps one after the other
     s = fast_forward_rows(p, batch, d_coef, st);
     if (s == QTAM_OK && p->cta_rows) s = cta_forward_rows(p, batch, d_coef, st);
+    if (s == QTAM_OK && p->cl_rows) s = cluster_forward_rows(p, batch, d_coef, st);
     if (s == QTAM_OK) s = generic_forward_rows(p, batch, d_coef, st);
     if (s != QTAM_OK) return s;
     const int n1 = p->last_launches;
@@ -520,17 +534,21 @@ qtam_status qtam_inverse(qtam_plan *p, const void *d_coef, int batch, int plane,
   cudaStream_t st = static_cast<cudaStream_t>(stream);
   if (p->tiled_inv) return tiled_inverse(p, d_coef, batch, plane, d_x_out, st);
   qtam_status s = QTAM_OK;
-  if (p->fast_rows) {
-    s = fast_inverse_rows(p, d_coef, batch, plane, st);
+  if (p->use_runs) {
+    // float plans: every row kernel leaves its contributions as runs (tiles' and groups' partial sums, the band
+    // slots of the shortest rows); one pass adds them, applies 1/P and prepares the long C2R
+    s = p->tiles_ok ? tiles_only(p, d_coef, batch, plane, st) : fast_inverse_rows(p, d_coef, batch, plane, st);
+    if (s == QTAM_OK) s = fast_tiny_inverse(p, d_coef, batch, plane, st);
+    if (s == QTAM_OK && p->cta_rows) s = cta_inverse_rows(p, d_coef, batch, plane, st);
+    if (s == QTAM_OK && p->cl_rows) s = cluster_inverse_rows(p, d_coef, batch, plane, st);
+    if (s == QTAM_OK) s = generic_inverse_rows(p, d_coef, batch, plane, st);   // (no items on these plans)
+    if (s == QTAM_OK) s = combine_runs(p, batch, plane, st);
     if (s != QTAM_OK) return s;
-  }
-  if (p->cta_rows) {
-    s = cta_inverse_rows(p, d_coef, batch, plane, st);
-    if (s != QTAM_OK) return s;
+    if (p->fast_long) return fast_c2c_out(p, batch, d_x_out, st);
+    return generic_c2c_out(p, batch, d_x_out, st);
   }
   s = generic_inverse_rows(p, d_coef, batch, plane, st);
   if (s != QTAM_OK) return s;
-  if (p->fast_long) return fast_reduce_c2r(p, batch, plane, d_x_out, st);
   s = generic_inverse_reduce(p, batch, plane, st);
   if (s != QTAM_OK) return s;
   return generic_c2r(p, batch, d_x_out, st);
@@ -618,7 +636,8 @@ static const char *const kKernelNames[K_COUNT] = {
     "cfft_seq", "cfft_cols", "cfft_rows", "r2c_post", "c2r_pre", "fwd_rows", "fwd_combine",
     "inv_rows", "inv_reduce", "dense_place", "threshold", "r2c_fast", "fwd_rows_fast", "inv_rows_fast",
     "reduce_c2r_fast", "inv_fused", "inv_tiles", "combine_c2r", "threshold_fast", "rows_cta_fwd", "rows_cta_inv",
-    "tiny_rows_fwd", "tiny_rows_inv", "long_fft_a", "long_fft_b", "plane_metric", "best_plane", "remodulate", "inst_freq", "fwd_rows_thr", "gather_plane"};
+    "tiny_rows_fwd", "tiny_rows_inv", "long_fft_a", "long_fft_b", "plane_metric", "best_plane", "remodulate", "inst_freq", "fwd_rows_thr", "gather_plane",
+    "rows_cl_fwd", "rows_cl_inv", "combine_runs", "c2c_fast"};
 
 qtam_status qtam_profile_enable(qtam_plan *p, int on, int max_launches) {
   if (!p || p->host_only) return QTAM_ERR_INVALID_ARG;

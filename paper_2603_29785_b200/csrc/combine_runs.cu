@@ -1,0 +1,134 @@
+// combine_runs.cu -- a6 (last step) + a7 + the head of a8 for every float plan that is not on the tiled path:
+// the spectrum as the sum of RUNS.  The row kernels leave the inverse's contributions as contiguous pieces of
+// spectrum -- the tiles' partial sums (inv_tiled.cu), the groups' partial sums (rows_cta.cu, rows_cluster.cu) and
+// the band slots of the few rows that still write the band workspace (rows shorter than 32 points).  One pass
+// adds, for every bin, the runs that cover it in a fixed order (Eq. 11's sum over k, :135), multiplies by 1/P on
+// the cover set (C41 :558, C50 :602, R9) and applies the Hermitian pre-processing of the long C2R (row a8):
+//   Z[f] = E + i O,  E = (Xhat[f] + conj Xhat[Nc-f])/2,  O = (Xhat[f] - conj Xhat[Nc-f])/2 e^{+2 pi i f/N},
+// scaled 1/Nc, written to the spectrum buffer, from which the half-length complex FFT produces x.
+// A CTA takes a block of bins f and the mirrored block Nc - f; the runs that touch either are listed per block.
+#include <algorithm>
+#include <vector>
+
+#include "cplx.cuh"
+#include "device_plan.hpp"
+#include "fftreg.cuh"
+
+namespace qtam {
+
+constexpr int kRunBlock = 256;
+
+static int ilog2(long long v) { int l = 0; while ((1LL << l) < v) ++l; return l; }
+
+// sum of the runs of one list at bin f
+__device__ __forceinline__ float2 run_sum(const int4 *__restrict__ runs, const int *__restrict__ idx, int lo, int hi,
+                                          int f, int plane, const float2 *__restrict__ part,
+                                          const float2 *__restrict__ band) {
+  float2 acc = make_float2(0.f, 0.f);
+  for (int e = lo; e < hi; ++e) {
+    const int4 r = __ldg(runs + __ldg(idx + e));       // lo, nb, off, src | (plane + 1) << 1
+    const int rp = (r.w >> 1) - 1;
+    if (rp >= 0 && plane >= 0 && rp != plane) continue;
+    const unsigned d = (unsigned)(f - r.x);
+    if (d < (unsigned)r.y) acc = padd(acc, __ldcs(((r.w & 1) ? part : band) + (size_t)r.z + d));
+  }
+  return acc;
+}
+
+__global__ void __launch_bounds__(kRunBlock)
+k_combine_runs(const int4 *__restrict__ runs, const int *__restrict__ ptr, const int *__restrict__ idx,
+               const float2 *__restrict__ part, long long part_stride, const float2 *__restrict__ band,
+               long long sumL, const float *__restrict__ invP, int Nc, int plane, const float2 *__restrict__ tw,
+               int tw_shift, float2 *__restrict__ spec, long long xstride) {
+  const int b = blockIdx.x, seg = blockIdx.y;
+  const int f = b * kRunBlock + threadIdx.x;
+  if (f > Nc / 2) return;
+  const int g = Nc - f;
+  const float2 *ps = part + (size_t)seg * part_stride;
+  const float2 *bs = band + (size_t)seg * sumL;
+  float2 A = run_sum(runs, idx, ptr[2 * b], ptr[2 * b + 1], f, plane, ps, bs);
+  float2 B = run_sum(runs, idx, ptr[2 * b + 1], ptr[2 * b + 2], g, plane, ps, bs);
+  A = pscale(A, __ldg(invP + f));
+  B = pscale(B, __ldg(invP + g));
+  if (f == 0) { A.y = 0.f; B.y = 0.f; }
+  const float h = 0.5f / (float)Nc;
+  const float2 E = make_float2(h * (A.x + B.x), h * (A.y - B.y));
+  const float2 D = make_float2(h * (A.x - B.x), h * (A.y + B.y));
+  const float2 w = __ldg(tw + ((size_t)f << tw_shift));      // e^{+2 pi i f/N}
+  const float2 O = make_float2(D.x * w.x - D.y * w.y, D.x * w.y + D.y * w.x);
+  float2 *S = spec + (size_t)seg * xstride;
+  S[f] = make_float2(E.x - O.y, E.y + O.x);                          // E + i O
+  if (g != f && f != 0) S[g] = make_float2(E.x + O.y, -E.y + O.x);   // conj(E) + i conj(O)
+}
+
+// Run lists, the band-slot runs of the rows that no tile or group covers, and the partial-sum buffer (the tiles'
+// and the groups' pieces have been laid out by build_inv_tiled / build_rows_cta / build_rows_cluster).
+qtam_status build_runs(qtam_plan *p) {
+  const HostPlan &hp = p->hp;
+  p->use_runs = false;
+  auto up = [&](void **dst, const void *src, size_t bytes) -> bool {
+    *dst = nullptr;
+    if (cudaMalloc(dst, bytes ? bytes : 16) != cudaSuccess) return false;
+    p->device_bytes += bytes;
+    return !src || bytes == 0 || cudaMemcpy(*dst, src, bytes, cudaMemcpyHostToDevice) == cudaSuccess;
+  };
+  if (!p->fast_rows) return QTAM_OK;
+  if (p->part_stride >= (int64_t(1) << 31)) return QTAM_ERR_UNSUPPORTED;
+  if (!up(&p->d_part, nullptr, sizeof(float2) * (size_t)p->max_batch * (size_t)std::max<int64_t>(p->part_stride, 1)))
+    return QTAM_ERR_ALLOC;
+  if (p->tiled_inv) return QTAM_OK;
+  // band slots: rows shorter than 32 points (k_tiny_rows), and the rows of 32 .. 1024 points when no tiles exist
+  for (const HostRow &h : hp.rows) {
+    const int lm = ilog2(h.M);
+    if (!(lm < 5 || (lm <= 10 && !p->tiles_ok))) continue;
+    const int64_t lo = std::max<int64_t>(h.kc - h.dk, 0), hi = std::min<int64_t>(h.kc + h.dk, hp.nb - 1);
+    if (hi < lo) continue;
+    p->runs.push_back(HostRun{(int)lo, (int)(hi - lo + 1), h.goff + (lo - (h.kc - h.dk)), 0, h.plane});
+  }
+  const int Nc = (int)(hp.N / 2);
+  const int nblk = (Nc / 2 + 1 + kRunBlock - 1) / kRunBlock;
+  std::vector<int4> dev(p->runs.size());
+  for (size_t i = 0; i < p->runs.size(); ++i) {
+    const HostRun &r = p->runs[i];
+    dev[i] = make_int4(r.lo, r.nb, (int)r.off, r.src | ((r.plane + 1) << 1));
+  }
+  std::vector<int> ptr(2 * (size_t)nblk + 1, 0), idx;
+  for (int b = 0; b < nblk; ++b) {
+    const int f0 = b * kRunBlock, f1 = std::min(f0 + kRunBlock - 1, Nc / 2);    // bins f of the block
+    const int g0 = Nc - f1, g1 = Nc - f0;                                       // their mirrors
+    ptr[2 * (size_t)b] = (int)idx.size();
+    for (size_t i = 0; i < p->runs.size(); ++i)
+      if (p->runs[i].nb > 0 && p->runs[i].lo <= f1 && p->runs[i].lo + p->runs[i].nb - 1 >= f0) idx.push_back((int)i);
+    ptr[2 * (size_t)b + 1] = (int)idx.size();
+    for (size_t i = 0; i < p->runs.size(); ++i)
+      if (p->runs[i].nb > 0 && p->runs[i].lo <= g1 && p->runs[i].lo + p->runs[i].nb - 1 >= g0) idx.push_back((int)i);
+  }
+  ptr[2 * (size_t)nblk] = (int)idx.size();
+  p->n_run_blocks = nblk;
+  if (!up(reinterpret_cast<void **>(&p->d_runs), dev.data(), dev.size() * sizeof(int4))) return QTAM_ERR_ALLOC;
+  if (!up(reinterpret_cast<void **>(&p->d_run_ptr), ptr.data(), ptr.size() * sizeof(int))) return QTAM_ERR_ALLOC;
+  if (!up(reinterpret_cast<void **>(&p->d_run_idx), idx.data(), idx.size() * sizeof(int))) return QTAM_ERR_ALLOC;
+  p->use_runs = true;
+  return QTAM_OK;
+}
+
+qtam_status combine_runs(qtam_plan *p, int batch, int plane, cudaStream_t st) {
+  const int Nc = (int)(p->hp.N / 2);
+  const int tw_shift = ilog2(p->twn) - ilog2(p->hp.N);
+  if (tw_shift < 0) return QTAM_ERR_UNSUPPORTED;
+  double run_bins = 0;
+  for (const HostRun &r : p->runs) run_bins += (double)r.nb;
+  dim3 g((unsigned)p->n_run_blocks, (unsigned)batch);
+  {
+    LaunchScope ls(p, st, K_COMBINE_RUNS, 0.0, (double)batch * 8.0 * (run_bins + (double)p->hp.nb));
+    k_combine_runs<<<g, kRunBlock, 0, st>>>(
+        p->d_runs, p->d_run_ptr, p->d_run_idx, static_cast<const float2 *>(p->d_part), p->part_stride,
+        static_cast<const float2 *>(p->d_band), p->hp.sumL,
+        static_cast<const float *>(p->d_invP) + (size_t)(plane + 1) * (size_t)p->hp.nb, Nc, plane,
+        static_cast<const float2 *>(p->d_tw), tw_shift, static_cast<float2 *>(p->d_spec), p->xstride);
+  }
+  QTAM_LAUNCH_CHECK();
+  return QTAM_OK;
+}
+
+}  // namespace qtam

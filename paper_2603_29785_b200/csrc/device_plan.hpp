@@ -13,7 +13,8 @@ enum KernelId {
   K_CFFT_SEQ = 0, K_CFFT_COLS, K_CFFT_ROWS, K_R2C_POST, K_C2R_PRE, K_FWD_ROWS, K_FWD_COMBINE,
   K_INV_ROWS, K_INV_REDUCE, K_DENSE_PLACE, K_THRESHOLD, K_R2C_FAST, K_FWD_ROWS_FAST, K_INV_ROWS_FAST,
   K_REDUCE_C2R_FAST, K_INV_FUSED, K_INV_TILES, K_COMBINE_C2R, K_THRESHOLD_FAST, K_ROWS_CTA_FWD, K_ROWS_CTA_INV,
-  K_TINY_FWD, K_TINY_INV, K_LONG_A, K_LONG_B, K_PLANE_METRIC, K_BEST_PLANE, K_REMODULATE, K_INST_FREQ, K_FWD_ROWS_THR, K_GATHER_PLANE, K_COUNT
+  K_TINY_FWD, K_TINY_INV, K_LONG_A, K_LONG_B, K_PLANE_METRIC, K_BEST_PLANE, K_REMODULATE, K_INST_FREQ, K_FWD_ROWS_THR, K_GATHER_PLANE,
+  K_ROWS_CL_FWD, K_ROWS_CL_INV, K_COMBINE_RUNS, K_C2C_FAST, K_COUNT
 };
 // fast float path (fast.cu): rows with 32 <= M <= 1024, grouped by G = M/32 lanes per row
 struct FastRow { int kc, dk, woff, goff, offset, plane, wpad, pad; };   // wpad: offset into the padded window table
@@ -32,9 +33,20 @@ constexpr int kAccBins = 1280;
 // fast threshold (threshold_fast.cu): a warp task = up to 32/G rows of one length M = 32 G (or 32 rows of M < 32)
 struct ThrTask { int log2M, row0, nrows, pad; };
 constexpr int kThrFastLog2Max = 10;
-// CTA-level rows (rows_cta.cu): 2^11 .. 2^14 points in one shared-memory transform, up to 2^17 in 2, 4 or 8
-constexpr int kCtaLog2Min = 11, kCtaLog2Max = 17;
-constexpr int kCtaMaxMembers = 32;   // rows per leader (same centre bin and half-width) in rows_cta.cu
+// CTA-level rows (rows_cta.cu): 2^11 .. 2^13 points, one shared-memory transform per CTA;
+// cluster-level rows (rows_cluster.cu): 2^14 .. 2^17 points, one transform per thread-block cluster
+constexpr int kCtaLog2Min = 11, kCtaClasses = 3;
+constexpr int kClLog2Min = 14, kClClasses = 4;
+constexpr int kCtaLog2Max = kClLog2Min + kClClasses - 1;   // longest row of the tuned float kernels
+constexpr int kCtaMaxMembers = 32;   // rows per leader (same centre bin and half-width)
+// a leader = one set of identical rows (same centre bin and half-width: transformed once); a group = consecutive
+// leaders whose inverse contributions one CTA / cluster adds into one partial spectrum, in order
+struct ClLeader { int row, mem0, nmem, pad; };
+struct ClGroup { int lead0, nlead, lo, nb; long long part_off; };
+// a run = a contiguous piece of the spectrum held somewhere: `nb` bins from bin `lo` at element `off` of a
+// segment's partial-sum buffer (src 1) or band workspace (src 0); plane >= 0: only for the joint inverse and for
+// that plane's own (a band slot of one row).  k_combine_runs adds the runs that cover a bin in list order.
+struct HostRun { int lo, nb; long long off; int src, plane; };
 struct ProfRec { int kid; double bytes, design; cudaEvent_t e0, e1; };
 }  // namespace qtam
 
@@ -81,10 +93,6 @@ struct qtam_plan {
   int32_t *d_csr_idx = nullptr;
   long long max_plane_coeffs = 0;     // largest plane (coefficients), the row length of qtam_gather_plane's output
   long long *d_plane_off = nullptr;   // [nP+1] first coefficient of every plane (planes are contiguous)
-  // joint-inverse CSR without the band slots of follower rows (rows_cta.cu adds a set of identical rows
-  // into its leader's slot); one set per bin.  Null when the plan has no followers.
-  int32_t *d_csrj_ptr = nullptr;
-  int32_t *d_csrj_idx = nullptr;
   // generic-path work lists, one per smem size class
   static const int kClasses = 4;
   qtam::WorkItem *d_items[kClasses] = {nullptr, nullptr, nullptr, nullptr};
@@ -146,20 +154,34 @@ struct qtam_plan {
   int n_thr_tasks = 0;
   bool thr_has_big = false;       // some row is longer than 2^kThrFastLog2Max points (generic kernel)
 
-  // CTA-level rows (rows_cta.cu), one class per transform length 2^11 .. 2^14
+  // CTA-level rows (rows_cta.cu), one class per transform length 2^11 .. 2^13
   bool cta_rows = false;
-  int *d_cta_rowidx[4] = {nullptr, nullptr, nullptr, nullptr};   // one leader per set of identical rows
-  int *d_cta_memptr[4] = {nullptr, nullptr, nullptr, nullptr};   // members of leader i: d_cta_mem[memptr[i] .. memptr[i+1])
-  int *d_cta_mem[4] = {nullptr, nullptr, nullptr, nullptr};
-  int n_cta_rows[4] = {0, 0, 0, 0};
-  double cta_sumM[4] = {0, 0, 0, 0}, cta_sumL[4] = {0, 0, 0, 0};
-  int64_t cta_maxM = 0;           // longest row that needs the per-CTA scratch (0: none)
-  void *d_ptw_rows[4] = {nullptr, nullptr, nullptr, nullptr};   // pass tables per class
-  void *d_twb[3] = {nullptr, nullptr, nullptr};                 // e^{2 pi i n/M}, n < 2^14, M = 2^15..2^17
+  qtam::ClLeader *d_cta_lead[qtam::kCtaClasses] = {};   // one leader per set of identical rows, ascending centre bin
+  int *d_cta_mem[qtam::kCtaClasses] = {};               // members (row indices) of the leaders
+  qtam::ClGroup *d_cta_groups[qtam::kCtaClasses] = {};  // inverse: groups of consecutive leaders
+  int n_cta_rows[qtam::kCtaClasses] = {}, n_cta_groups[qtam::kCtaClasses] = {};
+  double cta_sumM[qtam::kCtaClasses] = {}, cta_sumL[qtam::kCtaClasses] = {};
+  void *d_ptw_rows[qtam::kCtaClasses] = {};             // pass tables per class
+  // cluster-level rows (rows_cluster.cu), one class per transform length 2^14 .. 2^17
+  bool cl_rows = false;
+  qtam::ClLeader *d_cl_lead[qtam::kClClasses] = {};
+  int *d_cl_mem[qtam::kClClasses] = {};
+  qtam::ClGroup *d_cl_groups[qtam::kClClasses] = {};
+  int n_cl_lead[qtam::kClClasses] = {}, n_cl_groups[qtam::kClClasses] = {};
+  double cl_sumM[qtam::kClClasses] = {}, cl_sumL[qtam::kClClasses] = {};
+  void *d_cl_ptw[2] = {nullptr, nullptr};               // pass tables of the 2048- and 4096-point sub-transforms
+  void *d_cl_ftw[qtam::kClClasses] = {};                // radix-F twiddles per class
+  // run-based combine (combine_runs.cu): the inverse of every float plan that is not on the tiled path
+  bool use_runs = false;
+  std::vector<qtam::HostRun> runs;                      // in summation order (tiles, CTA groups, cluster groups, band slots)
+  int4 *d_runs = nullptr;                               // (lo, nb, off, src | (plane + 1) << 1)
+  int *d_run_ptr = nullptr, *d_run_idx = nullptr;       // lists 2b (bins f) and 2b + 1 (mirror bins Nc - f) of block b
+  int n_run_blocks = 0;
+  bool tiles_ok = false;                                // rows of 32 .. 1024 points have tiles (k_inv_tiles)
 
   // launch configurations fixed at plan creation (see KernelCfg)
-  qtam::KernelCfg cfg_r2c, cfg_reduce_c2r, cfg_rows_fwd, cfg_rows_thr, cfg_rows_inv, cfg_tiles, cfg_combine,
-      cfg_long_b, cfg_rows_cta[4][2];
+  qtam::KernelCfg cfg_r2c, cfg_rows_fwd, cfg_rows_thr, cfg_rows_inv, cfg_tiles, cfg_combine,
+      cfg_rows_cta[qtam::kCtaClasses][2], cfg_rows_cl[qtam::kClClasses][2], cfg_c2c;
 
   int last_launches = 0;
   // launch profile (qtam_profile_enable / qtam_profile_read)
@@ -192,10 +214,9 @@ struct LaunchScope {
   ~LaunchScope() { if (slot >= 0) cudaEventRecord(p->prof_pool[(size_t)slot].e1, st); }
 };
 
-// which CSR a reduction over the band workspace walks: sets plo .. phi-1 of nsets per bin
+// which part of the CSR a reduction over the band workspace walks: sets plo .. phi-1 of nsets per bin
 struct CsrSel { const int32_t *ptr, *idx; int nsets, plo, phi; };
 inline CsrSel csr_select(const qtam_plan *p, int plane) {
-  if (plane < 0 && p->d_csrj_ptr) return CsrSel{p->d_csrj_ptr, p->d_csrj_idx, 1, 0, 1};
   return CsrSel{p->d_csr_ptr, p->d_csr_idx, p->hp.nP + 1, plane < 0 ? 0 : plane, plane < 0 ? p->hp.nP : plane + 1};
 }
 
@@ -205,6 +226,7 @@ qtam_status generic_forward_rows(qtam_plan *p, int batch, void *d_coef, cudaStre
 qtam_status generic_inverse_rows(qtam_plan *p, const void *d_coef, int batch, int plane, cudaStream_t st);
 qtam_status generic_inverse_reduce(qtam_plan *p, int batch, int plane, cudaStream_t st);
 qtam_status generic_c2r(qtam_plan *p, int batch, void *d_x_out, cudaStream_t st);
+qtam_status generic_c2c_out(qtam_plan *p, int batch, void *d_x_out, cudaStream_t st);
 qtam_status generic_dense(qtam_plan *p, int batch, int row_begin, int row_end, void *d_out, cudaStream_t st);
 qtam_status generic_dense_invert(qtam_plan *p, const void *d_tile, int batch, int row, void *d_x_out, cudaStream_t st);
 qtam_status generic_threshold(qtam_plan *p, void *d_coef, int batch, double kappa, int min_log2M, cudaStream_t st);
@@ -218,7 +240,8 @@ qtam_status fast_forward_rows(qtam_plan *p, int batch, void *d_coef, cudaStream_
 qtam_status fast_inverse_rows(qtam_plan *p, const void *d_coef, int batch, int plane, cudaStream_t st);
 qtam_status fast_forward_rows_threshold(qtam_plan *p, int batch, void *d_coef, float kappa, cudaStream_t st,
                                         bool *done);
-qtam_status fast_reduce_c2r(qtam_plan *p, int batch, int plane, void *d_x_out, cudaStream_t st);
+qtam_status fast_tiny_inverse(qtam_plan *p, const void *d_coef, int batch, int plane, cudaStream_t st);
+qtam_status fast_c2c_out(qtam_plan *p, int batch, void *d_x_out, cudaStream_t st);
 // long_fft.cu
 qtam_status build_long_fft(qtam_plan *p);
 bool fast_cfft_long_ok(const qtam_plan *p, int log2n);
@@ -233,14 +256,24 @@ qtam_status gather_plane(qtam_plan *p, const void *d_coef, int batch, const int3
 qtam_status remodulate(qtam_plan *p, const void *d_coef, int batch, void *d_out, cudaStream_t st);
 qtam_status instantaneous_frequency(qtam_plan *p, const void *d_coef, int batch, void *d_out, cudaStream_t st);
 // rows_cta.cu
+void build_leaders_and_groups(qtam_plan *p, const std::vector<int> &rows_in, int groups_wanted,
+                              std::vector<ClLeader> &lead, std::vector<int> &mem, std::vector<ClGroup> &groups);
 qtam_status build_rows_cta(qtam_plan *p);
 qtam_status cta_forward_rows(qtam_plan *p, int batch, void *d_coef, cudaStream_t st);
 qtam_status cta_inverse_rows(qtam_plan *p, const void *d_coef, int batch, int plane, cudaStream_t st);
+// rows_cluster.cu
+qtam_status build_rows_cluster(qtam_plan *p);
+qtam_status cluster_forward_rows(qtam_plan *p, int batch, void *d_coef, cudaStream_t st);
+qtam_status cluster_inverse_rows(qtam_plan *p, const void *d_coef, int batch, int plane, cudaStream_t st);
+// combine_runs.cu
+qtam_status build_runs(qtam_plan *p);
+qtam_status combine_runs(qtam_plan *p, int batch, int plane, cudaStream_t st);
 // threshold_fast.cu
 qtam_status build_thr_fast(qtam_plan *p);
 qtam_status fast_threshold(qtam_plan *p, void *d_coef, int batch, double kappa, cudaStream_t st);
 // inv_tiled.cu
 qtam_status build_inv_tiled(qtam_plan *p);
 qtam_status tiled_inverse(qtam_plan *p, const void *d_coef, int batch, int plane, void *d_x_out, cudaStream_t st);
+qtam_status tiles_only(qtam_plan *p, const void *d_coef, int batch, int plane, cudaStream_t st);
 
 }  // namespace qtam

@@ -9,9 +9,10 @@
 //                              (tinyrow.cuh); THRESH: the row-median threshold in the epilogue (thrselect.cuh)
 //   K3 k_rows_fast<.,false> a5 per-row forward FFT, sqrt(N/M), window; band values to the band workspace
 //                              (plans whose inverse does not run in inv_tiled.cu)
-//   K4 k_reduce_c2r_fast a6-a8 one CTA per segment: segmented reduction over bins (fixed order, no
-//                              atomics), 1/P, Hermitian pre-processing and the long inverse FFT in smem
-// Rows of 2^11 .. 2^17 points run in rows_cta.cu, N = 2^16 .. 2^20 in long_fft.cu, double precision in generic.cu.
+//   K4 k_c2c_fast        a8    one CTA per segment: the half-length complex FFT behind the long C2R for plans
+//                              whose spectrum comes out of k_combine_runs (N <= 2^15)
+// Rows of 2^11 .. 2^13 points run in rows_cta.cu, 2^14 .. 2^17 in rows_cluster.cu, N = 2^16 .. 2^20 in
+// long_fft.cu, double precision in generic.cu.
 #include <type_traits>
 
 #include "cplx.cuh"
@@ -250,42 +251,16 @@ k_rows_fast(FastParams P, const FastRow *frows, const void *__restrict__ tw1g_,
 }
 
 // --------------------------------------------------------------------------------------------------
-// K4: S[f] = sum of the bin's band values (CSR order = ascending row), Xhat = S/P on the cover set (R9),
-//     Z[f] = E + i O (E, O from Xhat[f], conj Xhat[Nc-f], e^{+2 pi i f/N}), scaled 1/Nc, then the long
-//     inverse FFT straight to x_out (row a8)
+// K4: the half-length complex FFT of the long C2R (row a8) for N <= 2^15, one CTA per segment: Z (already
+//     pre-processed by k_combine_runs) from the spectrum buffer straight to x_out
 // --------------------------------------------------------------------------------------------------
 template <int LOG2NC>
 __global__ void __launch_bounds__(CtaFftPlan<LOG2NC>::NT)
-k_reduce_c2r_fast(const float2 *__restrict__ band, long long sumL, const int32_t *__restrict__ ptr,
-                  const int32_t *__restrict__ idx, const float *__restrict__ invP, int nbins, int nsets,
-                  int plo, int phi, int plane, const float2 *__restrict__ tw, int log2twn,
-                  const float2 *__restrict__ ptw, float *__restrict__ x_out) {
+k_c2c_fast(const float2 *__restrict__ spec, long long xstride, const float2 *__restrict__ ptw, float *__restrict__ x_out) {
   constexpr int NC = 1 << LOG2NC, NT = CtaFftPlan<LOG2NC>::NT;
   float2 *s = reinterpret_cast<float2 *>(qtam_fast_smem);
-  const float2 *Gb = band + (size_t)blockIdx.x * sumL;
-  const float *ip = invP + (size_t)(plane + 1) * nbins;
-  for (int f = threadIdx.x; f <= NC; f += NT) {
-    const int lo = ptr[(size_t)f * nsets + plo], hi = ptr[(size_t)f * nsets + phi];
-    float2 acc = make_float2(0.f, 0.f);
-    for (int e = lo; e < hi; ++e) acc = padd(acc, Gb[idx[e]]);
-    s[f] = pscale(acc, ip[f]);
-  }
-  __syncthreads();
-  const float h = 0.5f / (float)NC;
-  for (int f = threadIdx.x; f <= NC / 2; f += NT) {
-    const int g = NC - f;
-    float2 A = s[f], B = s[g];
-    if (f == 0) { A.y = 0.f; B.y = 0.f; }
-    const float2 E = make_float2(h * (A.x + B.x), h * (A.y - B.y));
-    const float2 D = make_float2(h * (A.x - B.x), h * (A.y + B.y));
-    const float2 w = __ldg(tw + ((size_t)f << (log2twn - LOG2NC - 1)));
-    const float2 O = make_float2(D.x * w.x - D.y * w.y, D.x * w.y + D.y * w.x);
-    s[f] = make_float2(E.x - O.y, E.y + O.x);
-    if (g != f && f != 0) s[g] = make_float2(E.x + O.y, -E.y + O.x);
-  }
-  __syncthreads();
-  float2 *gout = reinterpret_cast<float2 *>(x_out) + (size_t)blockIdx.x * NC;
-  cta_fft<LOG2NC, NT, +1, false, true>(s, nullptr, gout, ptw, 1.f);
+  cta_fft<LOG2NC, NT, +1, true, true>(s, spec + (size_t)blockIdx.x * xstride,
+                                      reinterpret_cast<float2 *>(x_out) + (size_t)blockIdx.x * NC, ptw, 1.f);
 }
 
 // --------------------------------------------------------------------------------------------------
@@ -418,23 +393,21 @@ qtam_status fast_forward_rows_threshold(qtam_plan *p, int batch, void *d_coef, f
   return QTAM_OK;
 }
 
+// rows of 32 .. 1024 points to the band workspace (plans whose rows have no tiles)
 qtam_status fast_inverse_rows(qtam_plan *p, const void *d_coef, int batch, int plane, cudaStream_t st) {
-  const qtam_status s = rows_launch<false>(p, batch, d_coef, nullptr, plane, st, nullptr);
-  if (s != QTAM_OK) return s;
+  return rows_launch<false>(p, batch, d_coef, nullptr, plane, st, nullptr);
+}
+// rows shorter than 32 points to the band workspace
+qtam_status fast_tiny_inverse(qtam_plan *p, const void *d_coef, int batch, int plane, cudaStream_t st) {
   return tiny_launch<false>(p, batch, d_coef, plane, st);
 }
 
 template <int LOG2NC>
-static qtam_status reduce_c2r_launch(qtam_plan *p, int batch, int plane, void *d_x_out, cudaStream_t st) {
-  const size_t smem = p->cfg_reduce_c2r.smem;
+static qtam_status c2c_launch(qtam_plan *p, int batch, void *d_x_out, cudaStream_t st) {
   {
-    const CsrSel cs = csr_select(p, plane);
-    LaunchScope ls(p, st, K_REDUCE_C2R_FAST, (double)batch * 4.0 * (double)p->hp.N,
-                   (double)batch * (8.0 * (double)p->hp.sumL + 4.0 * (double)p->hp.N));
-    k_reduce_c2r_fast<LOG2NC><<<batch, CtaFftPlan<LOG2NC>::NT, smem, st>>>(
-        static_cast<const float2 *>(p->d_band), p->hp.sumL, cs.ptr, cs.idx,
-        static_cast<const float *>(p->d_invP), (int)p->hp.nb, cs.nsets, cs.plo, cs.phi, plane,
-        static_cast<const float2 *>(p->d_tw), ilog2(p->twn), static_cast<const float2 *>(p->d_ptw),
+    LaunchScope ls(p, st, K_C2C_FAST, (double)batch * 4.0 * (double)p->hp.N, (double)batch * 8.0 * (double)p->hp.N);
+    k_c2c_fast<LOG2NC><<<batch, CtaFftPlan<LOG2NC>::NT, p->cfg_c2c.smem, st>>>(
+        static_cast<const float2 *>(p->d_spec), p->xstride, static_cast<const float2 *>(p->d_ptw),
         static_cast<float *>(d_x_out));
   }
   QTAM_LAUNCH_CHECK();
@@ -445,7 +418,7 @@ static qtam_status reduce_c2r_launch(qtam_plan *p, int batch, int plane, void *d
 template <int LOG2NC> static bool prepare_long(qtam_plan *p) {
   const size_t smem = sizeof(float2) * (size_t)cta_fft_smem_elems<LOG2NC>();
   return kernel_prepare(p->cfg_r2c, k_r2c_fast<LOG2NC>, CtaFftPlan<LOG2NC>::NT, smem) &&
-         kernel_prepare(p->cfg_reduce_c2r, k_reduce_c2r_fast<LOG2NC>, CtaFftPlan<LOG2NC>::NT, smem);
+         kernel_prepare(p->cfg_c2c, k_c2c_fast<LOG2NC>, CtaFftPlan<LOG2NC>::NT, smem);
 }
 
 qtam_status prepare_fast(qtam_plan *p) {
@@ -473,12 +446,12 @@ qtam_status prepare_fast(qtam_plan *p) {
   return QTAM_OK;
 }
 
-qtam_status fast_reduce_c2r(qtam_plan *p, int batch, int plane, void *d_x_out, cudaStream_t st) {
+qtam_status fast_c2c_out(qtam_plan *p, int batch, void *d_x_out, cudaStream_t st) {
   switch (ilog2(p->hp.N) - 1) {
-    case 11: return reduce_c2r_launch<11>(p, batch, plane, d_x_out, st);
-    case 12: return reduce_c2r_launch<12>(p, batch, plane, d_x_out, st);
-    case 13: return reduce_c2r_launch<13>(p, batch, plane, d_x_out, st);
-    case 14: return reduce_c2r_launch<14>(p, batch, plane, d_x_out, st);
+    case 11: return c2c_launch<11>(p, batch, d_x_out, st);
+    case 12: return c2c_launch<12>(p, batch, d_x_out, st);
+    case 13: return c2c_launch<13>(p, batch, d_x_out, st);
+    case 14: return c2c_launch<14>(p, batch, d_x_out, st);
     default: return QTAM_ERR_UNSUPPORTED;
   }
 }

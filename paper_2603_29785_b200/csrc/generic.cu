@@ -626,6 +626,14 @@ static qtam_status c2r_t(qtam_plan *p, int batch, void *d_x_out, cudaStream_t st
                  p->hp.N, ilog2(Nc), batch, +1, (T)1, st, 0.0, (double)batch * sizeof(T) * (double)p->hp.N);
 }
 
+// the complex FFT alone, for a spectrum buffer that already holds the pre-processed Z (k_combine_runs)
+qtam_status generic_c2c_out(qtam_plan *p, int batch, void *d_x_out, cudaStream_t st) {
+  const int Nc = (int)(p->hp.N / 2);
+  return cfft<float>(p, static_cast<const float2 *>(p->d_spec), p->xstride, static_cast<float2 *>(d_x_out), Nc,
+                     static_cast<float2 *>(p->d_ws), p->hp.N, ilog2(Nc), batch, +1, 1.f, st, 0.0,
+                     (double)batch * 4.0 * (double)p->hp.N);
+}
+
 qtam_status generic_c2r(qtam_plan *p, int batch, void *d_x_out, cudaStream_t st) {
   return p->esz == 4 ? c2r_t<float>(p, batch, d_x_out, st) : c2r_t<double>(p, batch, d_x_out, st);
 }

@@ -40,9 +40,12 @@ qtam_status build_inv_tiled(qtam_plan *p) {
   const HostPlan &hp = p->hp;
   const FastParams &F = p->fast;
   p->tiled_inv = false;
-  if (!p->fast_long) return QTAM_OK;
-  if (ilog2(hp.N) - 1 > 14 || p->n_tiny > 256) return QTAM_OK;
-  for (const HostRow &h : hp.rows) if (h.M > 1024) return QTAM_OK;
+  p->tiles_ok = false;
+  if (!p->fast_rows || F.nbuckets == 0) return QTAM_OK;
+  // the whole inverse runs as tiles + k_combine_c2r when the long transform fits one CTA and no row is longer
+  // than 1024 points; otherwise the tiles are one of the sources of k_combine_runs (combine_runs.cu)
+  bool whole = p->fast_long && ilog2(hp.N) - 1 <= 14 && p->n_tiny <= 256;
+  for (const HostRow &h : hp.rows) if (h.M > 1024) whole = false;
   const int max_pass = 12;   // passes per tile: longer tiles mean fewer partial sums, shorter ones a finer schedule
   std::vector<TileRow> trows;
   std::vector<TileItem> items;
@@ -119,9 +122,11 @@ qtam_status build_inv_tiled(qtam_plan *p) {
     for (size_t i : order) sorted.push_back(items[i]);
     items.swap(sorted);
   }
-  int64_t off = 0;
-  for (TileItem &it : items) { it.part_off = (int)off; off += (it.nb + 1) & ~1; }   // 16-byte aligned slots
-  if (off * (int64_t)p->max_batch >= (int64_t(1) << 40)) return QTAM_OK;
+  int64_t off = p->part_stride;      // the tiles' partial sums open the per-segment partial-sum layout
+  for (TileItem &it : items) {
+    it.part_off = (int)off; off += (it.nb + 1) & ~1;                                // 16-byte aligned slots
+    p->runs.push_back(HostRun{it.lo, it.nb, it.part_off, 1, -1});
+  }
   p->part_stride = off;
   p->n_titems = (int)items.size();
   size_t *tot = &p->device_bytes;
@@ -134,10 +139,10 @@ qtam_status build_inv_tiled(qtam_plan *p) {
   if (!up(reinterpret_cast<void **>(&p->d_trows), trows.data(), trows.size() * sizeof(TileRow))) return QTAM_ERR_ALLOC;
   if (!up(reinterpret_cast<void **>(&p->d_titems), items.data(), items.size() * sizeof(TileItem))) return QTAM_ERR_ALLOC;
   if (!up(reinterpret_cast<void **>(&p->d_tmem), tmem.data(), tmem.size() * sizeof(int2))) return QTAM_ERR_ALLOC;
-  if (!up(&p->d_part, nullptr, sizeof(float2) * (size_t)p->max_batch * (size_t)off)) return QTAM_ERR_ALLOC;
   if (!up(reinterpret_cast<void **>(&p->d_counter), nullptr, 256)) return QTAM_ERR_ALLOC;
+  p->tiled_inv = whole;
   if (!prepare_tiled(p)) return QTAM_ERR_CUDA;
-  p->tiled_inv = true;
+  p->tiles_ok = true;
   return QTAM_OK;
 }
 
@@ -420,6 +425,7 @@ template <int LOG2NC, int NT> static bool prepare_combine(qtam_plan *p) {
 static bool prepare_tiled(qtam_plan *p) {
   const size_t smem = sizeof(float2) * ((size_t)((p->fast.tw_total + 1) & ~1) + (size_t)kTileWarps * (kExPerWarp + kAccBins));
   if (!kernel_prepare(p->cfg_tiles, k_inv_tiles<kTileWarps>, kTileWarps * 32, smem)) return false;
+  if (!p->tiled_inv) return true;
   switch (ilog2(p->hp.N) - 1) {
     case 11: return prepare_combine<11, 256>(p);
     case 12: return prepare_combine<12, 256>(p);
@@ -427,6 +433,11 @@ static bool prepare_tiled(qtam_plan *p) {
     case 14: return prepare_combine<14, 512>(p);
     default: return false;
   }
+}
+
+// the tiles alone: partial sums for k_combine_runs
+qtam_status tiles_only(qtam_plan *p, const void *d_coef, int batch, int plane, cudaStream_t st) {
+  return tiles_launch<kTileWarps>(p, d_coef, batch, plane, st);
 }
 
 qtam_status tiled_inverse(qtam_plan *p, const void *d_coef, int batch, int plane, void *d_x_out, cudaStream_t st) {

@@ -1,0 +1,343 @@
+// rows_cluster.cu -- rows of 2^14 .. 2^17 points (float): one thread-block CLUSTER per (segment, row), the row's
+// short FFT split over the cluster's CTAs with the engine of clfft.cuh.  Nothing but the compulsory bytes leaves
+// the chip: the intermediate of the split transform crosses between the CTAs through distributed shared memory.
+//
+//   forward (a2 + a3)  every CTA gathers its residues of the band, X[kc + jj] W_k[jj] (N M)^{-1/2} (A9 :323,
+//                      C46 :583, C47 :589), four consecutive bins every F bins, runs its four P-point
+//                      sub-transforms in shared memory, and after one cluster barrier takes the radix-F stage for
+//                      its P/CL values of nc: F inputs from the F/4 CTAs, F outputs Y[nc + P m] stored to every
+//                      member of the leader's set (identical rows are transformed once).
+//   inverse (a5 + a6)  the mirror image: the members' coefficient rows are added while they are loaded (Eq. 11's
+//                      sum over k by linearity), radix-F stage, scattered to the CTAs, P-point sub-transforms,
+//                      times sqrt(N/M) W_k (C49 :598), and ADDED into the partial spectrum of the leader's group:
+//                      a group is a run of leaders consecutive in centre bin that one cluster takes one after the
+//                      other, so every bin of the group's partial sum is updated in a fixed order by plain
+//                      read-modify-write from one cluster (cluster barriers order the updates): a segmented
+//                      reduction without atomics and without a band workspace.  The groups' partial sums are
+//                      added up, in a fixed order, by k_combine_runs (combine_runs.cu).
+// Classes: M = 4 P CL with P = 2048 (256 threads, two CTAs per SM) and CL = 2, 4, 8 for M = 2^14, 2^15, 2^16;
+// P = 4096 (512 threads), CL = 8 for M = 2^17.
+#include <cooperative_groups.h>
+
+#include <algorithm>
+#include <cmath>
+#include <vector>
+
+#include "clfft.cuh"
+#include "device_plan.hpp"
+
+namespace cg = cooperative_groups;
+
+namespace qtam {
+
+extern __shared__ __align__(16) unsigned char qtam_cl_smem[];
+
+static int ilog2(long long v) { int l = 0; while ((1LL << l) < v) ++l; return l; }
+
+__device__ __forceinline__ void cl_arrive() { asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory"); }
+__device__ __forceinline__ void cl_wait() { asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory"); }
+
+struct ClArgs {
+  const ClLeader *lead; const int *mem; int nlead;          // leaders of this class (ascending centre bin), members
+  const ClGroup *groups; int ngroups;                       // inverse: groups of consecutive leaders
+  const RowDev *rows; const float *win;
+  const float2 *spec; long long xstride; int nbins;
+  float2 *coef; long long ctot;
+  float2 *part; long long part_stride;
+  const float2 *ptw, *ftw;                                  // sub-transform pass tables; radix-F twiddles (rows 1, 4)
+  int batch, plane;
+};
+
+// band side of the forward: B[j] = X[kc + jj] W_k[jj] s at j = q + F jc (R6), zero off the support and off the
+// one-sided spectrum (R8)
+template <int LOG2P, int F> struct ClGather {
+  const float2 *__restrict__ X; const float *__restrict__ W; int kc, dk, nbins, q0; float scale;
+  __device__ __forceinline__ float2 operator()(int ja, int jc) const {
+    constexpr int P = 1 << LOG2P;
+    const int jj = q0 + ja + F * jc - (jc >= P / 2 ? F * P : 0);
+    const int f = kc + jj;
+    float2 v = make_float2(0.f, 0.f);
+    if (jj >= -dk && jj <= dk && (unsigned)f < (unsigned)nbins) v = pscale(__ldg(X + f), __ldg(W + jj) * scale);
+    return v;
+  }
+};
+
+template <int LOG2P, int LOG2CL, bool FWD>
+__global__ void __launch_bounds__(ClFft<LOG2P>::NT, LOG2P == 11 ? 2 : 1)
+k_rows_cluster(const ClArgs A) {
+  typedef ClFft<LOG2P> PL;
+  constexpr int P = PL::P, NT = PL::NT, CL = 1 << LOG2CL, F = 4 * CL;
+  constexpr int NCQ = P / CL;            // values of nc one CTA takes in the radix-F stage
+  constexpr int BPTF = NCQ / NT;         // ... per thread
+  static_assert(NCQ % NT == 0 && BPTF >= 1, "radix-F stage must divide among the threads");
+  cg::cluster_group cluster = cg::this_cluster();
+  const int crank = (int)cluster.block_rank();
+  const int cid = blockIdx.x >> LOG2CL, ncl = gridDim.x >> LOG2CL;
+  const int tid = threadIdx.x;
+  float2 *s = reinterpret_cast<float2 *>(qtam_cl_smem);
+  float2 *rs[CL];
+#pragma unroll
+  for (int jb = 0; jb < CL; ++jb) rs[jb] = cluster.map_shared_rank(s, jb);
+  __shared__ int s_nm;
+  __shared__ int s_off[kCtaMaxMembers];
+  bool pending = false;                  // a cluster-barrier arrive without its wait
+
+  if constexpr (FWD) {
+    const long long total = (long long)A.nlead * A.batch;
+    for (long long item = cid; item < total; item += ncl) {
+      const int seg = (int)(item / A.nlead);
+      const ClLeader L = A.lead[item - (long long)seg * A.nlead];
+      const RowDev r = A.rows[L.row];
+      __syncthreads();
+      if (tid == 0) {
+        for (int m = 0; m < L.nmem; ++m) s_off[m] = (int)A.rows[A.mem[L.mem0 + m]].offset;
+        s_nm = L.nmem;
+      }
+      __syncthreads();
+      const int nm = s_nm;
+      // sub-transforms: pass 1 straight from the spectrum
+      const ClGather<LOG2P, F> in{A.spec + (size_t)seg * A.xstride, A.win + r.woff + r.dk, r.kc, r.dk, A.nbins,
+                                  4 * crank, (float)r.fwd_scale};
+      auto before_write = [&]() { if (pending) { cl_wait(); pending = false; } };   // the others have read my last result
+      cl_pass<LOG2P, PL::R0, 0, +1, 2, true>(s, in, before_write, A.ptw);
+      __syncthreads();
+      cl_passes_23<LOG2P, +1>(s, A.ptw);
+      cl_arrive(); cl_wait();
+      // radix-F stage for nc = crank NCQ .. + NCQ
+      float2 *Yseg = A.coef + (size_t)seg * A.ctot;
+#pragma unroll 1
+      for (int u = 0; u < BPTF; ++u) {
+        const int nc = crank * NCQ + tid + NT * u;
+        float2 v[F];
+#pragma unroll
+        for (int jb = 0; jb < CL; ++jb) {
+          const float4 *src = reinterpret_cast<const float4 *>(rs[jb] + 4 * nc);
+          const float4 a = src[0], b = src[1];
+          v[4 * jb] = make_float2(a.x, a.y); v[4 * jb + 1] = make_float2(a.z, a.w);
+          v[4 * jb + 2] = make_float2(b.x, b.y); v[4 * jb + 3] = make_float2(b.z, b.w);
+        }
+        cl_twiddle<F>(v, __ldg(A.ftw + nc), __ldg(A.ftw + P + nc));
+        RegFFT<F, +1>::run(v);
+        for (int m = 0; m < nm; ++m) {
+          float2 *Y = Yseg + s_off[m] + nc;
+#pragma unroll
+          for (int mm = 0; mm < F; ++mm) __stcs(Y + mm * P, v[mm]);
+        }
+      }
+      cl_arrive(); pending = true;
+    }
+  } else {
+    const long long total = (long long)A.ngroups * A.batch;
+    for (long long item = cid; item < total; item += ncl) {
+      const int seg = (int)(item / A.ngroups);
+      const ClGroup Gp = A.groups[item - (long long)seg * A.ngroups];
+      float2 *pg = A.part + (size_t)seg * A.part_stride + Gp.part_off;
+      // the group's partial sum starts at zero (float4 stores: part_off and the padded length are even)
+      {
+        float4 *z = reinterpret_cast<float4 *>(pg);
+        const int n4 = ((Gp.nb + 1) & ~1) / 2;
+        for (int i = crank * NT + tid; i < n4; i += CL * NT) z[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+      }
+      const float2 *Yseg = A.coef + (size_t)seg * A.ctot;
+#pragma unroll 1
+      for (int l = 0; l < Gp.nlead; ++l) {
+        const ClLeader L = A.lead[Gp.lead0 + l];
+        const RowDev r = A.rows[L.row];
+        __syncthreads();
+        if (tid == 0) {
+          int n = 0;
+          for (int m = 0; m < L.nmem; ++m) {
+            const RowDev &rm = A.rows[A.mem[L.mem0 + m]];
+            if (A.plane < 0 || rm.plane == A.plane) s_off[n++] = (int)rm.offset;
+          }
+          s_nm = n;
+        }
+        __syncthreads();
+        const int nm = s_nm;
+        if (nm == 0) continue;           // the same decision in every CTA of the cluster
+        // radix-F stage on the sum of the members' rows, scattered to the CTA that owns the residue
+#pragma unroll 1
+        for (int u = 0; u < BPTF; ++u) {
+          const int nc = crank * NCQ + tid + NT * u;
+          float2 v[F];
+          {
+            const float2 *Y = Yseg + s_off[0] + nc;
+#pragma unroll
+            for (int mm = 0; mm < F; ++mm) v[mm] = __ldcs(Y + mm * P);
+          }
+          for (int m = 1; m < nm; ++m) {
+            const float2 *Y = Yseg + s_off[m] + nc;
+            float2 y[F];
+#pragma unroll
+            for (int mm = 0; mm < F; ++mm) y[mm] = __ldcs(Y + mm * P);
+#pragma unroll
+            for (int mm = 0; mm < F; ++mm) v[mm] = padd(v[mm], y[mm]);
+          }
+          RegFFT<F, -1>::run(v);
+          float2 w1 = __ldg(A.ftw + nc), w4 = __ldg(A.ftw + P + nc);
+          w1.y = -w1.y; w4.y = -w4.y;
+          cl_twiddle<F>(v, w1, w4);
+          if (pending) { cl_wait(); pending = false; }     // every CTA is done with the previous row's result
+#pragma unroll
+          for (int jb = 0; jb < CL; ++jb) {
+            float4 *dst = reinterpret_cast<float4 *>(rs[jb] + 4 * nc);
+            dst[0] = make_float4(v[4 * jb].x, v[4 * jb].y, v[4 * jb + 1].x, v[4 * jb + 1].y);
+            dst[1] = make_float4(v[4 * jb + 2].x, v[4 * jb + 2].y, v[4 * jb + 3].x, v[4 * jb + 3].y);
+          }
+        }
+        cl_arrive(); cl_wait();
+        // the four sub-transforms of this CTA's residues
+        cl_pass<LOG2P, PL::R0, 0, -1, 0, true>(s, ClNoMid{}, ClSyncMid{}, A.ptw);
+        __syncthreads();
+        cl_passes_23<LOG2P, -1>(s, A.ptw);
+        // G_k[jj] = sqrt(N/M) Bhat[jj] W_k[jj], added into the group's partial sum at bin kc + jj (R8 clip)
+        {
+          const int ja = tid & 3, ib = tid >> 2;
+          const float *W = A.win + r.woff + r.dk;
+          const float amp = (float)r.inv_amp;
+          float2 *pb = pg + (r.kc - Gp.lo);
+#pragma unroll 4
+          for (int jc = ib; jc < P; jc += NT / 4) {
+            const int jj = 4 * crank + ja + F * jc - (jc >= P / 2 ? F * P : 0);
+            const int f = r.kc + jj;
+            if (jj >= -r.dk && jj <= r.dk && (unsigned)f < (unsigned)A.nbins) {
+              const float2 old = __ldcg(pb + jj);
+              pb[jj] = pfma(s[4 * jc + ja], make_float2(amp * __ldg(W + jj), amp * __ldg(W + jj)), old);
+            }
+          }
+        }
+        cl_arrive(); pending = true;
+      }
+    }
+  }
+  if (pending) cl_wait();                // nobody leaves while a neighbour may still read its shared memory
+}
+
+// --------------------------------------------------------------------------------------------------
+// host side
+// --------------------------------------------------------------------------------------------------
+// class c = log2 M - kClLog2Min: (LOG2P, LOG2CL) = (11, 1), (11, 2), (11, 3), (12, 3)
+template <int LOG2P, int LOG2CL> static bool prepare_cl(qtam_plan *p, int c) {
+  typedef ClFft<LOG2P> PL;
+  const size_t smem = sizeof(float2) * (size_t)PL::SMEM_ELEMS;
+  for (int fwd = 0; fwd < 2; ++fwd) {
+    KernelCfg &cfg = p->cfg_rows_cl[c][fwd];
+    cfg.smem = smem; cfg.occ = 0; cfg.ready = false;
+    const void *kern = fwd ? (const void *)k_rows_cluster<LOG2P, LOG2CL, true> : (const void *)k_rows_cluster<LOG2P, LOG2CL, false>;
+    if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return false;
+    cudaLaunchConfig_t lc = {};
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeClusterDimension;
+    at[0].val.clusterDim.x = 1 << LOG2CL; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+    lc.gridDim = dim3((unsigned)(p->num_sms * 2 / (1 << LOG2CL)) << LOG2CL);
+    lc.blockDim = dim3(PL::NT); lc.dynamicSmemBytes = smem; lc.attrs = at; lc.numAttrs = 1;
+    int ncl = 0;
+    if (cudaOccupancyMaxActiveClusters(&ncl, kern, &lc) != cudaSuccess || ncl < 1) return false;
+    cfg.occ = ncl;                       // clusters that can be resident at once
+    cfg.ready = true;
+  }
+  return true;
+}
+
+qtam_status build_rows_cluster(qtam_plan *p) {
+  const HostPlan &hp = p->hp;
+  p->cl_rows = false;
+  if (!p->fast_rows) return QTAM_OK;
+  auto up = [&](void **dst, const void *src, size_t bytes) -> bool {
+    *dst = nullptr;
+    if (cudaMalloc(dst, bytes ? bytes : 16) != cudaSuccess) return false;
+    p->device_bytes += bytes;
+    return bytes == 0 || cudaMemcpy(*dst, src, bytes, cudaMemcpyHostToDevice) == cudaSuccess;
+  };
+  bool need_ptw[2] = {false, false};
+  for (int c = 0; c < kClClasses; ++c) {
+    const int lm = kClLog2Min + c;
+    const int64_t M = int64_t(1) << lm;
+    std::vector<int> idx;
+    for (size_t k = 0; k < hp.rows.size(); ++k)
+      if (hp.rows[k].M == M) { idx.push_back((int)k); p->cl_sumM[c] += (double)M; p->cl_sumL[c] += (double)hp.rows[k].L; }
+    p->n_cl_lead[c] = 0; p->n_cl_groups[c] = 0;
+    if (idx.empty()) continue;
+    std::vector<ClLeader> lead;
+    std::vector<int> mem;
+    std::vector<ClGroup> groups;
+    // about ten groups per class: (groups x segments) spreads over the resident clusters while the partial sums
+    // stay a fraction of the band values
+    build_leaders_and_groups(p, idx, 10, lead, mem, groups);
+    p->n_cl_lead[c] = (int)lead.size(); p->n_cl_groups[c] = (int)groups.size();
+    if (!up(reinterpret_cast<void **>(&p->d_cl_lead[c]), lead.data(), lead.size() * sizeof(ClLeader))) return QTAM_ERR_ALLOC;
+    if (!up(reinterpret_cast<void **>(&p->d_cl_mem[c]), mem.data(), mem.size() * sizeof(int))) return QTAM_ERR_ALLOC;
+    if (!up(reinterpret_cast<void **>(&p->d_cl_groups[c]), groups.data(), groups.size() * sizeof(ClGroup))) return QTAM_ERR_ALLOC;
+    std::vector<float> t;
+    fill_clfft_final(t, c == 3 ? 4096 : 2048, M);
+    if (!up(&p->d_cl_ftw[c], t.data(), t.size() * sizeof(float))) return QTAM_ERR_ALLOC;
+    need_ptw[c == 3 ? 1 : 0] = true;
+    bool ok = false;
+    switch (c) {
+      case 0: ok = prepare_cl<11, 1>(p, c); break;
+      case 1: ok = prepare_cl<11, 2>(p, c); break;
+      case 2: ok = prepare_cl<11, 3>(p, c); break;
+      default: ok = prepare_cl<12, 3>(p, c); break;
+    }
+    if (!ok) return QTAM_ERR_CUDA;
+    p->cl_rows = true;
+  }
+  for (int i = 0; i < 2; ++i) {
+    if (!need_ptw[i]) continue;
+    std::vector<float> t;
+    if (i == 0) fill_clfft_tables<11>(t); else fill_clfft_tables<12>(t);
+    if (!up(&p->d_cl_ptw[i], t.data(), t.size() * sizeof(float))) return QTAM_ERR_ALLOC;
+  }
+  return QTAM_OK;
+}
+
+template <int LOG2P, int LOG2CL, bool FWD>
+static qtam_status cl_launch(qtam_plan *p, int c, int batch, void *d_coef, int plane, cudaStream_t st) {
+  typedef ClFft<LOG2P> PL;
+  if (p->n_cl_lead[c] == 0) return QTAM_OK;
+  const KernelCfg &cfg = p->cfg_rows_cl[c][FWD ? 1 : 0];
+  if (!cfg.ready) return QTAM_ERR_CUDA;
+  ClArgs A{};
+  A.lead = p->d_cl_lead[c]; A.mem = p->d_cl_mem[c]; A.nlead = p->n_cl_lead[c];
+  A.groups = p->d_cl_groups[c]; A.ngroups = p->n_cl_groups[c];
+  A.rows = p->d_rows; A.win = static_cast<const float *>(p->d_win);
+  A.spec = static_cast<const float2 *>(p->d_spec); A.xstride = p->xstride; A.nbins = (int)p->hp.nb;
+  A.coef = static_cast<float2 *>(d_coef); A.ctot = p->hp.ctot;
+  A.part = static_cast<float2 *>(p->d_part); A.part_stride = p->part_stride;
+  A.ptw = static_cast<const float2 *>(p->d_cl_ptw[LOG2P == 12 ? 1 : 0]);
+  A.ftw = static_cast<const float2 *>(p->d_cl_ftw[c]);
+  A.batch = batch; A.plane = plane;
+  const long long items = (long long)(FWD ? A.nlead : A.ngroups) * batch;
+  const long long ncl = std::min<long long>(items, cfg.occ);
+  cudaLaunchConfig_t lc = {};
+  cudaLaunchAttribute at[1];
+  at[0].id = cudaLaunchAttributeClusterDimension;
+  at[0].val.clusterDim.x = 1 << LOG2CL; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+  lc.gridDim = dim3((unsigned)(ncl << LOG2CL)); lc.blockDim = dim3(PL::NT);
+  lc.dynamicSmemBytes = cfg.smem; lc.stream = st; lc.attrs = at; lc.numAttrs = 1;
+  const double bytes = (double)batch * 8.0 * p->cl_sumM[c];       // compulsory: the coefficients
+  {
+    LaunchScope ls(p, st, FWD ? K_ROWS_CL_FWD : K_ROWS_CL_INV, bytes, bytes + (double)batch * 8.0 * p->cl_sumL[c]);
+    if (cudaLaunchKernelEx(&lc, k_rows_cluster<LOG2P, LOG2CL, FWD>, A) != cudaSuccess) return QTAM_ERR_CUDA;
+  }
+  QTAM_LAUNCH_CHECK();
+  return QTAM_OK;
+}
+
+template <bool FWD>
+static qtam_status cl_all(qtam_plan *p, int batch, void *d_coef, int plane, cudaStream_t st) {
+  qtam_status s = cl_launch<12, 3, FWD>(p, 3, batch, d_coef, plane, st);
+  if (s == QTAM_OK) s = cl_launch<11, 3, FWD>(p, 2, batch, d_coef, plane, st);
+  if (s == QTAM_OK) s = cl_launch<11, 2, FWD>(p, 1, batch, d_coef, plane, st);
+  if (s == QTAM_OK) s = cl_launch<11, 1, FWD>(p, 0, batch, d_coef, plane, st);
+  return s;
+}
+
+qtam_status cluster_forward_rows(qtam_plan *p, int batch, void *d_coef, cudaStream_t st) {
+  return cl_all<true>(p, batch, d_coef, -1, st);
+}
+qtam_status cluster_inverse_rows(qtam_plan *p, const void *d_coef, int batch, int plane, cudaStream_t st) {
+  return cl_all<false>(p, batch, const_cast<void *>(d_coef), plane, st);
+}
+
+}  // namespace qtam
