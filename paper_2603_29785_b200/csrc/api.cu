@@ -51,7 +51,7 @@ void free_plan(qtam_plan *p) {
   cudaFree(p->d_thr_tasks); cudaFree(p->d_thr_offs);
   for (int c = 0; c < kCtaClasses; ++c) { cudaFree(p->d_cta_lead[c]); cudaFree(p->d_ptw_rows[c]); cudaFree(p->d_cta_groups[c]); cudaFree(p->d_cta_mem[c]); }
   for (int c = 0; c < kClClasses; ++c) { cudaFree(p->d_cl_lead[c]); cudaFree(p->d_cl_mem[c]); cudaFree(p->d_cl_groups[c]); cudaFree(p->d_cl_ftw[c]); }
-  cudaFree(p->d_cl_ptw[0]); cudaFree(p->d_cl_ptw[1]);
+  cudaFree(p->d_cl_ptw);
   cudaFree(p->d_runs); cudaFree(p->d_run_ptr); cudaFree(p->d_run_idx);
   cudaFree(p->d_trows); cudaFree(p->d_titems); cudaFree(p->d_part); cudaFree(p->d_counter);
   for (ProfRec &r : p->prof_pool) { cudaEventDestroy(r.e0); cudaEventDestroy(r.e1); }

@@ -20,34 +20,47 @@ constexpr int kRunBlock = 256;
 
 static int ilog2(long long v) { int l = 0; while ((1LL << l) < v) ++l; return l; }
 
-// sum of the runs of one list at bin f
-__device__ __forceinline__ float2 run_sum(const int4 *__restrict__ runs, const int *__restrict__ idx, int lo, int hi,
-                                          int f, int plane, const float2 *__restrict__ part,
-                                          const float2 *__restrict__ band) {
-  float2 acc = make_float2(0.f, 0.f);
-  for (int e = lo; e < hi; ++e) {
-    const int4 r = __ldg(runs + __ldg(idx + e));       // lo, nb, off, src | (plane + 1) << 1
-    const int rp = (r.w >> 1) - 1;
-    if (rp >= 0 && plane >= 0 && rp != plane) continue;
-    const unsigned d = (unsigned)(f - r.x);
-    if (d < (unsigned)r.y) acc = padd(acc, __ldcs(((r.w & 1) ? part : band) + (size_t)r.z + d));
-  }
-  return acc;
-}
+constexpr int kRunChunk = 128;     // run records staged in shared memory at a time
 
 __global__ void __launch_bounds__(kRunBlock)
 k_combine_runs(const int4 *__restrict__ runs, const int *__restrict__ ptr, const int *__restrict__ idx,
                const float2 *__restrict__ part, long long part_stride, const float2 *__restrict__ band,
                long long sumL, const float *__restrict__ invP, int Nc, int plane, const float2 *__restrict__ tw,
                int tw_shift, float2 *__restrict__ spec, long long xstride) {
+  __shared__ int4 s_runs[kRunChunk];
   const int b = blockIdx.x, seg = blockIdx.y;
   const int f = b * kRunBlock + threadIdx.x;
-  if (f > Nc / 2) return;
   const int g = Nc - f;
   const float2 *ps = part + (size_t)seg * part_stride;
   const float2 *bs = band + (size_t)seg * sumL;
-  float2 A = run_sum(runs, idx, ptr[2 * b], ptr[2 * b + 1], f, plane, ps, bs);
-  float2 B = run_sum(runs, idx, ptr[2 * b + 1], ptr[2 * b + 2], g, plane, ps, bs);
+  // lists 2b (runs that touch the block's bins f) and 2b + 1 (its mirror bins g) are adjacent in idx
+  const int e0 = ptr[2 * b], e1 = ptr[2 * b + 1], e2 = ptr[2 * b + 2];
+  float2 A = make_float2(0.f, 0.f), B = make_float2(0.f, 0.f);
+  for (int c0 = e0; c0 < e2; c0 += kRunChunk) {
+    const int n = min(kRunChunk, e2 - c0);
+    __syncthreads();
+    for (int i = threadIdx.x; i < n; i += kRunBlock) s_runs[i] = __ldg(runs + __ldg(idx + c0 + i));
+    __syncthreads();
+    // the runs are added in list order (a fixed order); the loads of four runs are in flight together
+    for (int i0 = 0; i0 < n; i0 += 4) {
+      float2 v[4]; bool forA[4];
+#pragma unroll
+      for (int k = 0; k < 4; ++k) {
+        v[k] = make_float2(0.f, 0.f);
+        forA[k] = c0 + i0 + k < e1;
+        if (i0 + k < n) {
+          const int4 r = s_runs[i0 + k];           // lo, nb, off, src | (plane + 1) << 1
+          const int rp = (r.w >> 1) - 1;
+          const unsigned d = (unsigned)((forA[k] ? f : g) - r.x);
+          if (d < (unsigned)r.y && !(rp >= 0 && plane >= 0 && rp != plane))
+            v[k] = __ldcs(((r.w & 1) ? ps : bs) + (size_t)r.z + d);
+        }
+      }
+#pragma unroll
+      for (int k = 0; k < 4; ++k) { if (forA[k]) A = padd(A, v[k]); else B = padd(B, v[k]); }
+    }
+  }
+  if (f > Nc / 2) return;
   A = pscale(A, __ldg(invP + f));
   B = pscale(B, __ldg(invP + g));
   if (f == 0) { A.y = 0.f; B.y = 0.f; }

@@ -41,7 +41,9 @@ constexpr int kCtaLog2Max = kClLog2Min + kClClasses - 1;   // longest row of the
 constexpr int kCtaMaxMembers = 32;   // rows per leader (same centre bin and half-width)
 // a leader = one set of identical rows (same centre bin and half-width: transformed once); a group = consecutive
 // leaders whose inverse contributions one CTA / cluster adds into one partial spectrum, in order
-struct ClLeader { int row, mem0, nmem, pad; };
+// (the leader's record carries what the row kernels need, so that an item costs one table read: centre bin,
+// half-width, window offset, (N M)^{-1/2} and sqrt(N/M); members are (coefficient offset, plane) pairs)
+struct __align__(16) ClLeader { int kc, dk, woff, mem0; int nmem, row; float fwd_scale, inv_amp; };
 struct ClGroup { int lead0, nlead, lo, nb; long long part_off; };
 // a run = a contiguous piece of the spectrum held somewhere: `nb` bins from bin `lo` at element `off` of a
 // segment's partial-sum buffer (src 1) or band workspace (src 0); plane >= 0: only for the joint inverse and for
@@ -157,7 +159,7 @@ struct qtam_plan {
   // CTA-level rows (rows_cta.cu), one class per transform length 2^11 .. 2^13
   bool cta_rows = false;
   qtam::ClLeader *d_cta_lead[qtam::kCtaClasses] = {};   // one leader per set of identical rows, ascending centre bin
-  int *d_cta_mem[qtam::kCtaClasses] = {};               // members (row indices) of the leaders
+  int2 *d_cta_mem[qtam::kCtaClasses] = {};              // members of the leaders: (coefficient offset, plane)
   qtam::ClGroup *d_cta_groups[qtam::kCtaClasses] = {};  // inverse: groups of consecutive leaders
   int n_cta_rows[qtam::kCtaClasses] = {}, n_cta_groups[qtam::kCtaClasses] = {};
   double cta_sumM[qtam::kCtaClasses] = {}, cta_sumL[qtam::kCtaClasses] = {};
@@ -165,11 +167,11 @@ struct qtam_plan {
   // cluster-level rows (rows_cluster.cu), one class per transform length 2^14 .. 2^17
   bool cl_rows = false;
   qtam::ClLeader *d_cl_lead[qtam::kClClasses] = {};
-  int *d_cl_mem[qtam::kClClasses] = {};
+  int2 *d_cl_mem[qtam::kClClasses] = {};
   qtam::ClGroup *d_cl_groups[qtam::kClClasses] = {};
   int n_cl_lead[qtam::kClClasses] = {}, n_cl_groups[qtam::kClClasses] = {};
   double cl_sumM[qtam::kClClasses] = {}, cl_sumL[qtam::kClClasses] = {};
-  void *d_cl_ptw[2] = {nullptr, nullptr};               // pass tables of the 2048- and 4096-point sub-transforms
+  void *d_cl_ptw = nullptr;                             // pass tables of the 4096-point sub-transforms
   void *d_cl_ftw[qtam::kClClasses] = {};                // radix-F twiddles per class
   // run-based combine (combine_runs.cu): the inverse of every float plan that is not on the tiled path
   bool use_runs = false;
@@ -257,7 +259,7 @@ qtam_status remodulate(qtam_plan *p, const void *d_coef, int batch, void *d_out,
 qtam_status instantaneous_frequency(qtam_plan *p, const void *d_coef, int batch, void *d_out, cudaStream_t st);
 // rows_cta.cu
 void build_leaders_and_groups(qtam_plan *p, const std::vector<int> &rows_in, int groups_wanted,
-                              std::vector<ClLeader> &lead, std::vector<int> &mem, std::vector<ClGroup> &groups);
+                              std::vector<ClLeader> &lead, std::vector<int2> &mem, std::vector<ClGroup> &groups);
 qtam_status build_rows_cta(qtam_plan *p);
 qtam_status cta_forward_rows(qtam_plan *p, int batch, void *d_coef, cudaStream_t st);
 qtam_status cta_inverse_rows(qtam_plan *p, const void *d_coef, int batch, int plane, cudaStream_t st);

@@ -32,6 +32,7 @@ extern __shared__ __align__(16) unsigned char qtam_tiled_smem[];
 
 static int ilog2(long long v) { int l = 0; while ((1LL << l) < v) ++l; return l; }
 static bool prepare_tiled(qtam_plan *p);   // launch configurations of the two kernels (end of this file)
+constexpr int kTileWarps = 11;   // warps per CTA of k_inv_tiles: 18 KB of shared memory each, one CTA per SM
 
 // --------------------------------------------------------------------------------------------------
 // host: tiles
@@ -46,67 +47,82 @@ qtam_status build_inv_tiled(qtam_plan *p) {
   // than 1024 points; otherwise the tiles are one of the sources of k_combine_runs (combine_runs.cu)
   bool whole = p->fast_long && ilog2(hp.N) - 1 <= 14 && p->n_tiny <= 256;
   for (const HostRow &h : hp.rows) if (h.M > 1024) whole = false;
-  const int max_pass = 12;   // passes per tile: longer tiles mean fewer partial sums, shorter ones a finer schedule
   std::vector<TileRow> trows;
   std::vector<TileItem> items;
   std::vector<int2> tmem;                 // (coefficient offset, plane) of every member
   std::vector<int> item_members;          // members per item, for the schedule
-  for (int q = 0; q < F.nbuckets; ++q) {
-    const FastBucket &B = F.b[q];
-    const int G = 1 << B.log2G, Fr = 32 / G;
-    std::vector<FastRow> all(p->h_frows.begin() + B.row_base, p->h_frows.begin() + B.row_base + B.nrows);
-    std::stable_sort(all.begin(), all.end(), [](const FastRow &a, const FastRow &b) {
-      return a.kc != b.kc ? a.kc < b.kc : a.dk < b.dk;
-    });
-    // rows with the same centre bin and half-width (the clamped rows of different Q-planes) share their
-    // window and their place in the spectrum: by linearity their coefficient rows are added before ONE
-    // transform.  `rows` = one leader per such set; pad0 / pad1 = first member / number of members.
-    std::vector<FastRow> rows;
-    for (size_t i = 0; i < all.size(); ++i) {
-      if (rows.empty() || rows.back().kc != all[i].kc || rows.back().dk != all[i].dk) {
-        rows.push_back(all[i]);
-        rows.back().pad = (int)tmem.size();
-        rows.back().goff = 0;            // member count
+  // Passes per tile: long tiles mean few partial sums (less traffic for the combine pass), short tiles a finer
+  // schedule.  12 at the batch sizes of configs 3 and 5; fewer when (tiles x max_batch) would not give every
+  // resident warp several items (config 4: 16 segments).
+  auto make_tiles = [&](int max_pass) -> bool {
+    trows.clear(); items.clear(); tmem.clear(); item_members.clear();
+    for (int q = 0; q < F.nbuckets; ++q) {
+      const FastBucket &B = F.b[q];
+      const int G = 1 << B.log2G, Fr = 32 / G;
+      std::vector<FastRow> all(p->h_frows.begin() + B.row_base, p->h_frows.begin() + B.row_base + B.nrows);
+      std::stable_sort(all.begin(), all.end(), [](const FastRow &a, const FastRow &b) {
+        return a.kc != b.kc ? a.kc < b.kc : a.dk < b.dk;
+      });
+      // rows with the same centre bin and half-width (the clamped rows of different Q-planes) share their
+      // window and their place in the spectrum: by linearity their coefficient rows are added before ONE
+      // transform.  `rows` = one leader per such set; pad0 / pad1 = first member / number of members.
+      std::vector<FastRow> rows;
+      for (size_t i = 0; i < all.size(); ++i) {
+        if (rows.empty() || rows.back().kc != all[i].kc || rows.back().dk != all[i].dk) {
+          rows.push_back(all[i]);
+          rows.back().pad = (int)tmem.size();
+          rows.back().goff = 0;            // member count
+        }
+        tmem.push_back(make_int2(all[i].offset, all[i].plane));
+        rows.back().goff += 1;
       }
-      tmem.push_back(make_int2(all[i].offset, all[i].plane));
-      rows.back().goff += 1;
-    }
-    size_t i = 0;
-    while (i < rows.size()) {
-      TileItem it{};
-      it.row0 = (int)trows.size(); it.log2G = B.log2G; it.tw_base = B.tw_base;
-      int lo = 1 << 30, hi = -(1 << 30), nmem = 0;
-      while (i < rows.size() && it.npass < max_pass) {
-        const size_t e = std::min(rows.size(), i + (size_t)Fr);
-        int lo2 = lo, hi2 = hi;
-        for (size_t r = i; r < e; ++r) {
-          const int jlo = std::max(-rows[r].dk, -rows[r].kc);
-          const int jhi = std::min(rows[r].dk, (int)hp.nb - 1 - rows[r].kc);
-          if (jlo > jhi) continue;
-          lo2 = std::min(lo2, rows[r].kc + jlo); hi2 = std::max(hi2, rows[r].kc + jhi);
+      size_t i = 0;
+      while (i < rows.size()) {
+        TileItem it{};
+        it.row0 = (int)trows.size(); it.log2G = B.log2G; it.tw_base = B.tw_base;
+        int lo = 1 << 30, hi = -(1 << 30), nmem = 0;
+        while (i < rows.size() && it.npass < max_pass) {
+          const size_t e = std::min(rows.size(), i + (size_t)Fr);
+          int lo2 = lo, hi2 = hi;
+          for (size_t r = i; r < e; ++r) {
+            const int jlo = std::max(-rows[r].dk, -rows[r].kc);
+            const int jhi = std::min(rows[r].dk, (int)hp.nb - 1 - rows[r].kc);
+            if (jlo > jhi) continue;
+            lo2 = std::min(lo2, rows[r].kc + jlo); hi2 = std::max(hi2, rows[r].kc + jhi);
+          }
+          if (hi2 >= lo2 && hi2 - lo2 + 1 > kAccBins) {
+            if (it.npass == 0) return false;     // one pass does not fit: leave the plan to the other paths
+            break;
+          }
+          lo = lo2; hi = hi2;
+          for (size_t r = i; r < e; ++r) {
+            TileRow t{};
+            t.kc = rows[r].kc; t.offset = rows[r].offset; t.wpad = rows[r].wpad; t.plane = rows[r].plane;
+            t.jlo = std::max(-rows[r].dk, -rows[r].kc);
+            t.jhi = std::min(rows[r].dk, (int)hp.nb - 1 - rows[r].kc);
+            t.pad0 = rows[r].pad; t.pad1 = rows[r].goff;
+            nmem += rows[r].goff;
+            trows.push_back(t);
+          }
+          it.npass += 1; it.nrows += (int)(e - i);
+          i = e;
         }
-        if (hi2 >= lo2 && hi2 - lo2 + 1 > kAccBins) {
-          if (it.npass == 0) return QTAM_OK;   // one pass does not fit: leave the plan to the other paths
-          break;
-        }
-        lo = lo2; hi = hi2;
-        for (size_t r = i; r < e; ++r) {
-          TileRow t{};
-          t.kc = rows[r].kc; t.offset = rows[r].offset; t.wpad = rows[r].wpad; t.plane = rows[r].plane;
-          t.jlo = std::max(-rows[r].dk, -rows[r].kc);
-          t.jhi = std::min(rows[r].dk, (int)hp.nb - 1 - rows[r].kc);
-          t.pad0 = rows[r].pad; t.pad1 = rows[r].goff;
-          nmem += rows[r].goff;
-          trows.push_back(t);
-        }
-        it.npass += 1; it.nrows += (int)(e - i);
-        i = e;
+        if (hi < lo) { lo = 0; hi = -1; }
+        it.lo = lo; it.nb = hi - lo + 1;
+        items.push_back(it);
+        item_members.push_back(nmem);
       }
-      if (hi < lo) { lo = 0; hi = -1; }
-      it.lo = lo; it.nb = hi - lo + 1;
-      items.push_back(it);
-      item_members.push_back(nmem);
     }
+    return true;
+  };
+  {
+    static const int tries[] = {12, 8, 6, 4, 3, 2, 1};
+    bool ok = false;
+    for (int mp : tries) {
+      ok = make_tiles(mp);
+      if (!ok || (long long)items.size() * p->max_batch >= 4LL * p->num_sms * kTileWarps) break;
+    }
+    if (!ok) return QTAM_OK;
   }
   // heaviest items first: the dynamic schedule then ends on the short ones
   {
@@ -373,8 +389,6 @@ k_combine_c2r(const TileItem *__restrict__ items, int n_items, const float2 *__r
 // --------------------------------------------------------------------------------------------------
 // host side
 // --------------------------------------------------------------------------------------------------
-constexpr int kTileWarps = 11;   // warps per CTA of k_inv_tiles: 18 KB of shared memory each, one CTA per SM
-
 template <int NW>
 static qtam_status tiles_launch(qtam_plan *p, const void *d_coef, int batch, int plane, cudaStream_t st) {
   const int twt = p->fast.tw_total;

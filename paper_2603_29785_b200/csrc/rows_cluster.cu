@@ -15,8 +15,10 @@
 //                      read-modify-write from one cluster (cluster barriers order the updates): a segmented
 //                      reduction without atomics and without a band workspace.  The groups' partial sums are
 //                      added up, in a fixed order, by k_combine_runs (combine_runs.cu).
-// Classes: M = 4 P CL with P = 2048 (256 threads, two CTAs per SM) and CL = 2, 4, 8 for M = 2^14, 2^15, 2^16;
-// P = 4096 (512 threads), CL = 8 for M = 2^17.
+// Classes: M = 4 P CL with P = 4096 (512 threads, one CTA per SM) and CL = 1, 2, 4, 8 CTAs per cluster for
+// M = 2^14 .. 2^17 (CL = 1: no exchange at all).  Measured on cfg4 against P = 2048 with twice the CTAs per
+// cluster and two CTAs per SM: the smaller cluster wins (less data through distributed shared memory, which
+// moves about 20 B/cycle/SM, and fewer CTAs to wait for at the cluster barrier).
 #include <cooperative_groups.h>
 
 #include <algorithm>
@@ -32,15 +34,46 @@ namespace qtam {
 
 extern __shared__ __align__(16) unsigned char qtam_cl_smem[];
 
-static int ilog2(long long v) { int l = 0; while ((1LL << l) < v) ++l; return l; }
+constexpr int kClLog2P = 12;
 
+// Cluster barrier.  release / acquire (the default pair) orders memory across the cluster: the arrive waits
+// until the CTA's earlier writes -- global ones too -- are performed, the wait invalidates L1.  The relaxed
+// arrive only counts the CTA in: enough where the barrier says "I have finished READING your shared memory".
 __device__ __forceinline__ void cl_arrive() { asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory"); }
+__device__ __forceinline__ void cl_arrive_relaxed() { asm volatile("barrier.cluster.arrive.relaxed.aligned;" ::: "memory"); }
 __device__ __forceinline__ void cl_wait() { asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory"); }
 
+// Predicated loads as volatile asm: a batch of them stays a batch (issued back to back, in program order), instead
+// of being interleaved with their uses by the scheduler when registers are tight -- every load of the batch then
+// waits out its latency at the same time.  The value is zero when the predicate is off.
+__device__ __forceinline__ float2 ld_nc_f2(const float2 *p, bool ok) {
+  float2 v;
+  asm volatile("{\n .reg .pred q;\n setp.ne.s32 q, %3, 0;\n mov.f32 %0, 0f00000000;\n mov.f32 %1, 0f00000000;\n"
+               " @q ld.global.nc.v2.f32 {%0, %1}, [%2];\n}" : "=f"(v.x), "=f"(v.y) : "l"(p), "r"((int)ok));
+  return v;
+}
+__device__ __forceinline__ float ld_nc_f1(const float *p, bool ok) {
+  float v;
+  asm volatile("{\n .reg .pred q;\n setp.ne.s32 q, %2, 0;\n mov.f32 %0, 0f00000000;\n"
+               " @q ld.global.nc.f32 %0, [%1];\n}" : "=f"(v) : "l"(p), "r"((int)ok));
+  return v;
+}
+__device__ __forceinline__ float2 ld_cg_f2(const float2 *p, bool ok) {
+  float2 v;
+  asm volatile("{\n .reg .pred q;\n setp.ne.s32 q, %3, 0;\n mov.f32 %0, 0f00000000;\n mov.f32 %1, 0f00000000;\n"
+               " @q ld.global.cg.v2.f32 {%0, %1}, [%2];\n}" : "=f"(v.x), "=f"(v.y) : "l"(p), "r"((int)ok) : "memory");
+  return v;
+}
+__device__ __forceinline__ float2 ld_cs_f2(const float2 *p) {
+  float2 v;
+  asm volatile("ld.global.cs.v2.f32 {%0, %1}, [%2];" : "=f"(v.x), "=f"(v.y) : "l"(p));
+  return v;
+}
+
 struct ClArgs {
-  const ClLeader *lead; const int *mem; int nlead;          // leaders of this class (ascending centre bin), members
+  const ClLeader *lead; const int2 *mem; int nlead;         // leaders of this class (ascending centre bin), members
   const ClGroup *groups; int ngroups;                       // inverse: groups of consecutive leaders
-  const RowDev *rows; const float *win;
+  const float *win;
   const float2 *spec; long long xstride; int nbins;
   float2 *coef; long long ctot;
   float2 *part; long long part_stride;
@@ -48,28 +81,54 @@ struct ClArgs {
   int batch, plane;
 };
 
-// band side of the forward: B[j] = X[kc + jj] W_k[jj] s at j = q + F jc (R6), zero off the support and off the
-// one-sided spectrum (R8)
-template <int LOG2P, int F> struct ClGather {
-  const float2 *__restrict__ X; const float *__restrict__ W; int kc, dk, nbins, q0; float scale;
-  __device__ __forceinline__ float2 operator()(int ja, int jc) const {
-    constexpr int P = 1 << LOG2P;
-    const int jj = q0 + ja + F * jc - (jc >= P / 2 ? F * P : 0);
-    const int f = kc + jj;
-    float2 v = make_float2(0.f, 0.f);
-    if (jj >= -dk && jj <= dk && (unsigned)f < (unsigned)nbins) v = pscale(__ldg(X + f), __ldg(W + jj) * scale);
-    return v;
+// Pass 1 of the forward's sub-transforms, straight from the spectrum: B[j] = X[kc + jj] W_k[jj] s at
+// j = q + F jc (R6), zero off the support and off the one-sided spectrum (R8).  All 2 R loads of a butterfly
+// are issued before the first multiply.
+template <int LOG2P, int F, class Mid>
+__device__ __forceinline__ void cl_pass1_gather(float2 *s, const float2 *__restrict__ X, const float *__restrict__ W,
+                                                int kc, int dk, int nbins, int q0, float scale, const Mid &mid) {
+  typedef ClFft<LOG2P> PL;
+  constexpr int P = PL::P, R = PL::R0, NBF = P / R, TPS = PL::NT / 4, BPT = NBF / TPS;
+  const int ja = threadIdx.x & 3, ib = threadIdx.x >> 2;
+  float2 v[BPT][R];
+#pragma unroll
+  for (int u = 0; u < BPT; ++u) {
+    const int i = ib + TPS * u;
+    float w[R];
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+      const int jc = i + r * NBF;
+      const int jj = q0 + ja + F * jc - (jc >= P / 2 ? F * P : 0);
+      const int f = kc + jj;
+      const bool ok = jj >= -dk && jj <= dk && (unsigned)f < (unsigned)nbins;
+      v[u][r] = ld_nc_f2(X + f, ok);
+      w[r] = ld_nc_f1(W + jj, ok);
+    }
+#pragma unroll
+    for (int r = 0; r < R; ++r) v[u][r] = pscale(v[u][r], w[r] * scale);
+    RegFFT<R, +1>::run(v[u]);
   }
-};
+  mid();
+#pragma unroll
+  for (int u = 0; u < BPT; ++u) {
+    const int i = ib + TPS * u;
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+      const int a = i * R + r;
+      s[4 * (a + (a >> 4)) + ja] = v[u][r];
+    }
+  }
+}
 
 template <int LOG2P, int LOG2CL, bool FWD>
-__global__ void __launch_bounds__(ClFft<LOG2P>::NT, LOG2P == 11 ? 2 : 1)
+__global__ void __launch_bounds__(ClFft<LOG2P>::NT, 1)
 k_rows_cluster(const ClArgs A) {
   typedef ClFft<LOG2P> PL;
   constexpr int P = PL::P, NT = PL::NT, CL = 1 << LOG2CL, F = 4 * CL;
   constexpr int NCQ = P / CL;            // values of nc one CTA takes in the radix-F stage
   constexpr int BPTF = NCQ / NT;         // ... per thread
   static_assert(NCQ % NT == 0 && BPTF >= 1, "radix-F stage must divide among the threads");
+  static_assert(PL::R0 == 16, "pass 1 writes the skew of radix 16");
   cg::cluster_group cluster = cg::this_cluster();
   const int crank = (int)cluster.block_rank();
   const int cid = blockIdx.x >> LOG2CL, ncl = gridDim.x >> LOG2CL;
@@ -87,27 +146,23 @@ k_rows_cluster(const ClArgs A) {
     for (long long item = cid; item < total; item += ncl) {
       const int seg = (int)(item / A.nlead);
       const ClLeader L = A.lead[item - (long long)seg * A.nlead];
-      const RowDev r = A.rows[L.row];
-      __syncthreads();
-      if (tid == 0) {
-        for (int m = 0; m < L.nmem; ++m) s_off[m] = (int)A.rows[A.mem[L.mem0 + m]].offset;
-        s_nm = L.nmem;
-      }
-      __syncthreads();
-      const int nm = s_nm;
+      __syncthreads();                   // the previous item's stores have read s_off
+      if (tid < L.nmem) s_off[tid] = A.mem[L.mem0 + tid].x;
       // sub-transforms: pass 1 straight from the spectrum
-      const ClGather<LOG2P, F> in{A.spec + (size_t)seg * A.xstride, A.win + r.woff + r.dk, r.kc, r.dk, A.nbins,
-                                  4 * crank, (float)r.fwd_scale};
       auto before_write = [&]() { if (pending) { cl_wait(); pending = false; } };   // the others have read my last result
-      cl_pass<LOG2P, PL::R0, 0, +1, 2, true>(s, in, before_write, A.ptw);
+      cl_pass1_gather<LOG2P, F>(s, A.spec + (size_t)seg * A.xstride, A.win + L.woff + L.dk, L.kc, L.dk, A.nbins,
+                                4 * crank, L.fwd_scale, before_write);
       __syncthreads();
       cl_passes_23<LOG2P, +1>(s, A.ptw);
-      cl_arrive(); cl_wait();
+      cl_arrive();
       // radix-F stage for nc = crank NCQ .. + NCQ
       float2 *Yseg = A.coef + (size_t)seg * A.ctot;
+      const int nm = L.nmem;
 #pragma unroll 1
       for (int u = 0; u < BPTF; ++u) {
         const int nc = crank * NCQ + tid + NT * u;
+        const float2 w1 = __ldg(A.ftw + nc), w4 = __ldg(A.ftw + P + nc);
+        if (u == 0) cl_wait();           // every CTA's sub-transforms are in its shared memory
         float2 v[F];
 #pragma unroll
         for (int jb = 0; jb < CL; ++jb) {
@@ -116,7 +171,7 @@ k_rows_cluster(const ClArgs A) {
           v[4 * jb] = make_float2(a.x, a.y); v[4 * jb + 1] = make_float2(a.z, a.w);
           v[4 * jb + 2] = make_float2(b.x, b.y); v[4 * jb + 3] = make_float2(b.z, b.w);
         }
-        cl_twiddle<F>(v, __ldg(A.ftw + nc), __ldg(A.ftw + P + nc));
+        cl_twiddle<F>(v, w1, w4);
         RegFFT<F, +1>::run(v);
         for (int m = 0; m < nm; ++m) {
           float2 *Y = Yseg + s_off[m] + nc;
@@ -124,7 +179,7 @@ k_rows_cluster(const ClArgs A) {
           for (int mm = 0; mm < F; ++mm) __stcs(Y + mm * P, v[mm]);
         }
       }
-      cl_arrive(); pending = true;
+      cl_arrive_relaxed(); pending = true;   // done reading the others' shared memory; the stores drain on their own
     }
   } else {
     const long long total = (long long)A.ngroups * A.batch;
@@ -142,15 +197,13 @@ k_rows_cluster(const ClArgs A) {
 #pragma unroll 1
       for (int l = 0; l < Gp.nlead; ++l) {
         const ClLeader L = A.lead[Gp.lead0 + l];
-        const RowDev r = A.rows[L.row];
         __syncthreads();
-        if (tid == 0) {
-          int n = 0;
-          for (int m = 0; m < L.nmem; ++m) {
-            const RowDev &rm = A.rows[A.mem[L.mem0 + m]];
-            if (A.plane < 0 || rm.plane == A.plane) s_off[n++] = (int)rm.offset;
-          }
-          s_nm = n;
+        if (tid < 32) {
+          // members that take part (all of them, or those of the requested plane), compacted in order
+          const bool ok = tid < L.nmem && (A.plane < 0 || A.mem[L.mem0 + tid].y == A.plane);
+          const unsigned b = __ballot_sync(0xffffffffu, ok);
+          if (ok) s_off[__popc(b & ((1u << tid) - 1u))] = A.mem[L.mem0 + tid].x;
+          if (tid == 0) s_nm = __popc(b);
         }
         __syncthreads();
         const int nm = s_nm;
@@ -159,22 +212,22 @@ k_rows_cluster(const ClArgs A) {
 #pragma unroll 1
         for (int u = 0; u < BPTF; ++u) {
           const int nc = crank * NCQ + tid + NT * u;
+          float2 w1 = __ldg(A.ftw + nc), w4 = __ldg(A.ftw + P + nc);
           float2 v[F];
           {
             const float2 *Y = Yseg + s_off[0] + nc;
 #pragma unroll
-            for (int mm = 0; mm < F; ++mm) v[mm] = __ldcs(Y + mm * P);
+            for (int mm = 0; mm < F; ++mm) v[mm] = ld_cs_f2(Y + mm * P);
           }
           for (int m = 1; m < nm; ++m) {
             const float2 *Y = Yseg + s_off[m] + nc;
             float2 y[F];
 #pragma unroll
-            for (int mm = 0; mm < F; ++mm) y[mm] = __ldcs(Y + mm * P);
+            for (int mm = 0; mm < F; ++mm) y[mm] = ld_cs_f2(Y + mm * P);
 #pragma unroll
             for (int mm = 0; mm < F; ++mm) v[mm] = padd(v[mm], y[mm]);
           }
           RegFFT<F, -1>::run(v);
-          float2 w1 = __ldg(A.ftw + nc), w4 = __ldg(A.ftw + P + nc);
           w1.y = -w1.y; w4.y = -w4.y;
           cl_twiddle<F>(v, w1, w4);
           if (pending) { cl_wait(); pending = false; }     // every CTA is done with the previous row's result
@@ -190,23 +243,37 @@ k_rows_cluster(const ClArgs A) {
         cl_pass<LOG2P, PL::R0, 0, -1, 0, true>(s, ClNoMid{}, ClSyncMid{}, A.ptw);
         __syncthreads();
         cl_passes_23<LOG2P, -1>(s, A.ptw);
-        // G_k[jj] = sqrt(N/M) Bhat[jj] W_k[jj], added into the group's partial sum at bin kc + jj (R8 clip)
+        // G_k[jj] = sqrt(N/M) Bhat[jj] W_k[jj], added into the group's partial sum at bin kc + jj (R8 clip).
+        // The loads of a batch are issued before its stores (a store may not be overtaken by a later load of
+        // the same array, which would serialise the round trips to L2).
         {
           const int ja = tid & 3, ib = tid >> 2;
-          const float *W = A.win + r.woff + r.dk;
-          const float amp = (float)r.inv_amp;
-          float2 *pb = pg + (r.kc - Gp.lo);
-#pragma unroll 4
-          for (int jc = ib; jc < P; jc += NT / 4) {
-            const int jj = 4 * crank + ja + F * jc - (jc >= P / 2 ? F * P : 0);
-            const int f = r.kc + jj;
-            if (jj >= -r.dk && jj <= r.dk && (unsigned)f < (unsigned)A.nbins) {
-              const float2 old = __ldcg(pb + jj);
-              pb[jj] = pfma(s[4 * jc + ja], make_float2(amp * __ldg(W + jj), amp * __ldg(W + jj)), old);
+          const float *W = A.win + L.woff + L.dk;
+          float2 *pb = pg + (L.kc - Gp.lo);
+          constexpr int TPS = NT / 4, CH = 8;
+          static_assert(P % (CH * TPS) == 0, "batches must tile the sub-transform");
+#pragma unroll 1
+          for (int jc0 = ib; jc0 < P; jc0 += CH * TPS) {
+            float2 old[CH]; float w[CH]; int jjs[CH];
+#pragma unroll
+            for (int c = 0; c < CH; ++c) {
+              const int jc = jc0 + c * TPS;
+              const int jj = 4 * crank + ja + F * jc - (jc >= P / 2 ? F * P : 0);
+              const int f = L.kc + jj;
+              const bool ok = jj >= -L.dk && jj <= L.dk && (unsigned)f < (unsigned)A.nbins;
+              jjs[c] = ok ? jj : (1 << 30);
+              old[c] = ld_cg_f2(pb + jj, ok);
+              w[c] = ld_nc_f1(W + jj, ok);
             }
+#pragma unroll
+            for (int c = 0; c < CH; ++c)
+              if (jjs[c] != (1 << 30)) {
+                const float a = L.inv_amp * w[c];
+                pb[jjs[c]] = pfma(s[4 * (jc0 + c * TPS) + ja], make_float2(a, a), old[c]);
+              }
           }
         }
-        cl_arrive(); pending = true;
+        cl_arrive(); pending = true;     // release: the next row's updates of these bins may come from another CTA
       }
     }
   }
@@ -216,7 +283,7 @@ k_rows_cluster(const ClArgs A) {
 // --------------------------------------------------------------------------------------------------
 // host side
 // --------------------------------------------------------------------------------------------------
-// class c = log2 M - kClLog2Min: (LOG2P, LOG2CL) = (11, 1), (11, 2), (11, 3), (12, 3)
+// class c = log2 M - kClLog2Min = log2 CL: the sub-transforms have P = 2^kClLog2P points in every class
 template <int LOG2P, int LOG2CL> static bool prepare_cl(qtam_plan *p, int c) {
   typedef ClFft<LOG2P> PL;
   const size_t smem = sizeof(float2) * (size_t)PL::SMEM_ELEMS;
@@ -229,7 +296,7 @@ template <int LOG2P, int LOG2CL> static bool prepare_cl(qtam_plan *p, int c) {
     cudaLaunchAttribute at[1];
     at[0].id = cudaLaunchAttributeClusterDimension;
     at[0].val.clusterDim.x = 1 << LOG2CL; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
-    lc.gridDim = dim3((unsigned)(p->num_sms * 2 / (1 << LOG2CL)) << LOG2CL);
+    lc.gridDim = dim3((unsigned)(p->num_sms / (1 << LOG2CL)) << LOG2CL);
     lc.blockDim = dim3(PL::NT); lc.dynamicSmemBytes = smem; lc.attrs = at; lc.numAttrs = 1;
     int ncl = 0;
     if (cudaOccupancyMaxActiveClusters(&ncl, kern, &lc) != cudaSuccess || ncl < 1) return false;
@@ -249,7 +316,6 @@ qtam_status build_rows_cluster(qtam_plan *p) {
     p->device_bytes += bytes;
     return bytes == 0 || cudaMemcpy(*dst, src, bytes, cudaMemcpyHostToDevice) == cudaSuccess;
   };
-  bool need_ptw[2] = {false, false};
   for (int c = 0; c < kClClasses; ++c) {
     const int lm = kClLog2Min + c;
     const int64_t M = int64_t(1) << lm;
@@ -259,34 +325,33 @@ qtam_status build_rows_cluster(qtam_plan *p) {
     p->n_cl_lead[c] = 0; p->n_cl_groups[c] = 0;
     if (idx.empty()) continue;
     std::vector<ClLeader> lead;
-    std::vector<int> mem;
+    std::vector<int2> mem;
     std::vector<ClGroup> groups;
     // about ten groups per class: (groups x segments) spreads over the resident clusters while the partial sums
     // stay a fraction of the band values
     build_leaders_and_groups(p, idx, 10, lead, mem, groups);
     p->n_cl_lead[c] = (int)lead.size(); p->n_cl_groups[c] = (int)groups.size();
     if (!up(reinterpret_cast<void **>(&p->d_cl_lead[c]), lead.data(), lead.size() * sizeof(ClLeader))) return QTAM_ERR_ALLOC;
-    if (!up(reinterpret_cast<void **>(&p->d_cl_mem[c]), mem.data(), mem.size() * sizeof(int))) return QTAM_ERR_ALLOC;
+    if (!up(reinterpret_cast<void **>(&p->d_cl_mem[c]), mem.data(), mem.size() * sizeof(int2))) return QTAM_ERR_ALLOC;
     if (!up(reinterpret_cast<void **>(&p->d_cl_groups[c]), groups.data(), groups.size() * sizeof(ClGroup))) return QTAM_ERR_ALLOC;
     std::vector<float> t;
-    fill_clfft_final(t, c == 3 ? 4096 : 2048, M);
+    fill_clfft_final(t, ClFft<kClLog2P>::P, M);
     if (!up(&p->d_cl_ftw[c], t.data(), t.size() * sizeof(float))) return QTAM_ERR_ALLOC;
-    need_ptw[c == 3 ? 1 : 0] = true;
+
     bool ok = false;
     switch (c) {
-      case 0: ok = prepare_cl<11, 1>(p, c); break;
-      case 1: ok = prepare_cl<11, 2>(p, c); break;
-      case 2: ok = prepare_cl<11, 3>(p, c); break;
-      default: ok = prepare_cl<12, 3>(p, c); break;
+      case 0: ok = prepare_cl<kClLog2P, 0>(p, c); break;
+      case 1: ok = prepare_cl<kClLog2P, 1>(p, c); break;
+      case 2: ok = prepare_cl<kClLog2P, 2>(p, c); break;
+      default: ok = prepare_cl<kClLog2P, 3>(p, c); break;
     }
     if (!ok) return QTAM_ERR_CUDA;
     p->cl_rows = true;
   }
-  for (int i = 0; i < 2; ++i) {
-    if (!need_ptw[i]) continue;
+  if (p->cl_rows) {
     std::vector<float> t;
-    if (i == 0) fill_clfft_tables<11>(t); else fill_clfft_tables<12>(t);
-    if (!up(&p->d_cl_ptw[i], t.data(), t.size() * sizeof(float))) return QTAM_ERR_ALLOC;
+    fill_clfft_tables<kClLog2P>(t);
+    if (!up(&p->d_cl_ptw, t.data(), t.size() * sizeof(float))) return QTAM_ERR_ALLOC;
   }
   return QTAM_OK;
 }
@@ -300,11 +365,11 @@ static qtam_status cl_launch(qtam_plan *p, int c, int batch, void *d_coef, int p
   ClArgs A{};
   A.lead = p->d_cl_lead[c]; A.mem = p->d_cl_mem[c]; A.nlead = p->n_cl_lead[c];
   A.groups = p->d_cl_groups[c]; A.ngroups = p->n_cl_groups[c];
-  A.rows = p->d_rows; A.win = static_cast<const float *>(p->d_win);
+  A.win = static_cast<const float *>(p->d_win);
   A.spec = static_cast<const float2 *>(p->d_spec); A.xstride = p->xstride; A.nbins = (int)p->hp.nb;
   A.coef = static_cast<float2 *>(d_coef); A.ctot = p->hp.ctot;
   A.part = static_cast<float2 *>(p->d_part); A.part_stride = p->part_stride;
-  A.ptw = static_cast<const float2 *>(p->d_cl_ptw[LOG2P == 12 ? 1 : 0]);
+  A.ptw = static_cast<const float2 *>(p->d_cl_ptw);
   A.ftw = static_cast<const float2 *>(p->d_cl_ftw[c]);
   A.batch = batch; A.plane = plane;
   const long long items = (long long)(FWD ? A.nlead : A.ngroups) * batch;
@@ -326,10 +391,10 @@ static qtam_status cl_launch(qtam_plan *p, int c, int batch, void *d_coef, int p
 
 template <bool FWD>
 static qtam_status cl_all(qtam_plan *p, int batch, void *d_coef, int plane, cudaStream_t st) {
-  qtam_status s = cl_launch<12, 3, FWD>(p, 3, batch, d_coef, plane, st);
-  if (s == QTAM_OK) s = cl_launch<11, 3, FWD>(p, 2, batch, d_coef, plane, st);
-  if (s == QTAM_OK) s = cl_launch<11, 2, FWD>(p, 1, batch, d_coef, plane, st);
-  if (s == QTAM_OK) s = cl_launch<11, 1, FWD>(p, 0, batch, d_coef, plane, st);
+  qtam_status s = cl_launch<kClLog2P, 3, FWD>(p, 3, batch, d_coef, plane, st);
+  if (s == QTAM_OK) s = cl_launch<kClLog2P, 2, FWD>(p, 2, batch, d_coef, plane, st);
+  if (s == QTAM_OK) s = cl_launch<kClLog2P, 1, FWD>(p, 1, batch, d_coef, plane, st);
+  if (s == QTAM_OK) s = cl_launch<kClLog2P, 0, FWD>(p, 0, batch, d_coef, plane, st);
   return s;
 }
 

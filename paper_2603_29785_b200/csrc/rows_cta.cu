@@ -55,8 +55,8 @@ struct CoefIn {       // sum of the members' coefficients
 
 template <int L2, bool FORWARD>
 __global__ void __launch_bounds__(CtaFftPlan<L2>::NT, (L2 == 13 || L2 == 12) ? 2 : 1)
-k_rows_cta(const ClLeader *__restrict__ lead, const int *__restrict__ mem, int nlead,
-           const ClGroup *__restrict__ groups, int ngroups, const RowDev *__restrict__ rows,
+k_rows_cta(const ClLeader *__restrict__ lead, const int2 *__restrict__ mem, int nlead,
+           const ClGroup *__restrict__ groups, int ngroups,
            const float *__restrict__ win, const float2 *__restrict__ spec, long long xstride, int nbins,
            float2 *__restrict__ coef, long long ctot, float2 *__restrict__ part, long long part_stride,
            const float2 *__restrict__ ptw, int batch, int plane) {
@@ -69,15 +69,11 @@ k_rows_cta(const ClLeader *__restrict__ lead, const int *__restrict__ mem, int n
     for (long long item = blockIdx.x; item < total; item += gridDim.x) {
       const int seg = (int)(item / nlead);
       const ClLeader L = lead[item - (long long)seg * nlead];
-      const RowDev r = rows[L.row];
       __syncthreads();
-      if (threadIdx.x == 0) {
-        for (int m = 0; m < L.nmem; ++m) s_off[m] = (int)rows[mem[L.mem0 + m]].offset;
-        s_nm = L.nmem;
-      }
+      if (threadIdx.x < L.nmem) s_off[threadIdx.x] = mem[L.mem0 + threadIdx.x].x;
       __syncthreads();
-      GatherIn in{spec + (size_t)seg * xstride, win + r.woff + r.dk, r.kc, r.dk, nbins, M};
-      cta_fft_io<L2, NT, +1, true, true>(s, in, CoefOut{coef + (size_t)seg * ctot, s_off, s_nm, (float)r.fwd_scale}, ptw);
+      GatherIn in{spec + (size_t)seg * xstride, win + L.woff + L.dk, L.kc, L.dk, nbins, M};
+      cta_fft_io<L2, NT, +1, true, true>(s, in, CoefOut{coef + (size_t)seg * ctot, s_off, L.nmem, L.fwd_scale}, ptw);
     }
   } else {
     const long long total = (long long)ngroups * batch;
@@ -94,31 +90,43 @@ k_rows_cta(const ClLeader *__restrict__ lead, const int *__restrict__ mem, int n
 #pragma unroll 1
       for (int l = 0; l < Gp.nlead; ++l) {
         const ClLeader L = lead[Gp.lead0 + l];
-        const RowDev r = rows[L.row];
         __syncthreads();      // the previous row's updates of the partial sum and its reads of s_off are done
-        if (threadIdx.x == 0) {
-          int n = 0;
-          for (int m = 0; m < L.nmem; ++m) {
-            const RowDev &rm = rows[mem[L.mem0 + m]];
-            if (plane < 0 || rm.plane == plane) s_off[n++] = (int)rm.offset;
-          }
-          s_nm = n;
+        if (threadIdx.x < 32) {
+          // members that take part (all of them, or those of the requested plane), compacted in order
+          const bool ok = threadIdx.x < L.nmem && (plane < 0 || mem[L.mem0 + threadIdx.x].y == plane);
+          const unsigned b = __ballot_sync(0xffffffffu, ok);
+          if (ok) s_off[__popc(b & ((1u << threadIdx.x) - 1u))] = mem[L.mem0 + threadIdx.x].x;
+          if (threadIdx.x == 0) s_nm = __popc(b);
         }
         __syncthreads();
         const int nm = s_nm;
         if (nm == 0) continue;
         cta_fft_io<L2, NT, -1, true, false>(s, CoefIn{Yseg, s_off, nm}, CtaFftNone{}, ptw);
-        // G_k[jj] = sqrt(N/M) Bhat[jj] W_k[jj] on the support, clipped to the one-sided spectrum (R8)
-        const float *W = win + r.woff + r.dk;
-        const float amp = (float)r.inv_amp;
-        float2 *pb = pg + (r.kc - Gp.lo);
-        for (int j = threadIdx.x; j < M; j += NT) {
-          const int jj = j < (M >> 1) ? j : j - M;
-          const int f = r.kc + jj;
-          if (jj >= -r.dk && jj <= r.dk && (unsigned)f < (unsigned)nbins) {
-            const float w = amp * __ldg(W + jj);
-            pb[jj] = pfma(s[j], make_float2(w, w), __ldcg(pb + jj));
+        // G_k[jj] = sqrt(N/M) Bhat[jj] W_k[jj] on the support, clipped to the one-sided spectrum (R8); the loads
+        // of a batch are issued before its stores (a store may not be overtaken by a later load of the same array)
+        const float *W = win + L.woff + L.dk;
+        float2 *pb = pg + (L.kc - Gp.lo);
+        constexpr int CH = 8;
+        static_assert(M % (CH * NT) == 0 || M < CH * NT, "batches must tile the row");
+#pragma unroll 1
+        for (int j0 = threadIdx.x; j0 < M; j0 += CH * NT) {
+          float2 old[CH]; float w[CH]; int jjs[CH];
+#pragma unroll
+          for (int c = 0; c < CH; ++c) {
+            const int j = j0 + c * NT;
+            const int jj = j < (M >> 1) ? j : j - M;
+            const int f = L.kc + jj;
+            const bool ok = j < M && jj >= -L.dk && jj <= L.dk && (unsigned)f < (unsigned)nbins;
+            jjs[c] = ok ? jj : (1 << 30);
+            old[c] = make_float2(0.f, 0.f); w[c] = 0.f;
+            if (ok) { old[c] = __ldcg(pb + jj); w[c] = __ldg(W + jj); }
           }
+#pragma unroll
+          for (int c = 0; c < CH; ++c)
+            if (jjs[c] != (1 << 30)) {
+              const float a = L.inv_amp * w[c];
+              pb[jjs[c]] = pfma(s[j0 + c * NT], make_float2(a, a), old[c]);
+            }
         }
       }
     }
@@ -141,7 +149,7 @@ template <int L2> static bool prepare_class(qtam_plan *p, int c) {
 // ascending centre bin, and groups of consecutive leaders for the inverse; the groups' partial sums are appended
 // to the plan's per-segment partial-sum layout and registered as runs for k_combine_runs.
 void build_leaders_and_groups(qtam_plan *p, const std::vector<int> &rows_in, int groups_wanted,
-                              std::vector<ClLeader> &lead, std::vector<int> &mem, std::vector<ClGroup> &groups) {
+                              std::vector<ClLeader> &lead, std::vector<int2> &mem, std::vector<ClGroup> &groups) {
   const HostPlan &hp = p->hp;
   std::vector<int> idx = rows_in;
   std::stable_sort(idx.begin(), idx.end(), [&](int a, int b) {
@@ -164,8 +172,14 @@ void build_leaders_and_groups(qtam_plan *p, const std::vector<int> &rows_in, int
     if (!joined) sets.push_back(std::vector<int>(1, k));
   }
   for (const auto &st : sets) {
-    lead.push_back(ClLeader{st[0], (int)mem.size(), (int)st.size(), 0});
-    mem.insert(mem.end(), st.begin(), st.end());
+    const HostRow &h = hp.rows[(size_t)st[0]];
+    ClLeader L{};
+    L.kc = (int)h.kc; L.dk = (int)h.dk; L.woff = (int)h.woff; L.mem0 = (int)mem.size(); L.nmem = (int)st.size();
+    L.row = st[0];
+    L.fwd_scale = (float)(1.0 / std::sqrt((double)hp.N * (double)h.M));
+    L.inv_amp = (float)std::sqrt((double)hp.N / (double)h.M);
+    lead.push_back(L);
+    for (int k : st) mem.push_back(make_int2((int)hp.rows[(size_t)k].offset, hp.rows[(size_t)k].plane));
   }
   const int per = std::max<int>(1, ((int)lead.size() + groups_wanted - 1) / groups_wanted);
   for (size_t i = 0; i < lead.size(); i += (size_t)per) {
@@ -207,12 +221,12 @@ qtam_status build_rows_cta(qtam_plan *p) {
     p->n_cta_rows[c] = 0; p->n_cta_groups[c] = 0;
     if (idx.empty()) continue;
     std::vector<ClLeader> lead;
-    std::vector<int> mem;
+    std::vector<int2> mem;
     std::vector<ClGroup> groups;
     build_leaders_and_groups(p, idx, 12, lead, mem, groups);
     p->n_cta_rows[c] = (int)lead.size(); p->n_cta_groups[c] = (int)groups.size();
     if (!up(reinterpret_cast<void **>(&p->d_cta_lead[c]), lead.data(), lead.size() * sizeof(ClLeader))) return QTAM_ERR_ALLOC;
-    if (!up(reinterpret_cast<void **>(&p->d_cta_mem[c]), mem.data(), mem.size() * sizeof(int))) return QTAM_ERR_ALLOC;
+    if (!up(reinterpret_cast<void **>(&p->d_cta_mem[c]), mem.data(), mem.size() * sizeof(int2))) return QTAM_ERR_ALLOC;
     if (!up(reinterpret_cast<void **>(&p->d_cta_groups[c]), groups.data(), groups.size() * sizeof(ClGroup))) return QTAM_ERR_ALLOC;
     std::vector<float> t;
     bool ok = false;
@@ -240,7 +254,7 @@ static qtam_status rows_cta_launch(qtam_plan *p, int c, int batch, void *d_coef,
   {
     LaunchScope ls(p, st, FORWARD ? K_ROWS_CTA_FWD : K_ROWS_CTA_INV, bytes, bytes + (double)batch * 8.0 * p->cta_sumL[c]);
     k_rows_cta<L2, FORWARD><<<(unsigned)grid, NT, cfg.smem, st>>>(
-        p->d_cta_lead[c], p->d_cta_mem[c], p->n_cta_rows[c], p->d_cta_groups[c], p->n_cta_groups[c], p->d_rows,
+        p->d_cta_lead[c], p->d_cta_mem[c], p->n_cta_rows[c], p->d_cta_groups[c], p->n_cta_groups[c],
         static_cast<const float *>(p->d_win), static_cast<const float2 *>(p->d_spec), p->xstride, (int)p->hp.nb,
         static_cast<float2 *>(d_coef), p->hp.ctot, static_cast<float2 *>(p->d_part), p->part_stride,
         static_cast<const float2 *>(p->d_ptw_rows[c]), batch, plane);
