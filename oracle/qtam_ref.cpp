@@ -66,6 +66,7 @@ int64_t next_pow2(int64_t v) {
   return m;
 }
 bool is_pow2(int64_t v) { return v > 0 && (v & (v - 1)) == 0; }
+bool is_fft_length(int64_t v) { return is_pow2(v) || (v % 3 == 0 && is_pow2(v / 3)); }   // 2^a or 3 * 2^a
 
 // ---- DFT engines ------------------------------------------------------------------------------
 
@@ -80,32 +81,55 @@ void dft_naive(const cd *in, cd *out, int64_t n, int sign) {
   }
 }
 
-// textbook recursive radix-2 decimation in time; tw[m] = e^{sign 2 pi i m/ntop}
-void fft_rec(cd *a, cd *tmp, int64_t n, const cd *tw, int64_t tw_step) {
+// textbook recursive decimation in time, radix 2 while the length is even and radix 3 for a remaining factor 3
+// (segment lengths N = 3 * 2^k: the paper's own benchmark shape is 6 s at 4096 Hz = 24576 samples, PAPER.md:178,
+// :339); tw[m] = e^{sign 2 pi i m/ntop}, m = 0 .. ntop-1
+void fft_rec(cd *a, cd *tmp, int64_t n, const cd *tw, int64_t tw_step, int64_t ntop) {
   if (n == 1) return;
-  int64_t h = n / 2;
-  for (int64_t i = 0; i < h; ++i) {
-    tmp[i] = a[2 * i];
-    tmp[h + i] = a[2 * i + 1];
-  }
-  std::memcpy(a, tmp, sizeof(cd) * (size_t)n);
-  fft_rec(a, tmp, h, tw, tw_step * 2);
-  fft_rec(a + h, tmp, h, tw, tw_step * 2);
-  for (int64_t k = 0; k < h; ++k) {
-    cd e = a[k], o = a[h + k] * tw[(size_t)(k * tw_step)];
-    a[k] = e + o;
-    a[h + k] = e - o;
+  if (n % 2 == 0) {
+    int64_t h = n / 2;
+    for (int64_t i = 0; i < h; ++i) {
+      tmp[i] = a[2 * i];
+      tmp[h + i] = a[2 * i + 1];
+    }
+    std::memcpy(a, tmp, sizeof(cd) * (size_t)n);
+    fft_rec(a, tmp, h, tw, tw_step * 2, ntop);
+    fft_rec(a + h, tmp, h, tw, tw_step * 2, ntop);
+    for (int64_t k = 0; k < h; ++k) {
+      cd e = a[k], o = a[h + k] * tw[(size_t)(k * tw_step)];
+      a[k] = e + o;
+      a[h + k] = e - o;
+    }
+  } else {
+    // n = 3 h: X[k + m h] = F0[k] + w_n^{k + m h} F1[k] + w_n^{2 (k + m h)} F2[k], F_r = DFT_h of a[3 i + r]
+    int64_t h = n / 3;
+    for (int64_t i = 0; i < h; ++i) {
+      tmp[i] = a[3 * i];
+      tmp[h + i] = a[3 * i + 1];
+      tmp[2 * h + i] = a[3 * i + 2];
+    }
+    std::memcpy(a, tmp, sizeof(cd) * (size_t)n);
+    for (int r = 0; r < 3; ++r) fft_rec(a + r * h, tmp, h, tw, tw_step * 3, ntop);
+    for (int64_t k = 0; k < h; ++k) {
+      const cd f0 = a[k], f1 = a[h + k], f2 = a[2 * h + k];
+      for (int64_t m = 0; m < 3; ++m) {
+        const int64_t e1 = ((k + m * h) * tw_step) % ntop, e2 = (2 * (k + m * h) * tw_step) % ntop;
+        tmp[k + m * h] = f0 + f1 * tw[(size_t)e1] + f2 * tw[(size_t)e2];
+      }
+    }
+    std::memcpy(a, tmp, sizeof(cd) * (size_t)n);
   }
 }
 
+// n = 2^a or 3 * 2^a
 void fft_radix2(const cd *in, cd *out, int64_t n, int sign) {
-  std::vector<cd> tw((size_t)std::max<int64_t>(n / 2, 1)), tmp((size_t)n);
-  for (int64_t m = 0; m < n / 2; ++m) {
+  std::vector<cd> tw((size_t)std::max<int64_t>(n, 1)), tmp((size_t)n);
+  for (int64_t m = 0; m < n; ++m) {
     cld c = cis(sign * m, n);
     tw[(size_t)m] = cd((double)c.real(), (double)c.imag());
   }
   if (out != in) std::memcpy(out, in, sizeof(cd) * (size_t)n);
-  fft_rec(out, tmp.data(), n, tw.data(), 1);
+  fft_rec(out, tmp.data(), n, tw.data(), 1, n);
 }
 
 // One-sided spectrum X[f] = sum_n x[n] e^{-2 pi i fn/N}, f = 0..N/2 (C1).
@@ -198,7 +222,7 @@ int qtam_ref_dft(const double *in, double *out, int64_t n, int sign) {
 }
 
 int qtam_ref_fft(const double *in, double *out, int64_t n, int sign) {
-  if (!in || !out || !is_pow2(n) || (sign != 1 && sign != -1)) return 1;
+  if (!in || !out || !is_fft_length(n) || (sign != 1 && sign != -1)) return 1;
   fft_radix2(reinterpret_cast<const cd *>(in), reinterpret_cast<cd *>(out), n, sign);
   return 0;
 }
@@ -247,7 +271,7 @@ static double raw_window(int type, double par, int64_t j, int64_t dk) {
 
 int qtam_ref_plan_create(qtam_ref_plan **out, double fs, int64_t N, const double *Q, int nQ,
                          double fmin, double fmax, double spacing, const qtam_ref_options *opt) {
-  if (!out || !Q || nQ < 1 || !(fs > 0) || !is_pow2(N) || N < 8) return 1;
+  if (!out || !Q || nQ < 1 || !(fs > 0) || !is_fft_length(N) || N % 8 != 0 || N < 8) return 1;
   qtam_ref_options o;
   o.window = 0; o.clamp_mode = 1; o.clamp_overlap = 1.0; o.max_window_bins = 0;
   o.cover_floor = 1e-2; o.rows_are_bins_per_octave = 0; o.window_param = 0.0; o.freqs = nullptr; o.n_freqs = 0; o.tile_length = 0; o.epsilon = 0.0;

@@ -120,7 +120,8 @@ int  qtam_ref_project_cover(const qtam_ref_plan *p, const double *x, int batch, 
 int  qtam_ref_spectrum(const qtam_ref_plan *p, const double *x, int batch, double *X_out, int engine);
 
 /* Raw DFT engines on n complex points (interleaved); sign = -1 forward (C1), +1 inverse kernel,
- * never scaled. qtam_ref_dft: naive sums. qtam_ref_fft: recursive radix-2, n a power of two.      */
+ * never scaled. qtam_ref_dft: naive sums. qtam_ref_fft: recursive radix-2 with a radix-3 step,
+ * n = 2^a or 3 * 2^a.                                                                            */
 int  qtam_ref_dft(const double *in, double *out, int64_t n, int sign);
 int  qtam_ref_fft(const double *in, double *out, int64_t n, int sign);
 /* Optimal-selection output: out[batch][max_p C_p] complex, plane best[b] of segment b at its

@@ -44,6 +44,18 @@ def test_p11_fft_vs_naive_dft(n):
         assert rel_l2(b, a) <= 1e-13
 
 
+@pytest.mark.parametrize("n", [3, 6, 12, 24, 48, 96, 192, 384, 768, 1536, 3072])
+def test_p11_mixed_radix_fft_vs_naive_dft(n):
+    """segment lengths 3 * 2^k (the paper's benchmark shape, 6 s at 4096 Hz = 24576 samples):
+    the engine's radix-3 step against the naive sums, and at the benchmark length against an outside library"""
+    rng = np.random.default_rng(n)
+    z = rng.standard_normal(n) + 1j * rng.standard_normal(n)
+    for sign in (-1, +1):
+        assert rel_l2(fft(z, sign), dft(z, sign)) <= 1e-13
+    z = rng.standard_normal(24576) + 1j * rng.standard_normal(24576)
+    assert rel_l2(fft(z, -1), np.fft.fft(z)) <= 1e-13
+
+
 @pytest.mark.parametrize("n", [8, 12, 64, 100, 1024])
 def test_naive_dft_vs_numpy_library(n):
     """C1/C2 sign and index convention against an outside library."""
@@ -157,7 +169,8 @@ def test_plan_table_sizes_match_survey():
 def test_plan_rejects_bad_arguments():
     ok = dict(fs=256.0, N=256, Q=[4.0], fmin=8.0, fmax=100.0, spacing=6)
     RefPlan(**ok)
-    for bad in (dict(N=300), dict(fmax=128.0), dict(fmin=0.0), dict(Q=[3.0]), dict(fmin=1.0, Q=[64.0])):
+    RefPlan(**{**ok, **dict(N=192, fs=192.0, fmax=90.0)})          # 3 * 2^k is a segment length too
+    for bad in (dict(N=300), dict(N=320), dict(N=12), dict(fmax=128.0), dict(fmin=0.0), dict(Q=[3.0]), dict(fmin=1.0, Q=[64.0])):
         with pytest.raises(ValueError):
             RefPlan(**{**ok, **bad})
 
@@ -179,6 +192,38 @@ def test_p1_bruteforce_tiny_n64():
     D = p.dense(x)[0]
     for k in range(p.n_rows):
         assert rel_l2(D[k], p.brute_tile(x, k)) <= 1e-12
+
+
+@pytest.mark.parametrize("N", [96, 192])
+def test_non_power_of_two_segment_length(N):
+    """N = 3 * 2^k: the same pins as for powers of two -- P1 dense tiles
+    against the brute-force circular convolution (no DFT of x), both engines; P2 against the dense tiles; P4 the
+    round trip against an outside library's projection; P6 the frame-energy identity; the engines agree."""
+    p = RefPlan(float(N), N, [4.0, 8.0], 5.0, 0.42 * N, 7.0)
+    assert p.N == N and p.n_bins == N // 2 + 1
+    x = inputs.white_noise(N, 60 + N, batch=2)
+    for engine in (0, 1):
+        D = p.dense(x[0], engine=engine)[0]
+        for k in range(p.n_rows):
+            assert rel_l2(D[k], p.brute_tile(x[0], k)) <= 1e-12, (engine, k)
+    Y0, Y1 = p.forward(x, engine=0), p.forward(x, engine=1)
+    assert rel_l2(Y1, Y0) <= 1e-13
+    D = p.dense(x[0], engine=0)[0]
+    for k, r in enumerate(p.rows):
+        if N % r.M:
+            continue                                   # P2 needs tau = n N / M on the sample grid
+        n = np.arange(r.M)
+        want = np.sqrt(N / r.M) * np.exp(-2j * np.pi * r.kc * n / r.M) * D[k][n * N // r.M]
+        assert rel_l2(Y0[0, p.row_slice(k)], want) <= 1e-12, k
+    X = np.fft.rfft(x, axis=-1)
+    P, _ = p.frame(-1)
+    tot = np.sum(np.abs(Y0) ** 2, axis=1)
+    assert np.all(np.abs(tot - np.sum(np.abs(X) ** 2 * P[None, :], axis=1) / N) <= 1e-13 * tot)
+    for plane in (-1, 0, 1):
+        _, C = p.frame(plane)
+        proj = np.fft.irfft(np.where(C[None, :], X, 0), n=N, axis=-1)
+        for engine in (0, 1):
+            assert rel_l2(p.inverse(Y0, plane=plane, engine=engine), proj) <= 1e-12, (plane, engine)
 
 
 def test_bruteforce_atom_is_time_domain_definition():
