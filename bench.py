@@ -545,7 +545,8 @@ def run_ours(args):
         if w is not None:
             w.close()
             w = None
-        for name, dt in (("cfg2", "f32"), ("cfg3", "f32"), ("cfg5", "f32"), ("cfg5", "f64"), ("cfg4", "f32"), ("cfg1", "f64")):
+        for name, dt in (("cfg2", "f32"), ("cfg3", "f32"), ("cfg5", "f32"), ("cfg5", "f64"), ("cfg4", "f32"), ("cfg1", "f64"),
+                         ("paper6s", "f32")):
             if name == args.workload and dt == dtype:
                 continue
             key = name if dt == inputs.CONFIGS[name]["dtype"] else f"{name}_{dt}"

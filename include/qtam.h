@@ -42,7 +42,7 @@ typedef enum { QTAM_F32 = 0, QTAM_F64 = 1 } qtam_dtype;  /* real in / complex ou
 
 typedef enum {
   QTAM_OK = 0,
-  QTAM_ERR_INVALID_ARG = 1,   /* NULL pointer, N not a power of two, fmax >= fs/2, fmin <= 0,
+  QTAM_ERR_INVALID_ARG = 1,   /* NULL pointer, N neither 2^k nor 3 * 2^k (k >= 3), fmax >= fs/2, fmin <= 0,
                                  Q < sqrt(11), half-width < 1 bin, batch > max_batch, bad row range,
                                  max_batch > 65535 */
   QTAM_ERR_UNSUPPORTED = 2,   /* window family / size outside what this build implements */
@@ -99,7 +99,9 @@ typedef struct {
 /* Plan (host, once): frequency grid f_r = fmin*(fmax/fmin)^(r/(R-1)) or fmin*2^(r/B),
  * centre bins, bandwidths, clamp A7/A8 (:307-311), the windows (App. A) and their normalisation
  * (Eq. 5-7 :63-72), output lengths, the frame operator and cover sets, device tables + workspace.
- * Q: nQ quality factors (host pointer), one plane each.  *out is written only on QTAM_OK. */
+ * Q: nQ quality factors (host pointer), one plane each.  *out is written only on QTAM_OK.
+ * N = 2^k or 3 * 2^k samples (the paper's benchmark segments are 6 s at 4096 Hz = 24576 = 3 * 2^13, PAPER.md:178,
+ * :339): the long transforms of the latter take one radix-3 step around power-of-two transforms. */
 qtam_status qtam_plan_create(qtam_plan **out, double fs, int64_t N, const double *Q, int nQ,
                              double fmin, double fmax, double spacing, qtam_dtype dtype,
                              const qtam_options *opt);

@@ -40,7 +40,9 @@ bool dev_alloc(void **dst, size_t bytes, size_t *total) {
 void free_plan(qtam_plan *p) {
   if (!p) return;
   if (p->host_only) { delete p; return; }
-  cudaFree(p->d_rows); cudaFree(p->d_win); cudaFree(p->d_tw); cudaFree(p->d_invP);
+  cudaFree(p->d_rows); cudaFree(p->d_win); cudaFree(p->d_invP);
+  if (p->d_twN != p->d_tw) cudaFree(p->d_twN);
+  cudaFree(p->d_tw); cudaFree(p->d_ws3);
   cudaFree(p->d_csr_ptr); cudaFree(p->d_csr_idx); cudaFree(p->d_plane_off);
   for (int c = 0; c < qtam_plan::kClasses; ++c) { cudaFree(p->d_items[c]); cudaFree(p->d_items_fwd[c]); }
   cudaFree(p->d_gfol_ptr); cudaFree(p->d_gfol_off); cudaFree(p->d_gfol_woff);
@@ -239,6 +241,14 @@ template <typename T> qtam_status build_device(qtam_plan *p) {
     T *d = nullptr;
     if (!upload(&d, tw.data(), tw.size(), tot)) return QTAM_ERR_ALLOC;
     p->d_tw = d;
+    p->d_twN = d;
+    if (!p->n_pow2) {
+      // e^{2 pi i k/N} for the steps whose period is the segment length (radix-3 combine, real pre / post-processing)
+      fill_twiddles<T>(tw, hp.N);
+      if (!upload(&d, tw.data(), tw.size(), tot)) return QTAM_ERR_ALLOC;
+      p->d_twN = d;
+      if (!dev_alloc(&p->d_ws3, 2 * 2 * sizeof(T) * size_t(p->max_batch) * size_t(hp.N), tot)) return QTAM_ERR_ALLOC;
+    }
   }
   // 1/P on the cover set, 0 elsewhere (a7; R9)
   {
@@ -365,14 +375,18 @@ qtam_status qtam_plan_create(qtam_plan **out, double fs, int64_t N, const double
   p->esz = dtype == QTAM_F32 ? 4 : 8;
   p->max_batch = p->hp.opt.max_batch;
   p->xstride = ((p->hp.nb + kSpecPad + 31) / 32) * 32;
-  p->twn = N;
+  p->n_pow2 = (N & (N - 1)) == 0;
+  // power-of-two periods come from tw (short FFTs of up to nextpow2(N/2 + 1) points, the power-of-two part of
+  // the long transform); for N = 3 * 2^k that is a table of 2^(k+1) entries
+  p->twn = p->n_pow2 ? N : (N / 3) * 2;
+  p->sub_n = p->n_pow2 ? N / 2 : N / 6;
   p->cap_log2 = dtype == QTAM_F32 ? 13 : 12;
   {
     int dev = 0, sms = 148;
     if (cudaGetDevice(&dev) == cudaSuccess &&
         cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && sms > 0)
       p->num_sms = sms;
-    const int lnc = ilog2(N) - 1;
+    const int lnc = p->n_pow2 ? ilog2(N) - 1 : -1;     // the tuned long transforms take N = 2^k only
     // the tuned float kernels keep coefficient offsets in 32-bit integers; a plan with more coefficients per
     // segment runs every row in the generic kernels (64-bit offsets)
     p->fast_rows = dtype == QTAM_F32 && p->hp.ctot < (int64_t(1) << 31);
@@ -637,7 +651,7 @@ static const char *const kKernelNames[K_COUNT] = {
     "inv_rows", "inv_reduce", "dense_place", "threshold", "r2c_fast", "fwd_rows_fast", "inv_rows_fast",
     "reduce_c2r_fast", "inv_fused", "inv_tiles", "combine_c2r", "threshold_fast", "rows_cta_fwd", "rows_cta_inv",
     "tiny_rows_fwd", "tiny_rows_inv", "long_fft_a", "long_fft_b", "plane_metric", "best_plane", "remodulate", "inst_freq", "fwd_rows_thr", "gather_plane",
-    "rows_cl_fwd", "rows_cl_inv", "combine_runs", "c2c_fast"};
+    "rows_cl_fwd", "rows_cl_inv", "combine_runs", "c2c_fast", "split3", "combine3"};
 
 qtam_status qtam_profile_enable(qtam_plan *p, int on, int max_launches) {
   if (!p || p->host_only) return QTAM_ERR_INVALID_ARG;

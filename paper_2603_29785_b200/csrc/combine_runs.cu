@@ -127,8 +127,7 @@ qtam_status build_runs(qtam_plan *p) {
 
 qtam_status combine_runs(qtam_plan *p, int batch, int plane, cudaStream_t st) {
   const int Nc = (int)(p->hp.N / 2);
-  const int tw_shift = ilog2(p->twn) - ilog2(p->hp.N);
-  if (tw_shift < 0) return QTAM_ERR_UNSUPPORTED;
+  const int tw_shift = 0;            // d_twN[f] = e^{2 pi i f/N}
   double run_bins = 0;
   for (const HostRun &r : p->runs) run_bins += (double)r.nb;
   dim3 g((unsigned)p->n_run_blocks, (unsigned)batch);
@@ -138,7 +137,7 @@ qtam_status combine_runs(qtam_plan *p, int batch, int plane, cudaStream_t st) {
         p->d_runs, p->d_run_ptr, p->d_run_idx, static_cast<const float2 *>(p->d_part), p->part_stride,
         static_cast<const float2 *>(p->d_band), p->hp.sumL,
         static_cast<const float *>(p->d_invP) + (size_t)(plane + 1) * (size_t)p->hp.nb, Nc, plane,
-        static_cast<const float2 *>(p->d_tw), tw_shift, static_cast<float2 *>(p->d_spec), p->xstride);
+        static_cast<const float2 *>(p->d_twN), tw_shift, static_cast<float2 *>(p->d_spec), p->xstride);
   }
   QTAM_LAUNCH_CHECK();
   return QTAM_OK;

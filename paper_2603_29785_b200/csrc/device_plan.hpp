@@ -14,7 +14,7 @@ enum KernelId {
   K_INV_ROWS, K_INV_REDUCE, K_DENSE_PLACE, K_THRESHOLD, K_R2C_FAST, K_FWD_ROWS_FAST, K_INV_ROWS_FAST,
   K_REDUCE_C2R_FAST, K_INV_FUSED, K_INV_TILES, K_COMBINE_C2R, K_THRESHOLD_FAST, K_ROWS_CTA_FWD, K_ROWS_CTA_INV,
   K_TINY_FWD, K_TINY_INV, K_LONG_A, K_LONG_B, K_PLANE_METRIC, K_BEST_PLANE, K_REMODULATE, K_INST_FREQ, K_FWD_ROWS_THR, K_GATHER_PLANE,
-  K_ROWS_CL_FWD, K_ROWS_CL_INV, K_COMBINE_RUNS, K_C2C_FAST, K_COUNT
+  K_ROWS_CL_FWD, K_ROWS_CL_INV, K_COMBINE_RUNS, K_C2C_FAST, K_SPLIT3, K_COMBINE3, K_COUNT
 };
 // fast float path (fast.cu): rows with 32 <= M <= 1024, grouped by G = M/32 lanes per row
 struct FastRow { int kc, dk, woff, goff, offset, plane, wpad, pad; };   // wpad: offset into the padded window table
@@ -83,13 +83,17 @@ struct qtam_plan {
   int esz = 4;                 // sizeof real: 4 or 8
   int max_batch = 1;
   int64_t xstride = 0;         // spectrum segment stride in complex elements (>= N/2+1, padded)
-  int64_t twn = 0;             // twiddle table length (= N): tw[k] = e^{+2 pi i k/N}
+  int64_t twn = 0;             // twiddle table length, a power of two: tw[k] = e^{+2 pi i k/twn} (= N when N = 2^k)
+  bool n_pow2 = true;          // N = 2^k; otherwise N = 3 * 2^k and the long transform takes a radix-3 step
+  int64_t sub_n = 0;           // points of the power-of-two complex FFT behind the long real transform (N/2 or N/6)
   int cap_log2 = 0;            // generic path: largest in-smem FFT is 2^cap_log2 points
 
   // device tables
   qtam::RowDev *d_rows = nullptr;
   void *d_win = nullptr;       // real[sumL]
   void *d_tw = nullptr;        // complex[twn]
+  void *d_twN = nullptr;       // complex[N]: e^{+2 pi i k/N} (the same table when N is a power of two)
+  void *d_ws3 = nullptr;       // complex[2][max_batch][N]: scratch of the radix-3 step (N = 3 * 2^k only)
   void *d_invP = nullptr;      // real[(nP+1)*nb], 0 outside the cover set
   int32_t *d_csr_ptr = nullptr;
   int32_t *d_csr_idx = nullptr;

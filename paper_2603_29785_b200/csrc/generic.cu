@@ -205,6 +205,37 @@ __global__ void k_cfft_rows(const C2<T> *__restrict__ in, long long in_stride, C
   }
 }
 
+// Radix-3 step of a complex FFT of n = 3 Np points (segment lengths N = 3 * 2^k: the paper's 6 s at 4096 Hz,
+// :178, :339), decimation in time: F_r = DFT_Np of z[3 n2 + r], Z[k + Np m] = sum_r w_3^{r m} w_n^{r k} F_r[k].
+// k_split3 separates the three decimated sequences, the power-of-two transform runs on them, k_combine3 is the
+// butterfly.  tw: e^{+2 pi i k/N} (period N = tw_mul * n).
+template <typename T>
+__global__ void k_split3(const C2<T> *__restrict__ in, long long in_stride, C2<T> *__restrict__ a, int Np) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= 3 * Np) return;
+  a[(long long)blockIdx.y * 3 * Np + (long long)(i % 3) * Np + i / 3] = in[(long long)blockIdx.y * in_stride + i];
+}
+
+template <typename T>
+__global__ void k_combine3(const C2<T> *__restrict__ b, C2<T> *__restrict__ out, long long out_stride, int Np,
+                           int dir, const C2<T> *__restrict__ tw, long long tw_mul, long long N, T scale) {
+  typedef C2<T> V;
+  const int k = blockIdx.x * blockDim.x + threadIdx.x;
+  if (k >= Np) return;
+  const V *B = b + (long long)blockIdx.y * 3 * Np;
+  const V f0 = B[k];
+  const V a1 = cmul(B[Np + k], tw_get(tw, ((long long)k * tw_mul) % N, dir));
+  const V a2 = cmul(B[2 * (long long)Np + k], tw_get(tw, (2LL * k * tw_mul) % N, dir));
+  // w_3 = -1/2 + dir i sqrt(3)/2:  w_3 a1 + w_3^2 a2 = -(a1 + a2)/2 + dir i (sqrt(3)/2) (a1 - a2)
+  const V s = cadd(a1, a2), d = csub(a1, a2);
+  const T h = (T)0.86602540378443864676 * (T)dir;
+  const V m = cmk<T>(f0.x - (T)0.5 * s.x, f0.y - (T)0.5 * s.y), r = cmk<T>(-h * d.y, h * d.x);
+  V *O = out + (long long)blockIdx.y * out_stride;
+  O[k] = cscale(cadd(f0, s), scale);
+  O[Np + k] = cscale(cadd(m, r), scale);
+  O[2 * (long long)Np + k] = cscale(csub(m, r), scale);
+}
+
 // a1 tail: X[f] from the half-length complex FFT Z of z[m] = x[2m] + i x[2m+1]; in place in `spec`
 //   X[f] = (Z[f] + conj Z[Nc-f])/2 - (i/2) e^{-2 pi i f/N} (Z[f] - conj Z[Nc-f]),  f = 0..Nc
 template <typename T>
@@ -506,18 +537,47 @@ static qtam_status cfft(qtam_plan *p, const C2<T> *in, long long in_stride, C2<T
   return QTAM_OK;
 }
 
+// complex FFT of n = 2^a or 3 * 2^a points (the latter through the plan's radix-3 scratch: in and out are free
+// to alias, tmp is not used)
+template <typename T>
+static qtam_status cfft_any(qtam_plan *p, const C2<T> *in, long long in_stride, C2<T> *out, long long out_stride,
+                            C2<T> *tmp, long long tmp_stride, long long n, int count, int dir, T scale,
+                            cudaStream_t st, double algo_in = 0.0, double algo_out = 0.0) {
+  if ((n & (n - 1)) == 0)
+    return cfft<T>(p, in, in_stride, out, out_stride, tmp, tmp_stride, ilog2(n), count, dir, scale, st, algo_in, algo_out);
+  if (n % 3 != 0 || !p->d_ws3 || p->hp.N % n != 0 || n > p->hp.N) return QTAM_ERR_UNSUPPORTED;
+  const int Np = (int)(n / 3);
+  C2<T> *A = static_cast<C2<T> *>(p->d_ws3), *B = A + (size_t)p->max_batch * (size_t)p->hp.N;
+  dim3 g3((unsigned)((3 * Np + 255) / 256), (unsigned)count), g1((unsigned)((Np + 255) / 256), (unsigned)count);
+  const double bytes = 2.0 * sizeof(C2<T>) * (double)count * (double)n;
+  {
+    LaunchScope ls(p, st, K_SPLIT3, algo_in, bytes);
+    k_split3<T><<<g3, 256, 0, st>>>(in, in_stride, A, Np);
+  }
+  QTAM_LAUNCH_CHECK();
+  qtam_status s = cfft<T>(p, A, Np, B, Np, A, Np, ilog2(Np), 3 * count, dir, (T)1, st);
+  if (s != QTAM_OK) return s;
+  {
+    LaunchScope ls(p, st, K_COMBINE3, algo_out, bytes);
+    k_combine3<T><<<g1, 256, 0, st>>>(B, out, out_stride, Np, dir, static_cast<const C2<T> *>(p->d_twN),
+                                      p->hp.N / n, p->hp.N, scale);
+  }
+  QTAM_LAUNCH_CHECK();
+  return QTAM_OK;
+}
+
 template <typename T>
 static qtam_status r2c_t(qtam_plan *p, const void *d_x, int batch, cudaStream_t st) {
   const int Nc = (int)(p->hp.N / 2);
   C2<T> *spec = static_cast<C2<T> *>(p->d_spec);
   C2<T> *ws = static_cast<C2<T> *>(p->d_ws);
-  qtam_status s = cfft<T>(p, static_cast<const C2<T> *>(d_x), Nc, spec, p->xstride, ws, p->hp.N,
-                          ilog2(Nc), batch, -1, (T)1, st, (double)batch * sizeof(T) * (double)p->hp.N, 0.0);
+  qtam_status s = cfft_any<T>(p, static_cast<const C2<T> *>(d_x), Nc, spec, p->xstride, ws, p->hp.N,
+                              Nc, batch, -1, (T)1, st, (double)batch * sizeof(T) * (double)p->hp.N, 0.0);
   if (s != QTAM_OK) return s;
   dim3 g((Nc / 2 + 1 + 255) / 256, batch);
   {
     LaunchScope ls(p, st, K_R2C_POST, 0.0, 2.0 * sizeof(C2<T>) * (double)batch * (double)Nc);
-    k_r2c_post<T><<<g, 256, 0, st>>>(spec, p->xstride, Nc, static_cast<const C2<T> *>(p->d_tw));
+    k_r2c_post<T><<<g, 256, 0, st>>>(spec, p->xstride, Nc, static_cast<const C2<T> *>(p->d_twN));
   }
   QTAM_LAUNCH_CHECK();
   return QTAM_OK;
@@ -619,19 +679,19 @@ static qtam_status c2r_t(qtam_plan *p, int batch, void *d_x_out, cudaStream_t st
   dim3 g((Nc / 2 + 1 + 255) / 256, batch);
   {
     LaunchScope ls(p, st, K_C2R_PRE, 0.0, 2.0 * sizeof(C2<T>) * (double)batch * (double)Nc);
-    k_c2r_pre<T><<<g, 256, 0, st>>>(spec, p->xstride, Nc, static_cast<const C2<T> *>(p->d_tw));
+    k_c2r_pre<T><<<g, 256, 0, st>>>(spec, p->xstride, Nc, static_cast<const C2<T> *>(p->d_twN));
   }
   QTAM_LAUNCH_CHECK();
-  return cfft<T>(p, spec, p->xstride, static_cast<C2<T> *>(d_x_out), Nc, static_cast<C2<T> *>(p->d_ws),
-                 p->hp.N, ilog2(Nc), batch, +1, (T)1, st, 0.0, (double)batch * sizeof(T) * (double)p->hp.N);
+  return cfft_any<T>(p, spec, p->xstride, static_cast<C2<T> *>(d_x_out), Nc, static_cast<C2<T> *>(p->d_ws),
+                     p->hp.N, Nc, batch, +1, (T)1, st, 0.0, (double)batch * sizeof(T) * (double)p->hp.N);
 }
 
 // the complex FFT alone, for a spectrum buffer that already holds the pre-processed Z (k_combine_runs)
 qtam_status generic_c2c_out(qtam_plan *p, int batch, void *d_x_out, cudaStream_t st) {
   const int Nc = (int)(p->hp.N / 2);
-  return cfft<float>(p, static_cast<const float2 *>(p->d_spec), p->xstride, static_cast<float2 *>(d_x_out), Nc,
-                     static_cast<float2 *>(p->d_ws), p->hp.N, ilog2(Nc), batch, +1, 1.f, st, 0.0,
-                     (double)batch * 4.0 * (double)p->hp.N);
+  return cfft_any<float>(p, static_cast<const float2 *>(p->d_spec), p->xstride, static_cast<float2 *>(d_x_out), Nc,
+                         static_cast<float2 *>(p->d_ws), p->hp.N, Nc, batch, +1, 1.f, st, 0.0,
+                         (double)batch * 4.0 * (double)p->hp.N);
 }
 
 qtam_status generic_c2r(qtam_plan *p, int batch, void *d_x_out, cudaStream_t st) {
@@ -653,8 +713,8 @@ static qtam_status dense_t(qtam_plan *p, int batch, int row_begin, int row_end, 
                                           (T)(p->hp.opt.epsilon * p->hp.rows[(size_t)k].norm));
     }
     QTAM_LAUNCH_CHECK();
-    qtam_status s = cfft<T>(p, ws, N, out + (long long)(k - row_begin) * N, (long long)nr * N, ws, N,
-                            ilog2(N), batch, +1, (T)1, st);
+    qtam_status s = cfft_any<T>(p, ws, N, out + (long long)(k - row_begin) * N, (long long)nr * N, ws, N,
+                                N, batch, +1, (T)1, st);
     if (s != QTAM_OK) return s;
   }
   return QTAM_OK;
@@ -667,7 +727,7 @@ static qtam_status dense_invert_t(qtam_plan *p, const void *d_tile, int batch, i
   // for small configurations, like qtam_dense)
   if (ilog2(N) > p->cap_log2) return QTAM_ERR_UNSUPPORTED;
   C2<T> *ws = static_cast<C2<T> *>(p->d_ws);
-  qtam_status s = cfft<T>(p, static_cast<const C2<T> *>(d_tile), N, ws, N, ws, N, ilog2(N), batch, -1, (T)1, st);
+  qtam_status s = cfft_any<T>(p, static_cast<const C2<T> *>(d_tile), N, ws, N, ws, N, N, batch, -1, (T)1, st);
   if (s != QTAM_OK) return s;
   dim3 g((unsigned)((p->hp.nb + 255) / 256), batch);
   {

@@ -114,7 +114,7 @@ qtam_status fast_cfft_long(qtam_plan *p, const void *in, long long in_stride, vo
 
 qtam_status build_long_fft(qtam_plan *p) {
   int lnc = 0;
-  while ((int64_t(2) << lnc) < p->hp.N) ++lnc;     // log2 (N/2)
+  while ((int64_t(1) << lnc) < p->sub_n) ++lnc;    // log2 of the power-of-two complex FFT behind the long transform
   if (p->esz != 4 || lnc <= kLongLog2N2 || lnc > kLongLog2N2 + 5) return QTAM_OK;
   std::vector<float> t;
   fill_cta_fft_tables<kLongLog2N2, CtaFftPlan<kLongLog2N2>::NT>(t);

@@ -34,7 +34,9 @@ static double window_value(int type, double par, int64_t j, int64_t dk) {
 
 qtam_status build_host_plan(HostPlan &hp, double fs, int64_t N, const double *Q, int nQ, double fmin,
                             double fmax, double spacing, qtam_dtype dtype, const qtam_options *uopt) {
-  if (!Q || nQ < 1 || !(fs > 0.0) || !pow2(N) || N < 8) return QTAM_ERR_INVALID_ARG;
+  // segment lengths: 2^k, or 3 * 2^k (the paper's own benchmark shape is 6 s at 4096 Hz = 24576 samples, :178, :339)
+  const bool n_ok = pow2(N) || (N % 3 == 0 && pow2(N / 3));
+  if (!Q || nQ < 1 || !(fs > 0.0) || !n_ok || N < 8 || N % 8 != 0) return QTAM_ERR_INVALID_ARG;
   if (dtype != QTAM_F32 && dtype != QTAM_F64) return QTAM_ERR_INVALID_ARG;
   if (N > (int64_t(1) << 26)) return QTAM_ERR_UNSUPPORTED;
 

@@ -185,6 +185,51 @@ def test_mid_length_segments(log2n):
     assert worst_segment(g.inverse(g.forward(dev(x))).cpu().numpy(), pi_c(x64, C)) <= 1e-5
 
 
+@pytest.mark.parametrize("N,dtype,kw", [(96, "f64", {}), (192, "f32", {}), (1536, "f64", dict(clamp_overlap=2.0)),
+                                        (12288, "f32", {}), (24576, "f32", {}), (24576, "f64", {}),
+                                        (49152, "f32", dict(tile_length=-1)), (3 * 2 ** 17, "f32", {})])
+def test_non_power_of_two_segment_length(N, dtype, kw):
+    """N = 3 * 2^k (the paper's own benchmark shape is 6 s at 4096 Hz = 24576 samples; SURVEY
+    8(f) item 1): the long transforms take a radix-3 step; every call against the oracle."""
+    if N >= 1536:
+        args = (4096.0, N, [5.0, 20.0], 40.0 if N == 1536 else 10.0, 0.44 * 4096.0, 14.0)
+    else:
+        args = (float(N), N, [4.0, 8.0], 5.0, 0.42 * N, 7.0)
+    g, r = make_plans(args, dtype, 2, **kw)
+    assert [(a.kc, a.dk, a.M, a.offset) for a in g.rows] == [(b.kc, b.dk, b.M, b.offset) for b in r.rows]
+    x = inputs.white_noise(N, 300 + N % 97, batch=2).astype(np_rdt(dtype))
+    x64 = x.astype(np.float64)
+    Yg = g.forward(dev(x)).cpu().numpy()
+    Yr = r.forward(x64, engine=1)
+    assert worst_segment(Yg, Yr) <= TOL[dtype]
+    assert worst_row(Yg, Yr, r) <= TOL_ROW[dtype]
+    rng = np.random.default_rng(N)
+    Yin = (rng.standard_normal((2, g.ctot)) + 1j * rng.standard_normal((2, g.ctot))).astype(Yg.dtype)
+    for plane in (-1, 1):
+        xg = g.inverse(dev(Yin), plane=plane).cpu().numpy()
+        assert worst_segment(xg, r.inverse(Yin.astype(np.complex128), plane=plane, engine=1)) <= TOL[dtype], plane
+    _, C = r.frame(-1)
+    assert worst_segment(g.inverse(g.forward(dev(x))).cpu().numpy(), pi_c(x64, C)) <= TOL_RT[dtype]
+    if N <= 1536:
+        Dg = g.dense(dev(x)).cpu().numpy()
+        assert worst_segment(Dg.reshape(2, -1), r.dense(x64, engine=1).reshape(2, -1)) <= TOL[dtype]
+    two = g.threshold_rowmedian(g.forward(dev(x)), 3.0)
+    assert torch.equal(torch.view_as_real(g.forward_threshold(dev(x), 3.0)), torch.view_as_real(two))
+
+
+def test_paper_benchmark_shape():
+    """6 s at 4096 Hz, 62 rows at a batch of 64: forward and round trip"""
+    name = "paper6s"
+    g, r = make_plans(inputs.plan_args(name), "f32", 64)
+    x = inputs.make_batch(name, batch=64)
+    x64 = x.astype(np.float64)
+    Y = g.forward(dev(x))
+    Yr = r.forward(x64, engine=1)
+    assert worst_segment(Y.cpu().numpy(), Yr) <= 2e-5 and worst_row(Y.cpu().numpy(), Yr, r) <= TOL_ROW["f32"]
+    _, C = r.frame(-1)
+    assert worst_segment(g.inverse(Y).cpu().numpy(), pi_c(x64, C)) <= 1e-5
+
+
 @pytest.mark.parametrize("window,par", [("hann", 0.0), ("kaiser", 6.5), ("tukey", 0.4), ("planck", 0.5)])
 @pytest.mark.parametrize("dtype", ["f32", "f64"])
 def test_window_families(window, par, dtype):

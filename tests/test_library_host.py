@@ -30,7 +30,7 @@ def test_status_strings():
     assert b"argument" in L.qtam_status_string(1)
 
 
-@pytest.mark.parametrize("name", ["cfg1", "cfg2", "cfg3", "cfg4", "cfg5"])
+@pytest.mark.parametrize("name", ["cfg1", "cfg2", "cfg3", "cfg4", "cfg5", "paper6s"])
 @pytest.mark.parametrize("ov", [1.0, 2.0])
 def test_host_plan_equals_oracle_plan(name, ov):
     fs, N, Q, fmin, fmax, rows = inputs.plan_args(name)
