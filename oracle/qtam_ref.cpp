@@ -638,6 +638,127 @@ int qtam_ref_inverse(const qtam_ref_plan *p, const double *coef, int batch, int 
   return 0;
 }
 
+// ---- the paper's output-length options (A22: PAPER.md:150, :158-160, :184, :343) ---------------------------------
+// Every row resampled to the same number n of time samples, n any integer >= the largest window (no power of two
+// needed): "standard" n = N/2 + 1 (64 x 410, 62 x 12289), "minimal" n = ceil(N_t Delta f_max) + 1 = the largest
+// window's 2 dk + 1 bins (64 x 33, 62 x 669), or user-set.  C46/C47 with N_out = n:
+//   Y'_k[m] = (N n)^{-1/2} sum_j X[kc + j] W_k[j] e^{+2 pi i j m / n},  m = 0..n-1.
+// Naive long-double sums (the definition); `engine` only selects how the long transform of x is evaluated.
+int64_t qtam_ref_output_length(const qtam_ref_plan *p, int mode) {
+  if (!p) return 0;
+  if (mode == -1) return p->N / 2 + 1;
+  int64_t lmax = 0;
+  for (const Row &r : p->rows) lmax = std::max(lmax, 2 * r.dk + 1);
+  return mode == -2 ? lmax : 0;
+}
+
+int qtam_ref_forward_length(const qtam_ref_plan *p, const double *x, int batch, int64_t n, double *out, int engine) {
+  if (!p || !x || !out || batch < 0 || n < qtam_ref_output_length(p, -2)) return 1;
+  const int K = (int)p->rows.size();
+  std::vector<uint8_t> need = needed_bins(p, 0, K);
+  std::vector<cld> tw((size_t)n);
+  for (int64_t m = 0; m < n; ++m) tw[(size_t)m] = cis(m, n);
+#pragma omp parallel for schedule(dynamic)
+  for (int b = 0; b < batch; ++b) {
+    std::vector<cd> X((size_t)p->nb);
+    spectrum_onesided(x + (size_t)b * p->N, p->N, X.data(), need.data(), engine);
+    cd *Y = reinterpret_cast<cd *>(out) + (size_t)b * (size_t)K * (size_t)n;
+    for (int k = 0; k < K; ++k) {
+      const Row &r = p->rows[(size_t)k];
+      const ld scale = 1.0L / sqrtl((ld)p->N * (ld)n);
+      for (int64_t m = 0; m < n; ++m) {
+        cld acc(0, 0);
+        for (int64_t j = -r.dk; j <= r.dk; ++j) {
+          const int64_t f = r.kc + j;
+          if (f < 0 || f >= p->nb) continue;
+          const int64_t ph = ((j % n + n) % n) * m % n;
+          acc += cld(X[(size_t)f]) * (ld)r.w[(size_t)(j + r.dk)] * tw[(size_t)ph];
+        }
+        acc *= scale;
+        Y[(size_t)k * (size_t)n + (size_t)m] = cd((double)acc.real(), (double)acc.imag());
+      }
+    }
+  }
+  return 0;
+}
+
+// band values of one resampled row: Bhat[j] = sqrt(N/n) sum_m Y'[m] e^{-2 pi i j m / n}, |j| <= dk (C49 with N_out = n)
+static void band_from_length(const qtam_ref_plan *p, const Row &r, const cd *Y, int64_t n, const std::vector<cld> &twn,
+                             std::vector<cld> &B) {
+  B.assign((size_t)(2 * r.dk + 1), cld(0, 0));
+  const ld amp = sqrtl((ld)p->N / (ld)n);
+  for (int64_t j = -r.dk; j <= r.dk; ++j) {
+    const int64_t jm = (j % n + n) % n;
+    cld acc(0, 0);
+    for (int64_t m = 0; m < n; ++m) acc += cld(Y[m]) * std::conj(twn[(size_t)(jm * m % n)]);
+    B[(size_t)(j + r.dk)] = acc * amp;
+  }
+}
+
+int qtam_ref_inverse_length(const qtam_ref_plan *p, const double *in, int batch, int64_t n, int plane, double *x_out,
+                            int engine) {
+  if (!p || !in || !x_out || batch < 0 || plane < -1 || plane >= p->nP || n < qtam_ref_output_length(p, -2)) return 1;
+  const int K = (int)p->rows.size();
+  const std::vector<double> &P = p->P[(size_t)(plane + 1)];
+  const std::vector<uint8_t> &C = p->cover[(size_t)(plane + 1)];
+  std::vector<cld> tw((size_t)n);
+  for (int64_t m = 0; m < n; ++m) tw[(size_t)m] = cis(m, n);
+#pragma omp parallel for schedule(dynamic)
+  for (int b = 0; b < batch; ++b) {
+    const cd *Y = reinterpret_cast<const cd *>(in) + (size_t)b * (size_t)K * (size_t)n;
+    std::vector<cld> S((size_t)p->nb, cld(0, 0)), B;
+    for (int k = 0; k < K; ++k) {
+      const Row &r = p->rows[(size_t)k];
+      if (plane >= 0 && r.plane != plane) continue;
+      band_from_length(p, r, Y + (size_t)k * (size_t)n, n, tw, B);
+      for (int64_t j = -r.dk; j <= r.dk; ++j) {
+        const int64_t f = r.kc + j;
+        if (f < 0 || f >= p->nb) continue;
+        S[(size_t)f] += B[(size_t)(j + r.dk)] * (ld)r.w[(size_t)(j + r.dk)];
+      }
+    }
+    std::vector<cd> Xh((size_t)p->nb, cd(0, 0));
+    for (int64_t f = 0; f < p->nb; ++f)
+      if (C[(size_t)f]) {
+        cld v = S[(size_t)f] / (ld)P[(size_t)f];
+        Xh[(size_t)f] = cd((double)v.real(), (double)v.imag());
+      }
+    inverse_onesided(Xh.data(), p->N, x_out + (size_t)b * p->N, engine);
+  }
+  return 0;
+}
+
+// Re-sampling of a [rows][n_in] image to [rows][n_out] (:160 "up-sampling the compressed image back to the original
+// size", Fig. 3): every row is band limited to its window's 2 dk + 1 bins, so its n_in samples determine the band
+// exactly (n_in >= 2 dk + 1) and the band determines the n_out samples.  With the energy normalisation of C47:
+//   Y''[m] = (n_in n_out)^{-1/2} sum_{|j| <= dk} ( sum_l Y'[l] e^{-2 pi i j l / n_in} ) e^{+2 pi i j m / n_out}.
+int qtam_ref_resample(const qtam_ref_plan *p, const double *in, int batch, int64_t n_in, int64_t n_out, double *out) {
+  const int64_t lmax = qtam_ref_output_length(p, -2);
+  if (!p || !in || !out || batch < 0 || n_in < lmax || n_out < lmax) return 1;
+  const int K = (int)p->rows.size();
+  std::vector<cld> twi((size_t)n_in), two((size_t)n_out);
+  for (int64_t m = 0; m < n_in; ++m) twi[(size_t)m] = cis(m, n_in);
+  for (int64_t m = 0; m < n_out; ++m) two[(size_t)m] = cis(m, n_out);
+#pragma omp parallel for schedule(dynamic) collapse(2)
+  for (int b = 0; b < batch; ++b)
+    for (int k = 0; k < K; ++k) {
+      const Row &r = p->rows[(size_t)k];
+      const cd *Y = reinterpret_cast<const cd *>(in) + ((size_t)b * (size_t)K + (size_t)k) * (size_t)n_in;
+      cd *O = reinterpret_cast<cd *>(out) + ((size_t)b * (size_t)K + (size_t)k) * (size_t)n_out;
+      std::vector<cld> B;
+      band_from_length(p, r, Y, n_in, twi, B);            // = sqrt(N/n_in) DFT
+      const ld scale = 1.0L / sqrtl((ld)p->N * (ld)n_out);
+      for (int64_t m = 0; m < n_out; ++m) {
+        cld acc(0, 0);
+        for (int64_t j = -r.dk; j <= r.dk; ++j)
+          acc += B[(size_t)(j + r.dk)] * two[(size_t)(((j % n_out + n_out) % n_out) * m % n_out)];
+        acc *= scale;
+        O[m] = cd((double)acc.real(), (double)acc.imag());
+      }
+    }
+  return 0;
+}
+
 int qtam_ref_project_cover(const qtam_ref_plan *p, const double *x, int batch, int plane,
                            double *x_out, int engine) {
   if (!p || !x || !x_out || batch < 0 || plane < -1 || plane >= p->nP) return 1;

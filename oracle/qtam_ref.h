@@ -116,6 +116,17 @@ int  qtam_ref_plane_metric(const qtam_ref_plan *p, const double *coef, int batch
 /* Projection onto the cover set: one-sided DFT of x, zero the bins outside C, inverse (R9). */
 int  qtam_ref_project_cover(const qtam_ref_plan *p, const double *x, int batch, int plane,
                             double *x_out, int engine);
+/* The paper's output-length options (A22: PAPER.md:150, :158-160, :184, :343): every row resampled to the same
+ * n time samples, n any integer >= the largest window.  qtam_ref_output_length: mode -1 "standard" N/2+1, mode -2
+ * "minimal" = the largest 2 dk + 1.  forward_length: out [batch][rows][n] complex,
+ * Y'_k[m] = (N n)^{-1/2} sum_j X[kc+j] W_k[j] e^{+2 pi i j m/n} (C46/C47 with N_out = n).  inverse_length: Eq. 11
+ * from such an image (C49 with N_out = n).  resample: [rows][n_in] -> [rows][n_out] through each row's band
+ * (:160, Fig. 3).  Naive long-double sums; `engine` only selects the long transform of x. */
+int64_t qtam_ref_output_length(const qtam_ref_plan *p, int mode);
+int  qtam_ref_forward_length(const qtam_ref_plan *p, const double *x, int batch, int64_t n, double *out, int engine);
+int  qtam_ref_inverse_length(const qtam_ref_plan *p, const double *in, int batch, int64_t n, int plane, double *x_out,
+                             int engine);
+int  qtam_ref_resample(const qtam_ref_plan *p, const double *in, int batch, int64_t n_in, int64_t n_out, double *out);
 /* One-sided spectrum X[f], f=0..N/2 (PAPER.md:365 C1); out is n_bins complex per segment. */
 int  qtam_ref_spectrum(const qtam_ref_plan *p, const double *x, int batch, double *X_out, int engine);
 

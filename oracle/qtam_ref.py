@@ -65,6 +65,11 @@ def lib():
         _lib.qtam_ref_dense_invert.argtypes = [vp, dp, C.c_int, C.c_int, dp]
         _lib.qtam_ref_plane_metric.argtypes = [vp, dp, C.c_int, C.c_int, dp, C.POINTER(C.c_int32)]
         _lib.qtam_ref_project_cover.argtypes = [vp, dp, C.c_int, C.c_int, dp, C.c_int]
+        _lib.qtam_ref_output_length.argtypes = [vp, C.c_int]
+        _lib.qtam_ref_output_length.restype = C.c_int64
+        _lib.qtam_ref_forward_length.argtypes = [vp, dp, C.c_int, C.c_int64, dp, C.c_int]
+        _lib.qtam_ref_inverse_length.argtypes = [vp, dp, C.c_int, C.c_int64, C.c_int, dp, C.c_int]
+        _lib.qtam_ref_resample.argtypes = [vp, dp, C.c_int, C.c_int64, C.c_int64, dp]
         _lib.qtam_ref_spectrum.argtypes = [vp, dp, C.c_int, dp, C.c_int]
         _lib.qtam_ref_dft.argtypes = [dp, dp, C.c_int64, C.c_int]
         _lib.qtam_ref_fft.argtypes = [dp, dp, C.c_int64, C.c_int]
@@ -252,6 +257,35 @@ class RefPlan:
         ptr = c.view(np.float32).ctypes.data_as(C.POINTER(C.c_float))
         assert lib().qtam_ref_threshold_rowmedian_f32(self._h, ptr, c.shape[0], kappa) == 0
         return c
+
+    def output_length(self, mode):
+        """'standard' (N/2 + 1) or 'minimal' (the largest window's 2 dk + 1)"""
+        return int(lib().qtam_ref_output_length(self._h, {"standard": -1, "minimal": -2}[mode]))
+
+    def forward_length(self, x, n, engine=0):
+        """[batch][rows][n]: every row resampled to n time samples (A22)"""
+        x = self._x(x)
+        out = np.empty((x.shape[0], self.n_rows, n), dtype=np.complex128)
+        assert lib().qtam_ref_forward_length(self._h, _dp(x), x.shape[0], n, _dp(out.view(np.float64)), engine) == 0
+        return out
+
+    def inverse_length(self, img, plane=-1, engine=0):
+        img = np.ascontiguousarray(img, dtype=np.complex128)
+        if img.ndim == 2:
+            img = img[None]
+        out = np.empty((img.shape[0], self.N), dtype=np.float64)
+        assert lib().qtam_ref_inverse_length(self._h, _dp(img.view(np.float64)), img.shape[0], img.shape[-1], plane,
+                                             _dp(out), engine) == 0
+        return out
+
+    def resample(self, img, n_out):
+        img = np.ascontiguousarray(img, dtype=np.complex128)
+        if img.ndim == 2:
+            img = img[None]
+        out = np.empty((img.shape[0], self.n_rows, n_out), dtype=np.complex128)
+        assert lib().qtam_ref_resample(self._h, _dp(img.view(np.float64)), img.shape[0], img.shape[-1], n_out,
+                                       _dp(out.view(np.float64))) == 0
+        return out
 
     def project_cover(self, x, plane=-1, engine=0):
         x = self._x(x)

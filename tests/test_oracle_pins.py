@@ -760,3 +760,60 @@ def test_single_tile_inversion_recovers_the_signal():
         assert rel_l2(p.dense_invert(T, k), np.fft.irfft(Xh, n=p.N, axis=-1)) <= 1e-10
     with pytest.raises(ValueError):
         p0.dense_invert(np.zeros((1, p0.N), complex), 0)             # epsilon = 0: undefined
+
+
+# ---- the paper's output-length options (A22) ------------------------------------------------------------------
+
+def test_output_length_options_closed_forms_and_identities():
+    """every row at the same number n of samples, n any integer >= the largest
+    window.  Pins: the lengths themselves; a pure sinusoid's closed form at a non-power-of-two n; row energy (C48);
+    n = the uniform power-of-two tile gives the uniform-tile layout; a numpy construction; re-sampling between any
+    two lengths is exact (Fig. 3); the round trip from the minimal image is Pi_C x."""
+    N = 512
+    p = RefPlan(512.0, N, [4.0, 8.0], 12.0, 200.0, 9)
+    n_std, n_min = p.output_length("standard"), p.output_length("minimal")
+    assert n_std == N // 2 + 1 == 257 and n_min == max(r.L for r in p.rows)
+    x = inputs.white_noise(N, 81, batch=2)
+    for n in (n_min, n_std, 100 if 100 >= n_min else n_min + 7):
+        Y = p.forward_length(x, n)
+        # row energy is that of the dense tile whatever the length (C48)
+        X = np.fft.rfft(x, axis=-1)
+        for k, r in enumerate(p.rows):
+            w = p.window(k)
+            f = np.arange(r.kc - r.dk, r.kc + r.dk + 1)
+            ok = (f >= 0) & (f < p.n_bins)
+            e = np.sum(np.abs(X[:, f[ok]] * w[None, ok]) ** 2, axis=1) / N
+            assert np.allclose(np.sum(np.abs(Y[:, k]) ** 2, axis=1), e, rtol=1e-12)
+            # numpy construction: the band placed at j mod n of an n-array, inverse DFT of length n
+            B = np.zeros((2, n), complex)
+            B[:, (f[ok] - r.kc) % n] = X[:, f[ok]] * w[None, ok]
+            assert rel_l2(Y[:, k], np.fft.ifft(B, axis=-1) * n / np.sqrt(N * n)) <= 1e-12
+    # closed form (P7 at a length that is no power of two): x = cos(2 pi k0 t / T)
+    k0 = 61
+    t = np.arange(N)
+    Yc = p.forward_length(np.cos(2 * np.pi * k0 * t / N), n_std)[0]
+    m = np.arange(n_std)
+    for k, r in enumerate(p.rows):
+        j = k0 - r.kc
+        want = 0.0 * m if abs(j) > r.dk else np.sqrt(N / n_std) * 0.5 * p.window(k)[j + r.dk] * np.exp(2j * np.pi * j * m / n_std)
+        assert np.max(np.abs(Yc[k] - want)) <= 1e-13
+    # n = the uniform power-of-two tile length: the uniform-tile layout of the plan with tile_length = -1
+    pu = RefPlan(512.0, N, [4.0, 8.0], 12.0, 200.0, 9, tile_length=-1)
+    Mu = pu.rows[0].M
+    assert rel_l2(p.forward_length(x, Mu).reshape(2, -1), pu.forward(x)) <= 1e-12
+    # re-sampling is exact in both directions, and composes (Fig. 3: down-sample, up-sample, residual ~ rounding)
+    Ymin, Ystd = p.forward_length(x, n_min), p.forward_length(x, n_std)
+    assert rel_l2(p.resample(Ymin, n_std), Ystd) <= 1e-12
+    assert rel_l2(p.resample(Ystd, n_min), Ymin) <= 1e-12
+    assert rel_l2(p.resample(p.resample(Ystd, n_min), n_std), Ystd) <= 1e-12
+    # round trip from either image
+    _, C = p.frame(-1)
+    proj = np.fft.irfft(np.where(C[None, :], np.fft.rfft(x, axis=-1), 0), n=N, axis=-1)
+    assert rel_l2(p.inverse_length(Ymin), proj) <= 1e-12 and rel_l2(p.inverse_length(Ystd), proj) <= 1e-12
+    for plane in (0, 1):
+        _, Cp = p.frame(plane)
+        projp = np.fft.irfft(np.where(Cp[None, :], np.fft.rfft(x, axis=-1), 0), n=N, axis=-1)
+        assert rel_l2(p.inverse_length(Ystd, plane=plane), projp) <= 1e-12
+    # a length below the largest window aliases: refused
+    with pytest.raises(AssertionError):
+        p.forward_length(x, n_min - 1)
