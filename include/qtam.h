@@ -78,6 +78,11 @@ typedef struct {
   double  epsilon;                  /* Eq. 12 (R17): unnormalised window value
                                        off the support (and floor on it) for qtam_dense and
                                        qtam_dense_invert only; 0 = plain windows [default]           */
+  int64_t out_length;               /* the paper's output-resolution option (:150, :158-160, :184, :343) for
+                                       qtam_forward_length / _inverse_length / _resample: 0 = not used
+                                       [default]; -1 = "standard" N/2 + 1; -2 = "minimal", the largest
+                                       window's 2 dk + 1 (= ceil(N_t Delta f_max) + 1, R18);
+                                       n > 0 = user-set, any integer >= the largest window             */
 } qtam_options;
 
 /* Host-side row table entry; rows are ordered plane-major (Q list order), ascending frequency. */
@@ -143,6 +148,21 @@ qtam_status qtam_dense(qtam_plan *p, const void *d_x, int batch, int row_begin, 
  * amplified by up to 1/epsilon.  N up to 8192 (float) / 4096 (double): a check path like qtam_dense.
  * QTAM_ERR_INVALID_ARG when the plan's epsilon is 0. */
 qtam_status qtam_dense_invert(qtam_plan *p, const void *d_tile, int batch, int row, void *d_x_out, void *stream);
+
+/* The paper's output-length options (plans created with out_length != 0).
+ * Every row at the same number n = qtam_output_length(p, 0) of time samples, n any integer >= the largest window
+ * (no power of two): d_img = [batch][n_rows][n] complex, row k at time t_m = m T / n,
+ *   forward_length   Y'_k[m] = (N n)^(-1/2) sum_j X[kc+j] W_k[j] e^{+2 pi i j m / n}      (C46 / C47 with N_out = n)
+ *   inverse_length   Eq. 11 from such an image (C49 with N_out = n); plane as in qtam_inverse
+ *   resample         to_standard = 1: [n_rows][n] -> [n_rows][N/2+1]  ("up-sampling the compressed image back to
+ *                    the original size", :160, Fig. 3); 0: the reverse.  Exact: every row is band limited to its window.
+ * qtam_output_length: mode 0 = the plan's n, -1 = N/2 + 1, -2 = the largest window (0 when the plan has none).
+ * The short transforms are direct sums over the window's support, O(n L) per row: a layout converter for images of
+ * the paper's sizes, not a step of the hot path.  QTAM_ERR_INVALID_ARG on a plan created with out_length = 0. */
+int64_t     qtam_output_length(const qtam_plan *p, int mode);
+qtam_status qtam_forward_length(qtam_plan *p, const void *d_x, int batch, void *d_img, void *stream);
+qtam_status qtam_inverse_length(qtam_plan *p, const void *d_img, int batch, int plane, void *d_x_out, void *stream);
+qtam_status qtam_resample(qtam_plan *p, const void *d_in, int batch, int to_standard, void *d_out, void *stream);
 
 /* Row-median threshold in place (BASELINE.json config 5; R11): per (segment,row),
  * m = median_n |Y_k[n]| (two middle values averaged), zero every Y_k[n] with |Y_k[n]| < kappa*m.

@@ -19,7 +19,8 @@ STATUS = {0: "ok", 1: "invalid argument", 2: "unsupported", 3: "alloc", 4: "cuda
 SYMBOLS = ["qtam_plan_create", "qtam_plan_create_host", "qtam_plan_destroy", "qtam_plan_info",
            "qtam_plan_rows", "qtam_plan_window", "qtam_plan_frame", "qtam_forward", "qtam_inverse",
            "qtam_dense", "qtam_dense_invert", "qtam_threshold_rowmedian", "qtam_forward_threshold", "qtam_plane_metric", "qtam_gather_plane", "qtam_max_plane_coeffs", "qtam_remodulate", "qtam_instantaneous_frequency", "qtam_last_launch_count", "qtam_status_string",
-           "qtam_profile_enable", "qtam_profile_read"]
+           "qtam_profile_enable", "qtam_profile_read", "qtam_output_length", "qtam_forward_length", "qtam_inverse_length",
+           "qtam_resample"]
 
 
 class QtamError(RuntimeError):
@@ -33,7 +34,8 @@ class Options(C.Structure):
                 ("clamp_overlap", C.c_double), ("max_window_bins", C.c_int64),
                 ("cover_floor", C.c_double), ("rows_are_bins_per_octave", C.c_int),
                 ("max_batch", C.c_int), ("window_param", C.c_double),
-                ("freqs", C.POINTER(C.c_double)), ("n_freqs", C.c_int), ("tile_length", C.c_int64), ("epsilon", C.c_double)]
+                ("freqs", C.POINTER(C.c_double)), ("n_freqs", C.c_int), ("tile_length", C.c_int64), ("epsilon", C.c_double),
+                ("out_length", C.c_int64)]
 
 
 WINDOWS = {"bisquare": 0, "hann": 1, "kaiser": 2, "tukey": 3, "planck": 4}
@@ -94,6 +96,11 @@ def lib():
         L.qtam_profile_enable.argtypes = [vp, C.c_int, C.c_int]
         L.qtam_profile_read.argtypes = [vp, C.POINTER(KernelStat), C.c_int]
         L.qtam_profile_read.restype = C.c_int
+        L.qtam_output_length.argtypes = [vp, C.c_int]
+        L.qtam_output_length.restype = C.c_int64
+        L.qtam_forward_length.argtypes = [vp, vp, C.c_int, vp, vp]
+        L.qtam_inverse_length.argtypes = [vp, vp, C.c_int, C.c_int, vp, vp]
+        L.qtam_resample.argtypes = [vp, vp, C.c_int, C.c_int, vp, vp]
         _lib = L
     return _lib
 
@@ -108,7 +115,8 @@ class Plan:
 
     def __init__(self, fs, N, Q, fmin, fmax, spacing, dtype="f32", max_batch=1, clamp_mode=1,
                  clamp_overlap=1.0, max_window_bins=0, cover_floor=1e-2, rows_are_bins_per_octave=0,
-                 host_only=False, window="bisquare", window_param=0.0, freqs=None, tile_length=0, epsilon=0.0):
+                 host_only=False, window="bisquare", window_param=0.0, freqs=None, tile_length=0, epsilon=0.0,
+                 out_length=0):
         L = lib()
         self._h = C.c_void_p()
         self.dtype = dtype
@@ -117,7 +125,8 @@ class Plan:
         opt = Options(C.sizeof(Options), WINDOWS[window], clamp_mode, clamp_overlap, max_window_bins,
                       cover_floor, rows_are_bins_per_octave, max_batch, float(window_param),
                       None if fr is None else fr.ctypes.data_as(C.POINTER(C.c_double)),
-                      0 if fr is None else fr.size, int(tile_length), float(epsilon))
+                      0 if fr is None else fr.size, int(tile_length), float(epsilon),
+                      {"standard": -1, "minimal": -2}.get(out_length, out_length))
         fn = L.qtam_plan_create_host if host_only else L.qtam_plan_create
         code = fn(C.byref(self._h), float(fs), int(N), q.ctypes.data_as(C.POINTER(C.c_double)), q.size,
                   float(fmin), float(fmax), float(spacing), QTAM_F64 if dtype == "f64" else QTAM_F32,
@@ -255,6 +264,48 @@ class Plan:
         out = t.empty((batch, self.N), dtype=self._rdt(), device=tile.device)
         _check(lib().qtam_dense_invert(self._h, tile.data_ptr(), batch, int(row), out.data_ptr(), self._stream()),
                "qtam_dense_invert")
+        return out
+
+    def output_length(self, mode=0):
+        """the plan's uniform output length (mode 0), the 'standard' N/2 + 1 (-1) or the 'minimal' one (-2)"""
+        return int(lib().qtam_output_length(self._h, {"standard": -1, "minimal": -2}.get(mode, mode)))
+
+    def forward_length(self, x):
+        """[batch][rows][n] image at the plan's uniform output length (the paper's output-resolution option)"""
+        t = self._torch()
+        n = self.output_length()
+        if n <= 0:
+            raise ValueError("the plan was created without out_length")
+        self._need(x, self._rdt(), "x", last=self.N)
+        batch = self._batch(x, self.N, "x")
+        out = t.empty((batch, self.n_rows, n), dtype=self._cdt(), device=x.device)
+        _check(lib().qtam_forward_length(self._h, x.data_ptr(), batch, out.data_ptr(), self._stream()), "qtam_forward_length")
+        return out
+
+    def inverse_length(self, img, plane=-1):
+        t = self._torch()
+        n = self.output_length()
+        if n <= 0:
+            raise ValueError("the plan was created without out_length")
+        self._need(img, self._cdt(), "img", last=n)
+        batch = self._batch(img, self.n_rows * n, "img")
+        out = t.empty((batch, self.N), dtype=self._rdt(), device=img.device)
+        _check(lib().qtam_inverse_length(self._h, img.data_ptr(), batch, plane, out.data_ptr(), self._stream()),
+               "qtam_inverse_length")
+        return out
+
+    def resample(self, img, to_standard=True):
+        """between the plan's length and the standard N/2 + 1 (Fig. 3 of the paper); exact for band-limited rows"""
+        t = self._torch()
+        n, ns = self.output_length(), self.output_length(-1)
+        n_in, n_out = (n, ns) if to_standard else (ns, n)
+        if n <= 0:
+            raise ValueError("the plan was created without out_length")
+        self._need(img, self._cdt(), "img", last=n_in)
+        batch = self._batch(img, self.n_rows * n_in, "img")
+        out = t.empty((batch, self.n_rows, n_out), dtype=self._cdt(), device=img.device)
+        _check(lib().qtam_resample(self._h, img.data_ptr(), batch, 1 if to_standard else 0, out.data_ptr(), self._stream()),
+               "qtam_resample")
         return out
 
     def threshold_rowmedian(self, coef, kappa=3.0):

@@ -55,6 +55,7 @@ void free_plan(qtam_plan *p) {
   for (int c = 0; c < kClClasses; ++c) { cudaFree(p->d_cl_lead[c]); cudaFree(p->d_cl_mem[c]); cudaFree(p->d_cl_groups[c]); cudaFree(p->d_cl_ftw[c]); }
   cudaFree(p->d_cl_ptw);
   cudaFree(p->d_runs); cudaFree(p->d_run_ptr); cudaFree(p->d_run_idx);
+  cudaFree(p->d_len_tw[0]); cudaFree(p->d_len_tw[1]);
   cudaFree(p->d_trows); cudaFree(p->d_titems); cudaFree(p->d_part); cudaFree(p->d_counter);
   for (ProfRec &r : p->prof_pool) { cudaEventDestroy(r.e0); cudaEventDestroy(r.e1); }
   delete p;
@@ -405,6 +406,7 @@ qtam_status qtam_plan_create(qtam_plan **out, double fs, int64_t N, const double
   if (s == QTAM_OK && p->fast_rows) s = build_rows_cluster(p);
   if (s == QTAM_OK && p->fast_rows) s = build_runs(p);
   if (s == QTAM_OK) s = prepare_fast(p);
+  if (s == QTAM_OK) s = build_length(p);
   if (s != QTAM_OK) { free_plan(p); cudaGetLastError(); return s; }
   if (cudaDeviceSynchronize() != cudaSuccess) { free_plan(p); return QTAM_ERR_CUDA; }
   *out = p;
@@ -592,6 +594,44 @@ qtam_status qtam_dense_invert(qtam_plan *p, const void *d_tile, int batch, int r
   return generic_dense_invert(p, d_tile, batch, row, d_x_out, static_cast<cudaStream_t>(stream));
 }
 
+int64_t qtam_output_length(const qtam_plan *p, int mode) {
+  if (!p) return 0;
+  if (mode == 0) return p->host_only ? length_resolve(p->hp, p->hp.opt.out_length) : p->len_n;
+  return mode == -1 || mode == -2 ? length_resolve(p->hp, mode) : 0;
+}
+
+qtam_status qtam_forward_length(qtam_plan *p, const void *d_x, int batch, void *d_img, void *stream) {
+  if (p && p->host_only) return QTAM_ERR_CUDA;
+  if (!check_call(p, d_x, d_img, batch) || p->len_n == 0) return QTAM_ERR_INVALID_ARG;
+  p->last_launches = 0;
+  if (batch == 0) return QTAM_OK;
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  const qtam_status s = p->fast_long ? fast_r2c(p, d_x, batch, st) : generic_r2c(p, d_x, batch, st);
+  if (s != QTAM_OK) return s;
+  return length_forward(p, batch, d_img, st);
+}
+
+qtam_status qtam_inverse_length(qtam_plan *p, const void *d_img, int batch, int plane, void *d_x_out, void *stream) {
+  if (p && p->host_only) return QTAM_ERR_CUDA;
+  if (!check_call(p, d_img, d_x_out, batch) || p->len_n == 0 || plane < -1 || plane >= p->hp.nP)
+    return QTAM_ERR_INVALID_ARG;
+  p->last_launches = 0;
+  if (batch == 0) return QTAM_OK;
+  cudaStream_t st = static_cast<cudaStream_t>(stream);
+  qtam_status s = length_inverse_bands(p, d_img, batch, plane, st);       // every row's windowed band (C49)
+  if (s == QTAM_OK) s = generic_inverse_reduce(p, batch, plane, st);      // sum over rows, 1/P (Eq. 11)
+  if (s == QTAM_OK) s = generic_c2r(p, batch, d_x_out, st);
+  return s;
+}
+
+qtam_status qtam_resample(qtam_plan *p, const void *d_in, int batch, int to_standard, void *d_out, void *stream) {
+  if (p && p->host_only) return QTAM_ERR_CUDA;
+  if (!check_call(p, d_in, d_out, batch) || p->len_n == 0) return QTAM_ERR_INVALID_ARG;
+  p->last_launches = 0;
+  if (batch == 0) return QTAM_OK;
+  return length_resample(p, d_in, batch, to_standard != 0, d_out, static_cast<cudaStream_t>(stream));
+}
+
 qtam_status qtam_threshold_rowmedian(qtam_plan *p, void *d_coef, int batch, double kappa, void *stream) {
   if (p && p->host_only) return QTAM_ERR_CUDA;
   if (!check_call(p, d_coef, d_coef, batch) || !(kappa >= 0.0)) return QTAM_ERR_INVALID_ARG;
@@ -651,7 +691,7 @@ static const char *const kKernelNames[K_COUNT] = {
     "inv_rows", "inv_reduce", "dense_place", "threshold", "r2c_fast", "fwd_rows_fast", "inv_rows_fast",
     "reduce_c2r_fast", "inv_fused", "inv_tiles", "combine_c2r", "threshold_fast", "rows_cta_fwd", "rows_cta_inv",
     "tiny_rows_fwd", "tiny_rows_inv", "long_fft_a", "long_fft_b", "plane_metric", "best_plane", "remodulate", "inst_freq", "fwd_rows_thr", "gather_plane",
-    "rows_cl_fwd", "rows_cl_inv", "combine_runs", "c2c_fast", "split3", "combine3"};
+    "rows_cl_fwd", "rows_cl_inv", "combine_runs", "c2c_fast", "split3", "combine3", "len_band", "len_synth", "len_analysis"};
 
 qtam_status qtam_profile_enable(qtam_plan *p, int on, int max_launches) {
   if (!p || p->host_only) return QTAM_ERR_INVALID_ARG;

@@ -14,7 +14,8 @@ enum KernelId {
   K_INV_ROWS, K_INV_REDUCE, K_DENSE_PLACE, K_THRESHOLD, K_R2C_FAST, K_FWD_ROWS_FAST, K_INV_ROWS_FAST,
   K_REDUCE_C2R_FAST, K_INV_FUSED, K_INV_TILES, K_COMBINE_C2R, K_THRESHOLD_FAST, K_ROWS_CTA_FWD, K_ROWS_CTA_INV,
   K_TINY_FWD, K_TINY_INV, K_LONG_A, K_LONG_B, K_PLANE_METRIC, K_BEST_PLANE, K_REMODULATE, K_INST_FREQ, K_FWD_ROWS_THR, K_GATHER_PLANE,
-  K_ROWS_CL_FWD, K_ROWS_CL_INV, K_COMBINE_RUNS, K_C2C_FAST, K_SPLIT3, K_COMBINE3, K_COUNT
+  K_ROWS_CL_FWD, K_ROWS_CL_INV, K_COMBINE_RUNS, K_C2C_FAST, K_SPLIT3, K_COMBINE3, K_LEN_BAND, K_LEN_SYNTH, K_LEN_ANALYSIS,
+  K_COUNT
 };
 // fast float path (fast.cu): rows with 32 <= M <= 1024, grouped by G = M/32 lanes per row
 struct FastRow { int kc, dk, woff, goff, offset, plane, wpad, pad; };   // wpad: offset into the padded window table
@@ -189,6 +190,10 @@ struct qtam_plan {
   qtam::KernelCfg cfg_r2c, cfg_rows_fwd, cfg_rows_thr, cfg_rows_inv, cfg_tiles, cfg_combine,
       cfg_rows_cta[qtam::kCtaClasses][2], cfg_rows_cl[qtam::kClClasses][2], cfg_c2c;
 
+  // output-length options (length.cu): the plan's uniform length n, the standard one, e^{2 pi i m/n} for both
+  long long len_n = 0, len_std = 0;
+  void *d_len_tw[2] = {nullptr, nullptr};
+
   int last_launches = 0;
   // launch profile (qtam_profile_enable / qtam_profile_read)
   bool prof_on = false;
@@ -274,6 +279,12 @@ qtam_status cluster_inverse_rows(qtam_plan *p, const void *d_coef, int batch, in
 // combine_runs.cu
 qtam_status build_runs(qtam_plan *p);
 qtam_status combine_runs(qtam_plan *p, int batch, int plane, cudaStream_t st);
+// length.cu
+long long length_resolve(const HostPlan &hp, long long mode);
+qtam_status build_length(qtam_plan *p);
+qtam_status length_forward(qtam_plan *p, int batch, void *d_out, cudaStream_t st);
+qtam_status length_inverse_bands(qtam_plan *p, const void *d_in, int batch, int plane, cudaStream_t st);
+qtam_status length_resample(qtam_plan *p, const void *d_in, int batch, int to_standard, void *d_out, cudaStream_t st);
 // threshold_fast.cu
 qtam_status build_thr_fast(qtam_plan *p);
 qtam_status fast_threshold(qtam_plan *p, void *d_coef, int batch, double kappa, cudaStream_t st);

@@ -57,6 +57,7 @@ qtam_status build_host_plan(HostPlan &hp, double fs, int64_t N, const double *Q,
   if (o.window == 2 && !(o.window_param > 0.0)) return QTAM_ERR_INVALID_ARG;
   if (o.window >= 3 && !(o.window_param > 0.0 && o.window_param <= 1.0)) return QTAM_ERR_INVALID_ARG;
   if (!(o.epsilon >= 0.0)) return QTAM_ERR_INVALID_ARG;
+  if (o.out_length < -2) return QTAM_ERR_INVALID_ARG;
   const bool manual = o.freqs != nullptr && o.n_freqs >= 2;
   if (manual) { fmin = o.freqs[0]; fmax = o.freqs[o.n_freqs - 1]; }
   if (!(fmin > 0.0) || !(fmax > fmin) || !(fmax < 0.5 * fs)) return QTAM_ERR_INVALID_ARG;

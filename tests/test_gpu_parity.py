@@ -687,3 +687,57 @@ def test_epsilon_windows_and_single_tile_inversion(dtype, eps, tol):
     g0, _ = make_plans(args, dtype, 2)
     with pytest.raises(binding.QtamError):
         g0.dense_invert(torch.zeros((2, args[1]), dtype=torch.complex128 if dtype == "f64" else torch.complex64, device="cuda"), 0)
+
+
+@pytest.mark.parametrize("dtype", ["f32", "f64"])
+@pytest.mark.parametrize("mode", ["minimal", "standard", 300])
+def test_output_length_options(dtype, mode):
+    """The paper's output-resolution options: [rows][n] images at a length n
+    that is no power of two, the inverse from such an image, and the re-sampling to / from the standard length
+    (Fig. 3) -- against the oracle's naive sums."""
+    args = (512.0, 512, [4.0, 8.0], 12.0, 200.0, 9.0)
+    g, r = make_plans(args, dtype, 3)
+    g.close()
+    g = binding.Plan(*args[:5], args[5], dtype=dtype, max_batch=3, out_length=mode)
+    n = g.output_length()
+    assert n == (r.output_length(mode) if isinstance(mode, str) else mode)
+    assert g.output_length("standard") == 257 and g.output_length("minimal") == r.output_length("minimal")
+    x = inputs.white_noise(512, 91, batch=3).astype(np_rdt(dtype))
+    x64 = x.astype(np.float64)
+    img = g.forward_length(dev(x))
+    want = r.forward_length(x64, n, engine=1)
+    assert worst_segment(img.cpu().numpy().reshape(3, -1), want.reshape(3, -1)) <= TOL[dtype]
+    # inverse of the oracle's image, joint and one plane; round trip through the GPU
+    cdt = np.complex64 if dtype == "f32" else np.complex128
+    for plane in (-1, 1):
+        xg = g.inverse_length(dev(want.astype(cdt)), plane=plane).cpu().numpy()
+        assert worst_segment(xg, r.inverse_length(want.astype(cdt).astype(np.complex128), plane=plane, engine=1)) <= TOL[dtype]
+    _, C = r.frame(-1)
+    assert worst_segment(g.inverse_length(img).cpu().numpy(), pi_c(x64, C)) <= TOL_RT[dtype]
+    # up-sampling to the standard length and back
+    up = g.resample(img, to_standard=True)
+    assert up.shape[-1] == 257
+    assert worst_segment(up.cpu().numpy().reshape(3, -1), r.forward_length(x64, 257, engine=1).reshape(3, -1)) <= 4 * TOL[dtype]
+    back = g.resample(up, to_standard=False)
+    assert worst_segment(back.cpu().numpy().reshape(3, -1), want.reshape(3, -1)) <= 4 * TOL[dtype]
+    g0 = binding.Plan(*args[:5], args[5], dtype=dtype, max_batch=3)
+    with pytest.raises(ValueError):
+        g0.forward_length(dev(x))
+
+
+def test_output_length_at_the_papers_shape():
+    """6 s at 4096 Hz (N = 24576): the 62 x 669-like minimal image and its 62 x 12289 standard one (:343)"""
+    name = "paper6s"
+    fs, N, Q, fmin, fmax, rows = inputs.plan_args(name)
+    g = binding.Plan(fs, N, Q, fmin, fmax, rows, dtype="f32", max_batch=2, out_length="minimal")
+    r = RefPlan(fs, N, Q, fmin, fmax, rows)
+    n = g.output_length()
+    assert n == r.output_length("minimal") and g.output_length("standard") == 12289 and g.n_rows == 62
+    x = inputs.make_batch(name, batch=2)
+    img = g.forward_length(dev(x))
+    want = r.forward_length(x.astype(np.float64), n, engine=1)
+    assert worst_segment(img.cpu().numpy().reshape(2, -1), want.reshape(2, -1)) <= 2e-5
+    up = g.resample(img, to_standard=True).cpu().numpy()
+    k = 40
+    w12289 = r.forward_length(x[:1].astype(np.float64), 12289, engine=1)
+    assert rel_l2(up[0, k], w12289[0, k]) <= 1e-4 and rel_l2(up[0], w12289[0]) <= 1e-4

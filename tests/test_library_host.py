@@ -161,3 +161,14 @@ def test_uniform_tile_length_host_plan_matches_oracle(tile_length):
         binding.Plan(*args, host_only=True, tile_length=96)
     with pytest.raises(binding.QtamError):
         binding.Plan(*args, host_only=True, tile_length=64)
+
+
+def test_output_length_modes_on_a_host_plan():
+    """standard = N/2 + 1, minimal = the largest window; a length below it is refused"""
+    kw = dict(dtype="f32", host_only=True)
+    p = binding.Plan(4096.0, 24576, [8.0], 20.0, 1800.0, 62.0, out_length="minimal", **kw)
+    lmax = max(int(r.L) for r in p.rows)
+    assert p.output_length() == lmax == p.output_length("minimal") and p.output_length("standard") == 12289
+    assert binding.Plan(4096.0, 24576, [8.0], 20.0, 1800.0, 62.0, out_length="standard", **kw).output_length() == 12289
+    assert binding.Plan(4096.0, 24576, [8.0], 20.0, 1800.0, 62.0, out_length=lmax + 5, **kw).output_length() == lmax + 5
+    assert binding.Plan(4096.0, 24576, [8.0], 20.0, 1800.0, 62.0, **kw).output_length() == 0
