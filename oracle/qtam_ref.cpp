@@ -759,6 +759,48 @@ int qtam_ref_resample(const qtam_ref_plan *p, const double *in, int batch, int64
   return 0;
 }
 
+// ---- clusters of active pixels ("a clustering algorithm to identify contiguous energetic regions
+// based on a tunable normalized threshold and minimum area ... a binary mask applied to the complex CQT") ----------
+// The image is one Q-plane in the uniform-tile layout, rows x M pixels; a pixel is ACTIVE where `mask` is non-zero
+// (the caller makes it from the row-median threshold, the "normalized threshold").  Clusters are the connected
+// components of the active pixels under 4-connectivity, the time axis circular like the transform, the frequency
+// axis not (R19); components with fewer than min_area pixels are dropped.  Plain flood fill.
+// labels[pixel] = 0 for background / dropped, else 1 + the smallest pixel index (row * M + n) of its cluster: a
+// canonical numbering, so that two implementations can be compared label by label.  count[b] = clusters kept.
+int qtam_ref_cluster_labels(const uint8_t *mask, int batch, int rows, int64_t M, int min_area, int32_t *labels,
+                            int32_t *count) {
+  if (!mask || !labels || batch < 0 || rows < 1 || M < 1 || (int64_t)rows * M >= (int64_t(1) << 31)) return 1;
+  const int64_t npx = (int64_t)rows * M;
+  for (int b = 0; b < batch; ++b) {
+    const uint8_t *A = mask + (size_t)b * (size_t)npx;
+    int32_t *Lb = labels + (size_t)b * (size_t)npx;
+    std::fill(Lb, Lb + npx, 0);
+    std::vector<uint8_t> seen((size_t)npx, 0);
+    std::vector<int64_t> stack, members;
+    int32_t kept = 0;
+    for (int64_t start = 0; start < npx; ++start) {        // ascending: `start` is the cluster's smallest index
+      if (!A[start] || seen[(size_t)start]) continue;
+      stack.assign(1, start); members.clear();
+      seen[(size_t)start] = 1;
+      while (!stack.empty()) {
+        const int64_t i = stack.back(); stack.pop_back();
+        members.push_back(i);
+        const int64_t r = i / M, n = i % M;
+        const int64_t nb[4] = {r * M + (n + 1) % M, r * M + (n + M - 1) % M, r + 1 < rows ? (r + 1) * M + n : -1,
+                               r > 0 ? (r - 1) * M + n : -1};
+        for (int64_t j : nb)
+          if (j >= 0 && A[j] && !seen[(size_t)j]) { seen[(size_t)j] = 1; stack.push_back(j); }
+      }
+      if ((int64_t)members.size() >= (int64_t)min_area) {
+        for (int64_t i : members) Lb[i] = (int32_t)(start + 1);
+        ++kept;
+      }
+    }
+    if (count) count[b] = kept;
+  }
+  return 0;
+}
+
 int qtam_ref_project_cover(const qtam_ref_plan *p, const double *x, int batch, int plane,
                            double *x_out, int engine) {
   if (!p || !x || !x_out || batch < 0 || plane < -1 || plane >= p->nP) return 1;

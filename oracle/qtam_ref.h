@@ -127,6 +127,11 @@ int  qtam_ref_forward_length(const qtam_ref_plan *p, const double *x, int batch,
 int  qtam_ref_inverse_length(const qtam_ref_plan *p, const double *in, int batch, int64_t n, int plane, double *x_out,
                              int engine);
 int  qtam_ref_resample(const qtam_ref_plan *p, const double *in, int batch, int64_t n_in, int64_t n_out, double *out);
+/* Clusters of active pixels of one Q-plane's [rows][M] image (R19): connected components
+ * under 4-connectivity, time axis circular; components smaller than min_area dropped.  mask: [batch][rows][M]
+ * non-zero = active.  labels: [batch][rows][M], 0 or 1 + the smallest pixel index of the cluster.  count: [batch]. */
+int  qtam_ref_cluster_labels(const uint8_t *mask, int batch, int rows, int64_t M, int min_area, int32_t *labels,
+                             int32_t *count);
 /* One-sided spectrum X[f], f=0..N/2 (PAPER.md:365 C1); out is n_bins complex per segment. */
 int  qtam_ref_spectrum(const qtam_ref_plan *p, const double *x, int batch, double *X_out, int engine);
 

@@ -65,6 +65,8 @@ def lib():
         _lib.qtam_ref_dense_invert.argtypes = [vp, dp, C.c_int, C.c_int, dp]
         _lib.qtam_ref_plane_metric.argtypes = [vp, dp, C.c_int, C.c_int, dp, C.POINTER(C.c_int32)]
         _lib.qtam_ref_project_cover.argtypes = [vp, dp, C.c_int, C.c_int, dp, C.c_int]
+        _lib.qtam_ref_cluster_labels.argtypes = [C.POINTER(C.c_uint8), C.c_int, C.c_int, C.c_int64, C.c_int,
+                                                 C.POINTER(C.c_int32), C.POINTER(C.c_int32)]
         _lib.qtam_ref_output_length.argtypes = [vp, C.c_int]
         _lib.qtam_ref_output_length.restype = C.c_int64
         _lib.qtam_ref_forward_length.argtypes = [vp, dp, C.c_int, C.c_int64, dp, C.c_int]
@@ -92,6 +94,20 @@ def threads():
 
 def set_threads(n):
     lib().qtam_ref_set_threads(int(n))
+
+
+def cluster_labels(mask, min_area=1):
+    """connected components (4-connectivity, time circular) of a [batch][rows][M] mask; labels = 1 + smallest pixel
+    index of the cluster, 0 for background and for clusters smaller than min_area"""
+    m = np.ascontiguousarray(mask, dtype=np.uint8)
+    if m.ndim == 2:
+        m = m[None]
+    labels = np.zeros(m.shape, dtype=np.int32)
+    count = np.zeros(m.shape[0], dtype=np.int32)
+    assert lib().qtam_ref_cluster_labels(m.ctypes.data_as(C.POINTER(C.c_uint8)), m.shape[0], m.shape[1], m.shape[2],
+                                         int(min_area), labels.ctypes.data_as(C.POINTER(C.c_int32)),
+                                         count.ctypes.data_as(C.POINTER(C.c_int32))) == 0
+    return labels, count
 
 
 def dft(z, sign):
@@ -257,6 +273,30 @@ class RefPlan:
         ptr = c.view(np.float32).ctypes.data_as(C.POINTER(C.c_float))
         assert lib().qtam_ref_threshold_rowmedian_f32(self._h, ptr, c.shape[0], kappa) == 0
         return c
+
+    def plane_slice(self, plane):
+        rows = [r for r in self.rows if r.plane == plane]
+        return slice(int(rows[0].offset), int(rows[-1].offset + rows[-1].M)), len(rows), int(rows[0].M)
+
+    def cluster(self, coef, plane, min_area=1):
+        """(labels[batch][rows][M] int32, count[batch]) of the clusters of NON-ZERO coefficients of one Q-plane in
+        the uniform-tile layout: apply the row-median threshold first (the normalized threshold)."""
+        c = np.atleast_2d(np.asarray(coef))
+        sl, R, M = self.plane_slice(plane)
+        assert all(r.M == M for r in self.rows if r.plane == plane), "uniform tile layout needed"
+        mask = np.ascontiguousarray((c[:, sl] != 0).astype(np.uint8))
+        return cluster_labels(mask.reshape(c.shape[0], R, M), min_area)
+
+    def apply_mask(self, coef, plane, labels, label=0):
+        """the binary mask of one cluster (label > 0) or of every kept cluster (label 0) applied to the plane's
+        coefficients; everything else, the other planes included, is zero"""
+        c = np.atleast_2d(np.asarray(coef))
+        out = np.zeros_like(c)
+        sl, R, M = self.plane_slice(plane)
+        L = np.asarray(labels).reshape(c.shape[0], R * M)
+        keep = (L == label) if label > 0 else (L > 0)
+        out[:, sl] = np.where(keep, c[:, sl], 0)
+        return out
 
     def output_length(self, mode):
         """'standard' (N/2 + 1) or 'minimal' (the largest window's 2 dk + 1)"""

@@ -12,7 +12,7 @@ import numpy as np
 import pytest
 
 from conftest import rel_l2
-from oracle.qtam_ref import RefPlan, dft, fft
+from oracle.qtam_ref import RefPlan, cluster_labels, dft, fft
 from paper_2603_29785_b200 import inputs
 
 GOLD = os.path.join(os.path.dirname(__file__), "golden")
@@ -817,3 +817,80 @@ def test_output_length_options_closed_forms_and_identities():
     # a length below the largest window aliases: refused
     with pytest.raises(AssertionError):
         p.forward_length(x, n_min - 1)
+
+
+# ---- clusters of active pixels -> binary mask ---------------------------------------------------
+
+def test_cluster_labels_hand_built_masks():
+    """4-connectivity, time axis circular, frequency axis not, minimum area, canonical labels (1 + smallest pixel
+    index): every rule on a mask small enough to check by eye"""
+    m = np.zeros((4, 8), np.uint8)
+    m[1, 6:8] = 1; m[1, 0] = 1; m[2, 0] = 1      # wraps around the time edge: pixels 14, 15, 8, 16 -> label 9
+    m[0, 3] = 1                                   # a single pixel: label 4
+    m[3, 4] = 1; m[2, 5] = 1                      # diagonal neighbours are NOT connected: labels 29 and 22
+    L, c = cluster_labels(m, 1)
+    want = np.zeros((4, 8), np.int32)
+    want[1, 6:8] = 9; want[1, 0] = 9; want[2, 0] = 9; want[0, 3] = 4; want[3, 4] = 29; want[2, 5] = 22
+    assert np.array_equal(L[0], want) and c[0] == 4
+    L, c = cluster_labels(m, 2)                   # minimum area 2 keeps the 4-pixel cluster only
+    assert np.array_equal(L[0], np.where(want == 9, 9, 0)) and c[0] == 1
+    # the frequency axis does not wrap: top and bottom rows stay apart
+    m = np.zeros((3, 4), np.uint8); m[0, 1] = 1; m[2, 1] = 1
+    L, c = cluster_labels(m, 1)
+    assert L[0, 0, 1] == 2 and L[0, 2, 1] == 10 and c[0] == 2
+    # a full row is one ring; an empty mask has no cluster
+    m = np.zeros((2, 5), np.uint8); m[1, :] = 1
+    L, c = cluster_labels(m, 1)
+    assert np.all(L[0, 1] == 6) and np.all(L[0, 0] == 0) and c[0] == 1
+    L, c = cluster_labels(np.zeros((2, 5), np.uint8), 1)
+    assert not L.any() and c[0] == 0
+
+
+@pytest.mark.parametrize("density", [0.2, 0.45, 0.6])
+def test_cluster_labels_vs_scipy(density):
+    """random masks against an outside library's labelling (scipy.ndimage.label, 4-connectivity); the first and
+    last time columns are cleared so that no cluster touches the circular edge, which scipy does not have"""
+    ndi = pytest.importorskip("scipy.ndimage")
+    rng = np.random.default_rng(int(density * 100))
+    m = (rng.random((3, 24, 40)) < density).astype(np.uint8)
+    m[:, :, 0] = 0; m[:, :, -1] = 0
+    for min_area in (1, 4):
+        L, c = cluster_labels(m, min_area)
+        for b in range(3):
+            lab, n = ndi.label(m[b])
+            want = np.zeros_like(L[b]); kept = 0
+            for i in range(1, n + 1):
+                idx = np.flatnonzero(lab.ravel() == i)
+                if idx.size >= min_area:
+                    want.ravel()[idx] = idx.min() + 1; kept += 1
+            assert np.array_equal(L[b], want) and c[b] == kept
+    # with the edge columns active the circular axis joins clusters scipy keeps apart: check against a rolled copy
+    m2 = (rng.random((1, 16, 32)) < 0.4).astype(np.uint8)
+    L0, c0 = cluster_labels(m2, 1)
+    L1, c1 = cluster_labels(np.roll(m2, 5, axis=2), 1)
+    assert c0[0] == c1[0]                                    # the partition does not depend on where the edge is
+    P0 = (L0[0][:, :, None, None] == L0[0][None, None, :, :]) & (L0[0] > 0)[:, :, None, None]
+    R1 = np.roll(L1[0], -5, axis=1)
+    P1 = (R1[:, :, None, None] == R1[None, None, :, :]) & (R1 > 0)[:, :, None, None]
+    assert np.array_equal(P0, P1)
+
+
+def test_cluster_mask_pipeline_isolates_a_burst():
+    """threshold -> clusters -> binary mask -> inverse (Fig. 8): a strong sine-Gaussian in weak noise is
+    the largest cluster of its plane, and inverting its mask alone gives back most of the burst"""
+    N = 2048
+    p = RefPlan(2048.0, N, [8.0], 32.0, 800.0, 24, tile_length=-1)
+    t = np.arange(N) / 2048.0
+    burst = inputs.sine_gaussian(t, 300.0, 12.0, 8.0, 0.5)
+    x = 0.05 * inputs.white_noise(N, 88)[0] + burst
+    Y = p.forward(x)
+    Yt = p.threshold(Y, 3.0)
+    L, c = p.cluster(Yt, 0, min_area=6)
+    assert c[0] >= 1
+    ids, areas = np.unique(L[L > 0], return_counts=True)
+    big = int(ids[np.argmax(areas)])
+    xr = p.inverse(p.apply_mask(Yt, 0, L, label=big), plane=0)[0]
+    assert rel_l2(xr, burst) < 0.2
+    # every kept cluster together = the thresholded plane restricted to cluster pixels
+    allm = p.apply_mask(Yt, 0, L, label=0)
+    assert np.count_nonzero(allm) == np.count_nonzero(L)
