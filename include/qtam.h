@@ -164,6 +164,24 @@ qtam_status qtam_forward_length(qtam_plan *p, const void *d_x, int batch, void *
 qtam_status qtam_inverse_length(qtam_plan *p, const void *d_img, int batch, int plane, void *d_x_out, void *stream);
 qtam_status qtam_resample(qtam_plan *p, const void *d_in, int batch, int to_standard, void *d_out, void *stream);
 
+/* Clusters of active pixels and their binary masks ("a clustering algorithm to identify contiguous
+ * energetic regions based on a tunable normalized threshold and minimum area. For each identified cluster, we
+ * generated a binary mask applied to the complex CQT, which was subsequently inverted"; R19).  For plans
+ * in the uniform-tile layout (tile_length != 0), where Q-plane `plane` is an image of R rows x M samples; call
+ * qtam_threshold_rowmedian (the normalized threshold) first: a pixel is ACTIVE where its coefficient is non-zero.
+ * qtam_cluster: connected components of the active pixels under 4-connectivity, time axis circular, frequency
+ *   axis not; components of fewer than min_area pixels are dropped.  d_labels [batch][R*M] int32 (device, caller-
+ *   owned): 0 = background / dropped, else 1 + the smallest pixel index (row*M + n) of the pixel's cluster;
+ *   d_count [batch] int32: clusters kept.  qtam_plane_pixels(p, plane) = R*M (0 if the plane is no image).
+ * qtam_mask: d_out [batch][coeffs_per_segment] = d_coef on the plane's pixels whose label equals `label` (label > 0)
+ *   or is non-zero (label = 0), zero everywhere else, the other planes included; d_out may equal d_coef.
+ *   qtam_inverse(d_out, plane) then gives the cluster's time series. */
+int64_t     qtam_plane_pixels(const qtam_plan *p, int plane);
+qtam_status qtam_cluster(qtam_plan *p, const void *d_coef, int batch, int plane, int min_area, int32_t *d_labels,
+                         int32_t *d_count, void *stream);
+qtam_status qtam_mask(qtam_plan *p, const void *d_coef, int batch, int plane, const int32_t *d_labels, int label,
+                      void *d_out, void *stream);
+
 /* Row-median threshold in place (BASELINE.json config 5; R11): per (segment,row),
  * m = median_n |Y_k[n]| (two middle values averaged), zero every Y_k[n] with |Y_k[n]| < kappa*m.
  * The decision is taken in the plan's dtype with the operation order of DESIGN.md.               */

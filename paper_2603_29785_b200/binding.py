@@ -20,7 +20,7 @@ SYMBOLS = ["qtam_plan_create", "qtam_plan_create_host", "qtam_plan_destroy", "qt
            "qtam_plan_rows", "qtam_plan_window", "qtam_plan_frame", "qtam_forward", "qtam_inverse",
            "qtam_dense", "qtam_dense_invert", "qtam_threshold_rowmedian", "qtam_forward_threshold", "qtam_plane_metric", "qtam_gather_plane", "qtam_max_plane_coeffs", "qtam_remodulate", "qtam_instantaneous_frequency", "qtam_last_launch_count", "qtam_status_string",
            "qtam_profile_enable", "qtam_profile_read", "qtam_output_length", "qtam_forward_length", "qtam_inverse_length",
-           "qtam_resample"]
+           "qtam_resample", "qtam_plane_pixels", "qtam_cluster", "qtam_mask"]
 
 
 class QtamError(RuntimeError):
@@ -101,6 +101,10 @@ def lib():
         L.qtam_forward_length.argtypes = [vp, vp, C.c_int, vp, vp]
         L.qtam_inverse_length.argtypes = [vp, vp, C.c_int, C.c_int, vp, vp]
         L.qtam_resample.argtypes = [vp, vp, C.c_int, C.c_int, vp, vp]
+        L.qtam_plane_pixels.argtypes = [vp, C.c_int]
+        L.qtam_plane_pixels.restype = C.c_int64
+        L.qtam_cluster.argtypes = [vp, vp, C.c_int, C.c_int, C.c_int, vp, vp, vp]
+        L.qtam_mask.argtypes = [vp, vp, C.c_int, C.c_int, vp, C.c_int, vp, vp]
         _lib = L
     return _lib
 
@@ -306,6 +310,35 @@ class Plan:
         out = t.empty((batch, self.n_rows, n_out), dtype=self._cdt(), device=img.device)
         _check(lib().qtam_resample(self._h, img.data_ptr(), batch, 1 if to_standard else 0, out.data_ptr(), self._stream()),
                "qtam_resample")
+        return out
+
+    def cluster(self, coef, plane, min_area=1):
+        """(labels[batch][R*M] int32, count[batch] int32): connected clusters of the non-zero coefficients of one
+        Q-plane (uniform-tile layout; threshold first), PAPER.md:208"""
+        t = self._torch()
+        npx = int(lib().qtam_plane_pixels(self._h, int(plane)))
+        if npx <= 0:
+            raise ValueError("qtam_cluster needs a plan in the uniform-tile layout (tile_length != 0)")
+        self._need(coef, self._cdt(), "coef")
+        batch = self._batch(coef, self.ctot, "coef")
+        labels = t.empty((batch, npx), dtype=t.int32, device=coef.device)
+        count = t.empty((batch,), dtype=t.int32, device=coef.device)
+        _check(lib().qtam_cluster(self._h, coef.data_ptr(), batch, int(plane), int(min_area), labels.data_ptr(),
+                                  count.data_ptr(), self._stream()), "qtam_cluster")
+        return labels, count
+
+    def mask(self, coef, plane, labels, label=0, out=None):
+        """the binary mask of one cluster (label > 0) or of all kept clusters (0) applied to the coefficients"""
+        t = self._torch()
+        npx = int(lib().qtam_plane_pixels(self._h, int(plane)))
+        self._need(coef, self._cdt(), "coef")
+        batch = self._batch(coef, self.ctot, "coef")
+        self._need(labels, t.int32, "labels", numel=batch * npx)
+        if out is None:
+            out = t.empty_like(coef)
+        self._need(out, self._cdt(), "out", numel=batch * self.ctot)
+        _check(lib().qtam_mask(self._h, coef.data_ptr(), batch, int(plane), labels.data_ptr(), int(label), out.data_ptr(),
+                               self._stream()), "qtam_mask")
         return out
 
     def threshold_rowmedian(self, coef, kappa=3.0):

@@ -55,7 +55,7 @@ void free_plan(qtam_plan *p) {
   for (int c = 0; c < kClClasses; ++c) { cudaFree(p->d_cl_lead[c]); cudaFree(p->d_cl_mem[c]); cudaFree(p->d_cl_groups[c]); cudaFree(p->d_cl_ftw[c]); }
   cudaFree(p->d_cl_ptw);
   cudaFree(p->d_runs); cudaFree(p->d_run_ptr); cudaFree(p->d_run_idx);
-  cudaFree(p->d_len_tw[0]); cudaFree(p->d_len_tw[1]);
+  cudaFree(p->d_len_tw[0]); cudaFree(p->d_len_tw[1]); cudaFree(p->d_ccl_area);
   cudaFree(p->d_trows); cudaFree(p->d_titems); cudaFree(p->d_part); cudaFree(p->d_counter);
   for (ProfRec &r : p->prof_pool) { cudaEventDestroy(r.e0); cudaEventDestroy(r.e1); }
   delete p;
@@ -407,6 +407,7 @@ qtam_status qtam_plan_create(qtam_plan **out, double fs, int64_t N, const double
   if (s == QTAM_OK && p->fast_rows) s = build_runs(p);
   if (s == QTAM_OK) s = prepare_fast(p);
   if (s == QTAM_OK) s = build_length(p);
+  if (s == QTAM_OK) s = build_cluster(p);
   if (s != QTAM_OK) { free_plan(p); cudaGetLastError(); return s; }
   if (cudaDeviceSynchronize() != cudaSuccess) { free_plan(p); return QTAM_ERR_CUDA; }
   *out = p;
@@ -594,6 +595,32 @@ qtam_status qtam_dense_invert(qtam_plan *p, const void *d_tile, int batch, int r
   return generic_dense_invert(p, d_tile, batch, row, d_x_out, static_cast<cudaStream_t>(stream));
 }
 
+int64_t qtam_plane_pixels(const qtam_plan *p, int plane) {
+  long long off; int R, M;
+  if (!p || plane < 0 || plane >= p->hp.nP || !plane_image(p, plane, &off, &R, &M)) return 0;
+  return (int64_t)R * M;
+}
+
+qtam_status qtam_cluster(qtam_plan *p, const void *d_coef, int batch, int plane, int min_area, int32_t *d_labels,
+                         int32_t *d_count, void *stream) {
+  if (p && p->host_only) return QTAM_ERR_CUDA;
+  if (!check_call(p, d_coef, d_labels, batch) || !d_count || plane < 0 || plane >= p->hp.nP || min_area < 1)
+    return QTAM_ERR_INVALID_ARG;
+  p->last_launches = 0;
+  if (batch == 0) return QTAM_OK;
+  return cluster_labels(p, d_coef, batch, plane, min_area, d_labels, d_count, static_cast<cudaStream_t>(stream));
+}
+
+qtam_status qtam_mask(qtam_plan *p, const void *d_coef, int batch, int plane, const int32_t *d_labels, int label,
+                      void *d_out, void *stream) {
+  if (p && p->host_only) return QTAM_ERR_CUDA;
+  if (!check_call(p, d_coef, d_out, batch) || !d_labels || plane < 0 || plane >= p->hp.nP || label < 0)
+    return QTAM_ERR_INVALID_ARG;
+  p->last_launches = 0;
+  if (batch == 0) return QTAM_OK;
+  return cluster_mask(p, d_coef, batch, plane, d_labels, label, d_out, static_cast<cudaStream_t>(stream));
+}
+
 int64_t qtam_output_length(const qtam_plan *p, int mode) {
   if (!p) return 0;
   if (mode == 0) return p->host_only ? length_resolve(p->hp, p->hp.opt.out_length) : p->len_n;
@@ -691,7 +718,7 @@ static const char *const kKernelNames[K_COUNT] = {
     "inv_rows", "inv_reduce", "dense_place", "threshold", "r2c_fast", "fwd_rows_fast", "inv_rows_fast",
     "reduce_c2r_fast", "inv_fused", "inv_tiles", "combine_c2r", "threshold_fast", "rows_cta_fwd", "rows_cta_inv",
     "tiny_rows_fwd", "tiny_rows_inv", "long_fft_a", "long_fft_b", "plane_metric", "best_plane", "remodulate", "inst_freq", "fwd_rows_thr", "gather_plane",
-    "rows_cl_fwd", "rows_cl_inv", "combine_runs", "c2c_fast", "split3", "combine3", "len_band", "len_synth", "len_analysis"};
+    "rows_cl_fwd", "rows_cl_inv", "combine_runs", "c2c_fast", "split3", "combine3", "len_band", "len_synth", "len_analysis", "cluster", "mask"};
 
 qtam_status qtam_profile_enable(qtam_plan *p, int on, int max_launches) {
   if (!p || p->host_only) return QTAM_ERR_INVALID_ARG;

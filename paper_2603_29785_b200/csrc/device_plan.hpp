@@ -15,7 +15,7 @@ enum KernelId {
   K_REDUCE_C2R_FAST, K_INV_FUSED, K_INV_TILES, K_COMBINE_C2R, K_THRESHOLD_FAST, K_ROWS_CTA_FWD, K_ROWS_CTA_INV,
   K_TINY_FWD, K_TINY_INV, K_LONG_A, K_LONG_B, K_PLANE_METRIC, K_BEST_PLANE, K_REMODULATE, K_INST_FREQ, K_FWD_ROWS_THR, K_GATHER_PLANE,
   K_ROWS_CL_FWD, K_ROWS_CL_INV, K_COMBINE_RUNS, K_C2C_FAST, K_SPLIT3, K_COMBINE3, K_LEN_BAND, K_LEN_SYNTH, K_LEN_ANALYSIS,
-  K_COUNT
+  K_CLUSTER, K_MASK, K_COUNT
 };
 // fast float path (fast.cu): rows with 32 <= M <= 1024, grouped by G = M/32 lanes per row
 struct FastRow { int kc, dk, woff, goff, offset, plane, wpad, pad; };   // wpad: offset into the padded window table
@@ -194,6 +194,9 @@ struct qtam_plan {
   long long len_n = 0, len_std = 0;
   void *d_len_tw[2] = {nullptr, nullptr};
 
+  int *d_ccl_area = nullptr;    // cluster.cu: pixel counts per component root, [max_batch][ccl_pixels]
+  long long ccl_pixels = 0;
+
   int last_launches = 0;
   // launch profile (qtam_profile_enable / qtam_profile_read)
   bool prof_on = false;
@@ -285,6 +288,13 @@ qtam_status build_length(qtam_plan *p);
 qtam_status length_forward(qtam_plan *p, int batch, void *d_out, cudaStream_t st);
 qtam_status length_inverse_bands(qtam_plan *p, const void *d_in, int batch, int plane, cudaStream_t st);
 qtam_status length_resample(qtam_plan *p, const void *d_in, int batch, int to_standard, void *d_out, cudaStream_t st);
+// cluster.cu
+bool plane_image(const qtam_plan *p, int plane, long long *off, int *R, int *M);
+qtam_status build_cluster(qtam_plan *p);
+qtam_status cluster_labels(qtam_plan *p, const void *d_coef, int batch, int plane, int min_area, int32_t *d_labels,
+                           int32_t *d_count, cudaStream_t st);
+qtam_status cluster_mask(qtam_plan *p, const void *d_coef, int batch, int plane, const int32_t *d_labels, int label,
+                         void *d_out, cudaStream_t st);
 // threshold_fast.cu
 qtam_status build_thr_fast(qtam_plan *p);
 qtam_status fast_threshold(qtam_plan *p, void *d_coef, int batch, double kappa, cudaStream_t st);

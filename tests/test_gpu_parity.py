@@ -741,3 +741,53 @@ def test_output_length_at_the_papers_shape():
     k = 40
     w12289 = r.forward_length(x[:1].astype(np.float64), 12289, engine=1)
     assert rel_l2(up[0, k], w12289[0, k]) <= 1e-4 and rel_l2(up[0], w12289[0]) <= 1e-4
+
+
+@pytest.mark.parametrize("dtype", ["f32", "f64"])
+def test_clusters_and_masks(dtype):
+    """threshold -> clusters -> binary mask -> inverse: labels and counts equal the oracle's flood fill
+    exactly (canonical numbering), on the thresholded transform of bursts in noise and on random patterns; the mask
+    of a cluster and its inverse against the oracle"""
+    N = 4096
+    args = (4096.0, N, [6.0, 12.0], 32.0, 1600.0, 24.0)
+    nseg = 3
+    g, r = make_plans(args, dtype, nseg, tile_length=-1)
+    t = np.arange(N) / 4096.0
+    x = 0.3 * inputs.white_noise(N, 97, batch=nseg)
+    x[0] += inputs.sine_gaussian(t, 300.0, 10.0, 6.0, 0.4) + inputs.sine_gaussian(t, 900.0, 20.0, 5.0, 0.7)
+    x[1] += inputs.sine_gaussian(t, 150.0, 6.0, 8.0, 0.999)          # wraps around the circular time axis
+    x = x.astype(np_rdt(dtype))
+    Y = g.forward_threshold(dev(x), 2.5)
+    Yh = Y.cpu().numpy()
+    cdt = torch.complex64 if dtype == "f32" else torch.complex128
+    for plane in (0, 1):
+        for min_area in (1, 5):
+            L, c = g.cluster(Y, plane, min_area)
+            Lr, cr = r.cluster(Yh, plane, min_area)
+            assert np.array_equal(L.cpu().numpy().reshape(Lr.shape), Lr) and np.array_equal(c.cpu().numpy(), cr)
+            assert cr.max() >= 1
+    plane = 1
+    L, c = g.cluster(Y, plane, 5)
+    Lr, _ = r.cluster(Yh, plane, 5)
+    ids, areas = np.unique(Lr[0][Lr[0] > 0], return_counts=True)
+    big = int(ids[np.argmax(areas)])
+    for label in (big, 0):
+        Mg = g.mask(Y, plane, L, label)
+        Mr = r.apply_mask(Yh, plane, Lr, label)
+        assert np.array_equal(Mg.cpu().numpy(), Mr)
+        xg = g.inverse(Mg, plane=plane).cpu().numpy()
+        assert worst_segment(xg, r.inverse(Mr.astype(np.complex128), plane=plane, engine=1)) <= TOL[dtype] * 10
+    # random patterns at several densities (most clusters merge into a few snakes around 0.5-0.6)
+    rng = np.random.default_rng(5)
+    for density in (0.15, 0.45, 0.6, 0.95):
+        Z = torch.zeros((nseg, g.ctot), dtype=cdt, device="cuda")
+        sl, R, M = r.plane_slice(0)
+        pat = (rng.random((nseg, R * M)) < density)
+        Z[:, sl] = torch.from_numpy(pat.astype(np.complex64 if dtype == "f32" else np.complex128)).cuda()
+        L, c = g.cluster(Z, 0, 3)
+        Lr, cr = r.cluster(Z.cpu().numpy(), 0, 3)
+        assert np.array_equal(L.cpu().numpy().reshape(Lr.shape), Lr) and np.array_equal(c.cpu().numpy(), cr)
+    # a plan in the ragged layout has no image to label
+    g0, _ = make_plans(args, dtype, nseg)
+    with pytest.raises(ValueError):
+        g0.cluster(g0.forward(dev(x)), 0)
