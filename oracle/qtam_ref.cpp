@@ -275,6 +275,7 @@ int qtam_ref_plan_create(qtam_ref_plan **out, double fs, int64_t N, const double
   qtam_ref_options o;
   o.window = 0; o.clamp_mode = 1; o.clamp_overlap = 1.0; o.max_window_bins = 0;
   o.cover_floor = 1e-2; o.rows_are_bins_per_octave = 0; o.window_param = 0.0; o.freqs = nullptr; o.n_freqs = 0; o.tile_length = 0; o.epsilon = 0.0;
+  o.plane_window = nullptr; o.plane_window_param = nullptr;
   if (opt) o = *opt;
   const bool manual = o.freqs != nullptr && o.n_freqs >= 2;
   if (manual) { fmin = o.freqs[0]; fmax = o.freqs[o.n_freqs - 1]; }
@@ -283,6 +284,13 @@ int qtam_ref_plan_create(qtam_ref_plan **out, double fs, int64_t N, const double
   if (o.window == 2 && !(o.window_param > 0)) return 1;
   if (o.window >= 3 && !(o.window_param > 0 && o.window_param <= 1.0)) return 1;
   if (!(o.epsilon >= 0.0)) return 1;
+  for (int pl = 0; o.plane_window && pl < nQ; ++pl) {          // a composite bank: one window family per plane (:327)
+    const int wt = o.plane_window[pl];
+    const double wp = o.plane_window_param ? o.plane_window_param[pl] : 0.0;
+    if (wt < 0 || wt > 4) return 2;
+    if (wt == 2 && !(wp > 0)) return 1;
+    if (wt >= 3 && !(wp > 0 && wp <= 1.0)) return 1;
+  }
   if (!(o.clamp_overlap > 0)) o.clamp_overlap = 1.0;
   if (!(o.cover_floor > 0)) o.cover_floor = 1e-2;
 
@@ -355,12 +363,14 @@ int qtam_ref_plan_create(qtam_ref_plan **out, double fs, int64_t N, const double
       row.M = Muni > 0 ? Muni : next_pow2(L);                               // R5 / uniform layout
       row.f_center = (double)row.kc / T;
       row.offset = offset; offset += row.M; sumL += L;
-      // bisquare window (Eq. 6) and unit-energy normalisation (Eq. 5 / R3);
-      // the sum runs over the unclipped support (R8)
+      // the plane's window (Eq. 6; App. A; a composite bank gives every plane its own family,
+      // :327) and unit-energy normalisation (Eq. 5 / R3); the sum runs over the unclipped support (R8)
+      const int wtype = o.plane_window ? o.plane_window[pl] : o.window;
+      const double wpar = o.plane_window_param ? o.plane_window_param[pl] : o.window_param;
       row.wraw.resize((size_t)L); row.w.resize((size_t)L);
       ld e = 0;
       for (int64_t j = -row.dk; j <= row.dk; ++j) {
-        double v = raw_window(o.window, o.window_param, j, row.dk);
+        double v = raw_window(wtype, wpar, j, row.dk);
         row.wraw[(size_t)(j + row.dk)] = v;
         e += (ld)v * (ld)v;
       }

@@ -49,6 +49,11 @@ typedef struct {
                                        layout :127-129); n > 0 = uniform user-set n, a power of two >= max L */
   double  epsilon;                  /* Eq. 12 (:143): unnormalised window value outside the support, used by
                                        the dense tiles and their single-tile inversion only; 0 = none       */
+  const int *plane_window;          /* composite filter bank (:327 "scanning not only across varying Quality
+                                       factors Q ... but also across diverse windowing functions and their
+                                       associated shape parameters"): nQ window families, one per plane (the Q
+                                       list may repeat a value); NULL = `window` for every plane           */
+  const double *plane_window_param; /* nQ shape parameters (NULL = 0 for every plane)                      */
 } qtam_ref_options;
 
 typedef struct {

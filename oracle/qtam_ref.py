@@ -21,7 +21,8 @@ class Options(C.Structure):
     _fields_ = [("window", C.c_int), ("clamp_mode", C.c_int), ("clamp_overlap", C.c_double),
                 ("max_window_bins", C.c_int64), ("cover_floor", C.c_double),
                 ("rows_are_bins_per_octave", C.c_int), ("window_param", C.c_double),
-                ("freqs", C.POINTER(C.c_double)), ("n_freqs", C.c_int), ("tile_length", C.c_int64), ("epsilon", C.c_double)]
+                ("freqs", C.POINTER(C.c_double)), ("n_freqs", C.c_int), ("tile_length", C.c_int64), ("epsilon", C.c_double),
+                ("plane_window", C.POINTER(C.c_int)), ("plane_window_param", C.POINTER(C.c_double))]
 
 
 WINDOWS = {"bisquare": 0, "hann": 1, "kaiser": 2, "tukey": 3, "planck": 4}
@@ -129,15 +130,22 @@ class RefPlan:
 
     def __init__(self, fs, N, Q, fmin, fmax, spacing, clamp_mode=1, clamp_overlap=1.0,
                  max_window_bins=0, cover_floor=1e-2, rows_are_bins_per_octave=0,
-                 window="bisquare", window_param=0.0, freqs=None, tile_length=0, epsilon=0.0):
+                 window="bisquare", window_param=0.0, freqs=None, tile_length=0, epsilon=0.0, plane_windows=None):
         L = lib()
         self._h = C.c_void_p()
         q = np.ascontiguousarray(Q, dtype=np.float64)
         fr = None if freqs is None else np.ascontiguousarray(freqs, dtype=np.float64)
+        pw = pp = None
+        if plane_windows is not None:       # [(family, parameter)] per plane: a composite filter bank
+            pw = np.ascontiguousarray([WINDOWS[w] for w, _ in plane_windows], dtype=np.int32)
+            pp = np.ascontiguousarray([float(a) for _, a in plane_windows], dtype=np.float64)
+            assert pw.size == len(Q)
         opt = Options(WINDOWS[window], clamp_mode, clamp_overlap, max_window_bins, cover_floor,
                       rows_are_bins_per_octave, float(window_param),
                       None if fr is None else fr.ctypes.data_as(C.POINTER(C.c_double)),
-                      0 if fr is None else fr.size, int(tile_length), float(epsilon))
+                      0 if fr is None else fr.size, int(tile_length), float(epsilon),
+                      None if pw is None else pw.ctypes.data_as(C.POINTER(C.c_int)),
+                      None if pp is None else pp.ctypes.data_as(C.POINTER(C.c_double)))
         rc = L.qtam_ref_plan_create(C.byref(self._h), float(fs), int(N), _dp(q), q.size,
                                     float(fmin), float(fmax), float(spacing), C.byref(opt))
         if rc != 0:

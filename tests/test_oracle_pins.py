@@ -894,3 +894,37 @@ def test_cluster_mask_pipeline_isolates_a_burst():
     # every kept cluster together = the thresholded plane restricted to cluster pixels
     allm = p.apply_mask(Yt, 0, L, label=0)
     assert np.count_nonzero(allm) == np.count_nonzero(L)
+
+
+# ---- composite filter bank: one window family per plane ---------------------------------------------
+
+def test_composite_bank_is_the_concatenation_of_its_single_window_banks():
+    """A23: "scanning not only across varying Quality factors Q ... but also across diverse windowing functions and
+    their associated shape parameters ... a composite filter bank concatenates all requested configurations".
+    Plane p of the composite bank IS the single-window bank of its (Q, family, parameter): windows, coefficients,
+    per-plane frame operator and per-plane inverse; the joint frame operator is the sum; P4 and P6 hold jointly."""
+    cfgs = [(8.0, "bisquare", 0.0), (8.0, "hann", 0.0), (8.0, "tukey", 0.5), (16.0, "kaiser", 6.0), (16.0, "planck", 0.4)]
+    base = (1024.0, 1024)
+    p = RefPlan(*base, [c[0] for c in cfgs], 16.0, 400.0, 12, plane_windows=[(c[1], c[2]) for c in cfgs])
+    x = inputs.white_noise(1024, 77, batch=2)
+    Y = p.forward(x)
+    Pj, Cj = p.frame(-1)
+    Psum = np.zeros_like(Pj)
+    off = 0
+    for q, (Q, w, a) in enumerate(cfgs):
+        s1 = RefPlan(*base, [Q], 16.0, 400.0, 12, window=w, window_param=a)
+        for k in range(s1.n_rows):
+            assert np.array_equal(p.window(q * s1.n_rows + k), s1.window(k))
+        assert rel_l2(Y[:, off:off + s1.ctot], s1.forward(x)) <= 1e-14
+        Pq, Cq = p.frame(q)
+        P1, C1 = s1.frame(-1)
+        assert np.array_equal(Cq, C1) and np.allclose(Pq, P1, rtol=1e-14)
+        assert rel_l2(p.inverse(Y, plane=q), s1.inverse(Y[:, off:off + s1.ctot])) <= 1e-13
+        Psum += Pq
+        off += s1.ctot
+    assert np.allclose(Pj, Psum, rtol=1e-13)
+    X = np.fft.rfft(x, axis=-1)
+    tot = np.sum(np.abs(Y) ** 2, axis=1)
+    assert np.all(np.abs(tot - np.sum(np.abs(X) ** 2 * Pj[None, :], axis=1) / 1024) <= 1e-13 * tot)
+    proj = np.fft.irfft(np.where(Cj[None, :], X, 0), n=1024, axis=-1)
+    assert rel_l2(p.inverse(Y), proj) <= 1e-12
