@@ -78,6 +78,12 @@ typedef struct {
   double  epsilon;                  /* Eq. 12 (R17): unnormalised window value
                                        off the support (and floor on it) for qtam_dense and
                                        qtam_dense_invert only; 0 = plain windows [default]           */
+  const int *plane_window;          /* composite filter bank (:327 "scanning not only across varying Quality
+                                       factors Q ... but also across diverse windowing functions and their
+                                       associated shape parameters"): nQ window families, one per plane (the Q
+                                       list may repeat a value; host pointer, read during plan creation only);
+                                       NULL = `window` for every plane [default]                         */
+  const double *plane_window_param; /* nQ shape parameters (NULL = 0 for every plane)                    */
   int64_t out_length;               /* the paper's output-resolution option (:150, :158-160, :184, :343) for
                                        qtam_forward_length / _inverse_length / _resample: 0 = not used
                                        [default]; -1 = "standard" N/2 + 1; -2 = "minimal", the largest

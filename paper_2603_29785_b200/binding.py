@@ -35,6 +35,7 @@ class Options(C.Structure):
                 ("cover_floor", C.c_double), ("rows_are_bins_per_octave", C.c_int),
                 ("max_batch", C.c_int), ("window_param", C.c_double),
                 ("freqs", C.POINTER(C.c_double)), ("n_freqs", C.c_int), ("tile_length", C.c_int64), ("epsilon", C.c_double),
+                ("plane_window", C.POINTER(C.c_int)), ("plane_window_param", C.POINTER(C.c_double)),
                 ("out_length", C.c_int64)]
 
 
@@ -120,16 +121,24 @@ class Plan:
     def __init__(self, fs, N, Q, fmin, fmax, spacing, dtype="f32", max_batch=1, clamp_mode=1,
                  clamp_overlap=1.0, max_window_bins=0, cover_floor=1e-2, rows_are_bins_per_octave=0,
                  host_only=False, window="bisquare", window_param=0.0, freqs=None, tile_length=0, epsilon=0.0,
-                 out_length=0):
+                 out_length=0, plane_windows=None):
         L = lib()
         self._h = C.c_void_p()
         self.dtype = dtype
         q = np.ascontiguousarray(Q, dtype=np.float64)
         fr = None if freqs is None else np.ascontiguousarray(freqs, dtype=np.float64)
+        pw = pp = None
+        if plane_windows is not None:       # [(family, parameter)] per plane: a composite filter bank
+            if len(plane_windows) != q.size:
+                raise ValueError("plane_windows: one (family, parameter) per entry of Q")
+            pw = np.ascontiguousarray([WINDOWS[w] for w, _ in plane_windows], dtype=np.int32)
+            pp = np.ascontiguousarray([float(a) for _, a in plane_windows], dtype=np.float64)
         opt = Options(C.sizeof(Options), WINDOWS[window], clamp_mode, clamp_overlap, max_window_bins,
                       cover_floor, rows_are_bins_per_octave, max_batch, float(window_param),
                       None if fr is None else fr.ctypes.data_as(C.POINTER(C.c_double)),
                       0 if fr is None else fr.size, int(tile_length), float(epsilon),
+                      None if pw is None else pw.ctypes.data_as(C.POINTER(C.c_int)),
+                      None if pp is None else pp.ctypes.data_as(C.POINTER(C.c_double)),
                       {"standard": -1, "minimal": -2}.get(out_length, out_length))
         fn = L.qtam_plan_create_host if host_only else L.qtam_plan_create
         code = fn(C.byref(self._h), float(fs), int(N), q.ctypes.data_as(C.POINTER(C.c_double)), q.size,

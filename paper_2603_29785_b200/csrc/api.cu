@@ -93,12 +93,13 @@ qtam_status build_fast(qtam_plan *p) {
   std::memset(&F, 0, sizeof(F));
   // one window per distinct half-width (the clamped rows all share one)
   std::vector<float> fwin;
-  std::vector<std::pair<int64_t, int>> seen;   // (dk, offset)
+  std::vector<std::pair<int64_t, int>> seen;   // (dk and window identity, offset)
+  auto wkey = [](const HostRow &h) -> int64_t { return h.dk * 64 + h.wid; };
   auto window_of = [&](const HostRow &h) -> int {
-    for (auto &e : seen) if (e.first == h.dk) return e.second;
+    for (auto &e : seen) if (e.first == wkey(h)) return e.second;
     const int off = (int)fwin.size();
     for (int64_t i = 0; i < h.L; ++i) fwin.push_back((float)hp.win[(size_t)(h.woff + i)]);
-    seen.push_back({h.dk, off});
+    seen.push_back({wkey(h), off});
     return off;
   };
   // the same windows zero-padded to the M points of the row's short FFT and stored at the M-array
@@ -106,12 +107,12 @@ qtam_status build_fast(qtam_plan *p) {
   std::vector<float> fwinp;
   std::vector<std::pair<int64_t, int>> seen2;
   auto wpad_of = [&](const HostRow &h) -> int {
-    for (auto &e : seen2) if (e.first == h.dk) return e.second;
+    for (auto &e : seen2) if (e.first == wkey(h)) return e.second;
     const int off = (int)fwinp.size();
     fwinp.resize(fwinp.size() + (size_t)h.M, 0.0f);
     for (int64_t jj = -h.dk; jj <= h.dk; ++jj)
       fwinp[(size_t)(off + (jj + h.M) % h.M)] = (float)hp.win[(size_t)(h.woff + jj + h.dk)];
-    seen2.push_back({h.dk, off});
+    seen2.push_back({wkey(h), off});
     return off;
   };
   std::vector<FastRow> frows;
@@ -141,7 +142,8 @@ qtam_status build_fast(qtam_plan *p) {
       frows.push_back(r);
       {
         size_t l = 0;
-        while (l < leaders.size() && !(leaders[l].kc == r.kc && leaders[l].dk == r.dk)) ++l;
+        // identical rows: same centre bin, half-width and window (the same entry of the window table)
+        while (l < leaders.size() && !(leaders[l].kc == r.kc && leaders[l].dk == r.dk && leaders[l].woff == r.woff)) ++l;
         if (l == leaders.size()) { leaders.push_back(r); members.emplace_back(); }
         members[l].push_back(r.offset);
       }
@@ -289,7 +291,7 @@ template <typename T> qtam_status build_device(qtam_plan *p) {
           int leader = -1;
           for (int l : gen_leaders)
             if (hp.rows[(size_t)l].kc == hp.rows[k].kc && hp.rows[(size_t)l].dk == hp.rows[k].dk &&
-                hp.rows[(size_t)l].M == hp.rows[k].M) { leader = l; break; }
+                hp.rows[(size_t)l].M == hp.rows[k].M && hp.rows[(size_t)l].wid == hp.rows[k].wid) { leader = l; break; }
           if (leader < 0) { gen_leaders.push_back((int)k); items_fwd[c].push_back(WorkItem{(int)k, 0, 1, lm}); }
           else { followers[(size_t)leader].push_back(hp.rows[k].offset); followers_w[(size_t)leader].push_back(hp.rows[k].woff); }
         }

@@ -61,14 +61,14 @@ qtam_status build_inv_tiled(qtam_plan *p) {
       const int G = 1 << B.log2G, Fr = 32 / G;
       std::vector<FastRow> all(p->h_frows.begin() + B.row_base, p->h_frows.begin() + B.row_base + B.nrows);
       std::stable_sort(all.begin(), all.end(), [](const FastRow &a, const FastRow &b) {
-        return a.kc != b.kc ? a.kc < b.kc : a.dk < b.dk;
+        return a.kc != b.kc ? a.kc < b.kc : (a.dk != b.dk ? a.dk < b.dk : a.woff < b.woff);
       });
       // rows with the same centre bin and half-width (the clamped rows of different Q-planes) share their
       // window and their place in the spectrum: by linearity their coefficient rows are added before ONE
       // transform.  `rows` = one leader per such set; pad0 / pad1 = first member / number of members.
       std::vector<FastRow> rows;
       for (size_t i = 0; i < all.size(); ++i) {
-        if (rows.empty() || rows.back().kc != all[i].kc || rows.back().dk != all[i].dk) {
+        if (rows.empty() || rows.back().kc != all[i].kc || rows.back().dk != all[i].dk || rows.back().woff != all[i].woff) {
           rows.push_back(all[i]);
           rows.back().pad = (int)tmem.size();
           rows.back().goff = 0;            // member count

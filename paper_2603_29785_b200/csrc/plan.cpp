@@ -58,13 +58,28 @@ qtam_status build_host_plan(HostPlan &hp, double fs, int64_t N, const double *Q,
   if (o.window >= 3 && !(o.window_param > 0.0 && o.window_param <= 1.0)) return QTAM_ERR_INVALID_ARG;
   if (!(o.epsilon >= 0.0)) return QTAM_ERR_INVALID_ARG;
   if (o.out_length < -2) return QTAM_ERR_INVALID_ARG;
+  // a composite bank: one window family (and shape parameter) per plane (:327)
+  std::vector<int> wtype(size_t(nQ), o.window);
+  std::vector<double> wpar(size_t(nQ), o.window_param);
+  std::vector<int> wident(size_t(nQ), 0);
+  for (int pl = 0; o.plane_window && pl < nQ; ++pl) {
+    wtype[size_t(pl)] = o.plane_window[pl];
+    wpar[size_t(pl)] = o.plane_window_param ? o.plane_window_param[pl] : 0.0;
+    if (wtype[size_t(pl)] < 0 || wtype[size_t(pl)] > 4) return QTAM_ERR_UNSUPPORTED;
+    if (wtype[size_t(pl)] == 2 && !(wpar[size_t(pl)] > 0.0)) return QTAM_ERR_INVALID_ARG;
+    if (wtype[size_t(pl)] >= 3 && !(wpar[size_t(pl)] > 0.0 && wpar[size_t(pl)] <= 1.0)) return QTAM_ERR_INVALID_ARG;
+    wident[size_t(pl)] = pl;
+    for (int q = 0; q < pl; ++q)
+      if (wtype[size_t(q)] == wtype[size_t(pl)] && wpar[size_t(q)] == wpar[size_t(pl)]) { wident[size_t(pl)] = wident[size_t(q)]; break; }
+  }
   const bool manual = o.freqs != nullptr && o.n_freqs >= 2;
   if (manual) { fmin = o.freqs[0]; fmax = o.freqs[o.n_freqs - 1]; }
   if (!(fmin > 0.0) || !(fmax > fmin) || !(fmax < 0.5 * fs)) return QTAM_ERR_INVALID_ARG;
   if (o.clamp_mode < 0 || o.clamp_mode > 2) return QTAM_ERR_INVALID_ARG;
 
   hp.fs = fs; hp.N = N; hp.nb = N / 2 + 1; hp.nP = nQ; hp.dtype = dtype; hp.opt = o;
-  hp.opt.freqs = nullptr;                     // the caller's list is only read here
+  hp.opt.freqs = nullptr;                     // the caller's lists are only read here
+  hp.opt.plane_window = nullptr; hp.opt.plane_window_param = nullptr;
   const double dur = double(N) / fs;          // N_t of the paper (:75)
   const double tile_c = std::sqrt(11.0);      // R1
 
@@ -138,12 +153,13 @@ qtam_status build_host_plan(HostPlan &hp, double fs, int64_t N, const double *Q,
       h.f_center = double(h.kc) / dur;
       h.offset = coff; coff += m;
       h.woff = woff; h.goff = woff; woff += len;
+      h.wid = wident[size_t(pl)];
       // the window (App. A), unit l2 energy over the unclipped support (Eq. 5 :63, R3, R8)
       const size_t base = hp.win.size();
       hp.win.resize(base + size_t(len));
       long double energy = 0.0L;
       for (int64_t j = -h.dk; j <= h.dk; ++j) {
-        const double raw = window_value(o.window, o.window_param, j, h.dk);
+        const double raw = window_value(wtype[size_t(pl)], wpar[size_t(pl)], j, h.dk);
         hp.win[base + size_t(j + h.dk)] = raw;
         energy += (long double)raw * (long double)raw;
       }

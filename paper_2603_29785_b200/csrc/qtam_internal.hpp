@@ -17,6 +17,7 @@ struct HostRow {
   int64_t woff;                   // offset of W_k[-dk] in the window table
   int64_t goff;                   // offset of the row's band in the band workspace (== woff)
   double norm;
+  int wid;                        // window identity: rows with the same (kc, dk, wid) are identical rows
 };
 
 struct HostPlan {

@@ -163,7 +163,7 @@ void build_leaders_and_groups(qtam_plan *p, const std::vector<int> &rows_in, int
     for (size_t l = sets.size(); l-- > 0 && !joined;) {
       const HostRow &hb = hp.rows[(size_t)sets[l][0]];
       if (hb.kc != h.kc) break;
-      if (hb.dk != h.dk || (int)sets[l].size() >= kCtaMaxMembers) continue;
+      if (hb.dk != h.dk || hb.wid != h.wid || (int)sets[l].size() >= kCtaMaxMembers) continue;
       bool plane_free = true;
       for (int m : sets[l]) if (hp.rows[(size_t)m].plane == h.plane) plane_free = false;
       if (!plane_free) continue;

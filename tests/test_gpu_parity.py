@@ -791,3 +791,29 @@ def test_clusters_and_masks(dtype):
     g0, _ = make_plans(args, dtype, nseg)
     with pytest.raises(ValueError):
         g0.cluster(g0.forward(dev(x)), 0)
+
+
+@pytest.mark.parametrize("dtype", ["f32", "f64"])
+def test_composite_bank_with_a_window_family_per_plane(dtype):
+    """A23: the planes of one bank differ in window family and shape parameter as well as in Q.  Planes
+    0-2 share Q = 8 (same centre bins and half-widths, different windows: such rows must NOT be merged), planes 3-4
+    share Q and window (identical rows under the clamp: merged).  Long rows included (N = 2^16)."""
+    cfgs = [(8.0, "bisquare", 0.0), (8.0, "hann", 0.0), (8.0, "tukey", 0.5), (16.0, "kaiser", 6.0), (16.0, "kaiser", 6.0)]
+    for N, fs in ((8192, 4096.0), (65536, 16384.0)):
+        args = (fs, N, [c[0] for c in cfgs], 20.0, 0.44 * fs, 20.0)
+        kw = dict(plane_windows=[(c[1], c[2]) for c in cfgs])
+        g, r = make_plans(args, dtype, 2, **kw)
+        for k in range(0, g.n_rows, 7):
+            assert np.abs(g.window(k) - r.window(k)).max() <= 1e-14 * r.window(k).max()
+        x = inputs.white_noise(N, 120, batch=2).astype(np_rdt(dtype))
+        x64 = x.astype(np.float64)
+        Yg = g.forward(dev(x)).cpu().numpy()
+        Yr = r.forward(x64, engine=1)
+        assert worst_segment(Yg, Yr) <= TOL[dtype] and worst_row(Yg, Yr, r) <= TOL_ROW[dtype]
+        rng = np.random.default_rng(121)
+        Yin = (rng.standard_normal((2, g.ctot)) + 1j * rng.standard_normal((2, g.ctot))).astype(Yg.dtype)
+        for plane in (-1, 1, 4, -1):
+            xg = g.inverse(dev(Yin), plane=plane).cpu().numpy()
+            assert worst_segment(xg, r.inverse(Yin.astype(np.complex128), plane=plane, engine=1)) <= TOL[dtype], plane
+        _, C = r.frame(-1)
+        assert worst_segment(g.inverse(g.forward(dev(x))).cpu().numpy(), pi_c(x64, C)) <= TOL_RT[dtype]

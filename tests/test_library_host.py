@@ -172,3 +172,21 @@ def test_output_length_modes_on_a_host_plan():
     assert binding.Plan(4096.0, 24576, [8.0], 20.0, 1800.0, 62.0, out_length="standard", **kw).output_length() == 12289
     assert binding.Plan(4096.0, 24576, [8.0], 20.0, 1800.0, 62.0, out_length=lmax + 5, **kw).output_length() == lmax + 5
     assert binding.Plan(4096.0, 24576, [8.0], 20.0, 1800.0, 62.0, **kw).output_length() == 0
+
+
+def test_composite_bank_host_plan_equals_oracle_plan():
+    cfgs = [(8.0, "bisquare", 0.0), (8.0, "hann", 0.0), (16.0, "tukey", 0.5), (16.0, "kaiser", 6.0), (32.0, "planck", 0.4)]
+    kw = dict(plane_windows=[(c[1], c[2]) for c in cfgs])
+    p = binding.Plan(4096.0, 8192, [c[0] for c in cfgs], 20.0, 1800.0, 24.0, dtype="f64", host_only=True, **kw)
+    r = RefPlan(4096.0, 8192, [c[0] for c in cfgs], 20.0, 1800.0, 24.0, **kw)
+    assert p.ctot == r.ctot and p.n_rows == r.n_rows
+    for k in range(p.n_rows):
+        wa, wb = p.window(k), r.window(k)
+        assert np.max(np.abs(wa - wb)) <= 1e-14 * np.max(wb)      # two independent evaluations of cos / I_0 / exp
+        assert abs(p.rows[k].norm - r.rows[k].norm) <= 1e-14 * r.rows[k].norm
+    for plane in range(-1, p.n_planes):
+        Pa, Ca = p.frame(plane)
+        Pb, Cb = r.frame(plane)
+        assert np.array_equal(Ca, Cb) and np.max(np.abs(Pa - Pb)) <= 1e-13 * np.max(Pb)
+    with pytest.raises(ValueError):
+        binding.Plan(4096.0, 8192, [8.0, 16.0], 20.0, 1800.0, 24.0, host_only=True, plane_windows=[("hann", 0.0)])
