@@ -24,7 +24,10 @@
  *     the call.  The plan owns its device tables and a workspace sized for `max_batch` segments;
  *     qtam_plan_destroy frees them.
  *   - Calls are asynchronous on `stream`, never synchronise the host, never allocate, do not modify
- *     their inputs, and in/out buffers must not alias.  One in-flight call per plan.
+ *     their inputs, and in/out buffers must not alias.  One in-flight call per plan.  A call may run
+ *     independent kernels on streams the plan owns; they start after the work already on `stream` and
+ *     `stream` waits for them before anything issued after the call (event fork / join: capturable in
+ *     a CUDA graph).
  *   - Errors: status codes only; nothing is thrown across the ABI; outputs are untouched on failure.
  *     There is no CPU fallback: without a CUDA device every compute call returns QTAM_ERR_CUDA.
  */
@@ -235,8 +238,11 @@ int         qtam_last_launch_count(const qtam_plan *p);
 const char *qtam_status_string(qtam_status s);
 
 /* Launch profile for bench.py's roofline line.  While enabled, every kernel launch of the compute
- * calls is bracketed by CUDA events on the launch stream (pre-created: up to `max_launches` launches
- * between two reads; further ones are not recorded).  qtam_profile_read waits for the recorded events,
+ * calls is bracketed by CUDA events on the launch stream, and the library issues all of its launches on the
+ * caller's stream (otherwise independent row kernels of one call run concurrently on the plan's own streams,
+ * forked from and joined back to the caller's stream with events, and a kernel's elapsed time would include its
+ * neighbours').  The events are pre-created: up to `max_launches` launches between two reads; further ones are
+ * not recorded.  qtam_profile_read waits for the recorded events,
  * sums per kernel the launches, the device time (ms), the COMPULSORY bytes of those launches (algo_bytes:
  * input samples read, coefficients written or read, output samples written -- SURVEY.md 8(d)) and the bytes
  * the launches move by design (design_bytes: compulsory + spectrum, partial sums, band workspace, scratch;

@@ -58,6 +58,8 @@ void free_plan(qtam_plan *p) {
   cudaFree(p->d_len_tw[0]); cudaFree(p->d_len_tw[1]); cudaFree(p->d_ccl_area);
   cudaFree(p->d_trows); cudaFree(p->d_titems); cudaFree(p->d_part); cudaFree(p->d_counter);
   for (ProfRec &r : p->prof_pool) { cudaEventDestroy(r.e0); cudaEventDestroy(r.e1); }
+  for (int i = 0; i < p->n_side; ++i) { cudaStreamDestroy(p->side[i]); cudaEventDestroy(p->ev_join[i]); }
+  if (p->ev_fork) cudaEventDestroy(p->ev_fork);
   delete p;
 }
 
@@ -410,6 +412,15 @@ qtam_status qtam_plan_create(qtam_plan **out, double fs, int64_t N, const double
   if (s == QTAM_OK) s = prepare_fast(p);
   if (s == QTAM_OK) s = build_length(p);
   if (s == QTAM_OK) s = build_cluster(p);
+  if (s == QTAM_OK && (p->cta_rows || p->cl_rows)) {
+    // side streams for the concurrent row launches (plans whose rows run in several kernels)
+    if (cudaEventCreateWithFlags(&p->ev_fork, cudaEventDisableTiming) != cudaSuccess) s = QTAM_ERR_CUDA;
+    for (int i = 0; s == QTAM_OK && i < qtam_plan::kSide; ++i) {
+      if (cudaStreamCreateWithFlags(&p->side[i], cudaStreamNonBlocking) != cudaSuccess ||
+          cudaEventCreateWithFlags(&p->ev_join[i], cudaEventDisableTiming) != cudaSuccess) s = QTAM_ERR_CUDA;
+      else p->n_side = i + 1;
+    }
+  }
   if (s != QTAM_OK) { free_plan(p); cudaGetLastError(); return s; }
   if (cudaDeviceSynchronize() != cudaSuccess) { free_plan(p); return QTAM_ERR_CUDA; }
   *out = p;
@@ -482,19 +493,15 @@ qtam_status qtam_forward(qtam_plan *p, const void *d_x, int batch, void *d_coef,
   cudaStream_t st = static_cast<cudaStream_t>(stream);
   qtam_status s = p->fast_long ? fast_r2c(p, d_x, batch, st) : generic_r2c(p, d_x, batch, st);
   if (s != QTAM_OK) return s;
-  if (p->fast_rows) {
-    s = fast_forward_rows(p, batch, d_coef, st);
-    if (s != QTAM_OK) return s;
-  }
-  if (p->cta_rows) {
-    s = cta_forward_rows(p, batch, d_coef, st);
-    if (s != QTAM_OK) return s;
-  }
-  if (p->cl_rows) {
-    s = cluster_forward_rows(p, batch, d_coef, st);
-    if (s != QTAM_OK) return s;
-  }
-  return generic_forward_rows(p, batch, d_coef, st);
+  // the row launches are independent of each other (they read the spectrum and write disjoint coefficients):
+  // the longest rows first, every launch on a stream of its own, joined before the call returns to the caller's
+  Fork fk(p, st);
+  if (p->cl_rows) s = cluster_forward_rows(p, batch, d_coef, fk);
+  if (s == QTAM_OK && p->cta_rows) s = cta_forward_rows(p, batch, d_coef, fk);
+  if (s == QTAM_OK && p->fast_rows) s = fast_forward_rows(p, batch, d_coef, st);
+  if (s == QTAM_OK) s = generic_forward_rows(p, batch, d_coef, st);
+  fk.join();
+  return s;
 }
 
 qtam_status qtam_forward_threshold(qtam_plan *p, const void *d_x, int batch, double kappa, void *d_coef,
@@ -512,22 +519,23 @@ qtam_status qtam_forward_threshold(qtam_plan *p, const void *d_x, int batch, dou
     s = fast_forward_rows_threshold(p, batch, d_coef, (float)kappa, st, &fused);
     if (s != QTAM_OK) return s;
     if (fused) {
-      if (p->cta_rows) {
-        s = cta_forward_rows(p, batch, d_coef, st);
-        if (s != QTAM_OK) return s;
-      }
-      if (p->cl_rows) {
-        s = cluster_forward_rows(p, batch, d_coef, st);
-        if (s != QTAM_OK) return s;
-      }
+      Fork fk(p, st);
+      if (p->cl_rows) s = cluster_forward_rows(p, batch, d_coef, fk);
+      if (s == QTAM_OK && p->cta_rows) s = cta_forward_rows(p, batch, d_coef, fk);
+      fk.join();
+      if (s != QTAM_OK) return s;
       s = generic_forward_rows(p, batch, d_coef, st);
       if (s != QTAM_OK || !p->thr_has_big) return s;
       return generic_threshold(p, d_coef, batch, kappa, kThrFastLog2Max + 1, st);   // rows longer than 1024 points
     }
     // not fusable for this plan / batch: the two steps one after the other
     s = fast_forward_rows(p, batch, d_coef, st);
-    if (s == QTAM_OK && p->cta_rows) s = cta_forward_rows(p, batch, d_coef, st);
-    if (s == QTAM_OK && p->cl_rows) s = cluster_forward_rows(p, batch, d_coef, st);
+    {
+      Fork fk(p, st);
+      if (s == QTAM_OK && p->cl_rows) s = cluster_forward_rows(p, batch, d_coef, fk);
+      if (s == QTAM_OK && p->cta_rows) s = cta_forward_rows(p, batch, d_coef, fk);
+      fk.join();
+    }
     if (s == QTAM_OK) s = generic_forward_rows(p, batch, d_coef, st);
     if (s != QTAM_OK) return s;
     const int n1 = p->last_launches;
@@ -556,11 +564,14 @@ qtam_status qtam_inverse(qtam_plan *p, const void *d_coef, int batch, int plane,
   if (p->use_runs) {
     // float plans: every row kernel leaves its contributions as runs (tiles' and groups' partial sums, the band
     // slots of the shortest rows); one pass adds them, applies 1/P and prepares the long C2R
-    s = p->tiles_ok ? tiles_only(p, d_coef, batch, plane, st) : fast_inverse_rows(p, d_coef, batch, plane, st);
-    if (s == QTAM_OK) s = fast_tiny_inverse(p, d_coef, batch, plane, st);
-    if (s == QTAM_OK && p->cta_rows) s = cta_inverse_rows(p, d_coef, batch, plane, st);
-    if (s == QTAM_OK && p->cl_rows) s = cluster_inverse_rows(p, d_coef, batch, plane, st);
+    // (independent launches, disjoint partial sums: forked onto the plan's side streams, the longest rows first)
+    Fork fk(p, st);
+    if (p->cl_rows) s = cluster_inverse_rows(p, d_coef, batch, plane, fk);
+    if (s == QTAM_OK && p->cta_rows) s = cta_inverse_rows(p, d_coef, batch, plane, fk);
+    if (s == QTAM_OK) s = p->tiles_ok ? tiles_only(p, d_coef, batch, plane, st) : fast_inverse_rows(p, d_coef, batch, plane, st);
+    if (s == QTAM_OK) s = fast_tiny_inverse(p, d_coef, batch, plane, fk.next());
     if (s == QTAM_OK) s = generic_inverse_rows(p, d_coef, batch, plane, st);   // (no items on these plans)
+    fk.join();
     if (s == QTAM_OK) s = combine_runs(p, batch, plane, st);
     if (s != QTAM_OK) return s;
     if (p->fast_long) return fast_c2c_out(p, batch, d_x_out, st);

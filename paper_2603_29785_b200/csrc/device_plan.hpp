@@ -197,6 +197,14 @@ struct qtam_plan {
   int *d_ccl_area = nullptr;    // cluster.cu: pixel counts per component root, [max_batch][ccl_pixels]
   long long ccl_pixels = 0;
 
+  // side streams: the row launches of one call are independent of each other (disjoint outputs), so they are
+  // forked onto these and joined back (events; nothing waits on the host): short classes fill the SMs the long
+  // ones leave idle
+  static const int kSide = 8;
+  cudaStream_t side[kSide] = {};
+  cudaEvent_t ev_fork = nullptr, ev_join[kSide] = {};
+  int n_side = 0;
+
   int last_launches = 0;
   // launch profile (qtam_profile_enable / qtam_profile_read)
   bool prof_on = false;
@@ -226,6 +234,30 @@ struct LaunchScope {
     cudaEventRecord(p->prof_pool[(size_t)slot].e0, st);
   }
   ~LaunchScope() { if (slot >= 0) cudaEventRecord(p->prof_pool[(size_t)slot].e1, st); }
+};
+
+// Fork-join over the plan's side streams.  next() hands out a stream that starts after everything issued on the
+// caller's stream before the fork; join() makes the caller's stream wait for all of them.  Capturable in a CUDA
+// graph (every forked stream joins back), never touches the host.  While the launch profile is on everything stays
+// on the caller's stream, so that the profile's events bracket one kernel at a time (qtam_profile_enable).
+struct Fork {
+  qtam_plan *p; cudaStream_t main; int used, avail;
+  Fork(qtam_plan *plan, cudaStream_t st) : p(plan), main(st), used(0), avail(plan->prof_on ? 0 : plan->n_side) {
+    if (avail > 0) cudaEventRecord(p->ev_fork, main);
+  }
+  cudaStream_t next() {
+    if (used >= avail) return main;
+    cudaStream_t s = p->side[used++];
+    cudaStreamWaitEvent(s, p->ev_fork, 0);
+    return s;
+  }
+  void join() {
+    for (int i = 0; i < used; ++i) {
+      cudaEventRecord(p->ev_join[i], p->side[i]);
+      cudaStreamWaitEvent(main, p->ev_join[i], 0);
+    }
+    used = 0;
+  }
 };
 
 // which part of the CSR a reduction over the band workspace walks: sets plo .. phi-1 of nsets per bin
@@ -273,12 +305,12 @@ qtam_status instantaneous_frequency(qtam_plan *p, const void *d_coef, int batch,
 void build_leaders_and_groups(qtam_plan *p, const std::vector<int> &rows_in, int groups_wanted,
                               std::vector<ClLeader> &lead, std::vector<int2> &mem, std::vector<ClGroup> &groups);
 qtam_status build_rows_cta(qtam_plan *p);
-qtam_status cta_forward_rows(qtam_plan *p, int batch, void *d_coef, cudaStream_t st);
-qtam_status cta_inverse_rows(qtam_plan *p, const void *d_coef, int batch, int plane, cudaStream_t st);
+qtam_status cta_forward_rows(qtam_plan *p, int batch, void *d_coef, Fork &fk);
+qtam_status cta_inverse_rows(qtam_plan *p, const void *d_coef, int batch, int plane, Fork &fk);
 // rows_cluster.cu
 qtam_status build_rows_cluster(qtam_plan *p);
-qtam_status cluster_forward_rows(qtam_plan *p, int batch, void *d_coef, cudaStream_t st);
-qtam_status cluster_inverse_rows(qtam_plan *p, const void *d_coef, int batch, int plane, cudaStream_t st);
+qtam_status cluster_forward_rows(qtam_plan *p, int batch, void *d_coef, Fork &fk);
+qtam_status cluster_inverse_rows(qtam_plan *p, const void *d_coef, int batch, int plane, Fork &fk);
 // combine_runs.cu
 qtam_status build_runs(qtam_plan *p);
 qtam_status combine_runs(qtam_plan *p, int batch, int plane, cudaStream_t st);

@@ -389,20 +389,22 @@ static qtam_status cl_launch(qtam_plan *p, int c, int batch, void *d_coef, int p
   return QTAM_OK;
 }
 
+// every class on a stream of its own, the longest rows first (the classes write disjoint coefficients / partial sums)
 template <bool FWD>
-static qtam_status cl_all(qtam_plan *p, int batch, void *d_coef, int plane, cudaStream_t st) {
-  qtam_status s = cl_launch<kClLog2P, 3, FWD>(p, 3, batch, d_coef, plane, st);
-  if (s == QTAM_OK) s = cl_launch<kClLog2P, 2, FWD>(p, 2, batch, d_coef, plane, st);
-  if (s == QTAM_OK) s = cl_launch<kClLog2P, 1, FWD>(p, 1, batch, d_coef, plane, st);
-  if (s == QTAM_OK) s = cl_launch<kClLog2P, 0, FWD>(p, 0, batch, d_coef, plane, st);
+static qtam_status cl_all(qtam_plan *p, int batch, void *d_coef, int plane, Fork &fk) {
+  qtam_status s = QTAM_OK;
+  if (p->n_cl_lead[3]) s = cl_launch<kClLog2P, 3, FWD>(p, 3, batch, d_coef, plane, fk.next());
+  if (s == QTAM_OK && p->n_cl_lead[2]) s = cl_launch<kClLog2P, 2, FWD>(p, 2, batch, d_coef, plane, fk.next());
+  if (s == QTAM_OK && p->n_cl_lead[1]) s = cl_launch<kClLog2P, 1, FWD>(p, 1, batch, d_coef, plane, fk.next());
+  if (s == QTAM_OK && p->n_cl_lead[0]) s = cl_launch<kClLog2P, 0, FWD>(p, 0, batch, d_coef, plane, fk.next());
   return s;
 }
 
-qtam_status cluster_forward_rows(qtam_plan *p, int batch, void *d_coef, cudaStream_t st) {
-  return cl_all<true>(p, batch, d_coef, -1, st);
+qtam_status cluster_forward_rows(qtam_plan *p, int batch, void *d_coef, Fork &fk) {
+  return cl_all<true>(p, batch, d_coef, -1, fk);
 }
-qtam_status cluster_inverse_rows(qtam_plan *p, const void *d_coef, int batch, int plane, cudaStream_t st) {
-  return cl_all<false>(p, batch, const_cast<void *>(d_coef), plane, st);
+qtam_status cluster_inverse_rows(qtam_plan *p, const void *d_coef, int batch, int plane, Fork &fk) {
+  return cl_all<false>(p, batch, const_cast<void *>(d_coef), plane, fk);
 }
 
 }  // namespace qtam

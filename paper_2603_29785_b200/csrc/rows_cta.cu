@@ -263,19 +263,21 @@ static qtam_status rows_cta_launch(qtam_plan *p, int c, int batch, void *d_coef,
   return QTAM_OK;
 }
 
+// every class on a stream of its own (the classes write disjoint coefficients / partial sums)
 template <bool FORWARD>
-static qtam_status rows_cta_all(qtam_plan *p, int batch, void *d_coef, int plane, cudaStream_t st) {
-  qtam_status s = rows_cta_launch<13, FORWARD>(p, 2, batch, d_coef, plane, st);
-  if (s == QTAM_OK) s = rows_cta_launch<12, FORWARD>(p, 1, batch, d_coef, plane, st);
-  if (s == QTAM_OK) s = rows_cta_launch<11, FORWARD>(p, 0, batch, d_coef, plane, st);
+static qtam_status rows_cta_all(qtam_plan *p, int batch, void *d_coef, int plane, Fork &fk) {
+  qtam_status s = QTAM_OK;
+  if (p->n_cta_rows[2]) s = rows_cta_launch<13, FORWARD>(p, 2, batch, d_coef, plane, fk.next());
+  if (s == QTAM_OK && p->n_cta_rows[1]) s = rows_cta_launch<12, FORWARD>(p, 1, batch, d_coef, plane, fk.next());
+  if (s == QTAM_OK && p->n_cta_rows[0]) s = rows_cta_launch<11, FORWARD>(p, 0, batch, d_coef, plane, fk.next());
   return s;
 }
 
-qtam_status cta_forward_rows(qtam_plan *p, int batch, void *d_coef, cudaStream_t st) {
-  return rows_cta_all<true>(p, batch, d_coef, -1, st);
+qtam_status cta_forward_rows(qtam_plan *p, int batch, void *d_coef, Fork &fk) {
+  return rows_cta_all<true>(p, batch, d_coef, -1, fk);
 }
-qtam_status cta_inverse_rows(qtam_plan *p, const void *d_coef, int batch, int plane, cudaStream_t st) {
-  return rows_cta_all<false>(p, batch, const_cast<void *>(d_coef), plane, st);
+qtam_status cta_inverse_rows(qtam_plan *p, const void *d_coef, int batch, int plane, Fork &fk) {
+  return rows_cta_all<false>(p, batch, const_cast<void *>(d_coef), plane, fk);
 }
 
 }  // namespace qtam
