@@ -73,7 +73,7 @@ struct ClSyncMid { __device__ __forceinline__ void operator()() const { __syncth
 // in(ja, a) (a = natural index of the sub-transform's input).  The results go to shared memory (natural or
 // skewed); mid() runs between the last read and the first write (a barrier when the pass works in place).
 template <int LOG2P, int R, int LOG2NS, int DIR, int IN_MODE, bool OUT_SKEW, class In, class Mid>
-__device__ __forceinline__ void cl_pass(float2 *s, const In &in, const Mid &mid, const float2 *__restrict__ ptw) {
+__device__ __forceinline__ void cl_pass(float2 *s, const In &in, const Mid &mid, const float2 *ptw) {
   typedef ClFft<LOG2P> PL;
   constexpr int NBF = PL::P / R;            // butterflies per sub-transform
   constexpr int TPS = PL::NT / 4;           // threads per sub-transform
@@ -99,12 +99,12 @@ __device__ __forceinline__ void cl_pass(float2 *s, const In &in, const Mid &mid,
       float2 wb[4], wa[RA];
 #pragma unroll
       for (int b = 1; b < 4; ++b) {
-        wb[b] = __ldg(ptw + (b - 1) * NS + k);
+        wb[b] = ptw[(b - 1) * NS + k];
         if (DIR < 0) wb[b].y = -wb[b].y;
       }
 #pragma unroll
       for (int a = 1; a < RA; ++a) {
-        wa[a] = __ldg(ptw + (2 + a) * NS + k);
+        wa[a] = ptw[(2 + a) * NS + k];
         if (DIR < 0) wa[a].y = -wa[a].y;
       }
 #pragma unroll
@@ -133,7 +133,7 @@ __device__ __forceinline__ void cl_pass(float2 *s, const In &in, const Mid &mid,
 // passes 2 and 3 of the batched sub-transforms (pass 1 is written out by the caller: its input or the barrier
 // before its writes differs between the forward and the inverse); natural layout on exit, ends with a barrier
 template <int LOG2P, int DIR>
-__device__ __forceinline__ void cl_passes_23(float2 *s, const float2 *__restrict__ ptw) {
+__device__ __forceinline__ void cl_passes_23(float2 *s, const float2 *ptw) {
   typedef ClFft<LOG2P> PL;
   cl_pass<LOG2P, PL::R1, 4, DIR, 1, false>(s, ClNoMid{}, ClSyncMid{}, ptw);
   __syncthreads();

@@ -82,27 +82,32 @@ struct ClArgs {
 };
 
 // Pass 1 of the forward's sub-transforms, straight from the spectrum: B[j] = X[kc + jj] W_k[jj] s at
-// j = q + F jc (R6), zero off the support and off the one-sided spectrum (R8).  All 2 R loads of a butterfly
-// are issued before the first multiply.
+// j = q + F jc (R6), zero off the support and off the one-sided spectrum (R8).  A butterfly's inputs sit at
+// compile-time distances from its first one (jc = i + r P/R, and jc >= P/2 -- the negative offsets -- exactly for
+// r >= R/2), so a load is one compare against a per-butterfly bound and one address with an immediate offset;
+// all 2 R loads of a butterfly are issued before the first multiply.
 template <int LOG2P, int F, class Mid>
 __device__ __forceinline__ void cl_pass1_gather(float2 *s, const float2 *__restrict__ X, const float *__restrict__ W,
                                                 int kc, int dk, int nbins, int q0, float scale, const Mid &mid) {
   typedef ClFft<LOG2P> PL;
   constexpr int P = PL::P, R = PL::R0, NBF = P / R, TPS = PL::NT / 4, BPT = NBF / TPS;
   const int ja = threadIdx.x & 3, ib = threadIdx.x >> 2;
+  const int hi = min(dk, nbins - 1 - kc), lo = max(-dk, -kc);      // offsets jj kept: lo <= jj <= hi
   float2 v[BPT][R];
 #pragma unroll
   for (int u = 0; u < BPT; ++u) {
-    const int i = ib + TPS * u;
+    const int jj0 = q0 + ja + F * (ib + TPS * u);                  // offset of the butterfly's first input (r = 0)
+    const float2 *Xp = X + kc + jj0;
+    const float *Wp = W + jj0;
+    const int a = hi - jj0, b = lo - jj0;
     float w[R];
 #pragma unroll
     for (int r = 0; r < R; ++r) {
-      const int jc = i + r * NBF;
-      const int jj = q0 + ja + F * jc - (jc >= P / 2 ? F * P : 0);
-      const int f = kc + jj;
-      const bool ok = jj >= -dk && jj <= dk && (unsigned)f < (unsigned)nbins;
-      v[u][r] = ld_nc_f2(X + f, ok);
-      w[r] = ld_nc_f1(W + jj, ok);
+      constexpr int dummy = 0; (void)dummy;
+      const int c = r * F * NBF - (r >= R / 2 ? F * P : 0);        // compile-time distance from the first input
+      const bool ok = r < R / 2 ? c <= a : c >= b;
+      v[u][r] = ld_nc_f2(Xp + c, ok);
+      w[r] = ld_nc_f1(Wp + c, ok);
     }
 #pragma unroll
     for (int r = 0; r < R; ++r) v[u][r] = pscale(v[u][r], w[r] * scale);
@@ -134,6 +139,11 @@ k_rows_cluster(const ClArgs A) {
   const int cid = blockIdx.x >> LOG2CL, ncl = gridDim.x >> LOG2CL;
   const int tid = threadIdx.x;
   float2 *s = reinterpret_cast<float2 *>(qtam_cl_smem);
+  // the pass tables of the sub-transforms live in shared memory: the cluster barrier's acquire invalidates L1, so
+  // table reads from global memory would go to L2 in every pass of every row
+  float2 *stw = s + PL::SMEM_ELEMS;
+  for (int i = tid; i < PL::PTW_ELEMS; i += NT) stw[i] = A.ptw[i];
+  __syncthreads();
   float2 *rs[CL];
 #pragma unroll
   for (int jb = 0; jb < CL; ++jb) rs[jb] = cluster.map_shared_rank(s, jb);
@@ -153,7 +163,7 @@ k_rows_cluster(const ClArgs A) {
       cl_pass1_gather<LOG2P, F>(s, A.spec + (size_t)seg * A.xstride, A.win + L.woff + L.dk, L.kc, L.dk, A.nbins,
                                 4 * crank, L.fwd_scale, before_write);
       __syncthreads();
-      cl_passes_23<LOG2P, +1>(s, A.ptw);
+      cl_passes_23<LOG2P, +1>(s, stw);
       cl_arrive();
       // radix-F stage for nc = crank NCQ .. + NCQ
       float2 *Yseg = A.coef + (size_t)seg * A.ctot;
@@ -240,9 +250,9 @@ k_rows_cluster(const ClArgs A) {
         }
         cl_arrive(); cl_wait();
         // the four sub-transforms of this CTA's residues
-        cl_pass<LOG2P, PL::R0, 0, -1, 0, true>(s, ClNoMid{}, ClSyncMid{}, A.ptw);
+        cl_pass<LOG2P, PL::R0, 0, -1, 0, true>(s, ClNoMid{}, ClSyncMid{}, stw);
         __syncthreads();
-        cl_passes_23<LOG2P, -1>(s, A.ptw);
+        cl_passes_23<LOG2P, -1>(s, stw);
         // G_k[jj] = sqrt(N/M) Bhat[jj] W_k[jj], added into the group's partial sum at bin kc + jj (R8 clip).
         // The loads of a batch are issued before its stores (a store may not be overtaken by a later load of
         // the same array, which would serialise the round trips to L2).
@@ -286,7 +296,7 @@ k_rows_cluster(const ClArgs A) {
 // class c = log2 M - kClLog2Min = log2 CL: the sub-transforms have P = 2^kClLog2P points in every class
 template <int LOG2P, int LOG2CL> static bool prepare_cl(qtam_plan *p, int c) {
   typedef ClFft<LOG2P> PL;
-  const size_t smem = sizeof(float2) * (size_t)PL::SMEM_ELEMS;
+  const size_t smem = sizeof(float2) * (size_t)(PL::SMEM_ELEMS + PL::PTW_ELEMS);
   for (int fwd = 0; fwd < 2; ++fwd) {
     KernelCfg &cfg = p->cfg_rows_cl[c][fwd];
     cfg.smem = smem; cfg.occ = 0; cfg.ready = false;
