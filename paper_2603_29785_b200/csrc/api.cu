@@ -52,6 +52,9 @@ void free_plan(qtam_plan *p) {
   cudaFree(p->d_tiny); cudaFree(p->d_ptw); cudaFree(p->d_ptw_long); cudaFree(p->d_frows_fwd); cudaFree(p->d_fmem); cudaFree(p->d_tmem);
   cudaFree(p->d_thr_tasks); cudaFree(p->d_thr_offs);
   for (int c = 0; c < kCtaClasses; ++c) { cudaFree(p->d_cta_lead[c]); cudaFree(p->d_ptw_rows[c]); cudaFree(p->d_cta_groups[c]); cudaFree(p->d_cta_mem[c]); }
+  cudaFree(p->d_sp_tw2);
+  for (int c = 0; c < kClClasses; ++c) { cudaFree(p->d_sp_ftw[c]); cudaFree(p->d_sp_scratch[c]); cudaFree(p->d_sp_ctl[c]); cudaFree(p->d_sp_order[c]); cudaFree(p->d_sp_wt[c]); cudaFree(p->d_sp_wtoff[c]); }
+  cudaFree(p->d_sp_xt);
   for (int c = 0; c < kClClasses; ++c) { cudaFree(p->d_cl_lead[c]); cudaFree(p->d_cl_mem[c]); cudaFree(p->d_cl_groups[c]); cudaFree(p->d_cl_ftw[c]); }
   cudaFree(p->d_cl_ptw);
   cudaFree(p->d_runs); cudaFree(p->d_run_ptr); cudaFree(p->d_run_idx);
@@ -492,6 +495,7 @@ qtam_status qtam_forward(qtam_plan *p, const void *d_x, int batch, void *d_coef,
   if (batch == 0) return QTAM_OK;
   cudaStream_t st = static_cast<cudaStream_t>(stream);
   qtam_status s = p->fast_long ? fast_r2c(p, d_x, batch, st) : generic_r2c(p, d_x, batch, st);
+  if (s == QTAM_OK) s = split_spectrum(p, batch, st);
   if (s != QTAM_OK) return s;
   // the row launches are independent of each other (they read the spectrum and write disjoint coefficients):
   // the longest rows first, every launch on a stream of its own, joined before the call returns to the caller's
@@ -513,7 +517,8 @@ qtam_status qtam_forward_threshold(qtam_plan *p, const void *d_x, int batch, dou
   cudaStream_t st = static_cast<cudaStream_t>(stream);
   if (p->fast_rows && p->esz == 4) {
     // the threshold rides in the epilogue of the row kernel for every row of at most 1024 points
-    qtam_status s = p->fast_long ? fast_r2c(p, d_x, batch, st) : generic_r2c(p, d_x, batch, st);
+      qtam_status s = p->fast_long ? fast_r2c(p, d_x, batch, st) : generic_r2c(p, d_x, batch, st);
+    if (s == QTAM_OK) s = split_spectrum(p, batch, st);
     if (s != QTAM_OK) return s;
     bool fused = false;
     s = fast_forward_rows_threshold(p, batch, d_coef, (float)kappa, st, &fused);
@@ -731,7 +736,7 @@ static const char *const kKernelNames[K_COUNT] = {
     "inv_rows", "inv_reduce", "dense_place", "threshold", "r2c_fast", "fwd_rows_fast", "inv_rows_fast",
     "reduce_c2r_fast", "inv_fused", "inv_tiles", "combine_c2r", "threshold_fast", "rows_cta_fwd", "rows_cta_inv",
     "tiny_rows_fwd", "tiny_rows_inv", "long_fft_a", "long_fft_b", "plane_metric", "best_plane", "remodulate", "inst_freq", "fwd_rows_thr", "gather_plane",
-    "rows_cl_fwd", "rows_cl_inv", "combine_runs", "c2c_fast", "split3", "combine3", "len_band", "len_synth", "len_analysis", "cluster", "mask"};
+    "rows_cl_fwd", "rows_cl_inv", "combine_runs", "c2c_fast", "split3", "combine3", "len_band", "len_synth", "len_analysis", "cluster", "mask", "spec_residues"};
 
 qtam_status qtam_profile_enable(qtam_plan *p, int on, int max_launches) {
   if (!p || p->host_only) return QTAM_ERR_INVALID_ARG;

@@ -28,9 +28,17 @@ k_combine_runs(const int4 *__restrict__ runs, const int *__restrict__ ptr, const
                long long sumL, const float *__restrict__ invP, int Nc, int plane, const float2 *__restrict__ tw,
                int tw_shift, float2 *__restrict__ spec, long long xstride) {
   __shared__ int4 s_runs[kRunChunk];
+  __shared__ float2 s_xch[2][kRunBlock];
   const int b = blockIdx.x, seg = blockIdx.y;
   const int f = b * kRunBlock + threadIdx.x;
   const int g = Nc - f;
+  // Runs sorted by residue (src 2, rows_split.cu) hold the block's 256 bins as 64 residues x 4 consecutive
+  // elements: they are read with a second thread -> bin map that follows that order (tf for the block's bins, tg
+  // for the mirrored ones) and handed to the bins' own threads through shared memory at the end.
+  const int tq = 64 * (threadIdx.x & 3) + (threadIdx.x >> 2);
+  const int tf = b * kRunBlock + tq;
+  const int tg = Nc - b * kRunBlock - (kRunBlock - 1) + tq;
+  float2 At = make_float2(0.f, 0.f), Bt = make_float2(0.f, 0.f);
   const float2 *ps = part + (size_t)seg * part_stride;
   const float2 *bs = band + (size_t)seg * sumL;
   // lists 2b (runs that touch the block's bins f) and 2b + 1 (its mirror bins g) are adjacent in idx
@@ -43,23 +51,41 @@ k_combine_runs(const int4 *__restrict__ runs, const int *__restrict__ ptr, const
     __syncthreads();
     // the runs are added in list order (a fixed order); the loads of four runs are in flight together
     for (int i0 = 0; i0 < n; i0 += 4) {
-      float2 v[4]; bool forA[4];
+      float2 v[4]; bool forA[4], byres[4];
 #pragma unroll
       for (int k = 0; k < 4; ++k) {
         v[k] = make_float2(0.f, 0.f);
         forA[k] = c0 + i0 + k < e1;
+        byres[k] = false;
         if (i0 + k < n) {
-          const int4 r = s_runs[i0 + k];           // lo, nb, off, src | (plane + 1) << 1
-          const int rp = (r.w >> 1) - 1;
-          const unsigned d = (unsigned)((forA[k] ? f : g) - r.x);
-          if (d < (unsigned)r.y && !(rp >= 0 && plane >= 0 && rp != plane))
-            v[k] = __ldcs(((r.w & 1) ? ps : bs) + (size_t)r.z + d);
+          const int4 r = s_runs[i0 + k];           // lo, nb, off, src | (plane + 1) << 2
+          const int rp = (r.w >> 2) - 1;
+          const int src = r.w & 3;
+          byres[k] = src == 2;
+          const int x = byres[k] ? (forA[k] ? tf : tg) : (forA[k] ? f : g);
+          const unsigned d = (unsigned)(x - r.x);
+          if (d < (unsigned)r.y && !(rp >= 0 && plane >= 0 && rp != plane)) {
+            if (byres[k]) {
+              const int len64 = ((r.x + r.y - 1) >> 6) - (r.x >> 6) + 1;
+              v[k] = __ldcs(ps + (size_t)r.z + (size_t)(x & 63) * len64 + ((x >> 6) - (r.x >> 6)));
+            } else {
+              v[k] = __ldcs((src == 1 ? ps : bs) + (size_t)r.z + d);
+            }
+          }
         }
       }
 #pragma unroll
-      for (int k = 0; k < 4; ++k) { if (forA[k]) A = padd(A, v[k]); else B = padd(B, v[k]); }
+      for (int k = 0; k < 4; ++k) {
+        if (byres[k]) { if (forA[k]) At = padd(At, v[k]); else Bt = padd(Bt, v[k]); }
+        else { if (forA[k]) A = padd(A, v[k]); else B = padd(B, v[k]); }
+      }
     }
   }
+  s_xch[0][tq] = At;
+  s_xch[1][kRunBlock - 1 - tq] = Bt;
+  __syncthreads();
+  A = padd(A, s_xch[0][threadIdx.x]);
+  B = padd(B, s_xch[1][threadIdx.x]);
   if (f > Nc / 2) return;
   A = pscale(A, __ldg(invP + f));
   B = pscale(B, __ldg(invP + g));
@@ -103,7 +129,7 @@ qtam_status build_runs(qtam_plan *p) {
   std::vector<int4> dev(p->runs.size());
   for (size_t i = 0; i < p->runs.size(); ++i) {
     const HostRun &r = p->runs[i];
-    dev[i] = make_int4(r.lo, r.nb, (int)r.off, r.src | ((r.plane + 1) << 1));
+    dev[i] = make_int4(r.lo, r.nb, (int)r.off, r.src | ((r.plane + 1) << 2));
   }
   std::vector<int> ptr(2 * (size_t)nblk + 1, 0), idx;
   for (int b = 0; b < nblk; ++b) {

@@ -15,7 +15,7 @@ enum KernelId {
   K_REDUCE_C2R_FAST, K_INV_FUSED, K_INV_TILES, K_COMBINE_C2R, K_THRESHOLD_FAST, K_ROWS_CTA_FWD, K_ROWS_CTA_INV,
   K_TINY_FWD, K_TINY_INV, K_LONG_A, K_LONG_B, K_PLANE_METRIC, K_BEST_PLANE, K_REMODULATE, K_INST_FREQ, K_FWD_ROWS_THR, K_GATHER_PLANE,
   K_ROWS_CL_FWD, K_ROWS_CL_INV, K_COMBINE_RUNS, K_C2C_FAST, K_SPLIT3, K_COMBINE3, K_LEN_BAND, K_LEN_SYNTH, K_LEN_ANALYSIS,
-  K_CLUSTER, K_MASK, K_COUNT
+  K_CLUSTER, K_MASK, K_SPEC_RES, K_COUNT
 };
 // fast float path (fast.cu): rows with 32 <= M <= 1024, grouped by G = M/32 lanes per row
 struct FastRow { int kc, dk, woff, goff, offset, plane, wpad, pad; };   // wpad: offset into the padded window table
@@ -48,7 +48,9 @@ struct __align__(16) ClLeader { int kc, dk, woff, mem0; int nmem, row; float fwd
 struct ClGroup { int lead0, nlead, lo, nb; long long part_off; };
 // a run = a contiguous piece of the spectrum held somewhere: `nb` bins from bin `lo` at element `off` of a
 // segment's partial-sum buffer (src 1) or band workspace (src 0); plane >= 0: only for the joint inverse and for
-// that plane's own (a band slot of one row).  k_combine_runs adds the runs that cover a bin in list order.
+// that plane's own (a band slot of one row); src 2: a partial sum sorted by residue, bin f at element
+// off - lo div 64 + (f mod 64) len64 + f div 64 (rows_split.cu).  k_combine_runs adds the runs that cover a bin
+// in list order.
 struct HostRun { int lo, nb; long long off; int src, plane; };
 struct ProfRec { int kid; double bytes, design; cudaEvent_t e0, e1; };
 }  // namespace qtam
@@ -178,17 +180,30 @@ struct qtam_plan {
   double cl_sumM[qtam::kClClasses] = {}, cl_sumL[qtam::kClClasses] = {};
   void *d_cl_ptw = nullptr;                             // pass tables of the 4096-point sub-transforms
   void *d_cl_ftw[qtam::kClClasses] = {};                // radix-F twiddles per class
+  // dataflow rows (rows_split.cu): the classes of 2^14 .. 2^16 points as sub-transform and radix-F items
+  bool sp_ok[qtam::kClClasses] = {};
+  int sp_lag[qtam::kClClasses] = {}, sp_nslots[qtam::kClClasses] = {};
+  void *d_sp_tw2 = nullptr;                             // pass-2 table of the 1024-point sub-transforms
+  void *d_sp_ftw[qtam::kClClasses] = {};                // radix-F twiddles per class
+  void *d_sp_scratch[qtam::kClClasses] = {};            // ring of row slots (the intermediate; stays in L2)
+  int *d_sp_ctl[qtam::kClClasses] = {};                 // item counter + per-row completion counts
+  void *d_sp_order[qtam::kClClasses] = {};              // inverse row order (SpOrder records)
+  long long sp_part_lo[qtam::kClClasses] = {}, sp_part_len[qtam::kClClasses] = {};   // the class's partial sums
+  int sp_nmem[qtam::kClClasses] = {};
+  void *d_sp_wt[qtam::kClClasses] = {}, *d_sp_wtoff[qtam::kClClasses] = {};   // windows by residue, first element per leader
+  void *d_sp_xt = nullptr;                              // spectrum by residue [max_batch][64][sp_xt_len]
+  int sp_xt_len = 0;
   // run-based combine (combine_runs.cu): the inverse of every float plan that is not on the tiled path
   bool use_runs = false;
   std::vector<qtam::HostRun> runs;                      // in summation order (tiles, CTA groups, cluster groups, band slots)
-  int4 *d_runs = nullptr;                               // (lo, nb, off, src | (plane + 1) << 1)
+  int4 *d_runs = nullptr;                               // (lo, nb, off, src | (plane + 1) << 2)
   int *d_run_ptr = nullptr, *d_run_idx = nullptr;       // lists 2b (bins f) and 2b + 1 (mirror bins Nc - f) of block b
   int n_run_blocks = 0;
   bool tiles_ok = false;                                // rows of 32 .. 1024 points have tiles (k_inv_tiles)
 
   // launch configurations fixed at plan creation (see KernelCfg)
   qtam::KernelCfg cfg_r2c, cfg_rows_fwd, cfg_rows_thr, cfg_rows_inv, cfg_tiles, cfg_combine,
-      cfg_rows_cta[qtam::kCtaClasses][2], cfg_rows_cl[qtam::kClClasses][2], cfg_c2c;
+      cfg_rows_cta[qtam::kCtaClasses][2], cfg_rows_cl[qtam::kClClasses][2], cfg_rows_sp[qtam::kClClasses][2], cfg_c2c;
 
   // output-length options (length.cu): the plan's uniform length n, the standard one, e^{2 pi i m/n} for both
   long long len_n = 0, len_std = 0;
@@ -303,7 +318,8 @@ qtam_status remodulate(qtam_plan *p, const void *d_coef, int batch, void *d_out,
 qtam_status instantaneous_frequency(qtam_plan *p, const void *d_coef, int batch, void *d_out, cudaStream_t st);
 // rows_cta.cu
 void build_leaders_and_groups(qtam_plan *p, const std::vector<int> &rows_in, int groups_wanted,
-                              std::vector<ClLeader> &lead, std::vector<int2> &mem, std::vector<ClGroup> &groups);
+                              std::vector<ClLeader> &lead, std::vector<int2> &mem, std::vector<ClGroup> &groups,
+                              int by_residue_max_lead, int by_residue_max_mem, bool *by_residue);
 qtam_status build_rows_cta(qtam_plan *p);
 qtam_status cta_forward_rows(qtam_plan *p, int batch, void *d_coef, Fork &fk);
 qtam_status cta_inverse_rows(qtam_plan *p, const void *d_coef, int batch, int plane, Fork &fk);
@@ -311,6 +327,13 @@ qtam_status cta_inverse_rows(qtam_plan *p, const void *d_coef, int batch, int pl
 qtam_status build_rows_cluster(qtam_plan *p);
 qtam_status cluster_forward_rows(qtam_plan *p, int batch, void *d_coef, Fork &fk);
 qtam_status cluster_inverse_rows(qtam_plan *p, const void *d_coef, int batch, int plane, Fork &fk);
+// rows_split.cu
+qtam_status build_rows_split(qtam_plan *p, int c, const std::vector<ClLeader> &lead, const std::vector<int2> &mem,
+                             const std::vector<ClGroup> &groups);
+int split_max_leaders();
+int split_max_members();
+qtam_status split_rows(qtam_plan *p, int c, bool fwd, int batch, void *d_coef, int plane, cudaStream_t st);
+qtam_status split_spectrum(qtam_plan *p, int batch, cudaStream_t st);
 // combine_runs.cu
 qtam_status build_runs(qtam_plan *p);
 qtam_status combine_runs(qtam_plan *p, int batch, int plane, cudaStream_t st);

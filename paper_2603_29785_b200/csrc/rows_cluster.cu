@@ -339,7 +339,12 @@ qtam_status build_rows_cluster(qtam_plan *p) {
     std::vector<ClGroup> groups;
     // about ten groups per class: (groups x segments) spreads over the resident clusters while the partial sums
     // stay a fraction of the band values
-    build_leaders_and_groups(p, idx, 10, lead, mem, groups);
+    // the classes of 2^15 and 2^16 points run as the dataflow of rows_split.cu (partial sums sorted by residue)
+    // when their tables fit its shared memory; one CTA holds a 2^14-point row, and the 2^17-point rows stay here
+    bool by_residue = false;
+    const bool want = c == 1 || c == 2;
+    build_leaders_and_groups(p, idx, want ? 6 : 10, lead, mem, groups, want ? split_max_leaders() : 0,
+                             want ? split_max_members() : 0, &by_residue);
     p->n_cl_lead[c] = (int)lead.size(); p->n_cl_groups[c] = (int)groups.size();
     if (!up(reinterpret_cast<void **>(&p->d_cl_lead[c]), lead.data(), lead.size() * sizeof(ClLeader))) return QTAM_ERR_ALLOC;
     if (!up(reinterpret_cast<void **>(&p->d_cl_mem[c]), mem.data(), mem.size() * sizeof(int2))) return QTAM_ERR_ALLOC;
@@ -357,6 +362,10 @@ qtam_status build_rows_cluster(qtam_plan *p) {
     }
     if (!ok) return QTAM_ERR_CUDA;
     p->cl_rows = true;
+    if (by_residue) {
+      const qtam_status ss = build_rows_split(p, c, lead, mem, groups);
+      if (ss != QTAM_OK) return ss;
+    }
   }
   if (p->cl_rows) {
     std::vector<float> t;
@@ -404,8 +413,12 @@ template <bool FWD>
 static qtam_status cl_all(qtam_plan *p, int batch, void *d_coef, int plane, Fork &fk) {
   qtam_status s = QTAM_OK;
   if (p->n_cl_lead[3]) s = cl_launch<kClLog2P, 3, FWD>(p, 3, batch, d_coef, plane, fk.next());
-  if (s == QTAM_OK && p->n_cl_lead[2]) s = cl_launch<kClLog2P, 2, FWD>(p, 2, batch, d_coef, plane, fk.next());
-  if (s == QTAM_OK && p->n_cl_lead[1]) s = cl_launch<kClLog2P, 1, FWD>(p, 1, batch, d_coef, plane, fk.next());
+  if (s == QTAM_OK && p->n_cl_lead[2])
+    s = p->sp_ok[2] ? split_rows(p, 2, FWD, batch, d_coef, plane, fk.next())
+                    : cl_launch<kClLog2P, 2, FWD>(p, 2, batch, d_coef, plane, fk.next());
+  if (s == QTAM_OK && p->n_cl_lead[1])
+    s = p->sp_ok[1] ? split_rows(p, 1, FWD, batch, d_coef, plane, fk.next())
+                    : cl_launch<kClLog2P, 1, FWD>(p, 1, batch, d_coef, plane, fk.next());
   if (s == QTAM_OK && p->n_cl_lead[0]) s = cl_launch<kClLog2P, 0, FWD>(p, 0, batch, d_coef, plane, fk.next());
   return s;
 }

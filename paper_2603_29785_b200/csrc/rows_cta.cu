@@ -149,7 +149,8 @@ template <int L2> static bool prepare_class(qtam_plan *p, int c) {
 // ascending centre bin, and groups of consecutive leaders for the inverse; the groups' partial sums are appended
 // to the plan's per-segment partial-sum layout and registered as runs for k_combine_runs.
 void build_leaders_and_groups(qtam_plan *p, const std::vector<int> &rows_in, int groups_wanted,
-                              std::vector<ClLeader> &lead, std::vector<int2> &mem, std::vector<ClGroup> &groups) {
+                              std::vector<ClLeader> &lead, std::vector<int2> &mem, std::vector<ClGroup> &groups,
+                              int by_residue_max_lead, int by_residue_max_mem, bool *by_residue) {
   const HostPlan &hp = p->hp;
   std::vector<int> idx = rows_in;
   std::stable_sort(idx.begin(), idx.end(), [&](int a, int b) {
@@ -181,6 +182,9 @@ void build_leaders_and_groups(qtam_plan *p, const std::vector<int> &rows_in, int
     lead.push_back(L);
     for (int k : st) mem.push_back(make_int2((int)hp.rows[(size_t)k].offset, hp.rows[(size_t)k].plane));
   }
+  // partial sums sorted by residue mod 64 (rows_split.cu) when the class is small enough for that kernel
+  const bool res64 = (int)lead.size() <= by_residue_max_lead && (int)mem.size() <= by_residue_max_mem;
+  if (by_residue) *by_residue = res64;
   const int per = std::max<int>(1, ((int)lead.size() + groups_wanted - 1) / groups_wanted);
   for (size_t i = 0; i < lead.size(); i += (size_t)per) {
     ClGroup g{};
@@ -194,8 +198,13 @@ void build_leaders_and_groups(qtam_plan *p, const std::vector<int> &rows_in, int
     if (hi < lo) { lo = 0; hi = -1; }
     g.lo = (int)lo; g.nb = (int)(hi - lo + 1);
     g.part_off = p->part_stride;
-    p->part_stride += (g.nb + 1) & ~1;
-    p->runs.push_back(HostRun{(int)lo, g.nb, g.part_off, 1, -1});
+    if (res64 && g.nb > 0) {
+      p->part_stride += 64 * (((lo + g.nb - 1) >> 6) - (lo >> 6) + 1);
+      p->runs.push_back(HostRun{(int)lo, g.nb, g.part_off, 2, -1});
+    } else {
+      p->part_stride += (g.nb + 1) & ~1;
+      p->runs.push_back(HostRun{(int)lo, g.nb, g.part_off, 1, -1});
+    }
     groups.push_back(g);
   }
 }
@@ -223,7 +232,7 @@ qtam_status build_rows_cta(qtam_plan *p) {
     std::vector<ClLeader> lead;
     std::vector<int2> mem;
     std::vector<ClGroup> groups;
-    build_leaders_and_groups(p, idx, 12, lead, mem, groups);
+    build_leaders_and_groups(p, idx, 12, lead, mem, groups, 0, 0, nullptr);
     p->n_cta_rows[c] = (int)lead.size(); p->n_cta_groups[c] = (int)groups.size();
     if (!up(reinterpret_cast<void **>(&p->d_cta_lead[c]), lead.data(), lead.size() * sizeof(ClLeader))) return QTAM_ERR_ALLOC;
     if (!up(reinterpret_cast<void **>(&p->d_cta_mem[c]), mem.data(), mem.size() * sizeof(int2))) return QTAM_ERR_ALLOC;
