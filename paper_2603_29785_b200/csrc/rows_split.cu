@@ -139,29 +139,40 @@ template <int F> __device__ __forceinline__ void sp_twiddleF(float2 (&v)[F], flo
   }
 }
 
-// Radix-2 step across a pair of threads (lanes l and l ^ 16; h says which of the two I am) around the 32-point
-// transforms of a 64-point stage.  DIF (forward: the thread holds t[32 h + i], i < 32): h = 0 keeps v + o,
-// h = 1 keeps (o - v) w_64^{+i}, o being the partner's value.  DIT (inverse: the thread holds U_h[i]): h = 1
-// first multiplies its values by w_64^{-i}; then h = 0 keeps v + o, h = 1 keeps o - v.
-template <int I, int N, bool DIF> struct SpPair {
-  static __device__ __forceinline__ void run(float2 (&v)[N], bool h) {
+// v[i] *= w_64^{DIR i}, i < N (compile-time twiddles)
+template <int I, int N, int DIR> struct SpTw64 {
+  static __device__ __forceinline__ void run(float2 (&v)[N]) {
     constexpr float c = cos64(I);
-    constexpr float sn = DIF ? sin64(I) : -sin64(I);
-    float2 x = v[I];
-    if constexpr (!DIF && I != 0) {
-      const float2 t = pfma(x, make_float2(c, c), pmul(make_float2(-x.y, x.x), make_float2(sn, sn)));
-      x = h ? t : x;
-    }
-    float2 o;
-    o.x = __shfl_xor_sync(0xffffffffu, x.x, 16);
-    o.y = __shfl_xor_sync(0xffffffffu, x.y, 16);
-    const float2 sum = padd(x, o);
-    float2 d = psub(o, x);
-    if constexpr (DIF && I != 0) d = pfma(d, make_float2(c, c), pmul(make_float2(-d.y, d.x), make_float2(sn, sn)));
-    v[I] = h ? d : sum;
-    if constexpr (I + 1 < N) SpPair<I + 1, N, DIF>::run(v, h);
+    constexpr float sn = DIR > 0 ? sin64(I) : -sin64(I);
+    if constexpr (I != 0) v[I] = pfma(v[I], make_float2(c, c), pmul(make_float2(-v[I].y, v[I].x), make_float2(sn, sn)));
+    if constexpr (I + 1 < N) SpTw64<I + 1, N, DIR>::run(v);
   }
 };
+
+// Radix-2 step across a pair of lanes (l and l ^ 16; h says which of the two I am) around the 32-point transforms
+// of a 64-point stage; the values cross through the warp's private shared memory (one store and one load per
+// value: shuffles under a lane-dependent mask cost three instructions each).  DIF (forward: the lane holds
+// t[32 h + i]): h = 0 keeps v + o, h = 1 keeps (o - v) w_64^{+i}, o being the partner's value.  DIT (inverse: the
+// lane holds U_h[i]): h = 1 first multiplies its values by w_64^{-i}; then h = 0 keeps v + o, h = 1 keeps o - v.
+template <int N, bool DIF>
+__device__ __forceinline__ void sp_pair(float2 (&v)[N], bool h, float2 *sw) {
+  const int lane = threadIdx.x & 31;
+  if (!DIF && h) SpTw64<0, N, -1>::run(v);
+  __syncwarp();
+#pragma unroll
+  for (int i = 0; i < N; ++i) sw[i * 32 + lane] = v[i];
+  __syncwarp();
+  const float2 *o = sw + (lane ^ 16);
+  if (h) {
+#pragma unroll
+    for (int i = 0; i < N; ++i) v[i] = psub(o[i * 32], v[i]);
+    if (DIF) SpTw64<0, N, +1>::run(v);
+  } else {
+#pragma unroll
+    for (int i = 0; i < N; ++i) v[i] = padd(v[i], o[i * 32]);
+  }
+  __syncwarp();
+}
 
 // Work items are warp-sized: a sub-transform item is one residue q of one row (a P-point transform in the warp's
 // registers and private shared memory), a radix-F item 32 values of nc (16 when a pair of lanes shares an nc).
@@ -219,7 +230,6 @@ __device__ __forceinline__ void sp_fwd_sub(const SpArgs &A, const SpShared &sh, 
     const int res = f0 & (kSpRes - 1), idx = (f0 >> 6) + kSpPad;   // floor semantics for negative bins
     const float2 *Xp = A.xt + (size_t)seg * A.xt_stride + (size_t)res * A.xt_len + idx + (lane - e) / S;
     const float *Wp = A.wt + sh.wt[li] + q * P + lane;
-    const float scale = L.fwd_scale;
     float w[32];
 #pragma unroll
     for (int r = 0; r < 32; ++r) {
@@ -227,7 +237,7 @@ __device__ __forceinline__ void sp_fwd_sub(const SpArgs &A, const SpShared &sh, 
       w[r] = __ldg(Wp + 32 * r);
     }
 #pragma unroll
-    for (int r = 0; r < 32; ++r) v[r] = pscale(v[r], w[r] * scale);
+    for (int r = 0; r < 32; ++r) v[r] = pscale(v[r], w[r]);        // (N M)^-1/2 rides on the radix-F twiddles
   }
   RegFFT<32, +1>::run(v);
 #pragma unroll
@@ -245,7 +255,8 @@ __device__ __forceinline__ void sp_fwd_sub(const SpArgs &A, const SpShared &sh, 
 }
 
 template <int F, class Mid>
-__device__ __forceinline__ void sp_fwd_radix(const SpArgs &A, const SpShared &sh, int row, int ncb, const Mid &mid) {
+__device__ __forceinline__ void sp_fwd_radix(const SpArgs &A, const SpShared &sh, float2 *sw, int row, int ncb,
+                                             const Mid &mid) {
   typedef SpGeo<F> G;
   constexpr int P = kSpP, M = F * P, FT = G::FT;
   const int lane = threadIdx.x & 31;
@@ -261,8 +272,9 @@ __device__ __forceinline__ void sp_fwd_radix(const SpArgs &A, const SpShared &sh
   const float2 w1 = __ldg(A.ftw + nc), w4 = __ldg(A.ftw + P + nc);
   float2 w0 = make_float2(1.f, 0.f);
   if (G::PAIR == 2 && h) w0 = __ldg(A.ftw + 2 * P + nc);
+  w0 = pscale(w0, L.fwd_scale);            // C47's (N M)^-1/2
   sp_twiddleF<FT>(v, w0, w1, w4);
-  if constexpr (G::PAIR == 2) SpPair<0, FT, true>::run(v, h != 0);
+  if constexpr (G::PAIR == 2) sp_pair<FT, true>(v, h != 0, sw);
   RegFFT<FT, +1>::run(v);
   // Y[nc + P m], m = PAIR mm + h, to every member of the leader's set (identical rows are transformed once)
   float2 *Yseg = A.coef + (size_t)seg * A.ctot + nc + (size_t)h * P;
@@ -279,12 +291,13 @@ __device__ __forceinline__ void sp_fwd_radix(const SpArgs &A, const SpShared &sh
 // inverse items (row t of the order: position oi = t / batch of the order table, segment t % batch)
 // --------------------------------------------------------------------------------------------------
 template <int F, class Mid>
-__device__ __forceinline__ void sp_inv_radix(const SpArgs &A, const SpShared &sh, const int *off, int nm, int row,
-                                             int ncb, const Mid &mid) {
+__device__ __forceinline__ void sp_inv_radix(const SpArgs &A, const SpShared &sh, float2 *sw, const int *off, int nm,
+                                             int row, int ncb, const Mid &mid) {
   typedef SpGeo<F> G;
   constexpr int P = kSpP, M = F * P, FT = G::FT;
   const int lane = threadIdx.x & 31;
   const int oi = row / A.batch, seg = row - oi * A.batch;
+  const float amp = sh.lead[sh.order[oi].lead].inv_amp;
   const int h = G::PAIR == 2 ? (lane >> 4) : 0;
   const int nc = ncb * G::NC_ITEM + (G::PAIR == 2 ? (lane & 15) : lane);
   const float2 *Yseg = A.coef + (size_t)seg * A.ctot + nc + (size_t)h * P;
@@ -306,8 +319,9 @@ __device__ __forceinline__ void sp_inv_radix(const SpArgs &A, const SpShared &sh
   float2 w0 = make_float2(1.f, 0.f);
   if (G::PAIR == 2 && h) w0 = __ldg(A.ftw + 2 * P + nc);
   w1.y = -w1.y; w4.y = -w4.y; w0.y = -w0.y;
+  w0 = pscale(w0, amp);                    // C49's sqrt(N/M)
   RegFFT<FT, -1>::run(v);
-  if constexpr (G::PAIR == 2) SpPair<0, FT, false>::run(v, h != 0);
+  if constexpr (G::PAIR == 2) sp_pair<FT, false>(v, h != 0, sw);
   sp_twiddleF<FT>(v, w0, w1, w4);          // lane h now holds u[q = FT h + i][nc]
   float2 *Z = A.scratch + (size_t)(row % A.nslots) * M;
   mid();
@@ -348,7 +362,6 @@ __device__ __forceinline__ void sp_inv_sub(const SpArgs &A, const SpShared &sh, 
   const int hi = min(L.dk, A.nbins - 1 - L.kc), lo = max(-L.dk, -L.kc);
   const int jj0 = q + F * lane;
   const int a = hi - jj0, b = lo - jj0;
-  const float amp = L.inv_amp;
 #pragma unroll
   for (int r0 = 0; r0 < 32; r0 += 16) {
     float2 old[16]; float w[16];
@@ -365,7 +378,7 @@ __device__ __forceinline__ void sp_inv_sub(const SpArgs &A, const SpShared &sh, 
       const int r = r0 + u;
       const int c = r * 32 * F - (r >= 16 ? M : 0);
       const bool ok = r < 16 ? c <= a : c >= b;
-      const float g = amp * w[u];
+      const float g = w[u];                // sqrt(N/M) rode on the radix-F twiddles
       if (ok) __stcg(pp + (32 / S) * r - (r >= 16 ? P / S : 0), pfma(v[r], make_float2(g, g), old[u]));
     }
   }
@@ -493,7 +506,7 @@ k_rows_split(const SpArgs A) {
         if (first) {
           for (int i = 0; i < kSpChunk; ++i) sp_fwd_sub<F>(A, sh, sw, stw, row, id + i, flush);
         } else {
-          for (int i = 0; i < kSpChunk; ++i) sp_fwd_radix<F>(A, sh, row, id + i, flush);
+          for (int i = 0; i < kSpChunk; ++i) sp_fwd_radix<F>(A, sh, sw, row, id + i, flush);
         }
       } else {
         // the members that take part: none -> the row contributes nothing (the same decision in all its items)
@@ -502,7 +515,7 @@ k_rows_split(const SpArgs A) {
         const int nm = sp_members(A, sh, L, first ? off : nullptr);
         if (nm > 0) {
           if (first) {
-            for (int i = 0; i < kSpChunk; ++i) sp_inv_radix<F>(A, sh, off, nm, row, id + i, flush);
+            for (int i = 0; i < kSpChunk; ++i) sp_inv_radix<F>(A, sh, sw, off, nm, row, id + i, flush);
           } else {
             for (int i = 0; i < kSpChunk; ++i) sp_inv_sub<F>(A, sh, sw, stw, row, id + i, flush);
           }
