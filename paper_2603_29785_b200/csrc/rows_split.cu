@@ -215,9 +215,9 @@ __device__ __forceinline__ int sp_members(const SpArgs &A, const SpShared &sh, c
 // --------------------------------------------------------------------------------------------------
 // One warp = one residue q: its P-point transform lives in the warp's registers (32 values per lane) and its
 // private piece of shared memory; no block barrier.
-template <int F, class Mid>
+template <int F, class Sched>
 __device__ __forceinline__ void sp_fwd_sub(const SpArgs &A, const SpShared &sh, float2 *sw, const float2 *stw,
-                                           int row, int q, const Mid &mid) {
+                                           int row, int q, const Sched &sc) {
   constexpr int P = kSpP, M = F * P, S = kSpRes / F;      // S interleaved runs of the residue-sorted spectrum
   const int lane = threadIdx.x & 31;
   const int seg = row / A.nlead, li = row - seg * A.nlead;
@@ -249,14 +249,15 @@ __device__ __forceinline__ void sp_fwd_sub(const SpArgs &A, const SpShared &sh, 
   sp_twiddle32<+1>(v, stw, lane);
   RegFFT<32, +1>::run(v);
   float2 *Z = A.scratch + (size_t)(row % A.nslots) * M + (size_t)q * P;
-  mid();
+  sc.wait0();                              // the slot's previous row has been read
+  sc.mid();
 #pragma unroll
   for (int r = 0; r < 32; ++r) __stcg(Z + lane + 32 * r, v[r]);             // nc = lane + 32 r
 }
 
-template <int F, class Mid>
+template <int F, class Sched>
 __device__ __forceinline__ void sp_fwd_radix(const SpArgs &A, const SpShared &sh, float2 *sw, int row, int ncb,
-                                             const Mid &mid) {
+                                             const Sched &sc) {
   typedef SpGeo<F> G;
   constexpr int P = kSpP, M = F * P, FT = G::FT;
   const int lane = threadIdx.x & 31;
@@ -266,12 +267,13 @@ __device__ __forceinline__ void sp_fwd_radix(const SpArgs &A, const SpShared &sh
   const int h = G::PAIR == 2 ? (lane >> 4) : 0;
   const int nc = ncb * G::NC_ITEM + (G::PAIR == 2 ? (lane & 15) : lane);
   const float2 *Z = A.scratch + (size_t)(row % A.nslots) * M;
-  float2 v[FT];
-#pragma unroll
-  for (int i = 0; i < FT; ++i) v[i] = __ldcg(Z + (size_t)(h * FT + i) * P + nc);
   const float2 w1 = __ldg(A.ftw + nc), w4 = __ldg(A.ftw + P + nc);
   float2 w0 = make_float2(1.f, 0.f);
   if (G::PAIR == 2 && h) w0 = __ldg(A.ftw + 2 * P + nc);
+  sc.wait0();                              // the row's sub-transforms are in the slot
+  float2 v[FT];
+#pragma unroll
+  for (int i = 0; i < FT; ++i) v[i] = __ldcg(Z + (size_t)(h * FT + i) * P + nc);
   w0 = pscale(w0, L.fwd_scale);            // C47's (N M)^-1/2
   sp_twiddleF<FT>(v, w0, w1, w4);
   if constexpr (G::PAIR == 2) sp_pair<FT, true>(v, h != 0, sw);
@@ -279,7 +281,7 @@ __device__ __forceinline__ void sp_fwd_radix(const SpArgs &A, const SpShared &sh
   // Y[nc + P m], m = PAIR mm + h, to every member of the leader's set (identical rows are transformed once)
   float2 *Yseg = A.coef + (size_t)seg * A.ctot + nc + (size_t)h * P;
   const int nm = L.nmem;
-  mid();
+  sc.mid();
   for (int m = 0; m < nm; ++m) {
     float2 *Y = Yseg + sh.mem[L.mem0 + m].x;
 #pragma unroll
@@ -290,9 +292,9 @@ __device__ __forceinline__ void sp_fwd_radix(const SpArgs &A, const SpShared &sh
 // --------------------------------------------------------------------------------------------------
 // inverse items (row t of the order: position oi = t / batch of the order table, segment t % batch)
 // --------------------------------------------------------------------------------------------------
-template <int F, class Mid>
+template <int F, class Sched>
 __device__ __forceinline__ void sp_inv_radix(const SpArgs &A, const SpShared &sh, float2 *sw, const int *off, int nm,
-                                             int row, int ncb, const Mid &mid) {
+                                             int row, int ncb, const Sched &sc) {
   typedef SpGeo<F> G;
   constexpr int P = kSpP, M = F * P, FT = G::FT;
   const int lane = threadIdx.x & 31;
@@ -324,20 +326,22 @@ __device__ __forceinline__ void sp_inv_radix(const SpArgs &A, const SpShared &sh
   if constexpr (G::PAIR == 2) sp_pair<FT, false>(v, h != 0, sw);
   sp_twiddleF<FT>(v, w0, w1, w4);          // lane h now holds u[q = FT h + i][nc]
   float2 *Z = A.scratch + (size_t)(row % A.nslots) * M;
-  mid();
+  sc.wait0();                              // the slot's previous row has been read
+  sc.mid();
 #pragma unroll
   for (int i = 0; i < FT; ++i) __stcg(Z + (size_t)(h * FT + i) * P + nc, v[i]);
 }
 
-template <int F, class Mid>
+template <int F, class Sched>
 __device__ __forceinline__ void sp_inv_sub(const SpArgs &A, const SpShared &sh, float2 *sw, const float2 *stw,
-                                           int row, int q, const Mid &mid) {
+                                           int row, int q, const Sched &sc) {
   constexpr int P = kSpP, M = F * P, S = kSpRes / F;
   const int lane = threadIdx.x & 31;
   const int oi = row / A.batch, seg = row - oi * A.batch;
   const SpOrder O = sh.order[oi];
   const ClLeader &L = sh.lead[O.lead];
   const float2 *Z = A.scratch + (size_t)(row % A.nslots) * M + (size_t)q * P;
+  sc.wait0();                              // the row's radix-F stage is in the slot
   float2 v[32];
 #pragma unroll
   for (int r = 0; r < 32; ++r) v[r] = __ldcg(Z + lane + 32 * r);            // nc = lane + 32 r
@@ -350,7 +354,8 @@ __device__ __forceinline__ void sp_inv_sub(const SpArgs &A, const SpShared &sh, 
   __syncwarp();
   sp_twiddle32<-1>(v, stw, lane);
   RegFFT<32, -1>::run(v);                  // v[r] = Bhat[q + F jc], jc = lane + 32 r
-  mid();
+  sc.wait1();                              // the previous leader of the group has added its bands
+  sc.mid();
   // G_k[jj] = sqrt(N/M) Bhat[jj] W_k[jj], added into the group's partial sum at bin kc + jj (R8 clip).  The
   // partial sum is sorted by residue like the spectrum copy (element of bin f: (f mod 64) len64 + f div 64),
   // so a warp's updates are whole lines.  The loads of a batch are issued before its stores.
@@ -406,6 +411,10 @@ k_spec_residues(const float2 *__restrict__ spec, long long xstride, int nbins, f
 // --------------------------------------------------------------------------------------------------
 // the kernel: item order, dependencies, signals (everything per warp)
 // --------------------------------------------------------------------------------------------------
+// the schedule's hooks inside an item: wait0 / wait1 before the first access that depends on the chunk's first /
+// second count, mid just before the item's stores
+template <class W0, class W1, class M> struct SpSched { const W0 &wait0; const W1 &wait1; const M &mid; };
+
 // what a chunk waits for (up to two counts) and what it signals
 struct SpDeps { const int *p0; int n0; const int *p1; int n1; int *sig; };
 
@@ -458,77 +467,78 @@ k_rows_split(const SpArgs A) {
   int *off = sh.off[wid];
   const unsigned int total = (unsigned int)(A.nrows + A.lag) * G::PER;
 
-  // lane 0 pops the chunks and looks after the counts.  The completion signal of a chunk (fence + atomicAdd) is
-  // sent from the middle of the NEXT chunk, just before that chunk's first stores: by then the signalled stores
-  // have long been performed and the fence costs nothing, where a fence right after the stores would hold the
-  // warp for a round trip to L2.  A pending signal is sent first whenever the warp has to wait.
+  // Lane 0 looks after the schedule, with no latency in the warp's way in the steady state:
+  //  - the counts a chunk depends on are read (relaxed loads) at its top and looked at only where the dependent
+  //    access starts -- for first-stage chunks that is just before their stores into the slot, at the very end;
+  //    a count that was not there yet is polled with acquire loads;
+  //  - the next chunk is popped in the middle of the running one, just before its stores (the number is needed
+  //    at the top of the next iteration: an atomicAdd whose result is used at once costs a round trip to L2);
+  //  - the completion signal of a chunk (fence + atomicAdd) is sent from that same point of the NEXT chunk: by
+  //    then the signalled stores have been performed and the fence is cheap.  A pending signal is sent first
+  //    whenever the warp has to wait.
   int *pend = nullptr;
-  auto flush = [&]() { if (lane == 0 && pend) { __threadfence(); atomicAdd(pend, kSpChunk); pend = nullptr; } };
-  unsigned int chunk = 0; int ready = 1;
-  if (lane == 0) {
-    chunk = atomicAdd(A.queue, 1u);
-    if (chunk < total) {
-      int row, id; bool first; SpDeps D;
-      if (sp_decode<F, FWD>(A, sh, chunk, row, id, first, D))
-        ready = (!D.p0 || ld_acquire(D.p0) >= D.n0) && (!D.p1 || ld_acquire(D.p1) >= D.n1);
+  unsigned int chunk = 0, popped_val = 0; bool popped = false;
+  int v0 = 0, v1 = 0; SpDeps D;
+  D.p0 = D.p1 = nullptr; D.n0 = D.n1 = 0; D.sig = nullptr;
+  auto flush = [&]() {
+    // release only: a fence (acq_rel) would also invalidate L1
+    if (lane == 0 && pend) {
+      asm volatile("red.release.gpu.global.add.s32 [%0], %1;" :: "l"(pend), "r"(kSpChunk) : "memory");
+      pend = nullptr;
     }
-  }
+  };
+  auto wait_on = [&](const int *p, int n, int v) {
+    if (lane == 0 && p && v < n) { flush(); while (ld_acquire(p) < n) __nanosleep(64); }
+    __syncwarp();
+  };
+  auto wait0 = [&]() { wait_on(D.p0, D.n0, v0); };
+  auto wait1 = [&]() { wait_on(D.p1, D.n1, v1); };
+  auto mid = [&]() {
+    flush();
+    if (lane == 0 && !popped) { popped_val = atomicAdd(A.queue, 1u); popped = true; }
+  };
+  const SpSched<decltype(wait0), decltype(wait1), decltype(mid)> sc{wait0, wait1, mid};
+  if (lane == 0) chunk = atomicAdd(A.queue, 1u);
   for (;;) {
     chunk = __shfl_sync(0xffffffffu, chunk, 0);
-    ready = __shfl_sync(0xffffffffu, ready, 0);
     if (chunk >= total) break;
-    int row, id; bool first; SpDeps D;
+    int row, id; bool first;
     const bool valid = sp_decode<F, FWD>(A, sh, chunk, row, id, first, D);
-    // lane 0: the next chunk's number and its counts arrive while this chunk runs
-    unsigned int nchunk = 0; int v0 = 0, v1 = 0; SpDeps ND; bool nvalid = false;
-    ND.p0 = ND.p1 = nullptr; ND.n0 = ND.n1 = 0;
-    if (lane == 0) {
-      nchunk = atomicAdd(A.queue, 1u);
-      if (nchunk < total) {
-        int nrow, nid; bool nfirst;
-        nvalid = sp_decode<F, FWD>(A, sh, nchunk, nrow, nid, nfirst, ND);
-        if (nvalid) {
-          if (ND.p0) asm volatile("ld.relaxed.gpu.global.s32 %0, [%1];" : "=r"(v0) : "l"(ND.p0) : "memory");
-          if (ND.p1) asm volatile("ld.relaxed.gpu.global.s32 %0, [%1];" : "=r"(v1) : "l"(ND.p1) : "memory");
-        }
-      }
+    popped = false; v0 = 0; v1 = 0;
+    if (lane == 0 && valid) {
+      // (relaxed: the data these counts guard is read through L2 -- ld.cg -- where the signalling warp's fence has
+      // put it before the count moved)
+      if (D.p0) asm volatile("ld.relaxed.gpu.global.s32 %0, [%1];" : "=r"(v0) : "l"(D.p0) : "memory");
+      if (D.p1) asm volatile("ld.relaxed.gpu.global.s32 %0, [%1];" : "=r"(v1) : "l"(D.p1) : "memory");
     }
     if (valid) {
-      if (!ready) {                        // rare: the counts were not there yet when lane 0 looked
-        flush();
-        if (lane == 0) {
-          if (D.p0) while (ld_acquire(D.p0) < D.n0) __nanosleep(64);
-          if (D.p1) while (ld_acquire(D.p1) < D.n1) __nanosleep(64);
-        }
-        __syncwarp();
-      }
       if constexpr (FWD) {
         if (first) {
-          for (int i = 0; i < kSpChunk; ++i) sp_fwd_sub<F>(A, sh, sw, stw, row, id + i, flush);
+          for (int i = 0; i < kSpChunk; ++i) sp_fwd_sub<F>(A, sh, sw, stw, row, id + i, sc);
         } else {
-          for (int i = 0; i < kSpChunk; ++i) sp_fwd_radix<F>(A, sh, sw, row, id + i, flush);
+          for (int i = 0; i < kSpChunk; ++i) sp_fwd_radix<F>(A, sh, sw, row, id + i, sc);
         }
       } else {
-        // the members that take part: none -> the row contributes nothing (the same decision in all its items)
+        // the members that take part: none -> the row contributes nothing (the same decision in all its items);
+        // its place in the order of the group's leaders is kept all the same
         const int oi = row / A.batch;
         const ClLeader &L = sh.lead[sh.order[oi].lead];
         const int nm = sp_members(A, sh, L, first ? off : nullptr);
         if (nm > 0) {
           if (first) {
-            for (int i = 0; i < kSpChunk; ++i) sp_inv_radix<F>(A, sh, sw, off, nm, row, id + i, flush);
+            for (int i = 0; i < kSpChunk; ++i) sp_inv_radix<F>(A, sh, sw, off, nm, row, id + i, sc);
           } else {
-            for (int i = 0; i < kSpChunk; ++i) sp_inv_sub<F>(A, sh, sw, stw, row, id + i, flush);
+            for (int i = 0; i < kSpChunk; ++i) sp_inv_sub<F>(A, sh, sw, stw, row, id + i, sc);
           }
+        } else if (!first) {
+          wait1();
         }
       }
     }
-    flush();
-    // (the counts were read with relaxed loads; the data they guard is read after this point, through L2 --
-    // ld.cg -- where the signalling warp's fence has put it before the count moved)
+    mid();
     if (lane == 0) {
-      ready = !nvalid || ((!ND.p0 || v0 >= ND.n0) && (!ND.p1 || v1 >= ND.n1));
       if (valid) pend = D.sig;
-      chunk = nchunk;
+      chunk = popped_val;
     }
     __syncwarp();
   }
