@@ -817,3 +817,46 @@ def test_composite_bank_with_a_window_family_per_plane(dtype):
             assert worst_segment(xg, r.inverse(Yin.astype(np.complex128), plane=plane, engine=1)) <= TOL[dtype], plane
         _, C = r.frame(-1)
         assert worst_segment(g.inverse(g.forward(dev(x))).cpu().numpy(), pi_c(x64, C)) <= TOL_RT[dtype]
+
+
+# ---- long rows as a dataflow of work items (rows_split.cu) ------------------------------------------------------------
+
+def test_long_rows_partial_batches_and_two_plans_at_once():
+    """Rows of 2^15 / 2^16 points run as work items popped from a counter, with completion counts between the
+    stages (rows_split.cu).  The schedule must not depend on how many CTAs are resident: two plans running at the
+    same time on two streams (each takes part of the SMs) give what they give alone; a plan sized for a larger batch
+    works on a smaller one, call after call (counters and partial sums are reset by every call)."""
+    args_a = (16384.0, 1 << 19, [4.0, 8.0], 5.0, 8000.0, 32.0)
+    args_b = (16384.0, 1 << 19, [4.0, 6.0, 12.0], 6.0, 7900.0, 24.0)
+    ga, ra = make_plans(args_a, "f32", 3)
+    gb, _ = make_plans(args_b, "f32", 3)
+    assert max(int(r.M) for r in ga.rows) >= 1 << 15 and max(int(r.M) for r in gb.rows) >= 1 << 15
+    rng = np.random.default_rng(77)
+    x = rng.standard_normal((3, 1 << 19)).astype(np.float32)
+    dx = dev(x)
+    # alone, full batch and a partial one, twice
+    Ya = ga.forward(dx)
+    Yr = ra.forward(x[:1].astype(np.float64), engine=1)
+    assert worst_segment(Ya[:1].cpu().numpy(), Yr) <= 2e-5
+    for nb in (1, 2, 3, 2):
+        Yp = ga.forward(dx[:nb])
+        assert torch.equal(Yp, Ya[:nb])
+    xa = ga.inverse(Ya)
+    xr = ra.inverse(Ya[:1].cpu().numpy().astype(np.complex128), engine=1)
+    assert worst_segment(xa[:1].cpu().numpy(), xr) <= 2e-5
+    for nb in (2, 1, 3):
+        assert torch.equal(ga.inverse(Ya[:nb]), xa[:nb])
+    Yb = gb.forward(dx)
+    xb = gb.inverse(Yb)
+    torch.cuda.synchronize()
+    # the two plans at once on two streams, several rounds
+    s1, s2 = torch.cuda.Stream(), torch.cuda.Stream()
+    for _ in range(3):
+        with torch.cuda.stream(s1):
+            Ya2 = ga.forward(dx); xa2 = ga.inverse(Ya2)
+        with torch.cuda.stream(s2):
+            Yb2 = gb.forward(dx); xb2 = gb.inverse(Yb2)
+        s1.synchronize(); s2.synchronize()
+        assert torch.equal(Ya2, Ya) and torch.equal(Yb2, Yb)
+        assert torch.equal(xa2, xa) and torch.equal(xb2, xb)
+    ga.close(); gb.close()
