@@ -143,6 +143,8 @@ struct qtam_plan {
   void *d_ftw_fwd = nullptr;   // float2 pass-1 twiddles [bucket][n1][t], forward (x (N M)^-1/2)
   void *d_ftw_inv = nullptr;   // same, inverse (conjugate, x sqrt(N/M))
   void *d_ptw = nullptr;       // pass tables of the long FFT (ctafft.cuh)
+  void *d_ptw_mid = nullptr;   // pass tables of k_cfft_cta (N = 3 * 2^k: transforms of N/6 = 2^11 .. 2^14 points)
+  int mid_log2n = 0;
   void *d_ptw_long = nullptr;  // pass tables of the 2^14-point stage of long_fft.cu (N = 2^16 .. 2^20)
   qtam::FastRow *d_tiny = nullptr;   // rows shorter than 32 points (goff holds log2 M), for the combine kernel of inv_tiled.cu
   int n_tiny = 0;
@@ -203,7 +205,7 @@ struct qtam_plan {
 
   // launch configurations fixed at plan creation (see KernelCfg)
   qtam::KernelCfg cfg_r2c, cfg_rows_fwd, cfg_rows_thr, cfg_rows_inv, cfg_tiles, cfg_combine,
-      cfg_rows_cta[qtam::kCtaClasses][2], cfg_rows_cl[qtam::kClClasses][2], cfg_rows_sp[qtam::kClClasses][2], cfg_c2c;
+      cfg_rows_cta[qtam::kCtaClasses][2], cfg_rows_cl[qtam::kClClasses][2], cfg_rows_sp[qtam::kClClasses][2], cfg_c2c, cfg_cfft_mid[2], cfg_r3[2];
 
   // output-length options (length.cu): the plan's uniform length n, the standard one, e^{2 pi i m/n} for both
   long long len_n = 0, len_std = 0;
@@ -306,6 +308,11 @@ qtam_status fast_c2c_out(qtam_plan *p, int batch, void *d_x_out, cudaStream_t st
 // long_fft.cu
 qtam_status build_long_fft(qtam_plan *p);
 bool fast_cfft_long_ok(const qtam_plan *p, int log2n);
+bool fast_cfft_mid_ok(const qtam_plan *p, int log2n);
+bool fast_r3_ok(const qtam_plan *p);
+qtam_status fast_r3(qtam_plan *p, bool fwd, const void *d_in, void *d_out, int batch, cudaStream_t st);
+qtam_status fast_cfft_mid(qtam_plan *p, const void *in, long long in_stride, void *out, long long out_stride,
+                          int log2n, int count, int dir, float scale, cudaStream_t st, double algo);
 qtam_status fast_cfft_long(qtam_plan *p, const void *in, long long in_stride, void *out, long long out_stride,
                            void *tmp, long long tmp_stride, int log2n, int count, int dir, float scale,
                            cudaStream_t st, double algo_in, double algo_out);

@@ -503,6 +503,8 @@ static qtam_status cfft(qtam_plan *p, const C2<T> *in, long long in_stride, C2<T
     if (fast_cfft_long_ok(p, log2n) && tmp != out)
       return fast_cfft_long(p, in, in_stride, out, out_stride, tmp, tmp_stride, log2n, count, dir, scale, st,
                             algo_in, algo_out);
+    if (fast_cfft_mid_ok(p, log2n) && in != out)
+      return fast_cfft_mid(p, in, in_stride, out, out_stride, log2n, count, dir, scale, st, algo_in + algo_out);
   }
   const int cap = p->cap_log2;
   const C2<T> *tw = static_cast<const C2<T> *>(p->d_tw);
@@ -568,6 +570,7 @@ static qtam_status cfft_any(qtam_plan *p, const C2<T> *in, long long in_stride, 
 
 template <typename T>
 static qtam_status r2c_t(qtam_plan *p, const void *d_x, int batch, cudaStream_t st) {
+  if (sizeof(T) == 4 && !p->n_pow2 && fast_r3_ok(p)) return fast_r3(p, true, d_x, nullptr, batch, st);
   const int Nc = (int)(p->hp.N / 2);
   C2<T> *spec = static_cast<C2<T> *>(p->d_spec);
   C2<T> *ws = static_cast<C2<T> *>(p->d_ws);
@@ -688,6 +691,7 @@ static qtam_status c2r_t(qtam_plan *p, int batch, void *d_x_out, cudaStream_t st
 
 // the complex FFT alone, for a spectrum buffer that already holds the pre-processed Z (k_combine_runs)
 qtam_status generic_c2c_out(qtam_plan *p, int batch, void *d_x_out, cudaStream_t st) {
+  if (!p->n_pow2 && fast_r3_ok(p)) return fast_r3(p, false, nullptr, d_x_out, batch, st);
   const int Nc = (int)(p->hp.N / 2);
   return cfft_any<float>(p, static_cast<const float2 *>(p->d_spec), p->xstride, static_cast<float2 *>(d_x_out), Nc,
                          static_cast<float2 *>(p->d_ws), p->hp.N, Nc, batch, +1, 1.f, st, 0.0,

@@ -93,6 +93,158 @@ static qtam_status long_launch(qtam_plan *p, const float2 *in, long long in_stri
   return QTAM_OK;
 }
 
+// Batched complex FFTs of 2^11 .. 2^14 points, one CTA per sequence in shared memory (ctafft.cuh): the power-of-two
+// transforms inside the radix-3 step of the segment lengths N = 3 * 2^k (the paper's 6 s at 4096 Hz = 3 * 2^13).
+template <int LOG2N, int DIR>
+__global__ void __launch_bounds__(CtaFftPlan<LOG2N>::NT)
+k_cfft_cta(const float2 *__restrict__ in, long long in_stride, float2 *__restrict__ out, long long out_stride,
+           const float2 *__restrict__ ptw, float scale) {
+  float2 *s = reinterpret_cast<float2 *>(qtam_long_smem);
+  cta_fft<LOG2N, CtaFftPlan<LOG2N>::NT, DIR, true, true>(s, in + (size_t)blockIdx.x * in_stride,
+                                                         out + (size_t)blockIdx.x * out_stride, ptw, scale);
+}
+
+template <int LOG2N> static bool mid_prepare(qtam_plan *p) {
+  std::vector<float> t;
+  fill_cta_fft_tables<LOG2N, CtaFftPlan<LOG2N>::NT>(t);
+  if (cudaMalloc(&p->d_ptw_mid, t.size() * sizeof(float)) != cudaSuccess) return false;
+  p->device_bytes += t.size() * sizeof(float);
+  if (cudaMemcpy(p->d_ptw_mid, t.data(), t.size() * sizeof(float), cudaMemcpyHostToDevice) != cudaSuccess) return false;
+  const size_t smem = sizeof(float2) * (size_t)cta_fft_smem_elems<LOG2N>();
+  return kernel_prepare(p->cfg_cfft_mid[0], k_cfft_cta<LOG2N, -1>, CtaFftPlan<LOG2N>::NT, smem) &&
+         kernel_prepare(p->cfg_cfft_mid[1], k_cfft_cta<LOG2N, +1>, CtaFftPlan<LOG2N>::NT, smem);
+}
+
+template <int LOG2N>
+static qtam_status mid_launch(qtam_plan *p, const float2 *in, long long in_stride, float2 *out, long long out_stride,
+                              int count, int dir, float scale, cudaStream_t st, double algo) {
+  const KernelCfg &cfg = p->cfg_cfft_mid[dir < 0 ? 0 : 1];
+  if (!cfg.ready) return QTAM_ERR_CUDA;
+  const float2 *ptw = static_cast<const float2 *>(p->d_ptw_mid);
+  {
+    LaunchScope ls(p, st, K_CFFT_SEQ, algo, 16.0 * (double)count * (double)(1 << LOG2N));
+    if (dir < 0) k_cfft_cta<LOG2N, -1><<<(unsigned)count, CtaFftPlan<LOG2N>::NT, cfg.smem, st>>>(in, in_stride, out, out_stride, ptw, scale);
+    else k_cfft_cta<LOG2N, +1><<<(unsigned)count, CtaFftPlan<LOG2N>::NT, cfg.smem, st>>>(in, in_stride, out, out_stride, ptw, scale);
+  }
+  QTAM_LAUNCH_CHECK();
+  return QTAM_OK;
+}
+
+// The whole long real FFT / inverse FFT of a segment of N = 3 * 2^k samples in ONE CTA (n = N/2 = 3 Np complex
+// points, Np = 2^11 .. 2^13): the three decimated sequences z[3 a + r] are gathered straight from global memory into
+// three shared-memory transforms F_r = DFT_Np; the radix-3 butterfly Z[f] = sum_r w_n^{dir r f} F_r[f mod Np] and the
+// real post-processing of row a1 (k_r2c_post) / the store of row a8 read them from shared memory.  One pass over
+// the data instead of four (split, transforms, butterfly, post-processing).
+struct Strided3In {
+  const float2 *__restrict__ p;
+  __device__ __forceinline__ float2 operator()(int a) const { return p[3 * a]; }
+};
+template <int LOG2NP> constexpr int r3_smem_elems() { return 3 * cta_fft_smem_elems<LOG2NP>(); }
+
+template <int LOG2NP, int DIR>
+__device__ __forceinline__ float2 r3_point(const float2 *s0, const float2 *s1, const float2 *s2, int f,
+                                           const float2 *__restrict__ twN) {
+  // Z[f] = F0[k] + w F1[k] + w^2 F2[k], k = f mod Np, w = e^{DIR 2 pi i f/n} = twN[2 f] (twN[j] = e^{2 pi i j/N})
+  constexpr int NP = 1 << LOG2NP, N = 6 * NP;
+  const int k = f & (NP - 1);
+  float2 w1 = __ldg(twN + (2 * f) % N), w2 = __ldg(twN + (4 * f) % N);
+  if (DIR < 0) { w1.y = -w1.y; w2.y = -w2.y; }
+  return padd(s0[k], padd(pcmul(s1[k], w1), pcmul(s2[k], w2)));
+}
+
+template <int LOG2NP>
+__global__ void __launch_bounds__(CtaFftPlan<LOG2NP>::NT)
+k_r2c3(const float *__restrict__ x, float2 *__restrict__ spec, long long xstride, const float2 *__restrict__ twN,
+       const float2 *__restrict__ ptw) {
+  constexpr int NP = 1 << LOG2NP, NC = 3 * NP, NT = CtaFftPlan<LOG2NP>::NT, SE = cta_fft_smem_elems<LOG2NP>();
+  float2 *s = reinterpret_cast<float2 *>(qtam_long_smem);
+  const float2 *z = reinterpret_cast<const float2 *>(x) + (size_t)blockIdx.x * NC;
+#pragma unroll 1
+  for (int r = 0; r < 3; ++r) {
+    cta_fft_io<LOG2NP, NT, -1, true, false>(s + r * SE, Strided3In{z + r}, CtaFftNone{}, ptw);
+    __syncthreads();
+  }
+  float2 *X = spec + (size_t)blockIdx.x * xstride;
+  for (int f = threadIdx.x; f <= NC / 2; f += NT) {
+    const int g = NC - f;
+    const float2 A = r3_point<LOG2NP, -1>(s, s + SE, s + 2 * SE, f, twN);
+    const float2 B = (f == 0) ? A : r3_point<LOG2NP, -1>(s, s + SE, s + 2 * SE, g, twN);
+    const float2 E = make_float2(0.5f * (A.x + B.x), 0.5f * (A.y - B.y));
+    const float2 D = make_float2(0.5f * (A.x - B.x), 0.5f * (A.y + B.y));
+    float2 w = __ldg(twN + f);                   // e^{+2 pi i f/N}
+    w.y = -w.y;
+    const float2 t = make_float2(w.x * D.x - w.y * D.y, w.x * D.y + w.y * D.x);
+    X[f] = make_float2(E.x + t.y, E.y - t.x);
+    if (g != f) X[g] = make_float2(E.x - t.y, -E.y - t.x);
+  }
+}
+
+template <int LOG2NP>
+__global__ void __launch_bounds__(CtaFftPlan<LOG2NP>::NT)
+k_c2c3(const float2 *__restrict__ spec, long long xstride, const float2 *__restrict__ twN,
+       const float2 *__restrict__ ptw, float *__restrict__ x_out) {
+  constexpr int NP = 1 << LOG2NP, NC = 3 * NP, NT = CtaFftPlan<LOG2NP>::NT, SE = cta_fft_smem_elems<LOG2NP>();
+  float2 *s = reinterpret_cast<float2 *>(qtam_long_smem);
+  const float2 *z = spec + (size_t)blockIdx.x * xstride;
+#pragma unroll 1
+  for (int r = 0; r < 3; ++r) {
+    cta_fft_io<LOG2NP, NT, +1, true, false>(s + r * SE, Strided3In{z + r}, CtaFftNone{}, ptw);
+    __syncthreads();
+  }
+  float2 *out = reinterpret_cast<float2 *>(x_out) + (size_t)blockIdx.x * NC;
+  for (int f = threadIdx.x; f < NC; f += NT) out[f] = r3_point<LOG2NP, +1>(s, s + SE, s + 2 * SE, f, twN);
+}
+
+template <int LOG2NP> static bool r3_prepare(qtam_plan *p) {
+  const size_t smem = sizeof(float2) * (size_t)r3_smem_elems<LOG2NP>();
+  return kernel_prepare(p->cfg_r3[0], k_r2c3<LOG2NP>, CtaFftPlan<LOG2NP>::NT, smem) &&
+         kernel_prepare(p->cfg_r3[1], k_c2c3<LOG2NP>, CtaFftPlan<LOG2NP>::NT, smem);
+}
+
+bool fast_r3_ok(const qtam_plan *p) { return p->cfg_r3[0].ready && p->cfg_r3[1].ready; }
+
+template <int LOG2NP> static qtam_status r3_launch(qtam_plan *p, bool fwd, const void *d_in, void *d_out, int batch,
+                                                   cudaStream_t st) {
+  const float2 *twN = static_cast<const float2 *>(p->d_twN), *ptw = static_cast<const float2 *>(p->d_ptw_mid);
+  const double nbytes = (double)batch * 4.0 * (double)p->hp.N;
+  if (fwd) {
+    LaunchScope ls(p, st, K_R2C_FAST, nbytes, nbytes + (double)batch * 8.0 * (double)p->hp.nb);
+    k_r2c3<LOG2NP><<<(unsigned)batch, CtaFftPlan<LOG2NP>::NT, p->cfg_r3[0].smem, st>>>(
+        static_cast<const float *>(d_in), static_cast<float2 *>(p->d_spec), p->xstride, twN, ptw);
+  } else {
+    LaunchScope ls(p, st, K_C2C_FAST, nbytes, 2.0 * nbytes);
+    k_c2c3<LOG2NP><<<(unsigned)batch, CtaFftPlan<LOG2NP>::NT, p->cfg_r3[1].smem, st>>>(
+        static_cast<const float2 *>(p->d_spec), p->xstride, twN, ptw, static_cast<float *>(d_out));
+  }
+  QTAM_LAUNCH_CHECK();
+  return QTAM_OK;
+}
+
+// fwd: x -> spectrum buffer (rows a1); else: pre-processed spectrum buffer (k_combine_runs) -> x_out (row a8)
+qtam_status fast_r3(qtam_plan *p, bool fwd, const void *d_in, void *d_out, int batch, cudaStream_t st) {
+  switch (p->mid_log2n) {
+    case 11: return r3_launch<11>(p, fwd, d_in, d_out, batch, st);
+    case 12: return r3_launch<12>(p, fwd, d_in, d_out, batch, st);
+    case 13: return r3_launch<13>(p, fwd, d_in, d_out, batch, st);
+    default: return QTAM_ERR_UNSUPPORTED;
+  }
+}
+
+bool fast_cfft_mid_ok(const qtam_plan *p, int log2n) { return p->d_ptw_mid != nullptr && log2n == p->mid_log2n; }
+
+qtam_status fast_cfft_mid(qtam_plan *p, const void *in, long long in_stride, void *out, long long out_stride,
+                          int log2n, int count, int dir, float scale, cudaStream_t st, double algo) {
+  const float2 *i = static_cast<const float2 *>(in);
+  float2 *o = static_cast<float2 *>(out);
+  switch (log2n) {
+    case 11: return mid_launch<11>(p, i, in_stride, o, out_stride, count, dir, scale, st, algo);
+    case 12: return mid_launch<12>(p, i, in_stride, o, out_stride, count, dir, scale, st, algo);
+    case 13: return mid_launch<13>(p, i, in_stride, o, out_stride, count, dir, scale, st, algo);
+    case 14: return mid_launch<14>(p, i, in_stride, o, out_stride, count, dir, scale, st, algo);
+    default: return QTAM_ERR_UNSUPPORTED;
+  }
+}
+
 bool fast_cfft_long_ok(const qtam_plan *p, int log2n) {
   return p->d_ptw_long != nullptr && log2n > kLongLog2N2 && log2n <= kLongLog2N2 + 5;
 }
@@ -115,6 +267,28 @@ qtam_status fast_cfft_long(qtam_plan *p, const void *in, long long in_stride, vo
 qtam_status build_long_fft(qtam_plan *p) {
   int lnc = 0;
   while ((int64_t(1) << lnc) < p->sub_n) ++lnc;    // log2 of the power-of-two complex FFT behind the long transform
+  if (p->esz == 4 && !p->n_pow2 && lnc >= 11 && lnc <= 14) {
+    // N = 3 * 2^k: the three transforms of N/6 points per segment run one CTA each
+    bool ok = false;
+    switch (lnc) {
+      case 11: ok = mid_prepare<11>(p); break;
+      case 12: ok = mid_prepare<12>(p); break;
+      case 13: ok = mid_prepare<13>(p); break;
+      default: ok = mid_prepare<14>(p); break;
+    }
+    if (!ok) return QTAM_ERR_CUDA;
+    p->mid_log2n = lnc;
+    // ... or, when three of them fit one CTA's shared memory, the whole long transform does
+    ok = true;
+    switch (lnc) {
+      case 11: ok = r3_prepare<11>(p); break;
+      case 12: ok = r3_prepare<12>(p); break;
+      case 13: ok = r3_prepare<13>(p); break;
+      default: break;
+    }
+    if (!ok) return QTAM_ERR_CUDA;
+    return QTAM_OK;
+  }
   if (p->esz != 4 || lnc <= kLongLog2N2 || lnc > kLongLog2N2 + 5) return QTAM_OK;
   std::vector<float> t;
   fill_cta_fft_tables<kLongLog2N2, CtaFftPlan<kLongLog2N2>::NT>(t);
