@@ -1,4 +1,4 @@
-// fftreg.cuh -- in-register complex FFTs of size 2..32 on float2 for sm_100a.
+// fftreg.cuh -- in-register complex FFTs of size 2..64 on float2 for sm_100a.
 // Complex add/sub go through Blackwell's packed add.f32x2 / sub.f32x2 (SASS FADD2: one issue slot
 // for both halves; a multiply by +-i folds into the FADD2 operand modifiers).  Twiddle constants
 // are compile-time, so the multiplies become FMUL/FFMA with immediates.
@@ -44,33 +44,35 @@ __device__ __forceinline__ float2 pcmul4(float2 a, float4 w) {
 }
 __device__ __forceinline__ float2 pscale(float2 a, float s) { return pmul(a, make_float2(s, s)); }
 
-// cos / sin of 2 pi k/32, exact on the axes
-__host__ __device__ constexpr float cos32(int k) {
-  constexpr float c[9] = {1.0f, 9.807852804e-01f, 9.238795325e-01f, 8.314696123e-01f, 7.071067812e-01f,
-                          5.555702330e-01f, 3.826834324e-01f, 1.950903220e-01f, 0.0f};
-  k &= 31;
-  return k <= 8 ? c[k] : k <= 16 ? -c[16 - k] : k <= 24 ? -c[k - 16] : c[32 - k];
+// cos / sin of 2 pi k/64, exact on the axes
+__host__ __device__ constexpr float cos64(int k) {
+  constexpr float c[17] = {1.0f, 9.951847267e-01f, 9.807852804e-01f, 9.569403357e-01f, 9.238795325e-01f,
+                           8.819212643e-01f, 8.314696123e-01f, 7.730104534e-01f, 7.071067812e-01f,
+                           6.343932842e-01f, 5.555702330e-01f, 4.713967368e-01f, 3.826834324e-01f,
+                           2.902846773e-01f, 1.950903220e-01f, 9.801714033e-02f, 0.0f};
+  k &= 63;
+  return k <= 16 ? c[k] : k <= 32 ? -c[32 - k] : k <= 48 ? -c[k - 32] : c[64 - k];
 }
-__host__ __device__ constexpr float sin32(int k) { return cos32(k - 8); }
+__host__ __device__ constexpr float sin64(int k) { return cos64(k - 16); }
 
-// o * e^{DIR 2 pi i Q/R} with compile-time Q, R (R | 32)
+// o * e^{DIR 2 pi i Q/R} with compile-time Q, R (R | 64)
 template <int Q, int R, int DIR>
 __device__ __forceinline__ float2 twmul(float2 o) {
-  constexpr int k = (Q * (32 / R)) & 31;
+  constexpr int k = (Q * (64 / R)) & 63;
   if constexpr (k == 0) return o;
-  else if constexpr (k == 8) return DIR > 0 ? make_float2(-o.y, o.x) : make_float2(o.y, -o.x);
-  else if constexpr (k == 16) return make_float2(-o.x, -o.y);
-  else if constexpr (k == 24) return DIR > 0 ? make_float2(o.y, -o.x) : make_float2(-o.y, o.x);
+  else if constexpr (k == 16) return DIR > 0 ? make_float2(-o.y, o.x) : make_float2(o.y, -o.x);
+  else if constexpr (k == 32) return make_float2(-o.x, -o.y);
+  else if constexpr (k == 48) return DIR > 0 ? make_float2(o.y, -o.x) : make_float2(-o.y, o.x);
   else {
     // o (c + i s) = o (c, c) + (-o.y, o.x) (s, s): two packed instructions -- the swap and the sign of the
     // second factor fold into FMUL2's operand modifiers, (c, c) and (s, s) are scalar-broadcast operands
-    constexpr float c = cos32(k);
-    constexpr float s = DIR > 0 ? sin32(k) : -sin32(k);
+    constexpr float c = cos64(k);
+    constexpr float s = DIR > 0 ? sin64(k) : -sin64(k);
     return pfma(o, make_float2(c, c), pmul(make_float2(-o.y, o.x), make_float2(s, s)));
   }
 }
 
-// In-register FFT of size R (power of two <= 32), natural order in and out, on v[0..R).
+// In-register FFT of size R (power of two <= 64), natural order in and out, on v[0..R).
 // out[n] = sum_j v[j] e^{DIR 2 pi i jn/R}.  Recursive decimation in time; everything unrolls.
 template <int R, int DIR> struct RegFFT {
   template <int Q> static __device__ __forceinline__ void combine(float2 (&v)[R], const float2 (&e)[R / 2],

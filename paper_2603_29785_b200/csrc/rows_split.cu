@@ -97,17 +97,6 @@ __device__ __forceinline__ float2 ldg_cg_f2(const float2 *p, bool ok) {
   return v;
 }
 
-// cos / sin of 2 pi k/64
-__host__ __device__ constexpr float cos64(int k) {
-  constexpr float c[17] = {1.0f, 9.951847267e-01f, 9.807852804e-01f, 9.569403357e-01f, 9.238795325e-01f,
-                           8.819212643e-01f, 8.314696123e-01f, 7.730104534e-01f, 7.071067812e-01f,
-                           6.343932842e-01f, 5.555702330e-01f, 4.713967368e-01f, 3.826834324e-01f,
-                           2.902846773e-01f, 1.950903220e-01f, 9.801714033e-02f, 0.0f};
-  k &= 63;
-  return k <= 16 ? c[k] : k <= 32 ? -c[32 - k] : k <= 48 ? -c[k - 32] : c[64 - k];
-}
-__host__ __device__ constexpr float sin64(int k) { return cos64(k - 16); }
-
 // pass-2 twiddles of one thread: w^{k r}, r = 4 a + b, from the table rows (see kSpTwRows) and one product each
 template <int DIR>
 __device__ __forceinline__ void sp_twiddle32(float2 (&v)[32], const float2 *tw2, int k) {
