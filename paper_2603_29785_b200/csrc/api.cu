@@ -54,7 +54,7 @@ void free_plan(qtam_plan *p) {
   for (int c = 0; c < kCtaClasses; ++c) { cudaFree(p->d_cta_lead[c]); cudaFree(p->d_ptw_rows[c]); cudaFree(p->d_cta_groups[c]); cudaFree(p->d_cta_mem[c]); }
   cudaFree(p->d_sp_tw2);
   for (int c = 0; c < kClClasses; ++c) { cudaFree(p->d_sp_ftw[c]); cudaFree(p->d_sp_scratch[c]); cudaFree(p->d_sp_ctl[c]); cudaFree(p->d_sp_order[c]); cudaFree(p->d_sp_wt[c]); cudaFree(p->d_sp_wtoff[c]); }
-  cudaFree(p->d_sp_xt); cudaFree(p->d_ptw_mid);
+  cudaFree(p->d_sp_xt); cudaFree(p->d_ptw_mid); cudaFree(p->d_tw_2k);
   for (int c = 0; c < kClClasses; ++c) { cudaFree(p->d_cl_lead[c]); cudaFree(p->d_cl_mem[c]); cudaFree(p->d_cl_groups[c]); cudaFree(p->d_cl_ftw[c]); }
   cudaFree(p->d_cl_ptw);
   cudaFree(p->d_runs); cudaFree(p->d_run_ptr); cudaFree(p->d_run_idx);
@@ -410,6 +410,7 @@ qtam_status qtam_plan_create(qtam_plan **out, double fs, int64_t N, const double
   // the inverse's partial sums, in summation order: tiles, CTA groups, cluster groups (then the band slots)
   if (s == QTAM_OK && p->fast_rows) s = build_inv_tiled(p);
   if (s == QTAM_OK && p->fast_rows) s = build_rows_cta(p);
+  if (s == QTAM_OK && p->fast_rows) s = build_rows_2k(p);
   if (s == QTAM_OK && p->fast_rows) s = build_rows_cluster(p);
   if (s == QTAM_OK && p->fast_rows) s = build_runs(p);
   if (s == QTAM_OK) s = prepare_fast(p);

@@ -173,6 +173,8 @@ struct qtam_plan {
   int n_cta_rows[qtam::kCtaClasses] = {}, n_cta_groups[qtam::kCtaClasses] = {};
   double cta_sumM[qtam::kCtaClasses] = {}, cta_sumL[qtam::kCtaClasses] = {};
   void *d_ptw_rows[qtam::kCtaClasses] = {};             // pass tables per class
+  bool rows2k_ok = false;                               // forward rows of 2^11 points run one warp each (rows_2k.cu)
+  void *d_tw_2k = nullptr;
   // cluster-level rows (rows_cluster.cu), one class per transform length 2^14 .. 2^17
   bool cl_rows = false;
   qtam::ClLeader *d_cl_lead[qtam::kClClasses] = {};
@@ -205,7 +207,7 @@ struct qtam_plan {
 
   // launch configurations fixed at plan creation (see KernelCfg)
   qtam::KernelCfg cfg_r2c, cfg_rows_fwd, cfg_rows_thr, cfg_rows_inv, cfg_tiles, cfg_combine,
-      cfg_rows_cta[qtam::kCtaClasses][2], cfg_rows_cl[qtam::kClClasses][2], cfg_rows_sp[qtam::kClClasses][2], cfg_c2c, cfg_cfft_mid[2], cfg_r3[2];
+      cfg_rows_cta[qtam::kCtaClasses][2], cfg_rows_cl[qtam::kClClasses][2], cfg_rows_sp[qtam::kClClasses][2], cfg_c2c, cfg_cfft_mid[2], cfg_r3[2], cfg_rows_2k;
 
   // output-length options (length.cu): the plan's uniform length n, the standard one, e^{2 pi i m/n} for both
   long long len_n = 0, len_std = 0;
@@ -330,6 +332,9 @@ void build_leaders_and_groups(qtam_plan *p, const std::vector<int> &rows_in, int
 qtam_status build_rows_cta(qtam_plan *p);
 qtam_status cta_forward_rows(qtam_plan *p, int batch, void *d_coef, Fork &fk);
 qtam_status cta_inverse_rows(qtam_plan *p, const void *d_coef, int batch, int plane, Fork &fk);
+// rows_2k.cu
+qtam_status build_rows_2k(qtam_plan *p);
+qtam_status rows_2k_forward(qtam_plan *p, int batch, void *d_coef, cudaStream_t st);
 // rows_cluster.cu
 qtam_status build_rows_cluster(qtam_plan *p);
 qtam_status cluster_forward_rows(qtam_plan *p, int batch, void *d_coef, Fork &fk);

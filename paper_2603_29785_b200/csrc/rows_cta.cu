@@ -278,7 +278,9 @@ static qtam_status rows_cta_all(qtam_plan *p, int batch, void *d_coef, int plane
   qtam_status s = QTAM_OK;
   if (p->n_cta_rows[2]) s = rows_cta_launch<13, FORWARD>(p, 2, batch, d_coef, plane, fk.next());
   if (s == QTAM_OK && p->n_cta_rows[1]) s = rows_cta_launch<12, FORWARD>(p, 1, batch, d_coef, plane, fk.next());
-  if (s == QTAM_OK && p->n_cta_rows[0]) s = rows_cta_launch<11, FORWARD>(p, 0, batch, d_coef, plane, fk.next());
+  if (s == QTAM_OK && p->n_cta_rows[0])
+    s = FORWARD && p->rows2k_ok ? rows_2k_forward(p, batch, d_coef, fk.next())
+                                : rows_cta_launch<11, FORWARD>(p, 0, batch, d_coef, plane, fk.next());
   return s;
 }
 
