@@ -163,6 +163,7 @@ struct qtam_plan {
   qtam::ThrTask *d_thr_tasks = nullptr;
   int *d_thr_offs = nullptr;      // coefficient offsets of the tasks' rows
   int n_thr_tasks = 0;
+  int thr_first[qtam::kThrFastLog2Max + 1] = {}, thr_count[qtam::kThrFastLog2Max + 1] = {};   // tasks per row length
   bool thr_has_big = false;       // some row is longer than 2^kThrFastLog2Max points (generic kernel)
 
   // CTA-level rows (rows_cta.cu), one class per transform length 2^11 .. 2^13

@@ -25,8 +25,10 @@ qtam_status build_thr_fast(qtam_plan *p) {
   std::vector<ThrTask> tasks;
   // offsets are kept as 32-bit integers: a plan with more coefficients per segment stays on the generic kernel
   const bool fits = hp.ctot < (int64_t(1) << 31);
+  for (int lm = 0; lm <= kThrFastLog2Max; ++lm) { p->thr_first[lm] = 0; p->thr_count[lm] = 0; }
   for (int lm = kThrFastLog2Max; fits && lm >= 2; --lm) {
     const int M = 1 << lm, G = M >= 32 ? M / 32 : 1, per = 32 / G;
+    p->thr_first[lm] = (int)tasks.size();
     std::vector<int> mine;
     for (const HostRow &h : hp.rows) if (h.M == M) mine.push_back((int)h.offset);
     for (size_t i = 0; i < mine.size(); i += (size_t)per) {
@@ -35,6 +37,7 @@ qtam_status build_thr_fast(qtam_plan *p) {
       for (int r = 0; r < t.nrows; ++r) offs.push_back(mine[i + (size_t)r]);
       tasks.push_back(t);
     }
+    p->thr_count[lm] = (int)tasks.size() - p->thr_first[lm];
   }
   p->n_thr_tasks = (int)tasks.size();
   p->thr_has_big = false;
@@ -73,7 +76,10 @@ __device__ __forceinline__ void thr_group(C2<T> *__restrict__ Y, int G, int t, T
   }
 }
 
-template <typename T, int NW>
+// One kernel per row length: the select of one length is a few thousand fully unrolled instructions (more in double
+// precision), and a kernel that switched between all lengths ran out of instruction cache (ncu: "no instruction" was
+// the first stall reason of the double-precision kernel, 424 us at config 5).
+template <typename T, int NW, int LM>
 __global__ void __launch_bounds__(NW * 32)
 k_threshold_fast(const ThrTask *__restrict__ tasks, int n_tasks, const int *__restrict__ offs,
                  C2<T> *__restrict__ coef, long long ctot, int batch, T kappa) {
@@ -82,23 +88,13 @@ k_threshold_fast(const ThrTask *__restrict__ tasks, int n_tasks, const int *__re
   if (item >= (long long)n_tasks * batch) return;
   const int seg = (int)(item / n_tasks);
   const ThrTask tk = tasks[item - (long long)seg * n_tasks];
-  const int M = 1 << tk.log2M;
-  const int G = M >= 32 ? M >> 5 : 1;
+  constexpr int M = 1 << LM;
+  constexpr int G = M >= 32 ? M >> 5 : 1;
   const int t = lane & (G - 1), rw = lane / G;
   C2<T> *Y = nullptr;
   if (rw < tk.nrows) Y = coef + (size_t)seg * ctot + offs[tk.row0 + rw];
-  switch (tk.log2M) {
-    case 2: thr_group<T, 4>(Y, 1, 0, kappa); break;
-    case 3: thr_group<T, 8>(Y, 1, 0, kappa); break;
-    case 4: thr_group<T, 16>(Y, 1, 0, kappa); break;
-    // (the lanes-per-row count as a literal: the shuffle loops of the select unroll)
-    case 5: thr_group<T, 32>(Y, 1, t, kappa); break;
-    case 6: thr_group<T, 32>(Y, 2, t, kappa); break;
-    case 7: thr_group<T, 32>(Y, 4, t, kappa); break;
-    case 8: thr_group<T, 32>(Y, 8, t, kappa); break;
-    case 9: thr_group<T, 32>(Y, 16, t, kappa); break;
-    default: thr_group<T, 32>(Y, 32, t, kappa); break;
-  }
+  if constexpr (LM < 5) thr_group<T, M>(Y, 1, 0, kappa);           // rows of 4, 8, 16 points: one lane each
+  else thr_group<T, 32>(Y, G, t, kappa);                           // (the lanes-per-row count is a literal)
 }
 
 template <typename T>
@@ -111,8 +107,19 @@ static qtam_status thr_launch(qtam_plan *p, void *d_coef, int batch, double kapp
   {
     // a separate threshold pass moves no compulsory bytes (zero extra when fused)
     LaunchScope ls(p, st, K_THRESHOLD_FAST, 0.0, 2.0 * sizeof(C2<T>) * (double)batch * elems);
-    k_threshold_fast<T, NW><<<(unsigned)((total + NW - 1) / NW), NW * 32, 0, st>>>(
-        p->d_thr_tasks, p->n_thr_tasks, p->d_thr_offs, static_cast<C2<T> *>(d_coef), p->hp.ctot, batch, (T)kappa);
+    C2<T> *Y = static_cast<C2<T> *>(d_coef);
+    int launched = 0;
+#define QTAM_THR_LM(LM)                                                                                        \
+    if (p->thr_count[LM] > 0) {                                                                                \
+      const long long n = (long long)p->thr_count[LM] * batch;                                                 \
+      k_threshold_fast<T, NW, LM><<<(unsigned)((n + NW - 1) / NW), NW * 32, 0, st>>>(                          \
+          p->d_thr_tasks + p->thr_first[LM], p->thr_count[LM], p->d_thr_offs, Y, p->hp.ctot, batch, (T)kappa); \
+      ++launched;                                                                                              \
+    }
+    QTAM_THR_LM(10) QTAM_THR_LM(9) QTAM_THR_LM(8) QTAM_THR_LM(7) QTAM_THR_LM(6) QTAM_THR_LM(5)
+    QTAM_THR_LM(4) QTAM_THR_LM(3) QTAM_THR_LM(2)
+#undef QTAM_THR_LM
+    if (launched > 1) p->last_launches += launched - 1;      // (the scope counted one)
   }
   QTAM_LAUNCH_CHECK();
   return QTAM_OK;
