@@ -496,7 +496,6 @@ qtam_status qtam_forward(qtam_plan *p, const void *d_x, int batch, void *d_coef,
   if (batch == 0) return QTAM_OK;
   cudaStream_t st = static_cast<cudaStream_t>(stream);
   qtam_status s = p->fast_long ? fast_r2c(p, d_x, batch, st) : generic_r2c(p, d_x, batch, st);
-  if (s == QTAM_OK) s = split_spectrum(p, batch, st);
   if (s != QTAM_OK) return s;
   // the row launches are independent of each other (they read the spectrum and write disjoint coefficients):
   // the longest rows first, every launch on a stream of its own, joined before the call returns to the caller's
@@ -519,8 +518,7 @@ qtam_status qtam_forward_threshold(qtam_plan *p, const void *d_x, int batch, dou
   if (p->fast_rows && p->esz == 4) {
     // the threshold rides in the epilogue of the row kernel for every row of at most 1024 points
       qtam_status s = p->fast_long ? fast_r2c(p, d_x, batch, st) : generic_r2c(p, d_x, batch, st);
-    if (s == QTAM_OK) s = split_spectrum(p, batch, st);
-    if (s != QTAM_OK) return s;
+      if (s != QTAM_OK) return s;
     bool fused = false;
     s = fast_forward_rows_threshold(p, batch, d_coef, (float)kappa, st, &fused);
     if (s != QTAM_OK) return s;

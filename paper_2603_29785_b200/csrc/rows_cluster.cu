@@ -413,12 +413,25 @@ template <bool FWD>
 static qtam_status cl_all(qtam_plan *p, int batch, void *d_coef, int plane, Fork &fk) {
   qtam_status s = QTAM_OK;
   if (p->n_cl_lead[3]) s = cl_launch<kClLog2P, 3, FWD>(p, 3, batch, d_coef, plane, fk.next());
-  if (s == QTAM_OK && p->n_cl_lead[2])
-    s = p->sp_ok[2] ? split_rows(p, 2, FWD, batch, d_coef, plane, fk.next())
-                    : cl_launch<kClLog2P, 2, FWD>(p, 2, batch, d_coef, plane, fk.next());
-  if (s == QTAM_OK && p->n_cl_lead[1])
-    s = p->sp_ok[1] ? split_rows(p, 1, FWD, batch, d_coef, plane, fk.next())
-                    : cl_launch<kClLog2P, 1, FWD>(p, 1, batch, d_coef, plane, fk.next());
+  // the dataflow classes share one stream: the forward's residue-sorted copy of the spectrum (k_spec_residues) goes
+  // first on it, so that only they wait for it -- every other row kernel of the call starts right after the long FFT
+  cudaStream_t sx = nullptr;
+  bool have_sx = false;
+  auto split_stream = [&]() -> cudaStream_t {
+    if (!have_sx) {
+      sx = fk.next(); have_sx = true;
+      if (FWD && s == QTAM_OK) s = split_spectrum(p, batch, sx);
+    }
+    return sx;
+  };
+  if (s == QTAM_OK && p->n_cl_lead[2]) {
+    if (p->sp_ok[2]) { cudaStream_t t = split_stream(); if (s == QTAM_OK) s = split_rows(p, 2, FWD, batch, d_coef, plane, t); }
+    else s = cl_launch<kClLog2P, 2, FWD>(p, 2, batch, d_coef, plane, fk.next());
+  }
+  if (s == QTAM_OK && p->n_cl_lead[1]) {
+    if (p->sp_ok[1]) { cudaStream_t t = split_stream(); if (s == QTAM_OK) s = split_rows(p, 1, FWD, batch, d_coef, plane, t); }
+    else s = cl_launch<kClLog2P, 1, FWD>(p, 1, batch, d_coef, plane, fk.next());
+  }
   if (s == QTAM_OK && p->n_cl_lead[0]) s = cl_launch<kClLog2P, 0, FWD>(p, 0, batch, d_coef, plane, fk.next());
   return s;
 }
