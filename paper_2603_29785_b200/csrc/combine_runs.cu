@@ -26,9 +26,11 @@ __global__ void __launch_bounds__(kRunBlock)
 k_combine_runs(const int4 *__restrict__ runs, const int *__restrict__ ptr, const int *__restrict__ idx,
                const float2 *__restrict__ part, long long part_stride, const float2 *__restrict__ band,
                long long sumL, const float *__restrict__ invP, int Nc, int plane, const float2 *__restrict__ tw,
-               int tw_shift, float2 *__restrict__ spec, long long xstride) {
+               int tw_shift, float2 *__restrict__ spec, long long xstride, float2 *__restrict__ rt,
+               long long rt_stride, int rt_len, int rt_pad) {
   __shared__ int4 s_runs[kRunChunk];
   __shared__ float2 s_xch[2][kRunBlock];
+  __shared__ unsigned char s_ok[2][kRunBlock];
   const int b = blockIdx.x, seg = blockIdx.y;
   const int f = b * kRunBlock + threadIdx.x;
   const int g = Nc - f;
@@ -86,18 +88,35 @@ k_combine_runs(const int4 *__restrict__ runs, const int *__restrict__ ptr, const
   __syncthreads();
   A = padd(A, s_xch[0][threadIdx.x]);
   B = padd(B, s_xch[1][threadIdx.x]);
-  if (f > Nc / 2) return;
-  A = pscale(A, __ldg(invP + f));
-  B = pscale(B, __ldg(invP + g));
-  if (f == 0) { A.y = 0.f; B.y = 0.f; }
-  const float h = 0.5f / (float)Nc;
-  const float2 E = make_float2(h * (A.x + B.x), h * (A.y - B.y));
-  const float2 D = make_float2(h * (A.x - B.x), h * (A.y + B.y));
-  const float2 w = __ldg(tw + ((size_t)f << tw_shift));      // e^{+2 pi i f/N}
-  const float2 O = make_float2(D.x * w.x - D.y * w.y, D.x * w.y + D.y * w.x);
-  float2 *S = spec + (size_t)seg * xstride;
-  S[f] = make_float2(E.x - O.y, E.y + O.x);                          // E + i O
-  if (g != f && f != 0) S[g] = make_float2(E.x + O.y, -E.y + O.x);   // conj(E) + i conj(O)
+  const bool okf = f <= Nc / 2, okg = okf && g != f && f != 0;
+  float2 vf = make_float2(0.f, 0.f), vg = vf;
+  if (okf) {
+    A = pscale(A, __ldg(invP + f));
+    B = pscale(B, __ldg(invP + g));
+    if (f == 0) { A.y = 0.f; B.y = 0.f; }
+    const float h = 0.5f / (float)Nc;
+    const float2 E = make_float2(h * (A.x + B.x), h * (A.y - B.y));
+    const float2 D = make_float2(h * (A.x - B.x), h * (A.y + B.y));
+    const float2 w = __ldg(tw + ((size_t)f << tw_shift));      // e^{+2 pi i f/N}
+    const float2 O = make_float2(D.x * w.x - D.y * w.y, D.x * w.y + D.y * w.x);
+    vf = make_float2(E.x - O.y, E.y + O.x);                    // E + i O
+    vg = make_float2(E.x + O.y, -E.y + O.x);                   // conj(E) + i conj(O)
+  }
+  if (rt == nullptr) {
+    float2 *S = spec + (size_t)seg * xstride;
+    if (okf) S[f] = vf;
+    if (okg) S[g] = vg;
+    return;
+  }
+  // the spectrum in residue order for the long inverse FFT of long_fft.cu (bin x at [x mod 64][pad + x div 64]):
+  // handed to the threads of the residue-ordered map, which write 4 consecutive elements of a residue each
+  __syncthreads();
+  s_xch[0][threadIdx.x] = vf; s_ok[0][threadIdx.x] = okf;
+  s_xch[1][threadIdx.x] = vg; s_ok[1][threadIdx.x] = okg;
+  __syncthreads();
+  float2 *R = rt + (size_t)seg * rt_stride + rt_pad;
+  if (s_ok[0][tq]) R[(size_t)(tf & 63) * rt_len + (tf >> 6)] = s_xch[0][tq];
+  if (s_ok[1][kRunBlock - 1 - tq]) R[(size_t)(tg & 63) * rt_len + (tg >> 6)] = s_xch[1][kRunBlock - 1 - tq];
 }
 
 // Run lists, the band-slot runs of the rows that no tile or group covers, and the partial-sum buffer (the tiles'
@@ -157,13 +176,15 @@ qtam_status combine_runs(qtam_plan *p, int batch, int plane, cudaStream_t st) {
   double run_bins = 0;
   for (const HostRun &r : p->runs) run_bins += (double)r.nb;
   dim3 g((unsigned)p->n_run_blocks, (unsigned)batch);
+  const bool res = long_residues_ok(p);      // the long inverse FFT takes the spectrum in residue order
   {
     LaunchScope ls(p, st, K_COMBINE_RUNS, 0.0, (double)batch * 8.0 * (run_bins + (double)p->hp.nb));
     k_combine_runs<<<g, kRunBlock, 0, st>>>(
         p->d_runs, p->d_run_ptr, p->d_run_idx, static_cast<const float2 *>(p->d_part), p->part_stride,
         static_cast<const float2 *>(p->d_band), p->hp.sumL,
         static_cast<const float *>(p->d_invP) + (size_t)(plane + 1) * (size_t)p->hp.nb, Nc, plane,
-        static_cast<const float2 *>(p->d_twN), tw_shift, static_cast<float2 *>(p->d_spec), p->xstride);
+        static_cast<const float2 *>(p->d_twN), tw_shift, static_cast<float2 *>(p->d_spec), p->xstride,
+        res ? static_cast<float2 *>(p->d_sp_xt) : nullptr, 64LL * p->sp_xt_len, p->sp_xt_len, p->sp_xt_pad);
   }
   QTAM_LAUNCH_CHECK();
   return QTAM_OK;

@@ -197,7 +197,8 @@ struct qtam_plan {
   int sp_nmem[qtam::kClClasses] = {};
   void *d_sp_wt[qtam::kClClasses] = {}, *d_sp_wtoff[qtam::kClClasses] = {};   // windows by residue, first element per leader
   void *d_sp_xt = nullptr;                              // spectrum by residue [max_batch][64][sp_xt_len]
-  int sp_xt_len = 0;
+  int sp_xt_len = 0, sp_xt_pad = 0;
+  bool sp_xt_fresh = false;                             // the long FFT has just written d_sp_xt (forward)
   // run-based combine (combine_runs.cu): the inverse of every float plan that is not on the tiled path
   bool use_runs = false;
   std::vector<qtam::HostRun> runs;                      // in summation order (tiles, CTA groups, cluster groups, band slots)
@@ -311,6 +312,9 @@ qtam_status fast_c2c_out(qtam_plan *p, int batch, void *d_x_out, cudaStream_t st
 // long_fft.cu
 qtam_status build_long_fft(qtam_plan *p);
 bool fast_cfft_long_ok(const qtam_plan *p, int log2n);
+bool long_residues_ok(const qtam_plan *p);
+qtam_status long_forward_residues(qtam_plan *p, const void *d_x, int batch, cudaStream_t st);
+qtam_status long_inverse_residues(qtam_plan *p, void *d_x_out, int batch, cudaStream_t st);
 bool fast_cfft_mid_ok(const qtam_plan *p, int log2n);
 bool fast_r3_ok(const qtam_plan *p);
 qtam_status fast_r3(qtam_plan *p, bool fwd, const void *d_in, void *d_out, int batch, cudaStream_t st);

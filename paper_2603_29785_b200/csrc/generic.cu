@@ -571,6 +571,12 @@ static qtam_status cfft_any(qtam_plan *p, const C2<T> *in, long long in_stride, 
 template <typename T>
 static qtam_status r2c_t(qtam_plan *p, const void *d_x, int batch, cudaStream_t st) {
   if (sizeof(T) == 4 && !p->n_pow2 && fast_r3_ok(p)) return fast_r3(p, true, d_x, nullptr, batch, st);
+  p->sp_xt_fresh = false;
+  if (sizeof(T) == 4 && long_residues_ok(p)) {
+    const qtam_status sr = long_forward_residues(p, d_x, batch, st);
+    p->sp_xt_fresh = sr == QTAM_OK;
+    return sr;
+  }
   const int Nc = (int)(p->hp.N / 2);
   C2<T> *spec = static_cast<C2<T> *>(p->d_spec);
   C2<T> *ws = static_cast<C2<T> *>(p->d_ws);
@@ -692,6 +698,7 @@ static qtam_status c2r_t(qtam_plan *p, int batch, void *d_x_out, cudaStream_t st
 // the complex FFT alone, for a spectrum buffer that already holds the pre-processed Z (k_combine_runs)
 qtam_status generic_c2c_out(qtam_plan *p, int batch, void *d_x_out, cudaStream_t st) {
   if (!p->n_pow2 && fast_r3_ok(p)) return fast_r3(p, false, nullptr, d_x_out, batch, st);
+  if (long_residues_ok(p)) return long_inverse_residues(p, d_x_out, batch, st);
   const int Nc = (int)(p->hp.N / 2);
   return cfft_any<float>(p, static_cast<const float2 *>(p->d_spec), p->xstride, static_cast<float2 *>(d_x_out), Nc,
                          static_cast<float2 *>(p->d_ws), p->hp.N, Nc, batch, +1, 1.f, st, 0.0,

@@ -94,6 +94,191 @@ static qtam_status long_launch(qtam_plan *p, const float2 *in, long long in_stri
   return QTAM_OK;
 }
 
+// --------------------------------------------------------------------------------------------------
+// The long transform with the spectrum in RESIDUE ORDER (N = 2^20: n = 2^19 = 64 * 2^13), for plans whose long rows
+// read the spectrum sorted by residue mod 64 anyway (rows_split.cu: bin f at [f mod 64][f div 64]).  With
+// f = f1 + 64 f2 and n = 2^13 n1 + n2 the two passes are contiguous on both sides:
+//   forward  k_long_a (radix 64 over n1, twiddle)  ->  k_long_b_res: Z[f1 + 64 f2] = FFT over n2, written to
+//            row f1 of the residue-sorted buffer  ->  k_post_residues: the real post-processing in that buffer, in
+//            place, and the spectrum in bin order for the other row kernels through shared-memory tiles
+//   inverse  k_combine_runs writes the pre-processed spectrum in residue order  ->  k_long_b_res (FFT over f2 for
+//            every f1)  ->  k_long_a_pre (twiddle, radix 64 over f1) straight to x_out
+// instead of a second pass whose output has stride 64 (8 bytes every 512).
+// --------------------------------------------------------------------------------------------------
+template <int DIR>
+__global__ void __launch_bounds__(CtaFftPlan<kLongLog2N2>::NT)
+k_long_b_res(const float2 *__restrict__ in, long long in_seg, long long in_row, float2 *__restrict__ out,
+             long long out_seg, long long out_row, const float2 *__restrict__ ptw) {
+  constexpr int NT = CtaFftPlan<kLongLog2N2>::NT;
+  float2 *s = reinterpret_cast<float2 *>(qtam_long_smem);
+  cta_fft<kLongLog2N2, NT, DIR, true, true>(s, in + (size_t)blockIdx.y * in_seg + (size_t)blockIdx.x * in_row,
+                                            out + (size_t)blockIdx.y * out_seg + (size_t)blockIdx.x * out_row, ptw, 1.f);
+}
+
+// x[N2 n1 + n2] = sum_f1 w_R^{dir f1 n1} (w_n^{dir f1 n2} A[f1][n2]): the twiddle BEFORE the radix-R transform
+template <int LOG2R, int DIR>
+__global__ void __launch_bounds__(256)
+k_long_a_pre(const float2 *__restrict__ in, long long in_stride, float2 *__restrict__ out, long long out_stride,
+             const float2 *__restrict__ tw, int tw_shift) {
+  constexpr int R = 1 << LOG2R, N2 = 1 << kLongLog2N2;
+  const int j2 = blockIdx.x * 256 + threadIdx.x;
+  const float2 *src = in + (size_t)blockIdx.y * in_stride + j2;
+  float2 v[R];
+#pragma unroll
+  for (int j1 = 0; j1 < R; ++j1) v[j1] = __ldcs(src + (size_t)j1 * N2);
+  float2 pw[R];
+  pw[0] = make_float2(1.f, 0.f);
+#pragma unroll
+  for (int b = 0; b < LOG2R; ++b) {
+    float2 w = __ldg(tw + ((size_t)(j2 << b) << tw_shift));
+    if (DIR < 0) w.y = -w.y;
+    pw[1 << b] = w;
+  }
+#pragma unroll
+  for (int k = 3; k < R; ++k)
+    if (k & (k - 1)) pw[k] = pcmul(pw[k & (k - 1)], pw[k & -k]);
+#pragma unroll
+  for (int k = 1; k < R; ++k) v[k] = pcmul(v[k], pw[k]);
+  RegFFT<R, DIR>::run(v);
+  float2 *dst = out + (size_t)blockIdx.y * out_stride + j2;
+#pragma unroll
+  for (int n1 = 0; n1 < R; ++n1) __stcs(dst + (size_t)n1 * N2, v[n1]);
+}
+
+// Real post-processing (k_r2c_post, row a1) on the residue-sorted half-length transform, in place, plus the spectrum
+// in bin order.  A CTA takes the 4096 bins f = 4096 t .. (64 of every residue) and their mirrors g = Nc - f (bins
+// G0 + 1 .. G0 + 4096, G0 = Nc - 4096 t - 4096): both tiles are read in runs of 64 elements per residue, paired in
+// shared memory (static: two tiles), and written back to the same places and, in bin order, to `spec`.  rt: [64][rt_len] per segment,
+// bin f at [f mod 64][pad + f div 64].
+template <int TI>                                 // TI elements of every residue per tile: 64 TI bins
+__global__ void __launch_bounds__(256)
+k_post_residues(float2 *__restrict__ rt, long long rt_stride, int rt_len, int pad, float2 *__restrict__ spec,
+                long long xstride, int Nc, const float2 *__restrict__ twN) {
+  constexpr int TB = 64 * TI;                        // bins per tile
+  __shared__ float2 tf[TI][65];                      // [f2 - TI t][residue]
+  __shared__ float2 tg[TI + 1][65];                  // [u div 64][u mod 64], u = g - G0 = 1 .. TB
+  const int seg = blockIdx.y, t = blockIdx.x, f0 = TB * t, G0 = Nc - f0 - TB;
+  float2 *R = rt + (size_t)seg * rt_stride + pad;
+  float2 *S = spec + (size_t)seg * xstride;
+  if (f0 == Nc / 2) {
+    // the middle bin alone (its own mirror); the rest of this block of bins belongs to the last tile's mirror
+    if (threadIdx.x == 0) {
+      const float2 A = R[f0 >> 6];                       // residue 0
+      float2 w = __ldg(twN + f0); w.y = -w.y;
+      const float2 D = make_float2(0.f, A.y);            // B = A: E = (Ax, 0), D = (0, Ay)
+      const float2 tt = make_float2(w.x * D.x - w.y * D.y, w.x * D.y + w.y * D.x);
+      const float2 xf = make_float2(A.x + tt.y, -tt.x);
+      R[f0 >> 6] = xf; S[f0] = xf;
+    }
+    return;
+  }
+  for (int i = threadIdx.x; i < TB; i += 256) {
+    const int res = i / TI, di = i - res * TI;
+    tf[di][res] = R[(size_t)res * rt_len + (f0 >> 6) + di];
+  }
+  for (int i = threadIdx.x; i < (TI + 1) * 64; i += 256) {
+    const int res = i / (TI + 1), di = i - res * (TI + 1);
+    const int u = 64 * di + res;
+    // (bin Nc itself -- u = TB of the first tile -- is not part of the half-length transform)
+    if (u >= 1 && u <= TB && G0 + u < Nc) tg[di][res] = R[(size_t)res * rt_len + (G0 >> 6) + di];
+  }
+  __syncthreads();
+  for (int j = threadIdx.x; j < TB; j += 256) {
+    const int f = f0 + j, u = TB - j;                    // g = Nc - f = G0 + u
+    const float2 A = tf[j >> 6][j & 63];
+    const float2 B = (f == 0) ? A : tg[u >> 6][u & 63];
+    const float2 E = make_float2(0.5f * (A.x + B.x), 0.5f * (A.y - B.y));
+    const float2 D = make_float2(0.5f * (A.x - B.x), 0.5f * (A.y + B.y));
+    float2 w = __ldg(twN + f); w.y = -w.y;               // e^{-2 pi i f/N}
+    const float2 tt = make_float2(w.x * D.x - w.y * D.y, w.x * D.y + w.y * D.x);
+    const float2 xf = make_float2(E.x + tt.y, E.y - tt.x), xg = make_float2(E.x - tt.y, -E.y - tt.x);
+    tf[j >> 6][j & 63] = xf; tg[u >> 6][u & 63] = xg;
+    S[f] = xf; S[Nc - f] = xg;
+  }
+  __syncthreads();
+  for (int i = threadIdx.x; i < TB; i += 256) {
+    const int res = i / TI, di = i - res * TI;
+    R[(size_t)res * rt_len + (f0 >> 6) + di] = tf[di][res];
+  }
+  for (int i = threadIdx.x; i < (TI + 1) * 64; i += 256) {
+    const int res = i / (TI + 1), di = i - res * (TI + 1);
+    const int u = 64 * di + res;
+    if (u >= 1 && u <= TB) R[(size_t)res * rt_len + (G0 >> 6) + di] = tg[di][res];
+  }
+}
+
+constexpr int kPostTI = 16;
+
+bool long_residues_ok(const qtam_plan *p) {
+  return p->esz == 4 && p->n_pow2 && p->d_sp_xt != nullptr && p->d_ptw_long != nullptr &&
+         p->hp.N == (int64_t(1) << (kLongLog2N2 + 7));     // n = N/2 = 64 * 2^13
+}
+
+static int long_tw_shift(const qtam_plan *p, int log2n) {
+  int log2twn = 0;
+  while ((int64_t(1) << log2twn) < p->twn) ++log2twn;
+  return log2twn - log2n;
+}
+
+// forward: x -> the residue-sorted spectrum (p->d_sp_xt) and the spectrum in bin order (p->d_spec)
+qtam_status long_forward_residues(qtam_plan *p, const void *d_x, int batch, cudaStream_t st) {
+  constexpr int NT = CtaFftPlan<kLongLog2N2>::NT, LOG2R = 6;
+  const int Nc = (int)(p->hp.N / 2);
+  const int tw_shift = long_tw_shift(p, kLongLog2N2 + LOG2R);
+  if (tw_shift < 0) return QTAM_ERR_UNSUPPORTED;
+  const float2 *tw = static_cast<const float2 *>(p->d_tw);
+  const float2 *ptw = static_cast<const float2 *>(p->d_ptw_long);
+  float2 *ws = static_cast<float2 *>(p->d_ws), *rt = static_cast<float2 *>(p->d_sp_xt);
+  const long long rt_stride = 64LL * p->sp_xt_len;
+  const size_t smem = sizeof(float2) * (size_t)cta_fft_smem_elems<kLongLog2N2>();
+  const double pass_bytes = 16.0 * (double)batch * (double)Nc;
+  dim3 ga((1 << kLongLog2N2) / 256, batch), gb(1 << LOG2R, batch);
+  {
+    LaunchScope ls(p, st, K_LONG_A, (double)batch * 4.0 * (double)p->hp.N, pass_bytes);
+    k_long_a<LOG2R, -1><<<ga, 256, 0, st>>>(static_cast<const float2 *>(d_x), Nc, ws, p->hp.N, tw, tw_shift);
+  }
+  QTAM_LAUNCH_CHECK();
+  {
+    LaunchScope ls(p, st, K_LONG_B, 0.0, pass_bytes);
+    k_long_b_res<-1><<<gb, NT, smem, st>>>(ws, p->hp.N, 1 << kLongLog2N2, rt + p->sp_xt_pad, rt_stride, p->sp_xt_len, ptw);
+  }
+  QTAM_LAUNCH_CHECK();
+  {
+    dim3 gp((unsigned)(Nc / 2 / (64 * kPostTI) + 1), batch);
+    LaunchScope ls(p, st, K_R2C_POST, 0.0, 3.0 * 8.0 * (double)batch * (double)Nc);
+    k_post_residues<kPostTI><<<gp, 256, 0, st>>>(rt, rt_stride, p->sp_xt_len, p->sp_xt_pad, static_cast<float2 *>(p->d_spec),
+                                            p->xstride, Nc, static_cast<const float2 *>(p->d_twN));
+  }
+  QTAM_LAUNCH_CHECK();
+  return QTAM_OK;
+}
+
+// inverse: the pre-processed spectrum in residue order (p->d_sp_xt, written by k_combine_runs) -> x_out
+qtam_status long_inverse_residues(qtam_plan *p, void *d_x_out, int batch, cudaStream_t st) {
+  constexpr int NT = CtaFftPlan<kLongLog2N2>::NT, LOG2R = 6;
+  const int Nc = (int)(p->hp.N / 2);
+  const int tw_shift = long_tw_shift(p, kLongLog2N2 + LOG2R);
+  if (tw_shift < 0) return QTAM_ERR_UNSUPPORTED;
+  const float2 *tw = static_cast<const float2 *>(p->d_tw);
+  const float2 *ptw = static_cast<const float2 *>(p->d_ptw_long);
+  float2 *ws = static_cast<float2 *>(p->d_ws), *rt = static_cast<float2 *>(p->d_sp_xt);
+  const long long rt_stride = 64LL * p->sp_xt_len;
+  const size_t smem = sizeof(float2) * (size_t)cta_fft_smem_elems<kLongLog2N2>();
+  const double pass_bytes = 16.0 * (double)batch * (double)Nc;
+  dim3 ga((1 << kLongLog2N2) / 256, batch), gb(1 << LOG2R, batch);
+  {
+    LaunchScope ls(p, st, K_LONG_B, 0.0, pass_bytes);
+    k_long_b_res<+1><<<gb, NT, smem, st>>>(rt + p->sp_xt_pad, rt_stride, p->sp_xt_len, ws, p->hp.N, 1 << kLongLog2N2, ptw);
+  }
+  QTAM_LAUNCH_CHECK();
+  {
+    LaunchScope ls(p, st, K_LONG_A, (double)batch * 4.0 * (double)p->hp.N, pass_bytes);
+    k_long_a_pre<LOG2R, +1><<<ga, 256, 0, st>>>(ws, p->hp.N, static_cast<float2 *>(d_x_out), Nc, tw, tw_shift);
+  }
+  QTAM_LAUNCH_CHECK();
+  return QTAM_OK;
+}
+
 // Batched complex FFTs of 2^11 .. 2^14 points, one CTA per sequence in shared memory (ctafft.cuh): the power-of-two
 // transforms inside the radix-3 step of the segment lengths N = 3 * 2^k (the paper's 6 s at 4096 Hz = 3 * 2^13).
 template <int LOG2N, int DIR>
@@ -300,7 +485,9 @@ qtam_status build_long_fft(qtam_plan *p) {
     return QTAM_ERR_CUDA;
   const size_t smem = sizeof(float2) * (size_t)cta_fft_smem_elems<kLongLog2N2>();
   if (cudaFuncSetAttribute(k_long_b<-1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess ||
-      cudaFuncSetAttribute(k_long_b<+1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
+      cudaFuncSetAttribute(k_long_b<+1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess ||
+      cudaFuncSetAttribute(k_long_b_res<-1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess ||
+      cudaFuncSetAttribute(k_long_b_res<+1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
     return QTAM_ERR_CUDA;
   return QTAM_OK;
 }

@@ -629,6 +629,7 @@ qtam_status build_rows_split(qtam_plan *p, int c, const std::vector<ClLeader> &l
   }
   if (!p->d_sp_xt) {
     p->sp_xt_len = 2 * kSpPad + (int)((p->hp.nb + kSpRes - 1) / kSpRes);
+    p->sp_xt_pad = kSpPad;
     const size_t bytes = sizeof(float2) * (size_t)p->max_batch * kSpRes * (size_t)p->sp_xt_len;
     if (!up(&p->d_sp_xt, nullptr, bytes)) return QTAM_ERR_ALLOC;
     if (cudaMemset(p->d_sp_xt, 0, bytes) != cudaSuccess) return QTAM_ERR_CUDA;   // the pads stay zero for good
@@ -703,6 +704,7 @@ static qtam_status sp_launch(qtam_plan *p, int c, int batch, void *d_coef, int p
 // the residue-sorted copy of the spectrum the forward sub-transforms read (after the long R2C, before the rows)
 qtam_status split_spectrum(qtam_plan *p, int batch, cudaStream_t st) {
   if (!p->d_sp_xt) return QTAM_OK;
+  if (p->sp_xt_fresh) { p->sp_xt_fresh = false; return QTAM_OK; }   // the long FFT has left it there
   const int nb = (int)p->hp.nb;
   const dim3 grid((unsigned)((nb + 4095) / 4096), (unsigned)batch);
   const double bytes = (double)batch * 8.0 * (double)nb;
