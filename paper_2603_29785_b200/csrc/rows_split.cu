@@ -1,33 +1,35 @@
-// rows_split.cu -- rows of 2^14 .. 2^16 points (float) as a DATAFLOW of small work items in one persistent
-// kernel: the row's short FFT of M = F * P points (P = 1024, F = 16, 32, 64) is split Cooley-Tukey-wise into
-//   sub-transform items (row, four residues q = 4 qb .. 4 qb + 3): four interleaved P-point FFTs in shared memory
-//   radix-F items       (row, a block of nc):                      the radix-F stage in registers
+// rows_split.cu -- rows of 2^15 and 2^16 points (float) as a DATAFLOW of warp-sized work items in one persistent
+// kernel: the row's short FFT of M = F * P points (P = 1024, F = 32, 64; F = 16 is built too) is split
+// Cooley-Tukey-wise into
+//   sub-transform items (row, residue q):        one P-point FFT in ONE WARP's registers (32 values per lane, two
+//                                                radix-32 passes around the warp's private piece of shared memory)
+//   radix-F items       (row, 32 or 16 values of nc):  the radix-F stage in registers (F = 64: a pair of lanes per nc)
 // and the intermediate Z[q][nc] crosses between them through a small ring of row-sized slots that stays in L2
 // (the items of a row run on different SMs).  Index split:
 //   band side   j = q + F jc   (q < F, jc < P),     time side   n = nc + P m   (m < F, nc < P)
-//   forward (a2 + a3, C47 :589)  Z[q][nc] = sum_jc B[q + F jc] w_P^{+jc nc},   B[j] = X[kc + jj] W_k[jj] (N M)^-1/2
-//                                Y[nc + P m] = sum_q w_M^{+q nc} Z[q][nc] w_F^{+q m}
-//   inverse (a5 + a6, C49 :598)  u[q][nc] = w_M^{-q nc} sum_m (sum over members Y[nc + P m]) w_F^{-q m}
-//                                Bhat[q + F jc] = sum_nc u[q][nc] w_P^{-jc nc},  G = sqrt(N/M) Bhat W_k  added into the
-//                                partial spectrum of the leader's group by plain read-modify-write; the leaders of a
-//                                group follow each other through a completion count, so every bin is updated in a
-//                                fixed order: a segmented reduction without atomics on data and without a band
-//                                workspace (Eq. 11 :135).  k_combine_runs adds the groups' partial sums.
+//   forward (a2 + a3, C47 :589)  Z[q][nc] = sum_jc B[q + F jc] w_P^{+jc nc},   B[j] = X[kc + jj] W_k[jj]
+//                                Y[nc + P m] = (N M)^-1/2 sum_q w_M^{+q nc} Z[q][nc] w_F^{+q m}
+//   inverse (a5 + a6, C49 :598)  u[q][nc] = sqrt(N/M) w_M^{-q nc} sum_m (sum over members Y[nc + P m]) w_F^{-q m}
+//                                Bhat[q + F jc] = sum_nc u[q][nc] w_P^{-jc nc},  G = Bhat W_k  added into the partial
+//                                spectrum of the leader's group by plain read-modify-write; the leaders of a group
+//                                follow each other through a completion count, so every bin is updated in a fixed
+//                                order: a segmented reduction without atomics on data and without a band workspace
+//                                (Eq. 11 :135).  k_combine_runs adds the groups' partial sums.
 // Why not one CTA (or one cluster) per row: a 2^16-point row is 512 KB, more than one SM holds, and the phases of a
 // cluster that owns a row (gather, sub-transforms, exchange through distributed shared memory, stores) run one
 // after the other on all of its SMs -- measured on cfg4: 38.6 k cycles per row and SM where HBM needs 14 k, the
-// exchange alone at 11 B/cycle/SM.  Here small items of many rows, in different phases, share an SM (4 CTAs of 128
-// threads), so gather latency, butterflies and the traffic of the coefficients overlap; the price is one round
-// trip of the intermediate through L2 (not DRAM: the ring holds a few dozen rows).
+// exchange alone at 11 B/cycle/SM.  Here 16 warps per SM work on items of many rows in different phases and never
+// meet (no block barrier after the tables are loaded); the price is one round trip of the intermediate through
+// L2 (the ring holds a few dozen rows).
 //
 // Scheduling.  Items are popped in a fixed order from one counter (atomicAdd): block t of the order holds the
 // first-stage items of row t followed by the second-stage items of row t - LAG.  A second-stage item needs the
 // first-stage items of its row (a completion count per row, release / acquire); a first-stage item needs the slot,
 // i.e. the second-stage items of row t - NSLOTS; an inverse sub-transform item also needs the previous leader of
-// its group.  Every wait is on items EARLIER in the order, and only running CTAs hold items, so the earliest
-// unfinished item can always run: no deadlock, whatever the number of resident CTAs (NSLOTS > LAG is all it
-// takes).  Thread 0 pops the next item and reads its counts while the current item runs, so in the steady state
-// nobody waits; the completion signal of an item (fence + atomicAdd by thread 0) overlaps the start of the next.
+// its group.  Every wait is on items EARLIER in the order, and only running warps hold items, so the earliest
+// unfinished item can always run: no deadlock, whatever the number of resident CTAs and whatever else runs on
+// the GPU (NSLOTS > LAG is all it takes).  See the kernel for how lane 0 keeps the schedule's latencies (pop, counts,
+// release) out of the warp's way.
 #include <algorithm>
 #include <cmath>
 #include <cstdint>
