@@ -1,5 +1,6 @@
 // rows_cta.cu -- rows of 2^11 .. 2^13 points (float): one CTA per (segment, row), the row's short FFT in
-// shared memory with the Stockham engine of ctafft.cuh (longer rows: rows_cluster.cu).
+// shared memory with the Stockham engine of ctafft.cuh (longer rows: rows_cluster.cu, rows_split.cu; the FORWARD of
+// the 2^11-point rows: rows_2k.cu, one warp per row).
 //
 //   forward (a2 + a3)  pass 1 gathers X[kc + jj] W_k[jj] straight from the spectrum (only the support is read,
 //                      the rest of the M-array is zero; A9 :323, C46 :583), the last pass writes the scaled

@@ -1,5 +1,5 @@
 // rows_split.cu -- rows of 2^15 and 2^16 points (float) as a DATAFLOW of warp-sized work items in one persistent
-// kernel: the row's short FFT of M = F * P points (P = 1024, F = 32, 64; F = 16 is built too) is split
+// kernel: the row's short FFT of M = F * P points (P = 1024, F = 32, 64) is split
 // Cooley-Tukey-wise into
 //   sub-transform items (row, residue q):        one P-point FFT in ONE WARP's registers (32 values per lane, two
 //                                                radix-32 passes around the warp's private piece of shared memory)
@@ -49,7 +49,7 @@ constexpr int kSpTwElems = kSpTwRows * 32;
 constexpr int kSpMaxLead = 96, kSpMaxMem = 384;           // leaders / members of a class kept in shared memory
 // The sub-transform of residue q reads the band at bins kc + q + F jc: every F-th bin.  k_spec_residues keeps a
 // second copy of the spectrum sorted by residue, XT[f mod 64][f div 64] (64 = the largest F), in which those bins
-// are consecutive (F = 64) or 64 / F interleaved runs (F = 32, 16), so that a warp reads whole lines; kSpPad zero
+// are consecutive (F = 64) or two interleaved runs (F = 32), so that a warp reads whole lines; kSpPad zero
 // entries on both sides of every residue stand for the bins outside 0 .. N/2 (R8) -- no bounds test anywhere.
 // The windows of these rows are kept the same way, WT[q][jc] = W_k[q + F jc'] (zero off the support).
 constexpr int kSpRes = 64, kSpPad = 520;
@@ -61,10 +61,9 @@ struct SpOrder { int lead, prev, pbase, len64; };
 struct SpArgs {
   const ClLeader *lead; const int2 *mem; int nlead, nmem;
   const SpOrder *order;
-  const float *win;
   const float *wt; const int *wt_off;      // windows by residue, first element per leader
   const float2 *xt; long long xt_stride; int xt_len;   // spectrum by residue: [segment][64][xt_len]
-  const float2 *spec; long long xstride; int nbins;
+  int nbins;
   float2 *coef; long long ctot;
   float2 *part; long long part_stride;
   const float2 *tw2;                       // pass-2 table of the sub-transforms
@@ -78,18 +77,6 @@ struct SpArgs {
 __device__ __forceinline__ int ld_acquire(const int *p) {
   int v;
   asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
-  return v;
-}
-__device__ __forceinline__ float2 ldg_nc_f2(const float2 *p, bool ok) {
-  float2 v;
-  asm volatile("{\n .reg .pred q;\n setp.ne.s32 q, %3, 0;\n mov.f32 %0, 0f00000000;\n mov.f32 %1, 0f00000000;\n"
-               " @q ld.global.nc.v2.f32 {%0, %1}, [%2];\n}" : "=f"(v.x), "=f"(v.y) : "l"(p), "r"((int)ok));
-  return v;
-}
-__device__ __forceinline__ float ldg_nc_f1(const float *p, bool ok) {
-  float v;
-  asm volatile("{\n .reg .pred q;\n setp.ne.s32 q, %2, 0;\n mov.f32 %0, 0f00000000;\n"
-               " @q ld.global.nc.f32 %0, [%1];\n}" : "=f"(v) : "l"(p), "r"((int)ok));
   return v;
 }
 __device__ __forceinline__ float2 ldg_cg_f2(const float2 *p, bool ok) {
@@ -564,7 +551,6 @@ qtam_status build_rows_split(qtam_plan *p, int c, const std::vector<ClLeader> &l
   const int F = (int)(M / kSpP);
   bool ok = false;
   switch (F) {
-    case 16: ok = sp_prepare<16>(p, c); break;
     case 32: ok = sp_prepare<32>(p, c); break;
     case 64: ok = sp_prepare<64>(p, c); break;
     default: break;
@@ -672,11 +658,10 @@ static qtam_status sp_launch(qtam_plan *p, int c, int batch, void *d_coef, int p
   SpArgs A{};
   A.lead = p->d_cl_lead[c]; A.mem = p->d_cl_mem[c]; A.nlead = p->n_cl_lead[c]; A.nmem = p->sp_nmem[c];
   A.order = static_cast<const SpOrder *>(p->d_sp_order[c]);
-  A.win = static_cast<const float *>(p->d_win);
   A.wt = static_cast<const float *>(p->d_sp_wt[c]); A.wt_off = static_cast<const int *>(p->d_sp_wtoff[c]);
   A.xt = static_cast<const float2 *>(p->d_sp_xt); A.xt_len = p->sp_xt_len;
   A.xt_stride = (long long)kSpRes * p->sp_xt_len;
-  A.spec = static_cast<const float2 *>(p->d_spec); A.xstride = p->xstride; A.nbins = (int)p->hp.nb;
+  A.nbins = (int)p->hp.nb;
   A.coef = static_cast<float2 *>(d_coef); A.ctot = p->hp.ctot;
   A.part = static_cast<float2 *>(p->d_part); A.part_stride = p->part_stride;
   A.tw2 = static_cast<const float2 *>(p->d_sp_tw2);
@@ -723,7 +708,6 @@ qtam_status split_spectrum(qtam_plan *p, int batch, cudaStream_t st) {
 qtam_status split_rows(qtam_plan *p, int c, bool fwd, int batch, void *d_coef, int plane, cudaStream_t st) {
   const int F = (int)((1LL << (kClLog2Min + c)) / kSpP);
   switch (F) {
-    case 16: return fwd ? sp_launch<16, true>(p, c, batch, d_coef, plane, st) : sp_launch<16, false>(p, c, batch, d_coef, plane, st);
     case 32: return fwd ? sp_launch<32, true>(p, c, batch, d_coef, plane, st) : sp_launch<32, false>(p, c, batch, d_coef, plane, st);
     case 64: return fwd ? sp_launch<64, true>(p, c, batch, d_coef, plane, st) : sp_launch<64, false>(p, c, batch, d_coef, plane, st);
     default: break;
