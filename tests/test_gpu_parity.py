@@ -577,7 +577,7 @@ def test_forward_inverse_under_cuda_graph_capture():
 
 
 @pytest.mark.parametrize("name,dtype,nseg", [("cfg5", "f32", 16), ("cfg3", "f32", 3), ("cfg2", "f32", 2), ("cfg5", "f64", 3),
-                                             ("cfg5", "f32", 1)])
+                                             ("cfg5", "f32", 1), ("cfg4", "f32", 1)])
 def test_forward_threshold_fused_equals_the_two_calls(name, dtype, nseg):
     """qtam_forward_threshold = qtam_forward then qtam_threshold_rowmedian, bit for bit (the decisions are taken
     on the same binary32 values, in registers instead of after a round trip through memory)."""
