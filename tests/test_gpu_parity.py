@@ -860,3 +860,19 @@ def test_long_rows_partial_batches_and_two_plans_at_once():
         assert torch.equal(Ya2, Ya) and torch.equal(Yb2, Yb)
         assert torch.equal(xa2, xa) and torch.equal(xb2, xb)
     ga.close(); gb.close()
+
+
+def test_longest_segment_without_long_rows():
+    """N = 2^20 with rows of at most 2^14 points: no residue-sorted spectrum, so the long transforms take the two-pass
+    path whose second pass writes with stride 64 (long_fft.cu), not the residue-order one of config 4."""
+    args = (16384.0, 1 << 20, [200.0], 2000.0, 7000.0, 24.0)
+    g, r = make_plans(args, "f32", 1)
+    assert max(int(a.M) for a in g.rows) <= 1 << 14
+    x = np.random.default_rng(5).standard_normal((1, 1 << 20)).astype(np.float32)
+    x64 = x.astype(np.float64)
+    Yg = g.forward(dev(x)).cpu().numpy()
+    Yr = r.forward(x64, engine=1)
+    assert worst_segment(Yg, Yr) <= 2e-5 and worst_row(Yg, Yr, r) <= TOL_ROW["f32"]
+    xg = g.inverse(dev(Yr.astype(np.complex64))).cpu().numpy()
+    assert worst_segment(xg, r.inverse(Yr.astype(np.complex64).astype(np.complex128), engine=1)) <= 2e-5
+    g.close()
