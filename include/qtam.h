@@ -51,7 +51,8 @@ typedef enum {
   QTAM_ERR_UNSUPPORTED = 2,   /* window family / size outside what this build implements */
   QTAM_ERR_ALLOC = 3,         /* host or device allocation failed at plan creation */
   QTAM_ERR_CUDA = 4,          /* a CUDA runtime call or launch failed (or no device) */
-  QTAM_ERR_EMPTY_FRAME = 5    /* the plan's cover set is empty */
+  QTAM_ERR_EMPTY_FRAME = 5,   /* the plan's cover set is empty */
+  QTAM_ERR_TOO_LARGE = 6      /* qtam_cluster_noalloc only: the problem does not fit the library's fixed scratch */
 } qtam_status;
 
 /* All fields optional; pass NULL for the defaults. struct_size = sizeof(qtam_options) (ABI version). */
@@ -190,6 +191,35 @@ qtam_status qtam_cluster(qtam_plan *p, const void *d_coef, int batch, int plane,
                          int32_t *d_count, void *stream);
 qtam_status qtam_mask(qtam_plan *p, const void *d_coef, int batch, int plane, const int32_t *d_labels, int label,
                       void *d_out, void *stream);
+
+/* Cluster labelling for callers that cannot allocate device memory.
+ * Every call above needs a qtam_plan, and creating one calls cudaMalloc.  That rules the library out for a stage of a
+ * running low-latency pipeline (a cudaMalloc or cudaFree there synchronises the device and holds up every stream), for
+ * a plug-in of an application whose own pool already owns the free device memory, and for code that is only ever
+ * lent its buffers.  This one entry point serves them: it takes no plan, and it calls neither cudaMalloc nor cudaFree
+ * nor anything else that allocates, on the host or on the device.  The labels, the counts and the image are the
+ * caller's; the single piece of scratch the method needs (a pixel counter per component root) is a fixed array that
+ * is part of the library's device image: QTAM_CLUSTER_NOALLOC_MAX_PIXELS 32-bit counters = 4 MiB on every GPU on
+ * which the process uses libqtam.so, held from the moment the CUDA runtime loads the library's kernels until exit.
+ *   d_img: the image of segment 0, [rows][samples] complex of `dtype`, contiguous (for a plan in the uniform-tile
+ *     layout: d_coef + the offset of the plane's first row, rows = the plane's rows, samples = M); segment b starts
+ *     segment_stride complex elements after segment b - 1 (coeffs_per_segment for a plan's array, rows * samples for
+ *     a bare stack of images).  Not modified.  A pixel is active where its coefficient is non-zero.
+ *   d_labels [batch][rows * samples] int32, d_count [batch] int32, min_area >= 1: exactly as for qtam_cluster, and
+ *     with the same values as qtam_cluster gives on the same image, bit for bit.
+ * Limit: batch * rows * samples <= QTAM_CLUSTER_NOALLOC_MAX_PIXELS (and batch <= 65535).  Beyond it the call
+ *   returns QTAM_ERR_TOO_LARGE, checked before anything touches the GPU; split the batch, or use qtam_cluster.
+ * First call: the first call on each device (that device being current, as for every call here) asks the runtime
+ *   where the array lives on that device and remembers the answer.  This is a host-side query that may make the
+ *   runtime load the library's device code; do it once at start-up (a call with batch = 1 on a small image will do),
+ *   before any stream capture begins.  Every later call on that device only enqueues kernels on `stream`.
+ * Sharing: all calls on one GPU use the same array, from any thread or stream.  A call first clears the counters it
+ *   is about to use, so what an earlier call left behind does no harm; but two calls whose kernels run at the same
+ *   time on one GPU overwrite each other's counters and return wrong labels.  Keep the calls of a device on one
+ *   stream, or order them with events. */
+#define QTAM_CLUSTER_NOALLOC_MAX_PIXELS 1048576
+qtam_status qtam_cluster_noalloc(qtam_dtype dtype, const void *d_img, int64_t segment_stride, int batch, int rows,
+                                 int samples, int min_area, int32_t *d_labels, int32_t *d_count, void *stream);
 
 /* Row-median threshold in place (BASELINE.json config 5; R11): per (segment,row),
  * m = median_n |Y_k[n]| (two middle values averaged), zero every Y_k[n] with |Y_k[n]| < kappa*m.

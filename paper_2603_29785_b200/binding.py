@@ -14,13 +14,14 @@ _LIBPATH = os.path.join(_HERE, "libqtam.so")
 _lib = None
 
 QTAM_F32, QTAM_F64 = 0, 1
-STATUS = {0: "ok", 1: "invalid argument", 2: "unsupported", 3: "alloc", 4: "cuda", 5: "empty frame"}
+STATUS = {0: "ok", 1: "invalid argument", 2: "unsupported", 3: "alloc", 4: "cuda", 5: "empty frame", 6: "too large"}
+CLUSTER_NOALLOC_MAX_PIXELS = 1 << 20      # QTAM_CLUSTER_NOALLOC_MAX_PIXELS of include/qtam.h
 
 SYMBOLS = ["qtam_plan_create", "qtam_plan_create_host", "qtam_plan_destroy", "qtam_plan_info",
            "qtam_plan_rows", "qtam_plan_window", "qtam_plan_frame", "qtam_forward", "qtam_inverse",
            "qtam_dense", "qtam_dense_invert", "qtam_threshold_rowmedian", "qtam_forward_threshold", "qtam_plane_metric", "qtam_gather_plane", "qtam_max_plane_coeffs", "qtam_remodulate", "qtam_instantaneous_frequency", "qtam_last_launch_count", "qtam_status_string",
            "qtam_profile_enable", "qtam_profile_read", "qtam_output_length", "qtam_forward_length", "qtam_inverse_length",
-           "qtam_resample", "qtam_plane_pixels", "qtam_cluster", "qtam_mask"]
+           "qtam_resample", "qtam_plane_pixels", "qtam_cluster", "qtam_mask", "qtam_cluster_noalloc"]
 
 
 class QtamError(RuntimeError):
@@ -106,6 +107,7 @@ def lib():
         L.qtam_plane_pixels.restype = C.c_int64
         L.qtam_cluster.argtypes = [vp, vp, C.c_int, C.c_int, C.c_int, vp, vp, vp]
         L.qtam_mask.argtypes = [vp, vp, C.c_int, C.c_int, vp, C.c_int, vp, vp]
+        L.qtam_cluster_noalloc.argtypes = [C.c_int, vp, C.c_int64, C.c_int, C.c_int, C.c_int, C.c_int, vp, vp, vp]
         _lib = L
     return _lib
 
@@ -113,6 +115,35 @@ def lib():
 def _check(code, where):
     if code != 0:
         raise QtamError(code, where)
+
+
+def cluster_noalloc(img, segment_stride, batch, rows, samples, min_area, labels, count):
+    """qtam_cluster_noalloc: the labelling of Plan.cluster for a caller that may not allocate device memory (no plan,
+    no cudaMalloc inside the library: its one piece of scratch is a fixed 4 MiB array inside libqtam.so, shared by all
+    calls on a GPU, so keep them on one stream).  Every tensor is the caller's, this wrapper creates none: `img` a
+    CUDA complex64 / complex128 tensor (or a view starting at a plane's first coefficient), segment b at
+    img.data_ptr() + b * segment_stride elements; `labels` int32 with batch * rows * samples elements and `count`
+    int32 with batch elements are overwritten.  batch * rows * samples <= CLUSTER_NOALLOC_MAX_PIXELS, else QtamError
+    with code 6 ('too large').  Runs on torch's current stream; make the first call per device at start-up."""
+    import torch
+    if not (img.is_cuda and labels.is_cuda and count.is_cuda):
+        raise ValueError("qtam_cluster_noalloc: img, labels and count must be CUDA tensors")
+    if img.dtype not in (torch.complex64, torch.complex128):
+        raise ValueError(f"img: dtype {img.dtype}, expected complex64 or complex128")
+    if labels.dtype != torch.int32 or count.dtype != torch.int32 or not labels.is_contiguous() or not count.is_contiguous():
+        raise ValueError("labels and count must be contiguous int32 tensors")
+    batch, rows, samples = int(batch), int(rows), int(samples)
+    if batch < 0 or rows < 1 or samples < 1:
+        raise ValueError("batch >= 0, rows >= 1 and samples >= 1 expected")
+    if labels.numel() != batch * rows * samples or count.numel() != batch:
+        raise ValueError("labels needs batch * rows * samples elements and count needs batch")
+    if batch > 0 and img.storage_offset() + (batch - 1) * int(segment_stride) + rows * samples > img.untyped_storage().nbytes() // img.element_size():
+        raise ValueError("img: the last segment's image ends beyond the tensor's storage")
+    _check(lib().qtam_cluster_noalloc(QTAM_F32 if img.dtype == torch.complex64 else QTAM_F64, img.data_ptr(),
+                                      int(segment_stride), batch, rows, samples, int(min_area), labels.data_ptr(),
+                                      count.data_ptr(), C.c_void_p(torch.cuda.current_stream().cuda_stream)),
+           "qtam_cluster_noalloc")
+    return labels, count
 
 
 class Plan:

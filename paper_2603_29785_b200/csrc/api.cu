@@ -785,6 +785,7 @@ const char *qtam_status_string(qtam_status s) {
     case QTAM_ERR_ALLOC: return "allocation failed";
     case QTAM_ERR_CUDA: return "CUDA error (or no CUDA device)";
     case QTAM_ERR_EMPTY_FRAME: return "empty cover set";
+    case QTAM_ERR_TOO_LARGE: return "problem larger than the library's fixed scratch (QTAM_CLUSTER_NOALLOC_MAX_PIXELS)";
   }
   return "unknown status";
 }
