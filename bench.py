@@ -8,8 +8,10 @@ window gather + baseband shift + short IFFT per row), [row-median threshold for 
 (per-row FFT, overlap reduction, 1/P, long C2R).  Default workload: BASELINE.json configs[3]
 ("cfg4": 16 x 64 s at 16384 Hz, N = 2^20, complex64, forward+inverse), the largest single-GPU
 configuration (2.93 GB of compulsory traffic per step); the same run also times configs 2, 3, 5 and the
-fp64 variant of 5 (`configs` in the JSON line), each at its own batch and at a larger one.
-"Measurement".  One JSON line is printed by rank 0.
+fp64 variant of 5, each at its own batch and at a larger one.  See DESIGN.md "Measurement".  Rank 0 prints ONE
+compact JSON line (under 2 KB: the contract's keys, roofline, e2e, cpu_baseline) as the last line of stdout;
+the per-kernel tables and the records of the other configurations go to gpurun_out/bench_detail.json
+(`--detail`), whose path the line carries.
 
 Timing: W >= 3 warm-up steps, then K steps each bracketed by CUDA events on the launch stream with an
 L2 flush (a 512 MB device memset) before every step, outside the event brackets; barrier +
@@ -51,6 +53,8 @@ def parse_args():
     ap.add_argument("--no-other-configs", action="store_true",
                     help="skip the records of the other BASELINE configurations (`configs` in the JSON line)")
     ap.add_argument("--dtype", default="", choices=["", "f32", "f64"], help="override the configuration's dtype")
+    ap.add_argument("--detail", default=os.path.join("gpurun_out", "bench_detail.json"),
+                    help="where the per-kernel tables and the records of the other configurations go")
     return ap.parse_args()
 
 
@@ -235,6 +239,41 @@ def run_reference(args):
         "gpu_launches": 0,
     }
     print(json.dumps(line))
+
+
+HEADLINE_LIMIT = 2048      # bytes: the driver keeps a bounded tail of stdout and parses the last line
+
+
+def headline_json(line):
+    """the ONE line rank 0 prints last: the contract's keys, the roofline of the top kernel, cpu_baseline and
+    e2e, compact separators, floats rounded to 6 significant digits.  Per-kernel tables, the other configurations
+    and the largest-batch records go to the detail file (write_detail), never into this line: round 2's line grew
+    to 23 KB and the driver could not parse it.  Raises if the line would not fit HEADLINE_LIMIT."""
+    def rnd(v):
+        if isinstance(v, float):
+            return float(f"{v:.6g}")
+        if isinstance(v, dict):
+            return {k: rnd(x) for k, x in v.items()}
+        if isinstance(v, (list, tuple)):
+            return [rnd(x) for x in v]
+        return v
+    text = json.dumps(rnd(line), separators=(",", ":"))
+    if len(text) >= HEADLINE_LIMIT:
+        raise ValueError(f"bench.py headline is {len(text)} bytes (limit {HEADLINE_LIMIT}): move keys to the detail file")
+    return text
+
+
+def write_detail(path, detail):
+    """per-kernel tables, largest-batch and other-configuration records as indented JSON; returns the path
+    written relative to the repo root (or why it was not written: the headline never depends on it)"""
+    try:
+        full = path if os.path.isabs(path) else os.path.join(ROOT, path)
+        os.makedirs(os.path.dirname(full), exist_ok=True)
+        with open(full, "w") as f:
+            json.dump(detail, f, indent=1)
+        return os.path.relpath(full, ROOT)
+    except Exception as exc:
+        return f"not written: {exc}"
 
 
 def workload_config(args, cfg, batch, plan):
@@ -538,6 +577,7 @@ def run_ours(args):
             w.close()
             wb = Workload(torch, binding, dev, args.workload, dtype, big, args.overlap, x_np=x_main)
             largest = record(wb, n_side, 3, flush, barrier, peak)
+            largest["round_trip_err"] = wb.round_trip_err()
             wb.close()
             del wb
             w = None
@@ -562,6 +602,7 @@ def run_ours(args):
                         big //= 2
                     wb = Workload(torch, binding, dev, name, dt, big, args.overlap, x_np=xo)
                     rec["largest_batch"] = record(wb, max(5, n_side // 2), 3, flush, barrier, peak)
+                    rec["largest_batch"]["round_trip_err"] = wb.round_trip_err()
                     wb.close()
                 others[key] = rec
             except Exception as exc:          # one configuration failing must not lose the headline
@@ -609,17 +650,29 @@ def run_ours(args):
         "gpu_launches": n_launch,
         "roofline": roof,
         "path": {"compulsory_bytes_per_step": comp, "achieved_gbs": path_gbs, "frac_of_peak": path_gbs / peak,
-                 "frac_of_8tbs": path_gbs / 8000.0, "ms_per_step_with_launch_profile": ms_total / args.steps,
-                 "ms_per_step_cuda_graph": ms_graph, "coeffs_per_segment": plan.ctot, "rows": plan.n_rows},
-        "kernels": kernels,
+                 "ms_per_step_cuda_graph": ms_graph},
         "round_trip_err": rt_err,
-        "largest_batch": largest,
-        "configs": others,
-        "cufft_side_by_side": cufft,
         "cpu_baseline": cpu,
         "csrc_hash": csrc_hash(),
     }
-    print(json.dumps(line))
+    detail = {
+        "headline": line,
+        "path": {"frac_of_8tbs": path_gbs / 8000.0, "ms_per_step_with_launch_profile": ms_total / args.steps,
+                 "coeffs_per_segment": plan.ctot, "rows": plan.n_rows},
+        "kernels": kernels, "largest_batch": largest, "configs": others, "cufft_side_by_side": cufft,
+    }
+    line["detail"] = write_detail(args.detail, detail)
+    try:
+        text = headline_json(line)
+    except ValueError:            # never lose the headline to its own size: fall back to the contract's keys alone
+        keep = ("metric", "value", "unit", "n_gpus", "steps", "warmup", "ms_per_step", "higher_is_better", "scaling",
+                "vs_baseline", "dtype", "data", "clocks", "e2e", "gpu_launches", "cpu_baseline", "csrc_hash", "detail")
+        small = {k: line[k] for k in keep}
+        small["config"] = {"workload": args.workload, "baseline_config_index": cfg["idx"] - 1, "batch_per_gpu": batch}
+        small["roofline"] = {k: roof[k] for k in ("bound", "kernel", "achieved", "peak", "unit", "frac", "traffic")} if roof else None
+        text = headline_json(small)
+    sys.stdout.flush()
+    print(text, flush=True)
     if world > 1:
         dist.destroy_process_group()
 
