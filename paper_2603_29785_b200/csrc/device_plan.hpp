@@ -3,6 +3,9 @@
 #pragma once
 #include <cuda_runtime.h>
 
+#include <map>
+#include <mutex>
+#include <utility>
 #include <vector>
 
 #include "qtam_internal.hpp"
@@ -15,7 +18,10 @@ enum KernelId {
   K_REDUCE_C2R_FAST, K_INV_FUSED, K_INV_TILES, K_COMBINE_C2R, K_THRESHOLD_FAST, K_ROWS_CTA_FWD, K_ROWS_CTA_INV,
   K_TINY_FWD, K_TINY_INV, K_LONG_A, K_LONG_B, K_PLANE_METRIC, K_BEST_PLANE, K_REMODULATE, K_INST_FREQ, K_FWD_ROWS_THR, K_GATHER_PLANE,
   K_ROWS_CL_FWD, K_ROWS_CL_INV, K_COMBINE_RUNS, K_C2C_FAST, K_SPLIT3, K_COMBINE3, K_LEN_BAND, K_LEN_SYNTH, K_LEN_ANALYSIS,
-  K_CLUSTER, K_MASK, K_SPEC_RES, K_COUNT
+  K_CLUSTER, K_MASK, K_SPEC_RES,
+  // rows of 2^14 .. 2^17 points, one name per length class (rows_cluster.cu, rows_split.cu): index + class
+  K_ROWS_L14_FWD, K_ROWS_L15_FWD, K_ROWS_L16_FWD, K_ROWS_L17_FWD, K_ROWS_L14_INV, K_ROWS_L15_INV, K_ROWS_L16_INV, K_ROWS_L17_INV,
+  K_COUNT
 };
 // fast float path (fast.cu): rows with 32 <= M <= 1024, grouped by G = M/32 lanes per row
 struct FastRow { int kc, dk, woff, goff, offset, plane, wpad, pad; };   // wpad: offset into the padded window table
@@ -38,6 +44,7 @@ constexpr int kThrFastLog2Max = 10;
 // cluster-level rows (rows_cluster.cu): 2^14 .. 2^17 points, one transform per thread-block cluster
 constexpr int kCtaLog2Min = 11, kCtaClasses = 3;
 constexpr int kClLog2Min = 14, kClClasses = 4;
+static_assert(kClLog2Min == 14 && kClClasses == 4, "K_ROWS_L14_FWD .. K_ROWS_L17_INV name these classes");
 constexpr int kCtaLog2Max = kClLog2Min + kClClasses - 1;   // longest row of the tuned float kernels
 constexpr int kCtaMaxMembers = 32;   // rows per leader (same centre bin and half-width)
 // a leader = one set of identical rows (same centre bin and half-width: transformed once); a group = consecutive
@@ -68,11 +75,26 @@ namespace qtam {
 // Launch configuration of one kernel instantiation, fixed when the plan is created (qtam_plan_create sets the
 // dynamic shared-memory limit and asks the occupancy calculator once; the compute calls only read this).
 struct KernelCfg { int occ = 0; size_t smem = 0; bool ready = false; };
+// cudaFuncAttributeMaxDynamicSharedMemorySize belongs to the kernel (per device, for the whole process), not to a
+// plan, and several kernels ask for a plan-dependent amount: a second plan that needs less must not lower the limit
+// under a live plan that needs more (its next launch would fail).  So the limit is only ever raised: the high-water
+// mark per (device, kernel) is kept here, and every plan's launches fit under it.
+inline bool raise_dynamic_smem(const void *kernel, size_t smem) {
+  static std::mutex mu;
+  static std::map<std::pair<int, const void *>, size_t> high;
+  if (smem <= 48 * 1024) return true;
+  int dev = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess) return false;
+  std::lock_guard<std::mutex> lock(mu);
+  size_t &h = high[std::make_pair(dev, kernel)];
+  if (smem <= h) return true;
+  if (cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return false;
+  h = smem;
+  return true;
+}
 template <typename K> inline bool kernel_prepare(KernelCfg &c, K kernel, int threads, size_t smem) {
   c.smem = smem; c.occ = 1; c.ready = false;
-  if (smem > 48 * 1024 &&
-      cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
-    return false;
+  if (!raise_dynamic_smem(reinterpret_cast<const void *>(kernel), smem)) return false;
   int occ = 0;
   if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kernel, threads, smem) != cudaSuccess) return false;
   c.occ = occ < 1 ? 1 : occ;

@@ -468,7 +468,7 @@ __global__ void k_threshold(const RowDev *__restrict__ rows, C2<T> *__restrict__
 static int ilog2(long long v) { int l = 0; while ((1LL << l) < v) ++l; return l; }
 
 template <typename K> static bool set_smem(K kernel, size_t bytes) {
-  return cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes) == cudaSuccess;
+  return raise_dynamic_smem(reinterpret_cast<const void *>(kernel), bytes);
 }
 
 constexpr int kThrCachePts = 8192;   // magnitudes k_threshold keeps in shared memory

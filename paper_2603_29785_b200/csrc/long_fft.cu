@@ -484,10 +484,10 @@ qtam_status build_long_fft(qtam_plan *p) {
   if (cudaMemcpy(p->d_ptw_long, t.data(), t.size() * sizeof(float), cudaMemcpyHostToDevice) != cudaSuccess)
     return QTAM_ERR_CUDA;
   const size_t smem = sizeof(float2) * (size_t)cta_fft_smem_elems<kLongLog2N2>();
-  if (cudaFuncSetAttribute(k_long_b<-1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess ||
-      cudaFuncSetAttribute(k_long_b<+1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess ||
-      cudaFuncSetAttribute(k_long_b_res<-1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess ||
-      cudaFuncSetAttribute(k_long_b_res<+1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
+  if (!raise_dynamic_smem(reinterpret_cast<const void *>(k_long_b<-1>), smem) ||
+      !raise_dynamic_smem(reinterpret_cast<const void *>(k_long_b<+1>), smem) ||
+      !raise_dynamic_smem(reinterpret_cast<const void *>(k_long_b_res<-1>), smem) ||
+      !raise_dynamic_smem(reinterpret_cast<const void *>(k_long_b_res<+1>), smem))
     return QTAM_ERR_CUDA;
   return QTAM_OK;
 }

@@ -303,7 +303,7 @@ template <int LOG2P, int LOG2CL> static bool prepare_cl(qtam_plan *p, int c) {
     KernelCfg &cfg = p->cfg_rows_cl[c][fwd];
     cfg.smem = smem; cfg.occ = 0; cfg.ready = false;
     const void *kern = fwd ? (const void *)k_rows_cluster<LOG2P, LOG2CL, true> : (const void *)k_rows_cluster<LOG2P, LOG2CL, false>;
-    if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return false;
+    if (!raise_dynamic_smem(kern, smem)) return false;
     cudaLaunchConfig_t lc = {};
     cudaLaunchAttribute at[1];
     at[0].id = cudaLaunchAttributeClusterDimension;
@@ -403,7 +403,7 @@ static qtam_status cl_launch(qtam_plan *p, int c, int batch, void *d_coef, int p
   lc.dynamicSmemBytes = cfg.smem; lc.stream = st; lc.attrs = at; lc.numAttrs = 1;
   const double bytes = (double)batch * 8.0 * p->cl_sumM[c];       // compulsory: the coefficients
   {
-    LaunchScope ls(p, st, FWD ? K_ROWS_CL_FWD : K_ROWS_CL_INV, bytes, bytes + (double)batch * 8.0 * p->cl_sumL[c]);
+    LaunchScope ls(p, st, (KernelId)((FWD ? K_ROWS_L14_FWD : K_ROWS_L14_INV) + c), bytes, bytes + (double)batch * 8.0 * p->cl_sumL[c]);
     if (cudaLaunchKernelEx(&lc, k_rows_cluster<LOG2P, LOG2CL, FWD>, A) != cudaSuccess) return QTAM_ERR_CUDA;
   }
   QTAM_LAUNCH_CHECK();
