@@ -83,23 +83,25 @@ def csrc_hash():
 
 
 def measured_traffic(workload, batch, kernel):
-    """(dram__bytes_read + dram__bytes_write of one launch, source) from the committed ncu --set full capture
-    profiles/r2_dram_traffic.csv (see the .md beside it).  A row counts only if it was captured from the very
-    kernel sources of this run (csrc hash) at this workload and batch: (None, why) otherwise -- ncu cannot
-    run inside a timed bench, so the number can only come from a capture, never from this process."""
-    path = os.path.join(ROOT, "profiles", "r2_dram_traffic.csv")
+    """(dram__bytes_read + dram__bytes_write of one launch, source) from the committed ncu --set full captures
+    profiles/r*_dram_traffic.csv (see the .md beside each), newest round first.  A row counts only if it was
+    captured from the very kernel sources of this run (csrc hash) at this workload and batch: (None, why)
+    otherwise -- ncu cannot run inside a timed bench, so the number can only come from a capture, never from
+    this process."""
+    import glob
     want = csrc_hash()
     seen = False
-    try:
-        with open(path) as f:
-            for line in f.read().splitlines()[1:]:
-                w, b, k, v, sha = line.split(",")[:5]
-                if w == workload and int(b) == batch and k == kernel:
-                    seen = True
-                    if sha == want:
-                        return float(v), f"profiles/r2_dram_traffic.csv (ncu --set full, csrc {sha})"
-    except Exception:
-        pass
+    for path in sorted(glob.glob(os.path.join(ROOT, "profiles", "r*_dram_traffic.csv")), reverse=True):
+        try:
+            with open(path) as f:
+                for line in f.read().splitlines()[1:]:
+                    w, b, k, v, sha = line.split(",")[:5]
+                    if w == workload and int(b) == batch and k == kernel:
+                        seen = True
+                        if sha == want:
+                            return float(v), f"profiles/{os.path.basename(path)} (ncu --set full, csrc {sha})"
+        except Exception:
+            pass
     return None, ("capture is from other kernel sources (csrc hash mismatch)" if seen
                   else "no ncu capture for this workload / batch / kernel")
 

@@ -99,7 +99,9 @@ qtam_status build_fast(qtam_plan *p) {
   // one window per distinct half-width (the clamped rows all share one)
   std::vector<float> fwin;
   std::vector<std::pair<int64_t, int>> seen;   // (dk and window identity, offset)
-  auto wkey = [](const HostRow &h) -> int64_t { return h.dk * 64 + h.wid; };
+  // the pair (half-width, window identity) as one key: wid is a plane index, so nP + 1 keeps any number of planes apart
+  const int64_t wid_span = (int64_t)hp.nP + 1;
+  auto wkey = [wid_span](const HostRow &h) -> int64_t { return h.dk * wid_span + h.wid; };
   auto window_of = [&](const HostRow &h) -> int {
     for (auto &e : seen) if (e.first == wkey(h)) return e.second;
     const int off = (int)fwin.size();
@@ -735,7 +737,8 @@ static const char *const kKernelNames[K_COUNT] = {
     "inv_rows", "inv_reduce", "dense_place", "threshold", "r2c_fast", "fwd_rows_fast", "inv_rows_fast",
     "reduce_c2r_fast", "inv_fused", "inv_tiles", "combine_c2r", "threshold_fast", "rows_cta_fwd", "rows_cta_inv",
     "tiny_rows_fwd", "tiny_rows_inv", "long_fft_a", "long_fft_b", "plane_metric", "best_plane", "remodulate", "inst_freq", "fwd_rows_thr", "gather_plane",
-    "rows_cl_fwd", "rows_cl_inv", "combine_runs", "c2c_fast", "split3", "combine3", "len_band", "len_synth", "len_analysis", "cluster", "mask", "spec_residues"};
+    "rows_cl_fwd", "rows_cl_inv", "combine_runs", "c2c_fast", "split3", "combine3", "len_band", "len_synth", "len_analysis", "cluster", "mask", "spec_residues",
+    "rows_2p14_fwd", "rows_2p15_fwd", "rows_2p16_fwd", "rows_2p17_fwd", "rows_2p14_inv", "rows_2p15_inv", "rows_2p16_inv", "rows_2p17_inv"};
 
 qtam_status qtam_profile_enable(qtam_plan *p, int on, int max_launches) {
   if (!p || p->host_only) return QTAM_ERR_INVALID_ARG;

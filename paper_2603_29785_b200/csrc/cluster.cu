@@ -16,9 +16,12 @@
 
 namespace qtam {
 
+// (volatile reads: other threads relink parent[] with atomicMin and plain stores while this thread walks it, so a
+// link must be fetched from memory every time it is followed, never kept in a register or taken from the read-only path)
 __device__ __forceinline__ int ccl_find(const int *parent, int x) {
-  int px = parent[x];
-  while (px != x) { x = px; px = parent[x]; }
+  const volatile int *p = parent;
+  int px = p[x];
+  while (px != x) { x = px; px = p[x]; }
   return x;
 }
 
@@ -45,7 +48,7 @@ __global__ void k_ccl_init(const C2<T> *__restrict__ coef, long long ctot, long 
   area[(long long)blockIdx.y * npx + i] = 0;
 }
 
-__global__ void k_ccl_merge(int *__restrict__ parent_all, int R, int M) {
+__global__ void k_ccl_merge(int *parent_all, int R, int M) {
   const int npx = R * M;
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= npx) return;
@@ -57,7 +60,7 @@ __global__ void k_ccl_merge(int *__restrict__ parent_all, int R, int M) {
   if (r + 1 < R && parent[i + M] >= 0) ccl_union(parent, i, i + M);
 }
 
-__global__ void k_ccl_compress(int *__restrict__ parent_all, int *__restrict__ area_all, int npx) {
+__global__ void k_ccl_compress(int *parent_all, int *area_all, int npx) {
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= npx) return;
   int *parent = parent_all + (long long)blockIdx.y * npx;
@@ -81,9 +84,10 @@ __global__ void k_ccl_filter(int *__restrict__ parent_all, const int *__restrict
   parent[i] = label;
 }
 
+// (coef and out are not __restrict__: qtam.h allows d_out == d_coef, masking in place)
 template <typename T>
-__global__ void k_apply_mask(const C2<T> *__restrict__ coef, long long ctot, long long plane_off, int npx,
-                             const int *__restrict__ labels, int label, C2<T> *__restrict__ out) {
+__global__ void k_apply_mask(const C2<T> *coef, long long ctot, long long plane_off, int npx,
+                             const int *__restrict__ labels, int label, C2<T> *out) {
   const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= ctot) return;
   const long long j = i - plane_off;

@@ -484,10 +484,11 @@ k_rows_split(const SpArgs A) {
     const bool valid = sp_decode<F, FWD>(A, sh, chunk, row, id, first, D);
     popped = false; v0 = 0; v1 = 0;
     if (lane == 0 && valid) {
-      // (relaxed: the data these counts guard is read through L2 -- ld.cg -- where the signalling warp's fence has
-      // put it before the count moved)
-      if (D.p0) asm volatile("ld.relaxed.gpu.global.s32 %0, [%1];" : "=r"(v0) : "l"(D.p0) : "memory");
-      if (D.p1) asm volatile("ld.relaxed.gpu.global.s32 %0, [%1];" : "=r"(v1) : "l"(D.p1) : "memory");
+      // (acquire loads: a count that is already there when it is first read is the common case, and a relaxed load
+      // that observes the signalling warp's red.release does not synchronise with it under the PTX memory model --
+      // the lanes' reads of the guarded slot after the __syncwarp need this load to be the acquire side)
+      if (D.p0) v0 = ld_acquire(D.p0);
+      if (D.p1) v1 = ld_acquire(D.p1);
     }
     if (valid) {
       if constexpr (FWD) {
@@ -595,14 +596,17 @@ qtam_status build_rows_split(qtam_plan *p, int c, const std::vector<ClLeader> &l
     const HostPlan &hp = p->hp;
     std::vector<float> wt;
     std::vector<int> wt_off(lead.size(), 0);
-    std::vector<std::pair<int, int>> seen;                 // (woff, first element)
+    // keyed on (half-width, window identity) like build_fast: a row's woff is its private offset into hp.win, so
+    // keying on it would give every leader (the clamped rows of every plane) a table of its own
+    std::vector<std::pair<std::pair<long long, int>, int>> seen;   // ((dk, wid), first element)
     for (size_t li = 0; li < lead.size(); ++li) {
       const ClLeader &L = lead[li];
+      const std::pair<long long, int> key((long long)L.dk, hp.rows[(size_t)L.row].wid);
       int at = -1;
-      for (const auto &e : seen) if (e.first == L.woff) at = e.second;
+      for (const auto &e : seen) if (e.first == key) at = e.second;
       if (at < 0) {
         at = (int)wt.size();
-        seen.push_back(std::make_pair(L.woff, at));
+        seen.push_back(std::make_pair(key, at));
         wt.resize(wt.size() + (size_t)M, 0.f);
         for (int q = 0; q < F; ++q)
           for (int jc = 0; jc < kSpP; ++jc) {
@@ -674,7 +678,7 @@ static qtam_status sp_launch(qtam_plan *p, int c, int batch, void *d_coef, int p
   const long long grid = std::min<long long>((chunks + kSpNT / 32 - 1) / (kSpNT / 32), (long long)p->num_sms * cfg.occ);
   const double bytes = (double)batch * 8.0 * p->cl_sumM[c];       // compulsory: the coefficients
   {
-    LaunchScope ls(p, st, FWD ? K_ROWS_CL_FWD : K_ROWS_CL_INV, bytes, bytes + (double)batch * 8.0 * p->cl_sumL[c]);
+    LaunchScope ls(p, st, (KernelId)((FWD ? K_ROWS_L14_FWD : K_ROWS_L14_INV) + c), bytes, bytes + (double)batch * 8.0 * p->cl_sumL[c]);
     if (cudaMemsetAsync(p->d_sp_ctl[c], 0, sizeof(int) * (2 * nrows + 4), st) != cudaSuccess) return QTAM_ERR_CUDA;
     if (!FWD) {
       // the groups' partial sums start at zero

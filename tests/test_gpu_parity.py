@@ -775,6 +775,9 @@ def test_clusters_and_masks(dtype):
         Mg = g.mask(Y, plane, L, label)
         Mr = r.apply_mask(Yh, plane, Lr, label)
         assert np.array_equal(Mg.cpu().numpy(), Mr)
+        Yc = Y.clone()                                   # in place: qtam.h allows d_out == d_coef
+        g.mask(Yc, plane, L, label, out=Yc)
+        assert torch.equal(Yc, Mg)
         xg = g.inverse(Mg, plane=plane).cpu().numpy()
         assert worst_segment(xg, r.inverse(Mr.astype(np.complex128), plane=plane, engine=1)) <= TOL[dtype] * 10
     # random patterns at several densities (most clusters merge into a few snakes around 0.5-0.6)
