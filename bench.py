@@ -53,6 +53,9 @@ def parse_args():
     ap.add_argument("--no-other-configs", action="store_true",
                     help="skip the records of the other BASELINE configurations (`configs` in the JSON line)")
     ap.add_argument("--dtype", default="", choices=["", "f32", "f64"], help="override the configuration's dtype")
+    ap.add_argument("--time-layout-calls", type=int, default=0, metavar="B",
+                    help="also time qtam_forward_length / qtam_resample / qtam_inverse_length at the paper's image shape "
+                         "(62 x 669 minimal, 62 x 12289 standard, PAPER.md:343) on B segments; goes to the detail file")
     ap.add_argument("--detail", default=os.path.join("gpurun_out", "bench_detail.json"),
                     help="where the per-kernel tables and the records of the other configurations go")
     return ap.parse_args()
@@ -276,6 +279,37 @@ def write_detail(path, detail):
         return os.path.relpath(full, ROOT)
     except Exception as exc:
         return f"not written: {exc}"
+
+
+def time_layout_calls(torch, binding, dev, nseg, flush):
+    """the paper's output-length calls (include/qtam.h says they are direct sums, a layout converter and
+    not a step of the hot path) at the paper's own shape: ms per call on `nseg` segments, CUDA events, L2 flushed"""
+    fs, N, Q, fmin, fmax, rows = inputs.plan_args("paper6s")
+    out = {"segments": nseg, "N": N}
+    x = torch.from_numpy(inputs.make_batch("paper6s", batch=min(nseg, 8))).to(dev).repeat((nseg + 7) // 8, 1)[:nseg].contiguous()
+
+    def ev(fn, reps=3):
+        fn(); torch.cuda.synchronize()
+        tot = 0.0
+        for _ in range(reps):
+            flush.zero_()
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(); fn(); b.record(); torch.cuda.synchronize()
+            tot += a.elapsed_time(b)
+        return tot / reps
+    for mode in ("minimal", "standard"):
+        g = binding.Plan(fs, N, Q, fmin, fmax, rows, dtype="f32", max_batch=nseg, out_length=mode)
+        n = g.output_length()
+        img = g.forward_length(x)
+        rec = {"rows": g.n_rows, "n": n, "forward_length_ms": ev(lambda: g.forward_length(x)),
+               "inverse_length_ms": ev(lambda: g.inverse_length(img))}
+        if mode == "minimal":
+            rec["resample_to_standard_ms"] = ev(lambda: g.resample(img, to_standard=True))
+        rec["image_bytes"] = img.numel() * img.element_size()
+        out[mode] = rec
+        del img
+        g.close()
+    return out
 
 
 def workload_config(args, cfg, batch, plan):
@@ -634,6 +668,13 @@ def run_ours(args):
         except Exception as exc:
             cufft = {"unavailable": str(exc)}
 
+    layout = None
+    if world == 1 and args.time_layout_calls > 0:
+        try:
+            layout = time_layout_calls(torch, binding, dev, args.time_layout_calls, flush)
+        except Exception as exc:
+            layout = {"error": str(exc)}
+
     cpu = None
     if world == 1 and not args.no_cpu_baseline:
         v, cores, nseg, dt = time_oracle(cfg, args.workload, args.overlap)
@@ -662,6 +703,7 @@ def run_ours(args):
         "path": {"frac_of_8tbs": path_gbs / 8000.0, "ms_per_step_with_launch_profile": ms_total / args.steps,
                  "coeffs_per_segment": plan.ctot, "rows": plan.n_rows},
         "kernels": kernels, "largest_batch": largest, "configs": others, "cufft_side_by_side": cufft,
+        "layout_calls_at_the_papers_shape": layout,
     }
     line["detail"] = write_detail(args.detail, detail)
     try:

@@ -29,8 +29,12 @@ k_combine_runs(const int4 *__restrict__ runs, const int *__restrict__ ptr, const
                int tw_shift, float2 *__restrict__ spec, long long xstride, float2 *__restrict__ rt,
                long long rt_stride, int rt_len, int rt_pad) {
   __shared__ int4 s_runs[kRunChunk];
-  __shared__ float2 s_xch[2][kRunBlock];
-  __shared__ unsigned char s_ok[2][kRunBlock];
+  // hand-over buffers between the bin-ordered and the residue-ordered thread maps.  The residue-ordered index
+  // tq = 64 a + b puts the four values of a (lanes 4 b .. 4 b + 3) on one bank; xi() shifts every block of 64 by four
+  // elements, which spreads a half-warp's 8-byte accesses (and the flags' bytes) over distinct banks in both maps
+  __shared__ float2 s_xch[2][kRunBlock + 16];
+  __shared__ unsigned char s_ok[2][kRunBlock + 16];
+  auto xi = [](int i) { return i + 4 * (i >> 6); };
   const int b = blockIdx.x, seg = blockIdx.y;
   const int f = b * kRunBlock + threadIdx.x;
   const int g = Nc - f;
@@ -83,11 +87,11 @@ k_combine_runs(const int4 *__restrict__ runs, const int *__restrict__ ptr, const
       }
     }
   }
-  s_xch[0][tq] = At;
-  s_xch[1][kRunBlock - 1 - tq] = Bt;
+  s_xch[0][xi(tq)] = At;
+  s_xch[1][xi(kRunBlock - 1 - tq)] = Bt;
   __syncthreads();
-  A = padd(A, s_xch[0][threadIdx.x]);
-  B = padd(B, s_xch[1][threadIdx.x]);
+  A = padd(A, s_xch[0][xi(threadIdx.x)]);
+  B = padd(B, s_xch[1][xi(threadIdx.x)]);
   const bool okf = f <= Nc / 2, okg = okf && g != f && f != 0;
   float2 vf = make_float2(0.f, 0.f), vg = vf;
   if (okf) {
@@ -111,12 +115,12 @@ k_combine_runs(const int4 *__restrict__ runs, const int *__restrict__ ptr, const
   // the spectrum in residue order for the long inverse FFT of long_fft.cu (bin x at [x mod 64][pad + x div 64]):
   // handed to the threads of the residue-ordered map, which write 4 consecutive elements of a residue each
   __syncthreads();
-  s_xch[0][threadIdx.x] = vf; s_ok[0][threadIdx.x] = okf;
-  s_xch[1][threadIdx.x] = vg; s_ok[1][threadIdx.x] = okg;
+  s_xch[0][xi(threadIdx.x)] = vf; s_ok[0][xi(threadIdx.x)] = okf;
+  s_xch[1][xi(threadIdx.x)] = vg; s_ok[1][xi(threadIdx.x)] = okg;
   __syncthreads();
   float2 *R = rt + (size_t)seg * rt_stride + rt_pad;
-  if (s_ok[0][tq]) R[(size_t)(tf & 63) * rt_len + (tf >> 6)] = s_xch[0][tq];
-  if (s_ok[1][kRunBlock - 1 - tq]) R[(size_t)(tg & 63) * rt_len + (tg >> 6)] = s_xch[1][kRunBlock - 1 - tq];
+  if (s_ok[0][xi(tq)]) R[(size_t)(tf & 63) * rt_len + (tf >> 6)] = s_xch[0][xi(tq)];
+  if (s_ok[1][xi(kRunBlock - 1 - tq)]) R[(size_t)(tg & 63) * rt_len + (tg >> 6)] = s_xch[1][xi(kRunBlock - 1 - tq)];
 }
 
 // Run lists, the band-slot runs of the rows that no tile or group covers, and the partial-sum buffer (the tiles'
