@@ -173,3 +173,28 @@ def test_no_write_outside_the_callers_buffers(name, dtype, nseg):
         assert b.intact()
         assert torch.equal(b.t[nseg].view(torch.uint8), s.view(torch.uint8))
     g.close()
+
+
+def test_composite_bank_with_more_than_64_window_identities():
+    """66 planes with 66 different Kaiser windows at one Q: the float row tables are keyed on (half-width, window
+    identity), and a key that packs the identity into 6 bits would hand plane 64 + b the window of plane b at the next
+    half-width.  Rows dense enough that consecutive half-widths occur; every row against the oracle."""
+    nP = 66
+    fs, N = 2048.0, 4096
+    args = (fs, N, [8.0] * nP, 16.0, 900.0, 40.0)
+    kw = dict(plane_windows=[("kaiser", 3.0 + 0.125 * i) for i in range(nP)])
+    g = binding.Plan(*args, dtype="f32", max_batch=2, **kw)
+    r = RefPlan(*args, **kw)
+    dks = sorted({int(a.dk) for a in g.rows})
+    assert any(b - a == 1 for a, b in zip(dks, dks[1:])) and g.n_planes == nP
+    x = inputs.white_noise(N, 4242, batch=2).astype(np.float32)
+    Y = g.forward(torch.from_numpy(x).cuda()).cpu().numpy()
+    Yr = r.forward(x.astype(np.float64), engine=1)
+    assert max(rel_l2(Y[b], Yr[b]) for b in range(2)) <= TOL["f32"]
+    assert worst_row(Y, Yr, r) <= TOL_ROW["f32"]
+    Yin = Yr.astype(np.complex64)
+    for plane in (-1, 1, 64, 65):
+        xg = g.inverse(torch.from_numpy(Yin).cuda(), plane=plane).cpu().numpy()
+        xr = r.inverse(Yin.astype(np.complex128), plane=plane, engine=1)
+        assert max(rel_l2(xg[b], xr[b]) for b in range(2)) <= TOL["f32"], plane
+    g.close()
